@@ -1,0 +1,238 @@
+"""oracle/ipm.py -- TEST INFRASTRUCTURE ONLY (see oracle/__init__.py).
+
+Algorithm 2 (LiftedIPM) and Algorithm 1 (NMPC loop), step by step, in
+the paper's order.  Where the paper is silent (constants, E_mu, mu update, step rule, inertia schedule) the
+readings are those of DESIGN.md §3 (G1..G19); the step labels S0..S10 below are the ones used there.
+
+Lifted problem (Eq. 16) with native variable bounds (reading G1):
+    min f(y;p)   s.t.  h(y;p) - gamma + s+ = 0,  -h(y;p) - gamma + s- = 0,  s+- >= 0,  lb <= y <= ub
+multipliers w+ , w- (omega of the lifted inequalities; beta == omega, reading G3), zL, zU for the bounds.
+
+Newton step (Eq. 10 with the lifted G^l = [J; -J], condensed as Eq. 14/17):
+    K dy = b,   K = W + eta I + Sigma_x + J^T (q+ + q-) J,      q+- = w+-/s+-   (Q_s = S^-1 B)
+    b = -( grad f - mu/(y-lb) + mu/(ub-y) + J^T t ),  t = q+ r_p+ + mu/s+ - q- r_p- - mu/s-
+which is -r_1^l - G^l^T (Q_s^l r_4^l - r_2^l) of Eq. 17 with r_2 = omega - mu S^-1 e (reading G2); the omega
+terms of r_1 and r_2 cancel.
+"""
+from __future__ import annotations
+
+import numpy as np
+import scipy.sparse as sp
+
+from .linalg import BlockTridiagCholesky, DenseCholesky, NotPositiveDefinite, SparseCholesky
+from .nlp import TranscribedOCP
+
+# S0 constants (every one an option; DESIGN.md §3 table "IPM constants")
+DEFAULTS = dict(gamma=1e-4, eps_outer=1e-5, mu0=0.1, mu_warm=None,  # None -> eps_outer/10
+                kappa_eps=10.0, kappa_mu=0.2, theta_mu=1.5, tau_min=0.99,
+                kappa_push=1e-2, s_floor=1e-2, s_max=100.0, max_iter=200,
+                eta_first=1e-4, eta_grow_first=100.0, eta_grow=8.0, eta_shrink=1.0 / 3.0,
+                eta_min=1e-20, eta_max=1e40, warm_push=1e-10)
+
+
+class IPMState:
+    """Primal-dual iterate z = (y, s+, s-, w+, w-, zL, zU) (PAPER.md:144 with beta == omega)."""
+
+    def __init__(self, y, sp_, sm, wp, wm, zL, zU):
+        self.y, self.sp, self.sm, self.wp, self.wm, self.zL, self.zU = y, sp_, sm, wp, wm, zL, zU
+
+    def copy(self):
+        return IPMState(*(v.copy() for v in (self.y, self.sp, self.sm, self.wp, self.wm, self.zL, self.zU)))
+
+
+class LiftedIPM:
+    def __init__(self, cfg, linsolve="sparse", perm=None, **options):
+        self.cfg = cfg
+        self.nlp = TranscribedOCP(cfg)
+        self.opt = dict(DEFAULTS)
+        self.opt.update(options)
+        if self.opt["mu_warm"] is None:
+            self.opt["mu_warm"] = self.opt["eps_outer"] / 10.0
+        self.linsolve, self.perm = linsolve, perm
+        self.chol = None                       # P, S_L = nothing (Alg. 1 line 4)
+        self.n_symbolic = 0
+        self.state = None
+        n = self.nlp.n
+        self.hasL, self.hasU = np.isfinite(self.nlp.lb), np.isfinite(self.nlp.ub)
+        self.lb = np.where(self.hasL, self.nlp.lb, 0.0)
+        self.ub = np.where(self.hasU, self.nlp.ub, 0.0)
+
+    # ---------------------------------------------------------------------------------------------
+    def _make_cholesky(self, K):
+        """SymCholesky, Eq. (18): only when P, S_L = nothing (Alg. 2 lines 10-12)."""
+        self.n_symbolic += 1
+        if self.linsolve == "dense":
+            return DenseCholesky(self.nlp.n)
+        if self.linsolve == "blocktri":
+            return BlockTridiagCholesky(self.nlp.N, self.nlp.nv)
+        return SparseCholesky(self.nlp.K_pattern(), self.perm)
+
+    # ---------------------------------------------------------------------------------------------
+    def _errors(self, st, gradf, c, J, mu):
+        """S2: residuals of the smoothed KKT system K_mu (Eq. 9) and the optimality error E_mu (Eq. 27/28)."""
+        o = self.opt
+        hasL, hasU = self.hasL, self.hasU
+        dL, dU = st.y - self.lb, self.ub - st.y
+        r_d = gradf + J.T @ (st.wp - st.wm) - np.where(hasL, st.zL, 0.0) + np.where(hasU, st.zU, 0.0)
+        r_pp = c - o["gamma"] + st.sp
+        r_pm = -c - o["gamma"] + st.sm
+        comp = np.concatenate([st.sp * st.wp - mu, st.sm * st.wm - mu,
+                               (dL * st.zL - mu)[hasL], (dU * st.zU - mu)[hasU]])
+        nmult = 2 * self.nlp.m + int(hasL.sum()) + int(hasU.sum())
+        l1 = st.wp.sum() + st.wm.sum() + st.zL[hasL].sum() + st.zU[hasU].sum()
+        s_d = max(o["s_max"], l1 / nmult) / o["s_max"]
+        E = max(np.max(np.abs(r_d)) / s_d, np.max(np.abs(r_pp)), np.max(np.abs(r_pm)),
+                np.max(np.abs(comp)) / s_d)
+        return E, r_d, r_pp, r_pm
+
+    # ---------------------------------------------------------------------------------------------
+    def cold_start(self, y0):
+        """S1 cold init."""
+        o, nlp = self.opt, self.nlp
+        y = np.array(y0, dtype=np.float64)
+        kp = o["kappa_push"]
+        both = self.hasL & self.hasU
+        pL = np.where(both, np.minimum(kp * np.maximum(1.0, np.abs(self.lb)), kp * (self.ub - self.lb)),
+                      kp * np.maximum(1.0, np.abs(self.lb)))
+        pU = np.where(both, np.minimum(kp * np.maximum(1.0, np.abs(self.ub)), kp * (self.ub - self.lb)),
+                      kp * np.maximum(1.0, np.abs(self.ub)))
+        y = np.where(self.hasL, np.maximum(y, self.lb + pL), y)
+        y = np.where(self.hasU, np.minimum(y, self.ub - pU), y)
+        c = nlp.constraints(y)
+        mu0 = o["mu0"]
+        s_p = np.maximum(o["gamma"] - c, o["s_floor"])
+        s_m = np.maximum(o["gamma"] + c, o["s_floor"])
+        zL = np.where(self.hasL, mu0 / np.where(self.hasL, y - self.lb, 1.0), 0.0)
+        zU = np.where(self.hasU, mu0 / np.where(self.hasU, self.ub - y, 1.0), 0.0)
+        return IPMState(y, s_p, s_m, mu0 / s_p, mu0 / s_m, zL, zU), mu0
+
+    def warm_start(self, prev):
+        """S1 warm init: z_{k+1} <- z*_k verbatim (Alg. 1 line 10), smaller mu."""
+        st = prev.copy()
+        wpush = self.opt["warm_push"]
+        st.y = np.where(self.hasL, np.maximum(st.y, self.lb + wpush), st.y)
+        st.y = np.where(self.hasU, np.minimum(st.y, self.ub - wpush), st.y)
+        return st, self.opt["mu_warm"]
+
+    # ---------------------------------------------------------------------------------------------
+    def solve(self, y0=None, warm=False, trace=None):
+        """Algorithm 2.  Returns dict(status, iters, factorizations, state, trace)."""
+        o, nlp = self.opt, self.nlp
+        hasL, hasU = self.hasL, self.hasU
+        if warm and self.state is not None:
+            st, mu = self.warm_start(self.state)
+        else:
+            st, mu = self.cold_start(nlp.cfg.y_cold(nlp.x0) if y0 is None else y0)
+        eta_last = 0.0
+        nfact = 0
+        tr = [] if trace is None else trace
+        it = 0
+        status = "maxiter"
+        while True:
+            # S2: evaluate (K_SIMD of the paper: f, grad f, c, J)            Alg. 2 line 5
+            gradf = nlp.gradient(st.y)
+            c = nlp.constraints(st.y)
+            J = nlp.jacobian(st.y)
+            E0, _, _, _ = self._errors(st, gradf, c, J, 0.0)
+            # S3: outer test, Eq. (28)
+            if E0 <= o["eps_outer"]:
+                status = "converged"
+                break
+            if it >= o["max_iter"]:
+                break
+            # S4: barrier update while the inner test Eq. (27) holds with eps_inner = kappa_eps*mu  (Alg. 2 line 18)
+            Emu, r_d, r_pp, r_pm = self._errors(st, gradf, c, J, mu)
+            while Emu <= o["kappa_eps"] * mu and mu > o["eps_outer"] / 10.0:
+                mu = max(o["eps_outer"] / 10.0, min(o["kappa_mu"] * mu, mu ** o["theta_mu"]))
+                Emu, r_d, r_pp, r_pm = self._errors(st, gradf, c, J, mu)
+            # S5
+            tau = max(o["tau_min"], 1.0 - mu)
+            # S6: condensed lifted KKT matrix and right-hand side (Eq. 17)      Alg. 2 lines 5-6
+            dL = np.where(hasL, st.y - self.lb, 1.0)
+            dU = np.where(hasU, self.ub - st.y, 1.0)
+            Sigma_x = np.where(hasL, st.zL / dL, 0.0) + np.where(hasU, st.zU / dU, 0.0)
+            q_p, q_m = st.wp / st.sp, st.wm / st.sm
+            W = nlp.hessian(st.y, st.wp - st.wm)
+            K0 = (W + sp.diags(Sigma_x) + J.T @ sp.diags(q_p + q_m) @ J).tocsc()
+            t = q_p * r_pp + mu / st.sp - q_m * r_pm - mu / st.sm
+            b = -(gradf - np.where(hasL, mu / dL, 0.0) + np.where(hasU, mu / dU, 0.0) + J.T @ t)
+            # S7: inertia correction (Eq. 13/15) + NumCholesky      Alg. 2 lines 7-13
+            if self.chol is None:
+                self.chol = self._make_cholesky(K0)
+            eta = 0.0
+            while True:
+                try:
+                    nfact += 1
+                    self.chol.factor(K0 + eta * sp.identity(nlp.n, format="csc") if eta > 0.0 else K0)
+                    break
+                except NotPositiveDefinite:
+                    if eta == 0.0:
+                        eta = o["eta_first"] if eta_last == 0.0 else max(o["eta_min"], o["eta_shrink"] * eta_last)
+                    else:
+                        eta = (o["eta_grow_first"] if eta_last == 0.0 else o["eta_grow"]) * eta
+                    if eta > o["eta_max"]:
+                        self.state = st
+                        return dict(status="inertia", iters=it, factorizations=nfact, state=st, trace=tr)
+            if eta > 0.0:
+                eta_last = eta
+            # S8: triangular solves Eq. (22)-(25), then the eliminated directions from Eq. (14)/(10)   line 14
+            dy = self.chol.solve(b)
+            Jdy = J @ dy
+            ds_p = -r_pp - Jdy
+            ds_m = -r_pm + Jdy
+            dw_p = -(st.wp - mu / st.sp) - q_p * ds_p
+            dw_m = -(st.wm - mu / st.sm) - q_m * ds_m
+            dzL = np.where(hasL, -(st.zL - mu / dL) - st.zL / dL * dy, 0.0)
+            dzU = np.where(hasU, -(st.zU - mu / dU) + st.zU / dU * dy, 0.0)
+            # S9: fraction to the boundary, separate primal / dual steps (reading G8)
+            a_pr = min(_max_step(st.sp, ds_p, tau), _max_step(st.sm, ds_m, tau),
+                       _max_step(dL[hasL], dy[hasL], tau), _max_step(dU[hasU], -dy[hasU], tau))
+            a_du = min(_max_step(st.wp, dw_p, tau), _max_step(st.wm, dw_m, tau),
+                       _max_step(st.zL[hasL], dzL[hasL], tau), _max_step(st.zU[hasU], dzU[hasU], tau))
+            tr.append(dict(it=it, mu=mu, E0=E0, Emu=Emu, eta=eta, alpha_pr=a_pr, alpha_du=a_du))
+            # kept for the pins (condensation algebra vs the un-condensed Newton system, Eq. 10)
+            self.last_step = dict(state=st, mu=mu, eta=eta, gradf=gradf, c=c, J=J, W=W, K0=K0, b=b, dy=dy,
+                                  ds_p=ds_p, ds_m=ds_m, dw_p=dw_p, dw_m=dw_m, dzL=dzL, dzU=dzU,
+                                  r_d=r_d, r_pp=r_pp, r_pm=r_pm)
+            # S10: Eq. (26)                                                     Alg. 2 line 15
+            st = IPMState(st.y + a_pr * dy, st.sp + a_pr * ds_p, st.sm + a_pr * ds_m,
+                          st.wp + a_du * dw_p, st.wm + a_du * dw_m, st.zL + a_du * dzL, st.zU + a_du * dzU)
+            if not np.all(np.isfinite(st.y)):
+                status = "step"
+                break
+            it += 1
+        self.state = st
+        return dict(status=status, iters=it, factorizations=nfact, state=st, trace=tr, E0=E0, mu=mu)
+
+
+def _max_step(v, dv, tau):
+    """Largest a in (0,1] with v + a dv >= (1-tau) v  (v > 0)."""
+    neg = dv < 0.0
+    if not np.any(neg):
+        return 1.0
+    return min(1.0, float(np.min(-tau * v[neg] / dv[neg])))
+
+
+# ==================================================================================================
+def nmpc_closed_loop(cfg, n_resolves=None, linsolve="sparse", perm=None, x0_sequence=None, **options):
+    """Algorithm 1 with plant == model (SURVEY.md §8(d) "common"):
+       solve j, extract u_1 / x_1 (line 6), x0^(j+1) = x_1* + noise_j (lines 8-9, clipped), z_{j+1} <- z*_j (line 10),
+       update p (line 11).  Solve 0 is cold; the rest are warm re-solves on the cached P, S_L.
+       If `x0_sequence` is given (replay mode) it overrides the closed-loop x0 of every solve."""
+    R = cfg.R if n_resolves is None else n_resolves
+    ipm = LiftedIPM(cfg, linsolve=linsolve, perm=perm, **options)
+    x0 = np.array(cfg.x0, dtype=np.float64)
+    out = []
+    for j in range(R + 1):
+        if x0_sequence is not None:
+            x0 = np.array(x0_sequence[j], dtype=np.float64)
+        ref = cfg.ref_for_solve(j)
+        ipm.nlp.set_params(x0, ref)
+        res = ipm.solve(warm=(j > 0))
+        y = res["state"].y
+        out.append(dict(solve=j, x0=x0.copy(), ref=ref, y=y.copy(), iters=res["iters"], status=res["status"],
+                        factorizations=res["factorizations"], trace=res["trace"], E0=res.get("E0"),
+                        state=res["state"].copy()))
+        x1 = y[: cfg.nx]
+        x0 = np.clip(x1 + cfg.noise_for_solve(j), cfg.x0_clip[0], cfg.x0_clip[1])
+    return out, ipm
