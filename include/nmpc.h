@@ -1,0 +1,193 @@
+/* include/nmpc.h -- C-ABI of the B200-native KKT hot path of the parametric interior-point NMPC method of
+ * arxiv/paper_2606_04725 ("GPU-Accelerated Direct Transcription-Based Nonlinear Model Predictive Control").
+ *
+ * The library implements, in hand-written CUDA for sm_100a (fp64), the per-IPM-iteration linear solve of the
+ * paper's Algorithm 2 (LiftedIPM):
+ *
+ *   symbolic analysis, once per OCP structure   SymCholesky, Eq. (18)-(19); Alg. 2 lines 10-12
+ *   numeric Cholesky on the fixed structure     NumCholesky, Eq. (20)-(21); Alg. 2 line 13
+ *   triangular solves                            Eq. (22)-(25);             Alg. 2 line 14
+ *   condensed lifted KKT assembly                Eq. (14), (16)-(17);        Alg. 2 lines 5-9
+ *   IPM iteration + NMPC parameter update        Eq. (26)-(28), Alg. 1 lines 9-11
+ *
+ * Conventions (all entry points)
+ *   - C99, no exceptions cross the boundary, no global state; every call returns an nmpc_status.
+ *   - "HOST" pointers are ordinary host memory; "DEVICE" pointers are CUDA device memory of the device that
+ *     was current when the handle was created (e.g. torch tensor.data_ptr()).
+ *   - Ownership: the caller owns every pointer it passes.  The library copies what it needs during the call and
+ *     never frees or retains caller memory; DEVICE buffers must stay valid until the handle's stream has
+ *     finished the work of the call (every call that returns a HOST result synchronises that stream itself).
+ *   - The handle owns all internal host and device memory; nmpc_destroy releases it.
+ *   - One handle <-> one CUDA stream <-> one host thread.  fp64 only.  There is no CPU fallback on the numeric
+ *     path: without a CUDA device nmpc_analyze returns NMPC_E_CUDA.
+ */
+#ifndef NMPC_H
+#define NMPC_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nmpc_handle_s*   nmpc_handle;   /* opaque: symbolic data + device buffers + IPM state     */
+typedef struct nmpc_symbolic_s* nmpc_symbolic; /* opaque: host-only symbolic analysis (no CUDA required)  */
+
+typedef enum {
+    NMPC_OK = 0,
+    NMPC_E_ARG = 1,      /* NULL / out-of-range argument                                                  */
+    NMPC_E_PATTERN = 2,  /* pattern not lower-triangular CSR, unsorted, duplicate or missing diagonal      */
+    NMPC_E_ALLOC = 3,    /* host or device allocation failed                                              */
+    NMPC_E_CUDA = 4,     /* CUDA runtime error (no device, launch failure); see nmpc_last_error           */
+    NMPC_E_STATE = 5,    /* wrong call order (solve before a successful factor, ipm_solve without a model) */
+    NMPC_E_NOT_SPD = 6,  /* a pivot was <= 0 or non-finite; *info = first failing column (original index)  */
+    NMPC_E_INERTIA = 7,  /* the eta schedule exceeded eta_max (Eq. 13)                   */
+    NMPC_E_MAXITER = 8,  /* max_iter IPM iterations without meeting Eq. (28)                               */
+    NMPC_E_STEP = 9      /* non-finite iterate                                                             */
+} nmpc_status;
+
+enum { NMPC_MODEL_NONE = 0, NMPC_MODEL_VDP = 1, NMPC_MODEL_DISTILL = 2, NMPC_MODEL_PLATE = 3 };
+enum { NMPC_ORDER_AUTO = 0, NMPC_ORDER_NATURAL = 1, NMPC_ORDER_AMD = 2, NMPC_ORDER_ND = 3, NMPC_ORDER_TIME_ND = 4 };
+
+/* Sparsity pattern of the condensed KKT matrix K (Eq. 17): HOST, lower triangle in CSR (row i holds the
+ * columns j <= i, strictly increasing, the diagonal present in every row).  nnz = rowptr[n].               */
+typedef struct {
+    int64_t n, nnz;
+    const int64_t* rowptr;   /* n+1 */
+    const int32_t* colind;   /* nnz */
+} nmpc_pattern;
+
+/* Stage-structured parametric OCP  P_k(p_k)  (Problems 4-6) with a built-in stage model.
+ * Variables y = [x_1,u_1,...,x_N,u_N] (nv = nx+nu per stage); x_0 and the references are PARAMETERS.
+ * Equalities h_k = x_k - x_{k-1} - dt F(x_k,u_k) (implicit Euler), bounds lb <= (x,u) <= ub.
+ * model_params (HOST, copied), by model:
+ *   VDP     [w_x, w_u]                      F = (x2, (1-x1^2) x2 - x1 + u);  l = w_x |x-r|^2 + w_u u^2
+ *   DISTILL [alpha, D, F_feed, x_feed, A_c, A_t, A_r, feed_index, u_bar, w_u]   (Problem 29)
+ *   PLATE   [g, a, kappa_r, T_amb, b, nseg, w_T, w_u]    5-point heat equation + radiative loss, edge heaters
+ * lb/ub: HOST, length nx+nu (one stage, repeated over stages); +-INFINITY = no bound.
+ * u_init: HOST, length nu, cold-start input guess.                                                        */
+typedef struct {
+    int32_t model;
+    int32_t N, nx, nu, nr;       /* nr = reference entries per stage                                        */
+    double  dt;
+    const double* model_params;
+    int32_t n_model_params;
+    const double* lb;
+    const double* ub;
+    const double* u_init;
+} nmpc_ocp;
+
+/* Options; pass NULL for the defaults (nmpc_default_options).  IPM constants are the readings S0 of
+ * DESIGN.md section 3 (the paper prints none).                                          */
+typedef struct {
+    int32_t ordering;            /* NMPC_ORDER_*                                                            */
+    int32_t nd_leaf;             /* nested-dissection leaf size (variables)                                 */
+    int32_t relax_small;         /* always merge a child supernode into its parent if the merged width <= this */
+    double  relax_zeros;         /* else merge if the explicit zeros introduced stay below this fraction      */
+    int32_t smem_front_max;      /* fronts with <= this many rows run in the one-CTA shared-memory kernel     */
+    int32_t use_graph;           /* capture factor / solve launch sequences in CUDA graphs                    */
+    /* IPM (Algorithm 2) */
+    double gamma, eps_outer, mu0, mu_warm, kappa_eps, kappa_mu, theta_mu, tau_min, kappa_push, s_floor, s_max;
+    int32_t max_iter;
+    double eta_first, eta_grow_first, eta_grow, eta_shrink, eta_min, eta_max, warm_push;
+    int32_t time_phases;         /* record CUDA-event phase times in nmpc_stats (adds event overhead)         */
+} nmpc_options;
+
+typedef struct {                 /* filled by nmpc_get_info; arrays are HOST pointers owned by the handle     */
+    int64_t n, nnz_K, nnz_L;     /* nnz_L = sum over supernodes of panel entries on or below the diagonal     */
+    int64_t panel_doubles, update_doubles;
+    double  flops;               /* sum_j cc_j^2 over the columns of L (cc_j = column count incl. diagonal)   */
+    int32_t nsuper, nlevels, max_front, max_width, n_large_fronts;
+    int32_t ordering_used;
+    double  analyze_ms;
+    const int32_t* perm;         /* n: perm[i] = original index of the variable at pivot position i (Eq. 19)  */
+    const int32_t* super_start;  /* nsuper+1                                                                  */
+    const int64_t* rows_ptr;     /* nsuper+1                                                                  */
+    const int32_t* rows;         /* rows of each supernode in pivot order (first w are its own columns)       */
+    const int32_t* super_parent; /* nsuper, -1 = root                                                         */
+    const int32_t* super_level;  /* nsuper, 0 = leaf level                                                    */
+    const int32_t* etree_parent; /* n, elimination tree on pivot positions, -1 = root      */
+} nmpc_sym_info;
+
+typedef struct {                 /* filled by nmpc_ipm_solve (HOST)                                           */
+    int32_t status, iters, factorizations, eta_retries;
+    double  E0, mu, eta_last, objective;
+    double  ms_total, ms_eval, ms_assemble, ms_factor, ms_solve, ms_vector;   /* CUDA-event phase sums        */
+} nmpc_stats;
+
+typedef struct {                 /* one row per IPM iteration, for parity traces (HOST, caller array)         */
+    double mu, E0, Emu, eta, alpha_pr, alpha_du;
+} nmpc_trace_row;
+
+void nmpc_default_options(nmpc_options* out);
+
+/* ---- host-only symbolic analysis (Eq. 18-19; no CUDA needed): ordering P, elimination tree, column counts,
+ *      supernode partition, level sets, scatter maps.  `ocp` may be NULL (bare pattern).  If `pattern` is NULL
+ *      and `ocp` names a model, the pattern of K = W + Sigma_x + J^T Q J is derived from the model.          */
+nmpc_status nmpc_symbolic_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const nmpc_options* opt,
+                                  nmpc_symbolic* out);
+nmpc_status nmpc_symbolic_info(nmpc_symbolic sym, nmpc_sym_info* out);
+/* Pattern of K derived from the model (lower CSR).  Two-call protocol: with rowptr == NULL only *nnz is set. */
+nmpc_status nmpc_symbolic_pattern(nmpc_symbolic sym, int64_t* nnz, int64_t* rowptr /*n+1*/, int32_t* colind);
+/* scatter map: for K value index e (pattern order), supernode and offset inside its column-major panel.     */
+nmpc_status nmpc_symbolic_kmap(nmpc_symbolic sym, int32_t* super_of_entry /*nnz*/, int64_t* panel_offset /*nnz*/);
+void        nmpc_symbolic_destroy(nmpc_symbolic sym);
+
+/* ---- Alg. 2 lines 10-12: analysis once per structure; uploads all integer maps; allocates L.  cuda_stream is a
+ *      cudaStream_t (NULL = default stream).                                                                 */
+nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const nmpc_options* opt,
+                         void* cuda_stream, nmpc_handle* out);
+
+/* ---- Alg. 1 line 11 / PAPER.md:362: parameter update p = (x0, ref); DEVICE pointers, x0[nx], ref[N*nr];
+ *      asynchronous on the stream; no structural work.                                                       */
+nmpc_status nmpc_update_params(nmpc_handle h, const double* x0_dev, const double* ref_dev);
+/*      same from HOST buffers (copies through pinned staging inside the call)                                */
+nmpc_status nmpc_update_params_host(nmpc_handle h, const double* x0_host, const double* ref_host);
+
+/* ---- Eq. (20)-(21): numeric Cholesky of K + eta I.  values_dev: DEVICE, nnz doubles in pattern order.
+ *      Synchronises the stream to read the pivot flag.  On NMPC_E_NOT_SPD *info_host = failing original column. */
+nmpc_status nmpc_factor(nmpc_handle h, const double* values_dev, double eta, int64_t* info_host);
+
+/* ---- Eq. (22)-(25): rhs_inout_dev DEVICE n*nrhs doubles (column-major), overwritten by K^-1 rhs.  Async.   */
+nmpc_status nmpc_solve(nmpc_handle h, double* rhs_inout_dev, int32_t nrhs);
+
+/* ---- y = K x with the values last passed to nmpc_factor (+eta I), for residual checks.  Async.            */
+nmpc_status nmpc_kkt_multiply(nmpc_handle h, const double* x_dev, double* y_dev);
+
+/* ---- Algorithm 2 (LiftedIPM) on the current parameters.  warm = 0: cold start (y_inout_dev is ignored on input
+ *      unless use_y0 != 0); warm = 1: z <- stored z* of the previous solve (Alg. 1 line 10).  y_inout_dev DEVICE n.
+ *      trace (HOST, may be NULL) receives up to trace_cap rows.                                               */
+nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* y_inout_dev, nmpc_stats* stats_host,
+                           nmpc_trace_row* trace_host, int32_t trace_cap);
+/*      end-to-end form with HOST buffers: parameters in, primal solution out (copies inside the call)        */
+nmpc_status nmpc_ipm_solve_host(nmpc_handle h, int32_t warm, const double* x0_host, const double* ref_host,
+                                double* y_out_host, nmpc_stats* stats_host);
+
+/* ---- current primal-dual iterate z (DEVICE outputs; any pointer may be NULL): s+,s-,w+,w- length m; zL,zU n */
+nmpc_status nmpc_get_iterate(nmpc_handle h, double* y_dev, double* sp_dev, double* sm_dev, double* wp_dev,
+                             double* wm_dev, double* zL_dev, double* zU_dev);
+/* ---- model evaluation at (y, lam) with the current parameters (DEVICE outputs, any may be NULL):
+ *      c[m], gradf[n], Jval[nnzJ], Wval[nnzW]; and the assembled K values (pattern order) for given Sigma_x[n],
+ *      q[m], eta.  Used by the parity tests of steps a2/a3.                                                  */
+nmpc_status nmpc_model_eval(nmpc_handle h, const double* y_dev, const double* lam_dev, double* c_dev,
+                            double* gradf_dev, double* Jval_dev, double* Wval_dev);
+nmpc_status nmpc_assemble(nmpc_handle h, const double* Jval_dev, const double* Wval_dev, const double* sigma_x_dev,
+                          const double* q_dev, double eta, double* Kval_dev);
+/* ---- patterns of J (CSR, m x n) and W (lower CSR, n x n) in the value order of nmpc_model_eval (HOST out).
+ *      Two-call protocol as nmpc_symbolic_pattern.                                                           */
+nmpc_status nmpc_get_jac_pattern(nmpc_handle h, int64_t* nnz, int64_t* rowptr, int32_t* colind);
+nmpc_status nmpc_get_hess_pattern(nmpc_handle h, int64_t* nnz, int64_t* rowptr, int32_t* colind);
+nmpc_status nmpc_get_kkt_pattern(nmpc_handle h, int64_t* nnz, int64_t* rowptr, int32_t* colind);
+
+nmpc_status nmpc_get_info(nmpc_handle h, nmpc_sym_info* out_host);
+/* ---- copy of the factor for tests: panels (column-major r x w per supernode) to a HOST buffer             */
+nmpc_status nmpc_get_factor(nmpc_handle h, double* panels_host /* panel_doubles */);
+/* ---- kernel launches issued by this handle since creation (graph replays count their kernel nodes)        */
+int64_t     nmpc_launch_count(nmpc_handle h);
+const char* nmpc_last_error(nmpc_handle h);      /* string owned by the handle                                */
+void        nmpc_destroy(nmpc_handle h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NMPC_H */

@@ -1,0 +1,593 @@
+// api.cu -- the C-ABI of include/nmpc.h: handle life cycle, level schedule, CUDA-graph capture of the factor and
+// solve launch sequences, and the host side of Algorithm 2 (LiftedIPM) / Algorithm 1 lines 9-11.
+// Every numeric step runs in the kernels of factor.cu / ipm.cu; the host only sequences launches and takes the
+// scalar decisions (barrier update, inertia schedule, termination) from a handful of reduced scalars.
+#include <algorithm>
+#include <chrono>
+#include <climits>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "device.h"
+#include "symbolic.h"
+
+using namespace nmpc;
+
+extern "C" void nmpc_fill_info(const nmpc::Symbolic& S, nmpc_sym_info* o);
+extern "C" nmpc_status nmpc_copy_pattern_internal(const nmpc::Csr& P, int64_t* nnz, int64_t* rowptr, int32_t* colind);
+
+namespace {
+
+struct StepPlan { int potrf_off, potrf_cnt, trsm_off, trsm_cnt, syrk_off, syrk_cnt; };
+struct LevelPlan {
+    int small_off = 0, small_cnt = 0, small_max_r = 0;     // into d_small_list
+    int asm_off = 0, asm_cnt = 0;                          // into d_items
+    std::vector<StepPlan> steps;
+    int all_off = 0, all_cnt = 0, all_max_r = 0;           // every supernode of the level (solves), into d_lvl_sn
+};
+
+}  // namespace
+
+struct nmpc_handle_s {
+    Symbolic S;
+    nmpc_options opt;
+    cudaStream_t stream = nullptr;
+    DevSym D;
+    DevModel M;
+    IpmVectors V{};
+    std::vector<void*> allocs;
+    std::vector<LevelPlan> plan;
+    int32_t* d_small_list = nullptr;
+    int32_t* d_lvl_sn = nullptr;
+    BigItem* d_items = nullptr;
+    int n_big_fronts = 0;
+    double* d_eta = nullptr;
+    double* d_Kval = nullptr;          // values last factored (pattern order)
+    double* d_x = nullptr;             // permuted right-hand side / solution
+    int64_t* d_full_ptr = nullptr; int32_t* d_full_idx = nullptr; int32_t* d_full_src = nullptr;   // symmetric CSR of K
+    double* d_uinit = nullptr;
+    double* h_pinned = nullptr;        // pinned host scratch: [0..15] scalars, [16] flag, staging for host-buffer calls
+    size_t pinned_doubles = 0;
+    cudaGraphExec_t g_factor = nullptr, g_fwdbwd = nullptr;
+    int g_factor_nodes = 0, g_fwdbwd_nodes = 0;
+    bool factored = false, have_state = false, has_model = false;
+    double eta_cur = 0.0;
+    int64_t launches = 0;
+    int nmult = 0;
+    std::string err;
+    cudaEvent_t ev[2] = {nullptr, nullptr};
+};
+
+namespace {
+
+#define CK(call)                                                                                      \
+    do {                                                                                              \
+        cudaError_t e__ = (call);                                                                     \
+        if (e__ != cudaSuccess) {                                                                     \
+            h->err = std::string(#call) + ": " + cudaGetErrorString(e__);                             \
+            return NMPC_E_CUDA;                                                                       \
+        }                                                                                             \
+    } while (0)
+
+template <class T>
+nmpc_status upload(nmpc_handle_s* h, const std::vector<T>& v, const T** out) {
+    T* d = nullptr;
+    size_t bytes = std::max<size_t>(1, v.size()) * sizeof(T);
+    if (cudaMalloc((void**)&d, bytes) != cudaSuccess) { h->err = "cudaMalloc failed (" + std::to_string(bytes) + " B)"; cudaGetLastError(); return NMPC_E_ALLOC; }
+    h->allocs.push_back(d);
+    if (!v.empty()) CK(cudaMemcpyAsync(d, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice, h->stream));
+    *out = d;
+    return NMPC_OK;
+}
+
+template <class T>
+nmpc_status dalloc(nmpc_handle_s* h, size_t count, T** out, bool zero = true) {
+    T* d = nullptr;
+    size_t bytes = std::max<size_t>(1, count) * sizeof(T);
+    if (cudaMalloc((void**)&d, bytes) != cudaSuccess) { h->err = "cudaMalloc failed (" + std::to_string(bytes) + " B)"; cudaGetLastError(); return NMPC_E_ALLOC; }
+    h->allocs.push_back(d);
+    if (zero) CK(cudaMemsetAsync(d, 0, bytes, h->stream));
+    *out = d;
+    return NMPC_OK;
+}
+
+#define TRY(x) do { nmpc_status s__ = (x); if (s__ != NMPC_OK) return s__; } while (0)
+
+// ---- level schedule: which supernodes run in the shared-memory kernel, and the tile work lists of the big ones ----
+nmpc_status build_plan(nmpc_handle_s* h, int smem_max_r) {
+    const Symbolic& S = h->S;
+    std::vector<int32_t> small_list;
+    std::vector<BigItem> items;
+    h->plan.assign(S.nlevels, LevelPlan());
+    h->n_big_fronts = 0;
+    for (int l = 0; l < S.nlevels; ++l) {
+        LevelPlan& P = h->plan[l];
+        P.all_off = S.lvl_ptr[l]; P.all_cnt = S.lvl_ptr[l + 1] - S.lvl_ptr[l];
+        P.small_off = (int)small_list.size();
+        std::vector<int32_t> big;
+        for (int q = S.lvl_ptr[l]; q < S.lvl_ptr[l + 1]; ++q) {
+            const int s = S.lvl_sn[q];
+            const int r = (int)(S.rows_ptr[s + 1] - S.rows_ptr[s]);
+            P.all_max_r = std::max(P.all_max_r, r);
+            if (r <= smem_max_r) { small_list.push_back(s); P.small_max_r = std::max(P.small_max_r, r); }
+            else big.push_back(s);
+        }
+        P.small_cnt = (int)small_list.size() - P.small_off;
+        h->n_big_fronts += (int)big.size();
+        if (big.empty()) continue;
+        P.asm_off = (int)items.size();
+        int max_w = 0;
+        for (int s : big) {
+            const int r = (int)(S.rows_ptr[s + 1] - S.rows_ptr[s]), w = S.sn_start[s + 1] - S.sn_start[s];
+            max_w = std::max(max_w, w);
+            const int cw = std::max(4, std::min(64, 32768 / r));
+            for (int c = 0; c < r; c += cw) items.push_back(BigItem{s, c, std::min(r, c + cw), 0});
+        }
+        P.asm_cnt = (int)items.size() - P.asm_off;
+        const int nsteps = (max_w + BIG_NB - 1) / BIG_NB;
+        for (int t = 0; t < nsteps; ++t) {
+            StepPlan sp{};
+            const int j0 = t * BIG_NB;
+            sp.potrf_off = (int)items.size();
+            for (int s : big) { const int w = S.sn_start[s + 1] - S.sn_start[s]; if (j0 < w) items.push_back(BigItem{s, j0, 0, 0}); }
+            sp.potrf_cnt = (int)items.size() - sp.potrf_off;
+            sp.trsm_off = (int)items.size();
+            for (int s : big) {
+                const int r = (int)(S.rows_ptr[s + 1] - S.rows_ptr[s]), w = S.sn_start[s + 1] - S.sn_start[s];
+                if (j0 >= w) continue;
+                const int j1 = std::min(w, j0 + BIG_NB);
+                for (int i0 = j1; i0 < r; i0 += BIG_NB) items.push_back(BigItem{s, j0, i0, 0});
+            }
+            sp.trsm_cnt = (int)items.size() - sp.trsm_off;
+            sp.syrk_off = (int)items.size();
+            for (int s : big) {
+                const int r = (int)(S.rows_ptr[s + 1] - S.rows_ptr[s]), w = S.sn_start[s + 1] - S.sn_start[s];
+                if (j0 >= w) continue;
+                const int j1 = std::min(w, j0 + BIG_NB);
+                for (int J0 = j1; J0 < r; J0 += BIG_NB)
+                    for (int I0 = J0; I0 < r; I0 += BIG_NB) items.push_back(BigItem{s, j0, I0, J0});
+            }
+            sp.syrk_cnt = (int)items.size() - sp.syrk_off;
+            P.steps.push_back(sp);
+        }
+    }
+    const int32_t* tmp = nullptr;
+    TRY(upload(h, small_list, &tmp)); h->d_small_list = const_cast<int32_t*>(tmp);
+    TRY(upload(h, S.lvl_sn, &tmp)); h->d_lvl_sn = const_cast<int32_t*>(tmp);
+    const BigItem* ti = nullptr;
+    TRY(upload(h, items, &ti)); h->d_items = const_cast<BigItem*>(ti);
+    return NMPC_OK;
+}
+
+int issue_factor(nmpc_handle_s* h) {          // returns the number of kernels launched
+    int nk = 0;
+    for (const LevelPlan& P : h->plan) {
+        if (P.small_cnt) { launch_front_small(h->D, h->d_small_list + P.small_off, P.small_cnt, P.small_max_r, h->d_Kval, h->stream); ++nk; }
+        if (P.asm_cnt) { launch_big_assemble(h->D, h->d_items + P.asm_off, P.asm_cnt, h->d_Kval, h->stream); ++nk; }
+        for (const StepPlan& sp : P.steps) {
+            if (sp.potrf_cnt) { launch_big_potrf(h->D, h->d_items + sp.potrf_off, sp.potrf_cnt, h->stream); ++nk; }
+            if (sp.trsm_cnt) { launch_big_trsm(h->D, h->d_items + sp.trsm_off, sp.trsm_cnt, h->stream); ++nk; }
+            if (sp.syrk_cnt) { launch_big_syrk(h->D, h->d_items + sp.syrk_off, sp.syrk_cnt, h->stream); ++nk; }
+        }
+    }
+    return nk;
+}
+
+int issue_fwdbwd(nmpc_handle_s* h) {
+    int nk = 0;
+    for (size_t l = 0; l < h->plan.size(); ++l) {
+        const LevelPlan& P = h->plan[l];
+        launch_solve_fwd(h->D, h->d_lvl_sn + P.all_off, P.all_cnt, P.all_max_r, h->d_x, h->stream); ++nk;
+    }
+    for (size_t l = h->plan.size(); l-- > 0;) {
+        const LevelPlan& P = h->plan[l];
+        launch_solve_bwd(h->D, h->d_lvl_sn + P.all_off, P.all_cnt, P.all_max_r, h->d_x, h->stream); ++nk;
+    }
+    return nk;
+}
+
+nmpc_status capture(nmpc_handle_s* h, int (*issue)(nmpc_handle_s*), cudaGraphExec_t* out, int* nodes) {
+    cudaGraph_t g = nullptr;
+    CK(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
+    *nodes = issue(h);
+    CK(cudaStreamEndCapture(h->stream, &g));
+    CK(cudaGetLastError());
+    CK(cudaGraphInstantiate(out, g, 0));
+    cudaGraphDestroy(g);
+    return NMPC_OK;
+}
+
+nmpc_status run_factor(nmpc_handle_s* h, double eta, int64_t* info) {
+    launch_reset_flag(h->D, h->d_eta, eta, h->stream); h->launches++;
+    if (h->g_factor) { CK(cudaGraphLaunch(h->g_factor, h->stream)); h->launches += h->g_factor_nodes; }
+    else h->launches += issue_factor(h);
+    int32_t* flag = reinterpret_cast<int32_t*>(h->h_pinned + 16);
+    CK(cudaMemcpyAsync(flag, h->D.fail_col, sizeof(int32_t), cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    CK(cudaGetLastError());
+    h->eta_cur = eta;
+    if (*flag != INT_MAX) {
+        h->factored = false;
+        if (info) *info = h->S.perm[*flag];
+        return NMPC_E_NOT_SPD;
+    }
+    h->factored = true;
+    if (info) *info = -1;
+    return NMPC_OK;
+}
+
+nmpc_status run_solve(nmpc_handle_s* h, double* rhs) {       // in place, async
+    launch_permute_in(h->D, rhs, h->d_x, h->stream);
+    if (h->g_fwdbwd) { CK(cudaGraphLaunch(h->g_fwdbwd, h->stream)); h->launches += h->g_fwdbwd_nodes; }
+    else h->launches += issue_fwdbwd(h);
+    launch_permute_out(h->D, h->d_x, rhs, h->stream);
+    h->launches += 2;
+    return NMPC_OK;
+}
+
+struct PhaseTimer {                 // optional CUDA-event phase timing (opt.time_phases)
+    nmpc_handle_s* h; bool on; double* acc = nullptr;
+    void begin(double* a) { if (!on) return; acc = a; cudaEventRecord(h->ev[0], h->stream); }
+    void end() { if (!on || !acc) return; cudaEventRecord(h->ev[1], h->stream); cudaEventSynchronize(h->ev[1]); float ms = 0; cudaEventElapsedTime(&ms, h->ev[0], h->ev[1]); *acc += ms; acc = nullptr; }
+};
+
+}  // namespace
+
+extern "C" {
+
+nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const nmpc_options* opt, void* cuda_stream, nmpc_handle* out) {
+    if (!out) return NMPC_E_ARG;
+    *out = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return NMPC_E_CUDA; }
+    nmpc_handle_s* h = new (std::nothrow) nmpc_handle_s();
+    if (!h) return NMPC_E_ALLOC;
+    auto fail = [&](nmpc_status s) { std::fprintf(stderr, "nmpc_analyze: %s\n", h->err.c_str()); nmpc_destroy(h); return s; };
+    if (opt) h->opt = *opt; else default_options(&h->opt);
+    if (h->opt.mu_warm <= 0.0) h->opt.mu_warm = h->opt.eps_outer / 10.0;
+    h->stream = (cudaStream_t)cuda_stream;
+    nmpc_status st;
+    try { st = analyze_symbolic(pattern, ocp, &h->opt, h->S); }
+    catch (const std::bad_alloc&) { st = NMPC_E_ALLOC; h->err = "host allocation failed"; }
+    if (st != NMPC_OK) { h->err = h->S.error; return fail(st); }
+    auto body = [&]() -> nmpc_status {
+        const Symbolic& S = h->S;
+        int dev = 0, smem_optin = 0;
+        CK(cudaGetDevice(&dev));
+        CK(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+        CK(configure_factor_kernels(smem_optin));
+        int smem_max_r = (int)std::floor(std::sqrt((double)smem_optin / 8.0));
+        if (h->opt.smem_front_max > 0) smem_max_r = std::min(smem_max_r, h->opt.smem_front_max);
+        else smem_max_r = std::min(smem_max_r, 160);
+        if (((size_t)((S.max_front + 1) & ~1) + (size_t)BIG_NB * (BIG_NB + 1)) * 8 > (size_t)smem_optin) { h->err = "front too large for the solve kernel"; return NMPC_E_ALLOC; }
+        DevSym& D = h->D;
+        D.ns = S.ns; D.n = S.n;
+        TRY(upload(h, S.sn_start, &D.sn_start)); TRY(upload(h, S.rows_ptr, &D.rows_ptr)); TRY(upload(h, S.rows, &D.rows));
+        TRY(upload(h, S.child_ptr, &D.child_ptr)); TRY(upload(h, S.child_idx, &D.child_idx));
+        TRY(upload(h, S.rel_ptr, &D.rel_ptr)); TRY(upload(h, S.rel, &D.rel));
+        TRY(upload(h, S.panel_ptr, &D.panel_ptr)); TRY(upload(h, S.upd_ptr, &D.upd_ptr));
+        TRY(upload(h, S.kent_ptr, &D.kent_ptr)); TRY(upload(h, S.kent_src, &D.kent_src)); TRY(upload(h, S.kent_dst, &D.kent_dst));
+        TRY(upload(h, S.perm, &D.perm));
+        TRY(dalloc(h, (size_t)S.panel_ptr.back(), &D.L)); TRY(dalloc(h, (size_t)S.upd_ptr.back(), &D.U, false));
+        TRY(dalloc(h, (size_t)S.rel_ptr.back(), &D.ctr)); TRY(dalloc(h, 1, &D.fail_col));
+        TRY(dalloc(h, 1, &h->d_eta)); D.eta = h->d_eta;
+        TRY(dalloc(h, (size_t)S.nnzK, &h->d_Kval)); TRY(dalloc(h, (size_t)S.n, &h->d_x));
+        TRY(build_plan(h, smem_max_r));
+        // symmetric CSR of K for nmpc_kkt_multiply
+        {
+            const int64_t n = S.n;
+            std::vector<int64_t> ptr(n + 1, 0);
+            for (int64_t i = 0; i < n; ++i)
+                for (int64_t p = S.K.ptr[i]; p < S.K.ptr[i + 1]; ++p) { ptr[i + 1]++; if (S.K.idx[p] != i) ptr[S.K.idx[p] + 1]++; }
+            for (int64_t i = 0; i < n; ++i) ptr[i + 1] += ptr[i];
+            std::vector<int32_t> idx(ptr[n]), src(ptr[n]);
+            std::vector<int64_t> pos(ptr.begin(), ptr.end() - 1);
+            for (int64_t i = 0; i < n; ++i)
+                for (int64_t p = S.K.ptr[i]; p < S.K.ptr[i + 1]; ++p) {
+                    const int32_t j = S.K.idx[p];
+                    idx[pos[i]] = j; src[pos[i]++] = (int32_t)p;
+                    if (j != i) { idx[pos[j]] = (int32_t)i; src[pos[j]++] = (int32_t)p; }
+                }
+            const int64_t* tp = nullptr; const int32_t* ti = nullptr;
+            TRY(upload(h, ptr, &tp)); h->d_full_ptr = const_cast<int64_t*>(tp);
+            TRY(upload(h, idx, &ti)); h->d_full_idx = const_cast<int32_t*>(ti);
+            TRY(upload(h, src, &ti)); h->d_full_src = const_cast<int32_t*>(ti);
+        }
+        size_t pinned = 64;
+        if (S.mm.present) {
+            const ModelMaps& mm = S.mm;
+            DevModel& M = h->M;
+            h->has_model = true;
+            M.desc = mm.desc; M.n = mm.n; M.m = mm.m; M.nnzJ = mm.J.nnz(); M.nnzW = mm.W.nnz(); M.nnzK = mm.K.nnz();
+            TRY(upload(h, mm.J.ptr, &M.J_ptr)); TRY(upload(h, mm.J.idx, &M.J_idx));
+            TRY(upload(h, mm.jt_ptr, &M.jt_ptr)); TRY(upload(h, mm.jt_idx, &M.jt_idx)); TRY(upload(h, mm.jt_row, &M.jt_row));
+            TRY(upload(h, mm.trip_ptr, &M.trip_ptr)); TRY(upload(h, mm.trip_a, &M.trip_a)); TRY(upload(h, mm.trip_b, &M.trip_b)); TRY(upload(h, mm.trip_r, &M.trip_r));
+            TRY(upload(h, mm.k_w, &M.k_w)); TRY(upload(h, mm.k_diag, &M.k_diag));
+            const int nv = mm.desc.nv;
+            std::vector<double> lb(mm.n), ub(mm.n), ui(std::max(1, mm.desc.nu), 0.0);
+            h->nmult = 2 * (int)mm.m;
+            for (int64_t i = 0; i < mm.n; ++i) {
+                lb[i] = ocp->lb ? ocp->lb[i % nv] : -INFINITY; ub[i] = ocp->ub ? ocp->ub[i % nv] : INFINITY;
+                if (std::isfinite(lb[i])) h->nmult++;
+                if (std::isfinite(ub[i])) h->nmult++;
+                if (!(lb[i] < ub[i])) { h->err = "lb >= ub"; return NMPC_E_ARG; }
+            }
+            for (int a = 0; a < mm.desc.nu; ++a) ui[a] = ocp->u_init ? ocp->u_init[a] : 0.0;
+            TRY(upload(h, lb, &M.lb)); TRY(upload(h, ub, &M.ub));
+            const double* tu = nullptr; TRY(upload(h, ui, &tu)); h->d_uinit = const_cast<double*>(tu);
+            TRY(dalloc(h, (size_t)mm.desc.nx, &M.x0)); TRY(dalloc(h, (size_t)std::max<int64_t>(1, (int64_t)mm.desc.N * mm.desc.nr), &M.ref));
+            IpmVectors& V = h->V;
+            const size_t n = mm.n, m = mm.m;
+            TRY(dalloc(h, n, &V.y)); TRY(dalloc(h, m, &V.sp)); TRY(dalloc(h, m, &V.sm)); TRY(dalloc(h, m, &V.wp)); TRY(dalloc(h, m, &V.wm));
+            TRY(dalloc(h, n, &V.zL)); TRY(dalloc(h, n, &V.zU)); TRY(dalloc(h, m, &V.c)); TRY(dalloc(h, n, &V.gradf));
+            TRY(dalloc(h, (size_t)M.nnzJ, &V.Jval)); TRY(dalloc(h, (size_t)M.nnzW, &V.Wval));
+            V.Kval = h->d_Kval;
+            TRY(dalloc(h, m, &V.r_pp)); TRY(dalloc(h, m, &V.r_pm)); TRY(dalloc(h, m, &V.q)); TRY(dalloc(h, m, &V.t));
+            TRY(dalloc(h, n, &V.sigx)); TRY(dalloc(h, n, &V.b)); TRY(dalloc(h, n, &V.dy));
+            TRY(dalloc(h, m, &V.dsp)); TRY(dalloc(h, m, &V.dsm)); TRY(dalloc(h, m, &V.dwp)); TRY(dalloc(h, m, &V.dwm));
+            TRY(dalloc(h, n, &V.dzL)); TRY(dalloc(h, n, &V.dzU));
+            TRY(dalloc(h, (size_t)RED_BLOCKS * 8, &V.partial)); TRY(dalloc(h, (size_t)NSCAL, &V.scal));
+            pinned += (size_t)mm.desc.nx + (size_t)mm.desc.N * mm.desc.nr + n;
+        }
+        h->pinned_doubles = pinned;
+        CK(cudaMallocHost((void**)&h->h_pinned, pinned * sizeof(double)));
+        CK(cudaEventCreate(&h->ev[0])); CK(cudaEventCreate(&h->ev[1]));
+        CK(cudaStreamSynchronize(h->stream));
+        if (h->opt.use_graph) {
+            TRY(capture(h, issue_factor, &h->g_factor, &h->g_factor_nodes));
+            TRY(capture(h, issue_fwdbwd, &h->g_fwdbwd, &h->g_fwdbwd_nodes));
+        }
+        return NMPC_OK;
+    };
+    st = body();
+    if (st != NMPC_OK) return fail(st);
+    *out = h;
+    return NMPC_OK;
+}
+
+void nmpc_destroy(nmpc_handle h) {
+    if (!h) return;
+    if (h->g_factor) cudaGraphExecDestroy(h->g_factor);
+    if (h->g_fwdbwd) cudaGraphExecDestroy(h->g_fwdbwd);
+    for (void* p : h->allocs) cudaFree(p);
+    if (h->h_pinned) cudaFreeHost(h->h_pinned);
+    if (h->ev[0]) cudaEventDestroy(h->ev[0]);
+    if (h->ev[1]) cudaEventDestroy(h->ev[1]);
+    delete h;
+}
+
+const char* nmpc_last_error(nmpc_handle h) { return h ? h->err.c_str() : "null handle"; }
+int64_t nmpc_launch_count(nmpc_handle h) { return h ? h->launches : 0; }
+
+nmpc_status nmpc_get_info(nmpc_handle h, nmpc_sym_info* out) {
+    if (!h || !out) return NMPC_E_ARG;
+    nmpc_fill_info(h->S, out);
+    out->n_large_fronts = h->n_big_fronts;
+    return NMPC_OK;
+}
+
+nmpc_status nmpc_get_factor(nmpc_handle h, double* panels_host) {
+    if (!h || !panels_host) return NMPC_E_ARG;
+    if (!h->factored) { h->err = "no successful factorization"; return NMPC_E_STATE; }
+    CK(cudaMemcpyAsync(panels_host, h->D.L, (size_t)h->S.panel_ptr.back() * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    return NMPC_OK;
+}
+
+nmpc_status nmpc_factor(nmpc_handle h, const double* values_dev, double eta, int64_t* info_host) {
+    if (!h || !values_dev) return NMPC_E_ARG;
+    if (values_dev != h->d_Kval)
+        CK(cudaMemcpyAsync(h->d_Kval, values_dev, (size_t)h->S.nnzK * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+    return run_factor(h, eta, info_host);
+}
+
+nmpc_status nmpc_solve(nmpc_handle h, double* rhs, int32_t nrhs) {
+    if (!h || !rhs || nrhs < 1) return NMPC_E_ARG;
+    if (!h->factored) { h->err = "nmpc_solve before a successful nmpc_factor"; return NMPC_E_STATE; }
+    for (int k = 0; k < nrhs; ++k) TRY(run_solve(h, rhs + (int64_t)k * h->S.n));
+    CK(cudaGetLastError());
+    return NMPC_OK;
+}
+
+nmpc_status nmpc_kkt_multiply(nmpc_handle h, const double* x_dev, double* y_dev) {
+    if (!h || !x_dev || !y_dev) return NMPC_E_ARG;
+    launch_kkt_multiply(h->S.n, h->d_full_ptr, h->d_full_idx, h->d_full_src, h->d_Kval, h->eta_cur, x_dev, y_dev, h->stream);
+    h->launches++;
+    CK(cudaGetLastError());
+    return NMPC_OK;
+}
+
+nmpc_status nmpc_update_params(nmpc_handle h, const double* x0_dev, const double* ref_dev) {
+    if (!h) return NMPC_E_ARG;
+    if (!h->has_model) { h->err = "handle has no model"; return NMPC_E_STATE; }
+    const ModelDesc& d = h->M.desc;
+    if (x0_dev) CK(cudaMemcpyAsync(h->M.x0, x0_dev, sizeof(double) * d.nx, cudaMemcpyDeviceToDevice, h->stream));
+    if (ref_dev && d.nr > 0) CK(cudaMemcpyAsync(h->M.ref, ref_dev, sizeof(double) * (size_t)d.N * d.nr, cudaMemcpyDeviceToDevice, h->stream));
+    return NMPC_OK;
+}
+
+nmpc_status nmpc_update_params_host(nmpc_handle h, const double* x0_host, const double* ref_host) {
+    if (!h) return NMPC_E_ARG;
+    if (!h->has_model) { h->err = "handle has no model"; return NMPC_E_STATE; }
+    const ModelDesc& d = h->M.desc;
+    double* stage = h->h_pinned + 64;
+    CK(cudaStreamSynchronize(h->stream));               // staging buffer reuse
+    if (x0_host) {
+        std::memcpy(stage, x0_host, sizeof(double) * d.nx);
+        CK(cudaMemcpyAsync(h->M.x0, stage, sizeof(double) * d.nx, cudaMemcpyHostToDevice, h->stream));
+    }
+    if (ref_host && d.nr > 0) {
+        double* s2 = stage + d.nx;
+        std::memcpy(s2, ref_host, sizeof(double) * (size_t)d.N * d.nr);
+        CK(cudaMemcpyAsync(h->M.ref, s2, sizeof(double) * (size_t)d.N * d.nr, cudaMemcpyHostToDevice, h->stream));
+    }
+    return NMPC_OK;
+}
+
+nmpc_status nmpc_get_iterate(nmpc_handle h, double* y, double* sp, double* sm, double* wp, double* wm, double* zL, double* zU) {
+    if (!h) return NMPC_E_ARG;
+    if (!h->has_model) return NMPC_E_STATE;
+    const size_t n = h->M.n * sizeof(double), m = h->M.m * sizeof(double);
+    const IpmVectors& V = h->V;
+    if (y) CK(cudaMemcpyAsync(y, V.y, n, cudaMemcpyDeviceToDevice, h->stream));
+    if (sp) CK(cudaMemcpyAsync(sp, V.sp, m, cudaMemcpyDeviceToDevice, h->stream));
+    if (sm) CK(cudaMemcpyAsync(sm, V.sm, m, cudaMemcpyDeviceToDevice, h->stream));
+    if (wp) CK(cudaMemcpyAsync(wp, V.wp, m, cudaMemcpyDeviceToDevice, h->stream));
+    if (wm) CK(cudaMemcpyAsync(wm, V.wm, m, cudaMemcpyDeviceToDevice, h->stream));
+    if (zL) CK(cudaMemcpyAsync(zL, V.zL, n, cudaMemcpyDeviceToDevice, h->stream));
+    if (zU) CK(cudaMemcpyAsync(zU, V.zU, n, cudaMemcpyDeviceToDevice, h->stream));
+    return NMPC_OK;
+}
+
+nmpc_status nmpc_model_eval(nmpc_handle h, const double* y, const double* lam, double* c, double* gradf, double* Jval, double* Wval) {
+    if (!h || !y) return NMPC_E_ARG;
+    if (!h->has_model) return NMPC_E_STATE;
+    if (Wval && !lam) return NMPC_E_ARG;
+    launch_model_eval(h->M, y, nullptr, nullptr, lam, c, gradf, Jval, Wval, h->stream);
+    h->launches++;
+    CK(cudaGetLastError());
+    return NMPC_OK;
+}
+
+nmpc_status nmpc_assemble(nmpc_handle h, const double* Jval, const double* Wval, const double* sigx, const double* q, double eta, double* Kval) {
+    if (!h || !Jval || !Wval || !sigx || !q || !Kval) return NMPC_E_ARG;
+    if (!h->has_model) return NMPC_E_STATE;
+    launch_assemble_K(h->M, Jval, Wval, sigx, q, eta, Kval, h->stream);
+    h->launches++;
+    CK(cudaGetLastError());
+    return NMPC_OK;
+}
+
+nmpc_status nmpc_get_jac_pattern(nmpc_handle h, int64_t* nnz, int64_t* rowptr, int32_t* colind) {
+    if (!h) return NMPC_E_ARG;
+    if (!h->has_model) return NMPC_E_STATE;
+    return nmpc_copy_pattern_internal(h->S.mm.J, nnz, rowptr, colind);
+}
+nmpc_status nmpc_get_hess_pattern(nmpc_handle h, int64_t* nnz, int64_t* rowptr, int32_t* colind) {
+    if (!h) return NMPC_E_ARG;
+    if (!h->has_model) return NMPC_E_STATE;
+    return nmpc_copy_pattern_internal(h->S.mm.W, nnz, rowptr, colind);
+}
+nmpc_status nmpc_get_kkt_pattern(nmpc_handle h, int64_t* nnz, int64_t* rowptr, int32_t* colind) {
+    if (!h) return NMPC_E_ARG;
+    return nmpc_copy_pattern_internal(h->S.K, nnz, rowptr, colind);
+}
+
+// ---- Algorithm 2 (LiftedIPM), steps S1..S10 of DESIGN.md section 3 ----
+nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* y_inout, nmpc_stats* stats, nmpc_trace_row* trace, int32_t trace_cap) {
+    if (!h) return NMPC_E_ARG;
+    if (!h->has_model) { h->err = "nmpc_ipm_solve needs a model (nmpc_ocp)"; return NMPC_E_STATE; }
+    if (use_y0 && !y_inout) return NMPC_E_ARG;
+    const nmpc_options& o = h->opt;
+    const DevModel& M = h->M;
+    const IpmVectors& V = h->V;
+    cudaStream_t st = h->stream;
+    auto t_begin = std::chrono::steady_clock::now();
+    nmpc_stats S{};
+    PhaseTimer pt{h, o.time_phases != 0 && stats != nullptr};
+    double mu;
+    if (warm && h->have_state) {                                               // S1 warm: z <- z* (Alg. 1 line 10)
+        launch_warm_push(M, V, o.warm_push, st); h->launches++;
+        mu = o.mu_warm;
+    } else {                                                                   // S1 cold
+        if (use_y0) CK(cudaMemcpyAsync(V.y, y_inout, sizeof(double) * M.n, cudaMemcpyDeviceToDevice, st));
+        launch_cold_init_y(M, V, h->d_uinit, use_y0, o.kappa_push, o.mu0, st);
+        launch_model_eval(M, V.y, nullptr, nullptr, nullptr, V.c, nullptr, nullptr, nullptr, st);
+        launch_cold_init_s(M, V, o.gamma, o.s_floor, o.mu0, st);
+        h->launches += 3;
+        mu = o.mu0;
+    }
+    double eta_last = 0.0, E0 = 0.0;
+    int it = 0, nfact = 0, retries = 0;
+    nmpc_status status = NMPC_E_MAXITER;
+    double* hs = h->h_pinned;
+    while (true) {
+        // S2: evaluate c, grad f, J, W (K_SIMD of the paper, Alg. 2 line 5) and the residuals of Eq. (9)
+        pt.begin(&S.ms_eval);
+        launch_model_eval(M, V.y, V.wp, V.wm, nullptr, V.c, V.gradf, V.Jval, V.Wval, st); h->launches++;
+        pt.end();
+        pt.begin(&S.ms_vector);
+        launch_residuals(M, V, o.gamma, st); h->launches += 2;
+        CK(cudaMemcpyAsync(hs, V.scal, sizeof(double) * 10, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        pt.end();
+        if (it > 0 && trace && it - 1 < trace_cap) { trace[it - 1].alpha_pr = hs[7]; trace[it - 1].alpha_du = hs[8]; }
+        if (hs[6] != 0.0) { status = NMPC_E_STEP; break; }
+        const double l1 = hs[5];
+        const double s_d = std::max(o.s_max, l1 / (double)h->nmult) / o.s_max;
+        auto err_mu = [&](double m_) {
+            const double comp = std::max(std::fabs(hs[3] - m_), std::fabs(hs[4] - m_));
+            return std::max(std::max(hs[0] / s_d, hs[1]), std::max(hs[2], comp / s_d));
+        };
+        E0 = err_mu(0.0);
+        if (E0 <= o.eps_outer) { status = NMPC_OK; break; }                     // S3: Eq. (28)
+        if (it >= o.max_iter) { status = NMPC_E_MAXITER; break; }
+        double Emu = err_mu(mu);                                               // S4: Eq. (27), barrier update
+        while (Emu <= o.kappa_eps * mu && mu > o.eps_outer / 10.0) {
+            mu = std::max(o.eps_outer / 10.0, std::min(o.kappa_mu * mu, std::pow(mu, o.theta_mu)));
+            Emu = err_mu(mu);
+        }
+        const double tau = std::max(o.tau_min, 1.0 - mu);                      // S5
+        pt.begin(&S.ms_vector);
+        launch_sigma_rhs(M, V, mu, st); h->launches += 2;                      // S6
+        pt.end();
+        pt.begin(&S.ms_assemble);
+        launch_assemble_K(M, V.Jval, V.Wval, V.sigx, V.q, 0.0, V.Kval, st); h->launches++;
+        pt.end();
+        double eta = 0.0;                                                      // S7: inertia correction, Eq. (13)/(15)
+        while (true) {
+            ++nfact;
+            pt.begin(&S.ms_factor);
+            nmpc_status fs = run_factor(h, eta, nullptr);
+            pt.end();
+            if (fs == NMPC_OK) break;
+            if (fs != NMPC_E_NOT_SPD) return fs;
+            ++retries;
+            if (eta == 0.0) eta = (eta_last == 0.0) ? o.eta_first : std::max(o.eta_min, o.eta_shrink * eta_last);
+            else eta = ((eta_last == 0.0) ? o.eta_grow_first : o.eta_grow) * eta;
+            if (eta > o.eta_max) { status = NMPC_E_INERTIA; goto done; }
+        }
+        if (eta > 0.0) eta_last = eta;
+        pt.begin(&S.ms_solve);                                                 // S8: Eq. (22)-(25)
+        CK(cudaMemcpyAsync(V.dy, V.b, sizeof(double) * M.n, cudaMemcpyDeviceToDevice, st));
+        TRY(run_solve(h, V.dy));
+        pt.end();
+        pt.begin(&S.ms_vector);
+        launch_step(M, V, mu, tau, st); h->launches += 2;                      // S8-S9
+        launch_update(M, V, st); h->launches++;                                // S10: Eq. (26)
+        pt.end();
+        if (trace && it < trace_cap) { trace[it].mu = mu; trace[it].E0 = E0; trace[it].Emu = Emu; trace[it].eta = eta; trace[it].alpha_pr = trace[it].alpha_du = 0.0; }
+        ++it;
+    }
+done:
+    h->have_state = true;
+    launch_objective(M, V, st); h->launches += 2;
+    CK(cudaMemcpyAsync(hs + 9, V.scal + 9, sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (y_inout) CK(cudaMemcpyAsync(y_inout, V.y, sizeof(double) * M.n, cudaMemcpyDeviceToDevice, st));
+    CK(cudaStreamSynchronize(st));
+    CK(cudaGetLastError());
+    S.status = status; S.iters = it; S.factorizations = nfact; S.eta_retries = retries; S.E0 = E0; S.mu = mu; S.eta_last = eta_last;
+    S.objective = hs[9];
+    S.ms_total = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
+    if (stats) *stats = S;
+    return status;
+}
+
+nmpc_status nmpc_ipm_solve_host(nmpc_handle h, int32_t warm, const double* x0_host, const double* ref_host, double* y_out_host, nmpc_stats* stats) {
+    if (!h) return NMPC_E_ARG;
+    TRY(nmpc_update_params_host(h, x0_host, ref_host));
+    nmpc_status st = nmpc_ipm_solve(h, warm, 0, nullptr, stats, nullptr, 0);
+    if (y_out_host) {
+        double* stage = h->h_pinned + 64 + h->M.desc.nx + (size_t)h->M.desc.N * h->M.desc.nr;
+        CK(cudaMemcpyAsync(stage, h->V.y, sizeof(double) * h->M.n, cudaMemcpyDeviceToHost, h->stream));
+        CK(cudaStreamSynchronize(h->stream));
+        std::memcpy(y_out_host, stage, sizeof(double) * h->M.n);
+    }
+    return st;
+}
+
+}  // extern "C"

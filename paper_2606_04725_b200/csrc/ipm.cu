@@ -1,0 +1,365 @@
+// ipm.cu -- model/derivative evaluation (step a2), condensed lifted KKT assembly (step a3, Eq. 14/17)
+// and the fused IPM vector kernels (step a6: residuals of Eq. 9/11, right-hand side of Eq. 17, eliminated directions of
+// Eq. 10/14, fraction-to-the-boundary min-reductions, Eq. 26 update, error norms of Eq. 27-28).
+//
+// Reductions use a FIXED grid (RED_BLOCKS x 256 threads, grid-stride) and a fixed shuffle/shared-memory tree, then a
+// one-block finalize kernel: results are bitwise reproducible run to run.  No floating-point atomics anywhere.
+// Compiled with -fmad=false: the element-wise expressions below round like the plain fp64 statements of the method.
+#include <algorithm>
+#include <cfloat>
+#include <climits>
+
+#include "device.h"
+
+namespace nmpc {
+
+namespace {
+
+constexpr int NT = 256;
+constexpr double INF = __builtin_huge_val();
+
+struct LamDiff { const double* p; const double* m; __device__ __forceinline__ double operator[](int i) const { return p[i] - m[i]; } };
+
+// ------------------------------------------------------------------------------------------------------------
+// a2: one thread per Jacobian row / per variable / per Hessian entry
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(NT) model_eval_kernel(DevModel M, const double* __restrict__ y, const double* __restrict__ wp,
+                                                        const double* __restrict__ wm, const double* __restrict__ lam_in,
+                                                        double* __restrict__ c_out, double* __restrict__ gradf,
+                                                        double* __restrict__ Jval, double* __restrict__ Wval) {
+    const ModelDesc& D = M.desc;
+    const int nx = D.nx, nv = D.nv;
+    const int hc = hess_count(D);
+    const int64_t nW = (int64_t)D.N * hc;
+    const int64_t idx = blockIdx.x * (int64_t)NT + threadIdx.x;
+    if (idx < M.m) {                                             // constraint row (k, c): h and its Jacobian row
+        if (!c_out && !Jval) return;
+        const int k = (int)(idx / nx), c = (int)(idx - (int64_t)k * nx);
+        const double* x = y + (int64_t)k * nv;
+        const double* u = x + nx;
+        int64_t pos = M.J_ptr[idx];
+        double xprev;
+        if (k > 0) { xprev = y[(int64_t)(k - 1) * nv + c]; if (Jval) Jval[pos] = -1.0; ++pos; }
+        else xprev = M.x0[c];
+        const double F = model_row(D, c, x, u, [&](int, double v) { if (Jval) Jval[pos] = v; ++pos; });
+        if (c_out) c_out[idx] = x[c] - xprev - D.dt * F;
+    } else if (idx < M.m + M.n) {                                // gradient entry
+        if (!gradf) return;
+        const int64_t v = idx - M.m;
+        const int k = (int)(v / nv), a = (int)(v - (int64_t)k * nv);
+        const double* x = y + (int64_t)k * nv;
+        gradf[v] = cost_grad(D, a, x, x + nx, M.ref + (int64_t)k * D.nr);
+    } else if (idx < M.m + M.n + nW) {                           // Lagrangian Hessian entry, lam = w+ - w-
+        if (!Wval) return;
+        const int64_t q = idx - M.m - M.n;
+        const int k = (int)(q / hc), e = (int)(q - (int64_t)k * hc);
+        const double* x = y + (int64_t)k * nv;
+        const int64_t r0 = (int64_t)k * nx;
+        if (lam_in) { Wval[q] = hess_val(D, e, x, x + nx, lam_in + r0); return; }
+        LamDiff lam{wp + r0, wm + r0};                           // lam = w+ - w- formed on the fly
+        Wval[q] = hess_val(D, e, x, x + nx, lam);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// a3: K = W + diag(Sigma_x + eta) + J^T diag(q) J on the fixed pattern, one thread per K entry (gather form)
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(NT) assemble_K_kernel(DevModel M, const double* __restrict__ Jval, const double* __restrict__ Wval,
+                                                        const double* __restrict__ sigx, const double* __restrict__ q,
+                                                        double eta, double* __restrict__ Kval) {
+    const int64_t e = blockIdx.x * (int64_t)NT + threadIdx.x;
+    if (e >= M.nnzK) return;
+    double acc = 0.0;
+    for (int64_t p = M.trip_ptr[e]; p < M.trip_ptr[e + 1]; ++p)
+        acc += Jval[M.trip_a[p]] * q[M.trip_r[p]] * Jval[M.trip_b[p]];
+    const int wi = M.k_w[e], di = M.k_diag[e];
+    if (wi >= 0) acc += Wval[wi];
+    if (di >= 0) acc += sigx[di] + eta;
+    Kval[e] = acc;
+}
+
+// y = (K + eta I) x from the full symmetric CSR (ptr/idx index the lower-pattern value array through src)
+__global__ void __launch_bounds__(NT) kkt_multiply_kernel(int64_t n, const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx,
+                                                          const int32_t* __restrict__ src, const double* __restrict__ Kval,
+                                                          double eta, const double* __restrict__ x, double* __restrict__ y) {
+    const int64_t i = blockIdx.x * (int64_t)NT + threadIdx.x;
+    if (i >= n) return;
+    double acc = eta * x[i];
+    for (int64_t p = ptr[i]; p < ptr[i + 1]; ++p) acc += Kval[src[p]] * x[idx[p]];
+    y[i] = acc;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// block reductions (fixed tree)
+// ------------------------------------------------------------------------------------------------------------
+template <int NV>
+struct Red { double v[NV]; };
+
+// op codes per slot: 0 = max, 1 = min, 2 = sum
+template <int NV>
+__device__ __forceinline__ void block_reduce(Red<NV>& a, const int* ops, double* out /* NV */) {
+    __shared__ double sh[NV][NT / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < NV; ++k) {
+        double v = a.v[k];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const double w = __shfl_xor_sync(0xffffffffu, v, o);
+            v = ops[k] == 0 ? fmax(v, w) : (ops[k] == 1 ? fmin(v, w) : v + w);
+        }
+        if (lane == 0) sh[k][warp] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < NV; ++k) {
+            double v = sh[k][0];
+            for (int w2 = 1; w2 < NT / 32; ++w2) v = ops[k] == 0 ? fmax(v, sh[k][w2]) : (ops[k] == 1 ? fmin(v, sh[k][w2]) : v + sh[k][w2]);
+            out[k] = v;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// S1 cold start: push y0 into the interior, slacks from c, multipliers mu0/(.)
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(NT) cold_y_kernel(DevModel M, IpmVectors V, const double* __restrict__ u_init, int use_y0,
+                                                    double kp, double mu0) {
+    const int64_t i = blockIdx.x * (int64_t)NT + threadIdx.x;
+    if (i >= M.n) return;
+    const int nv = M.desc.nv, nx = M.desc.nx;
+    const int a = (int)(i % nv);
+    double y = use_y0 ? V.y[i] : (a < nx ? M.x0[a] : u_init[a - nx]);
+    const double lb = M.lb[i], ub = M.ub[i];
+    const bool hasL = lb > -INF, hasU = ub < INF;
+    double pL = kp * fmax(1.0, fabs(lb)), pU = kp * fmax(1.0, fabs(ub));
+    if (hasL && hasU) { pL = fmin(pL, kp * (ub - lb)); pU = fmin(pU, kp * (ub - lb)); }
+    if (hasL) y = fmax(y, lb + pL);
+    if (hasU) y = fmin(y, ub - pU);
+    V.y[i] = y;
+    V.zL[i] = hasL ? mu0 / (y - lb) : 0.0;
+    V.zU[i] = hasU ? mu0 / (ub - y) : 0.0;
+}
+
+__global__ void __launch_bounds__(NT) cold_s_kernel(DevModel M, IpmVectors V, double gamma, double s_floor, double mu0) {
+    const int64_t r = blockIdx.x * (int64_t)NT + threadIdx.x;
+    if (r >= M.m) return;
+    const double c = V.c[r];
+    const double sp = fmax(gamma - c, s_floor), sm = fmax(gamma + c, s_floor);
+    V.sp[r] = sp; V.sm[r] = sm; V.wp[r] = mu0 / sp; V.wm[r] = mu0 / sm;
+}
+
+__global__ void __launch_bounds__(NT) warm_push_kernel(DevModel M, IpmVectors V, double wpush) {
+    const int64_t i = blockIdx.x * (int64_t)NT + threadIdx.x;
+    if (i >= M.n) return;
+    double y = V.y[i];
+    const double lb = M.lb[i], ub = M.ub[i];
+    if (lb > -INF) y = fmax(y, lb + wpush);
+    if (ub < INF) y = fmin(y, ub - wpush);
+    V.y[i] = y;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// S2: residuals of the smoothed KKT system (Eq. 9) and the ingredients of E_mu (Eq. 27/28)
+//   partial[b][0..6] = max|r_d|, max|r_p+|, max|r_p-|, max comp product, min comp product, sum multipliers, #non-finite
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(NT) residual_kernel(DevModel M, IpmVectors V, double gamma) {
+    Red<7> a;
+    a.v[0] = a.v[1] = a.v[2] = 0.0; a.v[3] = -INF; a.v[4] = INF; a.v[5] = 0.0; a.v[6] = 0.0;
+    const int64_t total = M.n + M.m;
+    for (int64_t idx = blockIdx.x * (int64_t)NT + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * NT) {
+        if (idx < M.n) {
+            const int64_t i = idx;
+            double jt = 0.0;
+            for (int64_t p = M.jt_ptr[i]; p < M.jt_ptr[i + 1]; ++p) { const int r = M.jt_row[p]; jt += V.Jval[M.jt_idx[p]] * (V.wp[r] - V.wm[r]); }
+            const double lb = M.lb[i], ub = M.ub[i], y = V.y[i];
+            const bool hasL = lb > -INF, hasU = ub < INF;
+            const double zL = hasL ? V.zL[i] : 0.0, zU = hasU ? V.zU[i] : 0.0;
+            const double rd = V.gradf[i] + jt - zL + zU;
+            a.v[0] = fmax(a.v[0], fabs(rd));
+            if (!isfinite(rd) || !isfinite(y)) a.v[6] += 1.0;
+            if (hasL) { const double cp = (y - lb) * zL; a.v[3] = fmax(a.v[3], cp); a.v[4] = fmin(a.v[4], cp); a.v[5] += zL; }
+            if (hasU) { const double cp = (ub - y) * zU; a.v[3] = fmax(a.v[3], cp); a.v[4] = fmin(a.v[4], cp); a.v[5] += zU; }
+        } else {
+            const int64_t r = idx - M.n;
+            const double c = V.c[r], sp = V.sp[r], sm = V.sm[r], wp = V.wp[r], wm = V.wm[r];
+            const double rpp = c - gamma + sp, rpm = -c - gamma + sm;
+            V.r_pp[r] = rpp; V.r_pm[r] = rpm;
+            a.v[1] = fmax(a.v[1], fabs(rpp)); a.v[2] = fmax(a.v[2], fabs(rpm));
+            if (!isfinite(rpp) || !isfinite(rpm)) a.v[6] += 1.0;
+            const double c1 = sp * wp, c2 = sm * wm;
+            a.v[3] = fmax(a.v[3], fmax(c1, c2)); a.v[4] = fmin(a.v[4], fmin(c1, c2));
+            a.v[5] += wp + wm;
+        }
+    }
+    const int ops[7] = {0, 0, 0, 0, 1, 2, 2};
+    block_reduce<7>(a, ops, V.partial + (int64_t)blockIdx.x * 8);
+}
+
+__global__ void __launch_bounds__(NT) finalize_residual_kernel(IpmVectors V, int nblocks) {
+    Red<7> a;
+    a.v[0] = a.v[1] = a.v[2] = 0.0; a.v[3] = -INF; a.v[4] = INF; a.v[5] = 0.0; a.v[6] = 0.0;
+    for (int b = threadIdx.x; b < nblocks; b += NT) {
+        const double* p = V.partial + (int64_t)b * 8;
+        a.v[0] = fmax(a.v[0], p[0]); a.v[1] = fmax(a.v[1], p[1]); a.v[2] = fmax(a.v[2], p[2]);
+        a.v[3] = fmax(a.v[3], p[3]); a.v[4] = fmin(a.v[4], p[4]); a.v[5] += p[5]; a.v[6] += p[6];
+    }
+    const int ops[7] = {0, 0, 0, 0, 1, 2, 2};
+    block_reduce<7>(a, ops, V.scal);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// S6: Sigma, q, t (rows) then Sigma_x and the right-hand side b of Eq. 17 (variables)
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(NT) sigma_rows_kernel(DevModel M, IpmVectors V, double mu) {
+    const int64_t r = blockIdx.x * (int64_t)NT + threadIdx.x;
+    if (r >= M.m) return;
+    const double sp = V.sp[r], sm = V.sm[r];
+    const double qp = V.wp[r] / sp, qm = V.wm[r] / sm;
+    V.q[r] = qp + qm;
+    V.t[r] = qp * V.r_pp[r] + mu / sp - qm * V.r_pm[r] - mu / sm;
+}
+
+__global__ void __launch_bounds__(NT) sigma_vars_kernel(DevModel M, IpmVectors V, double mu) {
+    const int64_t i = blockIdx.x * (int64_t)NT + threadIdx.x;
+    if (i >= M.n) return;
+    double jt = 0.0;
+    for (int64_t p = M.jt_ptr[i]; p < M.jt_ptr[i + 1]; ++p) jt += V.Jval[M.jt_idx[p]] * V.t[M.jt_row[p]];
+    const double lb = M.lb[i], ub = M.ub[i], y = V.y[i];
+    const bool hasL = lb > -INF, hasU = ub < INF;
+    const double dL = hasL ? y - lb : 1.0, dU = hasU ? ub - y : 1.0;
+    V.sigx[i] = (hasL ? V.zL[i] / dL : 0.0) + (hasU ? V.zU[i] / dU : 0.0);
+    V.b[i] = -(V.gradf[i] - (hasL ? mu / dL : 0.0) + (hasU ? mu / dU : 0.0) + jt);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// S8 + S9: eliminated directions (Eq. 10/14) and fraction-to-the-boundary step lengths
+//   partial[b][0..1] = min primal step, min dual step
+// ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double max_step(double v, double dv, double tau) { return dv < 0.0 ? fmin(1.0, -tau * v / dv) : 1.0; }
+
+__global__ void __launch_bounds__(NT) step_kernel(DevModel M, IpmVectors V, double mu, double tau) {
+    Red<2> a; a.v[0] = 1.0; a.v[1] = 1.0;
+    const int64_t total = M.n + M.m;
+    for (int64_t idx = blockIdx.x * (int64_t)NT + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * NT) {
+        if (idx < M.n) {
+            const int64_t i = idx;
+            const double lb = M.lb[i], ub = M.ub[i], y = V.y[i], dy = V.dy[i];
+            const bool hasL = lb > -INF, hasU = ub < INF;
+            double dzL = 0.0, dzU = 0.0;
+            if (hasL) {
+                const double dL = y - lb, zL = V.zL[i];
+                dzL = -(zL - mu / dL) - zL / dL * dy;
+                a.v[0] = fmin(a.v[0], max_step(dL, dy, tau)); a.v[1] = fmin(a.v[1], max_step(zL, dzL, tau));
+            }
+            if (hasU) {
+                const double dU = ub - y, zU = V.zU[i];
+                dzU = -(zU - mu / dU) + zU / dU * dy;
+                a.v[0] = fmin(a.v[0], max_step(dU, -dy, tau)); a.v[1] = fmin(a.v[1], max_step(zU, dzU, tau));
+            }
+            V.dzL[i] = dzL; V.dzU[i] = dzU;
+        } else {
+            const int64_t r = idx - M.n;
+            double jdy = 0.0;
+            for (int64_t p = M.J_ptr[r]; p < M.J_ptr[r + 1]; ++p) jdy += V.Jval[p] * V.dy[M.J_idx[p]];
+            const double sp = V.sp[r], sm = V.sm[r], wp = V.wp[r], wm = V.wm[r];
+            const double dsp = -V.r_pp[r] - jdy, dsm = -V.r_pm[r] + jdy;
+            const double dwp = -(wp - mu / sp) - wp / sp * dsp, dwm = -(wm - mu / sm) - wm / sm * dsm;
+            V.dsp[r] = dsp; V.dsm[r] = dsm; V.dwp[r] = dwp; V.dwm[r] = dwm;
+            a.v[0] = fmin(a.v[0], fmin(max_step(sp, dsp, tau), max_step(sm, dsm, tau)));
+            a.v[1] = fmin(a.v[1], fmin(max_step(wp, dwp, tau), max_step(wm, dwm, tau)));
+        }
+    }
+    const int ops[2] = {1, 1};
+    block_reduce<2>(a, ops, V.partial + (int64_t)blockIdx.x * 8);
+}
+
+__global__ void __launch_bounds__(NT) finalize_step_kernel(IpmVectors V, int nblocks) {
+    Red<2> a; a.v[0] = 1.0; a.v[1] = 1.0;
+    for (int b = threadIdx.x; b < nblocks; b += NT) { a.v[0] = fmin(a.v[0], V.partial[(int64_t)b * 8]); a.v[1] = fmin(a.v[1], V.partial[(int64_t)b * 8 + 1]); }
+    const int ops[2] = {1, 1};
+    block_reduce<2>(a, ops, V.scal + 7);
+}
+
+// S10: Eq. (26) with the step lengths read from device memory
+__global__ void __launch_bounds__(NT) update_kernel(DevModel M, IpmVectors V) {
+    const double apr = V.scal[7], adu = V.scal[8];
+    const int64_t idx = blockIdx.x * (int64_t)NT + threadIdx.x;
+    if (idx < M.n) {
+        V.y[idx] += apr * V.dy[idx]; V.zL[idx] += adu * V.dzL[idx]; V.zU[idx] += adu * V.dzU[idx];
+    } else if (idx < M.n + M.m) {
+        const int64_t r = idx - M.n;
+        V.sp[r] += apr * V.dsp[r]; V.sm[r] += apr * V.dsm[r]; V.wp[r] += adu * V.dwp[r]; V.wm[r] += adu * V.dwm[r];
+    }
+}
+
+__global__ void __launch_bounds__(NT) objective_kernel(DevModel M, IpmVectors V) {
+    Red<1> a; a.v[0] = 0.0;
+    const int nv = M.desc.nv, nx = M.desc.nx;
+    for (int64_t i = blockIdx.x * (int64_t)NT + threadIdx.x; i < M.n; i += (int64_t)gridDim.x * NT) {
+        const int k = (int)(i / nv), e = (int)(i - (int64_t)k * nv);
+        const double* x = V.y + (int64_t)k * nv;
+        a.v[0] += cost_value_entry(M.desc, e, x, x + nx, M.ref + (int64_t)k * M.desc.nr);
+    }
+    const int ops[1] = {2};
+    block_reduce<1>(a, ops, V.partial + (int64_t)blockIdx.x * 8);
+}
+__global__ void __launch_bounds__(NT) finalize_objective_kernel(IpmVectors V, int nblocks) {
+    Red<1> a; a.v[0] = 0.0;
+    for (int b = threadIdx.x; b < nblocks; b += NT) a.v[0] += V.partial[(int64_t)b * 8];
+    const int ops[1] = {2};
+    block_reduce<1>(a, ops, V.scal + 9);
+}
+
+inline unsigned blocks_for(int64_t work) { return (unsigned)((work + NT - 1) / NT); }
+inline int red_blocks(int64_t work) { return (int)std::min<int64_t>(RED_BLOCKS, (work + NT - 1) / NT); }
+
+}  // namespace
+
+void launch_model_eval(const DevModel& M, const double* y, const double* wp, const double* wm, const double* lam,
+                       double* c, double* gradf, double* Jval, double* Wval, cudaStream_t st) {
+    const int64_t work = M.m + M.n + (int64_t)M.desc.N * hess_count(M.desc);
+    model_eval_kernel<<<blocks_for(work), NT, 0, st>>>(M, y, wp, wm, lam, c, gradf, Jval, Wval);
+}
+void launch_assemble_K(const DevModel& M, const double* Jval, const double* Wval, const double* sigx, const double* q,
+                       double eta, double* Kval, cudaStream_t st) {
+    assemble_K_kernel<<<blocks_for(M.nnzK), NT, 0, st>>>(M, Jval, Wval, sigx, q, eta, Kval);
+}
+void launch_kkt_multiply(int64_t n, const int64_t* ptr, const int32_t* idx, const int32_t* src, const double* Kval, double eta,
+                         const double* x, double* y, cudaStream_t st) {
+    kkt_multiply_kernel<<<blocks_for(n), NT, 0, st>>>(n, ptr, idx, src, Kval, eta, x, y);
+}
+void launch_cold_init_y(const DevModel& M, const IpmVectors& V, const double* u_init, int use_y0, double kappa_push, double mu0, cudaStream_t st) {
+    cold_y_kernel<<<blocks_for(M.n), NT, 0, st>>>(M, V, u_init, use_y0, kappa_push, mu0);
+}
+void launch_cold_init_s(const DevModel& M, const IpmVectors& V, double gamma, double s_floor, double mu0, cudaStream_t st) {
+    cold_s_kernel<<<blocks_for(M.m), NT, 0, st>>>(M, V, gamma, s_floor, mu0);
+}
+void launch_warm_push(const DevModel& M, const IpmVectors& V, double warm_push, cudaStream_t st) {
+    warm_push_kernel<<<blocks_for(M.n), NT, 0, st>>>(M, V, warm_push);
+}
+void launch_residuals(const DevModel& M, const IpmVectors& V, double gamma, cudaStream_t st) {
+    const int nb = red_blocks(M.n + M.m);
+    residual_kernel<<<nb, NT, 0, st>>>(M, V, gamma);
+    finalize_residual_kernel<<<1, NT, 0, st>>>(V, nb);
+}
+void launch_sigma_rhs(const DevModel& M, const IpmVectors& V, double mu, cudaStream_t st) {
+    sigma_rows_kernel<<<blocks_for(M.m), NT, 0, st>>>(M, V, mu);
+    sigma_vars_kernel<<<blocks_for(M.n), NT, 0, st>>>(M, V, mu);
+}
+void launch_step(const DevModel& M, const IpmVectors& V, double mu, double tau, cudaStream_t st) {
+    const int nb = red_blocks(M.n + M.m);
+    step_kernel<<<nb, NT, 0, st>>>(M, V, mu, tau);
+    finalize_step_kernel<<<1, NT, 0, st>>>(V, nb);
+}
+void launch_update(const DevModel& M, const IpmVectors& V, cudaStream_t st) {
+    update_kernel<<<blocks_for(M.n + M.m), NT, 0, st>>>(M, V);
+}
+void launch_objective(const DevModel& M, const IpmVectors& V, cudaStream_t st) {
+    const int nb = red_blocks(M.n);
+    objective_kernel<<<nb, NT, 0, st>>>(M, V);
+    finalize_objective_kernel<<<1, NT, 0, st>>>(V, nb);
+}
+
+}  // namespace nmpc
