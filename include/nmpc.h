@@ -134,7 +134,8 @@ nmpc_status nmpc_symbolic_kmap(nmpc_symbolic sym, int32_t* super_of_entry /*nnz*
 void        nmpc_symbolic_destroy(nmpc_symbolic sym);
 
 /* ---- Alg. 2 lines 10-12: analysis once per structure; uploads all integer maps; allocates L.  cuda_stream is a
- *      cudaStream_t (NULL = default stream).                                                                 */
+ *      cudaStream_t.  NULL = the library creates its own blocking stream (ordered with the legacy default stream,
+ *      which itself cannot carry the CUDA-graph capture of the factor / solve launch sequences).               */
 nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const nmpc_options* opt,
                          void* cuda_stream, nmpc_handle* out);
 
@@ -166,6 +167,11 @@ nmpc_status nmpc_ipm_solve_host(nmpc_handle h, int32_t warm, const double* x0_ho
 /* ---- current primal-dual iterate z (DEVICE outputs; any pointer may be NULL): s+,s-,w+,w- length m; zL,zU n */
 nmpc_status nmpc_get_iterate(nmpc_handle h, double* y_dev, double* sp_dev, double* sm_dev, double* wp_dev,
                              double* wm_dev, double* zL_dev, double* zU_dev);
+/* ---- overwrite the stored iterate (the paper's warmstart_backend_start_values; Alg. 1 line 10): DEVICE
+ *      inputs, all seven required, strictly interior (s, w > 0; z > 0 where the bound is finite).  The next
+ *      nmpc_ipm_solve(warm = 1) starts from it.  Async.                                                      */
+nmpc_status nmpc_set_iterate(nmpc_handle h, const double* y_dev, const double* sp_dev, const double* sm_dev,
+                             const double* wp_dev, const double* wm_dev, const double* zL_dev, const double* zU_dev);
 /* ---- model evaluation at (y, lam) with the current parameters (DEVICE outputs, any may be NULL):
  *      c[m], gradf[n], Jval[nnzJ], Wval[nnzW]; and the assembled K values (pattern order) for given Sigma_x[n],
  *      q[m], eta.  Used by the parity tests of steps a2/a3.                                                  */
@@ -178,6 +184,11 @@ nmpc_status nmpc_assemble(nmpc_handle h, const double* Jval_dev, const double* W
 nmpc_status nmpc_get_jac_pattern(nmpc_handle h, int64_t* nnz, int64_t* rowptr, int32_t* colind);
 nmpc_status nmpc_get_hess_pattern(nmpc_handle h, int64_t* nnz, int64_t* rowptr, int32_t* colind);
 nmpc_status nmpc_get_kkt_pattern(nmpc_handle h, int64_t* nnz, int64_t* rowptr, int32_t* colind);
+
+/* ---- measurement aid (not on the hot path): sustained fp64 rate of the current device in TFLOP/s, kind 0 = DFMA
+ *      (vector pipe), 1 = DMMA (mma.sync m8n8k4 f64); best of `repeats` launches of a register-resident kernel.
+ *      HOST outputs; ms_out may be NULL.  These are the denominators of the factorization roofline.            */
+nmpc_status nmpc_fp64_peak(int32_t kind, int32_t repeats, double* tflops_out, double* ms_out);
 
 nmpc_status nmpc_get_info(nmpc_handle h, nmpc_sym_info* out_host);
 /* ---- copy of the factor for tests: panels (column-major r x w per supernode) to a HOST buffer             */

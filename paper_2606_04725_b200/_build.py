@@ -26,6 +26,7 @@ SOURCES = [
     ("factor.cu", []),
     ("ipm.cu", ["-fmad=false"]),
     ("api.cu", []),
+    ("peak.cu", []),
 ]
 HEADERS = ["device.h", "symbolic.h", "models.cuh", os.path.join(ROOT, "include", "nmpc.h")]
 

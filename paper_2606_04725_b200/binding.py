@@ -79,11 +79,13 @@ SIGNATURES = {
     "nmpc_ipm_solve": (c_i32, [c_vp, c_i32, c_i32, c_vp, P(nmpc_stats), c_vp, c_i32]),
     "nmpc_ipm_solve_host": (c_i32, [c_vp, c_i32, c_vp, c_vp, c_vp, P(nmpc_stats)]),
     "nmpc_get_iterate": (c_i32, [c_vp] * 8),
+    "nmpc_set_iterate": (c_i32, [c_vp] * 8),
     "nmpc_model_eval": (c_i32, [c_vp] * 7),
     "nmpc_assemble": (c_i32, [c_vp, c_vp, c_vp, c_vp, c_vp, c_dbl, c_vp]),
     "nmpc_get_jac_pattern": (c_i32, [c_vp, P(c_i64), c_vp, c_vp]),
     "nmpc_get_hess_pattern": (c_i32, [c_vp, P(c_i64), c_vp, c_vp]),
     "nmpc_get_kkt_pattern": (c_i32, [c_vp, P(c_i64), c_vp, c_vp]),
+    "nmpc_fp64_peak": (c_i32, [c_i32, c_i32, P(c_dbl), P(c_dbl)]),
     "nmpc_get_info": (c_i32, [c_vp, P(nmpc_sym_info)]),
     "nmpc_get_factor": (c_i32, [c_vp, c_vp]),
     "nmpc_launch_count": (c_i64, [c_vp]),
@@ -174,6 +176,15 @@ def _get_pattern(fn, h):
     if st:
         raise NmpcError(st, fn.__name__)
     return nnz.value
+
+
+def fp64_peak(kind: int, repeats: int = 5):
+    """nmpc_fp64_peak: (TFLOP/s, ms) of the DFMA (kind 0) / DMMA (kind 1) microbenchmark on the current device."""
+    tf, ms = c_dbl(), c_dbl()
+    st = load_library().nmpc_fp64_peak(kind, repeats, C.byref(tf), C.byref(ms))
+    if st:
+        raise NmpcError(st, "nmpc_fp64_peak")
+    return tf.value, ms.value
 
 
 class Symbolic:
@@ -282,6 +293,9 @@ class Handle:
 
     def get_iterate(self, y=None, sp=None, sm=None, wp=None, wm=None, zL=None, zU=None):
         self._ck(self.lib.nmpc_get_iterate(self._h, *[_ptr(a) for a in (y, sp, sm, wp, wm, zL, zU)]), "nmpc_get_iterate")
+
+    def set_iterate(self, y, sp, sm, wp, wm, zL, zU):
+        self._ck(self.lib.nmpc_set_iterate(self._h, *[_ptr(a) for a in (y, sp, sm, wp, wm, zL, zU)]), "nmpc_set_iterate")
 
     def model_eval(self, y, lam=None, c=None, gradf=None, Jval=None, Wval=None):
         self._ck(self.lib.nmpc_model_eval(self._h, _ptr(y), _ptr(lam), _ptr(c), _ptr(gradf), _ptr(Jval), _ptr(Wval)),

@@ -36,6 +36,7 @@ struct nmpc_handle_s {
     Symbolic S;
     nmpc_options opt;
     cudaStream_t stream = nullptr;
+    bool own_stream = false;
     DevSym D;
     DevModel M;
     IpmVectors V{};
@@ -250,6 +251,12 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
     if (opt) h->opt = *opt; else default_options(&h->opt);
     if (h->opt.mu_warm <= 0.0) h->opt.mu_warm = h->opt.eps_outer / 10.0;
     h->stream = (cudaStream_t)cuda_stream;
+    if (!h->stream) {
+        // the legacy default stream cannot be captured into a graph: use an own BLOCKING stream, which keeps the implicit
+        // ordering with work the caller issues on the legacy default stream (e.g. torch's default stream)
+        if (cudaStreamCreate(&h->stream) != cudaSuccess) { h->err = "cudaStreamCreate failed"; cudaGetLastError(); return fail(NMPC_E_CUDA); }
+        h->own_stream = true;
+    }
     nmpc_status st;
     try { st = analyze_symbolic(pattern, ocp, &h->opt, h->S); }
     catch (const std::bad_alloc&) { st = NMPC_E_ALLOC; h->err = "host allocation failed"; }
@@ -357,6 +364,7 @@ void nmpc_destroy(nmpc_handle h) {
     if (h->h_pinned) cudaFreeHost(h->h_pinned);
     if (h->ev[0]) cudaEventDestroy(h->ev[0]);
     if (h->ev[1]) cudaEventDestroy(h->ev[1]);
+    if (h->own_stream) cudaStreamDestroy(h->stream);
     delete h;
 }
 
@@ -440,6 +448,22 @@ nmpc_status nmpc_get_iterate(nmpc_handle h, double* y, double* sp, double* sm, d
     if (wm) CK(cudaMemcpyAsync(wm, V.wm, m, cudaMemcpyDeviceToDevice, h->stream));
     if (zL) CK(cudaMemcpyAsync(zL, V.zL, n, cudaMemcpyDeviceToDevice, h->stream));
     if (zU) CK(cudaMemcpyAsync(zU, V.zU, n, cudaMemcpyDeviceToDevice, h->stream));
+    return NMPC_OK;
+}
+
+nmpc_status nmpc_set_iterate(nmpc_handle h, const double* y, const double* sp, const double* sm, const double* wp, const double* wm, const double* zL, const double* zU) {
+    if (!h || !y || !sp || !sm || !wp || !wm || !zL || !zU) return NMPC_E_ARG;
+    if (!h->has_model) return NMPC_E_STATE;
+    const size_t n = h->M.n * sizeof(double), m = h->M.m * sizeof(double);
+    const IpmVectors& V = h->V;
+    CK(cudaMemcpyAsync(V.y, y, n, cudaMemcpyDeviceToDevice, h->stream));
+    CK(cudaMemcpyAsync(V.sp, sp, m, cudaMemcpyDeviceToDevice, h->stream));
+    CK(cudaMemcpyAsync(V.sm, sm, m, cudaMemcpyDeviceToDevice, h->stream));
+    CK(cudaMemcpyAsync(V.wp, wp, m, cudaMemcpyDeviceToDevice, h->stream));
+    CK(cudaMemcpyAsync(V.wm, wm, m, cudaMemcpyDeviceToDevice, h->stream));
+    CK(cudaMemcpyAsync(V.zL, zL, n, cudaMemcpyDeviceToDevice, h->stream));
+    CK(cudaMemcpyAsync(V.zU, zU, n, cudaMemcpyDeviceToDevice, h->stream));
+    h->have_state = true;
     return NMPC_OK;
 }
 

@@ -1,0 +1,90 @@
+// peak.cu -- measured fp64 roofline denominators.  MEASURED_PEAKS.json holds only the HBM copy bandwidth and the bf16
+// GEMM rate; the numeric factorization (step a4) is fp64, so bench.py measures the chip's sustained DFMA (vector pipe)
+// and DMMA (mma.sync m8n8k4 f64 tensor path) rates with these two register-resident kernels and reports the factor
+// kernels against them.  Not on the hot path.
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "../../include/nmpc.h"
+
+namespace {
+
+constexpr int PEAK_NT = 256;
+constexpr int PEAK_ILP = 8;
+constexpr int PEAK_INNER = 512;
+
+__global__ void __launch_bounds__(PEAK_NT) dfma_peak_kernel(double* out, int iters, double a0) {
+    double acc[PEAK_ILP];
+#pragma unroll
+    for (int k = 0; k < PEAK_ILP; ++k) acc[k] = threadIdx.x * 1e-3 + k;
+    const double a = a0, b = 1e-9;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll 8
+        for (int j = 0; j < PEAK_INNER; ++j) {
+#pragma unroll
+            for (int k = 0; k < PEAK_ILP; ++k) acc[k] = fma(acc[k], a, b);
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < PEAK_ILP; ++k) s += acc[k];
+    if (s == 123.456) out[blockIdx.x * PEAK_NT + threadIdx.x] = s;      // keeps the loop alive, never true in practice
+}
+
+__global__ void __launch_bounds__(PEAK_NT) dmma_peak_kernel(double* out, int iters, double a0) {
+    double c[PEAK_ILP][2];
+#pragma unroll
+    for (int k = 0; k < PEAK_ILP; ++k) { c[k][0] = threadIdx.x * 1e-3 + k; c[k][1] = 0.5 * k; }
+    const double a = a0, b = 1e-9 * (threadIdx.x & 3);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll 4
+        for (int j = 0; j < PEAK_INNER; ++j) {
+#pragma unroll
+            for (int k = 0; k < PEAK_ILP; ++k)
+                asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                             : "+d"(c[k][0]), "+d"(c[k][1]) : "d"(a), "d"(b));
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < PEAK_ILP; ++k) s += c[k][0] + c[k][1];
+    if (s == 123.456) out[blockIdx.x * PEAK_NT + threadIdx.x] = s;
+}
+
+}  // namespace
+
+extern "C" nmpc_status nmpc_fp64_peak(int32_t kind, int32_t repeats, double* tflops_out, double* ms_out) {
+    if (!tflops_out || kind < 0 || kind > 1 || repeats < 1) return NMPC_E_ARG;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return NMPC_E_CUDA;
+    }
+    const int blocks = sms * 8, iters = 24;
+    double* out = nullptr;
+    if (cudaMalloc((void**)&out, sizeof(double) * (size_t)blocks * PEAK_NT) != cudaSuccess) { cudaGetLastError(); return NMPC_E_ALLOC; }
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    double best_ms = 1e300;
+    for (int r = 0; r < repeats + 1; ++r) {                    // first pass is the warm-up
+        cudaEventRecord(e0);
+        if (kind == 0) dfma_peak_kernel<<<blocks, PEAK_NT>>>(out, iters, 0.999999);
+        else dmma_peak_kernel<<<blocks, PEAK_NT>>>(out, iters, 0.999999);
+        cudaEventRecord(e1);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (r > 0 && ms < best_ms) best_ms = ms;
+    }
+    cudaError_t err = cudaGetLastError();
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(out);
+    if (err != cudaSuccess) return NMPC_E_CUDA;
+    // flops per thread: DFMA 2 per fma;  DMMA m8n8k4 = 2*8*8*4 = 512 per warp instruction = 16 per thread
+    const double per_thread = (kind == 0 ? 2.0 : 16.0) * PEAK_ILP * (double)PEAK_INNER * iters;
+    const double flops = per_thread * (double)blocks * PEAK_NT;
+    *tflops_out = flops / (best_ms * 1e-3) / 1e12;
+    if (ms_out) *ms_out = best_ms;
+    return NMPC_OK;
+}

@@ -1,0 +1,321 @@
+"""Parity of the CUDA path (through the C-ABI of include/nmpc.h) against the CPU oracle, element by element on the
+same seeded inputs.  Tolerances are north_star's: factor backward error <= 1e-12 (reading G17), normwise solve
+residual <= 1e-10 (reading G16), converged primal solution <= 1e-6 relative, IPM iteration counts equal.
+
+Steps covered: a1 parameter update, a2 model/derivative evaluation, a3 condensed assembly,
+a4 numeric supernodal Cholesky (+ pivot failure, a4' inertia retry), a5 triangular solves, a6/a7 IPM vector kernels
+and the barrier loop (via nmpc_ipm_solve), Algorithm 1 re-solves.
+"""
+import numpy as np
+import pytest
+import scipy.sparse as sp
+import torch
+
+import paper_2606_04725_b200 as nb
+from ocp_inputs import make_config, sigma_sweep_draws
+from oracle.ipm import LiftedIPM, nmpc_closed_loop
+from oracle.linalg import SparseCholesky
+from oracle.nlp import TranscribedOCP
+from paper_2606_04725_b200 import binding
+
+from gpu_util import factor_as_sparse, factor_backward_error, normwise_backward_error, values_on_pattern
+
+pytestmark = pytest.mark.gpu
+
+DEV = "cuda:0"
+ORDERINGS = [binding.ORDER_NATURAL, binding.ORDER_AMD, binding.ORDER_ND, binding.ORDER_TIME_ND]
+# sizes the oracle finishes in seconds that still span several tiles and a ragged tail:
+#   C1m: fronts ~40-80 rows (shared-memory kernel, several supernodes per level)
+#   C2m: g=9 -> fronts of a few hundred rows -> tiled big-front path with ragged 64-blocks
+MID = [("C0", {}), ("C1", dict(trays=18, N=30)), ("C2", dict(g=9, N=7)), ("C3", dict(g=8, nseg=2, N=5)),
+       ("C4", dict(trays=40, N=25))]
+
+
+def dev(a):
+    return torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64).to(DEV)
+
+
+def kkt_from_oracle(cfg, iters=3):
+    """A genuine condensed lifted KKT matrix and right-hand side from a few oracle IPM iterations."""
+    ipm = LiftedIPM(cfg, linsolve="blocktri", max_iter=iters)
+    ipm.solve()
+    ls = ipm.last_step
+    K = ls["K0"] if ls["eta"] == 0.0 else (ls["K0"] + ls["eta"] * sp.identity(cfg.n)).tocsc()   # Eq. (13)/(17)
+    return K, ls["b"], ipm
+
+
+@pytest.mark.parametrize("name,ov", MID)
+@pytest.mark.parametrize("ordering", ORDERINGS)
+def test_factor_and_solve_vs_oracle(name, ov, ordering):
+    cfg = make_config(name, **ov)
+    K, b, _ = kkt_from_oracle(cfg)
+    h = nb.Handle(None, nb.make_ocp(cfg), nb.default_options(ordering=ordering))
+    info = h.get_info()
+    rp, ci = h.get_kkt_pattern(cfg.n)
+    vals = dev(values_on_pattern(K, rp, ci))
+    st, _ = h.factor(vals, 0.0)
+    assert st == 0
+    L = factor_as_sparse(info, h.get_factor())
+    assert factor_backward_error(L, K, info["perm"]) <= 1e-12
+    x = dev(b)
+    h.solve(x)
+    xg = x.cpu().numpy()
+    assert normwise_backward_error(K, xg, b) <= 1e-10
+    xo = SparseCholesky(K, None).factor(K).solve(b)
+    # forward error: two backward-stable solves differ by at most ~cond(K) * eps (K unique, x unique)
+    cond = np.linalg.cond(K.toarray())
+    assert np.abs(xg - xo).max() <= max(1e-10, 50.0 * cond * np.finfo(float).eps) * np.abs(xo).max()
+    # nmpc_kkt_multiply reproduces K x
+    yv = torch.empty_like(x)
+    h.kkt_multiply(x, yv)
+    assert np.abs(yv.cpu().numpy() - K @ xg).max() <= 1e-12 * abs(K).sum(axis=1).max() * np.abs(xg).max()
+    h.close()
+
+
+@pytest.mark.parametrize("smem_front_max", [16, 48, 0])
+def test_factor_kernel_families_agree(smem_front_max):
+    """The shared-memory and the tiled front kernels must give the same factor (to rounding) on the same matrix."""
+    cfg = make_config("C2", g=9, N=7)
+    K, b, _ = kkt_from_oracle(cfg)
+    h = nb.Handle(None, nb.make_ocp(cfg), nb.default_options(smem_front_max=smem_front_max))
+    info = h.get_info()
+    rp, ci = h.get_kkt_pattern(cfg.n)
+    h.factor(dev(values_on_pattern(K, rp, ci)), 0.0)
+    L = factor_as_sparse(info, h.get_factor())
+    assert factor_backward_error(L, K, info["perm"]) <= 1e-12
+    x = dev(b)
+    h.solve(x)
+    assert normwise_backward_error(K, x.cpu().numpy(), b) <= 1e-10
+    h.close()
+
+
+def test_bare_pattern_handle_multiple_rhs_and_state_errors():
+    """nmpc_analyze(pattern) without a model: random SPD matrix on a random sparse pattern, nrhs = 3."""
+    rng = np.random.default_rng(5)
+    n = 700
+    A = sp.random(n, n, density=0.004, random_state=7, format="csr")
+    A = A + A.T + sp.identity(n)
+    A.data[:] = rng.uniform(-1.0, 1.0, len(A.data))
+    A = (A + A.T) * 0.5
+    K = (A + sp.diags(np.asarray(abs(A).sum(axis=1)).ravel() + 0.1)).tocsr()
+    Kl = sp.tril(K, format="csr")
+    Kl.sort_indices()
+    pat = nb.make_pattern(n, Kl.indptr, Kl.indices)
+    h = nb.Handle(pat, None, None)
+    B = rng.normal(size=(3, n))
+    X = dev(B)
+    with pytest.raises(nb.NmpcError) as ei:
+        h.solve(X, 3)
+    assert ei.value.status == binding.NMPC_E_STATE
+    h.factor(dev(Kl.data), 0.0)
+    h.solve(X, 3)
+    Xg = X.cpu().numpy()
+    for k in range(3):
+        assert normwise_backward_error(K, Xg[k], B[k]) <= 1e-10
+    with pytest.raises(nb.NmpcError) as ei:
+        h.ipm_solve(0)
+    assert ei.value.status == binding.NMPC_E_STATE
+    h.close()
+
+
+def test_pivot_failure_and_eta_shift():
+    cfg = make_config("C1", trays=6, N=8)
+    K, b, _ = kkt_from_oracle(cfg)
+    K = sp.lil_matrix(K)
+    bad = 17
+    K[bad, bad] = -5.0                                      # indefinite: some pivot must fail
+    K = sp.csr_matrix(K)
+    for ordering in ORDERINGS:
+        h = nb.Handle(None, nb.make_ocp(cfg), nb.default_options(ordering=ordering))
+        rp, ci = h.get_kkt_pattern(cfg.n)
+        vals = dev(values_on_pattern(K, rp, ci))
+        st, col = h.factor(vals, 0.0, check=False)
+        assert st == binding.NMPC_E_NOT_SPD and 0 <= col < cfg.n
+        # oracle on the same permutation fails at the same (original) column
+        perm = h.get_info()["perm"]
+        from oracle.linalg import NotPositiveDefinite
+        with pytest.raises(NotPositiveDefinite) as ei:
+            SparseCholesky(K, perm).factor(K)
+        assert ei.value.column == col
+        # Eq. (13): a large enough eta_y restores positive definiteness; the factor is that of K + eta I
+        eta = 1e3
+        st, _ = h.factor(vals, eta)
+        assert st == 0
+        Ke = (K + eta * sp.identity(cfg.n)).tocsr()
+        L = factor_as_sparse(h.get_info(), h.get_factor())
+        assert factor_backward_error(L, Ke, perm) <= 1e-12
+        x = dev(b)
+        h.solve(x)
+        assert normwise_backward_error(Ke, x.cpu().numpy(), b) <= 1e-10
+        h.close()
+
+
+@pytest.mark.parametrize("name,ov", MID)
+def test_model_eval_and_assembly_vs_oracle(name, ov):
+    cfg = make_config(name, **ov)
+    nlp = TranscribedOCP(cfg)
+    rng = np.random.default_rng(11)
+    lo = np.where(np.isfinite(nlp.lb), nlp.lb, 280.0)
+    hi = np.where(np.isfinite(nlp.ub), nlp.ub, 450.0)
+    y = lo + (hi - lo) * rng.uniform(0.1, 0.9, cfg.n)
+    lam = rng.normal(size=cfg.m)
+    x0 = np.clip(cfg.x0 + 0.01 * rng.normal(size=cfg.nx), *cfg.x0_clip)
+    ref = cfg.ref_for_solve(1)
+    nlp.set_params(x0, ref)
+    h = nb.Handle(None, nb.make_ocp(cfg), None)
+    h.update_params(dev(x0), dev(ref))                                         # a1
+    jrp, jci = h.get_jac_pattern(cfg.m)
+    wrp, wci = h.get_hess_pattern(cfg.n)
+    krp, kci = h.get_kkt_pattern(cfg.n)
+    c, g = torch.empty(cfg.m, dtype=torch.float64, device=DEV), torch.empty(cfg.n, dtype=torch.float64, device=DEV)
+    Jv = torch.empty(int(jrp[-1]), dtype=torch.float64, device=DEV)
+    Wv = torch.empty(int(wrp[-1]), dtype=torch.float64, device=DEV)
+    h.model_eval(dev(y), dev(lam), c, g, Jv, Wv)                               # a2
+    assert np.abs(c.cpu().numpy() - nlp.constraints(y)).max() <= 1e-12 * max(1.0, np.abs(nlp.constraints(y)).max())
+    assert np.abs(g.cpu().numpy() - nlp.gradient(y)).max() <= 1e-13 * max(1.0, np.abs(nlp.gradient(y)).max())
+    Jg = sp.csr_matrix((Jv.cpu().numpy(), jci, jrp), shape=(cfg.m, cfg.n))
+    Jo = nlp.jacobian(y)
+    assert abs(Jg - Jo).max() <= 1e-13 * abs(Jo).max()
+    Wl = sp.csr_matrix((Wv.cpu().numpy(), wci, wrp), shape=(cfg.n, cfg.n))
+    Wg = Wl + sp.tril(Wl, -1).T
+    Wo = nlp.hessian(y, lam)
+    assert abs(Wg - Wo).max() <= 1e-12 * max(1e-300, abs(Wo).max())
+    # a3: K = W + Sigma_x + J^T Q J + eta I on the fixed pattern
+    sigx = 10.0 ** rng.uniform(-6, 6, cfg.n)
+    q = 10.0 ** rng.uniform(-6, 6, cfg.m)
+    eta = 0.37
+    Kv = torch.empty(int(krp[-1]), dtype=torch.float64, device=DEV)
+    h.assemble(Jv, Wv, dev(sigx), dev(q), eta, Kv)
+    Ko = (Wo + sp.diags(sigx + eta) + Jo.T @ sp.diags(q) @ Jo).tocsr()
+    Kg = Kv.cpu().numpy()
+    Ko_vals = values_on_pattern(Ko, krp, kci)
+    # entrywise relative to the magnitude of the terms summed into the entry
+    scale = values_on_pattern(abs(Wo) + sp.diags(sigx + eta) + abs(Jo).T @ sp.diags(q) @ abs(Jo), krp, kci)
+    assert np.all(np.abs(Kg - Ko_vals) <= 1e-13 * scale)
+    assert sp.tril(Ko).nnz <= len(Kg)
+    h.close()
+
+
+def _gpu_ipm(cfg, ordering=binding.ORDER_AUTO, **opts):
+    h = nb.Handle(None, nb.make_ocp(cfg), nb.default_options(ordering=ordering, **opts))
+    return h
+
+
+@pytest.mark.parametrize("name,ov", MID + [("C1", {})])
+def test_ipm_solve_vs_oracle(name, ov):
+    cfg = make_config(name, **ov)
+    ref = LiftedIPM(cfg, linsolve="blocktri")
+    ro = ref.solve()
+    assert ro["status"] == "converged"
+    h = _gpu_ipm(cfg)
+    h.update_params(dev(cfg.x0), dev(cfg.ref_for_solve(0)))
+    y = torch.zeros(cfg.n, dtype=torch.float64, device=DEV)
+    rg = h.ipm_solve(0, y, trace_cap=256)
+    assert rg["status"] == 0
+    assert rg["iters"] == ro["iters"], (rg["iters"], ro["iters"], rg["trace"], ro["trace"])
+    yo = ro["state"].y
+    assert np.abs(y.cpu().numpy() - yo).max() <= 1e-6 * np.abs(yo).max()
+    for tg, to in zip(rg["trace"], ro["trace"]):
+        assert tg["mu"] == to["mu"] and tg["eta"] == to["eta"]
+        # step lengths are ratios of small quantities: they agree to the conditioning of K, not to rounding
+        assert abs(tg["alpha_pr"] - to["alpha_pr"]) <= 1e-3 and abs(tg["alpha_du"] - to["alpha_du"]) <= 1e-3
+    # full primal-dual iterate
+    m, n = cfg.m, cfg.n
+    bufs = [torch.empty(k, dtype=torch.float64, device=DEV) for k in (n, m, m, m, m, n, n)]
+    h.get_iterate(*bufs)
+    so = ro["state"]
+    for g_, o_ in zip(bufs, (so.y, so.sp, so.sm, so.wp, so.wm, so.zL, so.zU)):
+        assert np.abs(g_.cpu().numpy() - o_).max() <= 1e-5 * max(1.0, np.abs(o_).max())
+    assert rg["objective"] == pytest.approx(ref.nlp.objective(yo), rel=1e-6, abs=1e-9)
+    h.close()
+
+
+@pytest.mark.parametrize("ordering", ORDERINGS)
+def test_ipm_result_independent_of_ordering(ordering):
+    cfg = make_config("C1", trays=10, N=14)
+    ro = LiftedIPM(cfg, linsolve="sparse").solve()
+    h = _gpu_ipm(cfg, ordering)
+    h.update_params(dev(cfg.x0), dev(cfg.ref_for_solve(0)))
+    y = torch.zeros(cfg.n, dtype=torch.float64, device=DEV)
+    rg = h.ipm_solve(0, y)
+    assert rg["iters"] == ro["iters"]
+    assert np.abs(y.cpu().numpy() - ro["state"].y).max() <= 1e-6 * np.abs(ro["state"].y).max()
+    h.close()
+
+
+def test_ipm_inertia_correction_path_matches_oracle():
+    """Steps a4' / S7: a VdP solve started (nmpc_set_iterate) from a poor multiplier guess has an indefinite W, so
+    the first factorizations fail and eta_y is raised by the schedule of Eq. (13) -- same etas, same counts."""
+    cfg = make_config("C0")
+    ipm = LiftedIPM(cfg, linsolve="dense")
+    st, _ = ipm.cold_start(cfg.y_cold(cfg.x0))
+    st.wp[:] = 500.0                                         # lam = w+ - w- strongly positive -> W indefinite
+    ipm.state = st.copy()
+    ro = ipm.solve(warm=True)
+    assert ro["status"] == "converged" and any(t["eta"] > 0 for t in ro["trace"])
+    h = _gpu_ipm(cfg)
+    h.update_params(dev(cfg.x0), dev(cfg.ref_for_solve(0)))
+    h.set_iterate(*[dev(v) for v in (st.y, st.sp, st.sm, st.wp, st.wm, st.zL, st.zU)])
+    y = torch.zeros(cfg.n, dtype=torch.float64, device=DEV)
+    rg = h.ipm_solve(1, y, trace_cap=256)
+    assert rg["iters"] == ro["iters"] and rg["factorizations"] == ro["factorizations"]
+    assert rg["eta_retries"] == ro["factorizations"] - ro["iters"] > 0
+    assert [t["eta"] for t in rg["trace"]] == [t["eta"] for t in ro["trace"]]
+    assert np.abs(y.cpu().numpy() - ro["state"].y).max() <= 1e-6 * np.abs(ro["state"].y).max()
+    h.close()
+
+
+@pytest.mark.parametrize("name,ov,R", [("C0", {}, 20), ("C1", dict(trays=14, N=20), 6), ("C2", dict(g=6, N=5), 3)])
+def test_nmpc_resolves_replay_vs_oracle(name, ov, R):
+    """Algorithm 1 in replay mode: the GPU run is fed the oracle's recorded x0 / ref sequence;
+    every re-solve must take the same number of IPM iterations and reach the same primal solution.  The symbolic
+    analysis is done once (nmpc_analyze) and reused by every re-solve."""
+    cfg = make_config(name, **ov)
+    out, _ = nmpc_closed_loop(cfg, n_resolves=R, linsolve="blocktri")
+    h = _gpu_ipm(cfg)
+    y = torch.zeros(cfg.n, dtype=torch.float64, device=DEV)
+    yh = np.empty(cfg.n)
+    for j, o in enumerate(out):
+        if j % 2 == 0:
+            h.update_params(dev(o["x0"]), dev(o["ref"]))
+            rg = h.ipm_solve(int(j > 0), y)
+            yg = y.cpu().numpy()
+        else:                                                # end-to-end entry with HOST buffers
+            rg = h.ipm_solve_host(int(j > 0), o["x0"], np.ascontiguousarray(o["ref"]), yh)
+            yg = yh.copy()
+        assert rg["status"] == 0
+        assert rg["iters"] == o["iters"], (j, rg["iters"], o["iters"])
+        assert np.abs(yg - o["y"]).max() <= 1e-6 * np.abs(o["y"]).max()
+    # invariant: re-solving the unchanged problem warm takes 0 iterations
+    rg = h.ipm_solve(1, y)
+    assert rg["iters"] == 0 and rg["status"] == 0
+    h.close()
+
+
+def test_bitwise_reproducible():
+    cfg = make_config("C2", g=8, N=6)
+    ys = []
+    for _ in range(2):
+        h = _gpu_ipm(cfg)
+        h.update_params(dev(cfg.x0), dev(cfg.ref_for_solve(0)))
+        y = torch.zeros(cfg.n, dtype=torch.float64, device=DEV)
+        h.ipm_solve(0, y)
+        ys.append(y.cpu().numpy().copy())
+        h.close()
+    assert np.array_equal(ys[0], ys[1])
+
+
+def test_graph_and_plain_launch_paths_agree():
+    cfg = make_config("C1", trays=12, N=16)
+    K, b, _ = kkt_from_oracle(cfg)
+    xs = []
+    for use_graph in (0, 1):
+        h = nb.Handle(None, nb.make_ocp(cfg), nb.default_options(use_graph=use_graph))
+        rp, ci = h.get_kkt_pattern(cfg.n)
+        h.factor(dev(values_on_pattern(K, rp, ci)), 0.0)
+        x = dev(b)
+        h.solve(x)
+        xs.append(x.cpu().numpy())
+        assert h.launch_count() > 0
+        h.close()
+    assert np.array_equal(xs[0], xs[1])
