@@ -129,7 +129,8 @@ nmpc_status nmpc_symbolic_analyze(const nmpc_pattern* pattern, const nmpc_ocp* o
 nmpc_status nmpc_symbolic_info(nmpc_symbolic sym, nmpc_sym_info* out);
 /* Pattern of K derived from the model (lower CSR).  Two-call protocol: with rowptr == NULL only *nnz is set. */
 nmpc_status nmpc_symbolic_pattern(nmpc_symbolic sym, int64_t* nnz, int64_t* rowptr /*n+1*/, int32_t* colind);
-/* scatter map: for K value index e (pattern order), supernode and offset inside its column-major panel.     */
+/* scatter map: for K value index e (pattern order), supernode and offset into the concatenated panels (layout as
+ * nmpc_get_factor: column-major, leading dimension r_s rounded up to even).                                 */
 nmpc_status nmpc_symbolic_kmap(nmpc_symbolic sym, int32_t* super_of_entry /*nnz*/, int64_t* panel_offset /*nnz*/);
 void        nmpc_symbolic_destroy(nmpc_symbolic sym);
 
@@ -191,7 +192,8 @@ nmpc_status nmpc_get_kkt_pattern(nmpc_handle h, int64_t* nnz, int64_t* rowptr, i
 nmpc_status nmpc_fp64_peak(int32_t kind, int32_t repeats, double* tflops_out, double* ms_out);
 
 nmpc_status nmpc_get_info(nmpc_handle h, nmpc_sym_info* out_host);
-/* ---- copy of the factor for tests: panels (column-major r x w per supernode) to a HOST buffer             */
+/* ---- copy of the factor for tests: the panels of all supernodes, one after the other, to a HOST buffer.  Panel of
+ *      supernode s: column-major r_s x w_s with leading dimension r_s rounded up to even (rows = nmpc_sym_info.rows). */
 nmpc_status nmpc_get_factor(nmpc_handle h, double* panels_host /* panel_doubles */);
 /* ---- kernel launches issued by this handle since creation (graph replays count their kernel nodes)        */
 int64_t     nmpc_launch_count(nmpc_handle h);

@@ -24,6 +24,7 @@ COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", os.path
 SOURCES = [
     ("symbolic.cpp", []),
     ("factor.cu", []),
+    ("solve.cu", []),
     ("ipm.cu", ["-fmad=false"]),
     ("api.cu", []),
     ("peak.cu", []),

@@ -22,11 +22,7 @@ extern "C" nmpc_status nmpc_copy_pattern_internal(const nmpc::Csr& P, int64_t* n
 
 namespace {
 
-struct StepPlan { int potrf_off, potrf_cnt, trsm_off, trsm_cnt, syrk_off, syrk_cnt; };
 struct LevelPlan {
-    int small_off = 0, small_cnt = 0, small_max_r = 0;     // into d_small_list
-    int asm_off = 0, asm_cnt = 0;                          // into d_items
-    std::vector<StepPlan> steps;
     int all_off = 0, all_cnt = 0, all_max_r = 0;           // every supernode of the level (solves), into d_lvl_sn
 };
 
@@ -42,9 +38,8 @@ struct nmpc_handle_s {
     IpmVectors V{};
     std::vector<void*> allocs;
     std::vector<LevelPlan> plan;
-    int32_t* d_small_list = nullptr;
     int32_t* d_lvl_sn = nullptr;
-    BigItem* d_items = nullptr;
+    FactorPlan F;
     int n_big_fronts = 0;
     double* d_eta = nullptr;
     double* d_Kval = nullptr;          // values last factored (pattern order)
@@ -53,8 +48,8 @@ struct nmpc_handle_s {
     double* d_uinit = nullptr;
     double* h_pinned = nullptr;        // pinned host scratch: [0..15] scalars, [16] flag, staging for host-buffer calls
     size_t pinned_doubles = 0;
-    cudaGraphExec_t g_factor = nullptr, g_fwdbwd = nullptr;
-    int g_factor_nodes = 0, g_fwdbwd_nodes = 0;
+    cudaGraphExec_t g_fwdbwd = nullptr;
+    int g_fwdbwd_nodes = 0;
     bool factored = false, have_state = false, has_model = false;
     double eta_cur = 0.0;
     int64_t launches = 0;
@@ -98,84 +93,123 @@ nmpc_status dalloc(nmpc_handle_s* h, size_t count, T** out, bool zero = true) {
 
 #define TRY(x) do { nmpc_status s__ = (x); if (s__ != NMPC_OK) return s__; } while (0)
 
-// ---- level schedule: which supernodes run in the shared-memory kernel, and the tile work lists of the big ones ----
-nmpc_status build_plan(nmpc_handle_s* h, int smem_max_r) {
+// ---- task list of the persistent factorization kernel + level lists of the solves ----
+nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_t smem_bytes, int num_sms) {
     const Symbolic& S = h->S;
-    std::vector<int32_t> small_list;
-    std::vector<BigItem> items;
+    const int ns = S.ns;
     h->plan.assign(S.nlevels, LevelPlan());
-    h->n_big_fronts = 0;
     for (int l = 0; l < S.nlevels; ++l) {
         LevelPlan& P = h->plan[l];
         P.all_off = S.lvl_ptr[l]; P.all_cnt = S.lvl_ptr[l + 1] - S.lvl_ptr[l];
-        P.small_off = (int)small_list.size();
-        std::vector<int32_t> big;
-        for (int q = S.lvl_ptr[l]; q < S.lvl_ptr[l + 1]; ++q) {
-            const int s = S.lvl_sn[q];
-            const int r = (int)(S.rows_ptr[s + 1] - S.rows_ptr[s]);
-            P.all_max_r = std::max(P.all_max_r, r);
-            if (r <= smem_max_r) { small_list.push_back(s); P.small_max_r = std::max(P.small_max_r, r); }
-            else big.push_back(s);
-        }
-        P.small_cnt = (int)small_list.size() - P.small_off;
-        h->n_big_fronts += (int)big.size();
-        if (big.empty()) continue;
-        P.asm_off = (int)items.size();
-        int max_w = 0;
-        for (int s : big) {
-            const int r = (int)(S.rows_ptr[s + 1] - S.rows_ptr[s]), w = S.sn_start[s + 1] - S.sn_start[s];
-            max_w = std::max(max_w, w);
-            const int cw = std::max(4, std::min(64, 32768 / r));
-            for (int c = 0; c < r; c += cw) items.push_back(BigItem{s, c, std::min(r, c + cw), 0});
-        }
-        P.asm_cnt = (int)items.size() - P.asm_off;
-        const int nsteps = (max_w + BIG_NB - 1) / BIG_NB;
-        for (int t = 0; t < nsteps; ++t) {
-            StepPlan sp{};
-            const int j0 = t * BIG_NB;
-            sp.potrf_off = (int)items.size();
-            for (int s : big) { const int w = S.sn_start[s + 1] - S.sn_start[s]; if (j0 < w) items.push_back(BigItem{s, j0, 0, 0}); }
-            sp.potrf_cnt = (int)items.size() - sp.potrf_off;
-            sp.trsm_off = (int)items.size();
-            for (int s : big) {
-                const int r = (int)(S.rows_ptr[s + 1] - S.rows_ptr[s]), w = S.sn_start[s + 1] - S.sn_start[s];
-                if (j0 >= w) continue;
-                const int j1 = std::min(w, j0 + BIG_NB);
-                for (int i0 = j1; i0 < r; i0 += BIG_NB) items.push_back(BigItem{s, j0, i0, 0});
-            }
-            sp.trsm_cnt = (int)items.size() - sp.trsm_off;
-            sp.syrk_off = (int)items.size();
-            for (int s : big) {
-                const int r = (int)(S.rows_ptr[s + 1] - S.rows_ptr[s]), w = S.sn_start[s + 1] - S.sn_start[s];
-                if (j0 >= w) continue;
-                const int j1 = std::min(w, j0 + BIG_NB);
-                for (int J0 = j1; J0 < r; J0 += BIG_NB)
-                    for (int I0 = J0; I0 < r; I0 += BIG_NB) items.push_back(BigItem{s, j0, I0, J0});
-            }
-            sp.syrk_cnt = (int)items.size() - sp.syrk_off;
-            P.steps.push_back(sp);
-        }
+        for (int q = S.lvl_ptr[l]; q < S.lvl_ptr[l + 1]; ++q)
+            P.all_max_r = std::max(P.all_max_r, (int)(S.rows_ptr[S.lvl_sn[q] + 1] - S.rows_ptr[S.lvl_sn[q]]));
     }
-    const int32_t* tmp = nullptr;
-    TRY(upload(h, small_list, &tmp)); h->d_small_list = const_cast<int32_t*>(tmp);
-    TRY(upload(h, S.lvl_sn, &tmp)); h->d_lvl_sn = const_cast<int32_t*>(tmp);
-    const BigItem* ti = nullptr;
-    TRY(upload(h, items, &ti)); h->d_items = const_cast<BigItem*>(ti);
-    return NMPC_OK;
-}
+    auto R = [&](int s) { return (int)(S.rows_ptr[s + 1] - S.rows_ptr[s]); };
+    auto W = [&](int s) { return S.sn_start[s + 1] - S.sn_start[s]; };
+    std::vector<int32_t> cls(ns), tbase(ns, 0), target(ns, 1), nbp(ns, 0), nbt(ns, 0);
+    int64_t slots = 0;
+    h->n_big_fronts = 0;
+    for (int s = 0; s < ns; ++s) {
+        cls[s] = R(s) > small_max_r;
+        if (!cls[s]) continue;
+        h->n_big_fronts++;
+        nbp[s] = tile_nbp(W(s)); nbt[s] = nbp[s] + tile_nbu(W(s), R(s));
+        tbase[s] = (int32_t)slots;
+        slots += (int64_t)nbp[s] * nbt[s] + 1;
+        target[s] = nbt[s] * (nbt[s] + 1) / 2;
+        if (slots > INT32_MAX / 2) { h->err = "too many tiles"; return NMPC_E_ALLOC; }
+    }
+    // K scatter map per front class: small = packed lower offset; tiled = tile-local offset, entries sorted by tile slot
+    std::vector<int32_t> ksrc(S.kent_src), kdst(S.kent_dst);
+    std::vector<int64_t> tile_kptr((size_t)slots + 1, 0);
+    for (int s = 0; s < ns; ++s) {
+        const int r = R(s), w = W(s), ld = ld_even(r);
+        const int64_t q0 = S.kent_ptr[s], q1 = S.kent_ptr[s + 1];
+        if (!cls[s]) {
+            for (int64_t q = q0; q < q1; ++q) {
+                const int j = S.kent_dst[q] / ld, i = S.kent_dst[q] - j * ld;
+                kdst[q] = j * r - (j * (j - 1)) / 2 + (i - j);
+            }
+            continue;
+        }
+        std::vector<int32_t> bof(r);                     // block of every front row
+        for (int k = 0, i = 0; k < nbt[s]; ++k) { const int e = tile_bound(k + 1, w, r, nbp[s]); for (; i < e; ++i) bof[i] = k; }
+        std::vector<std::pair<int64_t, int64_t>> key((size_t)(q1 - q0));   // (slot, q)
+        for (int64_t q = q0; q < q1; ++q) {
+            const int j = S.kent_dst[q] / ld, i = S.kent_dst[q] - j * ld;
+            key[q - q0] = {(int64_t)bof[j] * nbt[s] + bof[i], q};
+        }
+        std::sort(key.begin(), key.end());
+        const int64_t nslot = (int64_t)nbp[s] * nbt[s];
+        std::vector<int64_t> cnt((size_t)nslot + 1, 0);
+        for (int64_t e = 0; e < q1 - q0; ++e) {
+            const int64_t q = key[e].second;
+            const int j = S.kent_dst[q] / ld, i = S.kent_dst[q] - j * ld;
+            const int I = bof[i], J = bof[j];
+            ksrc[q0 + e] = S.kent_src[q];
+            kdst[q0 + e] = (i - tile_bound(I, w, r, nbp[s])) + (j - tile_bound(J, w, r, nbp[s])) * 66;
+            cnt[key[e].first + 1]++;
+        }
+        for (int64_t k = 0; k <= nslot; ++k) { if (k) cnt[k] += cnt[k - 1]; tile_kptr[tbase[s] + k] = q0 + cnt[k]; }
+    }
+    // block boundaries of every child of a tiled parent inside that parent's rows
+    std::vector<int64_t> cb_ptr(ns, -1);
+    std::vector<int32_t> cbnd;
+    for (int c = 0; c < ns; ++c) {
+        const int p = S.sn_parent[c];
+        if (p < 0 || !cls[p]) continue;
+        cb_ptr[c] = (int64_t)cbnd.size();
+        const int32_t* rel = S.rel.data() + S.rel_ptr[c];
+        const int mc = (int)(S.rel_ptr[c + 1] - S.rel_ptr[c]);
+        for (int k = 0; k <= nbt[p]; ++k)
+            cbnd.push_back((int32_t)(std::lower_bound(rel, rel + mc, tile_bound(k, W(p), R(p), nbp[p])) - rel));
+    }
+    // task order: descending upward rank (longest remaining path, microseconds of a crude cost model); children rank above
+    // their parent, tile (I,k) above tile (I,J) for k < J -> the order is topological
+    const double STEP_US = 10.0;                         // one block column of a tiled front: potrf + trsm + flag hops
+    auto front_time = [&](int s) {
+        if (!cls[s]) { const double r = R(s), m = R(s) - W(s); return 2.0 + (r * r * r - m * m * m) / 3.0 * 2.0 / 50e3; }   // ~50 GFLOP/s per CTA
+        return nbp[s] * STEP_US + 2.0 + W(s) / 16.0 * 0.4;
+    };
+    std::vector<double> rank_end(ns, 0.0);
+    for (int s = ns - 1; s >= 0; --s) {                  // parents have larger indices (postorder)
+        const int p = S.sn_parent[s];
+        rank_end[s] = p < 0 ? 0.0 : rank_end[p] + front_time(p);
+    }
+    struct TK { double rank; int32_t lvl, type, s, I, J; };
+    std::vector<TK> tk;
+    for (int s = 0; s < ns; ++s) {
+        if (!cls[s]) { tk.push_back(TK{rank_end[s] + front_time(s), S.sn_level[s], 0, s, 0, 0}); continue; }
+        const double tail = 2.0 + W(s) / 16.0 * 0.4;
+        for (int J = 0; J < nbt[s]; ++J)
+            for (int I = J; I < nbt[s]; ++I)
+                tk.push_back(TK{rank_end[s] + tail + (J < nbp[s] ? (nbp[s] - J) * STEP_US : 0.0), S.sn_level[s], 1, s, I, J});
+    }
+    std::stable_sort(tk.begin(), tk.end(), [](const TK& a, const TK& b) {
+        if (a.rank != b.rank) return a.rank > b.rank;
+        if (a.lvl != b.lvl) return a.lvl < b.lvl;
+        if (a.J != b.J) return a.J < b.J;
+        if (a.s != b.s) return a.s < b.s;
+        return a.I < b.I;
+    });
+    std::vector<int4> tasks(tk.size());
+    for (size_t t = 0; t < tk.size(); ++t) tasks[t] = make_int4(tk[t].type, tk[t].s, tk[t].I, tk[t].J);
 
-int issue_factor(nmpc_handle_s* h) {          // returns the number of kernels launched
-    int nk = 0;
-    for (const LevelPlan& P : h->plan) {
-        if (P.small_cnt) { launch_front_small(h->D, h->d_small_list + P.small_off, P.small_cnt, P.small_max_r, h->d_Kval, h->stream); ++nk; }
-        if (P.asm_cnt) { launch_big_assemble(h->D, h->d_items + P.asm_off, P.asm_cnt, h->d_Kval, h->stream); ++nk; }
-        for (const StepPlan& sp : P.steps) {
-            if (sp.potrf_cnt) { launch_big_potrf(h->D, h->d_items + sp.potrf_off, sp.potrf_cnt, h->stream); ++nk; }
-            if (sp.trsm_cnt) { launch_big_trsm(h->D, h->d_items + sp.trsm_off, sp.trsm_cnt, h->stream); ++nk; }
-            if (sp.syrk_cnt) { launch_big_syrk(h->D, h->d_items + sp.syrk_off, sp.syrk_cnt, h->stream); ++nk; }
-        }
-    }
-    return nk;
+    FactorPlan& F = h->F;
+    const int32_t* ti = nullptr; const int64_t* tl = nullptr; const int4* t4 = nullptr;
+    TRY(upload(h, S.lvl_sn, &ti)); h->d_lvl_sn = const_cast<int32_t*>(ti);
+    TRY(upload(h, tasks, &t4)); F.tasks = t4; F.ntasks = (int32_t)tasks.size();
+    TRY(upload(h, cls, &F.cls)); TRY(upload(h, tbase, &F.tbase)); TRY(upload(h, target, &F.target));
+    TRY(upload(h, tile_kptr, &tl)); F.tile_kptr = tl;
+    TRY(upload(h, cb_ptr, &tl)); F.cb_ptr = tl;
+    TRY(upload(h, cbnd, &F.cbnd));
+    TRY(upload(h, ksrc, &h->D.kent_src)); TRY(upload(h, kdst, &h->D.kent_dst));
+    F.sync_words = (int32_t)(1 + ns + slots);
+    TRY(dalloc(h, (size_t)F.sync_words, &F.sync));
+    F.small_max_r = small_max_r;
+    F.smem_bytes = smem_bytes;
+    F.grid = (int32_t)std::max<int64_t>(1, std::min<int64_t>((int64_t)tasks.size(), (int64_t)num_sms * ctas_per_sm));
+    return NMPC_OK;
 }
 
 int issue_fwdbwd(nmpc_handle_s* h) {
@@ -203,9 +237,7 @@ nmpc_status capture(nmpc_handle_s* h, int (*issue)(nmpc_handle_s*), cudaGraphExe
 }
 
 nmpc_status run_factor(nmpc_handle_s* h, double eta, int64_t* info) {
-    launch_reset_flag(h->D, h->d_eta, eta, h->stream); h->launches++;
-    if (h->g_factor) { CK(cudaGraphLaunch(h->g_factor, h->stream)); h->launches += h->g_factor_nodes; }
-    else h->launches += issue_factor(h);
+    launch_factor(h->D, h->F, h->d_Kval, h->d_eta, eta, h->stream); h->launches += 2;
     int32_t* flag = reinterpret_cast<int32_t*>(h->h_pinned + 16);
     CK(cudaMemcpyAsync(flag, h->D.fail_col, sizeof(int32_t), cudaMemcpyDeviceToHost, h->stream));
     CK(cudaStreamSynchronize(h->stream));
@@ -266,10 +298,12 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
         int dev = 0, smem_optin = 0;
         CK(cudaGetDevice(&dev));
         CK(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
-        CK(configure_factor_kernels(smem_optin));
-        int smem_max_r = (int)std::floor(std::sqrt((double)smem_optin / 8.0));
-        if (h->opt.smem_front_max > 0) smem_max_r = std::min(smem_max_r, h->opt.smem_front_max);
-        else smem_max_r = std::min(smem_max_r, 160);
+        int num_sms = 0, ctas_per_sm = 1, small_max_r = 0;
+        size_t factor_smem = 0;
+        CK(cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev));
+        CK(configure_factor_kernels(smem_optin, &ctas_per_sm, &factor_smem, &small_max_r));
+        CK(configure_solve_kernels(smem_optin));
+        if (h->opt.smem_front_max > 0) small_max_r = std::min(small_max_r, h->opt.smem_front_max);
         if (((size_t)((S.max_front + 1) & ~1) + (size_t)BIG_NB * (BIG_NB + 1)) * 8 > (size_t)smem_optin) { h->err = "front too large for the solve kernel"; return NMPC_E_ALLOC; }
         DevSym& D = h->D;
         D.ns = S.ns; D.n = S.n;
@@ -277,13 +311,13 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
         TRY(upload(h, S.child_ptr, &D.child_ptr)); TRY(upload(h, S.child_idx, &D.child_idx));
         TRY(upload(h, S.rel_ptr, &D.rel_ptr)); TRY(upload(h, S.rel, &D.rel));
         TRY(upload(h, S.panel_ptr, &D.panel_ptr)); TRY(upload(h, S.upd_ptr, &D.upd_ptr));
-        TRY(upload(h, S.kent_ptr, &D.kent_ptr)); TRY(upload(h, S.kent_src, &D.kent_src)); TRY(upload(h, S.kent_dst, &D.kent_dst));
+        TRY(upload(h, S.kent_ptr, &D.kent_ptr));                 // kent_src / kent_dst: per front class, in build_plan
         TRY(upload(h, S.perm, &D.perm));
-        TRY(dalloc(h, (size_t)S.panel_ptr.back(), &D.L)); TRY(dalloc(h, (size_t)S.upd_ptr.back(), &D.U, false));
+        TRY(dalloc(h, (size_t)S.panel_ptr.back() + 4 * TILE, &D.L)); TRY(dalloc(h, (size_t)S.upd_ptr.back(), &D.U, false));
         TRY(dalloc(h, (size_t)S.rel_ptr.back(), &D.ctr)); TRY(dalloc(h, 1, &D.fail_col));
         TRY(dalloc(h, 1, &h->d_eta)); D.eta = h->d_eta;
         TRY(dalloc(h, (size_t)S.nnzK, &h->d_Kval)); TRY(dalloc(h, (size_t)S.n, &h->d_x));
-        TRY(build_plan(h, smem_max_r));
+        TRY(build_plan(h, small_max_r, ctas_per_sm, factor_smem, num_sms));
         // symmetric CSR of K for nmpc_kkt_multiply
         {
             const int64_t n = S.n;
@@ -345,7 +379,6 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
         CK(cudaEventCreate(&h->ev[0])); CK(cudaEventCreate(&h->ev[1]));
         CK(cudaStreamSynchronize(h->stream));
         if (h->opt.use_graph) {
-            TRY(capture(h, issue_factor, &h->g_factor, &h->g_factor_nodes));
             TRY(capture(h, issue_fwdbwd, &h->g_fwdbwd, &h->g_fwdbwd_nodes));
         }
         return NMPC_OK;
@@ -358,7 +391,6 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
 
 void nmpc_destroy(nmpc_handle h) {
     if (!h) return;
-    if (h->g_factor) cudaGraphExecDestroy(h->g_factor);
     if (h->g_fwdbwd) cudaGraphExecDestroy(h->g_fwdbwd);
     for (void* p : h->allocs) cudaFree(p);
     if (h->h_pinned) cudaFreeHost(h->h_pinned);

@@ -1,7 +1,7 @@
 // device.h -- device-side data layout and kernel launch wrappers shared by factor.cu / ipm.cu / api.cu.
 //
 // HBM layout (all owned by the handle, allocated once in nmpc_analyze):
-//   L   : one dense column-major panel per supernode s, r_s x w_s (leading dimension r_s), at panel_ptr[s]
+//   L   : one dense column-major panel per supernode s, r_s x w_s (leading dimension r_s rounded up to even), at panel_ptr[s]
 //   U   : one dense column-major update (Schur complement) matrix per supernode, (r_s-w_s)^2, at upd_ptr[s];
 //         only the lower triangle is written and read (multifrontal extend-add, parent pulls from children
 //         in a fixed order -> bitwise reproducible)
@@ -38,23 +38,55 @@ struct DevSym {                   // device copies of the symbolic arrays (symbo
     const double* eta = nullptr;  // device scalar: diagonal shift eta_y of Eq. (13)/(17), read by the assembly kernels
 };
 
-constexpr int BIG_NB = 64;        // block size of the tiled (global-memory) front path
+constexpr int BIG_NB = 64;        // block size used by the triangular-solve kernels for the diagonal blocks
+constexpr int TILE = 64;          // tile size of the tiled (HBM-resident) fronts
 
-struct BigItem { int32_t sn, a, b, c; };   // work item of the tiled path: supernode + tile coordinates
+__host__ __device__ inline int ld_even(int r) { return (r + 1) & ~1; }   // = symbolic.h: panel_ld
+
+// Block boundaries of a tiled front (rows == columns): nbp blocks of 64 over the pivot columns [0,w) (last one ragged),
+// then blocks over the update rows [w,r); when w is odd the first update block has 63 rows so that every later
+// boundary is even (16-byte aligned operand loads).
+__host__ __device__ inline int tile_bound(int k, int w, int r, int nbp) {
+    if (k < nbp) return k * TILE;
+    if (k == nbp) return w;
+    const int v = w + TILE - (w & 1) + TILE * (k - nbp - 1);
+    return v < r ? v : r;
+}
+__host__ __device__ inline int tile_nbp(int w) { return (w + TILE - 1) / TILE; }
+__host__ __device__ inline int tile_nbu(int w, int r) {
+    if (r <= w) return 0;
+    const int e1 = w + TILE - (w & 1);
+    return r <= e1 ? 1 : 1 + (r - e1 + TILE - 1) / TILE;
+}
+
+// Task list of the persistent task-DAG factorization kernel, built once by nmpc_analyze.
+//   task = (type, sn, I, J): type 0 = whole small front in shared memory, 1 = tile (I,J) of a tiled front, left-looking.
+// sync[0] = next task; sync[1 .. ns] = per-front completion counters; sync[1+ns ..] = per-panel-tile done flags.
+struct FactorPlan {
+    const int4* tasks = nullptr;
+    int32_t ntasks = 0;
+    const int32_t* cls = nullptr;        // ns: 0 small, 1 tiled
+    const int32_t* tbase = nullptr;      // ns: base of the front's (nbp x nbt + 1) slots in tile_done / tile_kptr
+    const int32_t* target = nullptr;     // ns: completions that finish the front (1, or the number of tiles)
+    const int64_t* tile_kptr = nullptr;  // per tile slot: start of its K entries (kent arrays sorted by tile for tiled fronts)
+    const int64_t* cb_ptr = nullptr;     // ns: offset into cbnd of the child's block boundaries in its (tiled) parent, else -1
+    const int32_t* cbnd = nullptr;
+    uint32_t* sync = nullptr;
+    int32_t sync_words = 0;
+    int32_t small_max_r = 0;             // largest front handled by the shared-memory task
+    int32_t grid = 0;
+    size_t smem_bytes = 0;
+};
 
 // ---- factor.cu ----
-void launch_front_small(const DevSym& D, const int32_t* sn_list, int count, int max_r, const double* Kval, cudaStream_t st);
-void launch_big_assemble(const DevSym& D, const BigItem* items, int count, const double* Kval, cudaStream_t st);
-void launch_big_potrf(const DevSym& D, const BigItem* items, int count, cudaStream_t st);
-void launch_big_trsm(const DevSym& D, const BigItem* items, int count, cudaStream_t st);
-void launch_big_syrk(const DevSym& D, const BigItem* items, int count, cudaStream_t st);
+cudaError_t configure_factor_kernels(int max_smem_bytes, int* ctas_per_sm, size_t* smem_bytes, int* small_max_r);
+void launch_factor(const DevSym& D, const FactorPlan& F, const double* Kval, double* eta_dev, double eta, cudaStream_t st);   // 2 launches
+// ---- solve.cu ----
+cudaError_t configure_solve_kernels(int max_smem_bytes);
 void launch_solve_fwd(const DevSym& D, const int32_t* sn_list, int count, int max_r, double* x, cudaStream_t st);
 void launch_solve_bwd(const DevSym& D, const int32_t* sn_list, int count, int max_r, double* x, cudaStream_t st);
 void launch_permute_in(const DevSym& D, const double* b, double* x, cudaStream_t st);     // x[i] = b[perm[i]]
 void launch_permute_out(const DevSym& D, const double* x, double* b, cudaStream_t st);    // b[perm[i]] = x[i]
-void launch_reset_flag(const DevSym& D, double* eta_dev, double eta, cudaStream_t st);   // fail_col = INT_MAX, *eta_dev = eta
-size_t small_front_smem_bytes(int max_r);
-cudaError_t configure_factor_kernels(int max_smem_bytes);
 
 // ---- ipm.cu ----
 struct DevModel {                 // device copies of the model maps (symbolic.h: ModelMaps) + parameters

@@ -1,16 +1,19 @@
-// factor.cu -- numeric multifrontal supernodal Cholesky (step a4, NumCholesky Eq. (20)-(21)) and the
-// supernodal triangular solves (step a5, Eq. (22)-(25)) on the fixed structure S_L produced once by
-// symbolic.cpp.  fp64 throughout, no atomics on floating-point data, fixed summation order -> bitwise reproducible.
+// factor.cu -- numeric multifrontal supernodal Cholesky (step a4, NumCholesky Eq. (20)-(21)) on the fixed
+// structure S_L produced once by symbolic.cpp, as ONE persistent task-DAG kernel.
 //
-// Two kernel families, chosen per supernode at analysis time by the front size r:
-//   small  (r <= smem_front_max): ONE CTA assembles the whole r x r front in shared memory (K entries through the
-//          scatter map + extend-add of the children's update matrices, pulled in fixed child order), factors its w
-//          pivot columns (Eq. 21 column by column), and writes the r x w panel of L and the (r-w)^2 update matrix.
-//   big    (r >  smem_front_max): the front lives in HBM (panel + update storage are the front); a column-slice
-//          assembly kernel, then per 64-column block step: POTRF of the diagonal block, TRSM of the block column,
-//          SYRK/GEMM update of the trailing front.  Launches are batched over all big fronts of a tree level.
+// The host analysis emits a topologically ordered task list (api.cu: build_plan).  CTAs claim tasks in order from an atomic
+// counter and wait on completion flags (acquire/release at gpu scope) instead of kernel boundaries:
+//   task type 0, small front (r <= small_max_r): ONE CTA assembles the whole front in shared memory (packed lower triangle):
+//          K entries through the scatter map + extend-add of the children's update matrices, pulled in fixed child order;
+//          blocked partial Cholesky of its w pivot columns; writes the panel of L and the (r-w)^2 update matrix.
+//   task type 1, tile (I,J) of a tiled front (r > small_max_r; the front lives in HBM as panel + update storage), LEFT-looking:
+//          acc = sum_k X(I,k) X(J,k)^T over the finished tiles of block rows I and J (fp64 DMMA mma.sync.m8n8k4, operands
+//          streamed with cp.async.cg through a 3-stage shared-memory ring, waiting on each 64-column block's flags as it is
+//          reached); C = assembled tile (K entries + children's contributions) - acc; then POTRF (I == J) or TRSM against the
+//          finished diagonal tile (I > J) in shared memory; each tile of L / of the update matrix is written exactly once.
+// In-order claiming of a topological order cannot deadlock: the lowest-numbered unfinished task depends only on finished ones.
+// fp64 throughout, no floating-point atomics, fixed summation order -> bitwise reproducible.
 #include <climits>
-#include <cstdio>
 
 #include "device.h"
 
@@ -18,391 +21,432 @@ namespace nmpc {
 
 namespace {
 
-constexpr int NT = 256;                 // threads per CTA for every kernel in this file
+constexpr int NT = 256;                 // threads per CTA
+constexpr int KC = 16;                  // k-columns per pipeline stage
+constexpr int ALD = 68;                 // leading dimension of an operand stage  (68 mod 16 == 4: conflict-free DMMA fragment loads)
+constexpr int CLD = 66;                 // leading dimension of the C / L_JJ tile (2*66 mod 16 == 4: conflict-free fragment stores)
+constexpr int NSTAGE = 3;
+constexpr int STAGE_DOUBLES = 2 * KC * ALD;
+constexpr int PIPE_DOUBLES = NSTAGE * STAGE_DOUBLES;          // 6528
+constexpr int CT_DOUBLES = TILE * CLD;                        // 4224
+constexpr int TILE_SMEM_DOUBLES = PIPE_DOUBLES + CT_DOUBLES;  // 10752 doubles = 86016 B
+static_assert(CT_DOUBLES + TILE <= PIPE_DOUBLES, "L_JJ tile + reciprocals alias the operand ring");
 
-struct FrontView {                      // the r x r front of a supernode, split over panel (cols < w) and update storage
-    double* P; double* Uu; int r, w, m;
-    __device__ __forceinline__ double* at(int i, int c) const {
-        return c < w ? P + (i + (int64_t)c * r) : Uu + ((i - w) + (int64_t)(c - w) * m);
-    }
-};
-
-__device__ __forceinline__ FrontView front_view(const DevSym& D, int s) {
-    FrontView F;
-    F.w = D.sn_start[s + 1] - D.sn_start[s];
-    F.r = (int)(D.rows_ptr[s + 1] - D.rows_ptr[s]);
-    F.m = F.r - F.w;
-    F.P = D.L + D.panel_ptr[s];
-    F.Uu = D.U + D.upd_ptr[s];
-    return F;
+// ---- gpu-scope acquire / release on the completion flags ----
+__device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
+    uint32_t v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release(uint32_t* p, uint32_t v) {
+    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void red_release_add(uint32_t* p, uint32_t v) {
+    asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void spin_until_ge(const uint32_t* p, uint32_t target) {
+    while (ld_acquire(p) < target) __nanosleep(40);
+}
+__device__ __forceinline__ void cp_async16(double* dst_smem, const double* src, int src_bytes) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
 }
 
-__device__ __forceinline__ bool bad_pivot(double d) { return !(d > 0.0) || isinf(d); }
+// =============================================================================================================
+// Blocked partial Cholesky of the first w columns of an r x r lower-stored matrix in shared memory (Eq. 21, 8 columns
+// per step).  colp(j)[i] addresses element (i,j), i >= j.  Per step: every thread factors the 8x8 diagonal block
+// redundantly in registers (identical arithmetic -> identical values, no barrier), thread t solves row j0+t of the block
+// column against it; barrier; rank-8 update of the trailing lower triangle (warp = 4 columns, lanes = rows); barrier.
+// Requires r - j0 <= NT.  A pivot <= 0 or non-finite (reading G11) is replaced by 1 and reported through fail_col.
+// =============================================================================================================
+template <class ColFn>
+__device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, int32_t* fail_col) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (int j0 = 0; j0 < w; j0 += 8) {
+        const int jb = min(8, w - j0);
+        double Dg[8][8], inv[8];
+#pragma unroll
+        for (int c = 0; c < 8; ++c)
+#pragma unroll
+            for (int i = c; i < 8; ++i) Dg[i][c] = (i < jb) ? colp(j0 + c)[j0 + i] : (i == c ? 1.0 : 0.0);   // i < jb implies c < jb
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            double d = Dg[c][c];
+            if (!(d > 0.0) || isinf(d)) {
+                d = 1.0;
+                if (tid == 0 && c < jb) atomicMin(fail_col, c0 + j0 + c);
+            }
+            const double sq = sqrt(d);
+            Dg[c][c] = sq;
+            inv[c] = 1.0 / sq;
+#pragma unroll
+            for (int i = c + 1; i < 8; ++i) Dg[i][c] *= inv[c];
+#pragma unroll
+            for (int k = c + 1; k < 8; ++k)
+#pragma unroll
+                for (int i = k; i < 8; ++i) Dg[i][k] = fma(-Dg[i][c], Dg[k][c], Dg[i][k]);
+        }
+        const int i = j0 + tid;
+        if (i < r) {
+            if (tid < jb) {                              // a row of the diagonal block: store L
+#pragma unroll
+                for (int ii = 0; ii < 8; ++ii)
+                    if (tid == ii) {
+#pragma unroll
+                        for (int c = 0; c <= ii; ++c) colp(j0 + c)[i] = Dg[ii][c];
+                    }
+            } else {                                     // a row below: x = f L_D^-T
+                double x[8];
+#pragma unroll
+                for (int c = 0; c < 8; ++c) x[c] = (c < jb) ? colp(j0 + c)[i] : 0.0;
+#pragma unroll
+                for (int c = 0; c < 8; ++c) {
+                    double v = x[c];
+#pragma unroll
+                    for (int k = 0; k < c; ++k) v = fma(-x[k], Dg[c][k], v);
+                    x[c] = v * inv[c];
+                }
+#pragma unroll
+                for (int c = 0; c < 8; ++c)
+                    if (c < jb) colp(j0 + c)[i] = x[c];
+            }
+        }
+        __syncthreads();
+        const int t0 = j0 + jb, ntr = r - t0;
+        for (int g = warp; g * 4 < ntr; g += NT / 32) {
+            const int cbase = t0 + 4 * g;
+            double xc[4][8];
+#pragma unroll
+            for (int cc = 0; cc < 4; ++cc)
+#pragma unroll
+                for (int k = 0; k < 8; ++k) xc[cc][k] = (cbase + cc < r && k < jb) ? colp(j0 + k)[cbase + cc] : 0.0;
+            for (int ii = cbase + lane; ii < r; ii += 32) {
+                double xi[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) xi[k] = (k < jb) ? colp(j0 + k)[ii] : 0.0;
+#pragma unroll
+                for (int cc = 0; cc < 4; ++cc) {
+                    const int c = cbase + cc;
+                    if (c < r && ii >= c) {
+                        double* fp = colp(c) + ii;
+                        double f = *fp;
+#pragma unroll
+                        for (int k = 0; k < 8; ++k) f = fma(-xi[k], xc[cc][k], f);
+                        *fp = f;
+                    }
+                }
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// X = C L^-T for an ni x nj tile C (column-major, CLD) against the nj x nj lower-triangular Ls (column-major, CLD), in place.
+__device__ __forceinline__ void trsm_tile(double* Cs, const double* Ls, const double* rinv, int ni, int nj) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (int j0 = 0; j0 < nj; j0 += 8) {
+        const int jb = min(8, nj - j0);
+        if (tid < ni) {
+            double x[8];
+#pragma unroll
+            for (int c = 0; c < 8; ++c) x[c] = (c < jb) ? Cs[(j0 + c) * CLD + tid] : 0.0;
+#pragma unroll
+            for (int c = 0; c < 8; ++c)
+                if (c < jb) {
+                    double v = x[c];
+#pragma unroll
+                    for (int k = 0; k < c; ++k) v = fma(-x[k], Ls[(j0 + k) * CLD + j0 + c], v);
+                    x[c] = v * rinv[j0 + c];
+                }
+#pragma unroll
+            for (int c = 0; c < 8; ++c)
+                if (c < jb) Cs[(j0 + c) * CLD + tid] = x[c];
+        }
+        __syncthreads();
+        const int t0 = j0 + jb, ntr = nj - t0;
+        for (int g = warp; g * 4 < ntr; g += NT / 32) {
+            const int cbase = t0 + 4 * g;
+            double lc[4][8];
+#pragma unroll
+            for (int cc = 0; cc < 4; ++cc)
+#pragma unroll
+                for (int k = 0; k < 8; ++k) lc[cc][k] = (cbase + cc < nj && k < jb) ? Ls[(j0 + k) * CLD + cbase + cc] : 0.0;
+            for (int ii = lane; ii < ni; ii += 32) {
+                double xi[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) xi[k] = (k < jb) ? Cs[(j0 + k) * CLD + ii] : 0.0;
+#pragma unroll
+                for (int cc = 0; cc < 4; ++cc)
+                    if (cbase + cc < nj) {
+                        double* fp = Cs + (cbase + cc) * CLD + ii;
+                        double f = *fp;
+#pragma unroll
+                        for (int k = 0; k < 8; ++k) f = fma(-xi[k], lc[cc][k], f);
+                        *fp = f;
+                    }
+            }
+        }
+        __syncthreads();
+    }
+}
 
 // =============================================================================================================
-// small fronts: whole front in shared memory
+// task type 0: whole front in shared memory, packed lower triangle: element (i,j), i >= j, at j*r - j(j-1)/2 + (i-j)
 // =============================================================================================================
-__global__ void __launch_bounds__(NT) front_small_kernel(DevSym D, const int32_t* __restrict__ sn_list,
-                                                         const double* __restrict__ Kval) {
-    extern __shared__ double F[];
-    const double eta = *D.eta;
+__device__ __forceinline__ void small_front_task(const DevSym& D, const FactorPlan& F, int s, const double* __restrict__ Kval,
+                                                 double eta, double* sm) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = NT / 32;
-    const int s = sn_list[blockIdx.x];
     const int c0 = D.sn_start[s], w = D.sn_start[s + 1] - c0;
     const int r = (int)(D.rows_ptr[s + 1] - D.rows_ptr[s]);
-    // 1. zero
-    for (int idx = tid; idx < r * r; idx += NT) F[idx] = 0.0;
+    uint32_t* front_done = F.sync + 1;
+    auto colp = [sm, r](int j) { return sm + (j * r - ((j * (j - 1)) >> 1) - j); };
+    const int ntri = (r * (r + 1)) >> 1;
+    for (int idx = tid; idx < ntri; idx += NT) sm[idx] = 0.0;
+    const int ch0 = D.child_ptr[s], ch1 = D.child_ptr[s + 1];
+    if (tid < ch1 - ch0) { const int c = D.child_idx[ch0 + tid]; spin_until_ge(front_done + c, F.target[c]); }
+    for (int ci = ch0 + NT + tid; ci < ch1; ci += NT) { const int c = D.child_idx[ci]; spin_until_ge(front_done + c, F.target[c]); }
     __syncthreads();
-    // 2. K entries of the pivot columns (scatter map: kent_dst = i + j*r)
-    for (int64_t q = D.kent_ptr[s] + tid; q < D.kent_ptr[s + 1]; q += NT) F[D.kent_dst[q]] = Kval[D.kent_src[q]];
+    for (int64_t q = D.kent_ptr[s] + tid; q < D.kent_ptr[s + 1]; q += NT) sm[D.kent_dst[q]] = Kval[D.kent_src[q]];
     __syncthreads();
-    if (eta != 0.0) for (int j = tid; j < w; j += NT) F[j + j * r] += eta;
-    // 3. extend-add of the children's update matrices, fixed child order
-    for (int ci = D.child_ptr[s]; ci < D.child_ptr[s + 1]; ++ci) {
+    if (eta != 0.0) for (int j = tid; j < w; j += NT) colp(j)[j] += eta;
+    for (int ci = ch0; ci < ch1; ++ci) {                 // extend-add, fixed child order
         const int c = D.child_idx[ci];
         const int mc = (int)(D.rel_ptr[c + 1] - D.rel_ptr[c]);
-        const double* __restrict__ Uc = D.U + D.upd_ptr[c];
+        const double* Uc = D.U + D.upd_ptr[c];
         const int32_t* __restrict__ rel = D.rel + D.rel_ptr[c];
         __syncthreads();
         for (int b = warp; b < mc; b += nwarp) {
-            const int cb = rel[b] * r;
-            for (int a = b + lane; a < mc; a += 32) F[rel[a] + cb] += Uc[a + (int64_t)b * mc];
+            double* cb = colp(rel[b]);
+            const double* ub = Uc + (int64_t)b * mc;
+            for (int a = b + lane; a < mc; a += 32) cb[rel[a]] += __ldcg(ub + a);
         }
     }
     __syncthreads();
-    // 4. partial Cholesky of the first w columns, right-looking (Eq. 21)
-    for (int j = 0; j < w; ++j) {
-        double* Fj = F + j * r;
-        const double d = Fj[j];
-        const bool bad = bad_pivot(d);
-        const double dj = bad ? 1.0 : sqrt(d);
-        __syncthreads();
-        if (tid == 0) { Fj[j] = dj; if (bad) atomicMin(D.fail_col, c0 + j); }
-        for (int i = j + 1 + tid; i < r; i += NT) Fj[i] /= dj;
-        __syncthreads();
-        for (int c = j + 1 + warp; c < r; c += nwarp) {
-            const double lc = Fj[c];
-            double* Fc = F + c * r;
-            for (int i = c + lane; i < r; i += 32) Fc[i] -= Fj[i] * lc;
-        }
-        __syncthreads();
+    partial_chol(colp, r, w, c0, D.fail_col);
+    const int ld = ld_even(r), m = r - w;
+    double* P = D.L + D.panel_ptr[s];
+    for (int j = warp; j < w; j += nwarp) {
+        const double* cj = colp(j);
+        for (int i = j + lane; i < r; i += 32) P[i + (int64_t)j * ld] = cj[i];
     }
-    // 5. write the panel of L and the update matrix
-    double* __restrict__ P = D.L + D.panel_ptr[s];
-    for (int j = warp; j < w; j += nwarp)
-        for (int i = j + lane; i < r; i += 32) P[i + (int64_t)j * r] = F[i + j * r];
-    const int m = r - w;
-    double* __restrict__ Uo = D.U + D.upd_ptr[s];
-    for (int j = warp; j < m; j += nwarp)
-        for (int i = j + lane; i < m; i += 32) Uo[i + (int64_t)j * m] = F[(i + w) + (j + w) * r];
+    double* Uo = D.U + D.upd_ptr[s];
+    for (int j = warp; j < m; j += nwarp) {
+        const double* cj = colp(j + w) + w;
+        for (int i = j + lane; i < m; i += 32) Uo[i + (int64_t)j * m] = cj[i];
+    }
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) red_release_add(front_done + s, 1u);
 }
 
 // =============================================================================================================
-// big fronts: tiled path in global memory
+// task type 1: tile (I,J) of a tiled front, left-looking
 // =============================================================================================================
-// item = (sn, c_lo, c_hi, -): this CTA owns front columns [c_lo, c_hi): zero, K entries, children, all in order.
-__global__ void __launch_bounds__(NT) big_assemble_kernel(DevSym D, const BigItem* __restrict__ items,
-                                                          const double* __restrict__ Kval) {
-    const double eta = *D.eta;
-    const BigItem it = items[blockIdx.x];
-    const int s = it.sn, c_lo = it.a, c_hi = it.b;
-    const FrontView F = front_view(D, s);
+__device__ __forceinline__ void tile_task(const DevSym& D, const FactorPlan& F, int s, int I, int J, const double* __restrict__ Kval,
+                                          double eta, double* sm) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = NT / 32;
-    for (int c = c_lo + warp; c < c_hi; c += nwarp)
-        for (int i = c + lane; i < F.r; i += 32) *F.at(i, c) = 0.0;
+    const int gid = lane >> 2, tig = lane & 3, wm = warp >> 1, wn = warp & 1;
+    const int c0 = D.sn_start[s], w = D.sn_start[s + 1] - c0;
+    const int r = (int)(D.rows_ptr[s + 1] - D.rows_ptr[s]), ld = ld_even(r), m = r - w;
+    const int nbp = tile_nbp(w), nbt = nbp + tile_nbu(w, r);
+    const int i0 = tile_bound(I, w, r, nbp), i1 = tile_bound(I + 1, w, r, nbp), ni = i1 - i0;
+    const int j0 = tile_bound(J, w, r, nbp), j1 = tile_bound(J + 1, w, r, nbp), nj = j1 - j0;
+    const int ia = i0 & ~1, ja = j0 & ~1, di = i0 - ia, dj = j0 - ja;
+    double* P = D.L + D.panel_ptr[s];
+    uint32_t* front_done = F.sync + 1;
+    uint32_t* tdone = F.sync + 1 + D.ns + F.tbase[s];
+    const int Kend = (J < nbp) ? j0 : w;
+    double* pipe = sm;
+    double* Cs = sm + PIPE_DOUBLES;
+
+    // ---- 1. acc = sum_{k < Kend} X(I,k) X(J,k)^T ----
+    double acc[2][4][2];
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
+    const int nch = (Kend + KC - 1) / KC;
+    auto wait_flags = [&](int c) {                       // thread 0: the 64-column block that chunk c starts must be finished
+        if (tid == 0 && c < nch && ((c * KC) & (TILE - 1)) == 0) {
+            const int kb = (c * KC) / TILE;
+            spin_until_ge(tdone + kb * nbt + I, 1u);
+            if (J != I) spin_until_ge(tdone + kb * nbt + J, 1u);
+        }
+    };
+    auto issue = [&](int c) {
+        if (c < nch) {
+            const int kc = c * KC;
+            double* st = pipe + (c % NSTAGE) * STAGE_DOUBLES;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int p = tid + NT * q;
+                const int op = p >> 9, rem = p & 511, kk = rem >> 5, seg = rem & 31;
+                const int k = kc + kk;
+                const int kcl = k < Kend ? k : Kend - 1;
+                const double* src = P + (op ? ja : ia) + 2 * seg + (int64_t)kcl * ld;
+                cp_async16(st + op * (KC * ALD) + kk * ALD + 2 * seg, src, k < Kend ? 16 : 0);
+            }
+        }
+        cp_async_commit();
+    };
+    wait_flags(0);
+    wait_flags(1);
     __syncthreads();
-    if (c_lo < F.w) {
-        // K entries are sorted by column: binary search the first entry with column >= c_lo and >= c_hi
-        const int64_t q0 = D.kent_ptr[s], q1 = D.kent_ptr[s + 1];
-        auto lower = [&](int col) {
-            int64_t a = q0, b = q1;
-            while (a < b) { int64_t mid = (a + b) >> 1; if (D.kent_dst[mid] / F.r < col) a = mid + 1; else b = mid; }
-            return a;
-        };
-        const int64_t qa = lower(c_lo), qb = lower(c_hi);
-        for (int64_t q = qa + tid; q < qb; q += NT) F.P[D.kent_dst[q]] = Kval[D.kent_src[q]];
+    issue(0);
+    issue(1);
+    for (int c = 0; c < nch; ++c) {
+        wait_flags(c + 2);
+        cp_async_wait<1>();
         __syncthreads();
-        if (eta != 0.0) for (int j = c_lo + tid; j < c_hi && j < F.w; j += NT) F.P[j + (int64_t)j * F.r] += eta;
+        issue(c + 2);
+        const double* As = pipe + (c % NSTAGE) * STAGE_DOUBLES + wm * 16 + gid + di;
+        const double* Bs = pipe + (c % NSTAGE) * STAGE_DOUBLES + KC * ALD + wn * 32 + gid + dj;
+#pragma unroll
+        for (int ks = 0; ks < KC; ks += 4) {
+            double a[2], b[4];
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt) a[mt] = As[(ks + tig) * ALD + mt * 8];
+#pragma unroll
+            for (int nt = 0; nt < 4; ++nt) b[nt] = Bs[(ks + tig) * ALD + nt * 8];
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+                for (int nt = 0; nt < 4; ++nt) dmma(acc[mt][nt], a[mt], b[nt]);
+        }
     }
-    for (int ci = D.child_ptr[s]; ci < D.child_ptr[s + 1]; ++ci) {
+    cp_async_wait<0>();
+
+    // ---- 2. assemble the tile: zero, K entries, eta, children's update matrices (fixed child order) ----
+    for (int idx = tid; idx < CT_DOUBLES; idx += NT) Cs[idx] = 0.0;
+    const int ch0 = D.child_ptr[s], ch1 = D.child_ptr[s + 1];
+    if (J == 0) {                                        // tiles with J > 0 inherit this through the flag of tile (I,0)
+        for (int ci = ch0 + tid; ci < ch1; ci += NT) { const int c = D.child_idx[ci]; spin_until_ge(front_done + c, F.target[c]); }
+    }
+    __syncthreads();
+    if (J < nbp) {
+        const int64_t q0 = F.tile_kptr[F.tbase[s] + J * nbt + I], q1 = F.tile_kptr[F.tbase[s] + J * nbt + I + 1];
+        for (int64_t q = q0 + tid; q < q1; q += NT) Cs[D.kent_dst[q]] = Kval[D.kent_src[q]];
+        __syncthreads();
+        if (I == J && eta != 0.0) for (int nn = tid; nn < nj; nn += NT) Cs[nn * CLD + nn] += eta;
+    }
+    for (int ci = ch0; ci < ch1; ++ci) {
         const int c = D.child_idx[ci];
+        const int32_t* cb = F.cbnd + F.cb_ptr[c];
+        const int a0 = cb[I], a1 = cb[I + 1], b0 = cb[J], b1 = cb[J + 1];
+        if (a0 == a1 || b0 == b1) continue;              // uniform over the CTA
         const int mc = (int)(D.rel_ptr[c + 1] - D.rel_ptr[c]);
-        const double* __restrict__ Uc = D.U + D.upd_ptr[c];
+        const double* Uc = D.U + D.upd_ptr[c];
         const int32_t* __restrict__ rel = D.rel + D.rel_ptr[c];
-        auto lower = [&](int col) { int a = 0, b = mc; while (a < b) { int mid = (a + b) >> 1; if (rel[mid] < col) a = mid + 1; else b = mid; } return a; };
-        const int b0 = lower(c_lo), b1 = lower(c_hi);
         __syncthreads();
         for (int b = b0 + warp; b < b1; b += nwarp) {
-            const int cb = rel[b];
-            for (int a = b + lane; a < mc; a += 32) *F.at(rel[a], cb) += Uc[a + (int64_t)b * mc];
+            double* cc = Cs + (rel[b] - j0) * CLD - i0;
+            const double* ub = Uc + (int64_t)b * mc;
+            for (int a = max(a0, b) + lane; a < a1; a += 32) cc[rel[a]] += __ldcg(ub + a);
         }
-    }
-}
-
-// item = (sn, j0): Cholesky of the diagonal block [j0, j0+nb) of the panel, one CTA.
-__global__ void __launch_bounds__(NT) big_potrf_kernel(DevSym D, const BigItem* __restrict__ items) {
-    __shared__ double A[BIG_NB][BIG_NB + 1];
-    const BigItem it = items[blockIdx.x];
-    const FrontView F = front_view(D, it.sn);
-    const int j0 = it.a, nb = min(BIG_NB, F.w - j0);
-    const int tid = threadIdx.x;
-    const int c0 = D.sn_start[it.sn];
-    for (int idx = tid; idx < nb * nb; idx += NT) {
-        const int i = idx % nb, c = idx / nb;
-        A[i][c] = (i >= c) ? F.P[(j0 + i) + (int64_t)(j0 + c) * F.r] : 0.0;
     }
     __syncthreads();
-    for (int j = 0; j < nb; ++j) {
-        const double d = A[j][j];
-        const bool bad = bad_pivot(d);
-        const double dj = bad ? 1.0 : sqrt(d);
-        __syncthreads();
-        if (tid == 0) { A[j][j] = dj; if (bad) atomicMin(D.fail_col, c0 + j0 + j); }
-        for (int i = j + 1 + tid; i < nb; i += NT) A[i][j] /= dj;
-        __syncthreads();
-        for (int idx = tid; idx < (nb - j - 1) * (nb - j - 1); idx += NT) {
-            const int i = j + 1 + idx % (nb - j - 1), c = j + 1 + idx / (nb - j - 1);
-            if (i >= c) A[i][c] -= A[i][j] * A[c][j];
-        }
-        __syncthreads();
-    }
-    for (int idx = tid; idx < nb * nb; idx += NT) {
-        const int i = idx % nb, c = idx / nb;
-        if (i >= c) F.P[(j0 + i) + (int64_t)(j0 + c) * F.r] = A[i][c];
-    }
-}
-
-// item = (sn, j0, i0): X = A D^-T for the 64-row tile starting at front row i0 of block column j0.
-__global__ void __launch_bounds__(NT) big_trsm_kernel(DevSym D, const BigItem* __restrict__ items) {
-    extern __shared__ double sm[];
-    double (*Dg)[BIG_NB + 1] = reinterpret_cast<double (*)[BIG_NB + 1]>(sm);
-    double (*X)[BIG_NB + 1] = reinterpret_cast<double (*)[BIG_NB + 1]>(sm + BIG_NB * (BIG_NB + 1));   // X[c][i]: column c of the tile
-    const BigItem it = items[blockIdx.x];
-    const FrontView F = front_view(D, it.sn);
-    const int j0 = it.a, i0 = it.b, nb = min(BIG_NB, F.w - j0), nr = min(BIG_NB, F.r - i0);
-    const int tid = threadIdx.x;
-    for (int idx = tid; idx < nb * nb; idx += NT) {
-        const int i = idx % nb, c = idx / nb;
-        Dg[i][c] = (i >= c) ? F.P[(j0 + i) + (int64_t)(j0 + c) * F.r] : 0.0;
-    }
-    for (int idx = tid; idx < nr * nb; idx += NT) {
-        const int i = idx % nr, c = idx / nr;
-        X[c][i] = F.P[(i0 + i) + (int64_t)(j0 + c) * F.r];
-    }
+#pragma unroll
+    for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+        for (int nt = 0; nt < 4; ++nt)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) Cs[(wn * 32 + nt * 8 + 2 * tig + e) * CLD + wm * 16 + mt * 8 + gid] -= acc[mt][nt][e];
     __syncthreads();
-    for (int c = 0; c < nb; ++c) {
-        const double dc = Dg[c][c];
-        for (int i = tid; i < nr; i += NT) X[c][i] /= dc;
-        __syncthreads();
-        for (int idx = tid; idx < nr * (nb - c - 1); idx += NT) {
-            const int i = idx % nr, k = c + 1 + idx / nr;
-            X[k][i] -= X[c][i] * Dg[k][c];
-        }
-        __syncthreads();
-    }
-    for (int idx = tid; idx < nr * nb; idx += NT) {
-        const int i = idx % nr, c = idx / nr;
-        F.P[(i0 + i) + (int64_t)(j0 + c) * F.r] = X[c][i];
-    }
-}
 
-// item = (sn, j0, I0, J0): C[I0.., J0..] -= X[I0.., :] X[J0.., :]^T on the lower triangle, X = block column j0 of the panel.
-__global__ void __launch_bounds__(NT) big_syrk_kernel(DevSym D, const BigItem* __restrict__ items) {
-    extern __shared__ double sm[];
-    double (*XI)[BIG_NB] = reinterpret_cast<double (*)[BIG_NB]>(sm);                       // [k][i]
-    double (*XJ)[BIG_NB] = reinterpret_cast<double (*)[BIG_NB]>(sm + BIG_NB * BIG_NB);
-    const BigItem it = items[blockIdx.x];
-    const FrontView F = front_view(D, it.sn);
-    const int j0 = it.a, I0 = it.b, J0 = it.c;
-    const int nb = min(BIG_NB, F.w - j0), ni = min(BIG_NB, F.r - I0), nj = min(BIG_NB, F.r - J0);
-    const int tid = threadIdx.x;
-    for (int idx = tid; idx < BIG_NB * nb; idx += NT) {
-        const int i = idx % BIG_NB, k = idx / BIG_NB;
-        XI[k][i] = (i < ni) ? F.P[(I0 + i) + (int64_t)(j0 + k) * F.r] : 0.0;
-        XJ[k][i] = (i < nj) ? F.P[(J0 + i) + (int64_t)(j0 + k) * F.r] : 0.0;
-    }
-    __syncthreads();
-    const int tx = tid & 15, ty = tid >> 4;         // thread computes rows ty*4.., cols tx*4..
-    double acc[4][4];
-#pragma unroll
-    for (int a = 0; a < 4; ++a)
-#pragma unroll
-        for (int b = 0; b < 4; ++b) acc[a][b] = 0.0;
-    for (int k = 0; k < nb; ++k) {
-        double av[4], bv[4];
-#pragma unroll
-        for (int a = 0; a < 4; ++a) { av[a] = XI[k][ty * 4 + a]; bv[a] = XJ[k][tx * 4 + a]; }
-#pragma unroll
-        for (int a = 0; a < 4; ++a)
-#pragma unroll
-            for (int b = 0; b < 4; ++b) acc[a][b] = fma(av[a], bv[b], acc[a][b]);
-    }
-#pragma unroll
-    for (int b = 0; b < 4; ++b) {
-        const int c = J0 + tx * 4 + b;
-        if (tx * 4 + b >= nj) continue;
-#pragma unroll
-        for (int a = 0; a < 4; ++a) {
-            const int i = I0 + ty * 4 + a;
-            if (ty * 4 + a < ni && i >= c) *F.at(i, c) -= acc[a][b];
-        }
-    }
-}
-
-// =============================================================================================================
-// triangular solves, one CTA per supernode, levels leaves->root (forward) and root->leaves (backward)
-// =============================================================================================================
-// forward (Eq. 23): t = [x[cols]; 0] + sum_children extend(ctr_child);  L11 y = t1;  t2 -= L21 y;  x[cols] = y; ctr = t2
-__global__ void __launch_bounds__(NT) solve_fwd_kernel(DevSym D, const int32_t* __restrict__ sn_list, double* __restrict__ x) {
-    extern __shared__ double sm[];
-    double* t = sm;                                  // r
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int s = sn_list[blockIdx.x];
-    const int c0 = D.sn_start[s], w = D.sn_start[s + 1] - c0;
-    const int r = (int)(D.rows_ptr[s + 1] - D.rows_ptr[s]);
-    double (*Ld)[BIG_NB + 1] = reinterpret_cast<double (*)[BIG_NB + 1]>(sm + ((r + 1) & ~1));
-    const double* __restrict__ P = D.L + D.panel_ptr[s];
-    for (int i = tid; i < r; i += NT) t[i] = (i < w) ? x[c0 + i] : 0.0;
-    for (int ci = D.child_ptr[s]; ci < D.child_ptr[s + 1]; ++ci) {
-        const int c = D.child_idx[ci];
-        const int mc = (int)(D.rel_ptr[c + 1] - D.rel_ptr[c]);
-        const double* __restrict__ cc = D.ctr + D.rel_ptr[c];
-        const int32_t* __restrict__ rel = D.rel + D.rel_ptr[c];
-        __syncthreads();
-        for (int a = tid; a < mc; a += NT) t[rel[a]] += cc[a];
-    }
-    __syncthreads();
-    for (int j0 = 0; j0 < w; j0 += BIG_NB) {
-        const int nb = min(BIG_NB, w - j0);
-        for (int idx = tid; idx < nb * nb; idx += NT) {
-            const int i = idx % nb, c = idx / nb;
-            if (i >= c) Ld[i][c] = P[(j0 + i) + (int64_t)(j0 + c) * r];
-        }
-        __syncthreads();
-        if (warp == 0) {                             // one warp: in-block forward substitution, no block barriers
-            for (int j = 0; j < nb; ++j) {
-                const double v = t[j0 + j] / Ld[j][j];
-                __syncwarp();
-                if (lane == 0) t[j0 + j] = v;
-                for (int i = j + 1 + lane; i < nb; i += 32) t[j0 + i] -= Ld[i][j] * v;
-                __syncwarp();
+    // ---- 3. finish: POTRF / TRSM for panel tiles, then store (each tile is written once) ----
+    if (J < nbp) {
+        if (I == J) {
+            partial_chol([Cs](int j) { return Cs + j * CLD; }, nj, nj, c0 + j0, D.fail_col);
+        } else {
+            double* Ls = pipe;
+            double* rinv = pipe + CT_DOUBLES;
+            if (tid == 0) spin_until_ge(tdone + J * nbt + J, 1u);
+            __syncthreads();
+            for (int idx = tid; idx < nj * nj; idx += NT) {
+                const int ii = idx % nj, cc = idx / nj;
+                if (ii >= cc) {
+                    const double v = __ldcg(P + (j0 + ii) + (int64_t)(j0 + cc) * ld);
+                    Ls[cc * CLD + ii] = v;
+                    if (ii == cc) rinv[cc] = 1.0 / v;
+                }
             }
+            __syncthreads();
+            trsm_tile(Cs, Ls, rinv, ni, nj);
         }
-        __syncthreads();
-        // rows below the block: t[i] -= sum_k L[i, j0+k] y[k]
-        for (int i = j0 + nb + tid; i < r; i += NT) {
-            double acc = 0.0;
-            const double* __restrict__ Pi = P + i + (int64_t)j0 * r;
-            for (int k = 0; k < nb; ++k) acc = fma(Pi[(int64_t)k * r], t[j0 + k], acc);
-            t[i] -= acc;
+        for (int idx = tid; idx < ni * nj; idx += NT) {
+            const int mm = idx % ni, nn = idx / ni;
+            if (I != J || mm >= nn) P[(i0 + mm) + (int64_t)(j0 + nn) * ld] = Cs[nn * CLD + mm];
         }
+        __threadfence();
         __syncthreads();
+        if (tid == 0) { st_release(tdone + J * nbt + I, 1u); red_release_add(front_done + s, 1u); }
+    } else {
+        double* Uo = D.U + D.upd_ptr[s];
+        for (int idx = tid; idx < ni * nj; idx += NT) {
+            const int mm = idx % ni, nn = idx / ni;
+            if (I != J || mm >= nn) Uo[(i0 + mm - w) + (int64_t)(j0 + nn - w) * m] = Cs[nn * CLD + mm];
+        }
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) red_release_add(front_done + s, 1u);
     }
-    for (int i = tid; i < w; i += NT) x[c0 + i] = t[i];
-    double* __restrict__ co = D.ctr + D.rel_ptr[s];
-    for (int i = w + tid; i < r; i += NT) co[i - w] = t[i];
 }
 
-// backward (Eq. 24): t2 = x[rows below];  L11^T z = y - L21^T t2;  x[cols] = z
-__global__ void __launch_bounds__(NT) solve_bwd_kernel(DevSym D, const int32_t* __restrict__ sn_list, double* __restrict__ x) {
-    extern __shared__ double sm[];
-    double* t = sm;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = NT / 32;
-    const int s = sn_list[blockIdx.x];
-    const int c0 = D.sn_start[s], w = D.sn_start[s + 1] - c0;
-    const int r = (int)(D.rows_ptr[s + 1] - D.rows_ptr[s]);
-    double (*Ld)[BIG_NB + 1] = reinterpret_cast<double (*)[BIG_NB + 1]>(sm + ((r + 1) & ~1));
-    const double* __restrict__ P = D.L + D.panel_ptr[s];
-    const int32_t* __restrict__ rows = D.rows + D.rows_ptr[s];
-    for (int i = tid; i < r; i += NT) t[i] = x[rows[i]];
-    __syncthreads();
-    const int nblk = (w + BIG_NB - 1) / BIG_NB;
-    for (int bk = nblk - 1; bk >= 0; --bk) {
-        const int j0 = bk * BIG_NB, nb = min(BIG_NB, w - j0);
-        for (int idx = tid; idx < nb * nb; idx += NT) {
-            const int i = idx % nb, c = idx / nb;
-            if (i >= c) Ld[i][c] = P[(j0 + i) + (int64_t)(j0 + c) * r];
-        }
-        // t[j] -= sum_{i >= j0+nb} L[i,j] t[i] : one warp per column, lanes over rows (coalesced), fixed shuffle tree
-        for (int j = warp; j < nb; j += nwarp) {
-            const double* __restrict__ Pj = P + (int64_t)(j0 + j) * r;
-            double acc = 0.0;
-            for (int i = j0 + nb + lane; i < r; i += 32) acc = fma(Pj[i], t[i], acc);
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-            if (lane == 0) t[j0 + j] -= acc;
-        }
+__global__ void __launch_bounds__(NT, 2) factor_dag_kernel(DevSym D, FactorPlan F, const double* __restrict__ Kval) {
+    extern __shared__ __align__(16) double sm[];
+    __shared__ int s_task;
+    const double eta = *D.eta;
+    while (true) {
         __syncthreads();
-        if (warp == 0) {                             // in-block backward substitution with L11^T
-            for (int j = nb - 1; j >= 0; --j) {
-                const double v = t[j0 + j] / Ld[j][j];
-                __syncwarp();
-                if (lane == 0) t[j0 + j] = v;
-                for (int i = lane; i < j; i += 32) t[j0 + i] -= Ld[j][i] * v;
-                __syncwarp();
-            }
-        }
+        if (threadIdx.x == 0) s_task = (int)atomicAdd(F.sync, 1u);
         __syncthreads();
+        const int t = s_task;
+        if (t >= F.ntasks) break;
+        const int4 tk = F.tasks[t];
+        if (tk.x == 0) small_front_task(D, F, tk.y, Kval, eta, sm);
+        else tile_task(D, F, tk.y, tk.z, tk.w, Kval, eta, sm);
     }
-    for (int i = tid; i < w; i += NT) x[c0 + i] = t[i];
 }
 
-__global__ void permute_in_kernel(int64_t n, const int32_t* __restrict__ perm, const double* __restrict__ b, double* __restrict__ x) {
-    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (i < n) x[i] = b[perm[i]];
+// fail_col = INT_MAX, *eta_dev = eta, all completion flags and the task counter = 0
+__global__ void __launch_bounds__(NT) factor_reset_kernel(int32_t* fail_col, double* eta_dev, double eta, uint32_t* sync, int words) {
+    const int i = blockIdx.x * NT + threadIdx.x;
+    if (i == 0) { *fail_col = INT_MAX; *eta_dev = eta; }
+    for (int k = i; k < words; k += gridDim.x * NT) sync[k] = 0u;
 }
-__global__ void permute_out_kernel(int64_t n, const int32_t* __restrict__ perm, const double* __restrict__ x, double* __restrict__ b) {
-    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (i < n) b[perm[i]] = x[i];
-}
-__global__ void reset_flag_kernel(int32_t* f, double* eta_dev, double eta) { *f = INT_MAX; *eta_dev = eta; }
 
 }  // namespace
 
-constexpr size_t TRSM_SMEM = 2 * BIG_NB * (BIG_NB + 1) * sizeof(double);
-constexpr size_t SYRK_SMEM = 2 * BIG_NB * BIG_NB * sizeof(double);
-size_t small_front_smem_bytes(int max_r) { return (size_t)max_r * max_r * sizeof(double); }
-static size_t solve_smem_bytes(int max_r) { return ((size_t)((max_r + 1) & ~1) + (size_t)BIG_NB * (BIG_NB + 1)) * sizeof(double); }
+cudaError_t configure_factor_kernels(int max_smem_bytes, int* ctas_per_sm, size_t* smem_bytes, int* small_max_r) {
+    // two CTAs per SM: half of the SM's shared memory each (minus the 1 KB per-CTA reservation), at least the tile layout
+    size_t bytes = (size_t)TILE_SMEM_DOUBLES * sizeof(double);
+    const size_t half = ((size_t)max_smem_bytes + 1024) / 2 - 1024 - 64;
+    if (half > bytes) bytes = half & ~(size_t)15;
+    if (bytes > (size_t)max_smem_bytes) return cudaErrorInvalidValue;
+    cudaError_t e = cudaFuncSetAttribute(factor_dag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e != cudaSuccess) return e;
+    int occ = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, factor_dag_kernel, NT, bytes);
+    if (e != cudaSuccess) return e;
+    *ctas_per_sm = occ < 1 ? 1 : occ;
+    *smem_bytes = bytes;
+    int rmax = 1;                                        // largest r with r(r+1)/2 doubles in `bytes`, and r <= NT
+    while (rmax < NT && (size_t)(rmax + 1) * (rmax + 2) / 2 * sizeof(double) <= bytes) ++rmax;
+    *small_max_r = rmax;
+    return cudaSuccess;
+}
 
-cudaError_t configure_factor_kernels(int max_smem_bytes) {
-    cudaError_t e = cudaFuncSetAttribute(front_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(big_trsm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TRSM_SMEM);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(big_syrk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SYRK_SMEM);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(solve_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(solve_bwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes);
+void launch_factor(const DevSym& D, const FactorPlan& F, const double* Kval, double* eta_dev, double eta, cudaStream_t st) {
+    const int rb = (F.sync_words + NT - 1) / NT;
+    factor_reset_kernel<<<rb < 64 ? (rb < 1 ? 1 : rb) : 64, NT, 0, st>>>(D.fail_col, eta_dev, eta, F.sync, F.sync_words);
+    if (F.ntasks > 0) factor_dag_kernel<<<F.grid, NT, F.smem_bytes, st>>>(D, F, Kval);
 }
-
-void launch_front_small(const DevSym& D, const int32_t* sn_list, int count, int max_r, const double* Kval, cudaStream_t st) {
-    if (count > 0) front_small_kernel<<<count, NT, small_front_smem_bytes(max_r), st>>>(D, sn_list, Kval);
-}
-void launch_big_assemble(const DevSym& D, const BigItem* items, int count, const double* Kval, cudaStream_t st) {
-    if (count > 0) big_assemble_kernel<<<count, NT, 0, st>>>(D, items, Kval);
-}
-void launch_big_potrf(const DevSym& D, const BigItem* items, int count, cudaStream_t st) {
-    if (count > 0) big_potrf_kernel<<<count, NT, 0, st>>>(D, items);
-}
-void launch_big_trsm(const DevSym& D, const BigItem* items, int count, cudaStream_t st) {
-    if (count > 0) big_trsm_kernel<<<count, NT, TRSM_SMEM, st>>>(D, items);
-}
-void launch_big_syrk(const DevSym& D, const BigItem* items, int count, cudaStream_t st) {
-    if (count > 0) big_syrk_kernel<<<count, NT, SYRK_SMEM, st>>>(D, items);
-}
-void launch_solve_fwd(const DevSym& D, const int32_t* sn_list, int count, int max_r, double* x, cudaStream_t st) {
-    if (count > 0) solve_fwd_kernel<<<count, NT, solve_smem_bytes(max_r), st>>>(D, sn_list, x);
-}
-void launch_solve_bwd(const DevSym& D, const int32_t* sn_list, int count, int max_r, double* x, cudaStream_t st) {
-    if (count > 0) solve_bwd_kernel<<<count, NT, solve_smem_bytes(max_r), st>>>(D, sn_list, x);
-}
-void launch_permute_in(const DevSym& D, const double* b, double* x, cudaStream_t st) {
-    permute_in_kernel<<<(unsigned)((D.n + 255) / 256), 256, 0, st>>>(D.n, D.perm, b, x);
-}
-void launch_permute_out(const DevSym& D, const double* x, double* b, cudaStream_t st) {
-    permute_out_kernel<<<(unsigned)((D.n + 255) / 256), 256, 0, st>>>(D.n, D.perm, x, b);
-}
-void launch_reset_flag(const DevSym& D, double* eta_dev, double eta, cudaStream_t st) { reset_flag_kernel<<<1, 1, 0, st>>>(D.fail_col, eta_dev, eta); }
 
 }  // namespace nmpc

@@ -656,13 +656,13 @@ nmpc_status analyze_symbolic(const nmpc_pattern* pattern, const nmpc_ocp* ocp, c
     S.nnzL = 0; S.max_front = 0; S.max_width = 0;
     for (int32_t s = 0; s < ns; ++s) {
         int64_t r = S.rows_ptr[s + 1] - S.rows_ptr[s], w = S.sn_start[s + 1] - S.sn_start[s];
-        S.panel_ptr[s + 1] = S.panel_ptr[s] + r * w;
+        S.panel_ptr[s + 1] = S.panel_ptr[s] + panel_ld(r) * w;
         S.upd_ptr[s + 1] = S.upd_ptr[s] + (r - w) * (r - w);
         S.rel_ptr[s + 1] = S.rel_ptr[s] + (r - w);
         S.nnzL += panel_nnz(r, w);
         S.max_front = std::max<int32_t>(S.max_front, (int32_t)r);
         S.max_width = std::max<int32_t>(S.max_width, (int32_t)w);
-        if (r * w > INT32_MAX) { S.error = "panel too large for int32 offsets"; return NMPC_E_ALLOC; }
+        if (panel_ld(r) * w > INT32_MAX || r > 65535) { S.error = "front too large (panel offsets are int32, front rows uint16)"; return NMPC_E_ALLOC; }
     }
     S.rel.assign(S.rel_ptr[ns], 0);
     for (int32_t s = 0; s < ns; ++s) {
@@ -681,7 +681,7 @@ nmpc_status analyze_symbolic(const nmpc_pattern* pattern, const nmpc_ocp* ocp, c
         int64_t q = 0;
         for (int32_t s = 0; s < ns; ++s) {
             const int32_t c0 = S.sn_start[s], c1 = S.sn_start[s + 1];
-            const int64_t r = S.rows_ptr[s + 1] - S.rows_ptr[s];
+            const int64_t r = S.rows_ptr[s + 1] - S.rows_ptr[s], ld = panel_ld(r);
             const int32_t* rw = &S.rows[S.rows_ptr[s]];
             for (int32_t j = c0; j < c1; ++j) {
                 int64_t pos = 0;
@@ -690,7 +690,7 @@ nmpc_status analyze_symbolic(const nmpc_pattern* pattern, const nmpc_ocp* ocp, c
                     while (pos < r && rw[pos] < i) ++pos;
                     if (pos == r || rw[pos] != i) { S.error = "internal: K entry outside the supernode structure"; return NMPC_E_ARG; }
                     S.kent_src[q] = B.csrc[p];
-                    S.kent_dst[q] = (int32_t)(pos + (int64_t)(j - c0) * r);
+                    S.kent_dst[q] = (int32_t)(pos + (int64_t)(j - c0) * ld);
                     ++q;
                 }
             }

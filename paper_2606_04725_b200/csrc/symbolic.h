@@ -11,6 +11,10 @@
 
 namespace nmpc {
 
+// Leading dimension of the column-major r x w panel of a supernode: r rounded up to even, so that every column (and every
+// even row offset) is 16-byte aligned for the vector / cp.async loads of the tile kernels.
+inline int64_t panel_ld(int64_t r) { return (r + 1) & ~(int64_t)1; }
+
 struct Csr {                       // generic int pattern, row-major
     int64_t nrows = 0, ncols = 0;
     std::vector<int64_t> ptr;
@@ -50,10 +54,10 @@ struct Symbolic {
     std::vector<int32_t> child_ptr, child_idx;     // children of each supernode, increasing index
     std::vector<int64_t> rel_ptr;       // ns+1 into rel: for supernode s, (r_s - w_s) positions in rows[parent]
     std::vector<int32_t> rel;
-    std::vector<int64_t> panel_ptr, upd_ptr;       // ns+1: offsets (doubles) of the r x w panel / (r-w)^2 update
+    std::vector<int64_t> panel_ptr, upd_ptr;       // ns+1: offsets (doubles) of the panel_ld(r) x w panel / (r-w)^2 update
     std::vector<int64_t> kent_ptr;      // ns+1: K entries landing in each supernode's panel
     std::vector<int32_t> kent_src;      // K value index
-    std::vector<int32_t> kent_dst;      // i + j*r inside the panel
+    std::vector<int32_t> kent_dst;      // i + j*panel_ld(r) inside the panel
     int32_t nlevels = 0;
     std::vector<int32_t> lvl_ptr, lvl_sn;
     double flops = 0.0;

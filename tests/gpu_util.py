@@ -26,8 +26,9 @@ def factor_as_sparse(info, panels):
         c0, c1 = int(info["super_start"][s]), int(info["super_start"][s + 1])
         rows = info["rows"][info["rows_ptr"][s]:info["rows_ptr"][s + 1]].astype(np.int64)
         r, w = len(rows), c1 - c0
-        P = panels[off:off + r * w].reshape(w, r).T          # P[i, j]
-        off += r * w
+        ld = (r + 1) & ~1                                    # panel leading dimension: r rounded up to even (include/nmpc.h)
+        P = panels[off:off + ld * w].reshape(w, ld).T[:r]    # P[i, j]
+        off += ld * w
         for j in range(w):
             rows_all.append(rows[j:])
             cols_all.append(np.full(r - j, c0 + j, dtype=np.int64))
