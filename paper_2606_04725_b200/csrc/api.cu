@@ -1,5 +1,5 @@
-// api.cu -- the C-ABI of include/nmpc.h: handle life cycle, level schedule, CUDA-graph capture of the factor and
-// solve launch sequences, and the host side of Algorithm 2 (LiftedIPM) / Algorithm 1 lines 9-11.
+// api.cu -- the C-ABI of include/nmpc.h: handle life cycle, task lists of the persistent factor / solve kernels, and the
+// host side of Algorithm 2 (LiftedIPM) / Algorithm 1 lines 9-11.
 // Every numeric step runs in the kernels of factor.cu / ipm.cu; the host only sequences launches and takes the
 // scalar decisions (barrier update, inertia schedule, termination) from a handful of reduced scalars.
 #include <algorithm>
@@ -22,10 +22,6 @@ extern "C" nmpc_status nmpc_copy_pattern_internal(const nmpc::Csr& P, int64_t* n
 
 namespace {
 
-struct LevelPlan {
-    int all_off = 0, all_cnt = 0, all_max_r = 0;           // every supernode of the level (solves), into d_lvl_sn
-};
-
 }  // namespace
 
 struct nmpc_handle_s {
@@ -37,19 +33,15 @@ struct nmpc_handle_s {
     DevModel M;
     IpmVectors V{};
     std::vector<void*> allocs;
-    std::vector<LevelPlan> plan;
-    int32_t* d_lvl_sn = nullptr;
-    FactorPlan F;
+    DagPlan F;
+    uint32_t epoch_f = 0, epoch_s = 0, epoch_limit = 1u << 16;    // call numbers of the epoch-valued completion flags
     int n_big_fronts = 0;
-    double* d_eta = nullptr;
     double* d_Kval = nullptr;          // values last factored (pattern order)
     double* d_x = nullptr;             // permuted right-hand side / solution
     int64_t* d_full_ptr = nullptr; int32_t* d_full_idx = nullptr; int32_t* d_full_src = nullptr;   // symmetric CSR of K
     double* d_uinit = nullptr;
     double* h_pinned = nullptr;        // pinned host scratch: [0..15] scalars, [16] flag, staging for host-buffer calls
     size_t pinned_doubles = 0;
-    cudaGraphExec_t g_fwdbwd = nullptr;
-    int g_fwdbwd_nodes = 0;
     bool factored = false, have_state = false, has_model = false;
     double eta_cur = 0.0;
     int64_t launches = 0;
@@ -94,20 +86,14 @@ nmpc_status dalloc(nmpc_handle_s* h, size_t count, T** out, bool zero = true) {
 #define TRY(x) do { nmpc_status s__ = (x); if (s__ != NMPC_OK) return s__; } while (0)
 
 // ---- task list of the persistent factorization kernel + level lists of the solves ----
-nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_t smem_bytes, int num_sms) {
+nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_t smem_bytes, int solve_ctas_per_sm,
+                       size_t solve_smem, int num_sms) {
     const Symbolic& S = h->S;
     const int ns = S.ns;
-    h->plan.assign(S.nlevels, LevelPlan());
-    for (int l = 0; l < S.nlevels; ++l) {
-        LevelPlan& P = h->plan[l];
-        P.all_off = S.lvl_ptr[l]; P.all_cnt = S.lvl_ptr[l + 1] - S.lvl_ptr[l];
-        for (int q = S.lvl_ptr[l]; q < S.lvl_ptr[l + 1]; ++q)
-            P.all_max_r = std::max(P.all_max_r, (int)(S.rows_ptr[S.lvl_sn[q] + 1] - S.rows_ptr[S.lvl_sn[q]]));
-    }
     auto R = [&](int s) { return (int)(S.rows_ptr[s + 1] - S.rows_ptr[s]); };
     auto W = [&](int s) { return S.sn_start[s + 1] - S.sn_start[s]; };
-    std::vector<int32_t> cls(ns), tbase(ns, 0), target(ns, 1), nbp(ns, 0), nbt(ns, 0);
-    int64_t slots = 0;
+    std::vector<int32_t> cls(ns), tbase(ns, 0), bbase(ns, 0), target(ns, 1), target_f(ns, 1), target_b(ns, 1), nbp(ns, 0), nbt(ns, 0);
+    int64_t slots = 0, bslots = 0;
     h->n_big_fronts = 0;
     for (int s = 0; s < ns; ++s) {
         cls[s] = R(s) > small_max_r;
@@ -117,6 +103,8 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
         tbase[s] = (int32_t)slots;
         slots += (int64_t)nbp[s] * nbt[s] + 1;
         target[s] = nbt[s] * (nbt[s] + 1) / 2;
+        bbase[s] = (int32_t)bslots; bslots += nbp[s];
+        target_f[s] = nbt[s]; target_b[s] = nbp[s];
         if (slots > INT32_MAX / 2) { h->err = "too many tiles"; return NMPC_E_ALLOC; }
     }
     // K scatter map per front class: small = packed lower offset; tiled = tile-local offset, entries sorted by tile slot
@@ -195,49 +183,71 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
     std::vector<int4> tasks(tk.size());
     for (size_t t = 0; t < tk.size(); ++t) tasks[t] = make_int4(tk[t].type, tk[t].s, tk[t].I, tk[t].J);
 
-    FactorPlan& F = h->F;
-    const int32_t* ti = nullptr; const int64_t* tl = nullptr; const int4* t4 = nullptr;
-    TRY(upload(h, S.lvl_sn, &ti)); h->d_lvl_sn = const_cast<int32_t*>(ti);
-    TRY(upload(h, tasks, &t4)); F.tasks = t4; F.ntasks = (int32_t)tasks.size();
-    TRY(upload(h, cls, &F.cls)); TRY(upload(h, tbase, &F.tbase)); TRY(upload(h, target, &F.target));
+    // solve tasks: forward in descending rank (children before parents, block rows in order), backward = reversed order
+    struct SK { double rank; int32_t lvl, type, s, I; };
+    std::vector<SK> sk;
+    {
+        auto solve_time = [&](int s) { return cls[s] ? 2.0 + 4.0 * nbp[s] : 3.0; };
+        std::vector<double> rend(ns, 0.0);
+        for (int s = ns - 1; s >= 0; --s) { const int p = S.sn_parent[s]; rend[s] = p < 0 ? 0.0 : rend[p] + solve_time(p); }
+        for (int s = 0; s < ns; ++s) {
+            if (!cls[s]) { sk.push_back(SK{rend[s] + solve_time(s), S.sn_level[s], 0, s, 0}); continue; }
+            for (int I = 0; I < nbt[s]; ++I)
+                sk.push_back(SK{rend[s] + 1.0 + (I < nbp[s] ? 4.0 * (nbp[s] - I) + 1.0 : 0.0), S.sn_level[s], 1, s, I});
+        }
+        std::stable_sort(sk.begin(), sk.end(), [](const SK& a, const SK& b) {
+            if (a.rank != b.rank) return a.rank > b.rank;
+            if (a.lvl != b.lvl) return a.lvl < b.lvl;
+            if (a.s != b.s) return a.s < b.s;
+            return a.I < b.I;
+        });
+    }
+    std::vector<int4> stasks;
+    stasks.reserve(2 * sk.size());
+    for (const SK& t : sk) stasks.push_back(make_int4(t.type, t.s, t.I, 0));
+    for (size_t t = sk.size(); t-- > 0;)
+        if (sk[t].type == 0 || sk[t].I < nbp[sk[t].s]) stasks.push_back(make_int4(sk[t].type, sk[t].s, sk[t].I, 1));
+
+    DagPlan& F = h->F;
+    const int64_t* tl = nullptr; const int4* t4 = nullptr;
+    TRY(upload(h, tasks, &t4)); F.ftasks = t4; F.n_ftasks = (int32_t)tasks.size();
+    TRY(upload(h, stasks, &t4)); F.stasks = t4; F.n_stasks = (int32_t)stasks.size();
+    TRY(upload(h, cls, &F.cls)); TRY(upload(h, tbase, &F.tbase)); TRY(upload(h, bbase, &F.bbase));
+    TRY(upload(h, target, &F.target)); TRY(upload(h, target_f, &F.target_f)); TRY(upload(h, target_b, &F.target_b));
     TRY(upload(h, tile_kptr, &tl)); F.tile_kptr = tl;
     TRY(upload(h, cb_ptr, &tl)); F.cb_ptr = tl;
     TRY(upload(h, cbnd, &F.cbnd));
+    TRY(upload(h, S.sn_parent, &F.sn_parent));
     TRY(upload(h, ksrc, &h->D.kent_src)); TRY(upload(h, kdst, &h->D.kent_dst));
-    F.sync_words = (int32_t)(1 + ns + slots);
+    F.sync_words = 2 + 3 * (int64_t)ns + slots + 2 * bslots;
     TRY(dalloc(h, (size_t)F.sync_words, &F.sync));
+    F.fac_done = F.sync + 2; F.sol_done_f = F.fac_done + ns; F.sol_done_b = F.sol_done_f + ns;
+    F.tile_done = F.sol_done_b + ns; F.blk_f = F.tile_done + slots; F.blk_b = F.blk_f + bslots;
     F.small_max_r = small_max_r;
-    F.smem_bytes = smem_bytes;
-    F.grid = (int32_t)std::max<int64_t>(1, std::min<int64_t>((int64_t)tasks.size(), (int64_t)num_sms * ctas_per_sm));
+    F.fsmem = smem_bytes; F.ssmem = solve_smem;
+    F.fgrid = (int32_t)std::max<int64_t>(1, std::min<int64_t>((int64_t)tasks.size(), (int64_t)num_sms * ctas_per_sm));
+    F.sgrid = (int32_t)std::max<int64_t>(1, std::min<int64_t>((int64_t)stasks.size(), (int64_t)num_sms * solve_ctas_per_sm));
+    // epoch-valued flags: counters reach epoch * target and the claim counters epoch * (ntasks + grid); reset before 2^31
+    int64_t per_epoch = std::max<int64_t>((int64_t)tasks.size() + F.fgrid, (int64_t)stasks.size() + F.sgrid);
+    for (int s = 0; s < ns; ++s) per_epoch = std::max<int64_t>(per_epoch, target[s]);
+    h->epoch_limit = (uint32_t)std::max<int64_t>(2, ((int64_t)1 << 31) / per_epoch - 2);
     return NMPC_OK;
 }
 
-int issue_fwdbwd(nmpc_handle_s* h) {
-    int nk = 0;
-    for (size_t l = 0; l < h->plan.size(); ++l) {
-        const LevelPlan& P = h->plan[l];
-        launch_solve_fwd(h->D, h->d_lvl_sn + P.all_off, P.all_cnt, P.all_max_r, h->d_x, h->stream); ++nk;
+// the next call number of the factor / solve kernels; both restart from 1 (flags zeroed) before any counter can overflow
+nmpc_status next_epoch(nmpc_handle_s* h, bool factor, uint32_t* out) {
+    if (std::max(h->epoch_f, h->epoch_s) + 1 >= h->epoch_limit) {
+        CK(cudaMemsetAsync(h->F.sync, 0, (size_t)h->F.sync_words * sizeof(uint32_t), h->stream));
+        h->epoch_f = h->epoch_s = 0;
     }
-    for (size_t l = h->plan.size(); l-- > 0;) {
-        const LevelPlan& P = h->plan[l];
-        launch_solve_bwd(h->D, h->d_lvl_sn + P.all_off, P.all_cnt, P.all_max_r, h->d_x, h->stream); ++nk;
-    }
-    return nk;
-}
-
-nmpc_status capture(nmpc_handle_s* h, int (*issue)(nmpc_handle_s*), cudaGraphExec_t* out, int* nodes) {
-    cudaGraph_t g = nullptr;
-    CK(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
-    *nodes = issue(h);
-    CK(cudaStreamEndCapture(h->stream, &g));
-    CK(cudaGetLastError());
-    CK(cudaGraphInstantiate(out, g, 0));
-    cudaGraphDestroy(g);
+    *out = factor ? ++h->epoch_f : ++h->epoch_s;
     return NMPC_OK;
 }
 
 nmpc_status run_factor(nmpc_handle_s* h, double eta, int64_t* info) {
-    launch_factor(h->D, h->F, h->d_Kval, h->d_eta, eta, h->stream); h->launches += 2;
+    uint32_t epoch = 0;
+    TRY(next_epoch(h, true, &epoch));
+    launch_factor(h->D, h->F, h->d_Kval, eta, epoch, h->stream); h->launches += 1;
     int32_t* flag = reinterpret_cast<int32_t*>(h->h_pinned + 16);
     CK(cudaMemcpyAsync(flag, h->D.fail_col, sizeof(int32_t), cudaMemcpyDeviceToHost, h->stream));
     CK(cudaStreamSynchronize(h->stream));
@@ -245,6 +255,7 @@ nmpc_status run_factor(nmpc_handle_s* h, double eta, int64_t* info) {
     h->eta_cur = eta;
     if (*flag != INT_MAX) {
         h->factored = false;
+        launch_reset_fail(h->D, h->stream); h->launches += 1;
         if (info) *info = h->S.perm[*flag];
         return NMPC_E_NOT_SPD;
     }
@@ -254,11 +265,9 @@ nmpc_status run_factor(nmpc_handle_s* h, double eta, int64_t* info) {
 }
 
 nmpc_status run_solve(nmpc_handle_s* h, double* rhs) {       // in place, async
-    launch_permute_in(h->D, rhs, h->d_x, h->stream);
-    if (h->g_fwdbwd) { CK(cudaGraphLaunch(h->g_fwdbwd, h->stream)); h->launches += h->g_fwdbwd_nodes; }
-    else h->launches += issue_fwdbwd(h);
-    launch_permute_out(h->D, h->d_x, rhs, h->stream);
-    h->launches += 2;
+    uint32_t epoch = 0;
+    TRY(next_epoch(h, false, &epoch));
+    launch_solve(h->D, h->F, rhs, h->d_x, epoch, h->stream); h->launches += 1;
     return NMPC_OK;
 }
 
@@ -302,9 +311,9 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
         size_t factor_smem = 0;
         CK(cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev));
         CK(configure_factor_kernels(smem_optin, &ctas_per_sm, &factor_smem, &small_max_r));
-        CK(configure_solve_kernels(smem_optin));
+        int solve_ctas = 1; size_t solve_smem = 0;
+        CK(configure_solve_kernels(smem_optin, &solve_ctas, &solve_smem));
         if (h->opt.smem_front_max > 0) small_max_r = std::min(small_max_r, h->opt.smem_front_max);
-        if (((size_t)((S.max_front + 1) & ~1) + (size_t)BIG_NB * (BIG_NB + 1)) * 8 > (size_t)smem_optin) { h->err = "front too large for the solve kernel"; return NMPC_E_ALLOC; }
         DevSym& D = h->D;
         D.ns = S.ns; D.n = S.n;
         TRY(upload(h, S.sn_start, &D.sn_start)); TRY(upload(h, S.rows_ptr, &D.rows_ptr)); TRY(upload(h, S.rows, &D.rows));
@@ -315,9 +324,10 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
         TRY(upload(h, S.perm, &D.perm));
         TRY(dalloc(h, (size_t)S.panel_ptr.back() + 4 * TILE, &D.L)); TRY(dalloc(h, (size_t)S.upd_ptr.back(), &D.U, false));
         TRY(dalloc(h, (size_t)S.rel_ptr.back(), &D.ctr)); TRY(dalloc(h, 1, &D.fail_col));
-        TRY(dalloc(h, 1, &h->d_eta)); D.eta = h->d_eta;
+        TRY(dalloc(h, (size_t)S.n, &D.dinv));
+        launch_reset_fail(D, h->stream);
         TRY(dalloc(h, (size_t)S.nnzK, &h->d_Kval)); TRY(dalloc(h, (size_t)S.n, &h->d_x));
-        TRY(build_plan(h, small_max_r, ctas_per_sm, factor_smem, num_sms));
+        TRY(build_plan(h, small_max_r, ctas_per_sm, factor_smem, solve_ctas, solve_smem, num_sms));
         // symmetric CSR of K for nmpc_kkt_multiply
         {
             const int64_t n = S.n;
@@ -378,9 +388,6 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
         CK(cudaMallocHost((void**)&h->h_pinned, pinned * sizeof(double)));
         CK(cudaEventCreate(&h->ev[0])); CK(cudaEventCreate(&h->ev[1]));
         CK(cudaStreamSynchronize(h->stream));
-        if (h->opt.use_graph) {
-            TRY(capture(h, issue_fwdbwd, &h->g_fwdbwd, &h->g_fwdbwd_nodes));
-        }
         return NMPC_OK;
     };
     st = body();
@@ -391,7 +398,6 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
 
 void nmpc_destroy(nmpc_handle h) {
     if (!h) return;
-    if (h->g_fwdbwd) cudaGraphExecDestroy(h->g_fwdbwd);
     for (void* p : h->allocs) cudaFree(p);
     if (h->h_pinned) cudaFreeHost(h->h_pinned);
     if (h->ev[0]) cudaEventDestroy(h->ev[0]);

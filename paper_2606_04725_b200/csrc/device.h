@@ -34,8 +34,8 @@ struct DevSym {                   // device copies of the symbolic arrays (symbo
     double* L = nullptr;
     double* U = nullptr;
     double* ctr = nullptr;
+    double* dinv = nullptr;       // n: 1 / L_jj at pivot position j (written by the factorization, used by the solves)
     int32_t* fail_col = nullptr;  // first failing pivot position (INT_MAX = none)
-    const double* eta = nullptr;  // device scalar: diagonal shift eta_y of Eq. (13)/(17), read by the assembly kernels
 };
 
 constexpr int BIG_NB = 64;        // block size used by the triangular-solve kernels for the diagonal blocks
@@ -59,34 +59,48 @@ __host__ __device__ inline int tile_nbu(int w, int r) {
     return r <= e1 ? 1 : 1 + (r - e1 + TILE - 1) / TILE;
 }
 
-// Task list of the persistent task-DAG factorization kernel, built once by nmpc_analyze.
-//   task = (type, sn, I, J): type 0 = whole small front in shared memory, 1 = tile (I,J) of a tiled front, left-looking.
-// sync[0] = next task; sync[1 .. ns] = per-front completion counters; sync[1+ns ..] = per-panel-tile done flags.
-struct FactorPlan {
-    const int4* tasks = nullptr;
-    int32_t ntasks = 0;
+// Task lists of the persistent task-DAG kernels, built once by nmpc_analyze.
+//   factor task   (type, sn, I, J): type 0 = whole small front in shared memory, 1 = tile (I,J) of a tiled front (left-looking)
+//   solve task    (type, sn, I, dir): type 0 = whole supernode, 1 = block row / block column I of a tiled supernode;
+//                 dir 0 = forward (L v = P b), 1 = backward (L^T x = v); forward tasks first, backward = reversed order
+// Completion flags are EPOCH-valued (no reset between calls): call number e stores e into a flag and adds 1 to a counter,
+// so "done in this call" is flag >= e, counter >= e * target; the claim counter advances by ntasks + grid per call.
+struct DagPlan {
+    const int4* ftasks = nullptr;        // factorization
+    int32_t n_ftasks = 0;
+    const int4* stasks = nullptr;        // solves
+    int32_t n_stasks = 0;
     const int32_t* cls = nullptr;        // ns: 0 small, 1 tiled
     const int32_t* tbase = nullptr;      // ns: base of the front's (nbp x nbt + 1) slots in tile_done / tile_kptr
-    const int32_t* target = nullptr;     // ns: completions that finish the front (1, or the number of tiles)
+    const int32_t* bbase = nullptr;      // ns: base of the front's nbp slots in blk_f / blk_b
+    const int32_t* target = nullptr;     // ns: factor completions that finish the front (1, or the number of tiles)
+    const int32_t* target_f = nullptr;   // ns: forward-solve completions (1 or nbt);  backward: 1 or nbp
+    const int32_t* target_b = nullptr;
     const int64_t* tile_kptr = nullptr;  // per tile slot: start of its K entries (kent arrays sorted by tile for tiled fronts)
     const int64_t* cb_ptr = nullptr;     // ns: offset into cbnd of the child's block boundaries in its (tiled) parent, else -1
     const int32_t* cbnd = nullptr;
-    uint32_t* sync = nullptr;
-    int32_t sync_words = 0;
-    int32_t small_max_r = 0;             // largest front handled by the shared-memory task
-    int32_t grid = 0;
-    size_t smem_bytes = 0;
+    const int32_t* sn_parent = nullptr;  // ns
+    uint32_t* sync = nullptr;            // [0] factor claim, [1] solve claim, then the arrays below
+    uint32_t* fac_done = nullptr;        // ns
+    uint32_t* sol_done_f = nullptr;      // ns
+    uint32_t* sol_done_b = nullptr;      // ns
+    uint32_t* tile_done = nullptr;       // tile slots
+    uint32_t* blk_f = nullptr;           // block slots
+    uint32_t* blk_b = nullptr;
+    int64_t sync_words = 0;
+    int32_t small_max_r = 0;
+    int32_t fgrid = 0, sgrid = 0;
+    size_t fsmem = 0, ssmem = 0;
 };
 
 // ---- factor.cu ----
 cudaError_t configure_factor_kernels(int max_smem_bytes, int* ctas_per_sm, size_t* smem_bytes, int* small_max_r);
-void launch_factor(const DevSym& D, const FactorPlan& F, const double* Kval, double* eta_dev, double eta, cudaStream_t st);   // 2 launches
+void launch_factor(const DevSym& D, const DagPlan& F, const double* Kval, double eta, uint32_t epoch, cudaStream_t st);
+void launch_reset_fail(const DevSym& D, cudaStream_t st);                                   // fail_col = INT_MAX
 // ---- solve.cu ----
-cudaError_t configure_solve_kernels(int max_smem_bytes);
-void launch_solve_fwd(const DevSym& D, const int32_t* sn_list, int count, int max_r, double* x, cudaStream_t st);
-void launch_solve_bwd(const DevSym& D, const int32_t* sn_list, int count, int max_r, double* x, cudaStream_t st);
-void launch_permute_in(const DevSym& D, const double* b, double* x, cudaStream_t st);     // x[i] = b[perm[i]]
-void launch_permute_out(const DevSym& D, const double* x, double* b, cudaStream_t st);    // b[perm[i]] = x[i]
+cudaError_t configure_solve_kernels(int max_smem_bytes, int* ctas_per_sm, size_t* smem_bytes);
+// rhs_inout (original ordering, n doubles) is overwritten by K^-1 rhs; x is the handle's permuted work vector
+void launch_solve(const DevSym& D, const DagPlan& F, double* rhs_inout, double* x, uint32_t epoch, cudaStream_t st);
 
 // ---- ipm.cu ----
 struct DevModel {                 // device copies of the model maps (symbolic.h: ModelMaps) + parameters

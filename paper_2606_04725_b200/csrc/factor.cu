@@ -67,7 +67,7 @@ __device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
 // Requires r - j0 <= NT.  A pivot <= 0 or non-finite (reading G11) is replaced by 1 and reported through fail_col.
 // =============================================================================================================
 template <class ColFn>
-__device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, int32_t* fail_col) {
+__device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, int32_t* fail_col, double* dinv) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     for (int j0 = 0; j0 < w; j0 += 8) {
         const int jb = min(8, w - j0);
@@ -86,6 +86,7 @@ __device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, i
             const double sq = sqrt(d);
             Dg[c][c] = sq;
             inv[c] = 1.0 / sq;
+            if (tid == 0 && c < jb) dinv[c0 + j0 + c] = inv[c];
 #pragma unroll
             for (int i = c + 1; i < 8; ++i) Dg[i][c] *= inv[c];
 #pragma unroll
@@ -200,18 +201,17 @@ __device__ __forceinline__ void trsm_tile(double* Cs, const double* Ls, const do
 // =============================================================================================================
 // task type 0: whole front in shared memory, packed lower triangle: element (i,j), i >= j, at j*r - j(j-1)/2 + (i-j)
 // =============================================================================================================
-__device__ __forceinline__ void small_front_task(const DevSym& D, const FactorPlan& F, int s, const double* __restrict__ Kval,
-                                                 double eta, double* sm) {
+__device__ __forceinline__ void small_front_task(const DevSym& D, const DagPlan& F, int s, const double* __restrict__ Kval,
+                                                 double eta, uint32_t epoch, double* sm) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = NT / 32;
     const int c0 = D.sn_start[s], w = D.sn_start[s + 1] - c0;
     const int r = (int)(D.rows_ptr[s + 1] - D.rows_ptr[s]);
-    uint32_t* front_done = F.sync + 1;
+    uint32_t* front_done = F.fac_done;
     auto colp = [sm, r](int j) { return sm + (j * r - ((j * (j - 1)) >> 1) - j); };
     const int ntri = (r * (r + 1)) >> 1;
     for (int idx = tid; idx < ntri; idx += NT) sm[idx] = 0.0;
     const int ch0 = D.child_ptr[s], ch1 = D.child_ptr[s + 1];
-    if (tid < ch1 - ch0) { const int c = D.child_idx[ch0 + tid]; spin_until_ge(front_done + c, F.target[c]); }
-    for (int ci = ch0 + NT + tid; ci < ch1; ci += NT) { const int c = D.child_idx[ci]; spin_until_ge(front_done + c, F.target[c]); }
+    for (int ci = ch0 + tid; ci < ch1; ci += NT) { const int c = D.child_idx[ci]; spin_until_ge(front_done + c, epoch * (uint32_t)F.target[c]); }
     __syncthreads();
     for (int64_t q = D.kent_ptr[s] + tid; q < D.kent_ptr[s + 1]; q += NT) sm[D.kent_dst[q]] = Kval[D.kent_src[q]];
     __syncthreads();
@@ -229,7 +229,7 @@ __device__ __forceinline__ void small_front_task(const DevSym& D, const FactorPl
         }
     }
     __syncthreads();
-    partial_chol(colp, r, w, c0, D.fail_col);
+    partial_chol(colp, r, w, c0, D.fail_col, D.dinv);
     const int ld = ld_even(r), m = r - w;
     double* P = D.L + D.panel_ptr[s];
     for (int j = warp; j < w; j += nwarp) {
@@ -249,8 +249,8 @@ __device__ __forceinline__ void small_front_task(const DevSym& D, const FactorPl
 // =============================================================================================================
 // task type 1: tile (I,J) of a tiled front, left-looking
 // =============================================================================================================
-__device__ __forceinline__ void tile_task(const DevSym& D, const FactorPlan& F, int s, int I, int J, const double* __restrict__ Kval,
-                                          double eta, double* sm) {
+__device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int s, int I, int J, const double* __restrict__ Kval,
+                                          double eta, uint32_t epoch, double* sm) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = NT / 32;
     const int gid = lane >> 2, tig = lane & 3, wm = warp >> 1, wn = warp & 1;
     const int c0 = D.sn_start[s], w = D.sn_start[s + 1] - c0;
@@ -260,8 +260,8 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const FactorPlan& F, 
     const int j0 = tile_bound(J, w, r, nbp), j1 = tile_bound(J + 1, w, r, nbp), nj = j1 - j0;
     const int ia = i0 & ~1, ja = j0 & ~1, di = i0 - ia, dj = j0 - ja;
     double* P = D.L + D.panel_ptr[s];
-    uint32_t* front_done = F.sync + 1;
-    uint32_t* tdone = F.sync + 1 + D.ns + F.tbase[s];
+    uint32_t* front_done = F.fac_done;
+    uint32_t* tdone = F.tile_done + F.tbase[s];
     const int Kend = (J < nbp) ? j0 : w;
     double* pipe = sm;
     double* Cs = sm + PIPE_DOUBLES;
@@ -276,8 +276,8 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const FactorPlan& F, 
     auto wait_flags = [&](int c) {                       // thread 0: the 64-column block that chunk c starts must be finished
         if (tid == 0 && c < nch && ((c * KC) & (TILE - 1)) == 0) {
             const int kb = (c * KC) / TILE;
-            spin_until_ge(tdone + kb * nbt + I, 1u);
-            if (J != I) spin_until_ge(tdone + kb * nbt + J, 1u);
+            spin_until_ge(tdone + kb * nbt + I, epoch);
+            if (J != I) spin_until_ge(tdone + kb * nbt + J, epoch);
         }
     };
     auto issue = [&](int c) {
@@ -327,7 +327,7 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const FactorPlan& F, 
     for (int idx = tid; idx < CT_DOUBLES; idx += NT) Cs[idx] = 0.0;
     const int ch0 = D.child_ptr[s], ch1 = D.child_ptr[s + 1];
     if (J == 0) {                                        // tiles with J > 0 inherit this through the flag of tile (I,0)
-        for (int ci = ch0 + tid; ci < ch1; ci += NT) { const int c = D.child_idx[ci]; spin_until_ge(front_done + c, F.target[c]); }
+        for (int ci = ch0 + tid; ci < ch1; ci += NT) { const int c = D.child_idx[ci]; spin_until_ge(front_done + c, epoch * (uint32_t)F.target[c]); }
     }
     __syncthreads();
     if (J < nbp) {
@@ -363,11 +363,11 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const FactorPlan& F, 
     // ---- 3. finish: POTRF / TRSM for panel tiles, then store (each tile is written once) ----
     if (J < nbp) {
         if (I == J) {
-            partial_chol([Cs](int j) { return Cs + j * CLD; }, nj, nj, c0 + j0, D.fail_col);
+            partial_chol([Cs](int j) { return Cs + j * CLD; }, nj, nj, c0 + j0, D.fail_col, D.dinv);
         } else {
             double* Ls = pipe;
             double* rinv = pipe + CT_DOUBLES;
-            if (tid == 0) spin_until_ge(tdone + J * nbt + J, 1u);
+            if (tid == 0) spin_until_ge(tdone + J * nbt + J, epoch);
             __syncthreads();
             for (int idx = tid; idx < nj * nj; idx += NT) {
                 const int ii = idx % nj, cc = idx / nj;
@@ -386,7 +386,7 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const FactorPlan& F, 
         }
         __threadfence();
         __syncthreads();
-        if (tid == 0) { st_release(tdone + J * nbt + I, 1u); red_release_add(front_done + s, 1u); }
+        if (tid == 0) { st_release(tdone + J * nbt + I, epoch); red_release_add(front_done + s, 1u); }
     } else {
         double* Uo = D.U + D.upd_ptr[s];
         for (int idx = tid; idx < ni * nj; idx += NT) {
@@ -399,28 +399,23 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const FactorPlan& F, 
     }
 }
 
-__global__ void __launch_bounds__(NT, 2) factor_dag_kernel(DevSym D, FactorPlan F, const double* __restrict__ Kval) {
+__global__ void __launch_bounds__(NT, 2) factor_dag_kernel(DevSym D, DagPlan F, const double* __restrict__ Kval, double eta, uint32_t epoch) {
     extern __shared__ __align__(16) double sm[];
     __shared__ int s_task;
-    const double eta = *D.eta;
+    const uint32_t base = (epoch - 1u) * (uint32_t)(F.n_ftasks + (int)gridDim.x);
     while (true) {
         __syncthreads();
-        if (threadIdx.x == 0) s_task = (int)atomicAdd(F.sync, 1u);
+        if (threadIdx.x == 0) s_task = (int)(atomicAdd(F.sync, 1u) - base);
         __syncthreads();
         const int t = s_task;
-        if (t >= F.ntasks) break;
-        const int4 tk = F.tasks[t];
-        if (tk.x == 0) small_front_task(D, F, tk.y, Kval, eta, sm);
-        else tile_task(D, F, tk.y, tk.z, tk.w, Kval, eta, sm);
+        if (t >= F.n_ftasks) break;
+        const int4 tk = F.ftasks[t];
+        if (tk.x == 0) small_front_task(D, F, tk.y, Kval, eta, epoch, sm);
+        else tile_task(D, F, tk.y, tk.z, tk.w, Kval, eta, epoch, sm);
     }
 }
 
-// fail_col = INT_MAX, *eta_dev = eta, all completion flags and the task counter = 0
-__global__ void __launch_bounds__(NT) factor_reset_kernel(int32_t* fail_col, double* eta_dev, double eta, uint32_t* sync, int words) {
-    const int i = blockIdx.x * NT + threadIdx.x;
-    if (i == 0) { *fail_col = INT_MAX; *eta_dev = eta; }
-    for (int k = i; k < words; k += gridDim.x * NT) sync[k] = 0u;
-}
+__global__ void reset_fail_kernel(int32_t* fail_col) { *fail_col = INT_MAX; }
 
 }  // namespace
 
@@ -443,10 +438,9 @@ cudaError_t configure_factor_kernels(int max_smem_bytes, int* ctas_per_sm, size_
     return cudaSuccess;
 }
 
-void launch_factor(const DevSym& D, const FactorPlan& F, const double* Kval, double* eta_dev, double eta, cudaStream_t st) {
-    const int rb = (F.sync_words + NT - 1) / NT;
-    factor_reset_kernel<<<rb < 64 ? (rb < 1 ? 1 : rb) : 64, NT, 0, st>>>(D.fail_col, eta_dev, eta, F.sync, F.sync_words);
-    if (F.ntasks > 0) factor_dag_kernel<<<F.grid, NT, F.smem_bytes, st>>>(D, F, Kval);
+void launch_factor(const DevSym& D, const DagPlan& F, const double* Kval, double eta, uint32_t epoch, cudaStream_t st) {
+    if (F.n_ftasks > 0) factor_dag_kernel<<<F.fgrid, NT, F.fsmem, st>>>(D, F, Kval, eta, epoch);
 }
+void launch_reset_fail(const DevSym& D, cudaStream_t st) { reset_fail_kernel<<<1, 1, 0, st>>>(D.fail_col); }
 
 }  // namespace nmpc
