@@ -195,6 +195,11 @@ nmpc_status nmpc_get_info(nmpc_handle h, nmpc_sym_info* out_host);
 /* ---- copy of the factor for tests: the panels of all supernodes, one after the other, to a HOST buffer.  Panel of
  *      supernode s: column-major r_s x w_s with leading dimension r_s rounded up to even (rows = nmpc_sym_info.rows). */
 nmpc_status nmpc_get_factor(nmpc_handle h, double* panels_host /* panel_doubles */);
+/* ---- measurement aid: per-task timestamps of the last factorization (kind 0) / solve (kind 1), recorded only by handles
+ *      created while the environment variable NMPC_TRACE is set.  tasks_host: 4 int32 per task (type, supernode, I, J|dir);
+ *      stamps_host: 8 uint64 per task (globaltimer ns: claimed, dependencies met / GEMM done, assembled, factored, done;
+ *      [5] = SM id).  Returns the number of tasks copied (<= cap), the task count if a pointer is NULL, 0 if not tracing. */
+int64_t     nmpc_get_task_trace(nmpc_handle h, int32_t kind, int32_t* tasks_host, uint64_t* stamps_host, int64_t cap);
 /* ---- kernel launches issued by this handle since creation (graph replays count their kernel nodes)        */
 int64_t     nmpc_launch_count(nmpc_handle h);
 const char* nmpc_last_error(nmpc_handle h);      /* string owned by the handle                                */

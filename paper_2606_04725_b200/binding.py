@@ -88,6 +88,7 @@ SIGNATURES = {
     "nmpc_fp64_peak": (c_i32, [c_i32, c_i32, P(c_dbl), P(c_dbl)]),
     "nmpc_get_info": (c_i32, [c_vp, P(nmpc_sym_info)]),
     "nmpc_get_factor": (c_i32, [c_vp, c_vp]),
+    "nmpc_get_task_trace": (c_i64, [c_vp, c_i32, c_vp, c_vp, c_i64]),
     "nmpc_launch_count": (c_i64, [c_vp]),
     "nmpc_last_error": (C.c_char_p, [c_vp]),
     "nmpc_destroy": (None, [c_vp]),
@@ -325,6 +326,14 @@ class Handle:
         out = np.empty(info["panel_doubles"], np.float64)
         self._ck(self.lib.nmpc_get_factor(self._h, out.ctypes.data), "nmpc_get_factor")
         return out
+
+    def get_task_trace(self, kind):
+        """nmpc_get_task_trace: (tasks[nt,4] int32, stamps[nt,8] uint64) of the last factorization (0) / solve (1)."""
+        nt = int(self.lib.nmpc_get_task_trace(self._h, kind, None, None, 0))
+        tasks, stamps = np.zeros((max(nt, 0), 4), np.int32), np.zeros((max(nt, 0), 8), np.uint64)
+        if nt > 0:
+            self.lib.nmpc_get_task_trace(self._h, kind, tasks.ctypes.data, stamps.ctypes.data, nt)
+        return tasks, stamps
 
     def launch_count(self):
         return int(self.lib.nmpc_launch_count(self._h))

@@ -7,6 +7,7 @@
 #include <climits>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -223,6 +224,9 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
     TRY(dalloc(h, (size_t)F.sync_words, &F.sync));
     F.fac_done = F.sync + 2; F.sol_done_f = F.fac_done + ns; F.sol_done_b = F.sol_done_f + ns;
     F.tile_done = F.sol_done_b + ns; F.blk_f = F.tile_done + slots; F.blk_b = F.blk_f + bslots;
+    if (std::getenv("NMPC_TRACE")) {                     // measurement aid: per-task timestamps (nmpc_get_task_trace)
+        TRY(dalloc(h, (size_t)F.n_ftasks * 8, &F.ftrace)); TRY(dalloc(h, (size_t)F.n_stasks * 8, &F.strace));
+    }
     F.small_max_r = small_max_r;
     F.fsmem = smem_bytes; F.ssmem = solve_smem;
     F.fgrid = (int32_t)std::max<int64_t>(1, std::min<int64_t>((int64_t)tasks.size(), (int64_t)num_sms * ctas_per_sm));
@@ -404,6 +408,19 @@ void nmpc_destroy(nmpc_handle h) {
     if (h->ev[1]) cudaEventDestroy(h->ev[1]);
     if (h->own_stream) cudaStreamDestroy(h->stream);
     delete h;
+}
+
+int64_t nmpc_get_task_trace(nmpc_handle h, int32_t kind, int32_t* tasks_host, uint64_t* stamps_host, int64_t cap) {
+    if (!h || kind < 0 || kind > 1) return -1;
+    const int64_t nt = kind == 0 ? h->F.n_ftasks : h->F.n_stasks;
+    const unsigned long long* tr = kind == 0 ? h->F.ftrace : h->F.strace;
+    if (!tr) return 0;
+    if (!tasks_host || !stamps_host) return nt;
+    const int64_t k = std::min(nt, cap);
+    if (cudaStreamSynchronize(h->stream) != cudaSuccess) return -1;
+    if (cudaMemcpy(tasks_host, kind == 0 ? h->F.ftasks : h->F.stasks, (size_t)k * sizeof(int4), cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
+    if (cudaMemcpy(stamps_host, tr, (size_t)k * 8 * sizeof(uint64_t), cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
+    return k;
 }
 
 const char* nmpc_last_error(nmpc_handle h) { return h ? h->err.c_str() : "null handle"; }

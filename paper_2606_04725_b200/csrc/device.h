@@ -87,6 +87,8 @@ struct DagPlan {
     uint32_t* tile_done = nullptr;       // tile slots
     uint32_t* blk_f = nullptr;           // block slots
     uint32_t* blk_b = nullptr;
+    unsigned long long* ftrace = nullptr;   // optional (NMPC_TRACE=1): 8 timestamps per factor task / per solve task
+    unsigned long long* strace = nullptr;
     int64_t sync_words = 0;
     int32_t small_max_r = 0;
     int32_t fgrid = 0, sgrid = 0;

@@ -30,7 +30,9 @@ constexpr int STAGE_DOUBLES = 2 * KC * ALD;
 constexpr int PIPE_DOUBLES = NSTAGE * STAGE_DOUBLES;          // 6528
 constexpr int CT_DOUBLES = TILE * CLD;                        // 4224
 constexpr int TILE_SMEM_DOUBLES = PIPE_DOUBLES + CT_DOUBLES;  // 10752 doubles = 86016 B
-static_assert(CT_DOUBLES + TILE <= PIPE_DOUBLES, "L_JJ tile + reciprocals alias the operand ring");
+constexpr int XLD = 180;                // leading dimension of the 8 x rows staging panel of the rank-8 updates (180 mod 16 == 4)
+constexpr int XS_DOUBLES = 8 * XLD;
+static_assert(CT_DOUBLES + TILE + XS_DOUBLES <= PIPE_DOUBLES, "L_JJ tile + reciprocals + staging panel alias the operand ring");
 
 // ---- gpu-scope acquire / release on the completion flags ----
 __device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
@@ -47,6 +49,8 @@ __device__ __forceinline__ void red_release_add(uint32_t* p, uint32_t v) {
 __device__ __forceinline__ void spin_until_ge(const uint32_t* p, uint32_t target) {
     while (ld_acquire(p) < target) __nanosleep(40);
 }
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define TRACE(slot) do { if (tr && threadIdx.x == 0) tr[slot] = gtime(); } while (0)
 __device__ __forceinline__ void cp_async16(double* dst_smem, const double* src, int src_bytes) {
     const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(src), "r"(src_bytes) : "memory");
@@ -61,16 +65,20 @@ __device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
 
 // =============================================================================================================
 // Blocked partial Cholesky of the first w columns of an r x r lower-stored matrix in shared memory (Eq. 21, 8 columns
-// per step).  colp(j)[i] addresses element (i,j), i >= j.  Per step: every thread factors the 8x8 diagonal block
-// redundantly in registers (identical arithmetic -> identical values, no barrier), thread t solves row j0+t of the block
-// column against it; barrier; rank-8 update of the trailing lower triangle (warp = 4 columns, lanes = rows); barrier.
-// Requires r - j0 <= NT.  A pivot <= 0 or non-finite (reading G11) is replaced by 1 and reported through fail_col.
+// per step).  colp(j)[i] addresses element (i,j), i >= j.  Per step:
+//   phase 1: every thread factors the 8x8 diagonal block redundantly in registers (identical arithmetic -> identical
+//            values, no barrier; 1/sqrt by rsqrt, L_jj = d * rsqrt(d)); thread t solves row j0+t of the block column against
+//            it and also stores the solved row in the staging panel Xs[k][u] (u = row - (j0+jb)); barrier;
+//   phase 2: rank-8 update of the trailing lower triangle in 8x8 tiles with fp64 DMMA (2 mma.m8n8k4 per tile, operands from
+//            Xs: conflict-free), tiles dealt round-robin to the warps; barrier.
+// Requires r - j0 <= NT and r <= XS_ROWS + 8.  A pivot <= 0 or non-finite (reading G11) is replaced by 1 and reported.
 // =============================================================================================================
 template <class ColFn>
-__device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, int32_t* fail_col, double* dinv) {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+__device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, int32_t* fail_col, double* dinv, double* Xs) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gid = lane >> 2, tig = lane & 3;
     for (int j0 = 0; j0 < w; j0 += 8) {
         const int jb = min(8, w - j0);
+        const int t0 = j0 + jb, ntr = r - t0;
         double Dg[8][8], inv[8];
 #pragma unroll
         for (int c = 0; c < 8; ++c)
@@ -83,10 +91,8 @@ __device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, i
                 d = 1.0;
                 if (tid == 0 && c < jb) atomicMin(fail_col, c0 + j0 + c);
             }
-            const double sq = sqrt(d);
-            Dg[c][c] = sq;
-            inv[c] = 1.0 / sq;
-            if (tid == 0 && c < jb) dinv[c0 + j0 + c] = inv[c];
+            inv[c] = rsqrt(d);
+            Dg[c][c] = d * inv[c];
 #pragma unroll
             for (int i = c + 1; i < 8; ++i) Dg[i][c] *= inv[c];
 #pragma unroll
@@ -94,104 +100,101 @@ __device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, i
 #pragma unroll
                 for (int i = k; i < 8; ++i) Dg[i][k] = fma(-Dg[i][c], Dg[k][c], Dg[i][k]);
         }
-        const int i = j0 + tid;
-        if (i < r) {
-            if (tid < jb) {                              // a row of the diagonal block: store L
+        if (tid < jb) {
 #pragma unroll
-                for (int ii = 0; ii < 8; ++ii)
-                    if (tid == ii) {
+            for (int ii = 0; ii < 8; ++ii)
+                if (tid == ii) {                         // a row of the diagonal block: store L and the pivot reciprocal
+                    dinv[c0 + j0 + ii] = inv[ii];
 #pragma unroll
-                        for (int c = 0; c <= ii; ++c) colp(j0 + c)[i] = Dg[ii][c];
-                    }
-            } else {                                     // a row below: x = f L_D^-T
-                double x[8];
-#pragma unroll
-                for (int c = 0; c < 8; ++c) x[c] = (c < jb) ? colp(j0 + c)[i] : 0.0;
-#pragma unroll
-                for (int c = 0; c < 8; ++c) {
-                    double v = x[c];
-#pragma unroll
-                    for (int k = 0; k < c; ++k) v = fma(-x[k], Dg[c][k], v);
-                    x[c] = v * inv[c];
+                    for (int c = 0; c <= ii; ++c) colp(j0 + c)[j0 + ii] = Dg[ii][c];
                 }
+        } else if (j0 + tid < r) {                       // a row below: x = f L_D^-T (right-looking over the 8 columns)
+            const int i = j0 + tid;
+            double x[8];
 #pragma unroll
-                for (int c = 0; c < 8; ++c)
-                    if (c < jb) colp(j0 + c)[i] = x[c];
+            for (int c = 0; c < 8; ++c) x[c] = (c < jb) ? colp(j0 + c)[i] : 0.0;
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                x[k] *= inv[k];
+#pragma unroll
+                for (int c = k + 1; c < 8; ++c) x[c] = fma(-x[k], Dg[c][k], x[c]);
+            }
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                if (c < jb) colp(j0 + c)[i] = x[c];
+                Xs[c * XLD + (i - t0)] = x[c];           // x[c] == 0 for c >= jb
             }
         }
         __syncthreads();
-        const int t0 = j0 + jb, ntr = r - t0;
-        for (int g = warp; g * 4 < ntr; g += NT / 32) {
-            const int cbase = t0 + 4 * g;
-            double xc[4][8];
-#pragma unroll
-            for (int cc = 0; cc < 4; ++cc)
-#pragma unroll
-                for (int k = 0; k < 8; ++k) xc[cc][k] = (cbase + cc < r && k < jb) ? colp(j0 + k)[cbase + cc] : 0.0;
-            for (int ii = cbase + lane; ii < r; ii += 32) {
-                double xi[8];
-#pragma unroll
-                for (int k = 0; k < 8; ++k) xi[k] = (k < jb) ? colp(j0 + k)[ii] : 0.0;
-#pragma unroll
-                for (int cc = 0; cc < 4; ++cc) {
-                    const int c = cbase + cc;
-                    if (c < r && ii >= c) {
-                        double* fp = colp(c) + ii;
-                        double f = *fp;
-#pragma unroll
-                        for (int k = 0; k < 8; ++k) f = fma(-xi[k], xc[cc][k], f);
-                        *fp = f;
-                    }
-                }
+        if (ntr > 0) {
+            const int T = (ntr + 7) >> 3, ntile = (T * (T + 1)) >> 1;
+            for (int q = warp; q < ntile; q += NT / 32) {
+                int U = (int)((sqrtf(8.0f * (float)q + 1.0f) - 1.0f) * 0.5f);
+                while ((U * (U + 1)) >> 1 > q) --U;
+                while (((U + 1) * (U + 2)) >> 1 <= q) ++U;
+                const int V = q - ((U * (U + 1)) >> 1);
+                const int u = 8 * U + gid, v0 = 8 * V + 2 * tig;
+                const double a0 = -Xs[tig * XLD + u], a1 = -Xs[(tig + 4) * XLD + u];
+                const double b0 = Xs[tig * XLD + 8 * V + gid], b1 = Xs[(tig + 4) * XLD + 8 * V + gid];
+                const bool ok0 = u < ntr && u >= v0, ok1 = u < ntr && u >= v0 + 1;       // u >= v implies v < ntr
+                double* p0 = colp(t0 + v0) + (t0 + u);
+                double* p1 = colp(t0 + v0 + 1) + (t0 + u);
+                double cfr[2];
+                cfr[0] = ok0 ? *p0 : 0.0;
+                cfr[1] = ok1 ? *p1 : 0.0;
+                dmma(cfr, a0, b0);
+                dmma(cfr, a1, b1);
+                if (ok0) *p0 = cfr[0];
+                if (ok1) *p1 = cfr[1];
             }
         }
         __syncthreads();
     }
 }
 
-// X = C L^-T for an ni x nj tile C (column-major, CLD) against the nj x nj lower-triangular Ls (column-major, CLD), in place.
-__device__ __forceinline__ void trsm_tile(double* Cs, const double* Ls, const double* rinv, int ni, int nj) {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+// X = C L^-T for an ni x nj tile C (column-major, CLD) against the nj x nj lower-triangular Ls (column-major, CLD), in place;
+// same two-phase scheme: thread i solves 8 columns of row i, then the remaining columns get a rank-8 DMMA update.
+__device__ __forceinline__ void trsm_tile(double* Cs, const double* Ls, const double* rinv, int ni, int nj, double* Xs) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gid = lane >> 2, tig = lane & 3;
     for (int j0 = 0; j0 < nj; j0 += 8) {
         const int jb = min(8, nj - j0);
-        if (tid < ni) {
+        if (tid < TILE) {
             double x[8];
 #pragma unroll
-            for (int c = 0; c < 8; ++c) x[c] = (c < jb) ? Cs[(j0 + c) * CLD + tid] : 0.0;
+            for (int c = 0; c < 8; ++c) x[c] = (c < jb && tid < ni) ? Cs[(j0 + c) * CLD + tid] : 0.0;
 #pragma unroll
-            for (int c = 0; c < 8; ++c)
-                if (c < jb) {
-                    double v = x[c];
+            for (int k = 0; k < 8; ++k)
+                if (k < jb) {
+                    x[k] *= rinv[j0 + k];
 #pragma unroll
-                    for (int k = 0; k < c; ++k) v = fma(-x[k], Ls[(j0 + k) * CLD + j0 + c], v);
-                    x[c] = v * rinv[j0 + c];
+                    for (int c = k + 1; c < 8; ++c)
+                        if (c < jb) x[c] = fma(-x[k], Ls[(j0 + k) * CLD + j0 + c], x[c]);
                 }
 #pragma unroll
-            for (int c = 0; c < 8; ++c)
-                if (c < jb) Cs[(j0 + c) * CLD + tid] = x[c];
+            for (int c = 0; c < 8; ++c) {
+                if (c < jb && tid < ni) Cs[(j0 + c) * CLD + tid] = x[c];
+                Xs[c * XLD + tid] = (c < jb) ? x[c] : 0.0;
+            }
         }
         __syncthreads();
         const int t0 = j0 + jb, ntr = nj - t0;
-        for (int g = warp; g * 4 < ntr; g += NT / 32) {
-            const int cbase = t0 + 4 * g;
-            double lc[4][8];
-#pragma unroll
-            for (int cc = 0; cc < 4; ++cc)
-#pragma unroll
-                for (int k = 0; k < 8; ++k) lc[cc][k] = (cbase + cc < nj && k < jb) ? Ls[(j0 + k) * CLD + cbase + cc] : 0.0;
-            for (int ii = lane; ii < ni; ii += 32) {
-                double xi[8];
-#pragma unroll
-                for (int k = 0; k < 8; ++k) xi[k] = (k < jb) ? Cs[(j0 + k) * CLD + ii] : 0.0;
-#pragma unroll
-                for (int cc = 0; cc < 4; ++cc)
-                    if (cbase + cc < nj) {
-                        double* fp = Cs + (cbase + cc) * CLD + ii;
-                        double f = *fp;
-#pragma unroll
-                        for (int k = 0; k < 8; ++k) f = fma(-xi[k], lc[cc][k], f);
-                        *fp = f;
-                    }
+        if (ntr > 0) {
+            const int TU = (ni + 7) >> 3, TV = (ntr + 7) >> 3;
+            for (int q = warp; q < TU * TV; q += NT / 32) {
+                const int U = q % TU, V = q / TU;
+                const int u = 8 * U + gid, v0 = t0 + 8 * V + 2 * tig, vb = t0 + 8 * V + gid;
+                const double a0 = -Xs[tig * XLD + u], a1 = -Xs[(tig + 4) * XLD + u];
+                const double b0 = (vb < nj && tig < jb) ? Ls[(j0 + tig) * CLD + vb] : 0.0;
+                const double b1 = (vb < nj && tig + 4 < jb) ? Ls[(j0 + tig + 4) * CLD + vb] : 0.0;
+                const bool ok0 = u < ni && v0 < nj, ok1 = u < ni && v0 + 1 < nj;
+                double* p0 = Cs + v0 * CLD + u;
+                double cfr[2];
+                cfr[0] = ok0 ? p0[0] : 0.0;
+                cfr[1] = ok1 ? p0[CLD] : 0.0;
+                dmma(cfr, a0, b0);
+                dmma(cfr, a1, b1);
+                if (ok0) p0[0] = cfr[0];
+                if (ok1) p0[CLD] = cfr[1];
             }
         }
         __syncthreads();
@@ -202,7 +205,7 @@ __device__ __forceinline__ void trsm_tile(double* Cs, const double* Ls, const do
 // task type 0: whole front in shared memory, packed lower triangle: element (i,j), i >= j, at j*r - j(j-1)/2 + (i-j)
 // =============================================================================================================
 __device__ __forceinline__ void small_front_task(const DevSym& D, const DagPlan& F, int s, const double* __restrict__ Kval,
-                                                 double eta, uint32_t epoch, double* sm) {
+                                                 double eta, uint32_t epoch, double* sm, unsigned long long* tr) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = NT / 32;
     const int c0 = D.sn_start[s], w = D.sn_start[s + 1] - c0;
     const int r = (int)(D.rows_ptr[s + 1] - D.rows_ptr[s]);
@@ -213,6 +216,7 @@ __device__ __forceinline__ void small_front_task(const DevSym& D, const DagPlan&
     const int ch0 = D.child_ptr[s], ch1 = D.child_ptr[s + 1];
     for (int ci = ch0 + tid; ci < ch1; ci += NT) { const int c = D.child_idx[ci]; spin_until_ge(front_done + c, epoch * (uint32_t)F.target[c]); }
     __syncthreads();
+    TRACE(1);
     for (int64_t q = D.kent_ptr[s] + tid; q < D.kent_ptr[s + 1]; q += NT) sm[D.kent_dst[q]] = Kval[D.kent_src[q]];
     __syncthreads();
     if (eta != 0.0) for (int j = tid; j < w; j += NT) colp(j)[j] += eta;
@@ -229,7 +233,9 @@ __device__ __forceinline__ void small_front_task(const DevSym& D, const DagPlan&
         }
     }
     __syncthreads();
-    partial_chol(colp, r, w, c0, D.fail_col, D.dinv);
+    TRACE(2);
+    partial_chol(colp, r, w, c0, D.fail_col, D.dinv, sm + ((ntri + 1) & ~1));
+    TRACE(3);
     const int ld = ld_even(r), m = r - w;
     double* P = D.L + D.panel_ptr[s];
     for (int j = warp; j < w; j += nwarp) {
@@ -244,13 +250,14 @@ __device__ __forceinline__ void small_front_task(const DevSym& D, const DagPlan&
     __threadfence();
     __syncthreads();
     if (tid == 0) red_release_add(front_done + s, 1u);
+    TRACE(4);
 }
 
 // =============================================================================================================
 // task type 1: tile (I,J) of a tiled front, left-looking
 // =============================================================================================================
 __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int s, int I, int J, const double* __restrict__ Kval,
-                                          double eta, uint32_t epoch, double* sm) {
+                                          double eta, uint32_t epoch, double* sm, unsigned long long* tr) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = NT / 32;
     const int gid = lane >> 2, tig = lane & 3, wm = warp >> 1, wn = warp & 1;
     const int c0 = D.sn_start[s], w = D.sn_start[s + 1] - c0;
@@ -322,6 +329,7 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
         }
     }
     cp_async_wait<0>();
+    TRACE(1);
 
     // ---- 2. assemble the tile: zero, K entries, eta, children's update matrices (fixed child order) ----
     for (int idx = tid; idx < CT_DOUBLES; idx += NT) Cs[idx] = 0.0;
@@ -360,10 +368,11 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
             for (int e = 0; e < 2; ++e) Cs[(wn * 32 + nt * 8 + 2 * tig + e) * CLD + wm * 16 + mt * 8 + gid] -= acc[mt][nt][e];
     __syncthreads();
 
+    TRACE(2);
     // ---- 3. finish: POTRF / TRSM for panel tiles, then store (each tile is written once) ----
     if (J < nbp) {
         if (I == J) {
-            partial_chol([Cs](int j) { return Cs + j * CLD; }, nj, nj, c0 + j0, D.fail_col, D.dinv);
+            partial_chol([Cs](int j) { return Cs + j * CLD; }, nj, nj, c0 + j0, D.fail_col, D.dinv, pipe + CT_DOUBLES + TILE);
         } else {
             double* Ls = pipe;
             double* rinv = pipe + CT_DOUBLES;
@@ -378,8 +387,9 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
                 }
             }
             __syncthreads();
-            trsm_tile(Cs, Ls, rinv, ni, nj);
+            trsm_tile(Cs, Ls, rinv, ni, nj, pipe + CT_DOUBLES + TILE);
         }
+        TRACE(3);
         for (int idx = tid; idx < ni * nj; idx += NT) {
             const int mm = idx % ni, nn = idx / ni;
             if (I != J || mm >= nn) P[(i0 + mm) + (int64_t)(j0 + nn) * ld] = Cs[nn * CLD + mm];
@@ -389,6 +399,7 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
         if (tid == 0) { st_release(tdone + J * nbt + I, epoch); red_release_add(front_done + s, 1u); }
     } else {
         double* Uo = D.U + D.upd_ptr[s];
+        TRACE(3);
         for (int idx = tid; idx < ni * nj; idx += NT) {
             const int mm = idx % ni, nn = idx / ni;
             if (I != J || mm >= nn) Uo[(i0 + mm - w) + (int64_t)(j0 + nn - w) * m] = Cs[nn * CLD + mm];
@@ -397,6 +408,7 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
         __syncthreads();
         if (tid == 0) red_release_add(front_done + s, 1u);
     }
+    TRACE(4);
 }
 
 __global__ void __launch_bounds__(NT, 2) factor_dag_kernel(DevSym D, DagPlan F, const double* __restrict__ Kval, double eta, uint32_t epoch) {
@@ -410,8 +422,10 @@ __global__ void __launch_bounds__(NT, 2) factor_dag_kernel(DevSym D, DagPlan F, 
         const int t = s_task;
         if (t >= F.n_ftasks) break;
         const int4 tk = F.ftasks[t];
-        if (tk.x == 0) small_front_task(D, F, tk.y, Kval, eta, epoch, sm);
-        else tile_task(D, F, tk.y, tk.z, tk.w, Kval, eta, epoch, sm);
+        unsigned long long* tr = F.ftrace ? F.ftrace + (size_t)t * 8 : nullptr;
+        if (tr && threadIdx.x == 0) { tr[0] = gtime(); unsigned sid; asm volatile("mov.u32 %0, %%smid;" : "=r"(sid)); tr[5] = sid; }
+        if (tk.x == 0) small_front_task(D, F, tk.y, Kval, eta, epoch, sm, tr);
+        else tile_task(D, F, tk.y, tk.z, tk.w, Kval, eta, epoch, sm, tr);
     }
 }
 
@@ -432,8 +446,8 @@ cudaError_t configure_factor_kernels(int max_smem_bytes, int* ctas_per_sm, size_
     if (e != cudaSuccess) return e;
     *ctas_per_sm = occ < 1 ? 1 : occ;
     *smem_bytes = bytes;
-    int rmax = 1;                                        // largest r with r(r+1)/2 doubles in `bytes`, and r <= NT
-    while (rmax < NT && (size_t)(rmax + 1) * (rmax + 2) / 2 * sizeof(double) <= bytes) ++rmax;
+    int rmax = 1;                                        // largest r with the packed front + the staging panel in `bytes`
+    while (rmax < NT && rmax < XLD - 8 && ((size_t)(rmax + 1) * (rmax + 2) / 2 + 1 + XS_DOUBLES) * sizeof(double) <= bytes) ++rmax;
     *small_max_r = rmax;
     return cudaSuccess;
 }

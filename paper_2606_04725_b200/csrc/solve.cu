@@ -312,8 +312,11 @@ __global__ void __launch_bounds__(NT) solve_dag_kernel(DevSym D, DagPlan F, doub
         const int t = s_task;
         if (t >= F.n_stasks) break;
         const int4 tk = F.stasks[t];
+        unsigned long long* tr = F.strace ? F.strace + (size_t)t * 8 : nullptr;
+        if (tr && threadIdx.x == 0) { unsigned long long g; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g)); tr[0] = g; }
         if (tk.w == 0) { if (tk.x == 0) fwd_small(D, F, tk.y, b, x, epoch, sm); else fwd_tiled(D, F, tk.y, tk.z, b, x, epoch, sm); }
         else           { if (tk.x == 0) bwd_small(D, F, tk.y, b, x, epoch, sm); else bwd_tiled(D, F, tk.y, tk.z, b, x, epoch, sm); }
+        if (tr && threadIdx.x == 0) { unsigned long long g; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g)); tr[4] = g; }
     }
 }
 
