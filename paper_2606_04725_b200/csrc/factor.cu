@@ -25,14 +25,12 @@ constexpr int NT = 256;                 // threads per CTA
 constexpr int KC = 16;                  // k-columns per pipeline stage
 constexpr int ALD = 68;                 // leading dimension of an operand stage  (68 mod 16 == 4: conflict-free DMMA fragment loads)
 constexpr int CLD = 66;                 // leading dimension of the C / L_JJ tile (2*66 mod 16 == 4: conflict-free fragment stores)
-constexpr int NSTAGE = 3;
+constexpr int NSTAGE = 4;
 constexpr int STAGE_DOUBLES = 2 * KC * ALD;
-constexpr int PIPE_DOUBLES = NSTAGE * STAGE_DOUBLES;          // 6528
+constexpr int PIPE_DOUBLES = NSTAGE * STAGE_DOUBLES;          // 8704
 constexpr int CT_DOUBLES = TILE * CLD;                        // 4224
-constexpr int TILE_SMEM_DOUBLES = PIPE_DOUBLES + CT_DOUBLES;  // 10752 doubles = 86016 B
-constexpr int XLD = 180;                // leading dimension of the 8 x rows staging panel of the rank-8 updates (180 mod 16 == 4)
-constexpr int XS_DOUBLES = 8 * XLD;
-static_assert(CT_DOUBLES + TILE + XS_DOUBLES <= PIPE_DOUBLES, "L_JJ tile + reciprocals + staging panel alias the operand ring");
+constexpr int TILE_SMEM_DOUBLES = PIPE_DOUBLES + CT_DOUBLES;  // 12928 doubles = 103424 B
+static_assert(CT_DOUBLES + TILE <= PIPE_DOUBLES, "L_JJ tile + reciprocals alias the operand ring");
 
 // ---- gpu-scope acquire / release on the completion flags ----
 __device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
@@ -58,146 +56,283 @@ __device__ __forceinline__ void cp_async16(double* dst_smem, const double* src, 
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+// 1/sqrt(d) for a normal d > 0: hardware approximation (rsqrt.approx.f64, ~2^-22) + two Newton steps -> rounding level
+__device__ __forceinline__ double rsqrt_newton(double d) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(d));
+    const double h = 0.5 * d;
+    double e = fma(-h * y, y, 0.5);
+    y = fma(y, e, y);
+    e = fma(-h * y, y, 0.5);
+    y = fma(y, e, y);
+    return y;
+}
 __device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                  : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
 }
 
 // =============================================================================================================
-// Blocked partial Cholesky of the first w columns of an r x r lower-stored matrix in shared memory (Eq. 21, 8 columns
-// per step).  colp(j)[i] addresses element (i,j), i >= j.  Per step:
-//   phase 1: every thread factors the 8x8 diagonal block redundantly in registers (identical arithmetic -> identical
-//            values, no barrier; 1/sqrt by rsqrt, L_jj = d * rsqrt(d)); thread t solves row j0+t of the block column against
-//            it and also stores the solved row in the staging panel Xs[k][u] (u = row - (j0+jb)); barrier;
-//   phase 2: rank-8 update of the trailing lower triangle in 8x8 tiles with fp64 DMMA (2 mma.m8n8k4 per tile, operands from
-//            Xs: conflict-free), tiles dealt round-robin to the warps; barrier.
-// Requires r - j0 <= NT and r <= XS_ROWS + 8.  A pivot <= 0 or non-finite (reading G11) is replaced by 1 and reported.
+// Blocked partial Cholesky of the first w columns of an r x r lower-stored matrix in shared memory (Eq. 21).
+// colp(j)[i] addresses element (i,j), i >= j.  Two-level blocking: panels of 32 columns, sub-steps of 8 columns.
+//   sub-step, phase 1: every thread factors the 8x8 diagonal block redundantly in registers (identical arithmetic ->
+//            identical values, no barrier; 1/sqrt by rsqrt, L_jj = d * rsqrt(d)); thread t solves row j0+t of the block
+//            column against it (x = f L_D^-T); barrier;
+//   sub-step, phase 2: rank-8 DMMA update of the REST OF THE PANEL only (<= 24 columns); barrier;
+//   panel end: rank-32 DMMA update of the trailing columns, 8 chained mma.m8n8k4 per 8x8 tile.
+// DMMA operands come straight from the finished columns of the front; tiles are dealt round-robin to the warps, two in
+// flight per warp.  Requires r <= NT.  A pivot <= 0 or non-finite (reading G11) is replaced by 1 and reported.
 // =============================================================================================================
 template <class ColFn>
-__device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, int32_t* fail_col, double* dinv, double* Xs) {
+__device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, int32_t* fail_col, double* dinv) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gid = lane >> 2, tig = lane & 3;
-    for (int j0 = 0; j0 < w; j0 += 8) {
-        const int jb = min(8, w - j0);
-        const int t0 = j0 + jb, ntr = r - t0;
-        double Dg[8][8], inv[8];
+    constexpr int NW = NT / 32;
+    __shared__ double s_inv[8];
+    const int rl = r - 1;
+    for (int p0 = 0; p0 < w; p0 += 32) {
+        const int p1 = min(w, p0 + 32);
+        for (int j0 = p0; j0 < p1; j0 += 8) {
+            const int jb = min(8, p1 - j0);
+            const int t0 = j0 + jb;
+            const bool full = jb == 8;
+            if (warp == 0) {                             // phase 1a: the 8x8 diagonal block, in registers
+                double Dg[8][8], inv[8];
+                if (full) {
 #pragma unroll
-        for (int c = 0; c < 8; ++c)
+                    for (int c = 0; c < 8; ++c) {
+                        const double* cp = colp(j0 + c) + j0;
 #pragma unroll
-            for (int i = c; i < 8; ++i) Dg[i][c] = (i < jb) ? colp(j0 + c)[j0 + i] : (i == c ? 1.0 : 0.0);   // i < jb implies c < jb
+                        for (int i = c; i < 8; ++i) Dg[i][c] = cp[i];
+                    }
+                } else {
 #pragma unroll
-        for (int c = 0; c < 8; ++c) {
-            double d = Dg[c][c];
-            if (!(d > 0.0) || isinf(d)) {
-                d = 1.0;
-                if (tid == 0 && c < jb) atomicMin(fail_col, c0 + j0 + c);
-            }
-            inv[c] = rsqrt(d);
-            Dg[c][c] = d * inv[c];
+                    for (int c = 0; c < 8; ++c) {
+                        const double* cp = colp(j0 + min(c, jb - 1)) + j0;
 #pragma unroll
-            for (int i = c + 1; i < 8; ++i) Dg[i][c] *= inv[c];
-#pragma unroll
-            for (int k = c + 1; k < 8; ++k)
-#pragma unroll
-                for (int i = k; i < 8; ++i) Dg[i][k] = fma(-Dg[i][c], Dg[k][c], Dg[i][k]);
-        }
-        if (tid < jb) {
-#pragma unroll
-            for (int ii = 0; ii < 8; ++ii)
-                if (tid == ii) {                         // a row of the diagonal block: store L and the pivot reciprocal
-                    dinv[c0 + j0 + ii] = inv[ii];
-#pragma unroll
-                    for (int c = 0; c <= ii; ++c) colp(j0 + c)[j0 + ii] = Dg[ii][c];
+                        for (int i = c; i < 8; ++i) { const double v = cp[min(i, jb - 1)]; Dg[i][c] = (i < jb) ? v : (i == c ? 1.0 : 0.0); }   // i < jb implies c < jb
+                    }
                 }
-        } else if (j0 + tid < r) {                       // a row below: x = f L_D^-T (right-looking over the 8 columns)
-            const int i = j0 + tid;
-            double x[8];
+                bool bad = false;
+                int badc = 8;
 #pragma unroll
-            for (int c = 0; c < 8; ++c) x[c] = (c < jb) ? colp(j0 + c)[i] : 0.0;
+                for (int c = 0; c < 8; ++c) {
+                    double d = Dg[c][c];
+                    if (!(d >= 2.2250738585072014e-308) || isinf(d)) {   // <= 0, non-finite (or subnormal): reading G11
+                        d = 1.0;
+                        if (!bad && c < jb) { bad = true; badc = c; }
+                    }
+                    inv[c] = rsqrt_newton(d);
+                    Dg[c][c] = d * inv[c];
 #pragma unroll
-            for (int k = 0; k < 8; ++k) {
-                x[k] *= inv[k];
+                    for (int i = c + 1; i < 8; ++i) Dg[i][c] *= inv[c];
 #pragma unroll
-                for (int c = k + 1; c < 8; ++c) x[c] = fma(-x[k], Dg[c][k], x[c]);
+                    for (int k = c + 1; k < 8; ++k)
+#pragma unroll
+                        for (int i = k; i < 8; ++i) Dg[i][k] = fma(-Dg[i][c], Dg[k][c], Dg[i][k]);
+                }
+                if (bad && lane == 0) atomicMin(fail_col, c0 + j0 + badc);
+#pragma unroll
+                for (int ii = 0; ii < 8; ++ii)
+                    if (lane == ii && ii < jb) {         // lane ii stores row ii of L_D and the pivot reciprocal
+                        dinv[c0 + j0 + ii] = inv[ii];
+                        s_inv[ii] = inv[ii];
+#pragma unroll
+                        for (int c = 0; c <= ii; ++c) colp(j0 + c)[j0 + ii] = Dg[ii][c];
+                    }
             }
+            __syncthreads();
+            if (tid >= jb && j0 + tid < r) {             // phase 1b: a row below: x = f L_D^-T (right-looking over the 8 columns)
+                const int i = j0 + tid;
+                double x[8], Lk[8][8], inv[8];
+                if (full) {
 #pragma unroll
-            for (int c = 0; c < 8; ++c) {
-                if (c < jb) colp(j0 + c)[i] = x[c];
-                Xs[c * XLD + (i - t0)] = x[c];           // x[c] == 0 for c >= jb
+                    for (int c = 0; c < 8; ++c) {
+                        const double* cp = colp(j0 + c);
+                        x[c] = cp[i];
+                        inv[c] = s_inv[c];
+#pragma unroll
+                        for (int k = c + 1; k < 8; ++k) Lk[k][c] = cp[j0 + k];
+                    }
+                } else {
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) {
+                        const double* cp = colp(j0 + min(c, jb - 1));
+                        const double xv = cp[i], iv = s_inv[min(c, jb - 1)];
+                        x[c] = (c < jb) ? xv : 0.0;
+                        inv[c] = (c < jb) ? iv : 1.0;
+#pragma unroll
+                        for (int k = c + 1; k < 8; ++k) { const double v = cp[j0 + min(k, jb - 1)]; Lk[k][c] = (k < jb) ? v : 0.0; }
+                    }
+                }
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    x[k] *= inv[k];
+#pragma unroll
+                    for (int c = k + 1; c < 8; ++c) x[c] = fma(-x[k], Lk[c][k], x[c]);
+                }
+#pragma unroll
+                for (int c = 0; c < 8; ++c)
+                    if (c < jb) colp(j0 + c)[i] = x[c];
+            }
+            __syncthreads();
+            if (t0 < p1) {                               // phase 2: rank-8 update of the panel's remaining columns [t0, p1)
+                const bool k0 = tig < jb, k1 = tig + 4 < jb;
+                const double* ck0 = colp(j0 + (k0 ? tig : 0));
+                const double* ck1 = colp(j0 + (k1 ? tig + 4 : 0));
+                const int TU = (r - t0 + 7) >> 3, TV = (p1 - t0 + 7) >> 3, ntile = TU * TV;
+                for (int qb = warp; qb < ntile; qb += 2 * NW) {
+                    double acc[2][2], cold[2][2];
+                    double* pc[2][2];
+                    bool ok[2][2];
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const int q = min(qb + e * NW, ntile - 1);
+                        const int V = q / TU, U = q - V * TU;
+                        const int u = t0 + 8 * U + gid, vb = t0 + 8 * V + gid, vc = t0 + 8 * V + 2 * tig;
+                        const bool live = qb + e * NW < ntile && U >= V;
+                        const int ucl = min(u, rl), vbl = min(vb, rl);
+                        const double a0 = ck0[ucl], a1 = ck1[ucl], b0 = ck0[vbl], b1 = ck1[vbl];
+                        ok[e][0] = live && u < r && vc < p1 && u >= vc;
+                        ok[e][1] = live && u < r && vc + 1 < p1 && u >= vc + 1;
+                        pc[e][0] = colp(min(vc, rl)) + ucl;
+                        pc[e][1] = colp(min(vc + 1, rl)) + ucl;
+                        cold[e][0] = *pc[e][0];
+                        cold[e][1] = *pc[e][1];
+                        acc[e][0] = acc[e][1] = 0.0;
+                        dmma(acc[e], (live && k0) ? a0 : 0.0, k0 ? b0 : 0.0);
+                        dmma(acc[e], (live && k1) ? a1 : 0.0, k1 ? b1 : 0.0);
+                    }
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        if (ok[e][0]) *pc[e][0] = cold[e][0] - acc[e][0];
+                        if (ok[e][1]) *pc[e][1] = cold[e][1] - acc[e][1];
+                    }
+                }
+                __syncthreads();
             }
         }
-        __syncthreads();
-        if (ntr > 0) {
-            const int T = (ntr + 7) >> 3, ntile = (T * (T + 1)) >> 1;
-            for (int q = warp; q < ntile; q += NT / 32) {
-                int U = (int)((sqrtf(8.0f * (float)q + 1.0f) - 1.0f) * 0.5f);
-                while ((U * (U + 1)) >> 1 > q) --U;
-                while (((U + 1) * (U + 2)) >> 1 <= q) ++U;
-                const int V = q - ((U * (U + 1)) >> 1);
-                const int u = 8 * U + gid, v0 = 8 * V + 2 * tig;
-                const double a0 = -Xs[tig * XLD + u], a1 = -Xs[(tig + 4) * XLD + u];
-                const double b0 = Xs[tig * XLD + 8 * V + gid], b1 = Xs[(tig + 4) * XLD + 8 * V + gid];
-                const bool ok0 = u < ntr && u >= v0, ok1 = u < ntr && u >= v0 + 1;       // u >= v implies v < ntr
-                double* p0 = colp(t0 + v0) + (t0 + u);
-                double* p1 = colp(t0 + v0 + 1) + (t0 + u);
-                double cfr[2];
-                cfr[0] = ok0 ? *p0 : 0.0;
-                cfr[1] = ok1 ? *p1 : 0.0;
-                dmma(cfr, a0, b0);
-                dmma(cfr, a1, b1);
-                if (ok0) *p0 = cfr[0];
-                if (ok1) *p1 = cfr[1];
+        if (p1 < r) {                                    // panel end: rank-(p1-p0) update of the trailing columns [p1, r)
+            const double* ck[8];
+            bool kv[8];
+#pragma unroll
+            for (int s8 = 0; s8 < 8; ++s8) { const int kc = p0 + 4 * s8 + tig; kv[s8] = kc < p1; ck[s8] = colp(kv[s8] ? kc : p0); }
+            const int T = (r - p1 + 7) >> 3, ntile = (T * (T + 1)) >> 1;
+            for (int qb = warp; qb < ntile; qb += 2 * NW) {
+                double acc[2][2], cold[2][2];
+                double* pc[2][2];
+                bool ok[2][2];
+                int ucl[2], vbl[2];
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int q = min(qb + e * NW, ntile - 1);
+                    int U = (int)((sqrtf(8.0f * (float)q + 1.0f) - 1.0f) * 0.5f);
+                    U += (((U + 1) * (U + 2)) >> 1 <= q) - (((U * (U + 1)) >> 1) > q);      // float rounding: off by at most one
+                    const int V = q - ((U * (U + 1)) >> 1);
+                    const bool live = qb + e * NW < ntile;
+                    const int u = p1 + 8 * U + gid, vb = p1 + 8 * V + gid, vc = p1 + 8 * V + 2 * tig;
+                    ucl[e] = min(u, rl); vbl[e] = min(vb, rl);
+                    ok[e][0] = live && u < r && vc < r && u >= vc;
+                    ok[e][1] = live && u < r && vc + 1 < r && u >= vc + 1;
+                    pc[e][0] = colp(min(vc, rl)) + ucl[e];
+                    pc[e][1] = colp(min(vc + 1, rl)) + ucl[e];
+                    cold[e][0] = *pc[e][0];
+                    cold[e][1] = *pc[e][1];
+                    acc[e][0] = acc[e][1] = 0.0;
+                }
+#pragma unroll
+                for (int s8 = 0; s8 < 8; ++s8) {
+                    double a[2], b[2];
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) { a[e] = ck[s8][ucl[e]]; b[e] = ck[s8][vbl[e]]; }
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) dmma(acc[e], kv[s8] ? a[e] : 0.0, kv[s8] ? b[e] : 0.0);
+                }
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    if (ok[e][0]) *pc[e][0] = cold[e][0] - acc[e][0];
+                    if (ok[e][1]) *pc[e][1] = cold[e][1] - acc[e][1];
+                }
             }
+            __syncthreads();
         }
-        __syncthreads();
     }
 }
 
-// X = C L^-T for an ni x nj tile C (column-major, CLD) against the nj x nj lower-triangular Ls (column-major, CLD), in place;
-// same two-phase scheme: thread i solves 8 columns of row i, then the remaining columns get a rank-8 DMMA update.
-__device__ __forceinline__ void trsm_tile(double* Cs, const double* Ls, const double* rinv, int ni, int nj, double* Xs) {
+// X = C L^-T for an ni x nj tile C (column-major, CLD) against the nj x nj lower-triangular Ls (column-major, CLD), in
+// place, same panel scheme: thread i substitutes 8 columns of row i, the rest of the 32-column panel gets a rank-8 DMMA
+// update, the columns after the panel a rank-32 one.  Rows >= ni / columns >= nj of the tiles are finite padding.
+__device__ __forceinline__ void trsm_tile(double* Cs, const double* Ls, const double* rinv, int ni, int nj) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gid = lane >> 2, tig = lane & 3;
-    for (int j0 = 0; j0 < nj; j0 += 8) {
-        const int jb = min(8, nj - j0);
-        if (tid < TILE) {
-            double x[8];
+    constexpr int NW = NT / 32;
+    const int TU = (ni + 7) >> 3;
+    for (int p0 = 0; p0 < nj; p0 += 32) {
+        const int p1 = min(nj, p0 + 32);
+        for (int j0 = p0; j0 < p1; j0 += 8) {
+            const int jb = min(8, p1 - j0), t0 = j0 + jb;
+            if (tid < ni) {
+                double x[8], Lk[8][8], inv[8];
 #pragma unroll
-            for (int c = 0; c < 8; ++c) x[c] = (c < jb && tid < ni) ? Cs[(j0 + c) * CLD + tid] : 0.0;
+                for (int c = 0; c < 8; ++c) {
+                    const int cc = j0 + min(c, jb - 1);
+                    const double xv = Cs[cc * CLD + tid], iv = rinv[cc];
+                    x[c] = (c < jb) ? xv : 0.0;
+                    inv[c] = (c < jb) ? iv : 1.0;
 #pragma unroll
-            for (int k = 0; k < 8; ++k)
-                if (k < jb) {
-                    x[k] *= rinv[j0 + k];
-#pragma unroll
-                    for (int c = k + 1; c < 8; ++c)
-                        if (c < jb) x[c] = fma(-x[k], Ls[(j0 + k) * CLD + j0 + c], x[c]);
+                    for (int k = c + 1; k < 8; ++k) { const double v = Ls[cc * CLD + j0 + min(k, jb - 1)]; Lk[k][c] = (k < jb) ? v : 0.0; }
                 }
 #pragma unroll
-            for (int c = 0; c < 8; ++c) {
-                if (c < jb && tid < ni) Cs[(j0 + c) * CLD + tid] = x[c];
-                Xs[c * XLD + tid] = (c < jb) ? x[c] : 0.0;
+                for (int k = 0; k < 8; ++k) {
+                    x[k] *= inv[k];
+#pragma unroll
+                    for (int c = k + 1; c < 8; ++c) x[c] = fma(-x[k], Lk[c][k], x[c]);
+                }
+#pragma unroll
+                for (int c = 0; c < 8; ++c)
+                    if (c < jb) Cs[(j0 + c) * CLD + tid] = x[c];
+            }
+            __syncthreads();
+            if (t0 < p1) {
+                const bool k0 = tig < jb, k1 = tig + 4 < jb;
+                const int kc0 = j0 + (k0 ? tig : 0), kc1 = j0 + (k1 ? tig + 4 : 0);
+                const int TV = (p1 - t0 + 7) >> 3;
+                for (int q = warp; q < TU * TV; q += NW) {
+                    const int U = q % TU, V = q / TU;
+                    const int u = 8 * U + gid, v0 = t0 + 8 * V + 2 * tig, vb = min(t0 + 8 * V + gid, TILE - 1);
+                    const double a0 = Cs[kc0 * CLD + u], a1 = Cs[kc1 * CLD + u];
+                    const double b0 = Ls[kc0 * CLD + vb], b1 = Ls[kc1 * CLD + vb];
+                    const bool ok0 = v0 < p1, ok1 = v0 + 1 < p1;
+                    double* pc = Cs + min(v0, TILE - 2) * CLD + u;
+                    const double c0v = pc[0], c1v = pc[CLD];
+                    double acc[2] = {0.0, 0.0};
+                    dmma(acc, k0 ? a0 : 0.0, k0 ? b0 : 0.0);
+                    dmma(acc, k1 ? a1 : 0.0, k1 ? b1 : 0.0);
+                    if (ok0) pc[0] = c0v - acc[0];
+                    if (ok1) pc[CLD] = c1v - acc[1];
+                }
+                __syncthreads();
             }
         }
-        __syncthreads();
-        const int t0 = j0 + jb, ntr = nj - t0;
-        if (ntr > 0) {
-            const int TU = (ni + 7) >> 3, TV = (ntr + 7) >> 3;
-            for (int q = warp; q < TU * TV; q += NT / 32) {
+        if (p1 < nj) {
+            const int TV = (nj - p1 + 7) >> 3;
+            for (int q = warp; q < TU * TV; q += NW) {
                 const int U = q % TU, V = q / TU;
-                const int u = 8 * U + gid, v0 = t0 + 8 * V + 2 * tig, vb = t0 + 8 * V + gid;
-                const double a0 = -Xs[tig * XLD + u], a1 = -Xs[(tig + 4) * XLD + u];
-                const double b0 = (vb < nj && tig < jb) ? Ls[(j0 + tig) * CLD + vb] : 0.0;
-                const double b1 = (vb < nj && tig + 4 < jb) ? Ls[(j0 + tig + 4) * CLD + vb] : 0.0;
-                const bool ok0 = u < ni && v0 < nj, ok1 = u < ni && v0 + 1 < nj;
-                double* p0 = Cs + v0 * CLD + u;
-                double cfr[2];
-                cfr[0] = ok0 ? p0[0] : 0.0;
-                cfr[1] = ok1 ? p0[CLD] : 0.0;
-                dmma(cfr, a0, b0);
-                dmma(cfr, a1, b1);
-                if (ok0) p0[0] = cfr[0];
-                if (ok1) p0[CLD] = cfr[1];
+                const int u = 8 * U + gid, v0 = p1 + 8 * V + 2 * tig, vb = min(p1 + 8 * V + gid, TILE - 1);
+                const bool ok0 = v0 < nj, ok1 = v0 + 1 < nj;
+                double* pc = Cs + min(v0, TILE - 2) * CLD + u;
+                const double c0v = pc[0], c1v = pc[CLD];
+                double acc[2] = {0.0, 0.0};
+#pragma unroll
+                for (int s8 = 0; s8 < 8; ++s8) {
+                    const int kc = p0 + 4 * s8 + tig;
+                    const bool kv = kc < p1;
+                    const int kcl = kv ? kc : p0;
+                    dmma(acc, kv ? Cs[kcl * CLD + u] : 0.0, kv ? Ls[kcl * CLD + vb] : 0.0);
+                }
+                if (ok0) pc[0] = c0v - acc[0];
+                if (ok1) pc[CLD] = c1v - acc[1];
             }
+            __syncthreads();
         }
-        __syncthreads();
     }
 }
 
@@ -209,40 +344,62 @@ __device__ __forceinline__ void small_front_task(const DevSym& D, const DagPlan&
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = NT / 32;
     const int c0 = D.sn_start[s], w = D.sn_start[s + 1] - c0;
     const int r = (int)(D.rows_ptr[s + 1] - D.rows_ptr[s]);
+    const int ch0 = D.child_ptr[s], ch1 = D.child_ptr[s + 1];
+    const int64_t kq0 = D.kent_ptr[s], kq1 = D.kent_ptr[s + 1];
     uint32_t* front_done = F.fac_done;
     auto colp = [sm, r](int j) { return sm + (j * r - ((j * (j - 1)) >> 1) - j); };
     const int ntri = (r * (r + 1)) >> 1;
+    int* rels = reinterpret_cast<int*>(sm + ((ntri + 1) & ~1));        // 2 x NT ints: the current / next child's relative indices
+    // everything that does not depend on the children first: zero, K entries, eta
     for (int idx = tid; idx < ntri; idx += NT) sm[idx] = 0.0;
-    const int ch0 = D.child_ptr[s], ch1 = D.child_ptr[s + 1];
-    for (int ci = ch0 + tid; ci < ch1; ci += NT) { const int c = D.child_idx[ci]; spin_until_ge(front_done + c, epoch * (uint32_t)F.target[c]); }
     __syncthreads();
-    TRACE(1);
-    for (int64_t q = D.kent_ptr[s] + tid; q < D.kent_ptr[s + 1]; q += NT) sm[D.kent_dst[q]] = Kval[D.kent_src[q]];
+    for (int64_t q = kq0 + tid; q < kq1; q += NT) sm[D.kent_dst[q]] = Kval[D.kent_src[q]];
     __syncthreads();
     if (eta != 0.0) for (int j = tid; j < w; j += NT) colp(j)[j] += eta;
+    for (int ci = ch0 + tid; ci < ch1; ci += NT) { const int c = D.child_idx[ci]; spin_until_ge(front_done + c, epoch * (uint32_t)F.target[c]); }
+    TRACE(1);
     for (int ci = ch0; ci < ch1; ++ci) {                 // extend-add, fixed child order
         const int c = D.child_idx[ci];
-        const int mc = (int)(D.rel_ptr[c + 1] - D.rel_ptr[c]);
+        const int64_t rp0 = D.rel_ptr[c];
+        const int mc = (int)(D.rel_ptr[c + 1] - rp0);
         const double* Uc = D.U + D.upd_ptr[c];
-        const int32_t* __restrict__ rel = D.rel + D.rel_ptr[c];
-        __syncthreads();
-        for (int b = warp; b < mc; b += nwarp) {
-            double* cb = colp(rel[b]);
-            const double* ub = Uc + (int64_t)b * mc;
-            for (int a = b + lane; a < mc; a += 32) cb[rel[a]] += __ldcg(ub + a);
+        int* rb = rels + NT * ((ci - ch0) & 1);
+        if (tid < mc) rb[tid] = D.rel[rp0 + tid];
+        __syncthreads();                                 // also orders the waits above / the previous child's additions
+        // columns b and mc-1-b of the child's lower triangle together hold mc+1 entries: a balanced flat index space,
+        // 8 loads in flight per thread
+        const int per = mc + 1, tot = ((mc + 1) >> 1) * per;
+        for (int f0 = tid; f0 < tot; f0 += 8 * NT) {
+            double v[8];
+            int dst[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                const int f = f0 + k * NT;
+                dst[k] = -1;
+                v[k] = 0.0;
+                if (f < tot) {
+                    const int p = f / per, e = f - p * per;
+                    int a, b;
+                    if (e < mc - p) { b = p; a = p + e; }
+                    else { b = mc - 1 - p; a = b + (e - (mc - p)); }
+                    if (b != p || e < mc - p) {          // the middle column of an odd mc is its own partner: count it once
+                        const int j = rb[b], i = rb[a];
+                        dst[k] = j * r - ((j * (j - 1)) >> 1) + (i - j);
+                        v[k] = __ldcg(Uc + a + (int64_t)b * mc);
+                    }
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < 8; ++k)
+                if (dst[k] >= 0) sm[dst[k]] += v[k];
         }
     }
     __syncthreads();
     TRACE(2);
-    partial_chol(colp, r, w, c0, D.fail_col, D.dinv, sm + ((ntri + 1) & ~1));
+    partial_chol(colp, r, w, c0, D.fail_col, D.dinv);
     TRACE(3);
     const int ld = ld_even(r), m = r - w;
-    double* P = D.L + D.panel_ptr[s];
-    for (int j = warp; j < w; j += nwarp) {
-        const double* cj = colp(j);
-        for (int i = j + lane; i < r; i += 32) P[i + (int64_t)j * ld] = cj[i];
-    }
-    double* Uo = D.U + D.upd_ptr[s];
+    double* Uo = D.U + D.upd_ptr[s];                     // the update matrix first: it is all the parent waits for
     for (int j = warp; j < m; j += nwarp) {
         const double* cj = colp(j + w) + w;
         for (int i = j + lane; i < m; i += 32) Uo[i + (int64_t)j * m] = cj[i];
@@ -251,6 +408,11 @@ __device__ __forceinline__ void small_front_task(const DevSym& D, const DagPlan&
     __syncthreads();
     if (tid == 0) red_release_add(front_done + s, 1u);
     TRACE(4);
+    double* P = D.L + D.panel_ptr[s];                    // the panel of L is read by the solves only (after the kernel)
+    for (int j = warp; j < w; j += nwarp) {
+        const double* cj = colp(j);
+        for (int i = j + lane; i < r; i += 32) P[i + (int64_t)j * ld] = cj[i];
+    }
 }
 
 // =============================================================================================================
@@ -273,7 +435,40 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
     double* pipe = sm;
     double* Cs = sm + PIPE_DOUBLES;
 
-    // ---- 1. acc = sum_{k < Kend} X(I,k) X(J,k)^T ----
+    // ---- 1. assemble the tile first (independent of the tiles to the left): zero, K entries, eta, children's update
+    //         matrices in fixed child order ----
+    for (int idx = tid; idx < CT_DOUBLES; idx += NT) Cs[idx] = 0.0;
+    const int ch0 = D.child_ptr[s], ch1 = D.child_ptr[s + 1];
+    if (J == 0) {                                        // tiles with J > 0 inherit this through the flag of tile (I,0)
+        for (int ci = ch0 + tid; ci < ch1; ci += NT) { const int c = D.child_idx[ci]; spin_until_ge(front_done + c, epoch * (uint32_t)F.target[c]); }
+    } else if (tid == 0) {
+        spin_until_ge(tdone + I, epoch);
+    }
+    __syncthreads();
+    if (J < nbp) {
+        const int64_t q0 = F.tile_kptr[F.tbase[s] + J * nbt + I], q1 = F.tile_kptr[F.tbase[s] + J * nbt + I + 1];
+        for (int64_t q = q0 + tid; q < q1; q += NT) Cs[D.kent_dst[q]] = Kval[D.kent_src[q]];
+        __syncthreads();
+        if (I == J && eta != 0.0) for (int nn = tid; nn < nj; nn += NT) Cs[nn * CLD + nn] += eta;
+    }
+    for (int ci = ch0; ci < ch1; ++ci) {
+        const int c = D.child_idx[ci];
+        const int32_t* cb = F.cbnd + F.cb_ptr[c];
+        const int a0 = cb[I], a1 = cb[I + 1], b0 = cb[J], b1 = cb[J + 1];
+        if (a0 == a1 || b0 == b1) continue;              // uniform over the CTA
+        const int mc = (int)(D.rel_ptr[c + 1] - D.rel_ptr[c]);
+        const double* Uc = D.U + D.upd_ptr[c];
+        const int32_t* __restrict__ rel = D.rel + D.rel_ptr[c];
+        __syncthreads();
+        for (int b = b0 + warp; b < b1; b += nwarp) {
+            double* cc = Cs + (rel[b] - j0) * CLD - i0;
+            const double* ub = Uc + (int64_t)b * mc;
+            for (int a = max(a0, b) + lane; a < a1; a += 32) cc[rel[a]] += __ldcg(ub + a);
+        }
+    }
+    TRACE(1);
+
+    // ---- 2. acc = sum_{k < Kend} X(I,k) X(J,k)^T ----
     double acc[2][4][2];
 #pragma unroll
     for (int a = 0; a < 2; ++a)
@@ -305,14 +500,16 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
     };
     wait_flags(0);
     wait_flags(1);
+    wait_flags(2);
     __syncthreads();
     issue(0);
     issue(1);
+    issue(2);
     for (int c = 0; c < nch; ++c) {
-        wait_flags(c + 2);
-        cp_async_wait<1>();
+        wait_flags(c + 3);
+        cp_async_wait<2>();
         __syncthreads();
-        issue(c + 2);
+        issue(c + 3);
         const double* As = pipe + (c % NSTAGE) * STAGE_DOUBLES + wm * 16 + gid + di;
         const double* Bs = pipe + (c % NSTAGE) * STAGE_DOUBLES + KC * ALD + wn * 32 + gid + dj;
 #pragma unroll
@@ -329,36 +526,8 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
         }
     }
     cp_async_wait<0>();
-    TRACE(1);
+    TRACE(2);
 
-    // ---- 2. assemble the tile: zero, K entries, eta, children's update matrices (fixed child order) ----
-    for (int idx = tid; idx < CT_DOUBLES; idx += NT) Cs[idx] = 0.0;
-    const int ch0 = D.child_ptr[s], ch1 = D.child_ptr[s + 1];
-    if (J == 0) {                                        // tiles with J > 0 inherit this through the flag of tile (I,0)
-        for (int ci = ch0 + tid; ci < ch1; ci += NT) { const int c = D.child_idx[ci]; spin_until_ge(front_done + c, epoch * (uint32_t)F.target[c]); }
-    }
-    __syncthreads();
-    if (J < nbp) {
-        const int64_t q0 = F.tile_kptr[F.tbase[s] + J * nbt + I], q1 = F.tile_kptr[F.tbase[s] + J * nbt + I + 1];
-        for (int64_t q = q0 + tid; q < q1; q += NT) Cs[D.kent_dst[q]] = Kval[D.kent_src[q]];
-        __syncthreads();
-        if (I == J && eta != 0.0) for (int nn = tid; nn < nj; nn += NT) Cs[nn * CLD + nn] += eta;
-    }
-    for (int ci = ch0; ci < ch1; ++ci) {
-        const int c = D.child_idx[ci];
-        const int32_t* cb = F.cbnd + F.cb_ptr[c];
-        const int a0 = cb[I], a1 = cb[I + 1], b0 = cb[J], b1 = cb[J + 1];
-        if (a0 == a1 || b0 == b1) continue;              // uniform over the CTA
-        const int mc = (int)(D.rel_ptr[c + 1] - D.rel_ptr[c]);
-        const double* Uc = D.U + D.upd_ptr[c];
-        const int32_t* __restrict__ rel = D.rel + D.rel_ptr[c];
-        __syncthreads();
-        for (int b = b0 + warp; b < b1; b += nwarp) {
-            double* cc = Cs + (rel[b] - j0) * CLD - i0;
-            const double* ub = Uc + (int64_t)b * mc;
-            for (int a = max(a0, b) + lane; a < a1; a += 32) cc[rel[a]] += __ldcg(ub + a);
-        }
-    }
     __syncthreads();
 #pragma unroll
     for (int mt = 0; mt < 2; ++mt)
@@ -368,11 +537,10 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
             for (int e = 0; e < 2; ++e) Cs[(wn * 32 + nt * 8 + 2 * tig + e) * CLD + wm * 16 + mt * 8 + gid] -= acc[mt][nt][e];
     __syncthreads();
 
-    TRACE(2);
     // ---- 3. finish: POTRF / TRSM for panel tiles, then store (each tile is written once) ----
     if (J < nbp) {
         if (I == J) {
-            partial_chol([Cs](int j) { return Cs + j * CLD; }, nj, nj, c0 + j0, D.fail_col, D.dinv, pipe + CT_DOUBLES + TILE);
+            partial_chol([Cs](int j) { return Cs + j * CLD; }, nj, nj, c0 + j0, D.fail_col, D.dinv);
         } else {
             double* Ls = pipe;
             double* rinv = pipe + CT_DOUBLES;
@@ -387,7 +555,7 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
                 }
             }
             __syncthreads();
-            trsm_tile(Cs, Ls, rinv, ni, nj, pipe + CT_DOUBLES + TILE);
+            trsm_tile(Cs, Ls, rinv, ni, nj);
         }
         TRACE(3);
         for (int idx = tid; idx < ni * nj; idx += NT) {
@@ -447,7 +615,7 @@ cudaError_t configure_factor_kernels(int max_smem_bytes, int* ctas_per_sm, size_
     *ctas_per_sm = occ < 1 ? 1 : occ;
     *smem_bytes = bytes;
     int rmax = 1;                                        // largest r with the packed front + the staging panel in `bytes`
-    while (rmax < NT && rmax < XLD - 8 && ((size_t)(rmax + 1) * (rmax + 2) / 2 + 1 + XS_DOUBLES) * sizeof(double) <= bytes) ++rmax;
+    while (rmax < NT && ((size_t)(rmax + 1) * (rmax + 2) / 2 + 1 + NT) * sizeof(double) <= bytes) ++rmax;   // front + 2 NT ints
     *small_max_r = rmax;
     return cudaSuccess;
 }
