@@ -40,6 +40,7 @@ struct DevSym {                   // device copies of the symbolic arrays (symbo
 
 constexpr int BIG_NB = 64;        // block size used by the triangular-solve kernels for the diagonal blocks
 constexpr int TILE = 64;          // tile size of the tiled (HBM-resident) fronts
+constexpr int SMALL_ROWS_MAX = 176;  // upper bound on the rows (leading dimension) of a front handled by one CTA in shared memory
 
 __host__ __device__ inline int ld_even(int r) { return (r + 1) & ~1; }   // = symbolic.h: panel_ld
 

@@ -604,7 +604,7 @@ __global__ void reset_fail_kernel(int32_t* fail_col) { *fail_col = INT_MAX; }
 cudaError_t configure_factor_kernels(int max_smem_bytes, int* ctas_per_sm, size_t* smem_bytes, int* small_max_r) {
     // two CTAs per SM: half of the SM's shared memory each (minus the 1 KB per-CTA reservation), at least the tile layout
     size_t bytes = (size_t)TILE_SMEM_DOUBLES * sizeof(double);
-    const size_t half = ((size_t)max_smem_bytes + 1024) / 2 - 1024 - 64;
+    const size_t half = ((size_t)max_smem_bytes + 1024) / 2 - 1024 - 256;       // 256 B of slack for the kernel's static shared memory
     if (half > bytes) bytes = half & ~(size_t)15;
     if (bytes > (size_t)max_smem_bytes) return cudaErrorInvalidValue;
     cudaError_t e = cudaFuncSetAttribute(factor_dag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
@@ -615,7 +615,7 @@ cudaError_t configure_factor_kernels(int max_smem_bytes, int* ctas_per_sm, size_
     *ctas_per_sm = occ < 1 ? 1 : occ;
     *smem_bytes = bytes;
     int rmax = 1;                                        // largest r with the packed front + the staging panel in `bytes`
-    while (rmax < NT && ((size_t)(rmax + 1) * (rmax + 2) / 2 + 1 + NT) * sizeof(double) <= bytes) ++rmax;   // front + 2 NT ints
+    while (rmax < NT && rmax + 2 <= SMALL_ROWS_MAX && ((size_t)(rmax + 1) * (rmax + 2) / 2 + 1 + NT) * sizeof(double) <= bytes) ++rmax;   // front + 2 NT ints
     *small_max_r = rmax;
     return cudaSuccess;
 }

@@ -19,9 +19,13 @@ namespace {
 
 constexpr int NT = 256;
 constexpr int DLD = 65;                 // leading dimension of the staged 64x64 diagonal tile
-constexpr int SLD = 33;                 // ... of the 32x32 diagonal block of a small supernode
-// shared memory (doubles): vec[256] | ys[64] | part[4*64] | Ld[64*65]
-constexpr int OFF_YS = 256, OFF_PART = OFF_YS + 64, OFF_LD = OFF_PART + 256, SOLVE_SMEM_DOUBLES = OFF_LD + TILE * DLD;
+constexpr int SLD = 33;                 // ... of the transposed-access copy of a 32x32 diagonal block (small supernodes)
+constexpr int SB = 32;                  // column block of the small-supernode solves
+constexpr int BUF_DOUBLES = SMALL_ROWS_MAX * SB;   // one staged column block: rows [j0, ld) x 32 columns
+// shared memory (doubles): vec[256] | ys[64] | part[4*64] | dv[2*32] | Lbt[32*33] | buf[2][BUF]  (tiled tasks: Ld[64*65] aliases buf)
+constexpr int OFF_YS = 256, OFF_PART = OFF_YS + 64, OFF_DV = OFF_PART + 256, OFF_LBT = OFF_DV + 2 * SB, OFF_BUF = OFF_LBT + SB * SLD,
+              OFF_LD = OFF_BUF, SOLVE_SMEM_DOUBLES = OFF_BUF + 2 * BUF_DOUBLES;
+static_assert(TILE * DLD <= 2 * BUF_DOUBLES, "the staged diagonal tile of the tiled tasks aliases the column-block buffers");
 constexpr unsigned FULL = 0xffffffffu;
 
 __device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
@@ -39,6 +43,18 @@ __device__ __forceinline__ void spin_until_ge(const uint32_t* p, uint32_t target
     while (ld_acquire(p) < target) __nanosleep(40);
 }
 
+__device__ __forceinline__ void cp_async16(double* dst_smem, const double* src) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async8(double* dst_smem, const double* src) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 struct Sn {                             // per-supernode scalars every task needs
     int c0, w, r, ld;
     const double* P;
@@ -52,52 +68,80 @@ __device__ __forceinline__ Sn sn_of(const DevSym& D, int s) {
     return q;
 }
 
-// ---------------- forward, whole small supernode ----------------
-__device__ __forceinline__ void fwd_small(const DevSym& D, const DagPlan& F, int s, const double* b, double* x, uint32_t epoch, double* sm) {
+// ---------------- small supernodes: column blocks of the panel are staged in shared memory ----------------
+// Column block k (columns [32k, 32k+nb), rows [32k, ld)) is copied with cp.async into buf[k & 1] (leading dimension
+// ld - 32k, 16-byte chunks: 32k and ld are even) together with the pivot reciprocals of its columns.  The first two blocks
+// are requested BEFORE the task waits for its dependencies, later ones two blocks ahead: no load from L sits on the
+// dependency chain of the solve.
+__device__ __forceinline__ void stage_block(const DevSym& D, const Sn& q, int k, double* sm) {
+    const int j0 = k * SB, nb = min(SB, q.w - j0), ldb = q.ld - j0, half = ldb >> 1;
+    double* buf = sm + OFF_BUF + (k & 1) * BUF_DOUBLES;
+    const double* src = q.P + j0 + (int64_t)j0 * q.ld;
+    for (int idx = threadIdx.x; idx < nb * half; idx += NT) {
+        const int c = idx / half, h = idx - c * half;
+        cp_async16(buf + c * ldb + 2 * h, src + (int64_t)c * q.ld + 2 * h);
+    }
+    if (threadIdx.x < nb) cp_async8(sm + OFF_DV + (k & 1) * SB + threadIdx.x, D.dinv + q.c0 + j0 + threadIdx.x);
+    cp_async_commit();
+}
+
+#define STRACE(slot) do { if (tr && threadIdx.x == 0) { unsigned long long g_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g_)); tr[slot] = g_; } } while (0)
+__device__ __forceinline__ void fwd_small(const DevSym& D, const DagPlan& F, int s, const double* b, double* x, uint32_t epoch, double* sm, unsigned long long* tr) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const Sn q = sn_of(D, s);
     double* t = sm;
-    double* Lb = sm + OFF_LD;
+    const int nblk = (q.w + SB - 1) / SB;
+    stage_block(D, q, 0, sm);
+    if (nblk > 1) stage_block(D, q, 1, sm);
     for (int i = tid; i < q.r; i += NT) t[i] = (i < q.w) ? b[D.perm[q.c0 + i]] : 0.0;
     const int ch0 = D.child_ptr[s], ch1 = D.child_ptr[s + 1];
     for (int ci = ch0 + tid; ci < ch1; ci += NT) { const int c = D.child_idx[ci]; spin_until_ge(F.sol_done_f + c, epoch * (uint32_t)F.target_f[c]); }
+    __syncthreads();
+    STRACE(1);
     for (int ci = ch0; ci < ch1; ++ci) {
         const int c = D.child_idx[ci];
-        const int mc = (int)(D.rel_ptr[c + 1] - D.rel_ptr[c]);
-        const double* cc = D.ctr + D.rel_ptr[c];
-        const int32_t* __restrict__ rel = D.rel + D.rel_ptr[c];
-        __syncthreads();
+        const int64_t rp0 = D.rel_ptr[c];
+        const int mc = (int)(D.rel_ptr[c + 1] - rp0);
+        const double* cc = D.ctr + rp0;
+        const int32_t* __restrict__ rel = D.rel + rp0;
+        if (ci > ch0) __syncthreads();
         for (int a = tid; a < mc; a += NT) t[rel[a]] += __ldcg(cc + a);
     }
-    __syncthreads();
-    for (int j0 = 0; j0 < q.w; j0 += 32) {
-        const int nb = min(32, q.w - j0);
-        for (int idx = tid; idx < nb * nb; idx += NT) {
-            const int i = idx % nb, c = idx / nb;
-            if (i >= c) Lb[c * SLD + i] = __ldcg(q.P + (j0 + i) + (int64_t)(j0 + c) * q.ld);
-        }
-        __syncthreads();
-        if (warp == 0) {
+    STRACE(2);
+    for (int k = 0; k < nblk; ++k) {
+        const int j0 = k * SB, nb = min(SB, q.w - j0), ldb = q.ld - j0;
+        const double* Bk = sm + OFF_BUF + (k & 1) * BUF_DOUBLES;
+        const double* dv = sm + OFF_DV + (k & 1) * SB;
+        if (k + 1 < nblk) cp_async_wait<1>(); else cp_async_wait<0>();
+        __syncthreads();                                 // block k has landed; t is complete up to the previous block's update
+        if (warp == 0) {                                 // L11 y = t1 on the diagonal block, one lane per row
             double tv = lane < nb ? t[j0 + lane] : 0.0;
-            const double dv = lane < nb ? __ldcg(D.dinv + q.c0 + j0 + lane) : 1.0;
+            const double dvl = lane < nb ? dv[lane] : 1.0;
+#pragma unroll 4
             for (int j = 0; j < nb; ++j) {
-                const double yj = __shfl_sync(FULL, tv * dv, j);
+                const double lij = Bk[j * ldb + min(lane, ldb - 1)];
+                const double yj = __shfl_sync(FULL, tv * dvl, j);
                 if (lane == j) tv = yj;
-                else if (lane > j && lane < nb) tv = fma(-Lb[j * SLD + lane], yj, tv);
+                else if (lane > j) tv = fma(-lij, yj, tv);
             }
-            if (lane < nb) t[j0 + lane] = tv;
+            if (lane < nb) { t[j0 + lane] = tv; x[q.c0 + j0 + lane] = tv; }
         }
         __syncthreads();
-        for (int i = j0 + nb + tid; i < q.r; i += NT) {
-            const double* Pi = q.P + i + (int64_t)j0 * q.ld;
-            double acc = 0.0;
-#pragma unroll 8
-            for (int k = 0; k < nb; ++k) acc = fma(__ldcg(Pi + (int64_t)k * q.ld), t[j0 + k], acc);
-            t[i] -= acc;
+        for (int i = j0 + nb + tid; i < q.r; i += NT) {  // t2 -= L21 y
+            const double* Bi = Bk + (i - j0);
+            double a0 = 0.0, a1 = 0.0;
+            int c = 0;
+            for (; c + 1 < nb; c += 2) { a0 = fma(Bi[c * ldb], t[j0 + c], a0); a1 = fma(Bi[(c + 1) * ldb], t[j0 + c + 1], a1); }
+            if (c < nb) a0 = fma(Bi[c * ldb], t[j0 + c], a0);
+            t[i] -= a0 + a1;
         }
-        __syncthreads();
+        if (k + 2 < nblk) {
+            __syncthreads();                             // everyone is done with buf[k & 1]
+            stage_block(D, q, k + 2, sm);
+        }
     }
-    for (int i = tid; i < q.w; i += NT) x[q.c0 + i] = t[i];
+    __syncthreads();
+    STRACE(3);
     double* co = D.ctr + D.rel_ptr[s];
     for (int i = q.w + tid; i < q.r; i += NT) co[i - q.w] = t[i];
     __threadfence();
@@ -106,6 +150,9 @@ __device__ __forceinline__ void fwd_small(const DevSym& D, const DagPlan& F, int
 }
 
 // ---------------- forward, block row I of a tiled supernode ----------------
+// Left-looking over the finished y_k.  Nothing that can be fetched early sits on the dependency chain: the children's
+// contributions are gathered first, the diagonal tile and the pivot reciprocals are staged at task start, and the 64x64
+// tile L(I,k+1) is loaded into registers BEFORE the task waits for y_k.
 __device__ __forceinline__ void fwd_tiled(const DevSym& D, const DagPlan& F, int s, int I, const double* b, double* x, uint32_t epoch, double* sm) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const Sn q = sn_of(D, s);
@@ -114,41 +161,62 @@ __device__ __forceinline__ void fwd_tiled(const DevSym& D, const DagPlan& F, int
     double* tI = sm; double* ys = sm + OFF_YS; double* part = sm + OFF_PART; double* Ld = sm + OFF_LD;
     uint32_t* bf = F.blk_f + F.bbase[s];
     const bool pivot = I < nbp;
-    if (pivot)
-        for (int idx = tid; idx < ni * ni; idx += NT) {
-            const int i = idx % ni, c = idx / ni;
-            if (i >= c) Ld[c * DLD + i] = __ldcg(q.P + (i0 + i) + (int64_t)(i0 + c) * q.ld);
+    double d0 = 1.0, d1 = 1.0;
+    if (pivot) {
+        for (int idx = tid; idx < TILE * TILE; idx += NT) {
+            const int i = idx & (TILE - 1), c = idx >> 6;
+            if (i >= c && i < ni) Ld[c * DLD + i] = __ldg(q.P + (i0 + i) + (int64_t)(i0 + c) * q.ld);
         }
-    if (tid < TILE) tI[tid] = (pivot && tid < ni) ? b[D.perm[q.c0 + i0 + tid]] : 0.0;
-    const int ch0 = D.child_ptr[s], ch1 = D.child_ptr[s + 1];
-    if (I == 0)                                          // block rows I > 0 inherit this through the flag of y_0
-        for (int ci = ch0 + tid; ci < ch1; ci += NT) { const int c = D.child_idx[ci]; spin_until_ge(F.sol_done_f + c, epoch * (uint32_t)F.target_f[c]); }
-    const int mrow = tid & 63, cg = tid >> 6;
-    const int nk = min(I, nbp);
-    double acc = 0.0;
-    for (int kb = 0; kb < nk; ++kb) {
-        if (tid == 0) spin_until_ge(bf + kb, epoch);
-        __syncthreads();
-        const int k0 = kb * TILE, nkk = min(TILE, q.w - k0);
-        if (tid < TILE) ys[tid] = tid < nkk ? __ldcg(x + q.c0 + k0 + tid) : 0.0;
-        __syncthreads();
-        if (mrow < ni) {
-            const double* Pm = q.P + (i0 + mrow) + (int64_t)k0 * q.ld;
-#pragma unroll 8
-            for (int kk = cg; kk < nkk; kk += 4) acc = fma(__ldcg(Pm + (int64_t)kk * q.ld), ys[kk], acc);
+        if (warp == 0) {
+            if (lane < ni) d0 = __ldcg(D.dinv + q.c0 + i0 + lane);
+            if (lane + 32 < ni) d1 = __ldcg(D.dinv + q.c0 + i0 + lane + 32);
         }
     }
-    part[cg * TILE + mrow] = acc;
-    for (int ci = ch0; ci < ch1; ++ci) {             // children are complete: waited above (I == 0) or through the flag of y_0
+    if (tid < TILE) tI[tid] = (pivot && tid < ni) ? b[D.perm[q.c0 + i0 + tid]] : 0.0;
+    const int ch0 = D.child_ptr[s], ch1 = D.child_ptr[s + 1];
+    if (I == 0) {                                        // block rows I > 0 inherit this through the flag of y_0
+        for (int ci = ch0 + tid; ci < ch1; ci += NT) { const int c = D.child_idx[ci]; spin_until_ge(F.sol_done_f + c, epoch * (uint32_t)F.target_f[c]); }
+    } else if (tid == 0) {
+        spin_until_ge(bf, epoch);
+    }
+    for (int ci = ch0; ci < ch1; ++ci) {
         const int c = D.child_idx[ci];
         const int32_t* cb = F.cbnd + F.cb_ptr[c];
         const int a0 = cb[I], a1 = cb[I + 1];
+        __syncthreads();                                 // orders the waits above / the previous child's additions
         if (a0 == a1) continue;
         const double* cc = D.ctr + D.rel_ptr[c];
         const int32_t* __restrict__ rel = D.rel + D.rel_ptr[c];
-        __syncthreads();
         for (int a = a0 + tid; a < a1; a += NT) tI[rel[a] - i0] += __ldcg(cc + a);
     }
+    const int mrow = tid & 63, cg = tid >> 6;
+    const int nk = min(I, nbp);
+    const bool rowok = mrow < ni;
+    double acc = 0.0;
+    double cur[16], nxt[16];
+    auto load_tile = [&](int kb, double (&v)[16]) {
+        const int k0 = kb * TILE, nkk = min(TILE, q.w - k0);
+        const double* Pm = q.P + (i0 + (rowok ? mrow : 0)) + (int64_t)k0 * q.ld;
+#pragma unroll
+        for (int e = 0; e < 16; ++e) { const int kk = cg + 4 * e; v[e] = (rowok && kk < nkk) ? __ldg(Pm + (int64_t)kk * q.ld) : 0.0; }
+    };
+    if (nk > 0) load_tile(0, cur);
+    for (int kb = 0; kb < nk; ++kb) {
+        if (kb + 1 < nk) load_tile(kb + 1, nxt);
+        if (tid < TILE) {
+            if (lane == 0) spin_until_ge(bf + kb, epoch);
+            __syncwarp();
+            const int k0 = kb * TILE;
+            ys[tid] = (k0 + tid < q.w) ? __ldcg(x + q.c0 + k0 + tid) : 0.0;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < 16; ++e) acc = fma(cur[e], ys[cg + 4 * e], acc);
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < 16; ++e) cur[e] = nxt[e];
+    }
+    part[cg * TILE + mrow] = acc;
     __syncthreads();
     if (tid < TILE) tI[tid] -= (part[tid] + part[TILE + tid]) + (part[2 * TILE + tid] + part[3 * TILE + tid]);
     __syncthreads();
@@ -156,25 +224,28 @@ __device__ __forceinline__ void fwd_tiled(const DevSym& D, const DagPlan& F, int
         if (warp == 0) {
             const bool h1 = lane + 32 < ni;
             double t0 = tI[lane], t1 = tI[lane + 32];
-            const double d0 = lane < ni ? __ldcg(D.dinv + q.c0 + i0 + lane) : 1.0, d1 = h1 ? __ldcg(D.dinv + q.c0 + i0 + lane + 32) : 1.0;
             const int n0 = min(ni, 32);
+#pragma unroll 4
             for (int j = 0; j < n0; ++j) {
+                const double l0 = Ld[j * DLD + lane], l1 = Ld[j * DLD + lane + 32];
                 const double yj = __shfl_sync(FULL, t0 * d0, j);
                 if (lane == j) t0 = yj;
-                else if (lane > j && lane < ni) t0 = fma(-Ld[j * DLD + lane], yj, t0);
-                if (h1) t1 = fma(-Ld[j * DLD + lane + 32], yj, t1);
+                else if (lane > j && lane < ni) t0 = fma(-l0, yj, t0);
+                if (h1) t1 = fma(-l1, yj, t1);
             }
+#pragma unroll 4
             for (int j = 32; j < ni; ++j) {
+                const double l1 = Ld[j * DLD + lane + 32];
                 const double yj = __shfl_sync(FULL, t1 * d1, j - 32);
                 if (lane + 32 == j) t1 = yj;
-                else if (lane + 32 > j && h1) t1 = fma(-Ld[j * DLD + lane + 32], yj, t1);
+                else if (lane + 32 > j && h1) t1 = fma(-l1, yj, t1);
             }
             if (lane < ni) x[q.c0 + i0 + lane] = t0;
             if (h1) x[q.c0 + i0 + lane + 32] = t1;
+            __threadfence();
+            __syncwarp();
+            if (lane == 0) { st_release(bf + I, epoch); red_release_add(F.sol_done_f + s, 1u); }
         }
-        __threadfence();
-        __syncthreads();
-        if (tid == 0) { st_release(bf + I, epoch); red_release_add(F.sol_done_f + s, 1u); }
     } else {
         double* co = D.ctr + D.rel_ptr[s];
         if (tid < ni) co[i0 + tid - q.w] = tI[tid];
@@ -185,47 +256,65 @@ __device__ __forceinline__ void fwd_tiled(const DevSym& D, const DagPlan& F, int
 }
 
 // ---------------- backward, whole small supernode ----------------
-__device__ __forceinline__ void bwd_small(const DevSym& D, const DagPlan& F, int s, double* b, double* x, uint32_t epoch, double* sm) {
+__device__ __forceinline__ void bwd_small(const DevSym& D, const DagPlan& F, int s, double* b, double* x, uint32_t epoch, double* sm, unsigned long long* tr) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = NT / 32;
     const Sn q = sn_of(D, s);
     double* t = sm;
-    double* Lb = sm + OFF_LD;
+    double* Lbt = sm + OFF_LBT;
+    const int nblk = (q.w + SB - 1) / SB;
+    stage_block(D, q, nblk - 1, sm);
+    if (nblk > 1) stage_block(D, q, nblk - 2, sm);
+    const int myrow = tid < q.r ? q.rows[tid] : 0;       // q.r <= SMALL_ROWS_MAX < NT: one front row per thread
     if (tid == 0) {
         spin_until_ge(F.sol_done_f + s, epoch * (uint32_t)F.target_f[s]);
         const int p = F.sn_parent[s];
         if (p >= 0) spin_until_ge(F.sol_done_b + p, epoch * (uint32_t)F.target_b[p]);
     }
     __syncthreads();
-    for (int i = tid; i < q.r; i += NT) t[i] = __ldcg(x + q.rows[i]);
-    __syncthreads();
-    const int nblk = (q.w + 31) / 32;
-    for (int bk = nblk - 1; bk >= 0; --bk) {
-        const int j0 = bk * 32, nb = min(32, q.w - j0);
-        for (int idx = tid; idx < nb * nb; idx += NT) {
-            const int i = idx % nb, c = idx / nb;
-            if (i >= c) Lb[c * SLD + i] = __ldcg(q.P + (j0 + i) + (int64_t)(j0 + c) * q.ld);
+    STRACE(1);
+    if (tid < q.r) t[tid] = __ldcg(x + myrow);
+    STRACE(2);
+    for (int k = nblk - 1; k >= 0; --k) {
+        const int j0 = k * SB, nb = min(SB, q.w - j0), ldb = q.ld - j0;
+        const double* Bk = sm + OFF_BUF + (k & 1) * BUF_DOUBLES;
+        const double* dv = sm + OFF_DV + (k & 1) * SB;
+        if (k > 0) cp_async_wait<1>(); else cp_async_wait<0>();
+        __syncthreads();                                 // block k has landed; t holds y1 and the finished x below
+        for (int idx = tid; idx < nb * SB; idx += NT) {  // padded copy of the diagonal block for the row-wise accesses below
+            const int c = idx >> 5, i = idx & 31;
+            if (i >= c && i < nb) Lbt[c * SLD + i] = Bk[c * ldb + i];
         }
-        for (int c = warp; c < nb; c += nwarp) {         // z_c = y_c - sum_{i >= j0+nb} L[i, j0+c] t_i
-            const double* Pc = q.P + (int64_t)(j0 + c) * q.ld;
-            double acc = 0.0;
-            for (int i = j0 + nb + lane; i < q.r; i += 32) acc = fma(__ldcg(Pc + i), t[i], acc);
+        for (int c = warp; c < nb; c += nwarp) {         // z_c = y_c - sum_{i >= j0+nb} L[i, j0+c] x_i
+            const double* Bc = Bk + c * ldb - j0;
+            double a0 = 0.0, a1 = 0.0;
+            int i = j0 + nb + lane;
+            for (; i + 32 < q.r; i += 64) { a0 = fma(Bc[i], t[i], a0); a1 = fma(Bc[i + 32], t[i + 32], a1); }
+            if (i < q.r) a0 = fma(Bc[i], t[i], a0);
+            a0 += a1;
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(FULL, acc, o);
-            if (lane == 0) t[j0 + c] -= acc;
+            for (int o = 16; o > 0; o >>= 1) a0 += __shfl_xor_sync(FULL, a0, o);
+            if (lane == 0) t[j0 + c] -= a0;
         }
         __syncthreads();
-        if (warp == 0) {
+        if (warp == 0) {                                 // L11^T x1 = z on the diagonal block
             double zv = lane < nb ? t[j0 + lane] : 0.0;
-            const double dv = lane < nb ? __ldcg(D.dinv + q.c0 + j0 + lane) : 1.0;
+            const double dvl = lane < nb ? dv[lane] : 1.0;
+#pragma unroll 4
             for (int j = nb - 1; j >= 0; --j) {
-                const double xj = __shfl_sync(FULL, zv * dv, j);
+                const double lji = Lbt[lane * SLD + j];
+                const double xj = __shfl_sync(FULL, zv * dvl, j);
                 if (lane == j) zv = xj;
-                else if (lane < j) zv = fma(-Lb[lane * SLD + j], xj, zv);
+                else if (lane < j) zv = fma(-lji, xj, zv);
             }
             if (lane < nb) t[j0 + lane] = zv;
         }
-        __syncthreads();
+        if (k >= 2) {
+            __syncthreads();                             // everyone is done with buf[k & 1]
+            stage_block(D, q, k - 2, sm);
+        }
     }
+    __syncthreads();
+    STRACE(3);
     for (int i = tid; i < q.w; i += NT) { x[q.c0 + i] = t[i]; b[D.perm[q.c0 + i]] = t[i]; }
     __threadfence();
     __syncthreads();
@@ -233,6 +322,7 @@ __device__ __forceinline__ void bwd_small(const DevSym& D, const DagPlan& F, int
 }
 
 // ---------------- backward, block column J of a tiled supernode ----------------
+// x_J = L(J,J)^-T (y_J - sum_{I>J} L(I,J)^T x_I): the tile L(I-1,J) is loaded into registers before the task waits for x_I.
 __device__ __forceinline__ void bwd_tiled(const DevSym& D, const DagPlan& F, int s, int J, double* b, double* x, uint32_t epoch, double* sm) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const Sn q = sn_of(D, s);
@@ -240,35 +330,55 @@ __device__ __forceinline__ void bwd_tiled(const DevSym& D, const DagPlan& F, int
     const int j0 = J * TILE, nj = min(TILE, q.w - j0);
     double* xs = sm + OFF_YS; double* zs = sm; double* Ld = sm + OFF_LD;
     uint32_t* bb = F.blk_b + F.bbase[s];
-    for (int idx = tid; idx < nj * nj; idx += NT) {
-        const int i = idx % nj, c = idx / nj;
-        if (i >= c) Ld[c * DLD + i] = __ldcg(q.P + (j0 + i) + (int64_t)(j0 + c) * q.ld);
+    for (int idx = tid; idx < TILE * TILE; idx += NT) {
+        const int i = idx & (TILE - 1), c = idx >> 6;
+        if (i >= c && i < nj) Ld[c * DLD + i] = __ldg(q.P + (j0 + i) + (int64_t)(j0 + c) * q.ld);
     }
+    double d0 = 1.0, d1 = 1.0;
+    if (warp == 0) {
+        if (lane < nj) d0 = __ldcg(D.dinv + q.c0 + j0 + lane);
+        if (lane + 32 < nj) d1 = __ldcg(D.dinv + q.c0 + j0 + lane + 32);
+    }
+    double cur[16], nxt[16];
+    auto load_tile = [&](int I, double (&v)[16]) {
+        const int i0 = tile_bound(I, q.w, q.r, nbp), ni = tile_bound(I + 1, q.w, q.r, nbp) - i0;
+#pragma unroll
+        for (int e = 0; e < 8; ++e) {
+            const int c = warp * 8 + e;
+            const double* Pc = q.P + i0 + (int64_t)(j0 + min(c, nj - 1)) * q.ld;
+            v[2 * e] = (c < nj && lane < ni) ? __ldg(Pc + lane) : 0.0;
+            v[2 * e + 1] = (c < nj && lane + 32 < ni) ? __ldg(Pc + lane + 32) : 0.0;
+        }
+    };
+    if (nbt - 1 > J) load_tile(nbt - 1, cur);
     if (tid == 0) {
         spin_until_ge(F.sol_done_f + s, epoch * (uint32_t)F.target_f[s]);
         const int p = F.sn_parent[s];
         if (p >= 0) spin_until_ge(F.sol_done_b + p, epoch * (uint32_t)F.target_b[p]);   // the rows below belong to finished ancestors
     }
+    __syncthreads();
     double acc[8];
 #pragma unroll
     for (int e = 0; e < 8; ++e) acc[e] = 0.0;
     for (int I = nbt - 1; I > J; --I) {
-        if (I < nbp && tid == 0) spin_until_ge(bb + I, epoch);
-        __syncthreads();
+        if (I - 1 > J) load_tile(I - 1, nxt);
         const int i0 = tile_bound(I, q.w, q.r, nbp), ni = tile_bound(I + 1, q.w, q.r, nbp) - i0;
-        if (tid < TILE) xs[tid] = tid < ni ? __ldcg(x + q.rows[i0 + tid]) : 0.0;
-        __syncthreads();
-#pragma unroll
-        for (int e = 0; e < 8; ++e) {
-            const int c = warp * 8 + e;
-            if (c < nj) {
-                const double* Pc = q.P + i0 + (int64_t)(j0 + c) * q.ld;
-                if (lane < ni) acc[e] = fma(__ldcg(Pc + lane), xs[lane], acc[e]);
-                if (lane + 32 < ni) acc[e] = fma(__ldcg(Pc + lane + 32), xs[lane + 32], acc[e]);
+        if (tid < TILE) {
+            if (I < nbp) {
+                if (lane == 0) spin_until_ge(bb + I, epoch);
+                __syncwarp();
+                xs[tid] = tid < ni ? __ldcg(x + q.c0 + i0 + tid) : 0.0;
+            } else {
+                xs[tid] = tid < ni ? __ldcg(x + q.rows[i0 + tid]) : 0.0;
             }
         }
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < 8; ++e) acc[e] = fma(cur[2 * e + 1], xs[lane + 32], fma(cur[2 * e], xs[lane], acc[e]));
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < 16; ++e) cur[e] = nxt[e];
     }
-    __syncthreads();                                     // also orders thread 0's waits when the loop above is empty
 #pragma unroll
     for (int e = 0; e < 8; ++e) {
         double v = acc[e];
@@ -281,27 +391,30 @@ __device__ __forceinline__ void bwd_tiled(const DevSym& D, const DagPlan& F, int
     if (warp == 0) {
         const bool h1 = lane + 32 < nj;
         double z0 = lane < nj ? zs[lane] : 0.0, z1 = h1 ? zs[lane + 32] : 0.0;
-        const double d0 = lane < nj ? __ldcg(D.dinv + q.c0 + j0 + lane) : 1.0, d1 = h1 ? __ldcg(D.dinv + q.c0 + j0 + lane + 32) : 1.0;
+#pragma unroll 4
         for (int j = nj - 1; j >= 32; --j) {
+            const double l1 = Ld[(lane + 32) * DLD + j], l0 = Ld[lane * DLD + j];
             const double xj = __shfl_sync(FULL, z1 * d1, j - 32);
             if (lane + 32 == j) z1 = xj;
-            else if (lane + 32 < j) z1 = fma(-Ld[(lane + 32) * DLD + j], xj, z1);
-            z0 = fma(-Ld[lane * DLD + j], xj, z0);
+            else if (lane + 32 < j) z1 = fma(-l1, xj, z1);
+            z0 = fma(-l0, xj, z0);
         }
+#pragma unroll 4
         for (int j = min(nj, 32) - 1; j >= 0; --j) {
+            const double l0 = Ld[lane * DLD + j];
             const double xj = __shfl_sync(FULL, z0 * d0, j);
             if (lane == j) z0 = xj;
-            else if (lane < j) z0 = fma(-Ld[lane * DLD + j], xj, z0);
+            else if (lane < j) z0 = fma(-l0, xj, z0);
         }
         if (lane < nj) { x[q.c0 + j0 + lane] = z0; b[D.perm[q.c0 + j0 + lane]] = z0; }
         if (h1) { x[q.c0 + j0 + lane + 32] = z1; b[D.perm[q.c0 + j0 + lane + 32]] = z1; }
+        __threadfence();
+        __syncwarp();
+        if (lane == 0) { st_release(bb + J, epoch); red_release_add(F.sol_done_b + s, 1u); }
     }
-    __threadfence();
-    __syncthreads();
-    if (tid == 0) { st_release(bb + J, epoch); red_release_add(F.sol_done_b + s, 1u); }
 }
 
-__global__ void __launch_bounds__(NT) solve_dag_kernel(DevSym D, DagPlan F, double* b, double* x, uint32_t epoch) {
+__global__ void __launch_bounds__(NT, 2) solve_dag_kernel(DevSym D, DagPlan F, double* b, double* x, uint32_t epoch) {
     extern __shared__ __align__(16) double sm[];
     __shared__ int s_task;
     const uint32_t base = (epoch - 1u) * (uint32_t)(F.n_stasks + (int)gridDim.x);
@@ -314,8 +427,8 @@ __global__ void __launch_bounds__(NT) solve_dag_kernel(DevSym D, DagPlan F, doub
         const int4 tk = F.stasks[t];
         unsigned long long* tr = F.strace ? F.strace + (size_t)t * 8 : nullptr;
         if (tr && threadIdx.x == 0) { unsigned long long g; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g)); tr[0] = g; }
-        if (tk.w == 0) { if (tk.x == 0) fwd_small(D, F, tk.y, b, x, epoch, sm); else fwd_tiled(D, F, tk.y, tk.z, b, x, epoch, sm); }
-        else           { if (tk.x == 0) bwd_small(D, F, tk.y, b, x, epoch, sm); else bwd_tiled(D, F, tk.y, tk.z, b, x, epoch, sm); }
+        if (tk.w == 0) { if (tk.x == 0) fwd_small(D, F, tk.y, b, x, epoch, sm, tr); else fwd_tiled(D, F, tk.y, tk.z, b, x, epoch, sm); }
+        else           { if (tk.x == 0) bwd_small(D, F, tk.y, b, x, epoch, sm, tr); else bwd_tiled(D, F, tk.y, tk.z, b, x, epoch, sm); }
         if (tr && threadIdx.x == 0) { unsigned long long g; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g)); tr[4] = g; }
     }
 }
