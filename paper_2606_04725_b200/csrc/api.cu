@@ -314,10 +314,14 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
         int num_sms = 0, ctas_per_sm = 1, small_max_r = 0;
         size_t factor_smem = 0;
         CK(cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev));
-        CK(configure_factor_kernels(smem_optin, &ctas_per_sm, &factor_smem, &small_max_r));
-        int solve_ctas = 1; size_t solve_smem = 0;
-        CK(configure_solve_kernels(smem_optin, &solve_ctas, &solve_smem));
+        // latency mode: a small problem (dependency-latency bound) whose largest fronts fit the whole
+        // shared memory of an SM keeps every front in the one-CTA kernel family; else two CTAs per SM and tiled big fronts
+        const bool latency_mode = S.flops <= 1e8 && S.max_front <= SMALL_ROWS_MAX - 2 && h->opt.smem_front_max <= 0;
+        CK(configure_factor_kernels(smem_optin, latency_mode, &ctas_per_sm, &factor_smem, &small_max_r));
         if (h->opt.smem_front_max > 0) small_max_r = std::min(small_max_r, h->opt.smem_front_max);
+        int solve_ctas = 1, sbuf = 0; size_t solve_smem = 0;
+        CK(configure_solve_kernels(smem_optin, small_max_r, &solve_ctas, &solve_smem, &sbuf));
+        h->F.sbuf = sbuf;
         DevSym& D = h->D;
         D.ns = S.ns; D.n = S.n;
         TRY(upload(h, S.sn_start, &D.sn_start)); TRY(upload(h, S.rows_ptr, &D.rows_ptr)); TRY(upload(h, S.rows, &D.rows));

@@ -40,7 +40,7 @@ struct DevSym {                   // device copies of the symbolic arrays (symbo
 
 constexpr int BIG_NB = 64;        // block size used by the triangular-solve kernels for the diagonal blocks
 constexpr int TILE = 64;          // tile size of the tiled (HBM-resident) fronts
-constexpr int SMALL_ROWS_MAX = 176;  // upper bound on the rows (leading dimension) of a front handled by one CTA in shared memory
+constexpr int SMALL_ROWS_MAX = 240;  // upper bound on the rows (leading dimension) of a front handled by one CTA in shared memory
 
 __host__ __device__ inline int ld_even(int r) { return (r + 1) & ~1; }   // = symbolic.h: panel_ld
 
@@ -92,16 +92,18 @@ struct DagPlan {
     unsigned long long* strace = nullptr;
     int64_t sync_words = 0;
     int32_t small_max_r = 0;
+    int32_t sbuf = 0;                    // doubles per staged column block of the small-supernode solves
     int32_t fgrid = 0, sgrid = 0;
     size_t fsmem = 0, ssmem = 0;
 };
 
 // ---- factor.cu ----
-cudaError_t configure_factor_kernels(int max_smem_bytes, int* ctas_per_sm, size_t* smem_bytes, int* small_max_r);
+// one_cta_per_sm: latency mode (small problems whose largest fronts then fit one CTA's shared memory), else two CTAs per SM
+cudaError_t configure_factor_kernels(int max_smem_bytes, bool one_cta_per_sm, int* ctas_per_sm, size_t* smem_bytes, int* small_max_r);
 void launch_factor(const DevSym& D, const DagPlan& F, const double* Kval, double eta, uint32_t epoch, cudaStream_t st);
 void launch_reset_fail(const DevSym& D, cudaStream_t st);                                   // fail_col = INT_MAX
 // ---- solve.cu ----
-cudaError_t configure_solve_kernels(int max_smem_bytes, int* ctas_per_sm, size_t* smem_bytes);
+cudaError_t configure_solve_kernels(int max_smem_bytes, int small_max_r, int* ctas_per_sm, size_t* smem_bytes, int* sbuf_doubles);
 // rhs_inout (original ordering, n doubles) is overwritten by K^-1 rhs; x is the handle's permuted work vector
 void launch_solve(const DevSym& D, const DagPlan& F, double* rhs_inout, double* x, uint32_t epoch, cudaStream_t st);
 

@@ -74,77 +74,84 @@ __device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
 
 // =============================================================================================================
 // Blocked partial Cholesky of the first w columns of an r x r lower-stored matrix in shared memory (Eq. 21).
-// colp(j)[i] addresses element (i,j), i >= j.  Two-level blocking: panels of 32 columns, sub-steps of 8 columns.
-//   sub-step, phase 1: every thread factors the 8x8 diagonal block redundantly in registers (identical arithmetic ->
-//            identical values, no barrier; 1/sqrt by rsqrt, L_jj = d * rsqrt(d)); thread t solves row j0+t of the block
-//            column against it (x = f L_D^-T); barrier;
-//   sub-step, phase 2: rank-8 DMMA update of the REST OF THE PANEL only (<= 24 columns); barrier;
-//   panel end: rank-32 DMMA update of the trailing columns, 8 chained mma.m8n8k4 per 8x8 tile.
-// DMMA operands come straight from the finished columns of the front; tiles are dealt round-robin to the warps, two in
-// flight per warp.  Requires r <= NT.  A pivot <= 0 or non-finite (reading G11) is replaced by 1 and reported.
+// colp(j)[i] addresses element (i,j), i >= j.  Two-level blocking: panels of 32 columns, sub-steps of 8 columns, and the
+// factorization of the NEXT 8x8 diagonal block is software-pipelined into the update of the current sub-step:
+//   row solve:   thread t solves row j0+t of the block column against the finished diagonal block (x = f L_D^-T); barrier;
+//   update:      rank-8 DMMA update of the rest of the panel (<= 24 columns); at a panel end the rank-32 DMMA update of the
+//                trailing columns (8 chained mma.m8n8k4 per 8x8 tile).  Warp 0 takes the tile that holds the next diagonal
+//                block first and then factors that block in registers (serial pivot chain: hardware rsqrt + two Newton
+//                steps, L_jj = d * rsqrt(d)) while warps 1..7 work through the other tiles, two in flight per warp; barrier.
+// DMMA operands come straight from the finished columns of the front, loads are unconditional with clamped indices
+// (no divergence).  Requires r <= NT.  A pivot <= 0 or non-finite (reading G11) is replaced by 1 and reported.
 // =============================================================================================================
+template <class ColFn>
+__device__ __forceinline__ void factor_diag8(ColFn colp, int j0, int jb, int c0, int32_t* fail_col, double* dinv, double* s_inv) {
+    const int lane = threadIdx.x & 31;
+    double Dg[8][8], inv[8];
+    if (jb == 8) {
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            const double* cp = colp(j0 + c) + j0;
+#pragma unroll
+            for (int i = c; i < 8; ++i) Dg[i][c] = cp[i];
+        }
+    } else {
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            const double* cp = colp(j0 + min(c, jb - 1)) + j0;
+#pragma unroll
+            for (int i = c; i < 8; ++i) { const double v = cp[min(i, jb - 1)]; Dg[i][c] = (i < jb) ? v : (i == c ? 1.0 : 0.0); }   // i < jb implies c < jb
+        }
+    }
+    int badc = 8;
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        const double d = Dg[c][c];
+        const bool bad = !(d >= 2.2250738585072014e-308) || isinf(d);          // <= 0, non-finite (or subnormal): reading G11
+        if (bad && c < jb && badc == 8) badc = c;
+        const double y = rsqrt_newton(d);                                      // speculative: the test above is off the chain
+        inv[c] = bad ? 1.0 : y;
+        Dg[c][c] = bad ? 1.0 : d * y;
+#pragma unroll
+        for (int i = c + 1; i < 8; ++i) Dg[i][c] *= inv[c];
+#pragma unroll
+        for (int k = c + 1; k < 8; ++k)
+#pragma unroll
+            for (int i = k; i < 8; ++i) Dg[i][k] = fma(-Dg[i][c], Dg[k][c], Dg[i][k]);
+    }
+    if (badc < 8 && lane == 0) atomicMin(fail_col, c0 + j0 + badc);
+    double mine = inv[0];
+#pragma unroll
+    for (int c = 1; c < 8; ++c) mine = (lane == c) ? inv[c] : mine;
+    if (lane < jb) { dinv[c0 + j0 + lane] = mine; s_inv[lane] = mine; }
+    if (lane == 0) {                                     // one lane stores the factored block (immediate offsets, no branches)
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            double* cp = colp(j0 + min(c, jb - 1)) + j0;
+#pragma unroll
+            for (int i = c; i < 8; ++i)
+                if (i < jb) cp[i] = Dg[i][c];
+        }
+    }
+}
+
 template <class ColFn>
 __device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, int32_t* fail_col, double* dinv) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gid = lane >> 2, tig = lane & 3;
-    constexpr int NW = NT / 32;
+    constexpr int NW1 = NT / 32 - 1;                     // warps 1..7 share the tiles warp 0 does not take
     __shared__ double s_inv[8];
     const int rl = r - 1;
+    if (warp == 0) factor_diag8(colp, 0, min(8, w), c0, fail_col, dinv, s_inv);
+    __syncthreads();
     for (int p0 = 0; p0 < w; p0 += 32) {
         const int p1 = min(w, p0 + 32);
         for (int j0 = p0; j0 < p1; j0 += 8) {
             const int jb = min(8, p1 - j0);
             const int t0 = j0 + jb;
-            const bool full = jb == 8;
-            if (warp == 0) {                             // phase 1a: the 8x8 diagonal block, in registers
-                double Dg[8][8], inv[8];
-                if (full) {
-#pragma unroll
-                    for (int c = 0; c < 8; ++c) {
-                        const double* cp = colp(j0 + c) + j0;
-#pragma unroll
-                        for (int i = c; i < 8; ++i) Dg[i][c] = cp[i];
-                    }
-                } else {
-#pragma unroll
-                    for (int c = 0; c < 8; ++c) {
-                        const double* cp = colp(j0 + min(c, jb - 1)) + j0;
-#pragma unroll
-                        for (int i = c; i < 8; ++i) { const double v = cp[min(i, jb - 1)]; Dg[i][c] = (i < jb) ? v : (i == c ? 1.0 : 0.0); }   // i < jb implies c < jb
-                    }
-                }
-                bool bad = false;
-                int badc = 8;
-#pragma unroll
-                for (int c = 0; c < 8; ++c) {
-                    double d = Dg[c][c];
-                    if (!(d >= 2.2250738585072014e-308) || isinf(d)) {   // <= 0, non-finite (or subnormal): reading G11
-                        d = 1.0;
-                        if (!bad && c < jb) { bad = true; badc = c; }
-                    }
-                    inv[c] = rsqrt_newton(d);
-                    Dg[c][c] = d * inv[c];
-#pragma unroll
-                    for (int i = c + 1; i < 8; ++i) Dg[i][c] *= inv[c];
-#pragma unroll
-                    for (int k = c + 1; k < 8; ++k)
-#pragma unroll
-                        for (int i = k; i < 8; ++i) Dg[i][k] = fma(-Dg[i][c], Dg[k][c], Dg[i][k]);
-                }
-                if (bad && lane == 0) atomicMin(fail_col, c0 + j0 + badc);
-#pragma unroll
-                for (int ii = 0; ii < 8; ++ii)
-                    if (lane == ii && ii < jb) {         // lane ii stores row ii of L_D and the pivot reciprocal
-                        dinv[c0 + j0 + ii] = inv[ii];
-                        s_inv[ii] = inv[ii];
-#pragma unroll
-                        for (int c = 0; c <= ii; ++c) colp(j0 + c)[j0 + ii] = Dg[ii][c];
-                    }
-            }
-            __syncthreads();
-            if (tid >= jb && j0 + tid < r) {             // phase 1b: a row below: x = f L_D^-T (right-looking over the 8 columns)
+            if (tid >= jb && j0 + tid < r) {             // a row below the diagonal block: x = f L_D^-T (right-looking over the 8 columns)
                 const int i = j0 + tid;
                 double x[8], Lk[8][8], inv[8];
-                if (full) {
+                if (jb == 8) {
 #pragma unroll
                     for (int c = 0; c < 8; ++c) {
                         const double* cp = colp(j0 + c);
@@ -175,21 +182,23 @@ __device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, i
                     if (c < jb) colp(j0 + c)[i] = x[c];
             }
             __syncthreads();
-            if (t0 < p1) {                               // phase 2: rank-8 update of the panel's remaining columns [t0, p1)
+            const bool has_next = t0 < w;
+            if (t0 < p1) {                               // rank-8 update of the panel's remaining columns [t0, p1)
                 const bool k0 = tig < jb, k1 = tig + 4 < jb;
                 const double* ck0 = colp(j0 + (k0 ? tig : 0));
                 const double* ck1 = colp(j0 + (k1 ? tig + 4 : 0));
                 const int TU = (r - t0 + 7) >> 3, TV = (p1 - t0 + 7) >> 3, ntile = TU * TV;
-                for (int qb = warp; qb < ntile; qb += 2 * NW) {
+                auto pair = [&](int qa, int qb) {
                     double acc[2][2], cold[2][2];
                     double* pc[2][2];
                     bool ok[2][2];
 #pragma unroll
                     for (int e = 0; e < 2; ++e) {
-                        const int q = min(qb + e * NW, ntile - 1);
+                        const int qq = e ? qb : qa;
+                        const int q = min(qq, ntile - 1);
                         const int V = q / TU, U = q - V * TU;
                         const int u = t0 + 8 * U + gid, vb = t0 + 8 * V + gid, vc = t0 + 8 * V + 2 * tig;
-                        const bool live = qb + e * NW < ntile && U >= V;
+                        const bool live = qq < ntile && U >= V;
                         const int ucl = min(u, rl), vbl = min(vb, rl);
                         const double a0 = ck0[ucl], a1 = ck1[ucl], b0 = ck0[vbl], b1 = ck1[vbl];
                         ok[e][0] = live && u < r && vc < p1 && u >= vc;
@@ -207,50 +216,63 @@ __device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, i
                         if (ok[e][0]) *pc[e][0] = cold[e][0] - acc[e][0];
                         if (ok[e][1]) *pc[e][1] = cold[e][1] - acc[e][1];
                     }
+                };
+                if (warp == 0) {
+                    pair(0, ntile);                      // the tile of the next diagonal block, then that block's factorization
+                    __syncwarp();
+                    factor_diag8(colp, t0, min(8, p1 - t0), c0, fail_col, dinv, s_inv);
+                } else {
+                    for (int q = warp; q < ntile; q += 2 * NW1) pair(q, q + NW1);
                 }
-                __syncthreads();
-            }
-        }
-        if (p1 < r) {                                    // panel end: rank-(p1-p0) update of the trailing columns [p1, r)
-            const double* ck[8];
-            bool kv[8];
+            } else if (p1 < r) {                         // panel end: rank-(p1-p0) update of the trailing columns [p1, r)
+                const double* ck[8];
+                bool kv[8];
 #pragma unroll
-            for (int s8 = 0; s8 < 8; ++s8) { const int kc = p0 + 4 * s8 + tig; kv[s8] = kc < p1; ck[s8] = colp(kv[s8] ? kc : p0); }
-            const int T = (r - p1 + 7) >> 3, ntile = (T * (T + 1)) >> 1;
-            for (int qb = warp; qb < ntile; qb += 2 * NW) {
-                double acc[2][2], cold[2][2];
-                double* pc[2][2];
-                bool ok[2][2];
-                int ucl[2], vbl[2];
+                for (int s8 = 0; s8 < 8; ++s8) { const int kc = p0 + 4 * s8 + tig; kv[s8] = kc < p1; ck[s8] = colp(kv[s8] ? kc : p0); }
+                const int T = (r - p1 + 7) >> 3, ntile = (T * (T + 1)) >> 1;
+                auto pair = [&](int qa, int qb) {
+                    double acc[2][2], cold[2][2];
+                    double* pc[2][2];
+                    bool ok[2][2];
+                    int ucl[2], vbl[2];
 #pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    const int q = min(qb + e * NW, ntile - 1);
-                    int U = (int)((sqrtf(8.0f * (float)q + 1.0f) - 1.0f) * 0.5f);
-                    U += (((U + 1) * (U + 2)) >> 1 <= q) - (((U * (U + 1)) >> 1) > q);      // float rounding: off by at most one
-                    const int V = q - ((U * (U + 1)) >> 1);
-                    const bool live = qb + e * NW < ntile;
-                    const int u = p1 + 8 * U + gid, vb = p1 + 8 * V + gid, vc = p1 + 8 * V + 2 * tig;
-                    ucl[e] = min(u, rl); vbl[e] = min(vb, rl);
-                    ok[e][0] = live && u < r && vc < r && u >= vc;
-                    ok[e][1] = live && u < r && vc + 1 < r && u >= vc + 1;
-                    pc[e][0] = colp(min(vc, rl)) + ucl[e];
-                    pc[e][1] = colp(min(vc + 1, rl)) + ucl[e];
-                    cold[e][0] = *pc[e][0];
-                    cold[e][1] = *pc[e][1];
-                    acc[e][0] = acc[e][1] = 0.0;
-                }
+                    for (int e = 0; e < 2; ++e) {
+                        const int qq = e ? qb : qa;
+                        const int q = min(qq, ntile - 1);
+                        int U = (int)((sqrtf(8.0f * (float)q + 1.0f) - 1.0f) * 0.5f);
+                        U += (((U + 1) * (U + 2)) >> 1 <= q) - (((U * (U + 1)) >> 1) > q);      // float rounding: off by at most one
+                        const int V = q - ((U * (U + 1)) >> 1);
+                        const bool live = qq < ntile;
+                        const int u = p1 + 8 * U + gid, vb = p1 + 8 * V + gid, vc = p1 + 8 * V + 2 * tig;
+                        ucl[e] = min(u, rl); vbl[e] = min(vb, rl);
+                        ok[e][0] = live && u < r && vc < r && u >= vc;
+                        ok[e][1] = live && u < r && vc + 1 < r && u >= vc + 1;
+                        pc[e][0] = colp(min(vc, rl)) + ucl[e];
+                        pc[e][1] = colp(min(vc + 1, rl)) + ucl[e];
+                        cold[e][0] = *pc[e][0];
+                        cold[e][1] = *pc[e][1];
+                        acc[e][0] = acc[e][1] = 0.0;
+                    }
 #pragma unroll
-                for (int s8 = 0; s8 < 8; ++s8) {
-                    double a[2], b[2];
+                    for (int s8 = 0; s8 < 8; ++s8) {
+                        double a[2], b[2];
 #pragma unroll
-                    for (int e = 0; e < 2; ++e) { a[e] = ck[s8][ucl[e]]; b[e] = ck[s8][vbl[e]]; }
+                        for (int e = 0; e < 2; ++e) { a[e] = ck[s8][ucl[e]]; b[e] = ck[s8][vbl[e]]; }
 #pragma unroll
-                    for (int e = 0; e < 2; ++e) dmma(acc[e], kv[s8] ? a[e] : 0.0, kv[s8] ? b[e] : 0.0);
-                }
+                        for (int e = 0; e < 2; ++e) dmma(acc[e], kv[s8] ? a[e] : 0.0, kv[s8] ? b[e] : 0.0);
+                    }
 #pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    if (ok[e][0]) *pc[e][0] = cold[e][0] - acc[e][0];
-                    if (ok[e][1]) *pc[e][1] = cold[e][1] - acc[e][1];
+                    for (int e = 0; e < 2; ++e) {
+                        if (ok[e][0]) *pc[e][0] = cold[e][0] - acc[e][0];
+                        if (ok[e][1]) *pc[e][1] = cold[e][1] - acc[e][1];
+                    }
+                };
+                if (warp == 0) {
+                    pair(0, ntile);
+                    __syncwarp();
+                    if (has_next) factor_diag8(colp, p1, min(8, w - p1), c0, fail_col, dinv, s_inv);
+                } else {
+                    for (int q = warp; q < ntile; q += 2 * NW1) pair(q, q + NW1);
                 }
             }
             __syncthreads();
@@ -601,20 +623,22 @@ __global__ void reset_fail_kernel(int32_t* fail_col) { *fail_col = INT_MAX; }
 
 }  // namespace
 
-cudaError_t configure_factor_kernels(int max_smem_bytes, int* ctas_per_sm, size_t* smem_bytes, int* small_max_r) {
-    // two CTAs per SM: half of the SM's shared memory each (minus the 1 KB per-CTA reservation), at least the tile layout
+cudaError_t configure_factor_kernels(int max_smem_bytes, bool one_cta_per_sm, int* ctas_per_sm, size_t* smem_bytes, int* small_max_r) {
+    // two CTAs per SM: half of the SM's shared memory each (minus the 1 KB per-CTA reservation), at least the tile layout;
+    // latency mode: one CTA per SM with all of it, so that fronts up to SMALL_ROWS_MAX rows stay in shared memory
     size_t bytes = (size_t)TILE_SMEM_DOUBLES * sizeof(double);
     const size_t half = ((size_t)max_smem_bytes + 1024) / 2 - 1024 - 256;       // 256 B of slack for the kernel's static shared memory
-    if (half > bytes) bytes = half & ~(size_t)15;
+    const size_t avail = one_cta_per_sm ? (size_t)max_smem_bytes - 256 : half;
+    if (avail > bytes) bytes = avail & ~(size_t)15;
     if (bytes > (size_t)max_smem_bytes) return cudaErrorInvalidValue;
-    cudaError_t e = cudaFuncSetAttribute(factor_dag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    cudaError_t e = cudaFuncSetAttribute(factor_dag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes - 256);
     if (e != cudaSuccess) return e;
     int occ = 0;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, factor_dag_kernel, NT, bytes);
     if (e != cudaSuccess) return e;
     *ctas_per_sm = occ < 1 ? 1 : occ;
     *smem_bytes = bytes;
-    int rmax = 1;                                        // largest r with the packed front + the staging panel in `bytes`
+    int rmax = 1;                                        // largest r with the packed front + the relative-index buffers in `bytes`
     while (rmax < NT && rmax + 2 <= SMALL_ROWS_MAX && ((size_t)(rmax + 1) * (rmax + 2) / 2 + 1 + NT) * sizeof(double) <= bytes) ++rmax;   // front + 2 NT ints
     *small_max_r = rmax;
     return cudaSuccess;

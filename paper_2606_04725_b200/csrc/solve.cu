@@ -21,11 +21,10 @@ constexpr int NT = 256;
 constexpr int DLD = 65;                 // leading dimension of the staged 64x64 diagonal tile
 constexpr int SLD = 33;                 // ... of the transposed-access copy of a 32x32 diagonal block (small supernodes)
 constexpr int SB = 32;                  // column block of the small-supernode solves
-constexpr int BUF_DOUBLES = SMALL_ROWS_MAX * SB;   // one staged column block: rows [j0, ld) x 32 columns
-// shared memory (doubles): vec[256] | ys[64] | part[4*64] | dv[2*32] | Lbt[32*33] | buf[2][BUF]  (tiled tasks: Ld[64*65] aliases buf)
+// shared memory (doubles): vec[256] | ys[64] | part[4*64] | dv[2*32] | Lbt[32*33] | buf[2][DagPlan::sbuf]
+// (one staged column block: rows [j0, ld) x 32 columns; tiled tasks: Ld[64*65] aliases buf)
 constexpr int OFF_YS = 256, OFF_PART = OFF_YS + 64, OFF_DV = OFF_PART + 256, OFF_LBT = OFF_DV + 2 * SB, OFF_BUF = OFF_LBT + SB * SLD,
-              OFF_LD = OFF_BUF, SOLVE_SMEM_DOUBLES = OFF_BUF + 2 * BUF_DOUBLES;
-static_assert(TILE * DLD <= 2 * BUF_DOUBLES, "the staged diagonal tile of the tiled tasks aliases the column-block buffers");
+              OFF_LD = OFF_BUF;
 constexpr unsigned FULL = 0xffffffffu;
 
 __device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
@@ -73,9 +72,9 @@ __device__ __forceinline__ Sn sn_of(const DevSym& D, int s) {
 // ld - 32k, 16-byte chunks: 32k and ld are even) together with the pivot reciprocals of its columns.  The first two blocks
 // are requested BEFORE the task waits for its dependencies, later ones two blocks ahead: no load from L sits on the
 // dependency chain of the solve.
-__device__ __forceinline__ void stage_block(const DevSym& D, const Sn& q, int k, double* sm) {
+__device__ __forceinline__ void stage_block(const DevSym& D, const Sn& q, int k, double* sm, int sbuf) {
     const int j0 = k * SB, nb = min(SB, q.w - j0), ldb = q.ld - j0, half = ldb >> 1;
-    double* buf = sm + OFF_BUF + (k & 1) * BUF_DOUBLES;
+    double* buf = sm + OFF_BUF + (k & 1) * sbuf;
     const double* src = q.P + j0 + (int64_t)j0 * q.ld;
     for (int idx = threadIdx.x; idx < nb * half; idx += NT) {
         const int c = idx / half, h = idx - c * half;
@@ -91,8 +90,8 @@ __device__ __forceinline__ void fwd_small(const DevSym& D, const DagPlan& F, int
     const Sn q = sn_of(D, s);
     double* t = sm;
     const int nblk = (q.w + SB - 1) / SB;
-    stage_block(D, q, 0, sm);
-    if (nblk > 1) stage_block(D, q, 1, sm);
+    stage_block(D, q, 0, sm, F.sbuf);
+    if (nblk > 1) stage_block(D, q, 1, sm, F.sbuf);
     for (int i = tid; i < q.r; i += NT) t[i] = (i < q.w) ? b[D.perm[q.c0 + i]] : 0.0;
     const int ch0 = D.child_ptr[s], ch1 = D.child_ptr[s + 1];
     for (int ci = ch0 + tid; ci < ch1; ci += NT) { const int c = D.child_idx[ci]; spin_until_ge(F.sol_done_f + c, epoch * (uint32_t)F.target_f[c]); }
@@ -110,7 +109,7 @@ __device__ __forceinline__ void fwd_small(const DevSym& D, const DagPlan& F, int
     STRACE(2);
     for (int k = 0; k < nblk; ++k) {
         const int j0 = k * SB, nb = min(SB, q.w - j0), ldb = q.ld - j0;
-        const double* Bk = sm + OFF_BUF + (k & 1) * BUF_DOUBLES;
+        const double* Bk = sm + OFF_BUF + (k & 1) * F.sbuf;
         const double* dv = sm + OFF_DV + (k & 1) * SB;
         if (k + 1 < nblk) cp_async_wait<1>(); else cp_async_wait<0>();
         __syncthreads();                                 // block k has landed; t is complete up to the previous block's update
@@ -137,7 +136,7 @@ __device__ __forceinline__ void fwd_small(const DevSym& D, const DagPlan& F, int
         }
         if (k + 2 < nblk) {
             __syncthreads();                             // everyone is done with buf[k & 1]
-            stage_block(D, q, k + 2, sm);
+            stage_block(D, q, k + 2, sm, F.sbuf);
         }
     }
     __syncthreads();
@@ -262,8 +261,8 @@ __device__ __forceinline__ void bwd_small(const DevSym& D, const DagPlan& F, int
     double* t = sm;
     double* Lbt = sm + OFF_LBT;
     const int nblk = (q.w + SB - 1) / SB;
-    stage_block(D, q, nblk - 1, sm);
-    if (nblk > 1) stage_block(D, q, nblk - 2, sm);
+    stage_block(D, q, nblk - 1, sm, F.sbuf);
+    if (nblk > 1) stage_block(D, q, nblk - 2, sm, F.sbuf);
     const int myrow = tid < q.r ? q.rows[tid] : 0;       // q.r <= SMALL_ROWS_MAX < NT: one front row per thread
     if (tid == 0) {
         spin_until_ge(F.sol_done_f + s, epoch * (uint32_t)F.target_f[s]);
@@ -276,7 +275,7 @@ __device__ __forceinline__ void bwd_small(const DevSym& D, const DagPlan& F, int
     STRACE(2);
     for (int k = nblk - 1; k >= 0; --k) {
         const int j0 = k * SB, nb = min(SB, q.w - j0), ldb = q.ld - j0;
-        const double* Bk = sm + OFF_BUF + (k & 1) * BUF_DOUBLES;
+        const double* Bk = sm + OFF_BUF + (k & 1) * F.sbuf;
         const double* dv = sm + OFF_DV + (k & 1) * SB;
         if (k > 0) cp_async_wait<1>(); else cp_async_wait<0>();
         __syncthreads();                                 // block k has landed; t holds y1 and the finished x below
@@ -310,7 +309,7 @@ __device__ __forceinline__ void bwd_small(const DevSym& D, const DagPlan& F, int
         }
         if (k >= 2) {
             __syncthreads();                             // everyone is done with buf[k & 1]
-            stage_block(D, q, k - 2, sm);
+            stage_block(D, q, k - 2, sm, F.sbuf);
         }
     }
     __syncthreads();
@@ -435,16 +434,20 @@ __global__ void __launch_bounds__(NT, 2) solve_dag_kernel(DevSym D, DagPlan F, d
 
 }  // namespace
 
-cudaError_t configure_solve_kernels(int max_smem_bytes, int* ctas_per_sm, size_t* smem_bytes) {
-    const size_t bytes = (size_t)SOLVE_SMEM_DOUBLES * sizeof(double);
+cudaError_t configure_solve_kernels(int max_smem_bytes, int small_max_r, int* ctas_per_sm, size_t* smem_bytes, int* sbuf_doubles) {
+    int sbuf = ld_even(small_max_r) * SB;
+    if (2 * sbuf < TILE * DLD) sbuf = (TILE * DLD + 1) / 2 + 1;      // the staged diagonal tile of the tiled tasks aliases the buffers
+    sbuf = (sbuf + 1) & ~1;
+    const size_t bytes = (size_t)(OFF_BUF + 2 * sbuf) * sizeof(double);
     if (bytes > (size_t)max_smem_bytes) return cudaErrorInvalidValue;
-    cudaError_t e = cudaFuncSetAttribute(solve_dag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    cudaError_t e = cudaFuncSetAttribute(solve_dag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes - 256);
     if (e != cudaSuccess) return e;
     int occ = 0;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, solve_dag_kernel, NT, bytes);
     if (e != cudaSuccess) return e;
     *ctas_per_sm = occ < 1 ? 1 : occ;
     *smem_bytes = bytes;
+    *sbuf_doubles = sbuf;
     return cudaSuccess;
 }
 
