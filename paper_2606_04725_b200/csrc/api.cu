@@ -588,6 +588,39 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
     int it = 0, nfact = 0, retries = 0;
     nmpc_status status = NMPC_E_MAXITER;
     double* hs = h->h_pinned;
+    // Without phase timing the factorization's pivot flag is NOT read back right after the factorization: the solve, the
+    // step and the (device-guarded) update are enqueued behind it and the flag travels with the next iteration's residual
+    // scalars -- one host synchronisation per IPM iteration.  A failed pivot leaves the iterate untouched (update_kernel
+    // checks the flag), so the inertia-correction retry below starts from exactly the state of the synchronous flow.
+    const bool async = !o.time_phases;
+    bool pending = false;                                // a factorization whose flag has not been checked yet
+    double pend_mu = 0.0, pend_tau = 0.0;
+    int32_t* flag = reinterpret_cast<int32_t*>(h->h_pinned + 16);
+    auto retry_with_eta = [&](double& eta) -> nmpc_status {   // S7: inertia correction, Eq. (13)/(15); synchronous
+        while (true) {
+            ++retries;
+            if (eta == 0.0) eta = (eta_last == 0.0) ? o.eta_first : std::max(o.eta_min, o.eta_shrink * eta_last);
+            else eta = ((eta_last == 0.0) ? o.eta_grow_first : o.eta_grow) * eta;
+            if (eta > o.eta_max) return NMPC_E_INERTIA;
+            ++nfact;
+            pt.begin(&S.ms_factor);
+            nmpc_status fs = run_factor(h, eta, nullptr);
+            pt.end();
+            if (fs == NMPC_OK) return NMPC_OK;
+            if (fs != NMPC_E_NOT_SPD) return fs;
+        }
+    };
+    auto solve_step_update = [&](double mu_, double tau_) -> nmpc_status {
+        pt.begin(&S.ms_solve);                                                 // S8: Eq. (22)-(25)
+        CK(cudaMemcpyAsync(V.dy, V.b, sizeof(double) * M.n, cudaMemcpyDeviceToDevice, st));
+        TRY(run_solve(h, V.dy));
+        pt.end();
+        pt.begin(&S.ms_vector);
+        launch_step(M, V, mu_, tau_, st); h->launches += 2;                    // S8-S9
+        launch_update(M, V, h->D.fail_col, st); h->launches++;                 // S10: Eq. (26)
+        pt.end();
+        return NMPC_OK;
+    };
     while (true) {
         // S2: evaluate c, grad f, J, W (K_SIMD of the paper, Alg. 2 line 5) and the residuals of Eq. (9)
         pt.begin(&S.ms_eval);
@@ -596,8 +629,25 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
         pt.begin(&S.ms_vector);
         launch_residuals(M, V, o.gamma, st); h->launches += 2;
         CK(cudaMemcpyAsync(hs, V.scal, sizeof(double) * 10, cudaMemcpyDeviceToHost, st));
+        if (pending) CK(cudaMemcpyAsync(flag, h->D.fail_col, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
         pt.end();
+        if (pending) {
+            pending = false;
+            if (*flag != INT_MAX) {                      // the step of iteration it-1 was not taken: redo it with eta > 0
+                h->factored = false;
+                launch_reset_fail(h->D, st); h->launches += 1;
+                double eta = 0.0;
+                nmpc_status rs = retry_with_eta(eta);
+                if (rs == NMPC_E_INERTIA) { status = rs; goto done; }
+                if (rs != NMPC_OK) return rs;
+                eta_last = eta;
+                TRY(solve_step_update(pend_mu, pend_tau));
+                if (trace && it - 1 < trace_cap) trace[it - 1].eta = eta;
+                continue;                                // re-evaluate at the new iterate
+            }
+            h->factored = true; h->eta_cur = 0.0;
+        }
         if (it > 0 && trace && it - 1 < trace_cap) { trace[it - 1].alpha_pr = hs[7]; trace[it - 1].alpha_du = hs[8]; }
         if (hs[6] != 0.0) { status = NMPC_E_STEP; break; }
         const double l1 = hs[5];
@@ -621,28 +671,25 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
         pt.begin(&S.ms_assemble);
         launch_assemble_K(M, V.Jval, V.Wval, V.sigx, V.q, 0.0, V.Kval, st); h->launches++;
         pt.end();
-        double eta = 0.0;                                                      // S7: inertia correction, Eq. (13)/(15)
-        while (true) {
-            ++nfact;
+        double eta = 0.0;
+        ++nfact;
+        if (async) {
+            uint32_t epoch = 0;
+            TRY(next_epoch(h, true, &epoch));
+            launch_factor(h->D, h->F, h->d_Kval, 0.0, epoch, st); h->launches += 1;
+            pending = true; pend_mu = mu; pend_tau = tau;
+        } else {
             pt.begin(&S.ms_factor);
-            nmpc_status fs = run_factor(h, eta, nullptr);
+            nmpc_status fs = run_factor(h, 0.0, nullptr);
             pt.end();
-            if (fs == NMPC_OK) break;
-            if (fs != NMPC_E_NOT_SPD) return fs;
-            ++retries;
-            if (eta == 0.0) eta = (eta_last == 0.0) ? o.eta_first : std::max(o.eta_min, o.eta_shrink * eta_last);
-            else eta = ((eta_last == 0.0) ? o.eta_grow_first : o.eta_grow) * eta;
-            if (eta > o.eta_max) { status = NMPC_E_INERTIA; goto done; }
+            if (fs == NMPC_E_NOT_SPD) {
+                nmpc_status rs = retry_with_eta(eta);
+                if (rs == NMPC_E_INERTIA) { status = rs; goto done; }
+                if (rs != NMPC_OK) return rs;
+            } else if (fs != NMPC_OK) return fs;
         }
         if (eta > 0.0) eta_last = eta;
-        pt.begin(&S.ms_solve);                                                 // S8: Eq. (22)-(25)
-        CK(cudaMemcpyAsync(V.dy, V.b, sizeof(double) * M.n, cudaMemcpyDeviceToDevice, st));
-        TRY(run_solve(h, V.dy));
-        pt.end();
-        pt.begin(&S.ms_vector);
-        launch_step(M, V, mu, tau, st); h->launches += 2;                      // S8-S9
-        launch_update(M, V, st); h->launches++;                                // S10: Eq. (26)
-        pt.end();
+        TRY(solve_step_update(mu, tau));
         if (trace && it < trace_cap) { trace[it].mu = mu; trace[it].E0 = E0; trace[it].Emu = Emu; trace[it].eta = eta; trace[it].alpha_pr = trace[it].alpha_du = 0.0; }
         ++it;
     }

@@ -144,7 +144,8 @@ void launch_warm_push(const DevModel& M, const IpmVectors& V, double warm_push, 
 void launch_residuals(const DevModel& M, const IpmVectors& V, double gamma, cudaStream_t st);
 void launch_sigma_rhs(const DevModel& M, const IpmVectors& V, double mu, cudaStream_t st);
 void launch_step(const DevModel& M, const IpmVectors& V, double mu, double tau, cudaStream_t st);
-void launch_update(const DevModel& M, const IpmVectors& V, cudaStream_t st);
+// fail_col (may be null): device flag of the factorization; the update is skipped when it reports a failed pivot
+void launch_update(const DevModel& M, const IpmVectors& V, const int32_t* fail_col, cudaStream_t st);
 void launch_objective(const DevModel& M, const IpmVectors& V, cudaStream_t st);
 
 }  // namespace nmpc

@@ -70,6 +70,7 @@ __global__ void __launch_bounds__(NT) assemble_K_kernel(DevModel M, const double
     const int64_t e = blockIdx.x * (int64_t)NT + threadIdx.x;
     if (e >= M.nnzK) return;
     double acc = 0.0;
+#pragma unroll 16
     for (int64_t p = M.trip_ptr[e]; p < M.trip_ptr[e + 1]; ++p)
         acc += Jval[M.trip_a[p]] * q[M.trip_r[p]] * Jval[M.trip_b[p]];
     const int wi = M.k_w[e], di = M.k_diag[e];
@@ -172,6 +173,7 @@ __global__ void __launch_bounds__(NT) residual_kernel(DevModel M, IpmVectors V, 
         if (idx < M.n) {
             const int64_t i = idx;
             double jt = 0.0;
+#pragma unroll 16
             for (int64_t p = M.jt_ptr[i]; p < M.jt_ptr[i + 1]; ++p) { const int r = M.jt_row[p]; jt += V.Jval[M.jt_idx[p]] * (V.wp[r] - V.wm[r]); }
             const double lb = M.lb[i], ub = M.ub[i], y = V.y[i];
             const bool hasL = lb > -INF, hasU = ub < INF;
@@ -225,6 +227,7 @@ __global__ void __launch_bounds__(NT) sigma_vars_kernel(DevModel M, IpmVectors V
     const int64_t i = blockIdx.x * (int64_t)NT + threadIdx.x;
     if (i >= M.n) return;
     double jt = 0.0;
+#pragma unroll 16
     for (int64_t p = M.jt_ptr[i]; p < M.jt_ptr[i + 1]; ++p) jt += V.Jval[M.jt_idx[p]] * V.t[M.jt_row[p]];
     const double lb = M.lb[i], ub = M.ub[i], y = V.y[i];
     const bool hasL = lb > -INF, hasU = ub < INF;
@@ -283,7 +286,8 @@ __global__ void __launch_bounds__(NT) finalize_step_kernel(IpmVectors V, int nbl
 }
 
 // S10: Eq. (26) with the step lengths read from device memory
-__global__ void __launch_bounds__(NT) update_kernel(DevModel M, IpmVectors V) {
+__global__ void __launch_bounds__(NT) update_kernel(DevModel M, IpmVectors V, const int32_t* __restrict__ fail_col) {
+    if (fail_col && *fail_col != INT_MAX) return;        // the factorization behind this step met a bad pivot: keep the iterate
     const double apr = V.scal[7], adu = V.scal[8];
     const int64_t idx = blockIdx.x * (int64_t)NT + threadIdx.x;
     if (idx < M.n) {
@@ -353,8 +357,8 @@ void launch_step(const DevModel& M, const IpmVectors& V, double mu, double tau, 
     step_kernel<<<nb, NT, 0, st>>>(M, V, mu, tau);
     finalize_step_kernel<<<1, NT, 0, st>>>(V, nb);
 }
-void launch_update(const DevModel& M, const IpmVectors& V, cudaStream_t st) {
-    update_kernel<<<blocks_for(M.n + M.m), NT, 0, st>>>(M, V);
+void launch_update(const DevModel& M, const IpmVectors& V, const int32_t* fail_col, cudaStream_t st) {
+    update_kernel<<<blocks_for(M.n + M.m), NT, 0, st>>>(M, V, fail_col);
 }
 void launch_objective(const DevModel& M, const IpmVectors& V, cudaStream_t st) {
     const int nb = red_blocks(M.n);
