@@ -51,6 +51,7 @@ def parse():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-extra", action="store_true", help="skip the short per-config summary of the other workloads")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the cpu_baseline sample")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs of the large workloads)")
     return ap.parse_args()
 
 
@@ -61,6 +62,19 @@ def measured_peaks():
             d = json.load(f)
         return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
     return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def profiled_traffic(kernel, workload):
+    """DRAM bytes per launch of `kernel` on `workload` from the committed `ncu --set full` summary (profiles/traffic.json,
+    written by hand from profiles/*_full.md); None when no capture of that pair is on file."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        with open(p) as f:
+            d = json.load(f)
+        e = d[workload][kernel]
+        return {"bytes_per_launch": float(e["dram_read_bytes"]) + float(e["dram_write_bytes"]), "source": e["source"]}
+    except (OSError, KeyError, ValueError):
+        return None
 
 
 def replica_x0(cfg, rank):
@@ -385,6 +399,7 @@ def run_own(args):
 
     value = dev_ms_max * 1e3 / max(1, tot_it)
     e2e = host_ms_max * 1e3 / max(1, tot_it)
+    tr_f, tr_s = profiled_traffic("factor_dag_kernel", cfg.name), profiled_traffic("solve_dag_kernel", cfg.name)
     ms_per_step = dev_ms_max / max(1, K)
     flops = float(info["flops"])
     line = {
@@ -414,19 +429,25 @@ def run_own(args):
         "wall_s_whole_loop": wall_s,
         "roofline": {"bound": "alu", "kernel": "numeric supernodal Cholesky (all launches of one factorization)",
                      "achieved": flops / factor_us * 1e-6, "peak": FP64_DERIVED_TFLOPS, "unit": "TFLOP/s",
-                     "frac": flops / factor_us * 1e-6 / FP64_DERIVED_TFLOPS, "traffic": None,
+                     "frac": flops / factor_us * 1e-6 / FP64_DERIVED_TFLOPS,
+                     "traffic": tr_f["bytes_per_launch"] if tr_f else None, "traffic_source": tr_f["source"] if tr_f else None,
+                     "note": "C0/C1/C4 are dependency-latency bound (DESIGN.md section 7): the floor of this kernel at peak is "
+                             "flops/peak; the large-front workloads C2/C3 are the ones the fp64 pipe bounds (other_workloads)",
                      "peak_source": "derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md section 7)",
                      "peak_live_dfma_tflops": dfma_tf, "peak_live_dmma_tflops": dmma_tf,
                      "flops_per_launch": flops, "avg_launch_us": factor_us},
         "roofline_solve": {"bound": "hbm", "kernel": "supernodal forward+backward triangular solves",
                            "achieved": 16.0 * info["nnz_L"] / solve_us * 1e-3, "peak": hbm_peak, "unit": "GB/s",
-                           "frac": 16.0 * info["nnz_L"] / solve_us * 1e-3 / hbm_peak, "traffic": None,
+                           "frac": 16.0 * info["nnz_L"] / solve_us * 1e-3 / hbm_peak,
+                           "traffic": tr_s["bytes_per_launch"] if tr_s else None, "traffic_source": tr_s["source"] if tr_s else None,
                            "peak_source": peak_src, "bytes_per_launch": 16.0 * info["nnz_L"], "avg_launch_us": solve_us},
         "clocks": clocks,
     }
 
     # ---- CPU oracle on a bounded sample of the same workload (rank 0, N = 1 only) ----
-    if world == 1:
+    if world == 1 and args.no_cpu:
+        line["cpu_baseline"] = None
+    elif world == 1:
         warm_s, warm_it, warm_n, cold_s, cold_it, ls = oracle_loop(cfg, K, 1, args.cpu_seconds, x0=x0_first)
         line["cpu_baseline"] = {
             "value": warm_s * 1e6 / max(1, warm_it), "unit": UNIT, "cores": oracle_threads() if ls == "blocktri" else 1,
@@ -444,6 +465,16 @@ def run_own(args):
                 except Exception as e:  # noqa: BLE001  (a summary must not take the bench line down)
                     extra[name] = {"error": str(e)}
             line["other_workloads"] = extra
+            big = extra.get("C3", {})
+            if "factor_us" in big:                        # the workload the fp64 pipe / HBM actually bound
+                tf3, ts3 = profiled_traffic("factor_dag_kernel", "C3"), profiled_traffic("solve_dag_kernel", "C3")
+                line["roofline_c3"] = {
+                    "factor": {"bound": "alu", "achieved": big["factor_tflops"], "peak": FP64_DERIVED_TFLOPS, "unit": "TFLOP/s",
+                               "frac": big["factor_frac_fp64"], "traffic": tf3["bytes_per_launch"] if tf3 else None,
+                               "flops_per_launch": big["flops_per_factor"], "avg_launch_us": big["factor_us"]},
+                    "solve": {"bound": "hbm", "achieved": big["solve_gbs"], "peak": hbm_peak, "unit": "GB/s",
+                              "frac": big["solve_frac_hbm"], "traffic": ts3["bytes_per_launch"] if ts3 else None,
+                              "bytes_per_launch": 16.0 * big["nnz_L"], "avg_launch_us": big["solve_us"]}}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
