@@ -116,12 +116,20 @@ __device__ __forceinline__ void fwd_small(const DevSym& D, const DagPlan& F, int
         if (warp == 0) {                                 // L11 y = t1 on the diagonal block, one lane per row
             double tv = lane < nb ? t[j0 + lane] : 0.0;
             const double dvl = lane < nb ? dv[lane] : 1.0;
-#pragma unroll 4
-            for (int j = 0; j < nb; ++j) {
-                const double lij = Bk[j * ldb + min(lane, ldb - 1)];
-                const double yj = __shfl_sync(FULL, tv * dvl, j);
-                if (lane == j) tv = yj;
-                else if (lane > j) tv = fma(-lij, yj, tv);
+            // pre-scaled substitution: s_i = d_i t_i, s_i -= (d_i L_ij) y_j; only (shuffle, fma) on the chain, the scaled
+            // column entries are loaded 8 columns ahead
+            tv *= dvl;
+            const int lcl = min(lane, ldb - 1);
+            for (int jb = 0; jb < nb; jb += 8) {
+                double lj[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) lj[e] = Bk[min(jb + e, nb - 1) * ldb + lcl] * dvl;
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int j = jb + e;
+                    const double yj = __shfl_sync(FULL, tv, j & 31);
+                    tv = (lane > j && j < nb) ? fma(-lj[e], yj, tv) : tv;
+                }
             }
             if (lane < nb) { t[j0 + lane] = tv; x[q.c0 + j0 + lane] = tv; }
         }
@@ -224,20 +232,33 @@ __device__ __forceinline__ void fwd_tiled(const DevSym& D, const DagPlan& F, int
             const bool h1 = lane + 32 < ni;
             double t0 = tI[lane], t1 = tI[lane + 32];
             const int n0 = min(ni, 32);
-#pragma unroll 4
-            for (int j = 0; j < n0; ++j) {
-                const double l0 = Ld[j * DLD + lane], l1 = Ld[j * DLD + lane + 32];
-                const double yj = __shfl_sync(FULL, t0 * d0, j);
-                if (lane == j) t0 = yj;
-                else if (lane > j && lane < ni) t0 = fma(-l0, yj, t0);
-                if (h1) t1 = fma(-l1, yj, t1);
+            // pre-scaled substitution (s_i = d_i t_i): only (shuffle, fma) on the chain, scaled entries loaded 8 columns ahead
+            t0 = lane < ni ? t0 * d0 : 0.0;
+            t1 = h1 ? t1 * d1 : 0.0;
+            const int r0 = min(lane, ni - 1), r1 = min(lane + 32, ni - 1);
+            for (int jb = 0; jb < n0; jb += 8) {
+                double la[8], lb[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) { const int jc = min(jb + e, ni - 1); la[e] = Ld[jc * DLD + r0] * d0; lb[e] = Ld[jc * DLD + r1] * d1; }
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int j = jb + e;
+                    const double yj = __shfl_sync(FULL, t0, j & 31);
+                    const bool on = j < n0;
+                    t0 = (on && lane > j && lane < ni) ? fma(-la[e], yj, t0) : t0;
+                    t1 = (on && h1) ? fma(-lb[e], yj, t1) : t1;
+                }
             }
-#pragma unroll 4
-            for (int j = 32; j < ni; ++j) {
-                const double l1 = Ld[j * DLD + lane + 32];
-                const double yj = __shfl_sync(FULL, t1 * d1, j - 32);
-                if (lane + 32 == j) t1 = yj;
-                else if (lane + 32 > j && h1) t1 = fma(-l1, yj, t1);
+            for (int jb = 32; jb < ni; jb += 8) {
+                double lb[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) lb[e] = Ld[min(jb + e, ni - 1) * DLD + r1] * d1;
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int j = jb + e;
+                    const double yj = __shfl_sync(FULL, t1, (j - 32) & 31);
+                    t1 = (j < ni && lane + 32 > j && h1) ? fma(-lb[e], yj, t1) : t1;
+                }
             }
             if (lane < ni) x[q.c0 + i0 + lane] = t0;
             if (h1) x[q.c0 + i0 + lane + 32] = t1;
@@ -298,12 +319,17 @@ __device__ __forceinline__ void bwd_small(const DevSym& D, const DagPlan& F, int
         if (warp == 0) {                                 // L11^T x1 = z on the diagonal block
             double zv = lane < nb ? t[j0 + lane] : 0.0;
             const double dvl = lane < nb ? dv[lane] : 1.0;
-#pragma unroll 4
-            for (int j = nb - 1; j >= 0; --j) {
-                const double lji = Lbt[lane * SLD + j];
-                const double xj = __shfl_sync(FULL, zv * dvl, j);
-                if (lane == j) zv = xj;
-                else if (lane < j) zv = fma(-lji, xj, zv);
+            zv *= dvl;                                   // pre-scaled: s_i = d_i z_i, s_i -= (d_i L_ji) x_j for i < j
+            for (int jb = ((nb - 1) >> 3) << 3; jb >= 0; jb -= 8) {
+                double lj[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) lj[e] = Lbt[lane * SLD + min(jb + e, nb - 1)] * dvl;
+#pragma unroll
+                for (int e = 7; e >= 0; --e) {
+                    const int j = jb + e;
+                    const double xj = __shfl_sync(FULL, zv, j & 31);
+                    zv = (lane < j && j < nb) ? fma(-lj[e], xj, zv) : zv;
+                }
             }
             if (lane < nb) t[j0 + lane] = zv;
         }
@@ -390,20 +416,32 @@ __device__ __forceinline__ void bwd_tiled(const DevSym& D, const DagPlan& F, int
     if (warp == 0) {
         const bool h1 = lane + 32 < nj;
         double z0 = lane < nj ? zs[lane] : 0.0, z1 = h1 ? zs[lane + 32] : 0.0;
-#pragma unroll 4
-        for (int j = nj - 1; j >= 32; --j) {
-            const double l1 = Ld[(lane + 32) * DLD + j], l0 = Ld[lane * DLD + j];
-            const double xj = __shfl_sync(FULL, z1 * d1, j - 32);
-            if (lane + 32 == j) z1 = xj;
-            else if (lane + 32 < j) z1 = fma(-l1, xj, z1);
-            z0 = fma(-l0, xj, z0);
+        // pre-scaled substitution (s_i = d_i z_i): only (shuffle, fma) on the chain, scaled entries loaded 8 rows ahead
+        z0 *= d0; z1 *= d1;
+        const int c0l = min(lane, nj - 1), c1l = min(lane + 32, nj - 1);
+        for (int jb = ((nj - 1) >> 3) << 3; jb >= 32; jb -= 8) {
+            double la[8], lb[8];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) { const int jr = min(jb + e, nj - 1); la[e] = Ld[c0l * DLD + jr] * d0; lb[e] = Ld[c1l * DLD + jr] * d1; }
+#pragma unroll
+            for (int e = 7; e >= 0; --e) {
+                const int j = jb + e;
+                const double xj = __shfl_sync(FULL, z1, (j - 32) & 31);
+                const bool on = j < nj;
+                z1 = (on && lane + 32 < j) ? fma(-lb[e], xj, z1) : z1;
+                z0 = (on && lane < nj) ? fma(-la[e], xj, z0) : z0;
+            }
         }
-#pragma unroll 4
-        for (int j = min(nj, 32) - 1; j >= 0; --j) {
-            const double l0 = Ld[lane * DLD + j];
-            const double xj = __shfl_sync(FULL, z0 * d0, j);
-            if (lane == j) z0 = xj;
-            else if (lane < j) z0 = fma(-l0, xj, z0);
+        for (int jb = ((min(nj, 32) - 1) >> 3) << 3; jb >= 0; jb -= 8) {
+            double la[8];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) la[e] = Ld[c0l * DLD + min(jb + e, nj - 1)] * d0;
+#pragma unroll
+            for (int e = 7; e >= 0; --e) {
+                const int j = jb + e;
+                const double xj = __shfl_sync(FULL, z0, j & 31);
+                z0 = (j < min(nj, 32) && lane < j) ? fma(-la[e], xj, z0) : z0;
+            }
         }
         if (lane < nj) { x[q.c0 + j0 + lane] = z0; b[D.perm[q.c0 + j0 + lane]] = z0; }
         if (h1) { x[q.c0 + j0 + lane + 32] = z1; b[D.perm[q.c0 + j0 + lane + 32]] = z1; }
