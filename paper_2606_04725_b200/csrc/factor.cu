@@ -22,6 +22,9 @@ namespace nmpc {
 namespace {
 
 constexpr int NT = 256;                 // threads per CTA
+constexpr int MAXCH = 24;               // children whose tables a small-front task keeps in shared memory (else: one by one)
+constexpr int RELCAP = 2048;            // total relative indices of those children
+constexpr int SMALL_WORK_DOUBLES = (2 * MAXCH * 8 + (2 * MAXCH + 4) * 4 + RELCAP * 4 + 7) / 8;
 constexpr int KC = 16;                  // k-columns per pipeline stage
 constexpr int ALD = 68;                 // leading dimension of an operand stage  (68 mod 16 == 4: conflict-free DMMA fragment loads)
 constexpr int CLD = 66;                 // leading dimension of the C / L_JJ tile (2*66 mod 16 == 4: conflict-free fragment stores)
@@ -371,49 +374,132 @@ __device__ __forceinline__ void small_front_task(const DevSym& D, const DagPlan&
     uint32_t* front_done = F.fac_done;
     auto colp = [sm, r](int j) { return sm + (j * r - ((j * (j - 1)) >> 1) - j); };
     const int ntri = (r * (r + 1)) >> 1;
-    int* rels = reinterpret_cast<int*>(sm + ((ntri + 1) & ~1));        // 2 x NT ints: the current / next child's relative indices
-    // everything that does not depend on the children first: zero, K entries, eta
+    // work area behind the front: child table + the relative indices of ALL children (fetched before the children are waited for)
+    long long* chRp = reinterpret_cast<long long*>(sm + ((ntri + 1) & ~1));   // [MAXCH] rel_ptr of the child
+    long long* chUp = chRp + MAXCH;                                           // [MAXCH] upd_ptr of the child
+    int* chMc = reinterpret_cast<int*>(chUp + MAXCH);                         // [MAXCH] rows of the child's update matrix
+    int* chOff = chMc + MAXCH;                                                // [MAXCH + 1] offset of its list in relS
+    int* relS = chOff + MAXCH + 2;                                            // [RELCAP] (fast path) / 2 x NT (fallback)
+    const int nch = ch1 - ch0;
+    // everything that does not depend on the children first: zero, K entries, eta, child table, relative indices
     for (int idx = tid; idx < ntri; idx += NT) sm[idx] = 0.0;
+    int myc = -1;
+    if (tid < nch) {
+        myc = D.child_idx[ch0 + tid];
+        if (nch <= MAXCH) {
+            const long long rp0 = D.rel_ptr[myc];
+            chRp[tid] = rp0; chMc[tid] = (int)(D.rel_ptr[myc + 1] - rp0); chUp[tid] = D.upd_ptr[myc];
+        }
+    }
     __syncthreads();
     for (int64_t q = kq0 + tid; q < kq1; q += NT) sm[D.kent_dst[q]] = Kval[D.kent_src[q]];
+    if (tid == 0 && nch <= MAXCH) { int off = 0; for (int i = 0; i < nch; ++i) { chOff[i] = off; off += chMc[i]; } chOff[nch] = off; }
     __syncthreads();
     if (eta != 0.0) for (int j = tid; j < w; j += NT) colp(j)[j] += eta;
-    for (int ci = ch0 + tid; ci < ch1; ci += NT) { const int c = D.child_idx[ci]; spin_until_ge(front_done + c, epoch * (uint32_t)F.target[c]); }
+    const bool fast = nch <= MAXCH && chOff[nch <= MAXCH ? nch : 0] <= RELCAP;
+    if (fast) {
+        const int tot_rel = chOff[nch];
+#pragma unroll 4
+        for (int idx = tid; idx < tot_rel; idx += NT) {
+            int i = 0;
+            while (idx >= chOff[i + 1]) ++i;
+            relS[idx] = D.rel[chRp[i] + (idx - chOff[i])];
+        }
+    }
+    for (int ci = tid; ci < nch; ci += NT) {             // wait for the children (thread ci < NT holds its child in myc)
+        const int c = ci == tid && myc >= 0 ? myc : D.child_idx[ch0 + ci];
+        spin_until_ge(front_done + c, epoch * (uint32_t)F.target[c]);
+    }
+    __syncthreads();
     TRACE(1);
-    for (int ci = ch0; ci < ch1; ++ci) {                 // extend-add, fixed child order
-        const int c = D.child_idx[ci];
-        const int64_t rp0 = D.rel_ptr[c];
-        const int mc = (int)(D.rel_ptr[c + 1] - rp0);
-        const double* Uc = D.U + D.upd_ptr[c];
-        int* rb = rels + NT * ((ci - ch0) & 1);
-        if (tid < mc) rb[tid] = D.rel[rp0 + tid];
-        __syncthreads();                                 // also orders the waits above / the previous child's additions
-        // columns b and mc-1-b of the child's lower triangle together hold mc+1 entries: a balanced flat index space,
-        // 8 loads in flight per thread
-        const int per = mc + 1, tot = ((mc + 1) >> 1) * per;
-        for (int f0 = tid; f0 < tot; f0 += 8 * NT) {
+    auto entry = [&](int mc, const int* rb, const double* Uc, int f, double& v, int& dst) {
+        // columns b and mc-1-b of a child's lower triangle together hold mc+1 entries: a balanced flat index space
+        const int per = mc + 1;
+        const int p = f / per, e = f - p * per;
+        int a, b2;
+        if (e < mc - p) { b2 = p; a = p + e; }
+        else { b2 = mc - 1 - p; a = b2 + (e - (mc - p)); }
+        dst = -1; v = 0.0;
+        if (b2 != p || e < mc - p) {                     // the middle column of an odd mc is its own partner: count it once
+            const int j = rb[b2], i = rb[a];
+            dst = j * r - ((j * (j - 1)) >> 1) + (i - j);
+            v = __ldcg(Uc + a + (int64_t)b2 * mc);
+        }
+    };
+    if (fast) {
+        // children are taken in their fixed order.  Consecutive small children whose entries together fit one batch (8 per
+        // thread) are LOADED together (one round trip to L2 for the group) and ADDED one child after the other (a barrier
+        // between children: two children may hit the same entry of the front, the order of the additions is fixed).
+        int i = 0;
+        while (i < nch) {
+            const int mci = chMc[i];
+            const int toti = ((mci + 1) >> 1) * (mci + 1);
+            if (toti > 8 * NT) {                         // a big child on its own, several batches
+                const int* rb = relS + chOff[i];
+                const double* Uc = D.U + chUp[i];
+                for (int f0 = tid; f0 < toti; f0 += 8 * NT) {
+                    double v[8];
+                    int dst[8];
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) { dst[k] = -1; v[k] = 0.0; if (f0 + k * NT < toti) entry(mci, rb, Uc, f0 + k * NT, v[k], dst[k]); }
+#pragma unroll
+                    for (int k = 0; k < 8; ++k)
+                        if (dst[k] >= 0) sm[dst[k]] += v[k];
+                }
+                __syncthreads();
+                ++i;
+                continue;
+            }
+            int e = i, gtot = 0;                         // group [i, e): cumulative entry counts in cum[]
+            int cum[9];
+            cum[0] = 0;
+#pragma unroll
+            for (int g = 0; g < 8; ++g) {
+                int tg = 0;
+                if (e < nch && e == i + g) { const int m2 = chMc[e]; tg = ((m2 + 1) >> 1) * (m2 + 1); if (gtot + tg <= 8 * NT) { gtot += tg; ++e; } }
+                cum[g + 1] = gtot;
+            }
             double v[8];
-            int dst[8];
+            int dst[8], who[8];
 #pragma unroll
             for (int k = 0; k < 8; ++k) {
-                const int f = f0 + k * NT;
-                dst[k] = -1;
-                v[k] = 0.0;
-                if (f < tot) {
-                    const int p = f / per, e = f - p * per;
-                    int a, b;
-                    if (e < mc - p) { b = p; a = p + e; }
-                    else { b = mc - 1 - p; a = b + (e - (mc - p)); }
-                    if (b != p || e < mc - p) {          // the middle column of an odd mc is its own partner: count it once
-                        const int j = rb[b], i = rb[a];
-                        dst[k] = j * r - ((j * (j - 1)) >> 1) + (i - j);
-                        v[k] = __ldcg(Uc + a + (int64_t)b * mc);
-                    }
+                const int Fk = tid + k * NT;
+                dst[k] = -1; v[k] = 0.0; who[k] = -1;
+                if (Fk < gtot) {
+                    int g = 0;
+#pragma unroll
+                    for (int t2 = 1; t2 < 8; ++t2) g += (Fk >= cum[t2] && i + t2 < e) ? 1 : 0;
+                    who[k] = g;
+                    entry(chMc[i + g], relS + chOff[i + g], D.U + chUp[i + g], Fk - cum[g], v[k], dst[k]);
                 }
             }
+            for (int g = 0; g < e - i; ++g) {
 #pragma unroll
-            for (int k = 0; k < 8; ++k)
-                if (dst[k] >= 0) sm[dst[k]] += v[k];
+                for (int k = 0; k < 8; ++k)
+                    if (who[k] == g && dst[k] >= 0) sm[dst[k]] += v[k];
+                __syncthreads();
+            }
+            i = e;
+        }
+    } else {
+        for (int ci = ch0; ci < ch1; ++ci) {             // many / large children: one by one, relative indices per child
+            const int c = D.child_idx[ci];
+            const int64_t rp0 = D.rel_ptr[c];
+            const int mc = (int)(D.rel_ptr[c + 1] - rp0);
+            const double* Uc = D.U + D.upd_ptr[c];
+            int* rb = relS + NT * ((ci - ch0) & 1);
+            if (tid < mc) rb[tid] = D.rel[rp0 + tid];
+            __syncthreads();                             // also orders the previous child's additions
+            const int tot = ((mc + 1) >> 1) * (mc + 1);
+            for (int f0 = tid; f0 < tot; f0 += 8 * NT) {
+                double v[8];
+                int dst[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) { dst[k] = -1; v[k] = 0.0; if (f0 + k * NT < tot) entry(mc, rb, Uc, f0 + k * NT, v[k], dst[k]); }
+#pragma unroll
+                for (int k = 0; k < 8; ++k)
+                    if (dst[k] >= 0) sm[dst[k]] += v[k];
+            }
         }
     }
     __syncthreads();
@@ -639,7 +725,7 @@ cudaError_t configure_factor_kernels(int max_smem_bytes, bool one_cta_per_sm, in
     *ctas_per_sm = occ < 1 ? 1 : occ;
     *smem_bytes = bytes;
     int rmax = 1;                                        // largest r with the packed front + the relative-index buffers in `bytes`
-    while (rmax < NT && rmax + 2 <= SMALL_ROWS_MAX && ((size_t)(rmax + 1) * (rmax + 2) / 2 + 1 + NT) * sizeof(double) <= bytes) ++rmax;   // front + 2 NT ints
+    while (rmax < NT && rmax + 2 <= SMALL_ROWS_MAX && ((size_t)(rmax + 1) * (rmax + 2) / 2 + 1 + SMALL_WORK_DOUBLES) * sizeof(double) <= bytes) ++rmax;   // front + work area
     *small_max_r = rmax;
     return cudaSuccess;
 }
