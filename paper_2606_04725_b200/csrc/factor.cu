@@ -583,11 +583,14 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
 #pragma unroll
         for (int b = 0; b < 4; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
     const int nch = (Kend + KC - 1) / KC;
-    auto wait_flags = [&](int c) {                       // thread 0: the 64-column block that chunk c starts must be finished
-        if (tid == 0 && c < nch && ((c * KC) & (TILE - 1)) == 0) {
-            const int kb = (c * KC) / TILE;
-            spin_until_ge(tdone + kb * nbt + I, epoch);
-            if (J != I) spin_until_ge(tdone + kb * nbt + J, epoch);
+    auto wait_flags = [&](int c) {                       // every warp: the 64-column block that chunk c starts must be finished
+        if (c < nch && ((c * KC) & (TILE - 1)) == 0) {
+            if (lane == 0) {
+                const int kb = (c * KC) / TILE;
+                spin_until_ge(tdone + kb * nbt + I, epoch);
+                if (J != I) spin_until_ge(tdone + kb * nbt + J, epoch);
+            }
+            __syncwarp();
         }
     };
     auto issue = [&](int c) {
@@ -606,18 +609,14 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
         }
         cp_async_commit();
     };
-    wait_flags(0);
-    wait_flags(1);
-    wait_flags(2);
-    __syncthreads();
-    issue(0);
-    issue(1);
-    issue(2);
+    // chunk c is multiplied BEFORE the warps wait for the flags of chunk c+3 (and request it): when a flag is late, the chunks
+    // already in shared memory are finished first and the newly released columns only add their own latency
+    wait_flags(0); issue(0);
+    wait_flags(1); issue(1);
+    wait_flags(2); issue(2);
     for (int c = 0; c < nch; ++c) {
-        wait_flags(c + 3);
         cp_async_wait<2>();
         __syncthreads();
-        issue(c + 3);
         const double* As = pipe + (c % NSTAGE) * STAGE_DOUBLES + wm * 16 + gid + di;
         const double* Bs = pipe + (c % NSTAGE) * STAGE_DOUBLES + KC * ALD + wn * 32 + gid + dj;
 #pragma unroll
@@ -632,6 +631,8 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
 #pragma unroll
                 for (int nt = 0; nt < 4; ++nt) dmma(acc[mt][nt], a[mt], b[nt]);
         }
+        wait_flags(c + 3);                               // stage (c+3) % 4 held chunk c-1: free since this iteration's barrier
+        issue(c + 3);
     }
     cp_async_wait<0>();
     TRACE(2);
@@ -654,13 +655,16 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
             double* rinv = pipe + CT_DOUBLES;
             if (tid == 0) spin_until_ge(tdone + J * nbt + J, epoch);
             __syncthreads();
-            for (int idx = tid; idx < nj * nj; idx += NT) {
-                const int ii = idx % nj, cc = idx / nj;
-                if (ii >= cc) {
-                    const double v = __ldcg(P + (j0 + ii) + (int64_t)(j0 + cc) * ld);
-                    Ls[cc * CLD + ii] = v;
-                    if (ii == cc) rinv[cc] = 1.0 / v;
+            {   // L_JJ and its pivot reciprocals: everything requested at once (cp.async, 16-byte chunks: j0, ld and CLD are even)
+                const int half = (nj + 1) >> 1;
+                const double* src = P + j0 + (int64_t)j0 * ld;
+                for (int idx = tid; idx < nj * half; idx += NT) {
+                    const int cc = idx / half, hh = idx - cc * half;
+                    cp_async16(Ls + cc * CLD + 2 * hh, src + (int64_t)cc * ld + 2 * hh, 16);
                 }
+                cp_async_commit();
+                if (tid < nj) rinv[tid] = __ldcg(D.dinv + c0 + j0 + tid);
+                cp_async_wait<0>();
             }
             __syncthreads();
             trsm_tile(Cs, Ls, rinv, ni, nj);
