@@ -36,6 +36,9 @@ constexpr int TILE_SMEM_DOUBLES = PIPE_DOUBLES + CT_DOUBLES;  // 12928 doubles =
 static_assert(CT_DOUBLES + TILE <= PIPE_DOUBLES, "L_JJ tile + reciprocals alias the operand ring");
 
 // ---- gpu-scope acquire / release on the completion flags ----
+// Publishing: all threads store, CTA barrier, then ONE thread fences and releases the flag (the release is cumulative over
+// what the barrier ordered before it -- the pattern of a grid-wide barrier).  Consuming: one thread acquires, CTA barrier
+// (or __syncwarp), then everybody reads the produced data with ld.global.cg.
 __device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
     uint32_t v;
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
@@ -512,9 +515,8 @@ __device__ __forceinline__ void small_front_task(const DevSym& D, const DagPlan&
         const double* cj = colp(j + w) + w;
         for (int i = j + lane; i < m; i += 32) Uo[i + (int64_t)j * m] = cj[i];
     }
-    __threadfence();
     __syncthreads();
-    if (tid == 0) red_release_add(front_done + s, 1u);
+    if (tid == 0) { __threadfence(); red_release_add(front_done + s, 1u); }
     TRACE(4);
     double* P = D.L + D.panel_ptr[s];                    // the panel of L is read by the solves only (after the kernel)
     for (int j = warp; j < w; j += nwarp) {
@@ -674,9 +676,8 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
             const int mm = idx % ni, nn = idx / ni;
             if (I != J || mm >= nn) P[(i0 + mm) + (int64_t)(j0 + nn) * ld] = Cs[nn * CLD + mm];
         }
-        __threadfence();
         __syncthreads();
-        if (tid == 0) { st_release(tdone + J * nbt + I, epoch); red_release_add(front_done + s, 1u); }
+        if (tid == 0) { __threadfence(); st_release(tdone + J * nbt + I, epoch); red_release_add(front_done + s, 1u); }
     } else {
         double* Uo = D.U + D.upd_ptr[s];
         TRACE(3);
@@ -684,9 +685,8 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
             const int mm = idx % ni, nn = idx / ni;
             if (I != J || mm >= nn) Uo[(i0 + mm - w) + (int64_t)(j0 + nn - w) * m] = Cs[nn * CLD + mm];
         }
-        __threadfence();
         __syncthreads();
-        if (tid == 0) red_release_add(front_done + s, 1u);
+        if (tid == 0) { __threadfence(); red_release_add(front_done + s, 1u); }
     }
     TRACE(4);
 }

@@ -151,9 +151,8 @@ __device__ __forceinline__ void fwd_small(const DevSym& D, const DagPlan& F, int
     STRACE(3);
     double* co = D.ctr + D.rel_ptr[s];
     for (int i = q.w + tid; i < q.r; i += NT) co[i - q.w] = t[i];
-    __threadfence();
     __syncthreads();
-    if (tid == 0) red_release_add(F.sol_done_f + s, 1u);
+    if (tid == 0) { __threadfence(); red_release_add(F.sol_done_f + s, 1u); }
 }
 
 // ---------------- forward, block row I of a tiled supernode ----------------
@@ -262,16 +261,14 @@ __device__ __forceinline__ void fwd_tiled(const DevSym& D, const DagPlan& F, int
             }
             if (lane < ni) x[q.c0 + i0 + lane] = t0;
             if (h1) x[q.c0 + i0 + lane + 32] = t1;
-            __threadfence();
             __syncwarp();
-            if (lane == 0) { st_release(bf + I, epoch); red_release_add(F.sol_done_f + s, 1u); }
+            if (lane == 0) { __threadfence(); st_release(bf + I, epoch); red_release_add(F.sol_done_f + s, 1u); }
         }
     } else {
         double* co = D.ctr + D.rel_ptr[s];
         if (tid < ni) co[i0 + tid - q.w] = tI[tid];
-        __threadfence();
         __syncthreads();
-        if (tid == 0) red_release_add(F.sol_done_f + s, 1u);
+        if (tid == 0) { __threadfence(); red_release_add(F.sol_done_f + s, 1u); }
     }
 }
 
@@ -341,9 +338,8 @@ __device__ __forceinline__ void bwd_small(const DevSym& D, const DagPlan& F, int
     __syncthreads();
     STRACE(3);
     for (int i = tid; i < q.w; i += NT) { x[q.c0 + i] = t[i]; b[D.perm[q.c0 + i]] = t[i]; }
-    __threadfence();
     __syncthreads();
-    if (tid == 0) red_release_add(F.sol_done_b + s, 1u);
+    if (tid == 0) { __threadfence(); red_release_add(F.sol_done_b + s, 1u); }
 }
 
 // ---------------- backward, block column J of a tiled supernode ----------------
@@ -445,9 +441,8 @@ __device__ __forceinline__ void bwd_tiled(const DevSym& D, const DagPlan& F, int
         }
         if (lane < nj) { x[q.c0 + j0 + lane] = z0; b[D.perm[q.c0 + j0 + lane]] = z0; }
         if (h1) { x[q.c0 + j0 + lane + 32] = z1; b[D.perm[q.c0 + j0 + lane + 32]] = z1; }
-        __threadfence();
         __syncwarp();
-        if (lane == 0) { st_release(bb + J, epoch); red_release_add(F.sol_done_b + s, 1u); }
+        if (lane == 0) { __threadfence(); st_release(bb + J, epoch); red_release_add(F.sol_done_b + s, 1u); }
     }
 }
 
