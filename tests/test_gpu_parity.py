@@ -230,6 +230,28 @@ def test_ipm_solve_vs_oracle(name, ov):
     h.close()
 
 
+@pytest.mark.parametrize("name,ov", [("C2", dict(g=9, N=7)), ("C4", dict(trays=40, N=25)), ("C1", {})])
+def test_ipm_solve_vs_oracle_tiled_fronts(name, ov):
+    """Same parity bar with the two-CTA-per-SM launch shape and every front above 48 rows forced through the tiled
+    (HBM-resident, left-looking 64x64 tile) kernel family -- the path the large workloads take (smem_front_max > 0
+    switches the latency mode off)."""
+    cfg = make_config(name, **ov)
+    ro = LiftedIPM(cfg, linsolve="blocktri" if name != "C1" else "sparse").solve()
+    assert ro["status"] == "converged"
+    h = _gpu_ipm(cfg, smem_front_max=48)
+    assert h.get_info()["n_large_fronts"] > 0
+    h.update_params(dev(cfg.x0), dev(cfg.ref_for_solve(0)))
+    y = torch.zeros(cfg.n, dtype=torch.float64, device=DEV)
+    rg = h.ipm_solve(0, y, trace_cap=256)
+    assert rg["status"] == 0
+    assert rg["iters"] == ro["iters"], (rg["iters"], ro["iters"])
+    yo = ro["state"].y
+    assert np.abs(y.cpu().numpy() - yo).max() <= 1e-6 * np.abs(yo).max()
+    for tg, to in zip(rg["trace"], ro["trace"]):
+        assert tg["mu"] == to["mu"] and tg["eta"] == to["eta"]
+    h.close()
+
+
 @pytest.mark.parametrize("ordering", ORDERINGS)
 def test_ipm_result_independent_of_ordering(ordering):
     cfg = make_config("C1", trays=10, N=14)
