@@ -276,6 +276,44 @@ def phase_pass(nb, torch, cfg, stream, x0s, warmup):
     return acc
 
 
+def sigma_sweep(nb, torch, cfg, stream, count=200):
+    """BASELINE.json:configs[4]: `count` numeric refactorizations + solves on the C4 pattern through nmpc_assemble /
+    nmpc_factor / nmpc_solve with Sigma_x, Sigma_s redrawn log-uniform in [1e-8, 1e8] per call (J, grad^2 f frozen at
+    the cold-start point; all draws resident in HBM before the timed loop; CUDA events on the handle's stream)."""
+    from ocp_inputs import sigma_sweep_draws
+    dev = torch.device("cuda", torch.cuda.current_device())
+    with torch.cuda.stream(stream):
+        h = nb.Handle(None, nb.make_ocp(cfg), nb.default_options(), stream=stream.cuda_stream)
+        td = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64).to(dev)   # noqa: E731
+        h.update_params(td(cfg.x0), td(cfg.ref_for_solve(0)))
+        jrp, _ = h.get_jac_pattern(cfg.m)
+        wrp, _ = h.get_hess_pattern(cfg.n)
+        krp, _ = h.get_kkt_pattern(cfg.n)
+        c, g = torch.empty(cfg.m, dtype=torch.float64, device=dev), torch.empty(cfg.n, dtype=torch.float64, device=dev)
+        Jv = torch.empty(int(jrp[-1]), dtype=torch.float64, device=dev)
+        Wv = torch.empty(int(wrp[-1]), dtype=torch.float64, device=dev)
+        Kv = torch.empty(int(krp[-1]), dtype=torch.float64, device=dev)
+        h.model_eval(td(cfg.y_cold(cfg.x0)), td(np.zeros(cfg.m)), c, g, Jv, Wv)
+        draws = [(td(sx), td(ss), td(b)) for sx, ss, b in sigma_sweep_draws(cfg, count=count)]
+    stream.synchronize()
+    fails = 0
+    for sx, ss, b in draws[:3]:                           # warm-up
+        h.assemble(Jv, Wv, sx, ss, 0.0, Kv); h.factor(Kv, 0.0, check=False); h.solve(b.clone())
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for sx, ss, b in draws:
+        h.assemble(Jv, Wv, sx, ss, 0.0, Kv)
+        st, _ = h.factor(Kv, 0.0, check=False)
+        fails += int(st != 0)
+        h.solve(b)
+    e1.record(stream)
+    e1.synchronize()
+    ms = e0.elapsed_time(e1)
+    h.close()
+    return {"calls": count, "pivot_failures": fails, "us_per_refactor_plus_solve": ms * 1e3 / count,
+            "note": "assemble + numeric Cholesky + both solves per call, host synchronisation on the pivot flag included"}
+
+
 def workload_summary(nb, torch, name, stream, hbm_peak, steps=3):
     """Short per-config summary (not the bench line): cold solve + `steps` warm re-solves with phase timing."""
     cfg = make_config(name)
@@ -297,6 +335,7 @@ def workload_summary(nb, torch, name, stream, hbm_peak, steps=3):
         "factor_tflops": info["flops"] / fus * 1e-6, "factor_frac_fp64": info["flops"] / fus * 1e-6 / FP64_DERIVED_TFLOPS,
         "solve_gbs": 16.0 * info["nnz_L"] / sus * 1e-3, "solve_frac_hbm": 16.0 * info["nnz_L"] / sus * 1e-3 / hbm_peak,
         "not_converged": res["bad"],
+        **({"sigma_sweep": sigma_sweep(nb, torch, cfg, stream)} if name == "C4" else {}),
     }
 
 

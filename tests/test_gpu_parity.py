@@ -72,6 +72,73 @@ def test_factor_and_solve_vs_oracle(name, ov, ordering):
     h.close()
 
 
+def _sweep_setup(cfg):
+    """Frozen J, grad^2 f at the cold-start point (C4 refactor sweep, BASELINE.json:configs[4]): GPU value arrays + the
+    same matrices from the oracle's model code."""
+    nlp = TranscribedOCP(cfg)
+    nlp.set_params(cfg.x0, cfg.ref_for_solve(0))
+    y0 = cfg.y_cold(cfg.x0)
+    h = nb.Handle(None, nb.make_ocp(cfg), None)
+    h.update_params(dev(cfg.x0), dev(cfg.ref_for_solve(0)))
+    jrp, _ = h.get_jac_pattern(cfg.m)
+    wrp, _ = h.get_hess_pattern(cfg.n)
+    krp, kci = h.get_kkt_pattern(cfg.n)
+    c, g = torch.empty(cfg.m, dtype=torch.float64, device=DEV), torch.empty(cfg.n, dtype=torch.float64, device=DEV)
+    Jv = torch.empty(int(jrp[-1]), dtype=torch.float64, device=DEV)
+    Wv = torch.empty(int(wrp[-1]), dtype=torch.float64, device=DEV)
+    h.model_eval(dev(y0), dev(np.zeros(cfg.m)), c, g, Jv, Wv)              # lambda = 0: W = grad^2 f
+    Jo, Wo = nlp.jacobian(y0), nlp.hessian(y0, np.zeros(cfg.m))
+    return h, Jv, Wv, krp, kci, Jo, Wo
+
+
+def test_sigma_sweep_midsize_vs_oracle():
+    """C4 refactor sweep at a size the oracle factors in seconds: every draw refactors on the fixed structure."""
+    cfg = make_config("C4", trays=40, N=25)
+    h, Jv, Wv, krp, kci, Jo, Wo = _sweep_setup(cfg)
+    info = h.get_info()
+    Kv = torch.empty(int(krp[-1]), dtype=torch.float64, device=DEV)
+    for k, (sx, ss, b) in enumerate(sigma_sweep_draws(cfg, count=6)):
+        h.assemble(Jv, Wv, dev(sx), dev(ss), 0.0, Kv)
+        st, _ = h.factor(Kv, 0.0)
+        assert st == 0, k
+        K = (Wo + sp.diags(sx) + Jo.T @ sp.diags(ss) @ Jo).tocsr()
+        L = factor_as_sparse(info, h.get_factor())
+        assert factor_backward_error(L, K, info["perm"]) <= 1e-12, k
+        x = dev(b)
+        h.solve(x)
+        xg = x.cpu().numpy()
+        assert normwise_backward_error(K, xg, b) <= 1e-10, k
+        xo = SparseCholesky(K, None).factor(K).solve(b)
+        # cond(K) ~ 1e16 here (Sigma in [1e-8, 1e8]): the two backward-stable solutions agree through K, not entrywise:
+        # K (x_gpu - x_oracle) must vanish to the backward-error level of either solve
+        Kn = abs(K).sum(axis=1).max()
+        assert np.abs(K @ (xg - xo)).max() <= 2e-10 * (Kn * max(np.abs(xg).max(), np.abs(xo).max()) + np.abs(b).max()), k
+    h.close()
+
+
+def test_sigma_sweep_full_size_properties():
+    """The sweep at BASELINE's full C4 size (n = 52 400), in the launch configuration bench.py times: properties that hold
+    at any size -- no pivot failure, normwise backward error of the solve against K rebuilt by SciPy from the oracle's
+    J and grad^2 f, and the same solution from a second refactorization (bitwise)."""
+    cfg = make_config("C4")
+    h, Jv, Wv, krp, kci, Jo, Wo = _sweep_setup(cfg)
+    Kv = torch.empty(int(krp[-1]), dtype=torch.float64, device=DEV)
+    for k, (sx, ss, b) in enumerate(sigma_sweep_draws(cfg, count=3)):
+        h.assemble(Jv, Wv, dev(sx), dev(ss), 0.0, Kv)
+        st, _ = h.factor(Kv, 0.0)
+        assert st == 0, k
+        x = dev(b)
+        h.solve(x)
+        xg = x.cpu().numpy()
+        K = (Wo + sp.diags(sx) + Jo.T @ sp.diags(ss) @ Jo).tocsr()
+        assert normwise_backward_error(K, xg, b) <= 1e-10, k
+        st, _ = h.factor(Kv, 0.0)
+        x2 = dev(b)
+        h.solve(x2)
+        assert np.array_equal(x2.cpu().numpy(), xg)
+    h.close()
+
+
 @pytest.mark.parametrize("smem_front_max", [16, 48, 0])
 def test_factor_kernel_families_agree(smem_front_max):
     """The shared-memory and the tiled front kernels must give the same factor (to rounding) on the same matrix."""
