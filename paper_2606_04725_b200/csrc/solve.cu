@@ -302,16 +302,24 @@ __device__ __forceinline__ void bwd_small(const DevSym& D, const DagPlan& F, int
             const int c = idx >> 5, i = idx & 31;
             if (i >= c && i < nb) Lbt[c * SLD + i] = Bk[c * ldb + i];
         }
-        for (int c = warp; c < nb; c += nwarp) {         // z_c = y_c - sum_{i >= j0+nb} L[i, j0+c] x_i
-            const double* Bc = Bk + c * ldb - j0;
-            double a0 = 0.0, a1 = 0.0;
-            int i = j0 + nb + lane;
-            for (; i + 32 < q.r; i += 64) { a0 = fma(Bc[i], t[i], a0); a1 = fma(Bc[i + 32], t[i + 32], a1); }
-            if (i < q.r) a0 = fma(Bc[i], t[i], a0);
-            a0 += a1;
+        {   // z_c = y_c - sum_{i >= j0+nb} L[i, j0+c] x_i: a warp takes columns warp, warp+8, warp+16, warp+24 TOGETHER (lanes over the
+            // rows), so that the four butterfly reductions interleave
+            double a[4] = {0.0, 0.0, 0.0, 0.0};
+            const double* Bc[4];
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) a0 += __shfl_xor_sync(FULL, a0, o);
-            if (lane == 0) t[j0 + c] -= a0;
+            for (int e = 0; e < 4; ++e) Bc[e] = Bk + min(warp + nwarp * e, nb - 1) * ldb - j0;
+            for (int i = j0 + nb + lane; i < q.r; i += 32) {
+                const double ti = t[i];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) a[e] = fma(Bc[e][i], ti, a[e]);
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) a[e] += __shfl_xor_sync(FULL, a[e], o);
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+                if (lane == 0 && warp + nwarp * e < nb) t[j0 + warp + nwarp * e] -= a[e];
         }
         __syncthreads();
         if (warp == 0) {                                 // L11^T x1 = z on the diagonal block
