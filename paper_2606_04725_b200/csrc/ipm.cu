@@ -16,6 +16,8 @@ namespace nmpc {
 namespace {
 
 constexpr int NT = 256;
+constexpr int GV = 8;                   // lanes that share one column of J in the J^T products (residual, right-hand side)
+constexpr int GK = 4;                   // lanes that share one entry of K in the condensed assembly
 constexpr double INF = __builtin_huge_val();
 
 struct LamDiff { const double* p; const double* m; __device__ __forceinline__ double operator[](int i) const { return p[i] - m[i]; } };
@@ -67,12 +69,19 @@ __global__ void __launch_bounds__(NT) model_eval_kernel(DevModel M, const double
 __global__ void __launch_bounds__(NT) assemble_K_kernel(DevModel M, const double* __restrict__ Jval, const double* __restrict__ Wval,
                                                         const double* __restrict__ sigx, const double* __restrict__ q,
                                                         double eta, double* __restrict__ Kval) {
-    const int64_t e = blockIdx.x * (int64_t)NT + threadIdx.x;
-    if (e >= M.nnzK) return;
+    const int64_t gtid = blockIdx.x * (int64_t)NT + threadIdx.x;
+    const int64_t e = gtid / GK;                         // GK lanes per K entry walk its triple list, fixed butterfly order
+    const int gl = (int)(gtid % GK);
+    const bool valid = e < M.nnzK;
     double acc = 0.0;
-#pragma unroll 16
-    for (int64_t p = M.trip_ptr[e]; p < M.trip_ptr[e + 1]; ++p)
-        acc += Jval[M.trip_a[p]] * q[M.trip_r[p]] * Jval[M.trip_b[p]];
+    if (valid) {
+#pragma unroll 4
+        for (int64_t p = M.trip_ptr[e] + gl; p < M.trip_ptr[e + 1]; p += GK)
+            acc += Jval[M.trip_a[p]] * q[M.trip_r[p]] * Jval[M.trip_b[p]];
+    }
+#pragma unroll
+    for (int o = 1; o < GK; o <<= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (!valid || gl != 0) return;
     const int wi = M.k_w[e], di = M.k_diag[e];
     if (wi >= 0) acc += Wval[wi];
     if (di >= 0) acc += sigx[di] + eta;
@@ -168,13 +177,20 @@ __global__ void __launch_bounds__(NT) warm_push_kernel(DevModel M, IpmVectors V,
 __global__ void __launch_bounds__(NT) residual_kernel(DevModel M, IpmVectors V, double gamma) {
     Red<7> a;
     a.v[0] = a.v[1] = a.v[2] = 0.0; a.v[3] = -INF; a.v[4] = INF; a.v[5] = 0.0; a.v[6] = 0.0;
-    const int64_t total = M.n + M.m;
-    for (int64_t idx = blockIdx.x * (int64_t)NT + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * NT) {
-        if (idx < M.n) {
-            const int64_t i = idx;
-            double jt = 0.0;
-#pragma unroll 16
-            for (int64_t p = M.jt_ptr[i]; p < M.jt_ptr[i + 1]; ++p) { const int r = M.jt_row[p]; jt += V.Jval[M.jt_idx[p]] * (V.wp[r] - V.wm[r]); }
+    // variables: GV lanes share one column of J (the input columns hold 2 nx entries), fixed butterfly order
+    const int64_t gthreads = (int64_t)gridDim.x * NT, gtid = blockIdx.x * (int64_t)NT + threadIdx.x;
+    const int gl = (int)(gtid % GV);
+    for (int64_t i0 = 0; i0 < M.n; i0 += gthreads / GV) {
+        const int64_t i = i0 + gtid / GV;
+        const bool valid = i < M.n;
+        double jt = 0.0;
+        if (valid) {
+#pragma unroll 4
+            for (int64_t p = M.jt_ptr[i] + gl; p < M.jt_ptr[i + 1]; p += GV) { const int r = M.jt_row[p]; jt += V.Jval[M.jt_idx[p]] * (V.wp[r] - V.wm[r]); }
+        }
+#pragma unroll
+        for (int o = 1; o < GV; o <<= 1) jt += __shfl_xor_sync(0xffffffffu, jt, o);
+        if (valid && gl == 0) {
             const double lb = M.lb[i], ub = M.ub[i], y = V.y[i];
             const bool hasL = lb > -INF, hasU = ub < INF;
             const double zL = hasL ? V.zL[i] : 0.0, zU = hasU ? V.zU[i] : 0.0;
@@ -183,17 +199,17 @@ __global__ void __launch_bounds__(NT) residual_kernel(DevModel M, IpmVectors V, 
             if (!isfinite(rd) || !isfinite(y)) a.v[6] += 1.0;
             if (hasL) { const double cp = (y - lb) * zL; a.v[3] = fmax(a.v[3], cp); a.v[4] = fmin(a.v[4], cp); a.v[5] += zL; }
             if (hasU) { const double cp = (ub - y) * zU; a.v[3] = fmax(a.v[3], cp); a.v[4] = fmin(a.v[4], cp); a.v[5] += zU; }
-        } else {
-            const int64_t r = idx - M.n;
-            const double c = V.c[r], sp = V.sp[r], sm = V.sm[r], wp = V.wp[r], wm = V.wm[r];
-            const double rpp = c - gamma + sp, rpm = -c - gamma + sm;
-            V.r_pp[r] = rpp; V.r_pm[r] = rpm;
-            a.v[1] = fmax(a.v[1], fabs(rpp)); a.v[2] = fmax(a.v[2], fabs(rpm));
-            if (!isfinite(rpp) || !isfinite(rpm)) a.v[6] += 1.0;
-            const double c1 = sp * wp, c2 = sm * wm;
-            a.v[3] = fmax(a.v[3], fmax(c1, c2)); a.v[4] = fmin(a.v[4], fmin(c1, c2));
-            a.v[5] += wp + wm;
         }
+    }
+    for (int64_t r = gtid; r < M.m; r += gthreads) {
+        const double c = V.c[r], sp = V.sp[r], sm = V.sm[r], wp = V.wp[r], wm = V.wm[r];
+        const double rpp = c - gamma + sp, rpm = -c - gamma + sm;
+        V.r_pp[r] = rpp; V.r_pm[r] = rpm;
+        a.v[1] = fmax(a.v[1], fabs(rpp)); a.v[2] = fmax(a.v[2], fabs(rpm));
+        if (!isfinite(rpp) || !isfinite(rpm)) a.v[6] += 1.0;
+        const double c1 = sp * wp, c2 = sm * wm;
+        a.v[3] = fmax(a.v[3], fmax(c1, c2)); a.v[4] = fmin(a.v[4], fmin(c1, c2));
+        a.v[5] += wp + wm;
     }
     const int ops[7] = {0, 0, 0, 0, 1, 2, 2};
     block_reduce<7>(a, ops, V.partial + (int64_t)blockIdx.x * 8);
@@ -224,11 +240,18 @@ __global__ void __launch_bounds__(NT) sigma_rows_kernel(DevModel M, IpmVectors V
 }
 
 __global__ void __launch_bounds__(NT) sigma_vars_kernel(DevModel M, IpmVectors V, double mu) {
-    const int64_t i = blockIdx.x * (int64_t)NT + threadIdx.x;
-    if (i >= M.n) return;
+    const int64_t gtid = blockIdx.x * (int64_t)NT + threadIdx.x;
+    const int64_t i = gtid / GV;                         // GV lanes per variable for the J^T t product
+    const int gl = (int)(gtid % GV);
+    const bool valid = i < M.n;
     double jt = 0.0;
-#pragma unroll 16
-    for (int64_t p = M.jt_ptr[i]; p < M.jt_ptr[i + 1]; ++p) jt += V.Jval[M.jt_idx[p]] * V.t[M.jt_row[p]];
+    if (valid) {
+#pragma unroll 4
+        for (int64_t p = M.jt_ptr[i] + gl; p < M.jt_ptr[i + 1]; p += GV) jt += V.Jval[M.jt_idx[p]] * V.t[M.jt_row[p]];
+    }
+#pragma unroll
+    for (int o = 1; o < GV; o <<= 1) jt += __shfl_xor_sync(0xffffffffu, jt, o);
+    if (!valid || gl != 0) return;
     const double lb = M.lb[i], ub = M.ub[i], y = V.y[i];
     const bool hasL = lb > -INF, hasU = ub < INF;
     const double dL = hasL ? y - lb : 1.0, dU = hasU ? ub - y : 1.0;
@@ -328,7 +351,7 @@ void launch_model_eval(const DevModel& M, const double* y, const double* wp, con
 }
 void launch_assemble_K(const DevModel& M, const double* Jval, const double* Wval, const double* sigx, const double* q,
                        double eta, double* Kval, cudaStream_t st) {
-    assemble_K_kernel<<<blocks_for(M.nnzK), NT, 0, st>>>(M, Jval, Wval, sigx, q, eta, Kval);
+    assemble_K_kernel<<<blocks_for(M.nnzK * GK), NT, 0, st>>>(M, Jval, Wval, sigx, q, eta, Kval);
 }
 void launch_kkt_multiply(int64_t n, const int64_t* ptr, const int32_t* idx, const int32_t* src, const double* Kval, double eta,
                          const double* x, double* y, cudaStream_t st) {
@@ -344,13 +367,13 @@ void launch_warm_push(const DevModel& M, const IpmVectors& V, double warm_push, 
     warm_push_kernel<<<blocks_for(M.n), NT, 0, st>>>(M, V, warm_push);
 }
 void launch_residuals(const DevModel& M, const IpmVectors& V, double gamma, cudaStream_t st) {
-    const int nb = red_blocks(M.n + M.m);
+    const int nb = red_blocks(M.n * GV + M.m);
     residual_kernel<<<nb, NT, 0, st>>>(M, V, gamma);
     finalize_residual_kernel<<<1, NT, 0, st>>>(V, nb);
 }
 void launch_sigma_rhs(const DevModel& M, const IpmVectors& V, double mu, cudaStream_t st) {
     sigma_rows_kernel<<<blocks_for(M.m), NT, 0, st>>>(M, V, mu);
-    sigma_vars_kernel<<<blocks_for(M.n), NT, 0, st>>>(M, V, mu);
+    sigma_vars_kernel<<<blocks_for(M.n * GV), NT, 0, st>>>(M, V, mu);
 }
 void launch_step(const DevModel& M, const IpmVectors& V, double mu, double tau, cudaStream_t st) {
     const int nb = red_blocks(M.n + M.m);
