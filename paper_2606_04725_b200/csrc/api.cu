@@ -220,10 +220,10 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
     TRY(upload(h, cbnd, &F.cbnd));
     TRY(upload(h, S.sn_parent, &F.sn_parent));
     TRY(upload(h, ksrc, &h->D.kent_src)); TRY(upload(h, kdst, &h->D.kent_dst));
-    F.sync_words = 2 + 3 * (int64_t)ns + slots + 2 * bslots;
+    F.sync_words = 2 + 3 * (int64_t)ns + slots + 3 * bslots;
     TRY(dalloc(h, (size_t)F.sync_words, &F.sync));
     F.fac_done = F.sync + 2; F.sol_done_f = F.fac_done + ns; F.sol_done_b = F.sol_done_f + ns;
-    F.tile_done = F.sol_done_b + ns; F.blk_f = F.tile_done + slots; F.blk_b = F.blk_f + bslots;
+    F.tile_done = F.sol_done_b + ns; F.blk_f = F.tile_done + slots; F.blk_b = F.blk_f + bslots; F.sub_done = F.blk_b + bslots;
     if (std::getenv("NMPC_TRACE")) {                     // measurement aid: per-task timestamps (nmpc_get_task_trace)
         TRY(dalloc(h, (size_t)F.n_ftasks * 8, &F.ftrace)); TRY(dalloc(h, (size_t)F.n_stasks * 8, &F.strace));
     }

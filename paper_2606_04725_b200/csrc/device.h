@@ -88,6 +88,7 @@ struct DagPlan {
     uint32_t* tile_done = nullptr;       // tile slots
     uint32_t* blk_f = nullptr;           // block slots
     uint32_t* blk_b = nullptr;
+    uint32_t* sub_done = nullptr;        // block slots: published 8-column blocks of the diagonal tile L_JJ, (epoch-1)*16 + count
     unsigned long long* ftrace = nullptr;   // optional (NMPC_TRACE=1): 8 timestamps per factor task / per solve task
     unsigned long long* strace = nullptr;
     int64_t sync_words = 0;

@@ -142,8 +142,11 @@ __device__ __forceinline__ void factor_diag8(ColFn colp, int j0, int jb, int c0,
     }
 }
 
-template <class ColFn>
-__device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, int32_t* fail_col, double* dinv) {
+struct NoPublish { __device__ __forceinline__ void operator()(int, int) const {} };
+// pub(j0, jb) is called by all threads right after the barrier that ends the row solve of columns [j0, j0 + jb): those columns
+// are final from then on (the diagonal tile of a tiled front streams them to the TRSM tiles of its block column)
+template <class ColFn, class Pub = NoPublish>
+__device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, int32_t* fail_col, double* dinv, Pub pub = Pub()) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gid = lane >> 2, tig = lane & 3;
     constexpr int NW1 = NT / 32 - 1;                     // warps 1..7 share the tiles warp 0 does not take
     __shared__ double s_inv[8];
@@ -189,6 +192,7 @@ __device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, i
                     if (c < jb) colp(j0 + c)[i] = x[c];
             }
             __syncthreads();
+            pub(j0, jb);
             const bool has_next = t0 < w;
             if (t0 < p1) {                               // rank-8 update of the panel's remaining columns [t0, p1)
                 const bool k0 = tig < jb, k1 = tig + 4 < jb;
@@ -290,7 +294,11 @@ __device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, i
 // X = C L^-T for an ni x nj tile C (column-major, CLD) against the nj x nj lower-triangular Ls (column-major, CLD), in
 // place, same panel scheme: thread i substitutes 8 columns of row i, the rest of the 32-column panel gets a rank-8 DMMA
 // update, the columns after the panel a rank-32 one.  Rows >= ni / columns >= nj of the tiles are finite padding.
-__device__ __forceinline__ void trsm_tile(double* Cs, const double* Ls, const double* rinv, int ni, int nj) {
+// The columns of L_JJ arrive in 8-column blocks as the diagonal task publishes them (sub[0] counts them, `sbase` = value before
+// this call's first block): block k is fetched from the panel in global memory (Lg, leading dimension ldg) right before
+// sub-step k needs it, so the TRSM runs one sub-step behind the POTRF instead of after it.
+__device__ __forceinline__ void trsm_tile(double* Cs, double* Ls, double* rinv, int ni, int nj, const uint32_t* sub, uint32_t sbase,
+                                          const double* __restrict__ Lg, int ldg, const double* __restrict__ dinv_g) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gid = lane >> 2, tig = lane & 3;
     constexpr int NW = NT / 32;
     const int TU = (ni + 7) >> 3;
@@ -298,6 +306,17 @@ __device__ __forceinline__ void trsm_tile(double* Cs, const double* Ls, const do
         const int p1 = min(nj, p0 + 32);
         for (int j0 = p0; j0 < p1; j0 += 8) {
             const int jb = min(8, p1 - j0), t0 = j0 + jb;
+            {   // fetch columns [j0, j0 + jb) of L_JJ (rows j0 .. nj-1) and their pivot reciprocals
+                if (lane == 0) spin_until_ge(sub, sbase + (uint32_t)(j0 >> 3) + 1u);
+                __syncwarp();
+                const int nr = nj - j0;
+                for (int idx = tid; idx < jb * nr; idx += NT) {
+                    const int cc = idx / nr, ii = idx - cc * nr;
+                    Ls[(j0 + cc) * CLD + j0 + ii] = __ldcg(Lg + (j0 + ii) + (int64_t)(j0 + cc) * ldg);
+                }
+                if (tid < jb) rinv[j0 + tid] = __ldcg(dinv_g + j0 + tid);
+                __syncthreads();
+            }
             if (tid < ni) {
                 double x[8], Lk[8][8], inv[8];
 #pragma unroll
@@ -651,31 +670,33 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
 
     // ---- 3. finish: POTRF / TRSM for panel tiles, then store (each tile is written once) ----
     if (J < nbp) {
+        uint32_t* sub = F.sub_done + F.bbase[s] + J;     // counts the published 8-column blocks of L_JJ: (epoch-1)*16 + blocks
+        const uint32_t sbase = (epoch - 1u) * 16u;
         if (I == J) {
-            partial_chol([Cs](int j) { return Cs + j * CLD; }, nj, nj, c0 + j0, D.fail_col, D.dinv);
+            // every finished 8-column block of L_JJ is stored and announced at once: the TRSM tiles of this block column
+            // run one sub-step behind this POTRF instead of after it (the chain POTRF -> TRSM -> POTRF of the front)
+            auto pub = [&](int js, int jbs) {
+                if (tid >= NT / 2) {                     // warps 4..7 store, warp 0 goes on with the next diagonal block
+                    const int nr = nj - js;
+                    for (int idx = tid - NT / 2; idx < jbs * nr; idx += NT / 2) {
+                        const int cc = idx / nr, ii = idx - cc * nr;
+                        if (ii >= cc) P[(j0 + js + ii) + (int64_t)(j0 + js + cc) * ld] = Cs[(js + cc) * CLD + js + ii];
+                    }
+                    asm volatile("bar.sync 1, %0;" ::"n"(NT / 2) : "memory");
+                    if (tid == NT - 1) { __threadfence(); st_release(sub, sbase + (uint32_t)(js >> 3) + 1u); }
+                }
+            };
+            partial_chol([Cs](int j) { return Cs + j * CLD; }, nj, nj, c0 + j0, D.fail_col, D.dinv, pub);
+            TRACE(3);
         } else {
             double* Ls = pipe;
             double* rinv = pipe + CT_DOUBLES;
-            if (tid == 0) spin_until_ge(tdone + J * nbt + J, epoch);
-            __syncthreads();
-            {   // L_JJ and its pivot reciprocals: everything requested at once (cp.async, 16-byte chunks: j0, ld and CLD are even)
-                const int half = (nj + 1) >> 1;
-                const double* src = P + j0 + (int64_t)j0 * ld;
-                for (int idx = tid; idx < nj * half; idx += NT) {
-                    const int cc = idx / half, hh = idx - cc * half;
-                    cp_async16(Ls + cc * CLD + 2 * hh, src + (int64_t)cc * ld + 2 * hh, 16);
-                }
-                cp_async_commit();
-                if (tid < nj) rinv[tid] = __ldcg(D.dinv + c0 + j0 + tid);
-                cp_async_wait<0>();
+            trsm_tile(Cs, Ls, rinv, ni, nj, sub, sbase, P + j0 + (int64_t)j0 * ld, ld, D.dinv + c0 + j0);
+            TRACE(3);
+            for (int idx = tid; idx < ni * nj; idx += NT) {
+                const int mm = idx % ni, nn = idx / ni;
+                P[(i0 + mm) + (int64_t)(j0 + nn) * ld] = Cs[nn * CLD + mm];
             }
-            __syncthreads();
-            trsm_tile(Cs, Ls, rinv, ni, nj);
-        }
-        TRACE(3);
-        for (int idx = tid; idx < ni * nj; idx += NT) {
-            const int mm = idx % ni, nn = idx / ni;
-            if (I != J || mm >= nn) P[(i0 + mm) + (int64_t)(j0 + nn) * ld] = Cs[nn * CLD + mm];
         }
         __syncthreads();
         if (tid == 0) { __threadfence(); st_release(tdone + J * nbt + I, epoch); red_release_add(front_done + s, 1u); }
