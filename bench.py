@@ -86,6 +86,21 @@ def replica_x0(cfg, rank):
     return np.clip(cfg.x0 + rng.normal(0.0, sd, cfg.nx), cfg.x0_clip[0], cfg.x0_clip[1])
 
 
+def aggregate_over_ranks(dist, world, device, dev_ms, host_ms, n_it, n_f, steps, launches):
+    """Replicas only: the job's time is the MAX over ranks, its work the SUM over ranks.  Returns
+    (dev_ms_max, host_ms_max, total_iters, total_factorizations, total_steps, total_launches).  `dist` is
+    torch.distributed (nccl on the GPU box, gloo in the CPU tests); no data-path collective exists besides this one."""
+    if world <= 1:
+        return dev_ms, host_ms, int(n_it), int(n_f), int(steps), int(launches)
+    import torch
+    t = torch.tensor([dev_ms, host_ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    c = torch.tensor([n_it, n_f, steps, launches], dtype=torch.float64, device=device)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    tot = [int(v) for v in c.tolist()]
+    return float(t[0]), float(t[1]), tot[0], tot[1], tot[2], tot[3]
+
+
 # ======================================================================================================================
 # reference arm: the CPU oracle, as it stands
 # ======================================================================================================================
@@ -422,15 +437,8 @@ def run_own(args):
     dmma_tf, _ = nb.fp64_peak(1, 3)
 
     # ---- max over ranks / totals ----
-    if world > 1:
-        t = torch.tensor([dev_ms, host_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        c = torch.tensor([n_it, n_f, K, timed_launches], dtype=torch.float64, device=dev)
-        dist.all_reduce(c, op=dist.ReduceOp.SUM)
-        dev_ms_max, host_ms_max = float(t[0]), float(t[1])
-        tot_it, tot_f, tot_steps, tot_launch = (int(v) for v in c.tolist())
-    else:
-        dev_ms_max, host_ms_max, tot_it, tot_f, tot_steps, tot_launch = dev_ms, host_ms, n_it, n_f, K, timed_launches
+    dev_ms_max, host_ms_max, tot_it, tot_f, tot_steps, tot_launch = aggregate_over_ranks(
+        dist, world, dev, dev_ms, host_ms, n_it, n_f, K, timed_launches)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
