@@ -21,6 +21,8 @@ constexpr int NT = 256;
 constexpr int DLD = 65;                 // leading dimension of the staged 64x64 diagonal tile
 constexpr int SLD = 33;                 // ... of the transposed-access copy of a 32x32 diagonal block (small supernodes)
 constexpr int SB = 32;                  // column block of the small-supernode solves
+constexpr int SCH = 16, SREL = 1024;    // children / total relative indices a forward task keeps in shared memory (else: one by one)
+constexpr int FWD_WORK_DOUBLES = (SCH * 8 + (SCH + 4) * 4 + 7) / 8 + 2;   // child table behind the staging buffers
 // shared memory (doubles): vec[256] | ys[64] | part[4*64] | dv[2*32] | Lbt[32*33] | buf[2][DagPlan::sbuf]
 // (one staged column block: rows [j0, ld) x 32 columns; tiled tasks: Ld[64*65] aliases buf)
 constexpr int OFF_YS = 256, OFF_PART = OFF_YS + 64, OFF_DV = OFF_PART + 256, OFF_LBT = OFF_DV + 2 * SB, OFF_BUF = OFF_LBT + SB * SLD,
@@ -94,18 +96,59 @@ __device__ __forceinline__ void fwd_small(const DevSym& D, const DagPlan& F, int
     stage_block(D, q, 0, sm, F.sbuf);
     if (nblk > 1) stage_block(D, q, 1, sm, F.sbuf);
     for (int i = tid; i < q.r; i += NT) t[i] = (i < q.w) ? b[D.perm[q.c0 + i]] : 0.0;
-    const int ch0 = D.child_ptr[s], ch1 = D.child_ptr[s + 1];
-    for (int ci = ch0 + tid; ci < ch1; ci += NT) { const int c = D.child_idx[ci]; spin_until_ge(F.sol_done_f + c, epoch * (uint32_t)F.target_f[c]); }
+    const int ch0 = D.child_ptr[s], ch1 = D.child_ptr[s + 1], nch = ch1 - ch0;
+    // child table + the relative indices of all children: fetched BEFORE the children are waited for (static data); the
+    // contributions are then loaded in one round trip and added child by child (fixed order)
+    long long* chRp = reinterpret_cast<long long*>(sm + OFF_BUF + 2 * F.sbuf);   // [SCH] rel_ptr of the child (= offset of its ctr)
+    int* chOff = reinterpret_cast<int*>(chRp + SCH);                              // [SCH + 1] offset of its list in relS
+    int myc = -1;
+    if (tid < nch) {
+        myc = D.child_idx[ch0 + tid];
+        if (nch <= SCH) { const long long rp0 = D.rel_ptr[myc]; chRp[tid] = rp0; chOff[tid + 1] = (int)(D.rel_ptr[myc + 1] - rp0); }
+    }
+    __syncthreads();
+    if (tid == 0 && nch <= SCH) { int off = 0; for (int i = 0; i < nch; ++i) { const int mc = chOff[i + 1]; chOff[i] = off; off += mc; } chOff[nch] = off; }
+    __syncthreads();
+    const bool fast = nch <= SCH && chOff[nch <= SCH ? nch : 0] <= SREL;
+    const int tot = fast ? chOff[nch] : 0;
+    int who[SREL / NT], dst[SREL / NT];
+    long long src[SREL / NT];
+#pragma unroll
+    for (int k = 0; k < SREL / NT; ++k) {
+        const int idx = tid + k * NT;
+        who[k] = -1; dst[k] = 0; src[k] = 0;
+        if (idx < tot) {
+            int i = 0;
+            while (idx >= chOff[i + 1]) ++i;
+            who[k] = i; src[k] = chRp[i] + (idx - chOff[i]); dst[k] = D.rel[src[k]];
+        }
+    }
+    for (int ci = tid; ci < nch; ci += NT) {
+        const int c = (ci == tid && myc >= 0) ? myc : D.child_idx[ch0 + ci];
+        spin_until_ge(F.sol_done_f + c, epoch * (uint32_t)F.target_f[c]);
+    }
     __syncthreads();
     STRACE(1);
-    for (int ci = ch0; ci < ch1; ++ci) {
-        const int c = D.child_idx[ci];
-        const int64_t rp0 = D.rel_ptr[c];
-        const int mc = (int)(D.rel_ptr[c + 1] - rp0);
-        const double* cc = D.ctr + rp0;
-        const int32_t* __restrict__ rel = D.rel + rp0;
-        if (ci > ch0) __syncthreads();
-        for (int a = tid; a < mc; a += NT) t[rel[a]] += __ldcg(cc + a);
+    if (fast) {
+        double v[SREL / NT];
+#pragma unroll
+        for (int k = 0; k < SREL / NT; ++k) v[k] = who[k] >= 0 ? __ldcg(D.ctr + src[k]) : 0.0;
+        for (int i = 0; i < nch; ++i) {
+#pragma unroll
+            for (int k = 0; k < SREL / NT; ++k)
+                if (who[k] == i) t[dst[k]] += v[k];
+            __syncthreads();
+        }
+    } else {
+        for (int ci = ch0; ci < ch1; ++ci) {
+            const int c = D.child_idx[ci];
+            const int64_t rp0 = D.rel_ptr[c];
+            const int mc = (int)(D.rel_ptr[c + 1] - rp0);
+            const double* cc = D.ctr + rp0;
+            const int32_t* __restrict__ rel = D.rel + rp0;
+            if (ci > ch0) __syncthreads();
+            for (int a = tid; a < mc; a += NT) t[rel[a]] += __ldcg(cc + a);
+        }
     }
     STRACE(2);
     for (int k = 0; k < nblk; ++k) {
@@ -480,7 +523,7 @@ cudaError_t configure_solve_kernels(int max_smem_bytes, int small_max_r, int* ct
     int sbuf = ld_even(small_max_r) * SB;
     if (2 * sbuf < TILE * DLD) sbuf = (TILE * DLD + 1) / 2 + 1;      // the staged diagonal tile of the tiled tasks aliases the buffers
     sbuf = (sbuf + 1) & ~1;
-    const size_t bytes = (size_t)(OFF_BUF + 2 * sbuf) * sizeof(double);
+    const size_t bytes = (size_t)(OFF_BUF + 2 * sbuf + FWD_WORK_DOUBLES) * sizeof(double);
     if (bytes > (size_t)max_smem_bytes) return cudaErrorInvalidValue;
     cudaError_t e = cudaFuncSetAttribute(solve_dag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes - 256);
     if (e != cudaSuccess) return e;
