@@ -616,7 +616,7 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
         TRY(run_solve(h, V.dy));
         pt.end();
         pt.begin(&S.ms_vector);
-        launch_step(M, V, mu_, tau_, st); h->launches += 2;                    // S8-S9
+        launch_step(M, V, mu_, tau_, st); h->launches += 1;                    // S8-S9
         launch_update(M, V, h->D.fail_col, st); h->launches++;                 // S10: Eq. (26)
         pt.end();
         return NMPC_OK;
@@ -627,7 +627,7 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
         launch_model_eval(M, V.y, V.wp, V.wm, nullptr, V.c, V.gradf, V.Jval, V.Wval, st); h->launches++;
         pt.end();
         pt.begin(&S.ms_vector);
-        launch_residuals(M, V, o.gamma, st); h->launches += 2;
+        launch_residuals(M, V, o.gamma, st); h->launches += 1;
         CK(cudaMemcpyAsync(hs, V.scal, sizeof(double) * 10, cudaMemcpyDeviceToHost, st));
         if (pending) CK(cudaMemcpyAsync(flag, h->D.fail_col, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
@@ -695,7 +695,7 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
     }
 done:
     h->have_state = true;
-    launch_objective(M, V, st); h->launches += 2;
+    launch_objective(M, V, st); h->launches += 1;
     CK(cudaMemcpyAsync(hs + 9, V.scal + 9, sizeof(double), cudaMemcpyDeviceToHost, st));
     if (y_inout) CK(cudaMemcpyAsync(y_inout, V.y, sizeof(double) * M.n, cudaMemcpyDeviceToDevice, st));
     CK(cudaStreamSynchronize(st));

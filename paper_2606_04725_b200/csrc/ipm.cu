@@ -131,6 +131,22 @@ __device__ __forceinline__ void block_reduce(Red<NV>& a, const int* ops, double*
     }
 }
 
+// The block whose ticket is the last one finishes the reduction over the per-block partials (fixed order over the blocks, so the
+// result does not depend on which block that is) -- saves the one-block finalize launch.  Tickets live in scal[12..14].
+__device__ __forceinline__ bool last_block_arrives(double* ticket_slot) {
+    __shared__ int s_last;
+    unsigned* ticket = reinterpret_cast<unsigned*>(ticket_slot);
+    __syncthreads();                                     // thread 0 has written this block's partials (block_reduce)
+    if (threadIdx.x == 0) {
+        __threadfence();
+        const unsigned t = atomicAdd(ticket, 1u);
+        s_last = (t == gridDim.x - 1);
+        if (s_last) { *ticket = 0u; __threadfence(); }
+    }
+    __syncthreads();
+    return s_last != 0;
+}
+
 // ------------------------------------------------------------------------------------------------------------
 // S1 cold start: push y0 into the interior, slacks from c, multipliers mu0/(.)
 // ------------------------------------------------------------------------------------------------------------
@@ -213,17 +229,13 @@ __global__ void __launch_bounds__(NT) residual_kernel(DevModel M, IpmVectors V, 
     }
     const int ops[7] = {0, 0, 0, 0, 1, 2, 2};
     block_reduce<7>(a, ops, V.partial + (int64_t)blockIdx.x * 8);
-}
-
-__global__ void __launch_bounds__(NT) finalize_residual_kernel(IpmVectors V, int nblocks) {
-    Red<7> a;
+    if (!last_block_arrives(V.scal + 12)) return;
     a.v[0] = a.v[1] = a.v[2] = 0.0; a.v[3] = -INF; a.v[4] = INF; a.v[5] = 0.0; a.v[6] = 0.0;
-    for (int b = threadIdx.x; b < nblocks; b += NT) {
+    for (int b = threadIdx.x; b < (int)gridDim.x; b += NT) {
         const double* p = V.partial + (int64_t)b * 8;
-        a.v[0] = fmax(a.v[0], p[0]); a.v[1] = fmax(a.v[1], p[1]); a.v[2] = fmax(a.v[2], p[2]);
-        a.v[3] = fmax(a.v[3], p[3]); a.v[4] = fmin(a.v[4], p[4]); a.v[5] += p[5]; a.v[6] += p[6];
+        a.v[0] = fmax(a.v[0], __ldcg(p)); a.v[1] = fmax(a.v[1], __ldcg(p + 1)); a.v[2] = fmax(a.v[2], __ldcg(p + 2));
+        a.v[3] = fmax(a.v[3], __ldcg(p + 3)); a.v[4] = fmin(a.v[4], __ldcg(p + 4)); a.v[5] += __ldcg(p + 5); a.v[6] += __ldcg(p + 6);
     }
-    const int ops[7] = {0, 0, 0, 0, 1, 2, 2};
     block_reduce<7>(a, ops, V.scal);
 }
 
@@ -299,12 +311,9 @@ __global__ void __launch_bounds__(NT) step_kernel(DevModel M, IpmVectors V, doub
     }
     const int ops[2] = {1, 1};
     block_reduce<2>(a, ops, V.partial + (int64_t)blockIdx.x * 8);
-}
-
-__global__ void __launch_bounds__(NT) finalize_step_kernel(IpmVectors V, int nblocks) {
-    Red<2> a; a.v[0] = 1.0; a.v[1] = 1.0;
-    for (int b = threadIdx.x; b < nblocks; b += NT) { a.v[0] = fmin(a.v[0], V.partial[(int64_t)b * 8]); a.v[1] = fmin(a.v[1], V.partial[(int64_t)b * 8 + 1]); }
-    const int ops[2] = {1, 1};
+    if (!last_block_arrives(V.scal + 13)) return;
+    a.v[0] = 1.0; a.v[1] = 1.0;
+    for (int b = threadIdx.x; b < (int)gridDim.x; b += NT) { a.v[0] = fmin(a.v[0], __ldcg(V.partial + (int64_t)b * 8)); a.v[1] = fmin(a.v[1], __ldcg(V.partial + (int64_t)b * 8 + 1)); }
     block_reduce<2>(a, ops, V.scal + 7);
 }
 
@@ -331,11 +340,9 @@ __global__ void __launch_bounds__(NT) objective_kernel(DevModel M, IpmVectors V)
     }
     const int ops[1] = {2};
     block_reduce<1>(a, ops, V.partial + (int64_t)blockIdx.x * 8);
-}
-__global__ void __launch_bounds__(NT) finalize_objective_kernel(IpmVectors V, int nblocks) {
-    Red<1> a; a.v[0] = 0.0;
-    for (int b = threadIdx.x; b < nblocks; b += NT) a.v[0] += V.partial[(int64_t)b * 8];
-    const int ops[1] = {2};
+    if (!last_block_arrives(V.scal + 14)) return;
+    a.v[0] = 0.0;
+    for (int b = threadIdx.x; b < (int)gridDim.x; b += NT) a.v[0] += __ldcg(V.partial + (int64_t)b * 8);
     block_reduce<1>(a, ops, V.scal + 9);
 }
 
@@ -369,7 +376,6 @@ void launch_warm_push(const DevModel& M, const IpmVectors& V, double warm_push, 
 void launch_residuals(const DevModel& M, const IpmVectors& V, double gamma, cudaStream_t st) {
     const int nb = red_blocks(M.n * GV + M.m);
     residual_kernel<<<nb, NT, 0, st>>>(M, V, gamma);
-    finalize_residual_kernel<<<1, NT, 0, st>>>(V, nb);
 }
 void launch_sigma_rhs(const DevModel& M, const IpmVectors& V, double mu, cudaStream_t st) {
     sigma_rows_kernel<<<blocks_for(M.m), NT, 0, st>>>(M, V, mu);
@@ -378,7 +384,6 @@ void launch_sigma_rhs(const DevModel& M, const IpmVectors& V, double mu, cudaStr
 void launch_step(const DevModel& M, const IpmVectors& V, double mu, double tau, cudaStream_t st) {
     const int nb = red_blocks(M.n + M.m);
     step_kernel<<<nb, NT, 0, st>>>(M, V, mu, tau);
-    finalize_step_kernel<<<1, NT, 0, st>>>(V, nb);
 }
 void launch_update(const DevModel& M, const IpmVectors& V, const int32_t* fail_col, cudaStream_t st) {
     update_kernel<<<blocks_for(M.n + M.m), NT, 0, st>>>(M, V, fail_col);
@@ -386,7 +391,6 @@ void launch_update(const DevModel& M, const IpmVectors& V, const int32_t* fail_c
 void launch_objective(const DevModel& M, const IpmVectors& V, cudaStream_t st) {
     const int nb = red_blocks(M.n);
     objective_kernel<<<nb, NT, 0, st>>>(M, V);
-    finalize_objective_kernel<<<1, NT, 0, st>>>(V, nb);
 }
 
 }  // namespace nmpc
