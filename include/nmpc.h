@@ -85,7 +85,7 @@ typedef struct {
     int32_t relax_small;         /* always merge a child supernode into its parent if the merged width <= this */
     double  relax_zeros;         /* else merge if the explicit zeros introduced stay below this fraction      */
     int32_t smem_front_max;      /* fronts with <= this many rows run in the one-CTA shared-memory kernel     */
-    int32_t use_graph;           /* capture factor / solve launch sequences in CUDA graphs                    */
+    int32_t use_graph;           /* replay one IPM iteration (S6-S10 + the next S2) as a CUDA graph, 1 launch/iter  */
     /* IPM (Algorithm 2) */
     double gamma, eps_outer, mu0, mu_warm, kappa_eps, kappa_mu, theta_mu, tau_min, kappa_push, s_floor, s_max;
     int32_t max_iter;
@@ -136,7 +136,7 @@ void        nmpc_symbolic_destroy(nmpc_symbolic sym);
 
 /* ---- Alg. 2 lines 10-12: analysis once per structure; uploads all integer maps; allocates L.  cuda_stream is a
  *      cudaStream_t.  NULL = the library creates its own blocking stream (ordered with the legacy default stream,
- *      which itself cannot carry the CUDA-graph capture of the factor / solve launch sequences).               */
+ *      which itself cannot carry the CUDA-graph capture of the IPM iteration).                                 */
 nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const nmpc_options* opt,
                          void* cuda_stream, nmpc_handle* out);
 

@@ -49,6 +49,9 @@ struct nmpc_handle_s {
     int nmult = 0;
     std::string err;
     cudaEvent_t ev[2] = {nullptr, nullptr};
+    double* d_par = nullptr;           // device {mu, tau, (uint32) factor call number, (uint32) solve call number}: read by the graph's kernels
+    cudaGraphExec_t iter_graph = nullptr;   // one IPM iteration (S6-S10 + the next S2), see capture_iteration_graph
+    bool graph_failed = false;
 };
 
 namespace {
@@ -251,7 +254,7 @@ nmpc_status next_epoch(nmpc_handle_s* h, bool factor, uint32_t* out) {
 nmpc_status run_factor(nmpc_handle_s* h, double eta, int64_t* info) {
     uint32_t epoch = 0;
     TRY(next_epoch(h, true, &epoch));
-    launch_factor(h->D, h->F, h->d_Kval, eta, epoch, h->stream); h->launches += 1;
+    launch_factor(h->D, h->F, h->d_Kval, eta, epoch, nullptr, h->stream); h->launches += 1;
     int32_t* flag = reinterpret_cast<int32_t*>(h->h_pinned + 16);
     CK(cudaMemcpyAsync(flag, h->D.fail_col, sizeof(int32_t), cudaMemcpyDeviceToHost, h->stream));
     CK(cudaStreamSynchronize(h->stream));
@@ -271,7 +274,39 @@ nmpc_status run_factor(nmpc_handle_s* h, double eta, int64_t* info) {
 nmpc_status run_solve(nmpc_handle_s* h, double* rhs) {       // in place, async
     uint32_t epoch = 0;
     TRY(next_epoch(h, false, &epoch));
-    launch_solve(h->D, h->F, rhs, h->d_x, epoch, h->stream); h->launches += 1;
+    launch_solve(h->D, h->F, rhs, h->d_x, epoch, nullptr, h->stream); h->launches += 1;
+    return NMPC_OK;
+}
+
+// One IPM iteration as a CUDA graph (opt.use_graph): parameter upload {mu, tau, call numbers} from pinned memory, S6 (Sigma, rhs),
+// a3 (assembly), a4 (factorization), a5 (solves), S8-S10 (step, device-guarded update), then S2 of the NEXT iteration (model
+// evaluation, residuals) and the read-back of the reduced scalars + pivot flag.  The kernels take mu / tau / the call numbers
+// from device memory (d_par), so the same executable graph is replayed every iteration with one launch.
+nmpc_status capture_iteration_graph(nmpc_handle_s* h) {
+    const DevModel& M = h->M;
+    const IpmVectors& V = h->V;
+    cudaStream_t st = h->stream;
+    double* hp = h->h_pinned + 24;                       // pinned mirror of d_par
+    double* hs = h->h_pinned;
+    int32_t* flag = reinterpret_cast<int32_t*>(h->h_pinned + 16);
+    const uint32_t* epo = reinterpret_cast<const uint32_t*>(h->d_par + 2);
+    cudaGraph_t g = nullptr;
+    if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); h->graph_failed = true; return NMPC_OK; }
+    cudaMemcpyAsync(h->d_par, hp, 4 * sizeof(double), cudaMemcpyHostToDevice, st);
+    launch_sigma_rhs(M, V, 0.0, h->d_par, st);
+    launch_assemble_K(M, V.Jval, V.Wval, V.sigx, V.q, 0.0, V.Kval, st);
+    launch_factor(h->D, h->F, h->d_Kval, 0.0, 0u, epo, st);
+    cudaMemcpyAsync(V.dy, V.b, sizeof(double) * M.n, cudaMemcpyDeviceToDevice, st);
+    launch_solve(h->D, h->F, V.dy, h->d_x, 0u, epo, st);
+    launch_step(M, V, 0.0, 0.0, h->d_par, st);
+    launch_update(M, V, h->D.fail_col, st);
+    launch_model_eval(M, V.y, V.wp, V.wm, nullptr, V.c, V.gradf, V.Jval, V.Wval, st);
+    launch_residuals(M, V, h->opt.gamma, st);
+    cudaMemcpyAsync(hs, V.scal, sizeof(double) * 10, cudaMemcpyDeviceToHost, st);
+    cudaMemcpyAsync(flag, h->D.fail_col, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+    if (cudaStreamEndCapture(st, &g) != cudaSuccess || !g) { cudaGetLastError(); h->graph_failed = true; return NMPC_OK; }
+    if (cudaGraphInstantiate(&h->iter_graph, g, 0) != cudaSuccess) { cudaGetLastError(); h->iter_graph = nullptr; h->graph_failed = true; }
+    cudaGraphDestroy(g);
     return NMPC_OK;
 }
 
@@ -390,6 +425,7 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
             TRY(dalloc(h, m, &V.dsp)); TRY(dalloc(h, m, &V.dsm)); TRY(dalloc(h, m, &V.dwp)); TRY(dalloc(h, m, &V.dwm));
             TRY(dalloc(h, n, &V.dzL)); TRY(dalloc(h, n, &V.dzU));
             TRY(dalloc(h, (size_t)RED_BLOCKS * 8, &V.partial)); TRY(dalloc(h, (size_t)NSCAL, &V.scal));
+            TRY(dalloc(h, 4, &h->d_par));
             pinned += (size_t)mm.desc.nx + (size_t)mm.desc.N * mm.desc.nr + n;
         }
         h->pinned_doubles = pinned;
@@ -408,6 +444,7 @@ void nmpc_destroy(nmpc_handle h) {
     if (!h) return;
     for (void* p : h->allocs) cudaFree(p);
     if (h->h_pinned) cudaFreeHost(h->h_pinned);
+    if (h->iter_graph) cudaGraphExecDestroy(h->iter_graph);
     if (h->ev[0]) cudaEventDestroy(h->ev[0]);
     if (h->ev[1]) cudaEventDestroy(h->ev[1]);
     if (h->own_stream) cudaStreamDestroy(h->stream);
@@ -593,6 +630,9 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
     // scalars -- one host synchronisation per IPM iteration.  A failed pivot leaves the iterate untouched (update_kernel
     // checks the flag), so the inertia-correction retry below starts from exactly the state of the synchronous flow.
     const bool async = !o.time_phases;
+    if (async && o.use_graph && !h->iter_graph && !h->graph_failed) TRY(capture_iteration_graph(h));
+    const bool graph = async && o.use_graph && h->iter_graph != nullptr;
+    bool top_done = false;                               // the previous graph replay already ran S2 + the read-back
     bool pending = false;                                // a factorization whose flag has not been checked yet
     double pend_mu = 0.0, pend_tau = 0.0;
     int32_t* flag = reinterpret_cast<int32_t*>(h->h_pinned + 16);
@@ -616,20 +656,23 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
         TRY(run_solve(h, V.dy));
         pt.end();
         pt.begin(&S.ms_vector);
-        launch_step(M, V, mu_, tau_, st); h->launches += 1;                    // S8-S9
+        launch_step(M, V, mu_, tau_, nullptr, st); h->launches += 1;                    // S8-S9
         launch_update(M, V, h->D.fail_col, st); h->launches++;                 // S10: Eq. (26)
         pt.end();
         return NMPC_OK;
     };
     while (true) {
         // S2: evaluate c, grad f, J, W (K_SIMD of the paper, Alg. 2 line 5) and the residuals of Eq. (9)
-        pt.begin(&S.ms_eval);
-        launch_model_eval(M, V.y, V.wp, V.wm, nullptr, V.c, V.gradf, V.Jval, V.Wval, st); h->launches++;
-        pt.end();
-        pt.begin(&S.ms_vector);
-        launch_residuals(M, V, o.gamma, st); h->launches += 1;
-        CK(cudaMemcpyAsync(hs, V.scal, sizeof(double) * 10, cudaMemcpyDeviceToHost, st));
-        if (pending) CK(cudaMemcpyAsync(flag, h->D.fail_col, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+        if (!top_done) {
+            pt.begin(&S.ms_eval);
+            launch_model_eval(M, V.y, V.wp, V.wm, nullptr, V.c, V.gradf, V.Jval, V.Wval, st); h->launches++;
+            pt.end();
+            pt.begin(&S.ms_vector);
+            launch_residuals(M, V, o.gamma, st); h->launches += 1;
+            CK(cudaMemcpyAsync(hs, V.scal, sizeof(double) * 10, cudaMemcpyDeviceToHost, st));
+            if (pending) CK(cudaMemcpyAsync(flag, h->D.fail_col, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+        }
+        top_done = false;
         CK(cudaStreamSynchronize(st));
         pt.end();
         if (pending) {
@@ -665,8 +708,24 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
             Emu = err_mu(mu);
         }
         const double tau = std::max(o.tau_min, 1.0 - mu);                      // S5
+        if (graph) {                                     // S6-S10 and the next S2 as one graph replay
+            uint32_t ef = 0, es = 0;
+            TRY(next_epoch(h, true, &ef));
+            TRY(next_epoch(h, false, &es));
+            double* hp = h->h_pinned + 24;
+            hp[0] = mu; hp[1] = tau;
+            uint32_t* he = reinterpret_cast<uint32_t*>(hp + 2);
+            he[0] = ef; he[1] = es;
+            CK(cudaGraphLaunch(h->iter_graph, st));
+            h->launches += 10;
+            ++nfact;
+            pending = true; pend_mu = mu; pend_tau = tau; top_done = true;
+            if (trace && it < trace_cap) { trace[it].mu = mu; trace[it].E0 = E0; trace[it].Emu = Emu; trace[it].eta = 0.0; trace[it].alpha_pr = trace[it].alpha_du = 0.0; }
+            ++it;
+            continue;
+        }
         pt.begin(&S.ms_vector);
-        launch_sigma_rhs(M, V, mu, st); h->launches += 2;                      // S6
+        launch_sigma_rhs(M, V, mu, nullptr, st); h->launches += 2;                      // S6
         pt.end();
         pt.begin(&S.ms_assemble);
         launch_assemble_K(M, V.Jval, V.Wval, V.sigx, V.q, 0.0, V.Kval, st); h->launches++;
@@ -676,7 +735,7 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
         if (async) {
             uint32_t epoch = 0;
             TRY(next_epoch(h, true, &epoch));
-            launch_factor(h->D, h->F, h->d_Kval, 0.0, epoch, st); h->launches += 1;
+            launch_factor(h->D, h->F, h->d_Kval, 0.0, epoch, nullptr, st); h->launches += 1;
             pending = true; pend_mu = mu; pend_tau = tau;
         } else {
             pt.begin(&S.ms_factor);

@@ -101,12 +101,15 @@ struct DagPlan {
 // ---- factor.cu ----
 // one_cta_per_sm: latency mode (small problems whose largest fronts then fit one CTA's shared memory), else two CTAs per SM
 cudaError_t configure_factor_kernels(int max_smem_bytes, bool one_cta_per_sm, int* ctas_per_sm, size_t* smem_bytes, int* small_max_r);
-void launch_factor(const DevSym& D, const DagPlan& F, const double* Kval, double eta, uint32_t epoch, cudaStream_t st);
+// epoch_dev (may be null): device words {factor call number, solve call number} that override `epoch` (CUDA-graph replay)
+void launch_factor(const DevSym& D, const DagPlan& F, const double* Kval, double eta, uint32_t epoch, const uint32_t* epoch_dev,
+                   cudaStream_t st);
 void launch_reset_fail(const DevSym& D, cudaStream_t st);                                   // fail_col = INT_MAX
 // ---- solve.cu ----
 cudaError_t configure_solve_kernels(int max_smem_bytes, int small_max_r, int* ctas_per_sm, size_t* smem_bytes, int* sbuf_doubles);
 // rhs_inout (original ordering, n doubles) is overwritten by K^-1 rhs; x is the handle's permuted work vector
-void launch_solve(const DevSym& D, const DagPlan& F, double* rhs_inout, double* x, uint32_t epoch, cudaStream_t st);
+void launch_solve(const DevSym& D, const DagPlan& F, double* rhs_inout, double* x, uint32_t epoch, const uint32_t* epoch_dev,
+                  cudaStream_t st);
 
 // ---- ipm.cu ----
 struct DevModel {                 // device copies of the model maps (symbolic.h: ModelMaps) + parameters
@@ -143,8 +146,9 @@ void launch_cold_init_y(const DevModel& M, const IpmVectors& V, const double* u_
 void launch_cold_init_s(const DevModel& M, const IpmVectors& V, double gamma, double s_floor, double mu0, cudaStream_t st);
 void launch_warm_push(const DevModel& M, const IpmVectors& V, double warm_push, cudaStream_t st);
 void launch_residuals(const DevModel& M, const IpmVectors& V, double gamma, cudaStream_t st);
-void launch_sigma_rhs(const DevModel& M, const IpmVectors& V, double mu, cudaStream_t st);
-void launch_step(const DevModel& M, const IpmVectors& V, double mu, double tau, cudaStream_t st);
+// par (may be null): device doubles {mu, tau} that override the scalar arguments (CUDA-graph replay)
+void launch_sigma_rhs(const DevModel& M, const IpmVectors& V, double mu, const double* par, cudaStream_t st);
+void launch_step(const DevModel& M, const IpmVectors& V, double mu, double tau, const double* par, cudaStream_t st);
 // fail_col (may be null): device flag of the factorization; the update is skipped when it reports a failed pivot
 void launch_update(const DevModel& M, const IpmVectors& V, const int32_t* fail_col, cudaStream_t st);
 void launch_objective(const DevModel& M, const IpmVectors& V, cudaStream_t st);

@@ -713,9 +713,11 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
     TRACE(4);
 }
 
-__global__ void __launch_bounds__(NT, 2) factor_dag_kernel(DevSym D, DagPlan F, const double* __restrict__ Kval, double eta, uint32_t epoch) {
+__global__ void __launch_bounds__(NT, 2) factor_dag_kernel(DevSym D, DagPlan F, const double* __restrict__ Kval, double eta, uint32_t epoch,
+                                                              const uint32_t* __restrict__ epoch_dev) {
     extern __shared__ __align__(16) double sm[];
     __shared__ int s_task;
+    if (epoch_dev) epoch = epoch_dev[0];                 // graph replay: the call number comes from device memory
     const uint32_t base = (epoch - 1u) * (uint32_t)(F.n_ftasks + (int)gridDim.x);
     while (true) {
         __syncthreads();
@@ -756,8 +758,9 @@ cudaError_t configure_factor_kernels(int max_smem_bytes, bool one_cta_per_sm, in
     return cudaSuccess;
 }
 
-void launch_factor(const DevSym& D, const DagPlan& F, const double* Kval, double eta, uint32_t epoch, cudaStream_t st) {
-    if (F.n_ftasks > 0) factor_dag_kernel<<<F.fgrid, NT, F.fsmem, st>>>(D, F, Kval, eta, epoch);
+void launch_factor(const DevSym& D, const DagPlan& F, const double* Kval, double eta, uint32_t epoch, const uint32_t* epoch_dev,
+                   cudaStream_t st) {
+    if (F.n_ftasks > 0) factor_dag_kernel<<<F.fgrid, NT, F.fsmem, st>>>(D, F, Kval, eta, epoch, epoch_dev);
 }
 void launch_reset_fail(const DevSym& D, cudaStream_t st) { reset_fail_kernel<<<1, 1, 0, st>>>(D.fail_col); }
 

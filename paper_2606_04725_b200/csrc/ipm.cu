@@ -242,7 +242,8 @@ __global__ void __launch_bounds__(NT) residual_kernel(DevModel M, IpmVectors V, 
 // ------------------------------------------------------------------------------------------------------------
 // S6: Sigma, q, t (rows) then Sigma_x and the right-hand side b of Eq. 17 (variables)
 // ------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(NT) sigma_rows_kernel(DevModel M, IpmVectors V, double mu) {
+__global__ void __launch_bounds__(NT) sigma_rows_kernel(DevModel M, IpmVectors V, double mu, const double* __restrict__ par) {
+    if (par) mu = par[0];                                // graph replay: the barrier parameter comes from device memory
     const int64_t r = blockIdx.x * (int64_t)NT + threadIdx.x;
     if (r >= M.m) return;
     const double sp = V.sp[r], sm = V.sm[r];
@@ -251,7 +252,8 @@ __global__ void __launch_bounds__(NT) sigma_rows_kernel(DevModel M, IpmVectors V
     V.t[r] = qp * V.r_pp[r] + mu / sp - qm * V.r_pm[r] - mu / sm;
 }
 
-__global__ void __launch_bounds__(NT) sigma_vars_kernel(DevModel M, IpmVectors V, double mu) {
+__global__ void __launch_bounds__(NT) sigma_vars_kernel(DevModel M, IpmVectors V, double mu, const double* __restrict__ par) {
+    if (par) mu = par[0];
     const int64_t gtid = blockIdx.x * (int64_t)NT + threadIdx.x;
     const int64_t i = gtid / GV;                         // GV lanes per variable for the J^T t product
     const int gl = (int)(gtid % GV);
@@ -277,7 +279,8 @@ __global__ void __launch_bounds__(NT) sigma_vars_kernel(DevModel M, IpmVectors V
 // ------------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ double max_step(double v, double dv, double tau) { return dv < 0.0 ? fmin(1.0, -tau * v / dv) : 1.0; }
 
-__global__ void __launch_bounds__(NT) step_kernel(DevModel M, IpmVectors V, double mu, double tau) {
+__global__ void __launch_bounds__(NT) step_kernel(DevModel M, IpmVectors V, double mu, double tau, const double* __restrict__ par) {
+    if (par) { mu = par[0]; tau = par[1]; }
     Red<2> a; a.v[0] = 1.0; a.v[1] = 1.0;
     const int64_t total = M.n + M.m;
     for (int64_t idx = blockIdx.x * (int64_t)NT + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * NT) {
@@ -377,13 +380,13 @@ void launch_residuals(const DevModel& M, const IpmVectors& V, double gamma, cuda
     const int nb = red_blocks(M.n * GV + M.m);
     residual_kernel<<<nb, NT, 0, st>>>(M, V, gamma);
 }
-void launch_sigma_rhs(const DevModel& M, const IpmVectors& V, double mu, cudaStream_t st) {
-    sigma_rows_kernel<<<blocks_for(M.m), NT, 0, st>>>(M, V, mu);
-    sigma_vars_kernel<<<blocks_for(M.n * GV), NT, 0, st>>>(M, V, mu);
+void launch_sigma_rhs(const DevModel& M, const IpmVectors& V, double mu, const double* par, cudaStream_t st) {
+    sigma_rows_kernel<<<blocks_for(M.m), NT, 0, st>>>(M, V, mu, par);
+    sigma_vars_kernel<<<blocks_for(M.n * GV), NT, 0, st>>>(M, V, mu, par);
 }
-void launch_step(const DevModel& M, const IpmVectors& V, double mu, double tau, cudaStream_t st) {
+void launch_step(const DevModel& M, const IpmVectors& V, double mu, double tau, const double* par, cudaStream_t st) {
     const int nb = red_blocks(M.n + M.m);
-    step_kernel<<<nb, NT, 0, st>>>(M, V, mu, tau);
+    step_kernel<<<nb, NT, 0, st>>>(M, V, mu, tau, par);
 }
 void launch_update(const DevModel& M, const IpmVectors& V, const int32_t* fail_col, cudaStream_t st) {
     update_kernel<<<blocks_for(M.n + M.m), NT, 0, st>>>(M, V, fail_col);

@@ -498,9 +498,10 @@ __device__ __forceinline__ void bwd_tiled(const DevSym& D, const DagPlan& F, int
     }
 }
 
-__global__ void __launch_bounds__(NT, 2) solve_dag_kernel(DevSym D, DagPlan F, double* b, double* x, uint32_t epoch) {
+__global__ void __launch_bounds__(NT, 2) solve_dag_kernel(DevSym D, DagPlan F, double* b, double* x, uint32_t epoch, const uint32_t* __restrict__ epoch_dev) {
     extern __shared__ __align__(16) double sm[];
     __shared__ int s_task;
+    if (epoch_dev) epoch = epoch_dev[1];                 // graph replay: the call number comes from device memory
     const uint32_t base = (epoch - 1u) * (uint32_t)(F.n_stasks + (int)gridDim.x);
     while (true) {
         __syncthreads();
@@ -536,8 +537,9 @@ cudaError_t configure_solve_kernels(int max_smem_bytes, int small_max_r, int* ct
     return cudaSuccess;
 }
 
-void launch_solve(const DevSym& D, const DagPlan& F, double* rhs_inout, double* x, uint32_t epoch, cudaStream_t st) {
-    if (F.n_stasks > 0) solve_dag_kernel<<<F.sgrid, NT, F.ssmem, st>>>(D, F, rhs_inout, x, epoch);
+void launch_solve(const DevSym& D, const DagPlan& F, double* rhs_inout, double* x, uint32_t epoch, const uint32_t* epoch_dev,
+                  cudaStream_t st) {
+    if (F.n_stasks > 0) solve_dag_kernel<<<F.sgrid, NT, F.ssmem, st>>>(D, F, rhs_inout, x, epoch, epoch_dev);
 }
 
 }  // namespace nmpc

@@ -408,3 +408,17 @@ def test_graph_and_plain_launch_paths_agree():
         assert h.launch_count() > 0
         h.close()
     assert np.array_equal(xs[0], xs[1])
+    # the IPM iteration replayed as one CUDA graph (parameters and call numbers read from device memory) must reproduce
+    # the plain launch sequence bit for bit, cold and warm
+    ys, its = [], []
+    for use_graph in (0, 1):
+        h = nb.Handle(None, nb.make_ocp(cfg), nb.default_options(use_graph=use_graph))
+        y = torch.zeros(cfg.n, dtype=torch.float64, device=DEV)
+        h.update_params(dev(cfg.x0), dev(cfg.ref_for_solve(0)))
+        r0 = h.ipm_solve(0, y)
+        h.update_params(dev(np.clip(cfg.x0 + 0.01, *cfg.x0_clip)), dev(cfg.ref_for_solve(1)))
+        r1 = h.ipm_solve(1, y)
+        ys.append(y.cpu().numpy().copy()); its.append((r0["iters"], r1["iters"], r0["status"], r1["status"]))
+        h.close()
+    assert its[0] == its[1] and its[0][2] == 0 and its[0][3] == 0
+    assert np.array_equal(ys[0], ys[1])
