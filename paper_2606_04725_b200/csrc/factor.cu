@@ -4,13 +4,16 @@
 // The host analysis emits a topologically ordered task list (api.cu: build_plan).  CTAs claim tasks in order from an atomic
 // counter and wait on completion flags (acquire/release at gpu scope) instead of kernel boundaries:
 //   task type 0, small front (r <= small_max_r): ONE CTA assembles the whole front in shared memory (packed lower triangle):
-//          K entries through the scatter map + extend-add of the children's update matrices, pulled in fixed child order;
-//          blocked partial Cholesky of its w pivot columns; writes the panel of L and the (r-w)^2 update matrix.
+//          K entries through the scatter map (before it waits for its children), extend-add of the children's update matrices
+//          (child tables and relative indices fetched before the wait; small children loaded as one group, added in fixed
+//          child order); panel-blocked partial Cholesky of its w pivot columns (partial_chol); publishes the (r-w)^2 update
+//          matrix, then writes the panel of L.
 //   task type 1, tile (I,J) of a tiled front (r > small_max_r; the front lives in HBM as panel + update storage), LEFT-looking:
-//          acc = sum_k X(I,k) X(J,k)^T over the finished tiles of block rows I and J (fp64 DMMA mma.sync.m8n8k4, operands
-//          streamed with cp.async.cg through a 3-stage shared-memory ring, waiting on each 64-column block's flags as it is
-//          reached); C = assembled tile (K entries + children's contributions) - acc; then POTRF (I == J) or TRSM against the
-//          finished diagonal tile (I > J) in shared memory; each tile of L / of the update matrix is written exactly once.
+//          assembles its tile first (K entries + children's contributions); acc = sum_k X(I,k) X(J,k)^T over the finished
+//          tiles of block rows I and J (fp64 DMMA mma.sync.m8n8k4, operands streamed with cp.async.cg through a 4-stage
+//          shared-memory ring; a chunk is multiplied before the warps wait for the flags of the chunk three ahead); C -= acc;
+//          then POTRF (I == J; every finished 8-column block of L_JJ is stored and announced at once) or TRSM (I > J; streams
+//          those blocks and runs one sub-step behind the POTRF) in shared memory; each tile is written exactly once.
 // In-order claiming of a topological order cannot deadlock: the lowest-numbered unfinished task depends only on finished ones.
 // fp64 throughout, no floating-point atomics, fixed summation order -> bitwise reproducible.
 #include <climits>

@@ -2,10 +2,12 @@
 // L v = P b (leaves -> root), L^T Omega = v (root -> leaves), dy = P^T Omega, as ONE persistent task-DAG kernel.
 //
 // Tasks (host-ordered, claimed in order, waiting on epoch-valued completion flags):
-//   forward,  small supernode: t = [b[P cols]; 0] + children's contribution vectors (fixed order); L11 y = t1 in 32-column
-//             blocks (one warp substitutes, all threads update the rows below); x[cols] = y; contribution = t2 - L21 y.
-//   forward,  block row I of a tiled supernode (left-looking): t_I = init_I - sum_{k<I} L(I,k) y_k, waiting for each y_k as it
-//             is reached; then L(I,I) y_I = t_I by one warp (64-step substitution on the staged diagonal tile).
+//   forward,  small supernode: t = [b[P cols]; 0] + children's contribution vectors (child table and relative indices fetched
+//             before the wait, contributions loaded in one round trip, added in fixed child order); the panel streams through
+//             shared memory in 32-column blocks (cp.async, requested before the task waits); L11 y = t1 by pre-scaled warp
+//             substitution (only shuffle + fma on the chain), one thread per row for the block below; contribution = t2 - L21 y.
+//   forward,  block row I of a tiled supernode (left-looking): t_I = init_I - sum_{k<I} L(I,k) y_k; the 64x64 tile L(I,k+1)
+//             is in registers before the task waits for y_k; then L(I,I) y_I = t_I by one warp on the staged diagonal tile.
 //   backward, small supernode / block column J of a tiled supernode: x_J = L(J,J)^-T (y_J - sum_{I>J} L(I,J)^T x_I), rows
 //             taken from the ancestors' finished x first, then from this supernode's later blocks as their flags arrive.
 // The permutations are fused: forward tasks read b[perm[.]], backward tasks write b[perm[.]] (in place, no hazard: a
