@@ -72,6 +72,74 @@ def test_factor_and_solve_vs_oracle(name, ov, ordering):
     h.close()
 
 
+def _random_interior_point(cfg, nlp, rng):
+    lo = np.where(np.isfinite(nlp.lb), nlp.lb, 280.0)
+    hi = np.where(np.isfinite(nlp.ub), nlp.ub, 450.0)
+    return lo + (hi - lo) * rng.uniform(0.1, 0.9, cfg.n)
+
+
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4"])
+def test_full_size_model_assembly_factor_solve(name):
+    """BASELINE.json's full sizes, in the launch configuration bench.py times (default options): a2 and a3 element by
+    element against the oracle's model code and SciPy, then a4/a5 on that K through properties that hold at any size:
+    no pivot failure, normwise backward error of the solve, and (C1, C2, C4) entries of L L^T sampled on the pattern of K."""
+    cfg = make_config(name)
+    nlp = TranscribedOCP(cfg)
+    rng = np.random.default_rng(23)
+    y = _random_interior_point(cfg, nlp, rng)
+    lam = rng.normal(size=cfg.m)
+    nlp.set_params(cfg.x0, cfg.ref_for_solve(0))
+    h = nb.Handle(None, nb.make_ocp(cfg), None)
+    h.update_params(dev(cfg.x0), dev(cfg.ref_for_solve(0)))
+    jrp, jci = h.get_jac_pattern(cfg.m)
+    wrp, wci = h.get_hess_pattern(cfg.n)
+    krp, kci = h.get_kkt_pattern(cfg.n)
+    c, g = torch.empty(cfg.m, dtype=torch.float64, device=DEV), torch.empty(cfg.n, dtype=torch.float64, device=DEV)
+    Jv = torch.empty(int(jrp[-1]), dtype=torch.float64, device=DEV)
+    Wv = torch.empty(int(wrp[-1]), dtype=torch.float64, device=DEV)
+    h.model_eval(dev(y), dev(lam), c, g, Jv, Wv)
+    co, go = nlp.constraints(y), nlp.gradient(y)
+    assert np.abs(c.cpu().numpy() - co).max() <= 1e-12 * max(1.0, np.abs(co).max())
+    assert np.abs(g.cpu().numpy() - go).max() <= 1e-13 * max(1.0, np.abs(go).max())
+    Jo, Wo = nlp.jacobian(y), nlp.hessian(y, lam)
+    Jg = sp.csr_matrix((Jv.cpu().numpy(), jci, jrp), shape=(cfg.m, cfg.n))
+    assert abs(Jg - Jo).max() <= 1e-13 * abs(Jo).max()
+    Wl = sp.csr_matrix((Wv.cpu().numpy(), wci, wrp), shape=(cfg.n, cfg.n))
+    assert abs(Wl + sp.tril(Wl, -1).T - Wo).max() <= 1e-12 * max(1e-300, abs(Wo).max())
+    # a3 with a late-iteration-like spread of Sigma; W = grad^2 f only (lambda = 0) keeps K positive definite
+    h.model_eval(dev(y), dev(np.zeros(cfg.m)), c, g, Jv, Wv)
+    W0 = nlp.hessian(y, np.zeros(cfg.m))
+    sigx = 10.0 ** rng.uniform(-3, 3, cfg.n)
+    q = 10.0 ** rng.uniform(-3, 3, cfg.m)
+    Kv = torch.empty(int(krp[-1]), dtype=torch.float64, device=DEV)
+    h.assemble(Jv, Wv, dev(sigx), dev(q), 0.0, Kv)
+    K = (W0 + sp.diags(sigx) + Jo.T @ sp.diags(q) @ Jo).tocsr()
+    scale = values_on_pattern(abs(W0) + sp.diags(sigx) + abs(Jo).T @ sp.diags(q) @ abs(Jo), krp, kci)
+    assert np.all(np.abs(Kv.cpu().numpy() - values_on_pattern(K, krp, kci)) <= 1e-13 * scale)
+    # a4 + a5
+    st, _ = h.factor(Kv, 0.0)
+    assert st == 0
+    b = rng.normal(size=cfg.n)
+    x = dev(b)
+    h.solve(x)
+    assert normwise_backward_error(K, x.cpu().numpy(), b) <= 1e-10
+    if name != "C3":                                         # 1.25 GB of panels: the sampled check is done on the other three
+        info = h.get_info()
+        L = factor_as_sparse(info, h.get_factor()).tocsr()
+        perm = info["perm"]
+        KP = K[perm, :][:, perm].tocsr()
+        rows = rng.integers(0, cfg.n, 200)
+        Knorm = abs(K).max()
+        for i in rows:
+            cols = KP.indices[KP.indptr[i]:KP.indptr[i + 1]]
+            cols = cols[cols <= i]
+            li = L.getrow(i)
+            for j in cols[:: max(1, len(cols) // 4)]:
+                v = (li.multiply(L.getrow(j))).sum()
+                assert abs(v - KP[i, j]) <= 1e-12 * Knorm, (i, j)
+    h.close()
+
+
 def _sweep_setup(cfg):
     """Frozen J, grad^2 f at the cold-start point (C4 refactor sweep, BASELINE.json:configs[4]): GPU value arrays + the
     same matrices from the oracle's model code."""
