@@ -341,6 +341,18 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
     try { st = analyze_symbolic(pattern, ocp, &h->opt, h->S); }
     catch (const std::bad_alloc&) { st = NMPC_E_ALLOC; h->err = "host allocation failed"; }
     if (st != NMPC_OK) { h->err = h->S.error; return fail(st); }
+    // Small problems are bound by the number of dependency hops, not by flops: with the amalgamation
+    // threshold on auto, merge more aggressively (fewer, wider supernodes: C1 8 -> 7 levels, 436 -> 189 fronts) as long as the
+    // problem stays eligible for the latency mode below.
+    if (h->opt.relax_small < 0 && h->opt.smem_front_max <= 0 && h->S.flops <= 1e8 && h->S.max_front <= SMALL_ROWS_MAX - 2) {
+        nmpc_options o2 = h->opt;
+        o2.relax_small = 32;
+        Symbolic S2;
+        nmpc_status st2;
+        try { st2 = analyze_symbolic(pattern, ocp, &o2, S2); }
+        catch (const std::bad_alloc&) { st2 = NMPC_E_ALLOC; }
+        if (st2 == NMPC_OK && S2.max_front <= SMALL_ROWS_MAX - 2) { S2.analyze_ms += h->S.analyze_ms; h->S = std::move(S2); }
+    }
     auto body = [&]() -> nmpc_status {
         const Symbolic& S = h->S;
         int dev = 0, smem_optin = 0;

@@ -15,7 +15,7 @@ void default_options(nmpc_options* o) {
     std::memset(o, 0, sizeof(*o));
     o->ordering = NMPC_ORDER_AUTO;
     o->nd_leaf = 0;                // 0 = choose from the structure
-    o->relax_small = 8;
+    o->relax_small = -1;           // auto: 8, or 32 for small (latency-mode) problems, see nmpc_analyze
     o->relax_zeros = 0.3;
     o->smem_front_max = 0;         // 0 = device default
     o->use_graph = 1;
@@ -592,7 +592,7 @@ nmpc_status analyze_symbolic(const nmpc_pattern* pattern, const nmpc_ocp* ocp, c
                 if (pc < cur.start || pc >= cur.start + cur.w) break;      // c is not a child of cur
                 int64_t w2 = (int64_t)c.w + cur.w, r2 = (int64_t)c.w + cur.r;
                 int64_t z2 = panel_nnz(r2, w2) - (panel_nnz(c.r, c.w) - c.zeros) - (panel_nnz(cur.r, cur.w) - cur.zeros);
-                bool merge = (w2 <= opt.relax_small) || ((double)z2 <= opt.relax_zeros * (double)panel_nnz(r2, w2));
+                bool merge = (w2 <= (opt.relax_small < 0 ? 8 : opt.relax_small)) || ((double)z2 <= opt.relax_zeros * (double)panel_nnz(r2, w2));
                 if (!merge) break;
                 cur.start = c.start; cur.w = (int32_t)w2; cur.r = (int32_t)r2; cur.zeros = z2;
                 out.pop_back();
