@@ -83,7 +83,8 @@ typedef struct {
     int32_t ordering;            /* NMPC_ORDER_*                                                            */
     int32_t nd_leaf;             /* nested-dissection leaf size (variables)                                 */
     int32_t relax_small;         /* always merge a child supernode into its parent if the merged width <= this;
-                                    -1 (default) = 8, raised to 32 by nmpc_analyze for small latency-bound problems */
+                                    -1 (default) = auto: nmpc_analyze uses 32 (small latency-bound problems) or 64,
+                                    the host-only nmpc_symbolic_analyze 8 */
     double  relax_zeros;         /* else merge if the explicit zeros introduced stay below this fraction      */
     int32_t smem_front_max;      /* fronts with <= this many rows run in the one-CTA shared-memory kernel     */
     int32_t use_graph;           /* replay one IPM iteration (S6-S10 + the next S2) as a CUDA graph, 1 launch/iter  */

@@ -337,14 +337,18 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
         if (cudaStreamCreate(&h->stream) != cudaSuccess) { h->err = "cudaStreamCreate failed"; cudaGetLastError(); return fail(NMPC_E_CUDA); }
         h->own_stream = true;
     }
+    // The amalgamation threshold on auto (relax_small < 0): dependency hops, not flops, bound most of the path (DESIGN.md section
+    // 6.2), so supernodes are merged more aggressively than the classical default of 8: 64 in general (C4: 6565 -> 1230 fronts,
+    // nnz(L) +30 % but factor + solve -9 %), 32 for a small problem that is then eligible for the latency mode below (C1: 8 -> 7
+    // levels, 436 -> 189 fronts); only small problems pay for a second analysis.
+    const bool auto_relax = h->opt.relax_small < 0;
+    nmpc_options o1 = h->opt;
+    if (auto_relax) o1.relax_small = 64;
     nmpc_status st;
-    try { st = analyze_symbolic(pattern, ocp, &h->opt, h->S); }
+    try { st = analyze_symbolic(pattern, ocp, &o1, h->S); }
     catch (const std::bad_alloc&) { st = NMPC_E_ALLOC; h->err = "host allocation failed"; }
     if (st != NMPC_OK) { h->err = h->S.error; return fail(st); }
-    // Small problems are bound by the number of dependency hops, not by flops: with the amalgamation
-    // threshold on auto, merge more aggressively (fewer, wider supernodes: C1 8 -> 7 levels, 436 -> 189 fronts) as long as the
-    // problem stays eligible for the latency mode below.
-    if (h->opt.relax_small < 0 && h->opt.smem_front_max <= 0 && h->S.flops <= 1e8 && h->S.max_front <= SMALL_ROWS_MAX - 2) {
+    if (auto_relax && h->opt.smem_front_max <= 0 && h->S.flops <= 1e8) {
         nmpc_options o2 = h->opt;
         o2.relax_small = 32;
         Symbolic S2;
