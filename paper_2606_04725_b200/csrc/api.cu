@@ -351,6 +351,7 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
     if (auto_relax && h->opt.smem_front_max <= 0 && h->S.flops <= 1e8) {
         nmpc_options o2 = h->opt;
         o2.relax_small = 32;
+        if (o2.nd_leaf <= 0) o2.nd_leaf = 32;             // smaller dissection leaves: C1 factor + solve another -11 %
         Symbolic S2;
         nmpc_status st2;
         try { st2 = analyze_symbolic(pattern, ocp, &o2, S2); }
