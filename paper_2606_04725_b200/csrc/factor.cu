@@ -299,9 +299,10 @@ __device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, i
 // update, the columns after the panel a rank-32 one.  Rows >= ni / columns >= nj of the tiles are finite padding.
 // The columns of L_JJ arrive in 8-column blocks as the diagonal task publishes them (sub[0] counts them, `sbase` = value before
 // this call's first block): block k is fetched from the panel in global memory (Lg, leading dimension ldg) right before
-// sub-step k needs it, so the TRSM runs one sub-step behind the POTRF instead of after it.
+// sub-step k needs it, so the TRSM runs one sub-step behind the POTRF instead of after it.  Xg: the tile of the panel that
+// receives X (same leading dimension ldg); finished entries are stored by the thread that solved them.
 __device__ __forceinline__ void trsm_tile(double* Cs, double* Ls, double* rinv, int ni, int nj, const uint32_t* sub, uint32_t sbase,
-                                          const double* __restrict__ Lg, int ldg, const double* __restrict__ dinv_g) {
+                                          const double* __restrict__ Lg, int ldg, const double* __restrict__ dinv_g, double* __restrict__ Xg) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gid = lane >> 2, tig = lane & 3;
     constexpr int NW = NT / 32;
     const int TU = (ni + 7) >> 3;
@@ -339,7 +340,7 @@ __device__ __forceinline__ void trsm_tile(double* Cs, double* Ls, double* rinv, 
                 }
 #pragma unroll
                 for (int c = 0; c < 8; ++c)
-                    if (c < jb) Cs[(j0 + c) * CLD + tid] = x[c];
+                    if (c < jb) { Cs[(j0 + c) * CLD + tid] = x[c]; Xg[tid + (int64_t)(j0 + c) * ldg] = x[c]; }   // final: straight to the panel
             }
             __syncthreads();
             if (t0 < p1) {
@@ -694,12 +695,8 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
         } else {
             double* Ls = pipe;
             double* rinv = pipe + CT_DOUBLES;
-            trsm_tile(Cs, Ls, rinv, ni, nj, sub, sbase, P + j0 + (int64_t)j0 * ld, ld, D.dinv + c0 + j0);
-            TRACE(3);
-            for (int idx = tid; idx < ni * nj; idx += NT) {
-                const int mm = idx % ni, nn = idx / ni;
-                P[(i0 + mm) + (int64_t)(j0 + nn) * ld] = Cs[nn * CLD + mm];
-            }
+            trsm_tile(Cs, Ls, rinv, ni, nj, sub, sbase, P + j0 + (int64_t)j0 * ld, ld, D.dinv + c0 + j0, P + i0 + (int64_t)j0 * ld);
+            TRACE(3);                                    // every row-solving thread has already stored its finished entries
         }
         __syncthreads();
         if (tid == 0) { __threadfence(); st_release(tdone + J * nbt + I, epoch); red_release_add(front_done + s, 1u); }
