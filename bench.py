@@ -65,16 +65,18 @@ def measured_peaks():
 
 
 def profiled_traffic(kernel, workload):
-    """DRAM bytes per launch of `kernel` on `workload` from the committed `ncu --set full` summary (profiles/traffic.json,
-    written by hand from profiles/*_full.md); None when no capture of that pair is on file."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+    """DRAM bytes per launch of `kernel` on `workload` from the committed `ncu --set full` summaries (profiles/traffic.csv,
+    copied by hand from profiles/*_full.md); None when no capture of that pair is on file."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
     try:
         with open(p) as f:
-            d = json.load(f)
-        e = d[workload][kernel]
-        return {"bytes_per_launch": float(e["dram_read_bytes"]) + float(e["dram_write_bytes"]), "source": e["source"]}
-    except (OSError, KeyError, ValueError):
-        return None
+            for ln in f.read().splitlines()[1:]:
+                c = ln.split(",")
+                if len(c) >= 5 and c[0] == workload and c[1] == kernel:
+                    return {"bytes_per_launch": float(c[2]) + float(c[3]), "source": c[4]}
+    except (OSError, ValueError):
+        pass
+    return None
 
 
 def replica_x0(cfg, rank):
