@@ -13,7 +13,8 @@
  * Conventions (all entry points)
  *   - C99, no exceptions cross the boundary, no global state; every call returns an nmpc_status.
  *   - "HOST" pointers are ordinary host memory; "DEVICE" pointers are CUDA device memory of the device that
- *     was current when the handle was created (e.g. torch tensor.data_ptr()).
+ *     was current when the handle was created (e.g. torch tensor.data_ptr()).  Every call selects that device
+ *     for its own duration and restores the caller's current device before it returns.
  *   - Ownership: the caller owns every pointer it passes.  The library copies what it needs during the call and
  *     never frees or retains caller memory; DEVICE buffers must stay valid until the handle's stream has
  *     finished the work of the call (every call that returns a HOST result synchronises that stream itself).
@@ -93,6 +94,9 @@ typedef struct {
     int32_t max_iter;
     double eta_first, eta_grow_first, eta_grow, eta_shrink, eta_min, eta_max, warm_push;
     int32_t time_phases;         /* record CUDA-event phase times in nmpc_stats (adds event overhead)         */
+    int32_t epoch_limit;         /* 0 = automatic.  Test hook: the completion flags of the persistent kernels are
+                                    call-number valued and are zeroed before a counter could overflow (after ~1e4..1e6
+                                    factorizations); a small value (>= 3) forces that restart every few calls           */
 } nmpc_options;
 
 typedef struct {                 /* filled by nmpc_get_info; arrays are HOST pointers owned by the handle     */
@@ -117,8 +121,12 @@ typedef struct {                 /* filled by nmpc_ipm_solve (HOST)             
     double  ms_total, ms_eval, ms_assemble, ms_factor, ms_solve, ms_vector;   /* CUDA-event phase sums        */
 } nmpc_stats;
 
-typedef struct {                 /* one row per IPM iteration, for parity traces (HOST, caller array)         */
+typedef struct {                 /* one row per IPM iteration, for parity traces and per-iteration timing (HOST,
+                                    caller array)                                                              */
     double mu, E0, Emu, eta, alpha_pr, alpha_du;
+    double ms_iter;              /* device time of the whole iteration (CUDA events on the handle's stream, from the
+                                    launch of S6 to the launch of the next iteration's S6 / the end of the solve)   */
+    double ms_eval, ms_assemble, ms_factor, ms_solve, ms_vector;   /* phase split, only with options.time_phases  */
 } nmpc_trace_row;
 
 void nmpc_default_options(nmpc_options* out);
@@ -160,7 +168,9 @@ nmpc_status nmpc_kkt_multiply(nmpc_handle h, const double* x_dev, double* y_dev)
 
 /* ---- Algorithm 2 (LiftedIPM) on the current parameters.  warm = 0: cold start (y_inout_dev is ignored on input
  *      unless use_y0 != 0); warm = 1: z <- stored z* of the previous solve (Alg. 1 line 10).  y_inout_dev DEVICE n.
- *      trace (HOST, may be NULL) receives up to trace_cap rows.                                               */
+ *      trace (HOST, may be NULL) receives up to trace_cap rows.  z* is stored for the next warm start only when the
+ *      solve converged (NMPC_OK) or stopped at max_iter with a finite iterate; after NMPC_E_STEP / NMPC_E_INERTIA the
+ *      next call with warm = 1 starts cold.                                                                     */
 nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* y_inout_dev, nmpc_stats* stats_host,
                            nmpc_trace_row* trace_host, int32_t trace_cap);
 /*      end-to-end form with HOST buffers: parameters in, primal solution out (copies inside the call)        */
@@ -188,23 +198,15 @@ nmpc_status nmpc_get_jac_pattern(nmpc_handle h, int64_t* nnz, int64_t* rowptr, i
 nmpc_status nmpc_get_hess_pattern(nmpc_handle h, int64_t* nnz, int64_t* rowptr, int32_t* colind);
 nmpc_status nmpc_get_kkt_pattern(nmpc_handle h, int64_t* nnz, int64_t* rowptr, int32_t* colind);
 
-/* ---- measurement aid (not on the hot path): sustained fp64 rate of the current device in TFLOP/s, kind 0 = DFMA
- *      (vector pipe), 1 = DMMA (mma.sync m8n8k4 f64); best of `repeats` launches of a register-resident kernel.
- *      HOST outputs; ms_out may be NULL.  These are the denominators of the factorization roofline.            */
-nmpc_status nmpc_fp64_peak(int32_t kind, int32_t repeats, double* tflops_out, double* ms_out);
-
 nmpc_status nmpc_get_info(nmpc_handle h, nmpc_sym_info* out_host);
 /* ---- copy of the factor for tests: the panels of all supernodes, one after the other, to a HOST buffer.  Panel of
  *      supernode s: column-major r_s x w_s with leading dimension r_s rounded up to even (rows = nmpc_sym_info.rows). */
 nmpc_status nmpc_get_factor(nmpc_handle h, double* panels_host /* panel_doubles */);
-/* ---- measurement aid: per-task timestamps of the last factorization (kind 0) / solve (kind 1), recorded only by handles
- *      created while the environment variable NMPC_TRACE is set.  tasks_host: 4 int32 per task (type, supernode, I, J|dir);
- *      stamps_host: 8 uint64 per task (globaltimer ns: claimed, dependencies met / GEMM done, assembled, factored, done;
- *      [5] = SM id).  Returns the number of tasks copied (<= cap), the task count if a pointer is NULL, 0 if not tracing. */
-int64_t     nmpc_get_task_trace(nmpc_handle h, int32_t kind, int32_t* tasks_host, uint64_t* stamps_host, int64_t cap);
 /* ---- kernel launches issued by this handle since creation (graph replays count their kernel nodes)        */
 int64_t     nmpc_launch_count(nmpc_handle h);
-const char* nmpc_last_error(nmpc_handle h);      /* string owned by the handle                                */
+/* ---- message of the last error of this handle (string owned by the handle).  h == NULL: message of the last failed
+ *      nmpc_analyze on the calling thread (thread-local; the library prints nothing).                          */
+const char* nmpc_last_error(nmpc_handle h);
 void        nmpc_destroy(nmpc_handle h);
 
 #ifdef __cplusplus

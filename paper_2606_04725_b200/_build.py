@@ -1,7 +1,11 @@
-"""Build paper_2606_04725_b200/libnmpc_b200.so (the C-ABI library of include/nmpc.h) with nvcc for sm_100a.
+"""Build the C-ABI library of include/nmpc.h with nvcc for sm_100a:
+
+  libnmpc_b200.so        the product
+  libnmpc_b200_aids.so   the same sources with -DNMPC_TRACE_BUILD (per-task timestamps in the persistent kernels) plus
+                         csrc/peak.cu: measurement aids of include/nmpc_aids.h, never loaded by the product path
 
 nvcc cross-compiles without a GPU, so this runs on the CPU-only container as well as on the B200 box.
-Objects are rebuilt only when a source or header is newer than the object (in-tree `build/` directory).
+Objects are rebuilt only when a source or header is newer than the object (in-tree `build/` directories).
 """
 from __future__ import annotations
 
@@ -14,7 +18,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 BUILD = os.path.join(HERE, "build")
+BUILD_AIDS = os.path.join(HERE, "build", "aids")
 LIB = os.path.join(HERE, "libnmpc_b200.so")
+LIB_AIDS = os.path.join(HERE, "libnmpc_b200_aids.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
@@ -27,9 +33,10 @@ SOURCES = [
     ("solve.cu", []),
     ("ipm.cu", ["-fmad=false"]),
     ("api.cu", []),
-    ("peak.cu", []),
 ]
-HEADERS = ["device.h", "symbolic.h", "models.cuh", os.path.join(ROOT, "include", "nmpc.h")]
+AIDS_ONLY = [("peak.cu", [])]
+HEADERS = ["device.h", "symbolic.h", "models.cuh", os.path.join(ROOT, "include", "nmpc.h"),
+           os.path.join(ROOT, "include", "nmpc_aids.h")]
 
 
 def _newest_header() -> float:
@@ -40,9 +47,9 @@ def _newest_header() -> float:
     return t
 
 
-def _compile(src: str, extra: list[str], force: bool, hdr_t: float) -> tuple[str, bool]:
+def _compile(src: str, extra: list[str], force: bool, hdr_t: float, bdir: str) -> tuple[str, bool]:
     s = os.path.join(CSRC, src)
-    o = os.path.join(BUILD, os.path.splitext(src)[0] + ".o")
+    o = os.path.join(bdir, os.path.splitext(src)[0] + ".o")
     if not force and os.path.exists(o) and os.path.getmtime(o) >= max(os.path.getmtime(s), hdr_t):
         return o, False
     cmd = [NVCC] + ARCH + COMMON + extra + ["-c", s, "-o", o]
@@ -50,18 +57,27 @@ def _compile(src: str, extra: list[str], force: bool, hdr_t: float) -> tuple[str
     return o, True
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    os.makedirs(BUILD, exist_ok=True)
+def _link(lib: str, objs: list[str], verbose: bool) -> None:
+    tmp = lib + f".tmp{os.getpid()}"
+    subprocess.check_call([NVCC] + ARCH + ["-shared", "-o", tmp] + objs + ["-lcudart"])
+    os.replace(tmp, lib)
+    if verbose:
+        print("built", lib)
+
+
+def build(force: bool = False, verbose: bool = False, aids: bool = True) -> str:
+    os.makedirs(BUILD_AIDS, exist_ok=True)
     hdr_t = _newest_header()
-    with ThreadPoolExecutor(max_workers=4) as ex:
-        res = list(ex.map(lambda a: _compile(a[0], a[1], force, hdr_t), SOURCES))
-    objs = [r[0] for r in res]
-    if force or any(r[1] for r in res) or not os.path.exists(LIB):
-        tmp = LIB + f".tmp{os.getpid()}"
-        subprocess.check_call([NVCC] + ARCH + ["-shared", "-o", tmp] + objs + ["-lcudart"])
-        os.replace(tmp, LIB)
-        if verbose:
-            print("built", LIB)
+    jobs = [(src, extra, BUILD) for src, extra in SOURCES]
+    if aids:
+        jobs += [(src, extra + ["-DNMPC_TRACE_BUILD"], BUILD_AIDS) for src, extra in SOURCES + AIDS_ONLY]
+    with ThreadPoolExecutor(max_workers=6) as ex:
+        res = list(ex.map(lambda a: _compile(a[0], a[1], force, hdr_t, a[2]), jobs))
+    prod, aid = res[: len(SOURCES)], res[len(SOURCES):]
+    if force or any(r[1] for r in prod) or not os.path.exists(LIB):
+        _link(LIB, [r[0] for r in prod], verbose)
+    if aids and (force or any(r[1] for r in aid) or not os.path.exists(LIB_AIDS)):
+        _link(LIB_AIDS, [r[0] for r in aid], verbose)
     return LIB
 
 

@@ -40,7 +40,7 @@ class nmpc_options(C.Structure):
                 + [("max_iter", c_i32)]
                 + [(k, c_dbl) for k in ("eta_first", "eta_grow_first", "eta_grow", "eta_shrink", "eta_min", "eta_max",
                                         "warm_push")]
-                + [("time_phases", c_i32)])
+                + [("time_phases", c_i32), ("epoch_limit", c_i32)])
 
 
 class nmpc_sym_info(C.Structure):
@@ -58,7 +58,8 @@ class nmpc_stats(C.Structure):
 
 
 class nmpc_trace_row(C.Structure):
-    _fields_ = [(k, c_dbl) for k in ("mu", "E0", "Emu", "eta", "alpha_pr", "alpha_du")]
+    _fields_ = [(k, c_dbl) for k in ("mu", "E0", "Emu", "eta", "alpha_pr", "alpha_du", "ms_iter", "ms_eval", "ms_assemble",
+                                     "ms_factor", "ms_solve", "ms_vector")]
 
 
 # every symbol include/nmpc.h declares: name -> (restype, argtypes)
@@ -85,31 +86,50 @@ SIGNATURES = {
     "nmpc_get_jac_pattern": (c_i32, [c_vp, P(c_i64), c_vp, c_vp]),
     "nmpc_get_hess_pattern": (c_i32, [c_vp, P(c_i64), c_vp, c_vp]),
     "nmpc_get_kkt_pattern": (c_i32, [c_vp, P(c_i64), c_vp, c_vp]),
-    "nmpc_fp64_peak": (c_i32, [c_i32, c_i32, P(c_dbl), P(c_dbl)]),
     "nmpc_get_info": (c_i32, [c_vp, P(nmpc_sym_info)]),
     "nmpc_get_factor": (c_i32, [c_vp, c_vp]),
-    "nmpc_get_task_trace": (c_i64, [c_vp, c_i32, c_vp, c_vp, c_i64]),
     "nmpc_launch_count": (c_i64, [c_vp]),
     "nmpc_last_error": (C.c_char_p, [c_vp]),
     "nmpc_destroy": (None, [c_vp]),
 }
 
+# the two extra symbols of include/nmpc_aids.h (measurement build, libnmpc_b200_aids.so)
+AIDS_SIGNATURES = {
+    "nmpc_fp64_peak": (c_i32, [c_i32, c_i32, P(c_dbl), P(c_dbl)]),
+    "nmpc_get_task_trace": (c_i64, [c_vp, c_i32, c_vp, c_vp, c_i64]),
+}
+AIDS_LIB_PATH = os.path.join(_HERE, "libnmpc_b200_aids.so")
+
 _lib = None
+_aids = None
+
+
+def _load(path, signatures):
+    if not os.path.exists(path):
+        raise RuntimeError(f"{path} is missing: run `python -m paper_2606_04725_b200._build` "
+                           "(or __graft_entry__.build()).  There is no CPU fallback.")
+    lib = C.CDLL(path)
+    for name, (res, args) in signatures.items():
+        fn = getattr(lib, name)              # AttributeError if the library does not export a declared symbol
+        fn.restype, fn.argtypes = res, args
+    return lib
 
 
 def load_library() -> C.CDLL:
     """Load libnmpc_b200.so (built by paper_2606_04725_b200/_build.py).  Raises if it is missing: no fallback."""
     global _lib
     if _lib is None:
-        if not os.path.exists(LIB_PATH):
-            raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2606_04725_b200._build` "
-                               "(or __graft_entry__.build()).  There is no CPU fallback.")
-        lib = C.CDLL(LIB_PATH)
-        for name, (res, args) in SIGNATURES.items():
-            fn = getattr(lib, name)          # AttributeError if the library does not export a declared symbol
-            fn.restype, fn.argtypes = res, args
-        _lib = lib
+        _lib = _load(LIB_PATH, SIGNATURES)
     return _lib
+
+
+def load_aids_library() -> C.CDLL:
+    """Load libnmpc_b200_aids.so: the measurement build (per-task timestamps, fp64 peak microbenchmarks) of
+    include/nmpc_aids.h.  Used by bench.py's live-peak line and by profiling runs, never by the product path."""
+    global _aids
+    if _aids is None:
+        _aids = _load(AIDS_LIB_PATH, {**SIGNATURES, **AIDS_SIGNATURES})
+    return _aids
 
 
 class NmpcError(RuntimeError):
@@ -182,7 +202,7 @@ def _get_pattern(fn, h):
 def fp64_peak(kind: int, repeats: int = 5):
     """nmpc_fp64_peak: (TFLOP/s, ms) of the DFMA (kind 0) / DMMA (kind 1) microbenchmark on the current device."""
     tf, ms = c_dbl(), c_dbl()
-    st = load_library().nmpc_fp64_peak(kind, repeats, C.byref(tf), C.byref(ms))
+    st = load_aids_library().nmpc_fp64_peak(kind, repeats, C.byref(tf), C.byref(ms))
     if st:
         raise NmpcError(st, "nmpc_fp64_peak")
     return tf.value, ms.value
@@ -234,8 +254,8 @@ class Symbolic:
 class Handle:
     """nmpc_handle: one OCP structure <-> one CUDA stream.  Methods carry the names of the C entry points."""
 
-    def __init__(self, pattern=None, ocp=None, options=None, stream=None):
-        self.lib = load_library()
+    def __init__(self, pattern=None, ocp=None, options=None, stream=None, aids=False):
+        self.lib = load_aids_library() if aids else load_library()      # aids=True: measurement build (task traces)
         self._h = c_vp()
         self._keep = (pattern, ocp, options)
         st = self.lib.nmpc_analyze(C.byref(pattern) if pattern is not None else None,
@@ -243,7 +263,7 @@ class Handle:
                                    C.byref(options) if options is not None else None,
                                    c_vp(stream) if stream else None, C.byref(self._h))
         if st:
-            raise NmpcError(st, "nmpc_analyze")
+            raise NmpcError(st, "nmpc_analyze", (self.lib.nmpc_last_error(None) or b"").decode())
 
     def _ck(self, st, where, allow=()):
         if st and st not in allow:
@@ -328,7 +348,8 @@ class Handle:
         return out
 
     def get_task_trace(self, kind):
-        """nmpc_get_task_trace: (tasks[nt,4] int32, stamps[nt,8] uint64) of the last factorization (0) / solve (1)."""
+        """nmpc_get_task_trace (handles created with aids=True): (tasks[nt,4] int32, stamps[nt,8] uint64) of the last
+        factorization (0) / solve (1)."""
         nt = int(self.lib.nmpc_get_task_trace(self._h, kind, None, None, 0))
         tasks, stamps = np.zeros((max(nt, 0), 4), np.int32), np.zeros((max(nt, 0), 8), np.uint64)
         if nt > 0:

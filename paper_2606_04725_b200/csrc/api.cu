@@ -30,6 +30,7 @@ struct nmpc_handle_s {
     nmpc_options opt;
     cudaStream_t stream = nullptr;
     bool own_stream = false;
+    int dev = 0;                       // the device that was current in nmpc_analyze; every entry point re-selects it
     DevSym D;
     DevModel M;
     IpmVectors V{};
@@ -49,12 +50,25 @@ struct nmpc_handle_s {
     int nmult = 0;
     std::string err;
     cudaEvent_t ev[2] = {nullptr, nullptr};
+    std::vector<cudaEvent_t> it_ev;    // per-iteration events of traced solves (created on first use)
     double* d_par = nullptr;           // device {mu, tau, (uint32) factor call number, (uint32) solve call number}: read by the graph's kernels
     cudaGraphExec_t iter_graph = nullptr;   // one IPM iteration (S6-S10 + the next S2), see capture_iteration_graph
     bool graph_failed = false;
 };
 
 namespace {
+
+// Every extern "C" entry point that touches the device runs on the handle's device (the one current in nmpc_analyze) and
+// restores the caller's current device on return: handles of several devices can be driven from one host thread.
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(const nmpc_handle_s* h) {
+        if (h && cudaGetDevice(&prev) == cudaSuccess && prev != h->dev) cudaSetDevice(h->dev); else prev = -1;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+thread_local std::string g_create_error;   // message of the last failed nmpc_analyze on this thread: nmpc_last_error(NULL)
 
 #define CK(call)                                                                                      \
     do {                                                                                              \
@@ -227,9 +241,9 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
     TRY(dalloc(h, (size_t)F.sync_words, &F.sync));
     F.fac_done = F.sync + 2; F.sol_done_f = F.fac_done + ns; F.sol_done_b = F.sol_done_f + ns;
     F.tile_done = F.sol_done_b + ns; F.blk_f = F.tile_done + slots; F.blk_b = F.blk_f + bslots; F.sub_done = F.blk_b + bslots;
-    if (std::getenv("NMPC_TRACE")) {                     // measurement aid: per-task timestamps (nmpc_get_task_trace)
-        TRY(dalloc(h, (size_t)F.n_ftasks * 8, &F.ftrace)); TRY(dalloc(h, (size_t)F.n_stasks * 8, &F.strace));
-    }
+#ifdef NMPC_TRACE_BUILD                                      // measurement build: per-task timestamps (nmpc_get_task_trace, include/nmpc_aids.h)
+    TRY(dalloc(h, (size_t)F.n_ftasks * 8, &F.ftrace)); TRY(dalloc(h, (size_t)F.n_stasks * 8, &F.strace));
+#endif
     F.small_max_r = small_max_r;
     F.fsmem = smem_bytes; F.ssmem = solve_smem;
     F.fgrid = (int32_t)std::max<int64_t>(1, std::min<int64_t>((int64_t)tasks.size(), (int64_t)num_sms * ctas_per_sm));
@@ -237,15 +251,25 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
     // epoch-valued flags: counters reach epoch * target and the claim counters epoch * (ntasks + grid); reset before 2^31
     int64_t per_epoch = std::max<int64_t>((int64_t)tasks.size() + F.fgrid, (int64_t)stasks.size() + F.sgrid);
     for (int s = 0; s < ns; ++s) per_epoch = std::max<int64_t>(per_epoch, target[s]);
-    h->epoch_limit = (uint32_t)std::max<int64_t>(2, ((int64_t)1 << 31) / per_epoch - 2);
+    h->epoch_limit = (uint32_t)std::max<int64_t>(3, ((int64_t)1 << 31) / per_epoch - 2);
+    if (h->opt.epoch_limit > 0) h->epoch_limit = std::min<uint32_t>(h->epoch_limit, (uint32_t)std::max(3, h->opt.epoch_limit));   // test hook
     return NMPC_OK;
 }
 
-// the next call number of the factor / solve kernels; both restart from 1 (flags zeroed) before any counter can overflow
+// The next call number of the factor / solve kernels.  Both restart from 1 (all flags zeroed, in stream order) before any
+// counter can overflow.  The restart is decided with a margin of TWO call numbers, so a factor number and the solve number
+// reserved right after it (one CUDA-graph replay holds both kernels) always lie on the same side of a restart.
 nmpc_status next_epoch(nmpc_handle_s* h, bool factor, uint32_t* out) {
-    if (std::max(h->epoch_f, h->epoch_s) + 1 >= h->epoch_limit) {
+    if (factor && std::max(h->epoch_f, h->epoch_s) + 2 >= h->epoch_limit) {
         CK(cudaMemsetAsync(h->F.sync, 0, (size_t)h->F.sync_words * sizeof(uint32_t), h->stream));
         h->epoch_f = h->epoch_s = 0;
+    }
+    if (!factor && h->epoch_s + 1 >= h->epoch_limit) {   // a long run of solves on one factorization: only the solve flags restart
+        const size_t off = (size_t)(h->F.sol_done_f - h->F.sync), cnt = (size_t)(h->F.tile_done - h->F.sol_done_f);
+        CK(cudaMemsetAsync(h->F.sync + 1, 0, sizeof(uint32_t), h->stream));
+        CK(cudaMemsetAsync(h->F.sync + off, 0, cnt * sizeof(uint32_t), h->stream));
+        CK(cudaMemsetAsync(h->F.blk_f, 0, (size_t)(h->F.sub_done - h->F.blk_f) * sizeof(uint32_t), h->stream));
+        h->epoch_s = 0;
     }
     *out = factor ? ++h->epoch_f : ++h->epoch_s;
     return NMPC_OK;
@@ -292,28 +316,48 @@ nmpc_status capture_iteration_graph(nmpc_handle_s* h) {
     const uint32_t* epo = reinterpret_cast<const uint32_t*>(h->d_par + 2);
     cudaGraph_t g = nullptr;
     if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); h->graph_failed = true; return NMPC_OK; }
-    cudaMemcpyAsync(h->d_par, hp, 4 * sizeof(double), cudaMemcpyHostToDevice, st);
-    launch_sigma_rhs(M, V, 0.0, h->d_par, st);
-    launch_assemble_K(M, V.Jval, V.Wval, V.sigx, V.q, 0.0, V.Kval, st);
-    launch_factor(h->D, h->F, h->d_Kval, 0.0, 0u, epo, st);
-    cudaMemcpyAsync(V.dy, V.b, sizeof(double) * M.n, cudaMemcpyDeviceToDevice, st);
-    launch_solve(h->D, h->F, V.dy, h->d_x, 0u, epo, st);
-    launch_step(M, V, 0.0, 0.0, h->d_par, st);
-    launch_update(M, V, h->D.fail_col, st);
-    launch_model_eval(M, V.y, V.wp, V.wm, nullptr, V.c, V.gradf, V.Jval, V.Wval, st);
-    launch_residuals(M, V, h->opt.gamma, st);
-    cudaMemcpyAsync(hs, V.scal, sizeof(double) * 10, cudaMemcpyDeviceToHost, st);
-    cudaMemcpyAsync(flag, h->D.fail_col, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
-    if (cudaStreamEndCapture(st, &g) != cudaSuccess || !g) { cudaGetLastError(); h->graph_failed = true; return NMPC_OK; }
+    // every captured call is checked; the first failure ends the capture and the plain launch sequence is used instead
+    cudaError_t ce = cudaSuccess;
+    auto ok = [&](cudaError_t e) { if (ce == cudaSuccess && e != cudaSuccess) ce = e; return ce == cudaSuccess; };
+    auto launched = [&]() { return ok(cudaGetLastError()); };
+    bool good = ok(cudaMemcpyAsync(h->d_par, hp, 4 * sizeof(double), cudaMemcpyHostToDevice, st));
+    if (good) { launch_sigma_rhs(M, V, 0.0, h->d_par, st); good = launched(); }
+    if (good) { launch_assemble_K(M, V.Jval, V.Wval, V.sigx, V.q, 0.0, V.Kval, st); good = launched(); }
+    if (good) { launch_factor(h->D, h->F, h->d_Kval, 0.0, 0u, epo, st); good = launched(); }
+    if (good) good = ok(cudaMemcpyAsync(V.dy, V.b, sizeof(double) * M.n, cudaMemcpyDeviceToDevice, st));
+    if (good) { launch_solve(h->D, h->F, V.dy, h->d_x, 0u, epo, st); good = launched(); }
+    if (good) { launch_step(M, V, 0.0, 0.0, h->d_par, st); good = launched(); }
+    if (good) { launch_update(M, V, h->D.fail_col, st); good = launched(); }
+    if (good) { launch_model_eval(M, V.y, V.wp, V.wm, nullptr, V.c, V.gradf, V.Jval, V.Wval, st); good = launched(); }
+    if (good) { launch_residuals(M, V, h->opt.gamma, st); good = launched(); }
+    if (good) good = ok(cudaMemcpyAsync(hs, V.scal, sizeof(double) * 10, cudaMemcpyDeviceToHost, st));
+    if (good) good = ok(cudaMemcpyAsync(flag, h->D.fail_col, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    const cudaError_t ee = cudaStreamEndCapture(st, &g);
+    if (!good || ee != cudaSuccess || !g) {
+        cudaGetLastError();
+        if (g) cudaGraphDestroy(g);
+        h->err = std::string("CUDA-graph capture of the IPM iteration failed (") + cudaGetErrorString(good ? ee : ce) + "); using plain launches";
+        h->graph_failed = true;
+        return NMPC_OK;
+    }
     if (cudaGraphInstantiate(&h->iter_graph, g, 0) != cudaSuccess) { cudaGetLastError(); h->iter_graph = nullptr; h->graph_failed = true; }
     cudaGraphDestroy(g);
     return NMPC_OK;
 }
 
-struct PhaseTimer {                 // optional CUDA-event phase timing (opt.time_phases)
-    nmpc_handle_s* h; bool on; double* acc = nullptr;
-    void begin(double* a) { if (!on) return; acc = a; cudaEventRecord(h->ev[0], h->stream); }
-    void end() { if (!on || !acc) return; cudaEventRecord(h->ev[1], h->stream); cudaEventSynchronize(h->ev[1]); float ms = 0; cudaEventElapsedTime(&ms, h->ev[0], h->ev[1]); *acc += ms; acc = nullptr; }
+struct PhaseTimer {                 // optional CUDA-event phase timing (opt.time_phases): sums per solve and per iteration
+    nmpc_handle_s* h; bool on; double* acc = nullptr; double* acc_it = nullptr;
+    double it_ms[5] = {0, 0, 0, 0, 0};   // eval, assemble, factor, solve, vector of the iteration being built
+    void begin(double* a, int phase) { if (!on) return; acc = a; acc_it = it_ms + phase; cudaEventRecord(h->ev[0], h->stream); }
+    void end() {
+        if (!on || !acc) return;
+        cudaEventRecord(h->ev[1], h->stream); cudaEventSynchronize(h->ev[1]);
+        float ms = 0; cudaEventElapsedTime(&ms, h->ev[0], h->ev[1]); *acc += ms; *acc_it += ms; acc = nullptr;
+    }
+    void flush(nmpc_trace_row* row) {    // S2 of iteration k+1 is booked on iteration k (as in the graph replay)
+        if (row) { row->ms_eval = it_ms[0]; row->ms_assemble = it_ms[1]; row->ms_factor = it_ms[2]; row->ms_solve = it_ms[3]; row->ms_vector = it_ms[4]; }
+        for (double& v : it_ms) v = 0.0;
+    }
 };
 
 }  // namespace
@@ -323,13 +367,21 @@ extern "C" {
 nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const nmpc_options* opt, void* cuda_stream, nmpc_handle* out) {
     if (!out) return NMPC_E_ARG;
     *out = nullptr;
+    g_create_error.clear();
     int ndev = 0;
-    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return NMPC_E_CUDA; }
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); g_create_error = "no CUDA device"; return NMPC_E_CUDA; }
     nmpc_handle_s* h = new (std::nothrow) nmpc_handle_s();
     if (!h) return NMPC_E_ALLOC;
-    auto fail = [&](nmpc_status s) { std::fprintf(stderr, "nmpc_analyze: %s\n", h->err.c_str()); nmpc_destroy(h); return s; };
+    auto fail = [&](nmpc_status s) { g_create_error = h->err; nmpc_destroy(h); return s; };
     if (opt) h->opt = *opt; else default_options(&h->opt);
     if (h->opt.mu_warm <= 0.0) h->opt.mu_warm = h->opt.eps_outer / 10.0;
+    int smem_optin = 0, num_sms = 0, lat_ctas = 1, lat_rmax = 0;
+    size_t lat_smem = 0;
+    if (cudaGetDevice(&h->dev) != cudaSuccess || cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, h->dev) != cudaSuccess ||
+        configure_factor_kernels(smem_optin, true, &lat_ctas, &lat_smem, &lat_rmax) != cudaSuccess) {
+        h->err = std::string("device query failed: ") + cudaGetErrorString(cudaGetLastError()); return fail(NMPC_E_CUDA);
+    }
     h->stream = (cudaStream_t)cuda_stream;
     if (!h->stream) {
         // the legacy default stream cannot be captured into a graph: use an own BLOCKING stream, which keeps the implicit
@@ -339,37 +391,36 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
     }
     // The amalgamation threshold on auto (relax_small < 0): dependency hops, not flops, bound most of the path (DESIGN.md section
     // 6.2), so supernodes are merged more aggressively than the classical default of 8: 64 in general (C4: 6565 -> 1230 fronts,
-    // nnz(L) +30 % but factor + solve -9 %), 32 for a small problem that is then eligible for the latency mode below (C1: 8 -> 7
-    // levels, 436 -> 189 fronts); only small problems pay for a second analysis.
-    const bool auto_relax = h->opt.relax_small < 0;
-    nmpc_options o1 = h->opt;
-    if (auto_relax) o1.relax_small = 64;
-    nmpc_status st;
-    try { st = analyze_symbolic(pattern, ocp, &o1, h->S); }
-    catch (const std::bad_alloc&) { st = NMPC_E_ALLOC; h->err = "host allocation failed"; }
+    // nnz(L) +30 % but factor + solve -9 %), 32 with dissection leaves of 32 for a small problem that is then eligible for the
+    // latency mode below (C1: 8 -> 7 levels, 436 -> 189 fronts).  Latency mode = every front fits ONE CTA's shared memory
+    // (lat_rmax rows, computed from the device's shared-memory size) and sum cc^2 <= 1e8.  The small-problem analysis is tried
+    // first when n is small, so C0/C1-class problems are analysed once; only a problem that turns out not to be eligible (or a
+    // large-n problem that turns out to be) pays for a second analysis.
+    const bool auto_relax = h->opt.relax_small < 0 && h->opt.smem_front_max <= 0;
+    auto eligible = [&](const Symbolic& S) { return S.flops <= 1e8 && S.max_front <= lat_rmax; };
+    auto analyze_with = [&](bool small_variant, Symbolic& S) -> nmpc_status {
+        nmpc_options o = h->opt;
+        if (o.relax_small < 0) o.relax_small = small_variant ? 32 : 64;
+        if (small_variant && o.nd_leaf <= 0) o.nd_leaf = 32;      // smaller dissection leaves: C1 factor + solve another -11 %
+        try { return analyze_symbolic(pattern, ocp, &o, S); }
+        catch (const std::bad_alloc&) { S.error = "host allocation failed"; return NMPC_E_ALLOC; }
+    };
+    const int64_t n_hint = pattern ? pattern->n : (ocp ? (int64_t)ocp->N * (ocp->nx + ocp->nu) : 0);
+    const bool small_first = auto_relax && n_hint <= 8192;
+    nmpc_status st = analyze_with(small_first, h->S);
     if (st != NMPC_OK) { h->err = h->S.error; return fail(st); }
-    if (auto_relax && h->opt.smem_front_max <= 0 && h->S.flops <= 1e8) {
-        nmpc_options o2 = h->opt;
-        o2.relax_small = 32;
-        if (o2.nd_leaf <= 0) o2.nd_leaf = 32;             // smaller dissection leaves: C1 factor + solve another -11 %
+    if (auto_relax && small_first != eligible(h->S)) {
         Symbolic S2;
-        nmpc_status st2;
-        try { st2 = analyze_symbolic(pattern, ocp, &o2, S2); }
-        catch (const std::bad_alloc&) { st2 = NMPC_E_ALLOC; }
-        if (st2 == NMPC_OK && S2.max_front <= SMALL_ROWS_MAX - 2) { S2.analyze_ms += h->S.analyze_ms; h->S = std::move(S2); }
+        if (analyze_with(!small_first, S2) == NMPC_OK && (small_first || eligible(S2))) { S2.analyze_ms += h->S.analyze_ms; h->S = std::move(S2); }
     }
     auto body = [&]() -> nmpc_status {
         const Symbolic& S = h->S;
-        int dev = 0, smem_optin = 0;
-        CK(cudaGetDevice(&dev));
-        CK(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
-        int num_sms = 0, ctas_per_sm = 1, small_max_r = 0;
-        size_t factor_smem = 0;
-        CK(cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev));
+        int ctas_per_sm = lat_ctas, small_max_r = lat_rmax;
+        size_t factor_smem = lat_smem;
         // latency mode: a small problem (dependency-latency bound) whose largest fronts fit the whole
         // shared memory of an SM keeps every front in the one-CTA kernel family; else two CTAs per SM and tiled big fronts
-        const bool latency_mode = S.flops <= 1e8 && S.max_front <= SMALL_ROWS_MAX - 2 && h->opt.smem_front_max <= 0;
-        CK(configure_factor_kernels(smem_optin, latency_mode, &ctas_per_sm, &factor_smem, &small_max_r));
+        const bool latency_mode = eligible(S) && h->opt.smem_front_max <= 0;
+        if (!latency_mode) CK(configure_factor_kernels(smem_optin, false, &ctas_per_sm, &factor_smem, &small_max_r));
         if (h->opt.smem_front_max > 0) small_max_r = std::min(small_max_r, h->opt.smem_front_max);
         int solve_ctas = 1, sbuf = 0; size_t solve_smem = 0;
         CK(configure_solve_kernels(smem_optin, small_max_r, &solve_ctas, &solve_smem, &sbuf));
@@ -459,17 +510,21 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
 
 void nmpc_destroy(nmpc_handle h) {
     if (!h) return;
+    DeviceGuard dg(h);
     for (void* p : h->allocs) cudaFree(p);
     if (h->h_pinned) cudaFreeHost(h->h_pinned);
     if (h->iter_graph) cudaGraphExecDestroy(h->iter_graph);
     if (h->ev[0]) cudaEventDestroy(h->ev[0]);
     if (h->ev[1]) cudaEventDestroy(h->ev[1]);
+    for (cudaEvent_t e : h->it_ev) cudaEventDestroy(e);
     if (h->own_stream) cudaStreamDestroy(h->stream);
     delete h;
 }
 
+#ifdef NMPC_TRACE_BUILD
 int64_t nmpc_get_task_trace(nmpc_handle h, int32_t kind, int32_t* tasks_host, uint64_t* stamps_host, int64_t cap) {
     if (!h || kind < 0 || kind > 1) return -1;
+    DeviceGuard dg(h);
     const int64_t nt = kind == 0 ? h->F.n_ftasks : h->F.n_stasks;
     const unsigned long long* tr = kind == 0 ? h->F.ftrace : h->F.strace;
     if (!tr) return 0;
@@ -480,8 +535,9 @@ int64_t nmpc_get_task_trace(nmpc_handle h, int32_t kind, int32_t* tasks_host, ui
     if (cudaMemcpy(stamps_host, tr, (size_t)k * 8 * sizeof(uint64_t), cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
     return k;
 }
+#endif
 
-const char* nmpc_last_error(nmpc_handle h) { return h ? h->err.c_str() : "null handle"; }
+const char* nmpc_last_error(nmpc_handle h) { return h ? h->err.c_str() : g_create_error.c_str(); }
 int64_t nmpc_launch_count(nmpc_handle h) { return h ? h->launches : 0; }
 
 nmpc_status nmpc_get_info(nmpc_handle h, nmpc_sym_info* out) {
@@ -493,6 +549,7 @@ nmpc_status nmpc_get_info(nmpc_handle h, nmpc_sym_info* out) {
 
 nmpc_status nmpc_get_factor(nmpc_handle h, double* panels_host) {
     if (!h || !panels_host) return NMPC_E_ARG;
+    DeviceGuard dg(h);
     if (!h->factored) { h->err = "no successful factorization"; return NMPC_E_STATE; }
     CK(cudaMemcpyAsync(panels_host, h->D.L, (size_t)h->S.panel_ptr.back() * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
     CK(cudaStreamSynchronize(h->stream));
@@ -501,6 +558,7 @@ nmpc_status nmpc_get_factor(nmpc_handle h, double* panels_host) {
 
 nmpc_status nmpc_factor(nmpc_handle h, const double* values_dev, double eta, int64_t* info_host) {
     if (!h || !values_dev) return NMPC_E_ARG;
+    DeviceGuard dg(h);
     if (values_dev != h->d_Kval)
         CK(cudaMemcpyAsync(h->d_Kval, values_dev, (size_t)h->S.nnzK * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
     return run_factor(h, eta, info_host);
@@ -508,6 +566,7 @@ nmpc_status nmpc_factor(nmpc_handle h, const double* values_dev, double eta, int
 
 nmpc_status nmpc_solve(nmpc_handle h, double* rhs, int32_t nrhs) {
     if (!h || !rhs || nrhs < 1) return NMPC_E_ARG;
+    DeviceGuard dg(h);
     if (!h->factored) { h->err = "nmpc_solve before a successful nmpc_factor"; return NMPC_E_STATE; }
     for (int k = 0; k < nrhs; ++k) TRY(run_solve(h, rhs + (int64_t)k * h->S.n));
     CK(cudaGetLastError());
@@ -516,6 +575,7 @@ nmpc_status nmpc_solve(nmpc_handle h, double* rhs, int32_t nrhs) {
 
 nmpc_status nmpc_kkt_multiply(nmpc_handle h, const double* x_dev, double* y_dev) {
     if (!h || !x_dev || !y_dev) return NMPC_E_ARG;
+    DeviceGuard dg(h);
     launch_kkt_multiply(h->S.n, h->d_full_ptr, h->d_full_idx, h->d_full_src, h->d_Kval, h->eta_cur, x_dev, y_dev, h->stream);
     h->launches++;
     CK(cudaGetLastError());
@@ -524,6 +584,7 @@ nmpc_status nmpc_kkt_multiply(nmpc_handle h, const double* x_dev, double* y_dev)
 
 nmpc_status nmpc_update_params(nmpc_handle h, const double* x0_dev, const double* ref_dev) {
     if (!h) return NMPC_E_ARG;
+    DeviceGuard dg(h);
     if (!h->has_model) { h->err = "handle has no model"; return NMPC_E_STATE; }
     const ModelDesc& d = h->M.desc;
     if (x0_dev) CK(cudaMemcpyAsync(h->M.x0, x0_dev, sizeof(double) * d.nx, cudaMemcpyDeviceToDevice, h->stream));
@@ -533,6 +594,7 @@ nmpc_status nmpc_update_params(nmpc_handle h, const double* x0_dev, const double
 
 nmpc_status nmpc_update_params_host(nmpc_handle h, const double* x0_host, const double* ref_host) {
     if (!h) return NMPC_E_ARG;
+    DeviceGuard dg(h);
     if (!h->has_model) { h->err = "handle has no model"; return NMPC_E_STATE; }
     const ModelDesc& d = h->M.desc;
     double* stage = h->h_pinned + 64;
@@ -551,6 +613,7 @@ nmpc_status nmpc_update_params_host(nmpc_handle h, const double* x0_host, const 
 
 nmpc_status nmpc_get_iterate(nmpc_handle h, double* y, double* sp, double* sm, double* wp, double* wm, double* zL, double* zU) {
     if (!h) return NMPC_E_ARG;
+    DeviceGuard dg(h);
     if (!h->has_model) return NMPC_E_STATE;
     const size_t n = h->M.n * sizeof(double), m = h->M.m * sizeof(double);
     const IpmVectors& V = h->V;
@@ -566,6 +629,7 @@ nmpc_status nmpc_get_iterate(nmpc_handle h, double* y, double* sp, double* sm, d
 
 nmpc_status nmpc_set_iterate(nmpc_handle h, const double* y, const double* sp, const double* sm, const double* wp, const double* wm, const double* zL, const double* zU) {
     if (!h || !y || !sp || !sm || !wp || !wm || !zL || !zU) return NMPC_E_ARG;
+    DeviceGuard dg(h);
     if (!h->has_model) return NMPC_E_STATE;
     const size_t n = h->M.n * sizeof(double), m = h->M.m * sizeof(double);
     const IpmVectors& V = h->V;
@@ -582,6 +646,7 @@ nmpc_status nmpc_set_iterate(nmpc_handle h, const double* y, const double* sp, c
 
 nmpc_status nmpc_model_eval(nmpc_handle h, const double* y, const double* lam, double* c, double* gradf, double* Jval, double* Wval) {
     if (!h || !y) return NMPC_E_ARG;
+    DeviceGuard dg(h);
     if (!h->has_model) return NMPC_E_STATE;
     if (Wval && !lam) return NMPC_E_ARG;
     launch_model_eval(h->M, y, nullptr, nullptr, lam, c, gradf, Jval, Wval, h->stream);
@@ -592,6 +657,7 @@ nmpc_status nmpc_model_eval(nmpc_handle h, const double* y, const double* lam, d
 
 nmpc_status nmpc_assemble(nmpc_handle h, const double* Jval, const double* Wval, const double* sigx, const double* q, double eta, double* Kval) {
     if (!h || !Jval || !Wval || !sigx || !q || !Kval) return NMPC_E_ARG;
+    DeviceGuard dg(h);
     if (!h->has_model) return NMPC_E_STATE;
     launch_assemble_K(h->M, Jval, Wval, sigx, q, eta, Kval, h->stream);
     h->launches++;
@@ -617,6 +683,7 @@ nmpc_status nmpc_get_kkt_pattern(nmpc_handle h, int64_t* nnz, int64_t* rowptr, i
 // ---- Algorithm 2 (LiftedIPM), steps S1..S10 of DESIGN.md section 3 ----
 nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* y_inout, nmpc_stats* stats, nmpc_trace_row* trace, int32_t trace_cap) {
     if (!h) return NMPC_E_ARG;
+    DeviceGuard dg(h);
     if (!h->has_model) { h->err = "nmpc_ipm_solve needs a model (nmpc_ocp)"; return NMPC_E_STATE; }
     if (use_y0 && !y_inout) return NMPC_E_ARG;
     const nmpc_options& o = h->opt;
@@ -660,7 +727,7 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
             else eta = ((eta_last == 0.0) ? o.eta_grow_first : o.eta_grow) * eta;
             if (eta > o.eta_max) return NMPC_E_INERTIA;
             ++nfact;
-            pt.begin(&S.ms_factor);
+            pt.begin(&S.ms_factor, 2);
             nmpc_status fs = run_factor(h, eta, nullptr);
             pt.end();
             if (fs == NMPC_OK) return NMPC_OK;
@@ -668,11 +735,11 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
         }
     };
     auto solve_step_update = [&](double mu_, double tau_) -> nmpc_status {
-        pt.begin(&S.ms_solve);                                                 // S8: Eq. (22)-(25)
+        pt.begin(&S.ms_solve, 3);                                                 // S8: Eq. (22)-(25)
         CK(cudaMemcpyAsync(V.dy, V.b, sizeof(double) * M.n, cudaMemcpyDeviceToDevice, st));
         TRY(run_solve(h, V.dy));
         pt.end();
-        pt.begin(&S.ms_vector);
+        pt.begin(&S.ms_vector, 4);
         launch_step(M, V, mu_, tau_, nullptr, st); h->launches += 1;                    // S8-S9
         launch_update(M, V, h->D.fail_col, st); h->launches++;                 // S10: Eq. (26)
         pt.end();
@@ -681,10 +748,10 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
     while (true) {
         // S2: evaluate c, grad f, J, W (K_SIMD of the paper, Alg. 2 line 5) and the residuals of Eq. (9)
         if (!top_done) {
-            pt.begin(&S.ms_eval);
+            pt.begin(&S.ms_eval, 0);
             launch_model_eval(M, V.y, V.wp, V.wm, nullptr, V.c, V.gradf, V.Jval, V.Wval, st); h->launches++;
             pt.end();
-            pt.begin(&S.ms_vector);
+            pt.begin(&S.ms_vector, 4);
             launch_residuals(M, V, o.gamma, st); h->launches += 1;
             CK(cudaMemcpyAsync(hs, V.scal, sizeof(double) * 10, cudaMemcpyDeviceToHost, st));
             if (pending) CK(cudaMemcpyAsync(flag, h->D.fail_col, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
@@ -741,10 +808,10 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
             ++it;
             continue;
         }
-        pt.begin(&S.ms_vector);
+        pt.begin(&S.ms_vector, 4);
         launch_sigma_rhs(M, V, mu, nullptr, st); h->launches += 2;                      // S6
         pt.end();
-        pt.begin(&S.ms_assemble);
+        pt.begin(&S.ms_assemble, 1);
         launch_assemble_K(M, V.Jval, V.Wval, V.sigx, V.q, 0.0, V.Kval, st); h->launches++;
         pt.end();
         double eta = 0.0;
@@ -755,7 +822,7 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
             launch_factor(h->D, h->F, h->d_Kval, 0.0, epoch, nullptr, st); h->launches += 1;
             pending = true; pend_mu = mu; pend_tau = tau;
         } else {
-            pt.begin(&S.ms_factor);
+            pt.begin(&S.ms_factor, 2);
             nmpc_status fs = run_factor(h, 0.0, nullptr);
             pt.end();
             if (fs == NMPC_E_NOT_SPD) {
@@ -770,7 +837,9 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
         ++it;
     }
 done:
-    h->have_state = true;
+    // z* is kept for the next warm start (Alg. 1 line 10) only if it is usable: converged, or stopped at max_iter with a finite
+    // iterate.  After a non-finite iterate or an exhausted inertia schedule the next solve falls back to the cold start.
+    h->have_state = status == NMPC_OK || (status == NMPC_E_MAXITER && hs[6] == 0.0);
     launch_objective(M, V, st); h->launches += 1;
     CK(cudaMemcpyAsync(hs + 9, V.scal + 9, sizeof(double), cudaMemcpyDeviceToHost, st));
     if (y_inout) CK(cudaMemcpyAsync(y_inout, V.y, sizeof(double) * M.n, cudaMemcpyDeviceToDevice, st));
@@ -785,6 +854,7 @@ done:
 
 nmpc_status nmpc_ipm_solve_host(nmpc_handle h, int32_t warm, const double* x0_host, const double* ref_host, double* y_out_host, nmpc_stats* stats) {
     if (!h) return NMPC_E_ARG;
+    DeviceGuard dg(h);
     TRY(nmpc_update_params_host(h, x0_host, ref_host));
     nmpc_status st = nmpc_ipm_solve(h, warm, 0, nullptr, stats, nullptr, 0);
     if (y_out_host) {

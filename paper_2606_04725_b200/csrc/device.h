@@ -89,8 +89,10 @@ struct DagPlan {
     uint32_t* blk_f = nullptr;           // block slots
     uint32_t* blk_b = nullptr;
     uint32_t* sub_done = nullptr;        // block slots: published 8-column blocks of the diagonal tile L_JJ, (epoch-1)*16 + count
-    unsigned long long* ftrace = nullptr;   // optional (NMPC_TRACE=1): 8 timestamps per factor task / per solve task
+#ifdef NMPC_TRACE_BUILD                     // measurement build only (libnmpc_b200_aids.so, include/nmpc_aids.h)
+    unsigned long long* ftrace = nullptr;   // 8 timestamps per factor task / per solve task
     unsigned long long* strace = nullptr;
+#endif
     int64_t sync_words = 0;
     int32_t small_max_r = 0;
     int32_t sbuf = 0;                    // doubles per staged column block of the small-supernode solves

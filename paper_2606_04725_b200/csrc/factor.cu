@@ -57,8 +57,12 @@ __device__ __forceinline__ void red_release_add(uint32_t* p, uint32_t v) {
 __device__ __forceinline__ void spin_until_ge(const uint32_t* p, uint32_t target) {
     while (ld_acquire(p) < target) __nanosleep(40);
 }
+#ifdef NMPC_TRACE_BUILD
 __device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
 #define TRACE(slot) do { if (tr && threadIdx.x == 0) tr[slot] = gtime(); } while (0)
+#else
+#define TRACE(slot) do { (void)tr; } while (0)
+#endif
 __device__ __forceinline__ void cp_async16(double* dst_smem, const double* src, int src_bytes) {
     const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(src), "r"(src_bytes) : "memory");
@@ -724,10 +728,14 @@ __global__ void __launch_bounds__(NT, 2) factor_dag_kernel(DevSym D, DagPlan F, 
         if (threadIdx.x == 0) s_task = (int)(atomicAdd(F.sync, 1u) - base);
         __syncthreads();
         const int t = s_task;
-        if (t >= F.n_ftasks) break;
+        if (t < 0 || t >= F.n_ftasks) break;             // t < 0: a call number that does not match the counters (never on a consistent handle)
         const int4 tk = F.ftasks[t];
+#ifdef NMPC_TRACE_BUILD
         unsigned long long* tr = F.ftrace ? F.ftrace + (size_t)t * 8 : nullptr;
         if (tr && threadIdx.x == 0) { tr[0] = gtime(); unsigned sid; asm volatile("mov.u32 %0, %%smid;" : "=r"(sid)); tr[5] = sid; }
+#else
+        unsigned long long* tr = nullptr;
+#endif
         if (tk.x == 0) small_front_task(D, F, tk.y, Kval, eta, epoch, sm, tr);
         else tile_task(D, F, tk.y, tk.z, tk.w, Kval, eta, epoch, sm, tr);
     }

@@ -2,8 +2,9 @@
 // and the fused IPM vector kernels (step a6: residuals of Eq. 9/11, right-hand side of Eq. 17, eliminated directions of
 // Eq. 10/14, fraction-to-the-boundary min-reductions, Eq. 26 update, error norms of Eq. 27-28).
 //
-// Reductions use a FIXED grid (RED_BLOCKS x 256 threads, grid-stride) and a fixed shuffle/shared-memory tree, then a
-// one-block finalize kernel: results are bitwise reproducible run to run.  No floating-point atomics anywhere.
+// Reductions use a FIXED grid (RED_BLOCKS x 256 threads, grid-stride) and a fixed shuffle/shared-memory tree; the block that
+// takes the last ticket (last_block_arrives) reduces the per-block partials in block order, so there is no separate finalize
+// launch and results are bitwise reproducible run to run.  No floating-point atomics anywhere.
 // Compiled with -fmad=false: the element-wise expressions below round like the plain fp64 statements of the method.
 #include <algorithm>
 #include <cfloat>

@@ -6,7 +6,7 @@
 
 #include <cstdint>
 
-#include "../../include/nmpc.h"
+#include "../../include/nmpc_aids.h"
 
 namespace {
 

@@ -89,7 +89,11 @@ __device__ __forceinline__ void stage_block(const DevSym& D, const Sn& q, int k,
     cp_async_commit();
 }
 
+#ifdef NMPC_TRACE_BUILD
 #define STRACE(slot) do { if (tr && threadIdx.x == 0) { unsigned long long g_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g_)); tr[slot] = g_; } } while (0)
+#else
+#define STRACE(slot) do { (void)tr; } while (0)
+#endif
 __device__ __forceinline__ void fwd_small(const DevSym& D, const DagPlan& F, int s, const double* b, double* x, uint32_t epoch, double* sm, unsigned long long* tr) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const Sn q = sn_of(D, s);
@@ -510,13 +514,17 @@ __global__ void __launch_bounds__(NT, 2) solve_dag_kernel(DevSym D, DagPlan F, d
         if (threadIdx.x == 0) s_task = (int)(atomicAdd(F.sync + 1, 1u) - base);
         __syncthreads();
         const int t = s_task;
-        if (t >= F.n_stasks) break;
+        if (t < 0 || t >= F.n_stasks) break;
         const int4 tk = F.stasks[t];
+#ifdef NMPC_TRACE_BUILD
         unsigned long long* tr = F.strace ? F.strace + (size_t)t * 8 : nullptr;
         if (tr && threadIdx.x == 0) { unsigned long long g; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g)); tr[0] = g; }
+#else
+        unsigned long long* tr = nullptr;
+#endif
         if (tk.w == 0) { if (tk.x == 0) fwd_small(D, F, tk.y, b, x, epoch, sm, tr); else fwd_tiled(D, F, tk.y, tk.z, b, x, epoch, sm); }
         else           { if (tk.x == 0) bwd_small(D, F, tk.y, b, x, epoch, sm, tr); else bwd_tiled(D, F, tk.y, tk.z, b, x, epoch, sm); }
-        if (tr && threadIdx.x == 0) { unsigned long long g; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g)); tr[4] = g; }
+        STRACE(4);
     }
 }
 

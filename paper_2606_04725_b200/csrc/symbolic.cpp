@@ -15,7 +15,7 @@ void default_options(nmpc_options* o) {
     std::memset(o, 0, sizeof(*o));
     o->ordering = NMPC_ORDER_AUTO;
     o->nd_leaf = 0;                // 0 = choose from the structure
-    o->relax_small = -1;           // auto: 8, or 32 for small (latency-mode) problems, see nmpc_analyze
+    o->relax_small = -1;           // auto: nmpc_analyze uses 64, or 32 for small (latency-mode) problems; the host-only nmpc_symbolic_analyze 8
     o->relax_zeros = 0.05;         // fraction-based merging lengthens the fronts at the top of the tree (the critical path): keep it small
     o->smem_front_max = 0;         // 0 = device default
     o->use_graph = 1;

@@ -1,0 +1,88 @@
+#!/usr/bin/env python
+"""Writes tests/golden/ipm_full_<config>.npz: the ORACLE's closed loop (Algorithm 1 + 2) at BASELINE size.
+
+    python tests/golden/make_fullsize_ipm.py C3 [--resolves 2] [--linsolve blocktri]
+
+Calls only `oracle/` and the seeded input generator `ocp_inputs.py` (never the CUDA path).  The stored values are what
+`tests/test_gpu_fullsize.py` compares the CUDA path with where the oracle needs tens of minutes (C3: block-tridiagonal
+dense Cholesky O2 over 50 stage blocks of 2516, SURVEY.md section 8(c) "Oracle linear algebra", BASELINE.md section 3:
+"cold + 2 re-solves, results cached on disk").  Cache key = (config, master seed, oracle option defaults, linsolve):
+stored in the file and checked by the test.
+
+Per solve j = 0..R (0 = cold): x0, iteration / factorization counts, status, the per-iteration trace (mu, eta, E0,
+alpha_pr, alpha_du), the converged primal y* and the full primal-dual iterate z* (float64).  Of the LAST solve additionally
+the iterate BEFORE its last Newton step (a late-iteration KKT system: mu small, Sigma spread over many decades).
+"""
+from __future__ import annotations
+
+import argparse
+import hashlib
+import json
+import os
+import sys
+import time
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+ROOT = os.path.dirname(os.path.dirname(HERE))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from ocp_inputs import MASTER_SEED, make_config  # noqa: E402
+from oracle.ipm import DEFAULTS, nmpc_closed_loop  # noqa: E402
+
+STATE_FIELDS = ("y", "sp", "sm", "wp", "wm", "zL", "zU")
+
+
+def cache_key(name, linsolve):
+    blob = json.dumps(dict(config=name, seed=MASTER_SEED, options={k: DEFAULTS[k] for k in sorted(DEFAULTS)},
+                           linsolve=linsolve), sort_keys=True, default=str)
+    return hashlib.sha256(blob.encode()).hexdigest()[:16]
+
+
+def golden_path(name):
+    return os.path.join(HERE, f"ipm_full_{name}.npz")
+
+
+def run(name, resolves, linsolve, log=print):
+    cfg = make_config(name)
+    t0 = time.perf_counter()
+    out, ipm = nmpc_closed_loop(cfg, n_resolves=resolves, linsolve=linsolve)
+    wall = time.perf_counter() - t0
+    d = dict(key=np.array(cache_key(name, linsolve)), n_solves=np.array(len(out)), wall_seconds=np.array(wall),
+             linsolve=np.array(linsolve))
+    for j, o in enumerate(out):
+        log(f"{name} solve {j}: status {o['status']} iters {o['iters']} factorizations {o['factorizations']}")
+        d[f"x0_{j}"] = o["x0"]
+        d[f"iters_{j}"] = np.array(o["iters"])
+        d[f"fact_{j}"] = np.array(o["factorizations"])
+        d[f"status_{j}"] = np.array(o["status"])
+        d[f"trace_{j}"] = np.array([[t["mu"], t["eta"], t["E0"], t["alpha_pr"], t["alpha_du"]] for t in o["trace"]]).reshape(-1, 5)
+        for f in STATE_FIELDS:
+            d[f"{f}_{j}"] = getattr(o["state"], f)
+    ls = ipm.last_step                                   # the iterate before the last Newton step of the last solve
+    for f in STATE_FIELDS:
+        d[f"late_{f}"] = getattr(ls["state"], f)
+    d["late_mu"] = np.array(ls["mu"])
+    d["late_eta"] = np.array(ls["eta"])
+    d["late_dy"] = ls["dy"]
+    return d
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("config", choices=["C1", "C2", "C3", "C4"])
+    ap.add_argument("--resolves", type=int, default=2)
+    ap.add_argument("--linsolve", default=None)
+    ap.add_argument("--out", default=None)
+    a = ap.parse_args()
+    linsolve = a.linsolve or ("blocktri" if a.config in ("C2", "C3") else "sparse")
+    d = run(a.config, a.resolves, linsolve)
+    path = a.out or golden_path(a.config)
+    np.savez_compressed(path, **d)
+    print(f"wrote {path} ({os.path.getsize(path) / 1e6:.1f} MB) in {float(d['wall_seconds']):.1f} s of oracle time")
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,219 @@
+"""Parity of nmpc_ipm_solve against the oracle's Algorithm 1 / 2 at BASELINE.json's FULL sizes, in the launch configuration
+bench.py times (default options, CUDA-graph iteration): C1 distill-34, C2 plate-20, C3 plate-50 (n = 125 800) and C4
+distill-130 (n = 52 400) -- north_star: "oracle-matching NMPC solutions on all five configs" (C0 is full size in
+test_gpu_parity.py).
+
+Oracle side: `tests/golden/make_fullsize_ipm.py` (calls only oracle/): cold solve + 2 warm re-solves of the closed loop.
+C1, C2 and C4 are computed when the test runs (seconds to a minute of CPU).  C3 needs the block-tridiagonal dense Cholesky O2
+over 50 stage blocks of 2516 (~2e12 flops per factorization, ~40 min for the three solves), so its result is the
+committed file tests/golden/ipm_full_C3.npz written by that script, keyed by (config, seed, oracle
+options, linsolve).
+
+Compared per solve, in REPLAY mode (the GPU run is fed the oracle's recorded x0 / ref sequence): status,
+IPM iteration and factorization counts, the mu and eta traces (==), step lengths (sanity band), the converged primal solution
+(<= 1e-6 relative, north_star) and the whole primal-dual iterate (1e-5).  The late-iteration KKT system of the last solve
+(mu ~ 1e-6, Sigma spread over > 10 decades) is then assembled, factored and solved on the GPU and checked against SciPy
+on the oracle's model code: K entries, factor backward error (reading G17: exactly on the pattern of L for C1/C2/C4, by 16
+random-vector probes ||L(L^T v) - P K P^T v|| / (||K||_F ||v||) for C3), solve backward error (reading G16).
+"""
+import importlib.util
+import os
+
+import numpy as np
+import pytest
+import scipy.sparse as sp
+import torch
+
+import paper_2606_04725_b200 as nb
+from ocp_inputs import make_config, sigma_sweep_draws
+from oracle.nlp import TranscribedOCP
+
+from gpu_util import factor_as_sparse, factor_backward_error, normwise_backward_error, values_on_pattern
+
+pytestmark = pytest.mark.gpu
+
+DEV = "cuda:0"
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+_spec = importlib.util.spec_from_file_location("make_fullsize_ipm", os.path.join(GOLD, "make_fullsize_ipm.py"))
+gold = importlib.util.module_from_spec(_spec)
+_spec.loader.exec_module(gold)
+
+LINSOLVE = {"C1": "sparse", "C2": "blocktri", "C3": "blocktri", "C4": "sparse"}
+STATE = gold.STATE_FIELDS
+
+
+def dev(a):
+    return torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64).to(DEV)
+
+
+_cache = {}
+
+
+def oracle_run(name):
+    """The oracle's closed loop at full size: the committed golden file when there is one (its key must match the
+    current oracle options), else computed now."""
+    if name not in _cache:
+        path = gold.golden_path(name)
+        if os.path.exists(path):
+            d = dict(np.load(path, allow_pickle=False))
+            assert str(d["key"]) == gold.cache_key(name, LINSOLVE[name]), "golden file is stale: rerun make_fullsize_ipm.py"
+        else:
+            d = gold.run(name, 2, LINSOLVE[name], log=lambda *_: None)
+        _cache[name] = d
+    return _cache[name]
+
+
+def _traces(tg, to):
+    """Both per-iteration traces side by side (printed when a count or a trace entry differs)."""
+    rows = ["  it |        mu       eta   alpha_pr   alpha_du         E0  (GPU) |        mu       eta   alpha_pr   alpha_du         E0  (oracle)"]
+    for k in range(max(len(tg), len(to))):
+        g = [tg[k][f] for f in ("mu", "eta", "alpha_pr", "alpha_du", "E0")] if k < len(tg) else None
+        o = [to[k][i] for i in (0, 1, 3, 4, 2)] if k < len(to) else None
+        fmt = lambda v: " ".join(f"{x:10.3e}" for x in v) if v is not None else " " * 54   # noqa: E731
+        rows.append(f"{k:4d} | {fmt(g)}        | {fmt(o)}")
+    return "\n".join(rows)
+
+
+@pytest.mark.parametrize("name", ["C1", "C2", "C4", "C3"])
+def test_ipm_fullsize_closed_loop_vs_oracle(name):
+    cfg = make_config(name)
+    d = oracle_run(name)
+    h = nb.Handle(None, nb.make_ocp(cfg), None)              # default options: what bench.py launches
+    y = torch.zeros(cfg.n, dtype=torch.float64, device=DEV)
+    n, m = cfg.n, cfg.m
+    bufs = [torch.empty(k, dtype=torch.float64, device=DEV) for k in (n, m, m, m, m, n, n)]
+    for j in range(int(d["n_solves"])):
+        assert str(d[f"status_{j}"]) == "converged"
+        h.update_params(dev(d[f"x0_{j}"]), dev(cfg.ref_for_solve(j)))
+        rg = h.ipm_solve(int(j > 0), y, trace_cap=256, check=False)
+        to = d[f"trace_{j}"]
+        report = f"{name} solve {j}: GPU {rg['iters']} iterations / oracle {int(d[f'iters_{j}'])}\n" + _traces(rg["trace"], to)
+        assert rg["status"] == 0, report
+        assert rg["iters"] == int(d[f"iters_{j}"]), report
+        assert rg["factorizations"] == int(d[f"fact_{j}"]), report
+        for k, tg in enumerate(rg["trace"]):
+            assert tg["mu"] == to[k, 0] and tg["eta"] == to[k, 1], report
+            # step lengths are ratios of small quantities and inherit cond(K) * eps from dy (cond ~ 1e11 in the middle of a cold
+            # solve at these sizes): a sanity band, not a parity bar -- the bars are the counts, the mu / eta traces and z*
+            assert abs(tg["alpha_pr"] - to[k, 3]) <= 5e-2 and abs(tg["alpha_du"] - to[k, 4]) <= 5e-2, report
+        yo = d[f"y_{j}"]
+        assert np.abs(y.cpu().numpy() - yo).max() <= 1e-6 * np.abs(yo).max(), report
+        h.get_iterate(*bufs)
+        for g_, f in zip(bufs, STATE):
+            o_ = d[f"{f}_{j}"]
+            assert np.abs(g_.cpu().numpy() - o_).max() <= 1e-5 * max(1.0, np.abs(o_).max()), (name, j, f)
+    h.close()
+
+
+def _probe_backward_error(info, panels, K, perm, rng, nvec=16):
+    """max_v ||L (L^T v) - P K P^T v||_2 / (||K||_F ||v||_2) over nvec random vectors, from the supernodal panels
+    (column-major r x w, leading dimension r rounded up to even), blockwise on the host."""
+    n = info["n"]
+    V = rng.normal(size=(n, nvec))
+    T = np.zeros((n, nvec))
+    off = 0
+    blocks = []
+    for s in range(info["nsuper"]):
+        c0, c1 = int(info["super_start"][s]), int(info["super_start"][s + 1])
+        rows = info["rows"][info["rows_ptr"][s]:info["rows_ptr"][s + 1]].astype(np.int64)
+        r, w = len(rows), c1 - c0
+        ld = (r + 1) & ~1
+        P = panels[off:off + ld * w].reshape(w, ld).T[:r]
+        off += ld * w
+        P = np.concatenate([np.tril(P[:w]), P[w:]], axis=0) if r > w else np.tril(P)
+        T[c0:c1] = P.T @ V[rows]                              # (L^T v) restricted to this supernode's columns
+        blocks.append((rows, c0, c1, P))
+    out = np.zeros((n, nvec))
+    for rows, c0, c1, P in blocks:
+        out[rows] += P @ T[c0:c1]
+    KP = sp.csr_matrix(K)[perm, :][:, perm]
+    R = out - KP @ V
+    Kf = np.sqrt((sp.csr_matrix(K).data ** 2).sum())
+    return float((np.linalg.norm(R, axis=0) / (Kf * np.linalg.norm(V, axis=0))).max())
+
+
+@pytest.mark.parametrize("name", ["C1", "C2", "C4", "C3"])
+def test_late_iteration_kkt_fullsize(name):
+    """The KKT system of the LAST Newton step of the oracle's last re-solve (the hardest conditioning the IPM produces):
+    a2/a3 element-wise, a4 factor backward error, a5 solve backward error and forward error against the oracle's step."""
+    cfg = make_config(name)
+    d = oracle_run(name)
+    st = {f: d[f"late_{f}"] for f in STATE}
+    mu, eta = float(d["late_mu"]), float(d["late_eta"])
+    nlp = TranscribedOCP(cfg)
+    last = int(d["n_solves"]) - 1
+    nlp.set_params(d[f"x0_{last}"], cfg.ref_for_solve(last))
+    lam = st["wp"] - st["wm"]
+    Jo, Wo = nlp.jacobian(st["y"]), nlp.hessian(st["y"], lam)
+    hasL, hasU = np.isfinite(nlp.lb), np.isfinite(nlp.ub)
+    sigx = np.where(hasL, st["zL"] / np.where(hasL, st["y"] - nlp.lb, 1.0), 0.0) + np.where(hasU, st["zU"] / np.where(hasU, nlp.ub - st["y"], 1.0), 0.0)
+    q = st["wp"] / st["sp"] + st["wm"] / st["sm"]
+    K = (Wo + sp.diags(sigx + eta) + Jo.T @ sp.diags(q) @ Jo).tocsr()
+    assert mu <= 1e-5                                         # genuinely a late system
+    h = nb.Handle(None, nb.make_ocp(cfg), None)
+    h.update_params(dev(d[f"x0_{last}"]), dev(cfg.ref_for_solve(last)))
+    jrp, _ = h.get_jac_pattern(cfg.m)
+    wrp, _ = h.get_hess_pattern(cfg.n)
+    krp, kci = h.get_kkt_pattern(cfg.n)
+    Jv = torch.empty(int(jrp[-1]), dtype=torch.float64, device=DEV)
+    Wv = torch.empty(int(wrp[-1]), dtype=torch.float64, device=DEV)
+    Kv = torch.empty(int(krp[-1]), dtype=torch.float64, device=DEV)
+    h.model_eval(dev(st["y"]), dev(lam), None, None, Jv, Wv)
+    h.assemble(Jv, Wv, dev(sigx), dev(q), eta, Kv)
+    scale = values_on_pattern(abs(Wo) + sp.diags(sigx + eta) + abs(Jo).T @ sp.diags(q) @ abs(Jo), krp, kci)
+    assert np.all(np.abs(Kv.cpu().numpy() - values_on_pattern(K, krp, kci)) <= 1e-13 * scale)
+    stf, _ = h.factor(Kv, 0.0)
+    assert stf == 0
+    info = h.get_info()
+    panels = h.get_factor()
+    rng = np.random.default_rng(77)
+    if name == "C3":
+        assert _probe_backward_error(info, panels, K, info["perm"], rng) <= 1e-12
+    else:
+        assert factor_backward_error(factor_as_sparse(info, panels), K, info["perm"]) <= 1e-12
+        assert _probe_backward_error(info, panels, K, info["perm"], rng) <= 1e-12      # the probe agrees with the exact measure
+    del panels
+    dy_o = d["late_dy"]                                       # the oracle's Newton step: K dy = b
+    b = K @ dy_o
+    x = dev(b)
+    h.solve(x)
+    xg = x.cpu().numpy()
+    assert normwise_backward_error(K, xg, b) <= 1e-10
+    # both are backward-stable solutions of the same system: they agree through K
+    Kn = abs(K).sum(axis=1).max()
+    assert np.abs(K @ (xg - dy_o)).max() <= 2e-10 * (Kn * max(np.abs(xg).max(), np.abs(dy_o).max()) + np.abs(b).max())
+    h.close()
+
+
+def test_sigma_sweep_full_size_20_draws():
+    """C4 refactor sweep at full size (BASELINE.json:configs[4]): 20 of the 200 draws, each checked for the pivot flag, the
+    solve's normwise backward error against K rebuilt by SciPy from the oracle's J and grad^2 f, and (every 5th draw) the
+    factor backward error on the pattern of L."""
+    cfg = make_config("C4")
+    nlp = TranscribedOCP(cfg)
+    nlp.set_params(cfg.x0, cfg.ref_for_solve(0))
+    y0 = cfg.y_cold(cfg.x0)
+    Jo, Wo = nlp.jacobian(y0), nlp.hessian(y0, np.zeros(cfg.m))
+    h = nb.Handle(None, nb.make_ocp(cfg), None)
+    h.update_params(dev(cfg.x0), dev(cfg.ref_for_solve(0)))
+    jrp, _ = h.get_jac_pattern(cfg.m)
+    wrp, _ = h.get_hess_pattern(cfg.n)
+    krp, kci = h.get_kkt_pattern(cfg.n)
+    Jv = torch.empty(int(jrp[-1]), dtype=torch.float64, device=DEV)
+    Wv = torch.empty(int(wrp[-1]), dtype=torch.float64, device=DEV)
+    Kv = torch.empty(int(krp[-1]), dtype=torch.float64, device=DEV)
+    h.model_eval(dev(y0), dev(np.zeros(cfg.m)), None, None, Jv, Wv)
+    info = h.get_info()
+    worst_s, worst_f = 0.0, 0.0
+    for k, (sx, ss, b) in enumerate(sigma_sweep_draws(cfg, count=20)):
+        h.assemble(Jv, Wv, dev(sx), dev(ss), 0.0, Kv)
+        stf, _ = h.factor(Kv, 0.0)
+        assert stf == 0, k
+        x = dev(b)
+        h.solve(x)
+        K = (Wo + sp.diags(sx) + Jo.T @ sp.diags(ss) @ Jo).tocsr()
+        worst_s = max(worst_s, normwise_backward_error(K, x.cpu().numpy(), b))
+        if k % 5 == 0:
+            worst_f = max(worst_f, factor_backward_error(factor_as_sparse(info, h.get_factor()), K, info["perm"]))
+    assert worst_s <= 1e-10 and worst_f <= 1e-12, (worst_s, worst_f)
+    h.close()

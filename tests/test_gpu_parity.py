@@ -490,3 +490,64 @@ def test_graph_and_plain_launch_paths_agree():
         h.close()
     assert its[0] == its[1] and its[0][2] == 0 and its[0][3] == 0
     assert np.array_equal(ys[0], ys[1])
+
+
+def test_flag_restart_across_call_number_limit():
+    """The completion flags of the persistent kernels are call-number valued and restart from zero before a counter could
+    overflow (api.cu: next_epoch).  With the limit forced down to 5 calls (options.epoch_limit, a test hook) a cold solve,
+    warm re-solves and bare refactor + solve calls cross the restart many times, on the CUDA-graph path and on the plain
+    one; every result must be bitwise what a handle that never restarts gives."""
+    cfg = make_config("C1", trays=12, N=16)
+    K, b, _ = kkt_from_oracle(cfg)
+    outs = []
+    for limit, use_graph in ((0, 1), (5, 1), (5, 0), (3, 1)):
+        h = nb.Handle(None, nb.make_ocp(cfg), nb.default_options(epoch_limit=limit, use_graph=use_graph))
+        y = torch.zeros(cfg.n, dtype=torch.float64, device=DEV)
+        h.update_params(dev(cfg.x0), dev(cfg.ref_for_solve(0)))
+        res = [h.ipm_solve(0, y)]
+        ys = [y.cpu().numpy().copy()]
+        for j in range(1, 5):
+            h.update_params(dev(np.clip(cfg.x0 + 0.01 * j, *cfg.x0_clip)), dev(cfg.ref_for_solve(j)))
+            res.append(h.ipm_solve(1, y))
+            ys.append(y.cpu().numpy().copy())
+        assert all(r["status"] == 0 for r in res)
+        assert sum(r["iters"] for r in res) >= 12            # a restart every 3 factorizations at limit 5
+        rp, ci = h.get_kkt_pattern(cfg.n)
+        vals = dev(values_on_pattern(K, rp, ci))
+        xs = []
+        for _ in range(4):                                   # a factorization followed by a run of solves longer than the limit
+            h.factor(vals, 0.0)
+            for _ in range(7):
+                x = dev(b)
+                h.solve(x)
+                xs.append(x.cpu().numpy())
+        assert all(np.array_equal(xs[0], v) for v in xs[1:])
+        assert normwise_backward_error(K, xs[0], b) <= 1e-10
+        outs.append(([r["iters"] for r in res], ys, xs[0]))
+        h.close()
+    for o in outs[1:]:
+        assert o[0] == outs[0][0]
+        assert all(np.array_equal(a, b_) for a, b_ in zip(o[1], outs[0][1]))
+        assert np.array_equal(o[2], outs[0][2])
+
+
+def test_warm_start_after_a_failed_solve_falls_back_to_cold():
+    """A solve that ends with a non-finite iterate (NMPC_E_STEP) must not leave that iterate behind as the next warm
+    start (include/nmpc.h, nmpc_ipm_solve): the following call with warm = 1 starts cold and converges like a cold solve."""
+    cfg = make_config("C0")
+    h = _gpu_ipm(cfg)
+    h.update_params(dev(cfg.x0), dev(cfg.ref_for_solve(0)))
+    y = torch.zeros(cfg.n, dtype=torch.float64, device=DEV)
+    r_cold = h.ipm_solve(0, y)
+    y_cold = y.cpu().numpy().copy()
+    assert r_cold["status"] == 0
+    n, m = cfg.n, cfg.m
+    bad = [torch.full((k,), 1.0, dtype=torch.float64, device=DEV) for k in (n, m, m, m, m, n, n)]
+    bad[1][3] = float("nan")                                # a slack: the warm-start push only repairs y
+    h.set_iterate(*bad)
+    r_bad = h.ipm_solve(1, y, check=False)
+    assert r_bad["status"] == binding.NMPC_E_STEP
+    r_next = h.ipm_solve(1, y)                               # warm requested, no usable z*: cold start
+    assert r_next["status"] == 0 and r_next["iters"] == r_cold["iters"]
+    assert np.array_equal(y.cpu().numpy(), y_cold)
+    h.close()

@@ -44,6 +44,20 @@ def test_library_exports_every_declared_symbol():
     assert declared == set(binding.SIGNATURES), "binding.SIGNATURES out of step with include/nmpc.h"
 
 
+def test_measurement_aids_live_in_their_own_library():
+    """include/nmpc_aids.h (fp64 peak microbenchmarks, per-task timestamps) is exported by libnmpc_b200_aids.so only:
+    the product library carries neither symbol."""
+    hdr = open(os.path.join(ROOT, "include", "nmpc_aids.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(nmpc_[a-z_0-9]+)\s*\(", hdr))
+    assert declared == set(binding.AIDS_SIGNATURES)
+    aids, prod = binding.load_aids_library(), nb.load_library()
+    for name in sorted(declared | set(binding.SIGNATURES)):
+        assert hasattr(aids, name), name
+    for name in sorted(declared):
+        assert not hasattr(prod, name), f"{name} must not be in the product library"
+
+
 def _lower_csr(A):
     L = sp.tril(sp.csr_matrix(A), format="csr")
     L.sort_indices()
