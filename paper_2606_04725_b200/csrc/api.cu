@@ -170,12 +170,20 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
         for (int k = 0; k <= nbt[p]; ++k)
             cbnd.push_back((int32_t)(std::lower_bound(rel, rel + mc, tile_bound(k, W(p), R(p), nbp[p])) - rel));
     }
-    // task order: descending upward rank (longest remaining path, microseconds of a crude cost model); children rank above
-    // their parent, tile (I,k) above tile (I,J) for k < J -> the order is topological
-    const double STEP_US = 10.0;                         // one block column of a tiled front: potrf + trsm + flag hops
+    // task order: descending upward rank (longest remaining path in micro-seconds of a cost model calibrated on the per-task
+    // timelines of profiles/: a block column of a tiled front costs ~30 us on the chain POTRF -> TRSM -> GEMM tail -> POTRF, a
+    // tiled front ~45 us of assembly / flag hops on top, and its tile GEMMs run at ~100 GFLOP/s per CTA on the whole machine);
+    // children rank above their parent, tile (I,k) above tile (I,J) for k < J -> the order is topological
+    const double STEP_US = 30.0, FRONT_US = 45.0, MACHINE_FLOPS_PER_US = 100e3 * (double)num_sms * ctas_per_sm;
+    auto upd_flops = [&](int s) {                        // update (Schur complement) tiles: (r-w)^2 w
+        const double m = R(s) - W(s); return m * m * W(s);
+    };
+    auto panel_flops = [&](int s) {                      // panel tiles
+        const double r = R(s), m = R(s) - W(s); return (r * r * r - m * m * m) / 3.0 - m * m * W(s);
+    };
     auto front_time = [&](int s) {
         if (!cls[s]) { const double r = R(s), m = R(s) - W(s); return 2.0 + (r * r * r - m * m * m) / 3.0 * 2.0 / 50e3; }   // ~50 GFLOP/s per CTA
-        return nbp[s] * STEP_US + 2.0 + W(s) / 16.0 * 0.4;
+        return FRONT_US + nbp[s] * STEP_US + (panel_flops(s) + upd_flops(s)) / MACHINE_FLOPS_PER_US;
     };
     std::vector<double> rank_end(ns, 0.0);
     for (int s = ns - 1; s >= 0; --s) {                  // parents have larger indices (postorder)
@@ -186,10 +194,10 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
     std::vector<TK> tk;
     for (int s = 0; s < ns; ++s) {
         if (!cls[s]) { tk.push_back(TK{rank_end[s] + front_time(s), S.sn_level[s], 0, s, 0, 0}); continue; }
-        const double tail = 2.0 + W(s) / 16.0 * 0.4;
+        const double tail = upd_flops(s) / MACHINE_FLOPS_PER_US;
         for (int J = 0; J < nbt[s]; ++J)
             for (int I = J; I < nbt[s]; ++I)
-                tk.push_back(TK{rank_end[s] + tail + (J < nbp[s] ? (nbp[s] - J) * STEP_US : 0.0), S.sn_level[s], 1, s, I, J});
+                tk.push_back(TK{rank_end[s] + (J < nbp[s] ? tail + (nbp[s] - J) * STEP_US : 0.0), S.sn_level[s], 1, s, I, J});
     }
     std::stable_sort(tk.begin(), tk.end(), [](const TK& a, const TK& b) {
         if (a.rank != b.rank) return a.rank > b.rank;
@@ -241,6 +249,7 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
     TRY(dalloc(h, (size_t)F.sync_words, &F.sync));
     F.fac_done = F.sync + 2; F.sol_done_f = F.fac_done + ns; F.sol_done_b = F.sol_done_f + ns;
     F.tile_done = F.sol_done_b + ns; F.blk_f = F.tile_done + slots; F.blk_b = F.blk_f + bslots; F.sub_done = F.blk_b + bslots;
+
 #ifdef NMPC_TRACE_BUILD                                      // measurement build: per-task timestamps (nmpc_get_task_trace, include/nmpc_aids.h)
     TRY(dalloc(h, (size_t)F.n_ftasks * 8, &F.ftrace)); TRY(dalloc(h, (size_t)F.n_stasks * 8, &F.strace));
 #endif
@@ -716,6 +725,13 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
     const bool async = !o.time_phases;
     if (async && o.use_graph && !h->iter_graph && !h->graph_failed) TRY(capture_iteration_graph(h));
     const bool graph = async && o.use_graph && h->iter_graph != nullptr;
+    // traced solves: one CUDA event per iteration, recorded (no synchronisation) right before the iteration's S6 is launched
+    const int n_ev = trace ? std::min(trace_cap, o.max_iter) + 1 : 0;
+    while ((int)h->it_ev.size() < n_ev) { cudaEvent_t e = nullptr; CK(cudaEventCreate(&e)); h->it_ev.push_back(e); }
+    auto mark_iteration = [&](int k) {                   // start of iteration k = end of iteration k-1
+        if (k < n_ev) cudaEventRecord(h->it_ev[k], st);
+        pt.flush(trace && k > 0 && k - 1 < trace_cap ? &trace[k - 1] : nullptr);
+    };
     bool top_done = false;                               // the previous graph replay already ran S2 + the read-back
     bool pending = false;                                // a factorization whose flag has not been checked yet
     double pend_mu = 0.0, pend_tau = 0.0;
@@ -792,6 +808,7 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
             Emu = err_mu(mu);
         }
         const double tau = std::max(o.tau_min, 1.0 - mu);                      // S5
+        mark_iteration(it);
         if (graph) {                                     // S6-S10 and the next S2 as one graph replay
             uint32_t ef = 0, es = 0;
             TRY(next_epoch(h, true, &ef));
@@ -804,7 +821,7 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
             h->launches += 10;
             ++nfact;
             pending = true; pend_mu = mu; pend_tau = tau; top_done = true;
-            if (trace && it < trace_cap) { trace[it].mu = mu; trace[it].E0 = E0; trace[it].Emu = Emu; trace[it].eta = 0.0; trace[it].alpha_pr = trace[it].alpha_du = 0.0; }
+            if (trace && it < trace_cap) { trace[it] = nmpc_trace_row{}; trace[it].mu = mu; trace[it].E0 = E0; trace[it].Emu = Emu; }
             ++it;
             continue;
         }
@@ -833,13 +850,14 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
         }
         if (eta > 0.0) eta_last = eta;
         TRY(solve_step_update(mu, tau));
-        if (trace && it < trace_cap) { trace[it].mu = mu; trace[it].E0 = E0; trace[it].Emu = Emu; trace[it].eta = eta; trace[it].alpha_pr = trace[it].alpha_du = 0.0; }
+        if (trace && it < trace_cap) { trace[it] = nmpc_trace_row{}; trace[it].mu = mu; trace[it].E0 = E0; trace[it].Emu = Emu; trace[it].eta = eta; }
         ++it;
     }
 done:
     // z* is kept for the next warm start (Alg. 1 line 10) only if it is usable: converged, or stopped at max_iter with a finite
     // iterate.  After a non-finite iterate or an exhausted inertia schedule the next solve falls back to the cold start.
     h->have_state = status == NMPC_OK || (status == NMPC_E_MAXITER && hs[6] == 0.0);
+    mark_iteration(it);
     launch_objective(M, V, st); h->launches += 1;
     CK(cudaMemcpyAsync(hs + 9, V.scal + 9, sizeof(double), cudaMemcpyDeviceToHost, st));
     if (y_inout) CK(cudaMemcpyAsync(y_inout, V.y, sizeof(double) * M.n, cudaMemcpyDeviceToDevice, st));
@@ -847,6 +865,10 @@ done:
     CK(cudaGetLastError());
     S.status = status; S.iters = it; S.factorizations = nfact; S.eta_retries = retries; S.E0 = E0; S.mu = mu; S.eta_last = eta_last;
     S.objective = hs[9];
+    for (int k = 0; k < it && k + 1 < n_ev && k < trace_cap; ++k) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, h->it_ev[k], h->it_ev[k + 1]) == cudaSuccess) trace[k].ms_iter = ms; else cudaGetLastError();
+    }
     S.ms_total = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
     if (stats) *stats = S;
     return status;

@@ -32,6 +32,7 @@ constexpr int KC = 16;                  // k-columns per pipeline stage
 constexpr int ALD = 68;                 // leading dimension of an operand stage  (68 mod 16 == 4: conflict-free DMMA fragment loads)
 constexpr int CLD = 66;                 // leading dimension of the C / L_JJ tile (2*66 mod 16 == 4: conflict-free fragment stores)
 constexpr int NSTAGE = 4;
+constexpr int TCH = 128;                // children whose tables a tile task fetches at once
 constexpr int STAGE_DOUBLES = 2 * KC * ALD;
 constexpr int PIPE_DOUBLES = NSTAGE * STAGE_DOUBLES;          // 8704
 constexpr int CT_DOUBLES = TILE * CLD;                        // 4224
@@ -54,14 +55,21 @@ __device__ __forceinline__ void st_release(uint32_t* p, uint32_t v) {
 __device__ __forceinline__ void red_release_add(uint32_t* p, uint32_t v) {
     asm volatile("red.relaxed.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
+#ifdef NMPC_TRACE_BUILD                     // measurement build: timestamps per task + the time thread 0 spends waiting on flags
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+__shared__ unsigned long long s_wait_ns;
+#define TRACE(slot) do { if (tr && threadIdx.x == 0) { tr[slot] = gtime(); if ((slot) == 4) tr[6] = s_wait_ns; } } while (0)
+__device__ __forceinline__ void spin_until_ge(const uint32_t* p, uint32_t target) {
+    if (threadIdx.x != 0) { while (ld_acquire(p) < target) __nanosleep(40); return; }
+    const unsigned long long t0 = gtime();
+    while (ld_acquire(p) < target) __nanosleep(40);
+    s_wait_ns += gtime() - t0;
+}
+#else
+#define TRACE(slot) do { (void)tr; } while (0)
 __device__ __forceinline__ void spin_until_ge(const uint32_t* p, uint32_t target) {
     while (ld_acquire(p) < target) __nanosleep(40);
 }
-#ifdef NMPC_TRACE_BUILD
-__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
-#define TRACE(slot) do { if (tr && threadIdx.x == 0) tr[slot] = gtime(); } while (0)
-#else
-#define TRACE(slot) do { (void)tr; } while (0)
 #endif
 __device__ __forceinline__ void cp_async16(double* dst_smem, const double* src, int src_bytes) {
     const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
@@ -310,11 +318,25 @@ __device__ __forceinline__ void trsm_tile(double* Cs, double* Ls, double* rinv, 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gid = lane >> 2, tig = lane & 3;
     constexpr int NW = NT / 32;
     const int TU = (ni + 7) >> 3;
+    // a tile that is not right behind its POTRF finds L_JJ complete: one fetch of the whole triangle instead of one round trip
+    // to L2 per sub-step
+    __shared__ int s_all;
+    if (tid == 0) s_all = ld_acquire(sub) >= sbase + (uint32_t)((nj + 7) >> 3);
+    __syncthreads();
+    const bool all = s_all != 0;
+    if (all) {
+        for (int idx = tid; idx < nj * nj; idx += NT) {
+            const int cc = idx / nj, ii = idx - cc * nj;
+            if (ii >= cc) Ls[cc * CLD + ii] = __ldcg(Lg + ii + (int64_t)cc * ldg);
+        }
+        if (tid < nj) rinv[tid] = __ldcg(dinv_g + tid);
+        __syncthreads();
+    }
     for (int p0 = 0; p0 < nj; p0 += 32) {
         const int p1 = min(nj, p0 + 32);
         for (int j0 = p0; j0 < p1; j0 += 8) {
             const int jb = min(8, p1 - j0), t0 = j0 + jb;
-            {   // fetch columns [j0, j0 + jb) of L_JJ (rows j0 .. nj-1) and their pivot reciprocals
+            if (!all) {   // fetch columns [j0, j0 + jb) of L_JJ (rows j0 .. nj-1) and their pivot reciprocals
                 if (lane == 0) spin_until_ge(sub, sbase + (uint32_t)(j0 >> 3) + 1u);
                 __syncwarp();
                 const int nr = nj - j0;
@@ -589,20 +611,56 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
         __syncthreads();
         if (I == J && eta != 0.0) for (int nn = tid; nn < nj; nn += NT) Cs[nn * CLD + nn] += eta;
     }
-    for (int ci = ch0; ci < ch1; ++ci) {
-        const int c = D.child_idx[ci];
-        const int32_t* cb = F.cbnd + F.cb_ptr[c];
-        const int a0 = cb[I], a1 = cb[I + 1], b0 = cb[J], b1 = cb[J + 1];
-        if (a0 == a1 || b0 == b1) continue;              // uniform over the CTA
-        const int mc = (int)(D.rel_ptr[c + 1] - D.rel_ptr[c]);
-        const double* Uc = D.U + D.upd_ptr[c];
-        const int32_t* __restrict__ rel = D.rel + D.rel_ptr[c];
-        __syncthreads();
-        for (int b = b0 + warp; b < b1; b += nwarp) {
-            double* cc = Cs + (rel[b] - j0) * CLD - i0;
-            const double* ub = Uc + (int64_t)b * mc;
-            for (int a = max(a0, b) + lane; a < a1; a += 32) cc[rel[a]] += __ldcg(ub + a);
+    // Children's update matrices, in fixed child order (two children may add into the same entry).  The child tables (block
+    // boundaries inside this front, offsets) are fetched for up to TCH children at once, one child per thread, so the
+    // dependent index loads cost one round trip per batch instead of one per child; a child that meets the tile stages its
+    // <= 64 + 64 relative indices in shared memory and its <= 64 x 64 values are then loaded eight per thread in flight.
+    {
+        int* ctab = reinterpret_cast<int*>(pipe);                            // [TCH][4]: a0, a1, b0, b1
+        long long* cptr = reinterpret_cast<long long*>(pipe + TCH * 2);      // [TCH][3]: update offset, rel offset, rows of the update matrix
+        int* relA = reinterpret_cast<int*>(pipe + TCH * 5);                  // [64] row of the tile, [64] column offset in the tile
+        int* relB = relA + TILE;
+        for (int base = ch0; base < ch1; base += TCH) {
+            const int nbat = min(TCH, ch1 - base);
+            __syncthreads();
+            if (tid < nbat) {
+                const int c = D.child_idx[base + tid];
+                const int32_t* cb = F.cbnd + F.cb_ptr[c];
+                ctab[4 * tid] = cb[I]; ctab[4 * tid + 1] = cb[I + 1]; ctab[4 * tid + 2] = cb[J]; ctab[4 * tid + 3] = cb[J + 1];
+                const long long rp0 = D.rel_ptr[c];
+                cptr[3 * tid] = D.upd_ptr[c]; cptr[3 * tid + 1] = rp0; cptr[3 * tid + 2] = D.rel_ptr[c + 1] - rp0;
+            }
+            __syncthreads();
+            for (int k = 0; k < nbat; ++k) {
+                const int a0 = ctab[4 * k], a1 = ctab[4 * k + 1], b0 = ctab[4 * k + 2], b1 = ctab[4 * k + 3];
+                if (a0 == a1 || b0 == b1) continue;      // uniform over the CTA
+                const int na = a1 - a0, nb = b1 - b0;
+                const double* Uc = D.U + cptr[3 * k];
+                const int32_t* __restrict__ rel = D.rel + cptr[3 * k + 1];
+                const long long mc = cptr[3 * k + 2];
+                __syncthreads();                         // the previous child's additions are done, relA / relB are free
+                if (tid < na) relA[tid] = rel[a0 + tid] - i0;
+                else if (tid >= NT / 2 && tid - NT / 2 < nb) relB[tid - NT / 2] = (rel[b0 + tid - NT / 2] - j0) * CLD;
+                __syncthreads();
+                const int tot = na * nb;
+                for (int f0 = tid; f0 < tot; f0 += 8 * NT) {
+                    double v[8];
+                    int dst[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        const int f = f0 + e * NT;
+                        const int bb = f / na, aa = f - bb * na;
+                        const bool on = f < tot && a0 + aa >= b0 + bb;       // the child's update matrix is stored as a lower triangle
+                        v[e] = on ? __ldcg(Uc + (a0 + aa) + (long long)(b0 + bb) * mc) : 0.0;
+                        dst[e] = on ? relB[bb] + relA[aa] : -1;
+                    }
+#pragma unroll
+                    for (int e = 0; e < 8; ++e)
+                        if (dst[e] >= 0) Cs[dst[e]] += v[e];
+                }
+            }
         }
+        if (ch1 > ch0) __syncthreads();                  // the tables alias the operand ring the GEMM fills next
     }
     TRACE(1);
 
@@ -732,6 +790,7 @@ __global__ void __launch_bounds__(NT, 2) factor_dag_kernel(DevSym D, DagPlan F, 
         const int4 tk = F.ftasks[t];
 #ifdef NMPC_TRACE_BUILD
         unsigned long long* tr = F.ftrace ? F.ftrace + (size_t)t * 8 : nullptr;
+        if (threadIdx.x == 0) s_wait_ns = 0;
         if (tr && threadIdx.x == 0) { tr[0] = gtime(); unsigned sid; asm volatile("mov.u32 %0, %%smid;" : "=r"(sid)); tr[5] = sid; }
 #else
         unsigned long long* tr = nullptr;

@@ -45,6 +45,13 @@ def golden_path(name):
     return os.path.join(HERE, f"ipm_full_{name}.npz")
 
 
+def slim(d):
+    """Keep the full primal-dual iterate z* of the LAST solve only (y* of every solve stays): a third of the file size."""
+    last = int(d["n_solves"]) - 1
+    return {k: v for k, v in d.items()
+            if not any(k == f"{f}_{j}" for f in STATE_FIELDS[1:] for j in range(last))}
+
+
 def run(name, resolves, linsolve, log=print):
     cfg = make_config(name)
     t0 = time.perf_counter()
@@ -76,9 +83,12 @@ def main():
     ap.add_argument("--resolves", type=int, default=2)
     ap.add_argument("--linsolve", default=None)
     ap.add_argument("--out", default=None)
+    ap.add_argument("--states", default="all", choices=["all", "last"], help="which solves keep their full iterate z*")
     a = ap.parse_args()
     linsolve = a.linsolve or ("blocktri" if a.config in ("C2", "C3") else "sparse")
     d = run(a.config, a.resolves, linsolve)
+    if a.states == "last":
+        d = slim(d)
     path = a.out or golden_path(a.config)
     np.savez_compressed(path, **d)
     print(f"wrote {path} ({os.path.getsize(path) / 1e6:.1f} MB) in {float(d['wall_seconds']):.1f} s of oracle time")
