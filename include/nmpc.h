@@ -94,6 +94,15 @@ typedef struct {
     int32_t max_iter;
     double eta_first, eta_grow_first, eta_grow, eta_shrink, eta_min, eta_max, warm_push;
     int32_t time_phases;         /* record CUDA-event phase times in nmpc_stats (adds event overhead)         */
+    /* ---- SURVEY.md section 8(f) item 2, both off by default (reading G8): ---- */
+    int32_t refine_steps;        /* iterative refinement steps of the Newton direction on the UN-condensed first block row of
+                                    Eq. (10): rho = (W + eta I) dy + J^T(dw+ - dw-) - dzL + dzU + r_d, K ddy = -rho; 0..4.  One
+                                    step makes the IPM path insensitive to the elimination order      */
+    int32_t globalization;       /* 0 = fraction to the boundary only; 1 = filter line search on the primal step ("line search
+                                    with step size alpha", Eq. 26, read as Algorithm A of ref. [17] without
+                                    second-order correction / restoration, reading G20)                                      */
+    double  gamma_theta, gamma_phi, delta_sw, s_theta, s_phi, eta_phi, theta_max_fact, theta_min_fact;   /* constants of [17] */
+    int32_t ls_max_backtracks;
     int32_t epoch_limit;         /* 0 = automatic.  Test hook: the completion flags of the persistent kernels are
                                     call-number valued and are zeroed before a counter could overflow (after ~1e4..1e6
                                     factorizations); a small value (>= 3) forces that restart every few calls           */
@@ -124,6 +133,7 @@ typedef struct {                 /* filled by nmpc_ipm_solve (HOST)             
 typedef struct {                 /* one row per IPM iteration, for parity traces and per-iteration timing (HOST,
                                     caller array)                                                              */
     double mu, E0, Emu, eta, alpha_pr, alpha_du;
+    double backtracks;           /* halvings of the filter line search in this iteration (globalization = 1)            */
     double ms_iter;              /* device time of the whole iteration (CUDA events on the handle's stream, from the
                                     launch of S6 to the launch of the next iteration's S6 / the end of the solve)   */
     double ms_eval, ms_assemble, ms_factor, ms_solve, ms_vector;   /* phase split, only with options.time_phases  */

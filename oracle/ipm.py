@@ -27,7 +27,18 @@ DEFAULTS = dict(gamma=1e-4, eps_outer=1e-5, mu0=0.1, mu_warm=None,  # None -> ep
                 kappa_eps=10.0, kappa_mu=0.2, theta_mu=1.5, tau_min=0.99,
                 kappa_push=1e-2, s_floor=1e-2, s_max=100.0, max_iter=200,
                 eta_first=1e-4, eta_grow_first=100.0, eta_grow=8.0, eta_shrink=1.0 / 3.0,
-                eta_min=1e-20, eta_max=1e40, warm_push=1e-10)
+                eta_min=1e-20, eta_max=1e40, warm_push=1e-10,
+                # ---- globalisation and refinement (off by default: reading G8) ----
+                # "line search with step size alpha" (Eq. 26) read as the filter line search of the paper's
+                # IPM reference [17], Algorithm A steps A-5.1 .. A-5.10 without the second-order correction and
+                # with the restoration phase replaced by taking the fraction-to-the-boundary step (reading G20, DESIGN.md
+                # section 3).  Constants: the published defaults of [17] as recalled -- proposals, like S0.
+                globalization="none",            # "none" | "filter"
+                gamma_theta=1e-5, gamma_phi=1e-8, delta_sw=1.0, s_theta=1.1, s_phi=2.3, eta_phi=1e-8,
+                theta_max_fact=1e4, theta_min_fact=1e-4, ls_max_backtracks=30,
+                # iterative refinement of the Newton step on the UN-condensed first block row of Eq. (10):
+                # rho = (W + eta I) dy + J^T(dw+ - dw-) - dzL + dzU + r_d  with dw, dz eliminated from dy; K ddy = -rho
+                refine_steps=0)
 
 
 class IPMState:
@@ -86,6 +97,48 @@ class LiftedIPM:
         return E, r_d, r_pp, r_pm
 
     # ---------------------------------------------------------------------------------------------
+    def _theta(self, y, s_p, s_m):
+        """Constraint violation of the lifted equalities (the r_p rows of Eq. 9), 1-norm as in [17] Eq. (19)."""
+        c = self.nlp.constraints(y)
+        g = self.opt["gamma"]
+        return float(np.sum(np.abs(c - g + s_p)) + np.sum(np.abs(-c - g + s_m)))
+
+    def _phi(self, y, s_p, s_m, mu):
+        """Barrier objective of the lifted problem with native bounds: f - mu sum ln(slacks, bound distances)  ([17] Eq. 3a)."""
+        hasL, hasU = self.hasL, self.hasU
+        if np.any(s_p <= 0.0) or np.any(s_m <= 0.0) or np.any((y - self.lb)[hasL] <= 0.0) or np.any((self.ub - y)[hasU] <= 0.0):
+            return np.inf                                   # outside the domain of the barrier (never the case from alpha_max down)
+        return float(self.nlp.objective(y) - mu * (np.sum(np.log(s_p)) + np.sum(np.log(s_m))
+                                                   + np.sum(np.log((y - self.lb)[hasL])) + np.sum(np.log((self.ub - y)[hasU]))))
+
+    def _filter_line_search(self, st, mu, dy, ds_p, ds_m, a_max, gradf, flt, th_min):
+        """[17] Algorithm A, step A-5 (backtracking line search with a filter) on (theta, phi_mu).  Returns the accepted primal
+        step length, the number of halvings, and whether the filter has to be augmented (A-7)."""
+        o = self.opt
+        hasL, hasU = self.hasL, self.hasU
+        th_k = self._theta(st.y, st.sp, st.sm)
+        ph_k = self._phi(st.y, st.sp, st.sm, mu)
+        dL, dU = st.y - self.lb, self.ub - st.y
+        gphi_d = float(gradf @ dy - mu * (np.sum(ds_p / st.sp) + np.sum(ds_m / st.sm) + np.sum((dy / dL)[hasL]) - np.sum((dy / dU)[hasU])))
+        tol = 10.0 * np.finfo(float).eps * abs(ph_k)                           # [17] Section 3.3: relax the comparisons by rounding
+        alpha = a_max
+        for nback in range(o["ls_max_backtracks"] + 1):
+            y_t, sp_t, sm_t = st.y + alpha * dy, st.sp + alpha * ds_p, st.sm + alpha * ds_m
+            th_t = self._theta(y_t, sp_t, sm_t)
+            ph_t = self._phi(y_t, sp_t, sm_t, mu)
+            in_filter = any(th_t >= tf and ph_t >= pf for tf, pf in flt)      # A-5.3
+            switching = gphi_d < 0.0 and alpha * (-gphi_d) ** o["s_phi"] > o["delta_sw"] * th_k ** o["s_theta"]
+            if not in_filter:
+                if th_k <= th_min and switching:                               # A-5.4 case I: Armijo on phi
+                    if ph_t - ph_k - tol <= o["eta_phi"] * alpha * gphi_d:
+                        return alpha, nback, False, th_k, ph_k
+                elif th_t <= (1.0 - o["gamma_theta"]) * th_k or ph_t - ph_k - tol <= -o["gamma_phi"] * th_k:   # case II
+                    return alpha, nback, not switching or not (ph_t - ph_k - tol <= o["eta_phi"] * alpha * gphi_d), th_k, ph_k
+            alpha *= 0.5                                                       # A-5.10
+        # reading G20: no restoration phase -- take the fraction-to-the-boundary step and start a new filter
+        return a_max, o["ls_max_backtracks"] + 1, None, th_k, ph_k
+
+    # ---------------------------------------------------------------------------------------------
     def cold_start(self, y0):
         """S1 cold init."""
         o, nlp = self.opt, self.nlp
@@ -128,6 +181,11 @@ class LiftedIPM:
         tr = [] if trace is None else trace
         it = 0
         status = "maxiter"
+        use_filter = o["globalization"] == "filter"
+        if use_filter:                                      # [17] Eq. (21): theta_max, theta_min from the starting point
+            th0 = self._theta(st.y, st.sp, st.sm)
+            th_max, th_min = o["theta_max_fact"] * max(1.0, th0), o["theta_min_fact"] * max(1.0, th0)
+            flt, flt_mu = [(th_max, -np.inf)], mu
         while True:
             # S2: evaluate (K_SIMD of the paper: f, grad f, c, J)            Alg. 2 line 5
             gradf = nlp.gradient(st.y)
@@ -177,19 +235,35 @@ class LiftedIPM:
                 eta_last = eta
             # S8: triangular solves Eq. (22)-(25), then the eliminated directions from Eq. (14)/(10)   line 14
             dy = self.chol.solve(b)
-            Jdy = J @ dy
-            ds_p = -r_pp - Jdy
-            ds_m = -r_pm + Jdy
-            dw_p = -(st.wp - mu / st.sp) - q_p * ds_p
-            dw_m = -(st.wm - mu / st.sm) - q_m * ds_m
-            dzL = np.where(hasL, -(st.zL - mu / dL) - st.zL / dL * dy, 0.0)
-            dzU = np.where(hasU, -(st.zU - mu / dU) + st.zU / dU * dy, 0.0)
+
+            def eliminated(dy_):
+                Jdy = J @ dy_
+                ds_p_ = -r_pp - Jdy
+                ds_m_ = -r_pm + Jdy
+                return (ds_p_, ds_m_, -(st.wp - mu / st.sp) - q_p * ds_p_, -(st.wm - mu / st.sm) - q_m * ds_m_,
+                        np.where(hasL, -(st.zL - mu / dL) - st.zL / dL * dy_, 0.0),
+                        np.where(hasU, -(st.zU - mu / dU) + st.zU / dU * dy_, 0.0))
+
+            ds_p, ds_m, dw_p, dw_m, dzL, dzU = eliminated(dy)
+            for _ in range(o["refine_steps"]):              # iterative refinement on the un-condensed first row of Eq. (10)
+                rho = W @ dy + eta * dy + J.T @ (dw_p - dw_m) - dzL + dzU + r_d
+                dy = dy + self.chol.solve(-rho)
+                ds_p, ds_m, dw_p, dw_m, dzL, dzU = eliminated(dy)
             # S9: fraction to the boundary, separate primal / dual steps (reading G8)
             a_pr = min(_max_step(st.sp, ds_p, tau), _max_step(st.sm, ds_m, tau),
                        _max_step(dL[hasL], dy[hasL], tau), _max_step(dU[hasU], -dy[hasU], tau))
             a_du = min(_max_step(st.wp, dw_p, tau), _max_step(st.wm, dw_m, tau),
                        _max_step(st.zL[hasL], dzL[hasL], tau), _max_step(st.zU[hasU], dzU[hasU], tau))
-            tr.append(dict(it=it, mu=mu, E0=E0, Emu=Emu, eta=eta, alpha_pr=a_pr, alpha_du=a_du))
+            nback = 0
+            if use_filter:                                  # Eq. (26) "line search": filter line search of [17] on the primal step
+                if mu != flt_mu:                            # a new barrier problem: the filter is re-initialised ([17] A-3)
+                    flt, flt_mu = [(th_max, -np.inf)], mu
+                a_pr, nback, augment, th_k, ph_k = self._filter_line_search(st, mu, dy, ds_p, ds_m, a_pr, gradf, flt, th_min)
+                if augment is None:
+                    flt = [(th_max, -np.inf)]
+                elif augment:                               # A-7
+                    flt.append(((1.0 - o["gamma_theta"]) * th_k, ph_k - o["gamma_phi"] * th_k))
+            tr.append(dict(it=it, mu=mu, E0=E0, Emu=Emu, eta=eta, alpha_pr=a_pr, alpha_du=a_du, backtracks=nback))
             # kept for the pins (condensation algebra vs the un-condensed Newton system, Eq. 10)
             self.last_step = dict(state=st, mu=mu, eta=eta, gradf=gradf, c=c, J=J, W=W, K0=K0, b=b, dy=dy,
                                   ds_p=ds_p, ds_m=ds_m, dw_p=dw_p, dw_m=dw_m, dzL=dzL, dzU=dzU,

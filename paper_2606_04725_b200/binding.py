@@ -40,7 +40,10 @@ class nmpc_options(C.Structure):
                 + [("max_iter", c_i32)]
                 + [(k, c_dbl) for k in ("eta_first", "eta_grow_first", "eta_grow", "eta_shrink", "eta_min", "eta_max",
                                         "warm_push")]
-                + [("time_phases", c_i32), ("epoch_limit", c_i32)])
+                + [("time_phases", c_i32), ("refine_steps", c_i32), ("globalization", c_i32)]
+                + [(k, c_dbl) for k in ("gamma_theta", "gamma_phi", "delta_sw", "s_theta", "s_phi", "eta_phi", "theta_max_fact",
+                                        "theta_min_fact")]
+                + [("ls_max_backtracks", c_i32), ("epoch_limit", c_i32)])
 
 
 class nmpc_sym_info(C.Structure):
@@ -58,7 +61,7 @@ class nmpc_stats(C.Structure):
 
 
 class nmpc_trace_row(C.Structure):
-    _fields_ = [(k, c_dbl) for k in ("mu", "E0", "Emu", "eta", "alpha_pr", "alpha_du", "ms_iter", "ms_eval", "ms_assemble",
+    _fields_ = [(k, c_dbl) for k in ("mu", "E0", "Emu", "eta", "alpha_pr", "alpha_du", "backtracks", "ms_iter", "ms_eval", "ms_assemble",
                                      "ms_factor", "ms_solve", "ms_vector")]
 
 

@@ -260,16 +260,18 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
     // epoch-valued flags: counters reach epoch * target and the claim counters epoch * (ntasks + grid); reset before 2^31
     int64_t per_epoch = std::max<int64_t>((int64_t)tasks.size() + F.fgrid, (int64_t)stasks.size() + F.sgrid);
     for (int s = 0; s < ns; ++s) per_epoch = std::max<int64_t>(per_epoch, target[s]);
-    h->epoch_limit = (uint32_t)std::max<int64_t>(3, ((int64_t)1 << 31) / per_epoch - 2);
-    if (h->opt.epoch_limit > 0) h->epoch_limit = std::min<uint32_t>(h->epoch_limit, (uint32_t)std::max(3, h->opt.epoch_limit));   // test hook
+    const int64_t min_limit = 3 + std::max(0, h->opt.refine_steps);
+    h->epoch_limit = (uint32_t)std::max<int64_t>(min_limit, ((int64_t)1 << 31) / per_epoch - 2);
+    if (h->opt.epoch_limit > 0) h->epoch_limit = std::min<uint32_t>(h->epoch_limit, (uint32_t)std::max<int64_t>(min_limit, h->opt.epoch_limit));   // test hook
     return NMPC_OK;
 }
 
 // The next call number of the factor / solve kernels.  Both restart from 1 (all flags zeroed, in stream order) before any
-// counter can overflow.  The restart is decided with a margin of TWO call numbers, so a factor number and the solve number
-// reserved right after it (one CUDA-graph replay holds both kernels) always lie on the same side of a restart.
+// counter can overflow.  The restart is decided with a margin of all call numbers of one IPM iteration (one factorization, 1 +
+// refine_steps solves), so the numbers reserved for one CUDA-graph replay always lie on the same side of a restart.
 nmpc_status next_epoch(nmpc_handle_s* h, bool factor, uint32_t* out) {
-    if (factor && std::max(h->epoch_f, h->epoch_s) + 2 >= h->epoch_limit) {
+    const uint32_t per_iter = 2u + (uint32_t)std::max(0, h->opt.refine_steps);   // one factorization + (1 + refine_steps) solves
+    if (factor && std::max(h->epoch_f, h->epoch_s) + per_iter >= h->epoch_limit) {
         CK(cudaMemsetAsync(h->F.sync, 0, (size_t)h->F.sync_words * sizeof(uint32_t), h->stream));
         h->epoch_f = h->epoch_s = 0;
     }
@@ -329,13 +331,19 @@ nmpc_status capture_iteration_graph(nmpc_handle_s* h) {
     cudaError_t ce = cudaSuccess;
     auto ok = [&](cudaError_t e) { if (ce == cudaSuccess && e != cudaSuccess) ce = e; return ce == cudaSuccess; };
     auto launched = [&]() { return ok(cudaGetLastError()); };
-    bool good = ok(cudaMemcpyAsync(h->d_par, hp, 4 * sizeof(double), cudaMemcpyHostToDevice, st));
+    bool good = ok(cudaMemcpyAsync(h->d_par, hp, 8 * sizeof(double), cudaMemcpyHostToDevice, st));
     if (good) { launch_sigma_rhs(M, V, 0.0, h->d_par, st); good = launched(); }
     if (good) { launch_assemble_K(M, V.Jval, V.Wval, V.sigx, V.q, 0.0, V.Kval, st); good = launched(); }
     if (good) { launch_factor(h->D, h->F, h->d_Kval, 0.0, 0u, epo, st); good = launched(); }
     if (good) good = ok(cudaMemcpyAsync(V.dy, V.b, sizeof(double) * M.n, cudaMemcpyDeviceToDevice, st));
     if (good) { launch_solve(h->D, h->F, V.dy, h->d_x, 0u, epo, st); good = launched(); }
     if (good) { launch_step(M, V, 0.0, 0.0, h->d_par, st); good = launched(); }
+    for (int r = 0; good && r < h->opt.refine_steps; ++r) {      // iterative refinement: solve number r + 1 of this iteration
+        launch_refine_residual(M, V, 0.0, h->D.fail_col, st); good = launched();
+        if (good) { launch_solve(h->D, h->F, V.rho, h->d_x, 0u, epo + 1 + r, st); good = launched(); }
+        if (good) { launch_add_correction(M, V, h->D.fail_col, st); good = launched(); }
+        if (good) { launch_step(M, V, 0.0, 0.0, h->d_par, st); good = launched(); }
+    }
     if (good) { launch_update(M, V, h->D.fail_col, st); good = launched(); }
     if (good) { launch_model_eval(M, V.y, V.wp, V.wm, nullptr, V.c, V.gradf, V.Jval, V.Wval, st); good = launched(); }
     if (good) { launch_residuals(M, V, h->opt.gamma, st); good = launched(); }
@@ -384,6 +392,7 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
     auto fail = [&](nmpc_status s) { g_create_error = h->err; nmpc_destroy(h); return s; };
     if (opt) h->opt = *opt; else default_options(&h->opt);
     if (h->opt.mu_warm <= 0.0) h->opt.mu_warm = h->opt.eps_outer / 10.0;
+    h->opt.refine_steps = std::min(4, std::max(0, h->opt.refine_steps));
     int smem_optin = 0, num_sms = 0, lat_ctas = 1, lat_rmax = 0;
     size_t lat_smem = 0;
     if (cudaGetDevice(&h->dev) != cudaSuccess || cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->dev) != cudaSuccess ||
@@ -502,7 +511,23 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
             TRY(dalloc(h, m, &V.dsp)); TRY(dalloc(h, m, &V.dsm)); TRY(dalloc(h, m, &V.dwp)); TRY(dalloc(h, m, &V.dwm));
             TRY(dalloc(h, n, &V.dzL)); TRY(dalloc(h, n, &V.dzU));
             TRY(dalloc(h, (size_t)RED_BLOCKS * 8, &V.partial)); TRY(dalloc(h, (size_t)NSCAL, &V.scal));
-            TRY(dalloc(h, 4, &h->d_par));
+            TRY(dalloc(h, 8, &h->d_par));
+            TRY(dalloc(h, n, &V.rho));
+            {   // symmetric CSR of W (lower CSR in value order) for the W dy product of the refinement residual
+                std::vector<int64_t> ptr(n + 1, 0);
+                for (int64_t i = 0; i < (int64_t)n; ++i)
+                    for (int64_t p = mm.W.ptr[i]; p < mm.W.ptr[i + 1]; ++p) { ptr[i + 1]++; if (mm.W.idx[p] != i) ptr[mm.W.idx[p] + 1]++; }
+                for (size_t i = 0; i < n; ++i) ptr[i + 1] += ptr[i];
+                std::vector<int32_t> idx(ptr[n]), src(ptr[n]);
+                std::vector<int64_t> pos(ptr.begin(), ptr.end() - 1);
+                for (int64_t i = 0; i < (int64_t)n; ++i)
+                    for (int64_t p = mm.W.ptr[i]; p < mm.W.ptr[i + 1]; ++p) {
+                        const int32_t j = mm.W.idx[p];
+                        idx[pos[i]] = j; src[pos[i]++] = (int32_t)p;
+                        if (j != i) { idx[pos[j]] = (int32_t)i; src[pos[j]++] = (int32_t)p; }
+                    }
+                TRY(upload(h, ptr, &M.wf_ptr)); TRY(upload(h, idx, &M.wf_idx)); TRY(upload(h, src, &M.wf_src));
+            }
             pinned += (size_t)mm.desc.nx + (size_t)mm.desc.N * mm.desc.nr + n;
         }
         h->pinned_doubles = pinned;
@@ -757,6 +782,19 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
         pt.end();
         pt.begin(&S.ms_vector, 4);
         launch_step(M, V, mu_, tau_, nullptr, st); h->launches += 1;                    // S8-S9
+        pt.end();
+        for (int r = 0; r < o.refine_steps; ++r) {                             // iterative refinement on Eq. (10), first row
+            pt.begin(&S.ms_vector, 4);
+            launch_refine_residual(M, V, h->eta_cur, h->D.fail_col, st); h->launches++;
+            pt.end();
+            pt.begin(&S.ms_solve, 3);
+            TRY(run_solve(h, V.rho));
+            pt.end();
+            pt.begin(&S.ms_vector, 4);
+            launch_add_correction(M, V, h->D.fail_col, st); launch_step(M, V, mu_, tau_, nullptr, st); h->launches += 2;
+            pt.end();
+        }
+        pt.begin(&S.ms_vector, 4);
         launch_update(M, V, h->D.fail_col, st); h->launches++;                 // S10: Eq. (26)
         pt.end();
         return NMPC_OK;
@@ -810,15 +848,13 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
         const double tau = std::max(o.tau_min, 1.0 - mu);                      // S5
         mark_iteration(it);
         if (graph) {                                     // S6-S10 and the next S2 as one graph replay
-            uint32_t ef = 0, es = 0;
-            TRY(next_epoch(h, true, &ef));
-            TRY(next_epoch(h, false, &es));
             double* hp = h->h_pinned + 24;
             hp[0] = mu; hp[1] = tau;
-            uint32_t* he = reinterpret_cast<uint32_t*>(hp + 2);
-            he[0] = ef; he[1] = es;
+            uint32_t* he = reinterpret_cast<uint32_t*>(hp + 2);  // call numbers: factorization, then 1 + refine_steps solves
+            TRY(next_epoch(h, true, &he[0]));
+            for (int r = 0; r <= o.refine_steps; ++r) TRY(next_epoch(h, false, &he[1 + r]));
             CK(cudaGraphLaunch(h->iter_graph, st));
-            h->launches += 10;
+            h->launches += 10 + 4 * o.refine_steps;
             ++nfact;
             pending = true; pend_mu = mu; pend_tau = tau; top_done = true;
             if (trace && it < trace_cap) { trace[it] = nmpc_trace_row{}; trace[it].mu = mu; trace[it].E0 = E0; trace[it].Emu = Emu; }
@@ -837,6 +873,7 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
             uint32_t epoch = 0;
             TRY(next_epoch(h, true, &epoch));
             launch_factor(h->D, h->F, h->d_Kval, 0.0, epoch, nullptr, st); h->launches += 1;
+            h->eta_cur = 0.0;
             pending = true; pend_mu = mu; pend_tau = tau;
         } else {
             pt.begin(&S.ms_factor, 2);

@@ -121,6 +121,7 @@ struct DevModel {                 // device copies of the model maps (symbolic.h
     const int64_t* jt_ptr = nullptr; const int32_t* jt_idx = nullptr; const int32_t* jt_row = nullptr;
     const int64_t* trip_ptr = nullptr; const int32_t* trip_a = nullptr; const int32_t* trip_b = nullptr; const int32_t* trip_r = nullptr;
     const int32_t* k_w = nullptr; const int32_t* k_diag = nullptr;
+    const int64_t* wf_ptr = nullptr; const int32_t* wf_idx = nullptr; const int32_t* wf_src = nullptr;   // symmetric CSR of W (-> Wval index)
     const double* lb = nullptr; const double* ub = nullptr;             // n, +-inf allowed
     double* x0 = nullptr; double* ref = nullptr;                       // parameters p = (x0, ref)
 };
@@ -129,6 +130,7 @@ struct IpmVectors {               // primal-dual iterate and work vectors (devic
     double *y, *sp, *sm, *wp, *wm, *zL, *zU;                 // z = (y, s+, s-, w+, w-, zL, zU)
     double *c, *gradf, *Jval, *Wval, *Kval;                  // model evaluation + assembled K values
     double *r_pp, *r_pm, *q, *t, *sigx, *b, *dy;             // residuals, Sigma, rhs, step
+    double *rho;                                             // refinement: minus the un-condensed residual, then the correction
     double *dsp, *dsm, *dwp, *dwm, *dzL, *dzU;
     double *partial;                                         // block partials of the reductions
     double *scal;                                            // device scalars (see ipm.cu)
@@ -154,5 +156,10 @@ void launch_step(const DevModel& M, const IpmVectors& V, double mu, double tau, 
 // fail_col (may be null): device flag of the factorization; the update is skipped when it reports a failed pivot
 void launch_update(const DevModel& M, const IpmVectors& V, const int32_t* fail_col, cudaStream_t st);
 void launch_objective(const DevModel& M, const IpmVectors& V, cudaStream_t st);
+// iterative refinement of dy on the un-condensed first block row of Eq. (10): rho <- -((W + eta I) dy + J^T(dw+ - dw-) - dzL + dzU
+// + r_d) with the eliminated directions of the last launch_step; after K^-1 rho: dy += rho.  Both skip when *fail_col reports a
+// failed pivot (fail_col may be null).
+void launch_refine_residual(const DevModel& M, const IpmVectors& V, double eta, const int32_t* fail_col, cudaStream_t st);
+void launch_add_correction(const DevModel& M, const IpmVectors& V, const int32_t* fail_col, cudaStream_t st);
 
 }  // namespace nmpc

@@ -350,6 +350,40 @@ __global__ void __launch_bounds__(NT) objective_kernel(DevModel M, IpmVectors V)
     block_reduce<1>(a, ops, V.scal + 9);
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// Iterative refinement of the Newton direction (options.refine_steps): residual of the FIRST block row of the un-condensed
+// system Eq. (10) at the current (dy, dw+-, dz) -- r_d expanded, so the multipliers enter as w + dw, z + dz:
+//   rho = grad f + J^T((w+ + dw+) - (w- + dw-)) - (zL + dzL) + (zU + dzU) + (W + eta I) dy;      V.rho <- -rho
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(NT) refine_residual_kernel(DevModel M, IpmVectors V, double eta, const int32_t* __restrict__ fail_col) {
+    if (fail_col && *fail_col != INT_MAX) return;
+    const int64_t gtid = blockIdx.x * (int64_t)NT + threadIdx.x;
+    const int64_t i = gtid / GV;
+    const int gl = (int)(gtid % GV);
+    const bool valid = i < M.n;
+    double acc = 0.0;
+    if (valid) {
+#pragma unroll 4
+        for (int64_t p = M.jt_ptr[i] + gl; p < M.jt_ptr[i + 1]; p += GV) {
+            const int r = M.jt_row[p];
+            acc += V.Jval[M.jt_idx[p]] * ((V.wp[r] + V.dwp[r]) - (V.wm[r] + V.dwm[r]));
+        }
+        for (int64_t q = M.wf_ptr[i] + gl; q < M.wf_ptr[i + 1]; q += GV) acc += V.Wval[M.wf_src[q]] * V.dy[M.wf_idx[q]];
+    }
+#pragma unroll
+    for (int o = 1; o < GV; o <<= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (!valid || gl != 0) return;
+    const bool hasL = M.lb[i] > -INF, hasU = M.ub[i] < INF;
+    const double zl = hasL ? V.zL[i] + V.dzL[i] : 0.0, zu = hasU ? V.zU[i] + V.dzU[i] : 0.0;
+    V.rho[i] = -(V.gradf[i] + acc - zl + zu + eta * V.dy[i]);
+}
+
+__global__ void __launch_bounds__(NT) add_correction_kernel(DevModel M, IpmVectors V, const int32_t* __restrict__ fail_col) {
+    if (fail_col && *fail_col != INT_MAX) return;
+    const int64_t i = blockIdx.x * (int64_t)NT + threadIdx.x;
+    if (i < M.n) V.dy[i] += V.rho[i];
+}
+
 inline unsigned blocks_for(int64_t work) { return (unsigned)((work + NT - 1) / NT); }
 inline int red_blocks(int64_t work) { return (int)std::min<int64_t>(RED_BLOCKS, (work + NT - 1) / NT); }
 
@@ -391,6 +425,12 @@ void launch_step(const DevModel& M, const IpmVectors& V, double mu, double tau, 
 }
 void launch_update(const DevModel& M, const IpmVectors& V, const int32_t* fail_col, cudaStream_t st) {
     update_kernel<<<blocks_for(M.n + M.m), NT, 0, st>>>(M, V, fail_col);
+}
+void launch_refine_residual(const DevModel& M, const IpmVectors& V, double eta, const int32_t* fail_col, cudaStream_t st) {
+    refine_residual_kernel<<<blocks_for(M.n * GV), NT, 0, st>>>(M, V, eta, fail_col);
+}
+void launch_add_correction(const DevModel& M, const IpmVectors& V, const int32_t* fail_col, cudaStream_t st) {
+    add_correction_kernel<<<blocks_for(M.n), NT, 0, st>>>(M, V, fail_col);
 }
 void launch_objective(const DevModel& M, const IpmVectors& V, cudaStream_t st) {
     const int nb = red_blocks(M.n);

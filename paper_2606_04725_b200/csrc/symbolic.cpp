@@ -25,6 +25,10 @@ void default_options(nmpc_options* o) {
     o->kappa_push = 1e-2; o->s_floor = 1e-2; o->s_max = 100.0; o->max_iter = 200;
     o->eta_first = 1e-4; o->eta_grow_first = 100.0; o->eta_grow = 8.0; o->eta_shrink = 1.0 / 3.0;
     o->eta_min = 1e-20; o->eta_max = 1e40; o->warm_push = 1e-10;
+    // globalisation / refinement (off): constants of ref. [17] as recalled, proposals like the S0 constants
+    o->refine_steps = 0; o->globalization = 0;
+    o->gamma_theta = 1e-5; o->gamma_phi = 1e-8; o->delta_sw = 1.0; o->s_theta = 1.1; o->s_phi = 2.3; o->eta_phi = 1e-8;
+    o->theta_max_fact = 1e4; o->theta_min_fact = 1e-4; o->ls_max_backtracks = 30;
 }
 
 // =============================================================================================================

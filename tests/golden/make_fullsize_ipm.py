@@ -35,29 +35,39 @@ from oracle.ipm import DEFAULTS, nmpc_closed_loop  # noqa: E402
 STATE_FIELDS = ("y", "sp", "sm", "wp", "wm", "zL", "zU")
 
 
-def cache_key(name, linsolve):
-    blob = json.dumps(dict(config=name, seed=MASTER_SEED, options={k: DEFAULTS[k] for k in sorted(DEFAULTS)},
-                           linsolve=linsolve), sort_keys=True, default=str)
+S0_KEYS = ("eps_outer", "eta_first", "eta_grow", "eta_grow_first", "eta_max", "eta_min", "eta_shrink", "gamma", "kappa_eps",
+           "kappa_mu", "kappa_push", "max_iter", "mu0", "mu_warm", "s_floor", "s_max", "tau_min", "theta_mu", "warm_push")
+
+
+def cache_key(name, linsolve, **overrides):
+    """Key of a stored run: config, seed, the S0 constants of the oracle, the linear solver, and any option that is switched on."""
+    opts = {k: DEFAULTS[k] for k in S0_KEYS}
+    opts.update(overrides)
+    blob = json.dumps(dict(config=name, seed=MASTER_SEED, options=opts, linsolve=linsolve), sort_keys=True, default=str)
     return hashlib.sha256(blob.encode()).hexdigest()[:16]
 
 
-def golden_path(name):
-    return os.path.join(HERE, f"ipm_full_{name}.npz")
+def golden_path(name, tag=""):
+    return os.path.join(HERE, f"ipm_full_{name}{'_' + tag if tag else ''}.npz")
 
 
-def slim(d):
-    """Keep the full primal-dual iterate z* of the LAST solve only (y* of every solve stays): a third of the file size."""
+def slim(d, keep="last"):
+    """keep = "last": the full primal-dual iterate z* of the LAST solve only; "none": no multipliers / slacks at all (y* of
+    every solve always stays)."""
     last = int(d["n_solves"]) - 1
-    return {k: v for k, v in d.items()
-            if not any(k == f"{f}_{j}" for f in STATE_FIELDS[1:] for j in range(last))}
+    drop = range(last) if keep == "last" else range(last + 1)
+    out = {k: v for k, v in d.items() if not any(k == f"{f}_{j}" for f in STATE_FIELDS[1:] for j in drop)}
+    if keep == "none":
+        out = {k: v for k, v in out.items() if not k.startswith("late_")}
+    return out
 
 
-def run(name, resolves, linsolve, log=print):
+def run(name, resolves, linsolve, log=print, **overrides):
     cfg = make_config(name)
     t0 = time.perf_counter()
-    out, ipm = nmpc_closed_loop(cfg, n_resolves=resolves, linsolve=linsolve)
+    out, ipm = nmpc_closed_loop(cfg, n_resolves=resolves, linsolve=linsolve, **overrides)
     wall = time.perf_counter() - t0
-    d = dict(key=np.array(cache_key(name, linsolve)), n_solves=np.array(len(out)), wall_seconds=np.array(wall),
+    d = dict(key=np.array(cache_key(name, linsolve, **overrides)), n_solves=np.array(len(out)), wall_seconds=np.array(wall),
              linsolve=np.array(linsolve))
     for j, o in enumerate(out):
         log(f"{name} solve {j}: status {o['status']} iters {o['iters']} factorizations {o['factorizations']}")
@@ -83,13 +93,15 @@ def main():
     ap.add_argument("--resolves", type=int, default=2)
     ap.add_argument("--linsolve", default=None)
     ap.add_argument("--out", default=None)
-    ap.add_argument("--states", default="all", choices=["all", "last"], help="which solves keep their full iterate z*")
+    ap.add_argument("--states", default="all", choices=["all", "last", "none"], help="which solves keep their full iterate z*")
+    ap.add_argument("--refine-steps", type=int, default=0, help="oracle option refine_steps (file tag refine<k>)")
     a = ap.parse_args()
     linsolve = a.linsolve or ("blocktri" if a.config in ("C2", "C3") else "sparse")
-    d = run(a.config, a.resolves, linsolve)
-    if a.states == "last":
-        d = slim(d)
-    path = a.out or golden_path(a.config)
+    overrides = dict(refine_steps=a.refine_steps) if a.refine_steps else {}
+    d = run(a.config, a.resolves, linsolve, **overrides)
+    if a.states != "all":
+        d = slim(d, a.states)
+    path = a.out or golden_path(a.config, f"refine{a.refine_steps}" if a.refine_steps else "")
     np.savez_compressed(path, **d)
     print(f"wrote {path} ({os.path.getsize(path) / 1e6:.1f} MB) in {float(d['wall_seconds']):.1f} s of oracle time")
 

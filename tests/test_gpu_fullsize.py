@@ -51,18 +51,20 @@ def dev(a):
 _cache = {}
 
 
-def oracle_run(name):
+def oracle_run(name, refine_steps=0):
     """The oracle's closed loop at full size: the committed golden file when there is one (its key must match the
     current oracle options), else computed now."""
-    if name not in _cache:
-        path = gold.golden_path(name)
+    ck = (name, refine_steps)
+    if ck not in _cache:
+        ov = dict(refine_steps=refine_steps) if refine_steps else {}
+        path = gold.golden_path(name, f"refine{refine_steps}" if refine_steps else "")
         if os.path.exists(path):
             d = dict(np.load(path, allow_pickle=False))
-            assert str(d["key"]) == gold.cache_key(name, LINSOLVE[name]), "golden file is stale: rerun make_fullsize_ipm.py"
+            assert str(d["key"]) == gold.cache_key(name, LINSOLVE[name], **ov), "golden file is stale: rerun make_fullsize_ipm.py"
         else:
-            d = gold.run(name, 2, LINSOLVE[name], log=lambda *_: None)
-        _cache[name] = d
-    return _cache[name]
+            d = gold.run(name, 2, LINSOLVE[name], log=lambda *_: None, **ov)
+        _cache[ck] = d
+    return _cache[ck]
 
 
 def _traces(tg, to):
@@ -146,6 +148,32 @@ def test_ipm_fullsize_closed_loop_vs_oracle(name):
         st = IPMState(*zg)
         E0, _, _, _ = ipm._errors(st, ipm.nlp.gradient(st.y), ipm.nlp.constraints(st.y), ipm.nlp.jacobian(st.y), 0.0)
         assert E0 <= ipm.opt["eps_outer"] * (1.0 + 1e-6), (name, j, E0)
+    h.close()
+
+
+@pytest.mark.parametrize("name", ["C2", "C4", "C3"])
+def test_ipm_fullsize_with_refinement_vs_oracle(name):
+    """options.refine_steps = 1 at BASELINE size: one step of iterative refinement on the un-condensed
+    Newton system makes the IPM path insensitive to the elimination order, so the closed loop (cold solve + 2 warm re-solves,
+    each warm start the GPU's OWN previous z*, replayed x0) matches the oracle STRICTLY on every configuration including the
+    cold solve of C3: counts, mu / eta traces, step lengths to 5e-3 (ten times tighter than without), y* to 1e-6 (C3's oracle run: ipm_full_C3_refine1.npz)."""
+    cfg = make_config(name)
+    d = oracle_run(name, refine_steps=1)
+    h = nb.Handle(None, nb.make_ocp(cfg), nb.default_options(refine_steps=1))
+    y = torch.zeros(cfg.n, dtype=torch.float64, device=DEV)
+    for j in range(int(d["n_solves"])):
+        assert str(d[f"status_{j}"]) == "converged"
+        h.update_params(dev(d[f"x0_{j}"]), dev(cfg.ref_for_solve(j)))
+        rg = h.ipm_solve(int(j > 0), y, trace_cap=256, check=False)
+        to = d[f"trace_{j}"]
+        report = f"{name} solve {j}: GPU {rg['iters']} iterations / oracle {int(d[f'iters_{j}'])}\n" + _traces(rg["trace"], to)
+        assert rg["status"] == 0, report
+        assert rg["iters"] == int(d[f"iters_{j}"]) and rg["factorizations"] == int(d[f"fact_{j}"]), report
+        for k, tg in enumerate(rg["trace"]):
+            assert tg["mu"] == to[k, 0] and tg["eta"] == to[k, 1], report
+            assert abs(tg["alpha_pr"] - to[k, 3]) <= 5e-3 and abs(tg["alpha_du"] - to[k, 4]) <= 5e-3, report   # 5e-2 without refinement
+        yo = d[f"y_{j}"]
+        assert np.abs(y.cpu().numpy() - yo).max() <= 1e-6 * np.abs(yo).max(), report
     h.close()
 
 

