@@ -512,7 +512,7 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
             TRY(dalloc(h, n, &V.dzL)); TRY(dalloc(h, n, &V.dzU));
             TRY(dalloc(h, (size_t)RED_BLOCKS * 8, &V.partial)); TRY(dalloc(h, (size_t)NSCAL, &V.scal));
             TRY(dalloc(h, 8, &h->d_par));
-            TRY(dalloc(h, n, &V.rho));
+            TRY(dalloc(h, n, &V.rho)); TRY(dalloc(h, n, &V.yt)); TRY(dalloc(h, m, &V.ct));
             {   // symmetric CSR of W (lower CSR in value order) for the W dy product of the refinement residual
                 std::vector<int64_t> ptr(n + 1, 0);
                 for (int64_t i = 0; i < (int64_t)n; ++i)
@@ -747,7 +747,7 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
     // step and the (device-guarded) update are enqueued behind it and the flag travels with the next iteration's residual
     // scalars -- one host synchronisation per IPM iteration.  A failed pivot leaves the iterate untouched (update_kernel
     // checks the flag), so the inertia-correction retry below starts from exactly the state of the synchronous flow.
-    const bool async = !o.time_phases;
+    const bool async = !o.time_phases && !o.globalization;   // the line search reads merit values back: synchronous flow
     if (async && o.use_graph && !h->iter_graph && !h->graph_failed) TRY(capture_iteration_graph(h));
     const bool graph = async && o.use_graph && h->iter_graph != nullptr;
     // traced solves: one CUDA event per iteration, recorded (no synchronisation) right before the iteration's S6 is launched
@@ -775,6 +775,60 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
             if (fs != NMPC_E_NOT_SPD) return fs;
         }
     };
+    // ---- filter line search on the primal step (options.globalization; ref. [17] Algorithm A, steps A-5.1 .. A-5.10 and A-7,
+    //      reading G20 of DESIGN.md section 3): theta and phi_mu of the trial points are reduced on the device, the filter
+    //      (a short list of pairs) and the acceptance tests are host scalars ----
+    std::vector<std::pair<double, double>> flt;
+    double th_max = 0.0, th_min = 0.0, flt_mu = -1.0;
+    bool flt_ready = false;
+    int last_backtracks = 0;
+    double* hm = h->h_pinned + 40;                        // pinned: merit scalars [0..4], step lengths [5..6], accepted alpha [7]
+    struct Merit { double theta, phi, g; };
+    auto merit_at = [&](double alpha, double mu_, int with_grad, Merit& out) -> nmpc_status {
+        launch_trial_point(M, V, alpha, st);
+        launch_model_eval(M, V.yt, nullptr, nullptr, nullptr, V.ct, nullptr, nullptr, nullptr, st);
+        launch_merit(M, V, alpha, mu_, o.gamma, with_grad, st);
+        h->launches += 3;
+        CK(cudaMemcpyAsync(hm, V.scal, 5 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        if (with_grad) CK(cudaMemcpyAsync(hm + 5, V.scal + 7, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        out.theta = hm[0]; out.phi = hm[3] > 0.0 ? INFINITY : hm[2] - mu_ * hm[1]; out.g = hm[4];
+        return NMPC_OK;
+    };
+    auto filter_line_search = [&](double mu_) -> nmpc_status {
+        Merit k{}, t{};
+        TRY(merit_at(0.0, mu_, 1, k));
+        const double a_max = hm[5];
+        if (!flt_ready) {                                 // [17] Eq. (21): theta_max, theta_min from the starting point
+            th_max = o.theta_max_fact * std::max(1.0, k.theta); th_min = o.theta_min_fact * std::max(1.0, k.theta);
+            flt_ready = true;
+        }
+        if (mu_ != flt_mu) { flt.assign(1, {th_max, -INFINITY}); flt_mu = mu_; }       // a new barrier problem: new filter (A-3)
+        const double tol = 10.0 * 2.220446049250313e-16 * std::fabs(k.phi);
+        double alpha = a_max, accepted = a_max;
+        int nback = 0, augment = -1;                      // -1: gave up (reading G20), 0 / 1: accepted without / with augmentation
+        for (; nback <= o.ls_max_backtracks; ++nback) {
+            TRY(merit_at(alpha, mu_, 0, t));
+            bool in_filter = false;
+            for (const auto& e : flt) if (t.theta >= e.first && t.phi >= e.second) { in_filter = true; break; }
+            const bool switching = k.g < 0.0 && alpha * std::pow(-k.g, o.s_phi) > o.delta_sw * std::pow(k.theta, o.s_theta);
+            const bool armijo = t.phi - k.phi - tol <= o.eta_phi * alpha * k.g;
+            if (!in_filter) {
+                if (k.theta <= th_min && switching) {
+                    if (armijo) { accepted = alpha; augment = 0; break; }
+                } else if (t.theta <= (1.0 - o.gamma_theta) * k.theta || t.phi - k.phi - tol <= -o.gamma_phi * k.theta) {
+                    accepted = alpha; augment = (!switching || !armijo) ? 1 : 0; break;
+                }
+            }
+            alpha *= 0.5;
+        }
+        if (augment < 0) { accepted = a_max; flt.assign(1, {th_max, -INFINITY}); }
+        else if (augment == 1) flt.push_back({(1.0 - o.gamma_theta) * k.theta, k.phi - o.gamma_phi * k.theta});
+        last_backtracks = nback;
+        hm[7] = accepted;
+        CK(cudaMemcpyAsync(V.scal + 7, hm + 7, sizeof(double), cudaMemcpyHostToDevice, st));
+        return NMPC_OK;
+    };
     auto solve_step_update = [&](double mu_, double tau_) -> nmpc_status {
         pt.begin(&S.ms_solve, 3);                                                 // S8: Eq. (22)-(25)
         CK(cudaMemcpyAsync(V.dy, V.b, sizeof(double) * M.n, cudaMemcpyDeviceToDevice, st));
@@ -795,6 +849,7 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
             pt.end();
         }
         pt.begin(&S.ms_vector, 4);
+        if (o.globalization) TRY(filter_line_search(mu_));                     // Eq. (26): "line search with step size alpha"
         launch_update(M, V, h->D.fail_col, st); h->launches++;                 // S10: Eq. (26)
         pt.end();
         return NMPC_OK;
@@ -887,7 +942,7 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
         }
         if (eta > 0.0) eta_last = eta;
         TRY(solve_step_update(mu, tau));
-        if (trace && it < trace_cap) { trace[it] = nmpc_trace_row{}; trace[it].mu = mu; trace[it].E0 = E0; trace[it].Emu = Emu; trace[it].eta = eta; }
+        if (trace && it < trace_cap) { trace[it] = nmpc_trace_row{}; trace[it].mu = mu; trace[it].E0 = E0; trace[it].Emu = Emu; trace[it].eta = eta; trace[it].backtracks = last_backtracks; }
         ++it;
     }
 done:

@@ -131,6 +131,7 @@ struct IpmVectors {               // primal-dual iterate and work vectors (devic
     double *c, *gradf, *Jval, *Wval, *Kval;                  // model evaluation + assembled K values
     double *r_pp, *r_pm, *q, *t, *sigx, *b, *dy;             // residuals, Sigma, rhs, step
     double *rho;                                             // refinement: minus the un-condensed residual, then the correction
+    double *yt, *ct;                                         // line search: trial point y + alpha dy and c(yt)
     double *dsp, *dsm, *dwp, *dwm, *dzL, *dzU;
     double *partial;                                         // block partials of the reductions
     double *scal;                                            // device scalars (see ipm.cu)
@@ -161,5 +162,10 @@ void launch_objective(const DevModel& M, const IpmVectors& V, cudaStream_t st);
 // failed pivot (fail_col may be null).
 void launch_refine_residual(const DevModel& M, const IpmVectors& V, double eta, const int32_t* fail_col, cudaStream_t st);
 void launch_add_correction(const DevModel& M, const IpmVectors& V, const int32_t* fail_col, cudaStream_t st);
+// filter line search (options.globalization): trial point yt = y + alpha dy, then (after a model evaluation c(yt) -> ct)
+// scal[0..4] <- theta (1-norm of the lifted equality residuals), sum of the logarithms of the barrier, f(yt), number of
+// arguments outside the barrier's domain, and (with_grad) grad phi_mu^T d at alpha = 0
+void launch_trial_point(const DevModel& M, const IpmVectors& V, double alpha, cudaStream_t st);
+void launch_merit(const DevModel& M, const IpmVectors& V, double alpha, double mu, double gamma, int with_grad, cudaStream_t st);
 
 }  // namespace nmpc

@@ -384,6 +384,62 @@ __global__ void __launch_bounds__(NT) add_correction_kernel(DevModel M, IpmVecto
     if (i < M.n) V.dy[i] += V.rho[i];
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// Filter line search of ref. [17] (options.globalization): the two measures of a trial point (y + alpha dy, s + alpha ds)
+//   theta = |c - gamma + s+|_1 + |-c - gamma + s-|_1,   phi_mu = f - mu (sum ln s+ + sum ln s- + sum ln(y - lb) + sum ln(ub - y))
+// reduced with the fixed tree; scal[0..4] = theta, sum of logs, f, #arguments <= 0, grad phi_mu^T d (alpha = 0 call only)
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(NT) trial_point_kernel(DevModel M, IpmVectors V, double alpha) {
+    const int64_t i = blockIdx.x * (int64_t)NT + threadIdx.x;
+    if (i < M.n) V.yt[i] = alpha != 0.0 ? V.y[i] + alpha * V.dy[i] : V.y[i];
+}
+
+__global__ void __launch_bounds__(NT) merit_kernel(DevModel M, IpmVectors V, double alpha, double mu, double gamma, int with_grad) {
+    Red<5> a;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) a.v[k] = 0.0;
+    const bool step = alpha != 0.0;
+    const int nv = M.desc.nv, nx = M.desc.nx;
+    const int64_t total = M.n + M.m;
+    for (int64_t idx = blockIdx.x * (int64_t)NT + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * NT) {
+        if (idx < M.n) {
+            const int64_t i = idx;
+            const double lb = M.lb[i], ub = M.ub[i], yt = V.yt[i];
+            const int k = (int)(i / nv), e = (int)(i - (int64_t)k * nv);
+            const double* x = V.yt + (int64_t)k * nv;
+            a.v[2] += cost_value_entry(M.desc, e, x, x + nx, M.ref + (int64_t)k * M.desc.nr);
+            if (lb > -INF) { const double d = yt - lb; if (d > 0.0) a.v[1] += log(d); else a.v[3] += 1.0; }
+            if (ub < INF) { const double d = ub - yt; if (d > 0.0) a.v[1] += log(d); else a.v[3] += 1.0; }
+            if (with_grad) {
+                const double dy = V.dy[i], y = V.y[i];
+                double g = V.gradf[i] * dy;
+                if (lb > -INF) g -= mu * (dy / (y - lb));
+                if (ub < INF) g += mu * (dy / (ub - y));
+                a.v[4] += g;
+            }
+        } else {
+            const int64_t r = idx - M.n;
+            const double c = V.ct[r];
+            const double sp = step ? V.sp[r] + alpha * V.dsp[r] : V.sp[r], sm = step ? V.sm[r] + alpha * V.dsm[r] : V.sm[r];
+            a.v[0] += fabs(c - gamma + sp) + fabs(-c - gamma + sm);
+            if (sp > 0.0) a.v[1] += log(sp); else a.v[3] += 1.0;
+            if (sm > 0.0) a.v[1] += log(sm); else a.v[3] += 1.0;
+            if (with_grad) a.v[4] -= mu * (V.dsp[r] / V.sp[r] + V.dsm[r] / V.sm[r]);
+        }
+    }
+    const int ops[5] = {2, 2, 2, 2, 2};
+    block_reduce<5>(a, ops, V.partial + (int64_t)blockIdx.x * 8);
+    if (!last_block_arrives(V.scal + 15)) return;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) a.v[k] = 0.0;
+    for (int b = threadIdx.x; b < (int)gridDim.x; b += NT) {
+        const double* p = V.partial + (int64_t)b * 8;
+#pragma unroll
+        for (int k = 0; k < 5; ++k) a.v[k] += __ldcg(p + k);
+    }
+    block_reduce<5>(a, ops, V.scal);
+}
+
 inline unsigned blocks_for(int64_t work) { return (unsigned)((work + NT - 1) / NT); }
 inline int red_blocks(int64_t work) { return (int)std::min<int64_t>(RED_BLOCKS, (work + NT - 1) / NT); }
 
@@ -431,6 +487,12 @@ void launch_refine_residual(const DevModel& M, const IpmVectors& V, double eta, 
 }
 void launch_add_correction(const DevModel& M, const IpmVectors& V, const int32_t* fail_col, cudaStream_t st) {
     add_correction_kernel<<<blocks_for(M.n), NT, 0, st>>>(M, V, fail_col);
+}
+void launch_trial_point(const DevModel& M, const IpmVectors& V, double alpha, cudaStream_t st) {
+    trial_point_kernel<<<blocks_for(M.n), NT, 0, st>>>(M, V, alpha);
+}
+void launch_merit(const DevModel& M, const IpmVectors& V, double alpha, double mu, double gamma, int with_grad, cudaStream_t st) {
+    merit_kernel<<<red_blocks(M.n + M.m), NT, 0, st>>>(M, V, alpha, mu, gamma, with_grad);
 }
 void launch_objective(const DevModel& M, const IpmVectors& V, cudaStream_t st) {
     const int nb = red_blocks(M.n);

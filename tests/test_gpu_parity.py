@@ -574,3 +574,38 @@ def test_ipm_with_iterative_refinement_vs_oracle(name, ov, steps):
         yo = ro["state"].y
         assert np.abs(y.cpu().numpy() - yo).max() <= 1e-8 * np.abs(yo).max()
         h.close()
+
+
+@pytest.mark.parametrize("name,ov", MID)
+def test_ipm_with_filter_line_search_vs_oracle(name, ov):
+    """options.globalization = 1: the filter line search of ref. [17] on the primal step, the same
+    algorithm step by step in the oracle (globalization="filter").  theta and phi_mu are reduced on the device, the acceptance
+    tests are host scalars; iteration counts, the number of halvings in every iteration and the converged point must agree
+    (C4's cold solve backtracks, the others accept every full step)."""
+    cfg = make_config(name, **ov)
+    ro = LiftedIPM(cfg, linsolve="blocktri", globalization="filter").solve()
+    assert ro["status"] == "converged"
+    h = _gpu_ipm(cfg, globalization=1)
+    h.update_params(dev(cfg.x0), dev(cfg.ref_for_solve(0)))
+    y = torch.zeros(cfg.n, dtype=torch.float64, device=DEV)
+    rg = h.ipm_solve(0, y, trace_cap=256)
+    assert rg["status"] == 0
+    assert rg["iters"] == ro["iters"], ([t["backtracks"] for t in rg["trace"]], [t["backtracks"] for t in ro["trace"]])
+    assert [int(t["backtracks"]) for t in rg["trace"]] == [t["backtracks"] for t in ro["trace"]]
+    for tg, to in zip(rg["trace"], ro["trace"]):
+        assert tg["mu"] == to["mu"] and tg["eta"] == to["eta"]
+        assert abs(tg["alpha_pr"] - to["alpha_pr"]) <= 1e-3 and abs(tg["alpha_du"] - to["alpha_du"]) <= 1e-3
+    yo = ro["state"].y
+    assert np.abs(y.cpu().numpy() - yo).max() <= 1e-6 * np.abs(yo).max()
+    if name == "C4":
+        assert sum(t["backtracks"] for t in ro["trace"]) > 0
+    # warm re-solve with the filter on: same count as the oracle's
+    h.update_params(dev(np.clip(cfg.x0 + cfg.noise_for_solve(0) + 1e-3, *cfg.x0_clip)), dev(cfg.ref_for_solve(1)))
+    ipm = LiftedIPM(cfg, linsolve="blocktri", globalization="filter")
+    ipm.state = ro["state"].copy()
+    ipm.nlp.set_params(np.clip(cfg.x0 + cfg.noise_for_solve(0) + 1e-3, *cfg.x0_clip), cfg.ref_for_solve(1))
+    rw = ipm.solve(warm=True)
+    rgw = h.ipm_solve(1, y, trace_cap=256)
+    assert rgw["status"] == 0 and rgw["iters"] == rw["iters"]
+    assert np.abs(y.cpu().numpy() - rw["state"].y).max() <= 1e-6 * np.abs(rw["state"].y).max()
+    h.close()
