@@ -476,6 +476,39 @@ def sigma_sweep(nb, torch, cfg, stream, count=200):
                     "flag included; backward error of every draw evaluated after the timed loop"}
 
 
+def batched_throughput(nb, torch, cfg, B, grid_limit, R):
+    """B independent instances of one OCP structure (seeded x0 perturbations) on B handles / B streams,
+    solved concurrently by nmpc_ipm_solve_batch, R warm re-solve rounds after a cold round.  Wall clock around the rounds
+    (device idle before and after), parameter uploads included."""
+    dev = torch.device("cuda", torch.cuda.current_device())
+    td = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64).to(dev)   # noqa: E731
+    streams = [torch.cuda.Stream() for _ in range(B)]
+    hs = [nb.Handle(None, nb.make_ocp(cfg), nb.default_options(grid_limit=grid_limit), stream=streams[b].cuda_stream) for b in range(B)]
+    ys = [torch.zeros(cfg.n, dtype=torch.float64, device=dev) for _ in range(B)]
+    x0 = [replica_x0(cfg, b) for b in range(B)]
+    lo, hi = float(cfg.x0_clip[0]), float(cfg.x0_clip[1])
+    iters, bad, t_timed = 0, 0, 0.0
+    for j in range(R + 1):
+        for b in range(B):
+            with torch.cuda.stream(streams[b]):
+                hs[b].update_params(td(x0[b]), td(cfg.ref_for_solve(j)))
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        stats = nb.ipm_solve_batch(hs, [int(j > 0)] * B, ys, check=False)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if j > 0:
+            t_timed += dt; iters += sum(s["iters"] for s in stats)
+        bad += sum(int(s["status"] != 0) for s in stats)
+        for b in range(B):
+            x0[b] = np.clip(ys[b][: cfg.nx].cpu().numpy() + cfg.noise_for_solve(j), lo, hi)
+    for h in hs:
+        h.close()
+    return {"instances": B, "grid_limit": grid_limit, "rounds": R, "resolves_per_s": B * R / t_timed,
+            "us_per_ipm_iter_aggregate": t_timed * 1e6 / max(1, iters), "ipm_iters": iters, "not_converged": bad,
+            "timing": "host wall clock around nmpc_ipm_solve_batch with the device idle on both sides; one host thread per instance"}
+
+
 def measure_workload(nb, torch, cfg, stream, K, W, flush_buf, x0_first, gpu_index, sample_clocks=True):
     """Everything bench.py reports about one configuration: analysis (a0), the device-resident closed loop with L2 flush
     and clock record, the HOST-buffer (e2e) loop on the recorded x0 sequence, and the phase split."""
@@ -644,6 +677,8 @@ def run_own(args):
                     extra[name] = workload_report(m2, hbm_peak)
                     if not args.no_cpu:
                         extra[name]["cpu_baseline"] = oracle_sample(name)
+                    if name in ("C0", "C1"):            # latency-bound single instances: what concurrent instances make of the GPU
+                        extra[name]["batched"] = batched_throughput(nb, torch, c2, 16, 18 if name == "C1" else 9, 10)
                     if name == "C4":
                         extra[name]["sigma_sweep"] = sigma_sweep(nb, torch, c2, stream)
                         if not args.no_cpu:

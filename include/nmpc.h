@@ -103,6 +103,8 @@ typedef struct {
                                     second-order correction / restoration, reading G20)                                      */
     double  gamma_theta, gamma_phi, delta_sw, s_theta, s_phi, eta_phi, theta_max_fact, theta_min_fact;   /* constants of [17] */
     int32_t ls_max_backtracks;
+    int32_t grid_limit;          /* 0 = none.  Upper bound on the CTAs of the persistent factor / solve kernels of this handle, so
+                                    that the kernels of several handles driven concurrently (nmpc_ipm_solve_batch) share the SMs */
     int32_t epoch_limit;         /* 0 = automatic.  Test hook: the completion flags of the persistent kernels are
                                     call-number valued and are zeroed before a counter could overflow (after ~1e4..1e6
                                     factorizations); a small value (>= 3) forces that restart every few calls           */
@@ -186,6 +188,16 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
 /*      end-to-end form with HOST buffers: parameters in, primal solution out (copies inside the call)        */
 nmpc_status nmpc_ipm_solve_host(nmpc_handle h, int32_t warm, const double* x0_host, const double* ref_host,
                                 double* y_out_host, nmpc_stats* stats_host);
+
+/* ---- Independent OCP instances (the scenarios of the uncertainty domain D_xi):
+ *      `count` handles, each created on its OWN CUDA stream (a handle's stream must not be shared), solved concurrently --
+ *      one host thread per handle runs nmpc_ipm_solve, the persistent kernels of the handles overlap on the device (bound
+ *      their grids with options.grid_limit so that they share the SMs).  warm_host: count flags or NULL (all cold);
+ *      y_inout_dev_host: HOST array of count DEVICE pointers (each n doubles) or NULL; stats_host: count records or NULL.
+ *      Every instance computes exactly what nmpc_ipm_solve on its handle alone computes (bitwise).  Returns NMPC_OK or the
+ *      first status that is not NMPC_OK (every instance is run to its end either way).                                  */
+nmpc_status nmpc_ipm_solve_batch(nmpc_handle* handles_host, int32_t count, const int32_t* warm_host,
+                                 double* const* y_inout_dev_host, nmpc_stats* stats_host);
 
 /* ---- current primal-dual iterate z (DEVICE outputs; any pointer may be NULL): s+,s-,w+,w- length m; zL,zU n */
 nmpc_status nmpc_get_iterate(nmpc_handle h, double* y_dev, double* sp_dev, double* sm_dev, double* wp_dev,

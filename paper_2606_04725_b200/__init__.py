@@ -4,4 +4,5 @@ csrc/); this package is its build script and a thin ctypes binding with the same
 callers only for device memory and streams.  There is no CPU fallback: importing `binding` and calling into it
 without the built library raises."""
 from . import binding  # noqa: F401
-from .binding import (Handle, NmpcError, Symbolic, default_options, fp64_peak, load_library, make_ocp, make_pattern)  # noqa: F401
+from .binding import (Handle, NmpcError, Symbolic, default_options, fp64_peak, ipm_solve_batch, load_library, make_ocp,
+                      make_pattern)  # noqa: F401

@@ -24,7 +24,7 @@ LIB_AIDS = os.path.join(HERE, "libnmpc_b200_aids.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
-COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include")]
+COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC,-pthread", "-I", os.path.join(ROOT, "include")]
 # (source, extra flags).  ipm.cu is built without FMA contraction so that its element-wise statements round like the
 # plain fp64 expressions of the method; the dense kernels of factor.cu use FMA.
 SOURCES = [
@@ -59,7 +59,7 @@ def _compile(src: str, extra: list[str], force: bool, hdr_t: float, bdir: str) -
 
 def _link(lib: str, objs: list[str], verbose: bool) -> None:
     tmp = lib + f".tmp{os.getpid()}"
-    subprocess.check_call([NVCC] + ARCH + ["-shared", "-o", tmp] + objs + ["-lcudart"])
+    subprocess.check_call([NVCC] + ARCH + ["-shared", "-o", tmp] + objs + ["-lcudart", "-lpthread"])
     os.replace(tmp, lib)
     if verbose:
         print("built", lib)

@@ -43,7 +43,7 @@ class nmpc_options(C.Structure):
                 + [("time_phases", c_i32), ("refine_steps", c_i32), ("globalization", c_i32)]
                 + [(k, c_dbl) for k in ("gamma_theta", "gamma_phi", "delta_sw", "s_theta", "s_phi", "eta_phi", "theta_max_fact",
                                         "theta_min_fact")]
-                + [("ls_max_backtracks", c_i32), ("epoch_limit", c_i32)])
+                + [("ls_max_backtracks", c_i32), ("grid_limit", c_i32), ("epoch_limit", c_i32)])
 
 
 class nmpc_sym_info(C.Structure):
@@ -82,6 +82,7 @@ SIGNATURES = {
     "nmpc_kkt_multiply": (c_i32, [c_vp, c_vp, c_vp]),
     "nmpc_ipm_solve": (c_i32, [c_vp, c_i32, c_i32, c_vp, P(nmpc_stats), c_vp, c_i32]),
     "nmpc_ipm_solve_host": (c_i32, [c_vp, c_i32, c_vp, c_vp, c_vp, P(nmpc_stats)]),
+    "nmpc_ipm_solve_batch": (c_i32, [c_vp, c_i32, c_vp, c_vp, c_vp]),
     "nmpc_get_iterate": (c_i32, [c_vp] * 8),
     "nmpc_set_iterate": (c_i32, [c_vp] * 8),
     "nmpc_model_eval": (c_i32, [c_vp] * 7),
@@ -133,6 +134,22 @@ def load_aids_library() -> C.CDLL:
     if _aids is None:
         _aids = _load(AIDS_LIB_PATH, {**SIGNATURES, **AIDS_SIGNATURES})
     return _aids
+
+
+def ipm_solve_batch(handles, warm, ys, check=True):
+    """nmpc_ipm_solve_batch: `handles` (each on its own stream) solved concurrently; warm: list of flags; ys: list of DEVICE
+    tensors (n doubles each) or None.  Returns the list of nmpc_stats dicts."""
+    lib = load_library()
+    n = len(handles)
+    harr = (c_vp * n)(*[h._h for h in handles])
+    warr = (c_i32 * n)(*[int(w) for w in warm])
+    yarr = (c_vp * n)(*[_ptr(y) for y in ys]) if ys is not None else None
+    stats = (nmpc_stats * n)()
+    st = lib.nmpc_ipm_solve_batch(C.cast(harr, c_vp), n, C.cast(warr, c_vp), C.cast(yarr, c_vp) if yarr is not None else None,
+                                  C.cast(stats, c_vp))
+    if st and (check or st not in (NMPC_E_MAXITER, NMPC_E_INERTIA, NMPC_E_STEP)):
+        raise NmpcError(st, "nmpc_ipm_solve_batch")
+    return [{k: getattr(stats[i], k) for k, _ in nmpc_stats._fields_} for i in range(n)]
 
 
 class NmpcError(RuntimeError):

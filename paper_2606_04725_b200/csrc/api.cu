@@ -11,6 +11,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <thread>
 #include <vector>
 
 #include "device.h"
@@ -257,6 +258,7 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
     F.fsmem = smem_bytes; F.ssmem = solve_smem;
     F.fgrid = (int32_t)std::max<int64_t>(1, std::min<int64_t>((int64_t)tasks.size(), (int64_t)num_sms * ctas_per_sm));
     F.sgrid = (int32_t)std::max<int64_t>(1, std::min<int64_t>((int64_t)stasks.size(), (int64_t)num_sms * solve_ctas_per_sm));
+    if (h->opt.grid_limit > 0) { F.fgrid = std::min(F.fgrid, h->opt.grid_limit); F.sgrid = std::min(F.sgrid, h->opt.grid_limit); }
     // epoch-valued flags: counters reach epoch * target and the claim counters epoch * (ntasks + grid); reset before 2^31
     int64_t per_epoch = std::max<int64_t>((int64_t)tasks.size() + F.fgrid, (int64_t)stasks.size() + F.sgrid);
     for (int s = 0; s < ns; ++s) per_epoch = std::max<int64_t>(per_epoch, target[s]);
@@ -964,6 +966,25 @@ done:
     S.ms_total = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
     if (stats) *stats = S;
     return status;
+}
+
+nmpc_status nmpc_ipm_solve_batch(nmpc_handle* handles, int32_t count, const int32_t* warm, double* const* y_inout, nmpc_stats* stats) {
+    if (!handles || count < 1) return NMPC_E_ARG;
+    for (int i = 0; i < count; ++i) {
+        if (!handles[i]) return NMPC_E_ARG;
+        for (int k = 0; k < i; ++k)
+            if (handles[k] == handles[i] || handles[k]->stream == handles[i]->stream) { handles[i]->err = "batch handles must be distinct and own distinct streams"; return NMPC_E_ARG; }
+    }
+    std::vector<nmpc_status> st((size_t)count, NMPC_OK);
+    auto work = [&](int i) { st[i] = nmpc_ipm_solve(handles[i], warm ? warm[i] : 0, 0, y_inout ? y_inout[i] : nullptr, stats ? &stats[i] : nullptr, nullptr, 0); };
+    std::vector<std::thread> th;
+    th.reserve((size_t)count);
+    try { for (int i = 1; i < count; ++i) th.emplace_back(work, i); }
+    catch (...) { for (auto& t : th) t.join(); return NMPC_E_ALLOC; }
+    work(0);                                              // the calling thread takes the first instance
+    for (auto& t : th) t.join();
+    for (int i = 0; i < count; ++i) if (st[i] != NMPC_OK) return st[i];
+    return NMPC_OK;
 }
 
 nmpc_status nmpc_ipm_solve_host(nmpc_handle h, int32_t warm, const double* x0_host, const double* ref_host, double* y_out_host, nmpc_stats* stats) {

@@ -609,3 +609,54 @@ def test_ipm_with_filter_line_search_vs_oracle(name, ov):
     assert rgw["status"] == 0 and rgw["iters"] == rw["iters"]
     assert np.abs(y.cpu().numpy() - rw["state"].y).max() <= 1e-6 * np.abs(rw["state"].y).max()
     h.close()
+
+
+def test_batched_instances_match_single_handle_runs():
+    """nmpc_ipm_solve_batch (independent OCP instances, the scenarios of D_xi): six
+    handles on six streams with bounded grids, solved concurrently (cold, then two warm re-solves).  Every instance must
+    reproduce bit for bit what its own handle computes alone, and instance 0 the oracle."""
+    cfg = make_config("C1", trays=14, N=20)
+    B = 6
+    rng = np.random.default_rng(12)
+    x0s = [np.clip(cfg.x0 + (b > 0) * rng.normal(0.0, 0.01, cfg.nx), *cfg.x0_clip) for b in range(B)]
+    streams = [torch.cuda.Stream() for _ in range(B)]
+
+    def make(b):
+        return nb.Handle(None, nb.make_ocp(cfg), nb.default_options(grid_limit=20), stream=streams[b].cuda_stream)
+
+    def params(h, b, j):
+        with torch.cuda.stream(streams[b]):
+            h.update_params(dev(np.clip(x0s[b] + 0.002 * j, *cfg.x0_clip)), dev(cfg.ref_for_solve(j)))
+        streams[b].synchronize()
+
+    hs = [make(b) for b in range(B)]
+    ys = [torch.zeros(cfg.n, dtype=torch.float64, device=DEV) for _ in range(B)]
+    got = []
+    for j in range(3):
+        for b in range(B):
+            params(hs[b], b, j)
+        stats = nb.ipm_solve_batch(hs, [int(j > 0)] * B, ys)
+        torch.cuda.synchronize()
+        assert all(s["status"] == 0 for s in stats)
+        got.append(([s["iters"] for s in stats], [y.cpu().numpy().copy() for y in ys]))
+    for h in hs:
+        h.close()
+    for b in range(B):                                       # the same instance on its own
+        h = make(b)
+        y = torch.zeros(cfg.n, dtype=torch.float64, device=DEV)
+        for j in range(3):
+            params(h, b, j)
+            r = h.ipm_solve(int(j > 0), y)
+            torch.cuda.synchronize()
+            assert r["iters"] == got[j][0][b]
+            assert np.array_equal(y.cpu().numpy(), got[j][1][b])
+        h.close()
+    ro = LiftedIPM(cfg, linsolve="sparse").solve()
+    assert got[0][0][0] == ro["iters"]
+    assert np.abs(got[0][1][0] - ro["state"].y).max() <= 1e-6 * np.abs(ro["state"].y).max()
+    with pytest.raises(nb.NmpcError):                        # a handle twice / a shared stream is refused
+        h1 = make(0)
+        try:
+            nb.ipm_solve_batch([h1, h1], [0, 0], None)
+        finally:
+            h1.close()
