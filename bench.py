@@ -604,6 +604,7 @@ def run_own(args):
     n_it, n_f = int(sum(res["iters"])), int(sum(res["facts"]))
     dfma_tf, _ = nb.fp64_peak(0, 3)                       # measurement build (libnmpc_b200_aids.so): live cross-check of the peak
     dmma_tf, _ = nb.fp64_peak(1, 3)
+    gemm_tf, _ = nb.tile_gemm_peak(2048, 3)               # the factorization's tile GEMM loop in isolation
 
     # ---- max over ranks / totals ----
     dev_ms_max, host_ms_max, tot_it, tot_f, tot_steps, tot_launch = aggregate_over_ranks(
@@ -652,7 +653,7 @@ def run_own(args):
                      "frac": flops / factor_us * 1e-6 / FP64_DERIVED_TFLOPS,
                      "traffic": tr_f["bytes_per_launch"] if tr_f else None, "traffic_source": tr_f["source"] if tr_f else None,
                      "peak_source": "derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md section 7); fp64 is not in MEASURED_PEAKS.json",
-                     "peak_live_dfma_tflops": dfma_tf, "peak_live_dmma_tflops": dmma_tf,
+                     "peak_live_dfma_tflops": dfma_tf, "peak_live_dmma_tflops": dmma_tf, "tile_gemm_isolated_tflops": gemm_tf,
                      "flops_per_launch": flops, "avg_launch_us": factor_us,
                      "share_of_iteration": factor_us * n_f / max(1e-9, dev_ms * 1e3)},
         "roofline_solve": {"bound": "hbm", "kernel": "solve_dag_kernel (supernodal forward + backward triangular solves)",

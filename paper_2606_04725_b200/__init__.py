@@ -5,4 +5,4 @@ callers only for device memory and streams.  There is no CPU fallback: importing
 without the built library raises."""
 from . import binding  # noqa: F401
 from .binding import (Handle, NmpcError, Symbolic, default_options, fp64_peak, ipm_solve_batch, load_library, make_ocp,
-                      make_pattern)  # noqa: F401
+                      make_pattern, tile_gemm_peak)  # noqa: F401

@@ -100,6 +100,7 @@ SIGNATURES = {
 # the two extra symbols of include/nmpc_aids.h (measurement build, libnmpc_b200_aids.so)
 AIDS_SIGNATURES = {
     "nmpc_fp64_peak": (c_i32, [c_i32, c_i32, P(c_dbl), P(c_dbl)]),
+    "nmpc_tile_gemm_peak": (c_i32, [c_i32, c_i32, P(c_dbl), P(c_dbl)]),
     "nmpc_get_task_trace": (c_i64, [c_vp, c_i32, c_vp, c_vp, c_i64]),
 }
 AIDS_LIB_PATH = os.path.join(_HERE, "libnmpc_b200_aids.so")
@@ -225,6 +226,15 @@ def fp64_peak(kind: int, repeats: int = 5):
     st = load_aids_library().nmpc_fp64_peak(kind, repeats, C.byref(tf), C.byref(ms))
     if st:
         raise NmpcError(st, "nmpc_fp64_peak")
+    return tf.value, ms.value
+
+
+def tile_gemm_peak(K: int = 2048, repeats: int = 3):
+    """nmpc_tile_gemm_peak: (TFLOP/s, ms) of the factorization's tile GEMM loop in isolation."""
+    tf, ms = c_dbl(), c_dbl()
+    st = load_aids_library().nmpc_tile_gemm_peak(K, repeats, C.byref(tf), C.byref(ms))
+    if st:
+        raise NmpcError(st, "nmpc_tile_gemm_peak")
     return tf.value, ms.value
 
 
