@@ -108,6 +108,10 @@ typedef struct {
     int32_t epoch_limit;         /* 0 = automatic.  Test hook: the completion flags of the persistent kernels are
                                     call-number valued and are zeroed before a counter could overflow (after ~1e4..1e6
                                     factorizations); a small value (>= 3) forces that restart every few calls           */
+    /* ---- the HyKKT variant (nmpc_hykkt_solve, reading G21) ---- */
+    double  gamma_h;             /* weight of the augmented-Lagrangian term in K_g = W + Sigma_x + eta I + gamma_h J^T J   */
+    double  cg_tol;              /* CG on S = J K_g^-1 J^T stops at |r|_2 <= cg_tol |rhs|_2                                 */
+    int32_t cg_max_iter;
 } nmpc_options;
 
 typedef struct {                 /* filled by nmpc_get_info; arrays are HOST pointers owned by the handle     */
@@ -135,7 +139,8 @@ typedef struct {                 /* filled by nmpc_ipm_solve (HOST)             
 typedef struct {                 /* one row per IPM iteration, for parity traces and per-iteration timing (HOST,
                                     caller array)                                                              */
     double mu, E0, Emu, eta, alpha_pr, alpha_du;
-    double backtracks;           /* halvings of the filter line search in this iteration (globalization = 1)            */
+    double backtracks;           /* halvings of the filter line search in this iteration (globalization = 1);
+                                    nmpc_hykkt_solve: conjugate-gradient iterations of this IPM iteration               */
     double ms_iter;              /* device time of the whole iteration (CUDA events on the handle's stream, from the
                                     launch of S6 to the launch of the next iteration's S6 / the end of the solve)   */
     double ms_eval, ms_assemble, ms_factor, ms_solve, ms_vector;   /* phase split, only with options.time_phases  */
@@ -188,6 +193,19 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
 /*      end-to-end form with HOST buffers: parameters in, primal solution out (copies inside the call)        */
 nmpc_status nmpc_ipm_solve_host(nmpc_handle h, int32_t warm, const double* x0_host, const double* ref_host,
                                 double* y_out_host, nmpc_stats* stats_host);
+
+/* ---- The HyKKT variant of Algorithm 2 ("the system can be reformulated using either Lifted-KKT or HyKKT
+ *      ... a hybrid direct-iterative approach based on an augmented Lagrangian formulation ... the proposed framework and its
+ *      implementation also support HyKKT"; reading G21 of DESIGN.md section 3).  The equalities h(y) = 0 are kept exact (no
+ *      gamma tube, no slacks); primal-dual iterate (y, lam, zL, zU).  Per IPM iteration: K_g = W + Sigma_x + eta I + gamma_h J^T J
+ *      is assembled, factored (Eq. 20-21, same pattern and kernels as Eq. 17's K) and used for 2 + #CG triangular-solve pairs
+ *      (Eq. 22-25): conjugate gradients on S dlam = J K_g^-1 (r1 + gamma_h J^T r2) - r2, then dy = K_g^-1 (r1 + gamma_h J^T r2
+ *      - J^T dlam).  Arguments, warm start, statuses, stats and trace as nmpc_ipm_solve (trace.backtracks = CG iterations of the
+ *      iteration; stats.eta_retries counts inertia retries).  The iterate shares the handle's storage with nmpc_ipm_solve
+ *      (lam lives in w+): do not alternate warm starts between the two variants on one handle.
+ *      nmpc_get_iterate returns lam in wp_dev (wm_dev == 0, slacks unused).                                              */
+nmpc_status nmpc_hykkt_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* y_inout_dev, nmpc_stats* stats_host,
+                             nmpc_trace_row* trace_host, int32_t trace_cap);
 
 /* ---- Independent OCP instances (the scenarios of the uncertainty domain D_xi):
  *      `count` handles, each created on its OWN CUDA stream (a handle's stream must not be shared), solved concurrently --

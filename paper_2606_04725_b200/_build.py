@@ -32,6 +32,7 @@ SOURCES = [
     ("factor.cu", []),
     ("solve.cu", []),
     ("ipm.cu", ["-fmad=false"]),
+    ("hykkt.cu", ["-fmad=false"]),
     ("api.cu", []),
 ]
 AIDS_ONLY = [("peak.cu", [])]

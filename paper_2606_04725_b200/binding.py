@@ -43,7 +43,8 @@ class nmpc_options(C.Structure):
                 + [("time_phases", c_i32), ("refine_steps", c_i32), ("globalization", c_i32)]
                 + [(k, c_dbl) for k in ("gamma_theta", "gamma_phi", "delta_sw", "s_theta", "s_phi", "eta_phi", "theta_max_fact",
                                         "theta_min_fact")]
-                + [("ls_max_backtracks", c_i32), ("grid_limit", c_i32), ("epoch_limit", c_i32)])
+                + [("ls_max_backtracks", c_i32), ("grid_limit", c_i32), ("epoch_limit", c_i32)]
+                + [("gamma_h", c_dbl), ("cg_tol", c_dbl), ("cg_max_iter", c_i32)])
 
 
 class nmpc_sym_info(C.Structure):
@@ -81,6 +82,7 @@ SIGNATURES = {
     "nmpc_solve": (c_i32, [c_vp, c_vp, c_i32]),
     "nmpc_kkt_multiply": (c_i32, [c_vp, c_vp, c_vp]),
     "nmpc_ipm_solve": (c_i32, [c_vp, c_i32, c_i32, c_vp, P(nmpc_stats), c_vp, c_i32]),
+    "nmpc_hykkt_solve": (c_i32, [c_vp, c_i32, c_i32, c_vp, P(nmpc_stats), c_vp, c_i32]),
     "nmpc_ipm_solve_host": (c_i32, [c_vp, c_i32, c_vp, c_vp, c_vp, P(nmpc_stats)]),
     "nmpc_ipm_solve_batch": (c_i32, [c_vp, c_i32, c_vp, c_vp, c_vp]),
     "nmpc_get_iterate": (c_i32, [c_vp] * 8),
@@ -323,17 +325,20 @@ class Handle:
     def kkt_multiply(self, x_dev, y_dev):
         self._ck(self.lib.nmpc_kkt_multiply(self._h, _ptr(x_dev), _ptr(y_dev)), "nmpc_kkt_multiply")
 
-    def ipm_solve(self, warm, y_inout_dev=None, use_y0=False, trace_cap=0, check=True):
+    def ipm_solve(self, warm, y_inout_dev=None, use_y0=False, trace_cap=0, check=True, _fn="nmpc_ipm_solve"):
         stats = nmpc_stats()
         trace = (nmpc_trace_row * trace_cap)() if trace_cap else None
-        st = self.lib.nmpc_ipm_solve(self._h, int(warm), int(use_y0), _ptr(y_inout_dev), C.byref(stats),
-                                     C.cast(trace, c_vp) if trace_cap else None, trace_cap)
-        self._ck(st, "nmpc_ipm_solve", allow=() if check else (NMPC_E_MAXITER, NMPC_E_INERTIA, NMPC_E_STEP))
+        st = getattr(self.lib, _fn)(self._h, int(warm), int(use_y0), _ptr(y_inout_dev), C.byref(stats),
+                                    C.cast(trace, c_vp) if trace_cap else None, trace_cap)
+        self._ck(st, _fn, allow=() if check else (NMPC_E_MAXITER, NMPC_E_INERTIA, NMPC_E_STEP))
         out = {k: getattr(stats, k) for k, _ in nmpc_stats._fields_}
         if trace_cap:
             out["trace"] = [{k: getattr(trace[i], k) for k, _ in nmpc_trace_row._fields_}
                             for i in range(min(trace_cap, stats.iters))]
         return out
+
+    def hykkt_solve(self, warm, y_inout_dev=None, use_y0=False, trace_cap=0, check=True):
+        return self.ipm_solve(warm, y_inout_dev, use_y0, trace_cap, check, _fn="nmpc_hykkt_solve")
 
     def ipm_solve_host(self, warm, x0_host, ref_host, y_out_host, check=True):
         stats = nmpc_stats()

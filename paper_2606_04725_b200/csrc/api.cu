@@ -968,6 +968,167 @@ done:
     return status;
 }
 
+// ---- the HyKKT variant of Algorithm 2 (reading G21 of DESIGN.md section 3): same S1..S10 skeleton as
+//      nmpc_ipm_solve with the slack rows removed; the direct part is the factorization / solves of K_g, the iterative part a
+//      conjugate-gradient loop on the Schur complement whose scalars (two dot products per iteration) are host scalars ----
+nmpc_status nmpc_hykkt_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* y_inout, nmpc_stats* stats, nmpc_trace_row* trace, int32_t trace_cap) {
+    if (!h) return NMPC_E_ARG;
+    DeviceGuard dg(h);
+    if (!h->has_model) { h->err = "nmpc_hykkt_solve needs a model (nmpc_ocp)"; return NMPC_E_STATE; }
+    if (use_y0 && !y_inout) return NMPC_E_ARG;
+    const nmpc_options& o = h->opt;
+    const DevModel& M = h->M;
+    const IpmVectors& V = h->V;
+    cudaStream_t st = h->stream;
+    auto t_begin = std::chrono::steady_clock::now();
+    nmpc_stats S{};
+    PhaseTimer pt{h, o.time_phases != 0 && stats != nullptr};
+    double mu;
+    if (warm && h->have_state) {
+        launch_warm_push(M, V, o.warm_push, st); h->launches++;
+        mu = o.mu_warm;
+    } else {
+        if (use_y0) CK(cudaMemcpyAsync(V.y, y_inout, sizeof(double) * M.n, cudaMemcpyDeviceToDevice, st));
+        launch_cold_init_y(M, V, h->d_uinit, use_y0, o.kappa_push, o.mu0, st);
+        launch_fill(M.m, 0.0, V.wp, st);                                       // lam = 0
+        h->launches += 2;
+        mu = o.mu0;
+    }
+    launch_fill(M.m, 0.0, V.wm, st);                                           // the model evaluation's lam = w+ - w-
+    launch_fill(M.m, o.gamma_h, V.q, st);                                      // J^T diag(q) J = gamma_h J^T J in the assembly
+    h->launches += 2;
+    const int nmult = h->nmult - (int)M.m;                                     // m equality multipliers + the bound multipliers
+    double eta_last = 0.0, E0 = 0.0;
+    int it = 0, nfact = 0, retries = 0;
+    int64_t ncg_total = 0;
+    nmpc_status status = NMPC_E_MAXITER;
+    double* hs = h->h_pinned;
+    double* hc = h->h_pinned + 40;                                             // pinned: the two CG dot products
+    const int n_ev = trace ? std::min(trace_cap, o.max_iter) + 1 : 0;
+    while ((int)h->it_ev.size() < n_ev) { cudaEvent_t e = nullptr; CK(cudaEventCreate(&e)); h->it_ev.push_back(e); }
+    auto mark_iteration = [&](int k) {
+        if (k < n_ev) cudaEventRecord(h->it_ev[k], st);
+        pt.flush(trace && k > 0 && k - 1 < trace_cap ? &trace[k - 1] : nullptr);
+    };
+    auto kg_solve = [&](double* rhs) -> nmpc_status {                          // Eq. (22)-(25) with the factor of K_g
+        pt.begin(&S.ms_solve, 3);
+        nmpc_status s = run_solve(h, rhs);
+        pt.end();
+        return s;
+    };
+    while (true) {
+        pt.begin(&S.ms_eval, 0);
+        launch_model_eval(M, V.y, V.wp, V.wm, nullptr, V.c, V.gradf, V.Jval, V.Wval, st); h->launches++;
+        pt.end();
+        pt.begin(&S.ms_vector, 4);
+        launch_hk_residuals(M, V, st); h->launches++;
+        CK(cudaMemcpyAsync(hs, V.scal, sizeof(double) * 10, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        pt.end();
+        if (it > 0 && trace && it - 1 < trace_cap) { trace[it - 1].alpha_pr = hs[7]; trace[it - 1].alpha_du = hs[8]; }
+        if (hs[6] != 0.0) { status = NMPC_E_STEP; break; }
+        const double s_d = std::max(o.s_max, hs[5] / (double)nmult) / o.s_max;
+        auto err_mu = [&](double m_) {
+            const double comp = hs[3] >= hs[4] ? std::max(std::fabs(hs[3] - m_), std::fabs(hs[4] - m_)) : 0.0;   // no bounds: none
+            return std::max(std::max(hs[0] / s_d, hs[1]), comp / s_d);
+        };
+        E0 = err_mu(0.0);
+        if (E0 <= o.eps_outer) { status = NMPC_OK; break; }
+        if (it >= o.max_iter) { status = NMPC_E_MAXITER; break; }
+        double Emu = err_mu(mu);
+        while (Emu <= o.kappa_eps * mu && mu > o.eps_outer / 10.0) {
+            mu = std::max(o.eps_outer / 10.0, std::min(o.kappa_mu * mu, std::pow(mu, o.theta_mu)));
+            Emu = err_mu(mu);
+        }
+        const double tau = std::max(o.tau_min, 1.0 - mu);
+        mark_iteration(it);
+        pt.begin(&S.ms_vector, 4);
+        launch_hk_rhs(M, V, mu, o.gamma_h, st); h->launches++;                 // Sigma_x, b_g = r1 + gamma_h J^T r2
+        pt.end();
+        pt.begin(&S.ms_assemble, 1);
+        launch_assemble_K(M, V.Jval, V.Wval, V.sigx, V.q, 0.0, V.Kval, st); h->launches++;
+        pt.end();
+        double eta = 0.0;
+        ++nfact;
+        pt.begin(&S.ms_factor, 2);
+        nmpc_status fs = run_factor(h, 0.0, nullptr);
+        pt.end();
+        while (fs == NMPC_E_NOT_SPD) {                                         // inertia correction: the schedule of Eq. (13)/(15)
+            ++retries;
+            if (eta == 0.0) eta = (eta_last == 0.0) ? o.eta_first : std::max(o.eta_min, o.eta_shrink * eta_last);
+            else eta = ((eta_last == 0.0) ? o.eta_grow_first : o.eta_grow) * eta;
+            if (eta > o.eta_max) { status = NMPC_E_INERTIA; goto done; }
+            ++nfact;
+            pt.begin(&S.ms_factor, 2);
+            fs = run_factor(h, eta, nullptr);
+            pt.end();
+        }
+        if (fs != NMPC_OK) return fs;
+        if (eta > 0.0) eta_last = eta;
+        // u = K_g^-1 b_g;  CG on S dlam = J u - r2 = J u + c;  dy = K_g^-1 (b_g - J^T dlam)
+        CK(cudaMemcpyAsync(V.dy, V.b, sizeof(double) * M.n, cudaMemcpyDeviceToDevice, st));
+        TRY(kg_solve(V.dy));
+        int ncg = 0;
+        {
+            double* r = V.r_pp; double* p = V.r_pm; double* Sp = V.t; double* x = V.dwp;
+            pt.begin(&S.ms_vector, 4);
+            launch_hk_j(M, V, V.dy, V.c, nullptr, r, st);                       // r = J u + c, scal[1] = r . r
+            launch_hk_cg_dir(M, 0.0, r, p, x, 1, st); h->launches += 2;         // p = r, x = 0
+            CK(cudaMemcpyAsync(hc, V.scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+            pt.end();
+            double rr = hc[1];
+            const double stop = o.cg_tol * o.cg_tol * rr;
+            while (ncg < o.cg_max_iter && rr > stop && rr > 0.0) {
+                pt.begin(&S.ms_vector, 4);
+                launch_hk_jt(M, V, p, nullptr, 1.0, V.rho, st); h->launches++;  // rho = J^T p
+                pt.end();
+                TRY(kg_solve(V.rho));
+                pt.begin(&S.ms_vector, 4);
+                launch_hk_j(M, V, V.rho, nullptr, p, Sp, st); h->launches++;    // Sp = J K_g^-1 J^T p, scal[0] = p . Sp
+                CK(cudaMemcpyAsync(hc, V.scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+                CK(cudaStreamSynchronize(st));
+                const double a = rr / hc[0];
+                launch_hk_cg_update(M, V, a, x, r, p, Sp, st); h->launches++;   // x += a p, r -= a Sp, scal[1] = r . r
+                CK(cudaMemcpyAsync(hc, V.scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+                CK(cudaStreamSynchronize(st));
+                const double rr_new = hc[1];
+                launch_hk_cg_dir(M, rr_new / rr, r, p, x, 0, st); h->launches++;
+                pt.end();
+                rr = rr_new;
+                ++ncg;
+            }
+            ncg_total += ncg;
+            pt.begin(&S.ms_vector, 4);
+            launch_hk_jt(M, V, x, V.b, -1.0, V.dy, st); h->launches++;          // dy <- b_g - J^T dlam
+            pt.end();
+            TRY(kg_solve(V.dy));
+        }
+        pt.begin(&S.ms_vector, 4);
+        launch_hk_step(M, V, mu, tau, st); launch_hk_update(M, V, st); h->launches += 2;
+        pt.end();
+        if (trace && it < trace_cap) { trace[it] = nmpc_trace_row{}; trace[it].mu = mu; trace[it].E0 = E0; trace[it].Emu = Emu; trace[it].eta = eta; trace[it].backtracks = ncg; }
+        ++it;
+    }
+done:
+    h->have_state = status == NMPC_OK || (status == NMPC_E_MAXITER && hs[6] == 0.0);
+    mark_iteration(it);
+    launch_objective(M, V, st); h->launches += 1;
+    CK(cudaMemcpyAsync(hs + 9, V.scal + 9, sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (y_inout) CK(cudaMemcpyAsync(y_inout, V.y, sizeof(double) * M.n, cudaMemcpyDeviceToDevice, st));
+    CK(cudaStreamSynchronize(st));
+    CK(cudaGetLastError());
+    S.status = status; S.iters = it; S.factorizations = nfact; S.eta_retries = retries; S.E0 = E0; S.mu = mu; S.eta_last = eta_last;
+    S.objective = hs[9];
+    for (int k = 0; k < it && k + 1 < n_ev && k < trace_cap; ++k) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, h->it_ev[k], h->it_ev[k + 1]) == cudaSuccess) trace[k].ms_iter = ms; else cudaGetLastError();
+    }
+    S.ms_total = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
+    if (stats) *stats = S;
+    return status;
+}
+
 nmpc_status nmpc_ipm_solve_batch(nmpc_handle* handles, int32_t count, const int32_t* warm, double* const* y_inout, nmpc_stats* stats) {
     if (!handles || count < 1) return NMPC_E_ARG;
     for (int i = 0; i < count; ++i) {

@@ -168,4 +168,20 @@ void launch_add_correction(const DevModel& M, const IpmVectors& V, const int32_t
 void launch_trial_point(const DevModel& M, const IpmVectors& V, double alpha, cudaStream_t st);
 void launch_merit(const DevModel& M, const IpmVectors& V, double alpha, double mu, double gamma, int with_grad, cudaStream_t st);
 
+
+// ---- hykkt.cu: vector kernels of the HyKKT variant (nmpc_hykkt_solve) ----
+void launch_hk_residuals(const DevModel& M, const IpmVectors& V, cudaStream_t st);
+void launch_hk_rhs(const DevModel& M, const IpmVectors& V, double mu, double gamma_h, cudaStream_t st);
+// out_n = a_n + sign * J^T v_m (a_n may be null)
+void launch_hk_jt(const DevModel& M, const IpmVectors& V, const double* v_m, const double* a_n, double sign, double* out_n, cudaStream_t st);
+// out_m = J u_n + shift_m (shift may be null); scal[0] = p . out (p may be null), scal[1] = out . out
+void launch_hk_j(const DevModel& M, const IpmVectors& V, const double* u_n, const double* shift_m, const double* p_m, double* out_m, cudaStream_t st);
+// x += alpha p, r -= alpha Sp, scal[1] = r . r
+void launch_hk_cg_update(const DevModel& M, const IpmVectors& V, double alpha, double* x, double* r, const double* p, const double* Sp, cudaStream_t st);
+// p = r + beta p (init: p = r, x = 0)
+void launch_hk_cg_dir(const DevModel& M, double beta, const double* r, double* p, double* x, int init, cudaStream_t st);
+void launch_hk_step(const DevModel& M, const IpmVectors& V, double mu, double tau, cudaStream_t st);
+void launch_hk_update(const DevModel& M, const IpmVectors& V, cudaStream_t st);
+void launch_fill(int64_t n, double v, double* out, cudaStream_t st);
+
 }  // namespace nmpc

@@ -29,6 +29,7 @@ void default_options(nmpc_options* o) {
     o->refine_steps = 0; o->globalization = 0;
     o->gamma_theta = 1e-5; o->gamma_phi = 1e-8; o->delta_sw = 1.0; o->s_theta = 1.1; o->s_phi = 2.3; o->eta_phi = 1e-8;
     o->theta_max_fact = 1e4; o->theta_min_fact = 1e-4; o->ls_max_backtracks = 30;
+    o->gamma_h = 1e6; o->cg_tol = 1e-10; o->cg_max_iter = 50;     // HyKKT (reading G21)
 }
 
 // =============================================================================================================
