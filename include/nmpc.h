@@ -112,6 +112,13 @@ typedef struct {
     double  gamma_h;             /* weight of the augmented-Lagrangian term in K_g = W + Sigma_x + eta I + gamma_h J^T J   */
     double  cg_tol;              /* CG on S = J K_g^-1 J^T stops at |r|_2 <= cg_tol |rhs|_2                                 */
     int32_t cg_max_iter;
+    /* ---- right-hand-side row: Eq. (22), L v = P b, computed INSIDE the numeric factorization ---- */
+    int32_t fuse_rhs;            /* 1: the analysed structure is [K b; b^T 0] (one extra variable ordered last), so that the
+                                    factorization leaves v = L^-1 P b in the last row of the panels and the Newton system of an
+                                    IPM iteration needs the backward solve (Eq. 24) only; nmpc_factor_rhs / nmpc_solve_fused
+                                    expose the same for a bare handle.  0: off.  -1 (default): on when the handle has a model.
+                                    nmpc_factor / nmpc_solve / nmpc_get_factor / nmpc_get_info behave the same either way (they
+                                    report the factor of K alone)                                                           */
 } nmpc_options;
 
 typedef struct {                 /* filled by nmpc_get_info; arrays are HOST pointers owned by the handle     */
@@ -127,7 +134,9 @@ typedef struct {                 /* filled by nmpc_get_info; arrays are HOST poi
     const int32_t* rows;         /* rows of each supernode in pivot order (first w are its own columns)       */
     const int32_t* super_parent; /* nsuper, -1 = root                                                         */
     const int32_t* super_level;  /* nsuper, 0 = leaf level                                                    */
-    const int32_t* etree_parent; /* n, elimination tree on pivot positions, -1 = root      */
+    const int32_t* etree_parent; /* n, elimination tree on pivot positions, -1 = root; with fused_rhs
+                                    the roots of K's forest point to n (the right-hand-side row)                        */
+    int32_t fused_rhs;           /* 1 if the handle carries the right-hand-side row (options.fuse_rhs)                   */
 } nmpc_sym_info;
 
 typedef struct {                 /* filled by nmpc_ipm_solve (HOST)                                           */
@@ -179,6 +188,13 @@ nmpc_status nmpc_factor(nmpc_handle h, const double* values_dev, double eta, int
 
 /* ---- Eq. (22)-(25): rhs_inout_dev DEVICE n*nrhs doubles (column-major), overwritten by K^-1 rhs.  Async.   */
 nmpc_status nmpc_solve(nmpc_handle h, double* rhs_inout_dev, int32_t nrhs);
+
+/* ---- Eq. (20)-(22) in one pass (handles with the right-hand-side row, options.fuse_rhs; else NMPC_E_STATE): numeric
+ *      Cholesky of K + eta I with b = rhs_dev (DEVICE, n doubles, copied) carried as an extra row, which leaves v = L^-1 P b
+ *      in the factor.  nmpc_solve_fused then runs the backward solve only: out_dev (DEVICE, n) <- P^T L^-T v = K^-1 b
+ *      (Eq. 24-25; async).  nmpc_solve stays valid on the same factorization for any other right-hand side.            */
+nmpc_status nmpc_factor_rhs(nmpc_handle h, const double* values_dev, const double* rhs_dev, double eta, int64_t* info_host);
+nmpc_status nmpc_solve_fused(nmpc_handle h, double* out_dev);
 
 /* ---- y = K x with the values last passed to nmpc_factor (+eta I), for residual checks.  Async.            */
 nmpc_status nmpc_kkt_multiply(nmpc_handle h, const double* x_dev, double* y_dev);

@@ -44,7 +44,7 @@ class nmpc_options(C.Structure):
                 + [(k, c_dbl) for k in ("gamma_theta", "gamma_phi", "delta_sw", "s_theta", "s_phi", "eta_phi", "theta_max_fact",
                                         "theta_min_fact")]
                 + [("ls_max_backtracks", c_i32), ("grid_limit", c_i32), ("epoch_limit", c_i32)]
-                + [("gamma_h", c_dbl), ("cg_tol", c_dbl), ("cg_max_iter", c_i32)])
+                + [("gamma_h", c_dbl), ("cg_tol", c_dbl), ("cg_max_iter", c_i32), ("fuse_rhs", c_i32)])
 
 
 class nmpc_sym_info(C.Structure):
@@ -52,7 +52,8 @@ class nmpc_sym_info(C.Structure):
                  ("flops", c_dbl), ("nsuper", c_i32), ("nlevels", c_i32), ("max_front", c_i32), ("max_width", c_i32),
                  ("n_large_fronts", c_i32), ("ordering_used", c_i32), ("analyze_ms", c_dbl)]
                 + [(k, c_vp) for k in ("perm", "super_start", "rows_ptr", "rows", "super_parent", "super_level",
-                                       "etree_parent")])
+                                       "etree_parent")]
+                + [("fused_rhs", c_i32)])
 
 
 class nmpc_stats(C.Structure):
@@ -80,6 +81,8 @@ SIGNATURES = {
     "nmpc_update_params_host": (c_i32, [c_vp, c_vp, c_vp]),
     "nmpc_factor": (c_i32, [c_vp, c_vp, c_dbl, P(c_i64)]),
     "nmpc_solve": (c_i32, [c_vp, c_vp, c_i32]),
+    "nmpc_factor_rhs": (c_i32, [c_vp, c_vp, c_vp, c_dbl, P(c_i64)]),
+    "nmpc_solve_fused": (c_i32, [c_vp, c_vp]),
     "nmpc_kkt_multiply": (c_i32, [c_vp, c_vp, c_vp]),
     "nmpc_ipm_solve": (c_i32, [c_vp, c_i32, c_i32, c_vp, P(nmpc_stats), c_vp, c_i32]),
     "nmpc_hykkt_solve": (c_i32, [c_vp, c_i32, c_i32, c_vp, P(nmpc_stats), c_vp, c_i32]),
@@ -200,6 +203,7 @@ def make_pattern(n, rowptr, colind):
 
 def _info_dict(info: nmpc_sym_info, copy_arrays=True):
     d = {k: getattr(info, k) for k, _ in nmpc_sym_info._fields_[:13]}
+    d["fused_rhs"] = info.fused_rhs
     if copy_arrays:
         def arr(ptr, count, ct):
             return np.ctypeslib.as_array(C.cast(ptr, P(ct)), shape=(count,)).copy()
@@ -321,6 +325,15 @@ class Handle:
 
     def solve(self, rhs_inout_dev, nrhs=1):
         self._ck(self.lib.nmpc_solve(self._h, _ptr(rhs_inout_dev), nrhs), "nmpc_solve")
+
+    def factor_rhs(self, values_dev, rhs_dev, eta=0.0, check=True):
+        info = c_i64(-1)
+        st = self.lib.nmpc_factor_rhs(self._h, _ptr(values_dev), _ptr(rhs_dev), float(eta), C.byref(info))
+        self._ck(st, "nmpc_factor_rhs", allow=() if check else (NMPC_E_NOT_SPD,))
+        return st, info.value
+
+    def solve_fused(self, out_dev):
+        self._ck(self.lib.nmpc_solve_fused(self._h, _ptr(out_dev)), "nmpc_solve_fused")
 
     def kkt_multiply(self, x_dev, y_dev):
         self._ck(self.lib.nmpc_kkt_multiply(self._h, _ptr(x_dev), _ptr(y_dev)), "nmpc_kkt_multiply")

@@ -37,7 +37,9 @@ struct nmpc_handle_s {
     IpmVectors V{};
     std::vector<void*> allocs;
     DagPlan F;
-    uint32_t epoch_f = 0, epoch_s = 0, epoch_limit = 1u << 16;    // call numbers of the epoch-valued completion flags
+    uint32_t epoch_f = 0, epoch_sf = 0, epoch_sb = 0, epoch_limit = 1u << 16;   // call numbers of the epoch-valued completion flags:
+                                       // factorization, forward half and backward half of the solves
+    bool rhs_row_valid = false;        // the factor holds v = L^-1 P b of the right-hand side a fused solve is asked for
     int n_big_fronts = 0;
     double* d_Kval = nullptr;          // values last factored (pattern order)
     double* d_x = nullptr;             // permuted right-hand side / solution
@@ -52,7 +54,7 @@ struct nmpc_handle_s {
     std::string err;
     cudaEvent_t ev[2] = {nullptr, nullptr};
     std::vector<cudaEvent_t> it_ev;    // per-iteration events of traced solves (created on first use)
-    double* d_par = nullptr;           // device {mu, tau, (uint32) factor call number, (uint32) solve call number}: read by the graph's kernels
+    double* d_par = nullptr;           // device {mu, tau, (uint32) factor call number, then (forward, backward) call numbers per solve}: read by the graph's kernels
     cudaGraphExec_t iter_graph = nullptr;   // one IPM iteration (S6-S10 + the next S2), see capture_iteration_graph
     bool graph_failed = false;
 };
@@ -232,13 +234,14 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
     std::vector<int4> stasks;
     stasks.reserve(2 * sk.size());
     for (const SK& t : sk) stasks.push_back(make_int4(t.type, t.s, t.I, 0));
+    const int32_t n_sfwd = (int32_t)stasks.size();
     for (size_t t = sk.size(); t-- > 0;)
         if (sk[t].type == 0 || sk[t].I < nbp[sk[t].s]) stasks.push_back(make_int4(sk[t].type, sk[t].s, sk[t].I, 1));
 
     DagPlan& F = h->F;
     const int64_t* tl = nullptr; const int4* t4 = nullptr;
     TRY(upload(h, tasks, &t4)); F.ftasks = t4; F.n_ftasks = (int32_t)tasks.size();
-    TRY(upload(h, stasks, &t4)); F.stasks = t4; F.n_stasks = (int32_t)stasks.size();
+    TRY(upload(h, stasks, &t4)); F.stasks = t4; F.n_stasks = (int32_t)stasks.size(); F.n_sfwd = n_sfwd;
     TRY(upload(h, cls, &F.cls)); TRY(upload(h, tbase, &F.tbase)); TRY(upload(h, bbase, &F.bbase));
     TRY(upload(h, target, &F.target)); TRY(upload(h, target_f, &F.target_f)); TRY(upload(h, target_b, &F.target_b));
     TRY(upload(h, tile_kptr, &tl)); F.tile_kptr = tl;
@@ -246,9 +249,9 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
     TRY(upload(h, cbnd, &F.cbnd));
     TRY(upload(h, S.sn_parent, &F.sn_parent));
     TRY(upload(h, ksrc, &h->D.kent_src)); TRY(upload(h, kdst, &h->D.kent_dst));
-    F.sync_words = 2 + 3 * (int64_t)ns + slots + 3 * bslots;
+    F.sync_words = 3 + 3 * (int64_t)ns + slots + 3 * bslots;
     TRY(dalloc(h, (size_t)F.sync_words, &F.sync));
-    F.fac_done = F.sync + 2; F.sol_done_f = F.fac_done + ns; F.sol_done_b = F.sol_done_f + ns;
+    F.fac_done = F.sync + 3; F.sol_done_f = F.fac_done + ns; F.sol_done_b = F.sol_done_f + ns;
     F.tile_done = F.sol_done_b + ns; F.blk_f = F.tile_done + slots; F.blk_b = F.blk_f + bslots; F.sub_done = F.blk_b + bslots;
 
 #ifdef NMPC_TRACE_BUILD                                      // measurement build: per-task timestamps (nmpc_get_task_trace, include/nmpc_aids.h)
@@ -268,29 +271,35 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
     return NMPC_OK;
 }
 
-// The next call number of the factor / solve kernels.  Both restart from 1 (all flags zeroed, in stream order) before any
+// The next call numbers of the factor / solve kernels.  All restart from 1 (all flags zeroed, in stream order) before any
 // counter can overflow.  The restart is decided with a margin of all call numbers of one IPM iteration (one factorization, 1 +
 // refine_steps solves), so the numbers reserved for one CUDA-graph replay always lie on the same side of a restart.
-nmpc_status next_epoch(nmpc_handle_s* h, bool factor, uint32_t* out) {
+nmpc_status next_factor_epoch(nmpc_handle_s* h, uint32_t* out) {
     const uint32_t per_iter = 2u + (uint32_t)std::max(0, h->opt.refine_steps);   // one factorization + (1 + refine_steps) solves
-    if (factor && std::max(h->epoch_f, h->epoch_s) + per_iter >= h->epoch_limit) {
+    if (std::max(h->epoch_f, std::max(h->epoch_sf, h->epoch_sb)) + per_iter >= h->epoch_limit) {
         CK(cudaMemsetAsync(h->F.sync, 0, (size_t)h->F.sync_words * sizeof(uint32_t), h->stream));
-        h->epoch_f = h->epoch_s = 0;
+        h->epoch_f = h->epoch_sf = h->epoch_sb = 0;
     }
-    if (!factor && h->epoch_s + 1 >= h->epoch_limit) {   // a long run of solves on one factorization: only the solve flags restart
+    *out = ++h->epoch_f;
+    return NMPC_OK;
+}
+// forward / backward call numbers of one solve; a fused solve (backward half only) gets *ef = 0
+nmpc_status next_solve_epochs(nmpc_handle_s* h, bool fused, uint32_t* ef, uint32_t* eb) {
+    if (std::max(h->epoch_sf, h->epoch_sb) + 1 >= h->epoch_limit) {   // a long run of solves on one factorization: only the solve flags restart
         const size_t off = (size_t)(h->F.sol_done_f - h->F.sync), cnt = (size_t)(h->F.tile_done - h->F.sol_done_f);
-        CK(cudaMemsetAsync(h->F.sync + 1, 0, sizeof(uint32_t), h->stream));
+        CK(cudaMemsetAsync(h->F.sync + 1, 0, 2 * sizeof(uint32_t), h->stream));
         CK(cudaMemsetAsync(h->F.sync + off, 0, cnt * sizeof(uint32_t), h->stream));
         CK(cudaMemsetAsync(h->F.blk_f, 0, (size_t)(h->F.sub_done - h->F.blk_f) * sizeof(uint32_t), h->stream));
-        h->epoch_s = 0;
+        h->epoch_sf = h->epoch_sb = 0;
     }
-    *out = factor ? ++h->epoch_f : ++h->epoch_s;
+    *eb = ++h->epoch_sb;
+    *ef = fused ? 0u : ++h->epoch_sf;
     return NMPC_OK;
 }
 
 nmpc_status run_factor(nmpc_handle_s* h, double eta, int64_t* info) {
     uint32_t epoch = 0;
-    TRY(next_epoch(h, true, &epoch));
+    TRY(next_factor_epoch(h, &epoch));
     launch_factor(h->D, h->F, h->d_Kval, eta, epoch, nullptr, h->stream); h->launches += 1;
     int32_t* flag = reinterpret_cast<int32_t*>(h->h_pinned + 16);
     CK(cudaMemcpyAsync(flag, h->D.fail_col, sizeof(int32_t), cudaMemcpyDeviceToHost, h->stream));
@@ -308,11 +317,18 @@ nmpc_status run_factor(nmpc_handle_s* h, double eta, int64_t* info) {
     return NMPC_OK;
 }
 
-nmpc_status run_solve(nmpc_handle_s* h, double* rhs) {       // in place, async
-    uint32_t epoch = 0;
-    TRY(next_epoch(h, false, &epoch));
-    launch_solve(h->D, h->F, rhs, h->d_x, epoch, nullptr, h->stream); h->launches += 1;
+nmpc_status run_solve(nmpc_handle_s* h, double* rhs, bool fused = false) {       // in place (fused: rhs is written only), async
+    uint32_t ef = 0, eb = 0;
+    TRY(next_solve_epochs(h, fused, &ef, &eb));
+    launch_solve(h->D, h->F, rhs, h->d_x, ef, eb, nullptr, fused, h->stream); h->launches += 1;
     return NMPC_OK;
+}
+// K^-1 b for the b of the IPM iteration (V.b): with the right-hand-side row b went through the factorization and only the
+// backward half runs; else b is copied and solved in place
+nmpc_status run_newton_solve(nmpc_handle_s* h) {
+    if (h->S.aug) return run_solve(h, h->V.dy, true);
+    CK(cudaMemcpyAsync(h->V.dy, h->V.b, sizeof(double) * h->M.n, cudaMemcpyDeviceToDevice, h->stream));
+    return run_solve(h, h->V.dy);
 }
 
 // One IPM iteration as a CUDA graph (opt.use_graph): parameter upload {mu, tau, call numbers} from pinned memory, S6 (Sigma, rhs),
@@ -337,12 +353,12 @@ nmpc_status capture_iteration_graph(nmpc_handle_s* h) {
     if (good) { launch_sigma_rhs(M, V, 0.0, h->d_par, st); good = launched(); }
     if (good) { launch_assemble_K(M, V.Jval, V.Wval, V.sigx, V.q, 0.0, V.Kval, st); good = launched(); }
     if (good) { launch_factor(h->D, h->F, h->d_Kval, 0.0, 0u, epo, st); good = launched(); }
-    if (good) good = ok(cudaMemcpyAsync(V.dy, V.b, sizeof(double) * M.n, cudaMemcpyDeviceToDevice, st));
-    if (good) { launch_solve(h->D, h->F, V.dy, h->d_x, 0u, epo, st); good = launched(); }
+    if (good && !h->S.aug) good = ok(cudaMemcpyAsync(V.dy, V.b, sizeof(double) * M.n, cudaMemcpyDeviceToDevice, st));
+    if (good) { launch_solve(h->D, h->F, V.dy, h->d_x, 0u, 0u, epo + 1, h->S.aug, st); good = launched(); }
     if (good) { launch_step(M, V, 0.0, 0.0, h->d_par, st); good = launched(); }
     for (int r = 0; good && r < h->opt.refine_steps; ++r) {      // iterative refinement: solve number r + 1 of this iteration
         launch_refine_residual(M, V, 0.0, h->D.fail_col, st); good = launched();
-        if (good) { launch_solve(h->D, h->F, V.rho, h->d_x, 0u, epo + 1 + r, st); good = launched(); }
+        if (good) { launch_solve(h->D, h->F, V.rho, h->d_x, 0u, 0u, epo + 3 + 2 * r, false, st); good = launched(); }
         if (good) { launch_add_correction(M, V, h->D.fail_col, st); good = launched(); }
         if (good) { launch_step(M, V, 0.0, 0.0, h->d_par, st); good = launched(); }
     }
@@ -422,7 +438,8 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
         nmpc_options o = h->opt;
         if (o.relax_small < 0) o.relax_small = small_variant ? 32 : 64;
         if (small_variant && o.nd_leaf <= 0) o.nd_leaf = 32;      // smaller dissection leaves: C1 factor + solve another -11 %
-        try { return analyze_symbolic(pattern, ocp, &o, S); }
+        const bool augment = o.fuse_rhs > 0 || (o.fuse_rhs < 0 && ocp && ocp->model != NMPC_MODEL_NONE);
+        try { return analyze_symbolic(pattern, ocp, &o, S, augment); }
         catch (const std::bad_alloc&) { S.error = "host allocation failed"; return NMPC_E_ALLOC; }
     };
     const int64_t n_hint = pattern ? pattern->n : (ocp ? (int64_t)ocp->N * (ocp->nx + ocp->nu) : 0);
@@ -446,7 +463,7 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
         CK(configure_solve_kernels(smem_optin, small_max_r, &solve_ctas, &solve_smem, &sbuf));
         h->F.sbuf = sbuf;
         DevSym& D = h->D;
-        D.ns = S.ns; D.n = S.n;
+        D.ns = S.ns; D.n = S.n; D.aug_col = S.aug ? (int32_t)S.n : -1;
         TRY(upload(h, S.sn_start, &D.sn_start)); TRY(upload(h, S.rows_ptr, &D.rows_ptr)); TRY(upload(h, S.rows, &D.rows));
         TRY(upload(h, S.child_ptr, &D.child_ptr)); TRY(upload(h, S.child_idx, &D.child_idx));
         TRY(upload(h, S.rel_ptr, &D.rel_ptr)); TRY(upload(h, S.rel, &D.rel));
@@ -455,9 +472,9 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
         TRY(upload(h, S.perm, &D.perm));
         TRY(dalloc(h, (size_t)S.panel_ptr.back() + 4 * TILE, &D.L)); TRY(dalloc(h, (size_t)S.upd_ptr.back(), &D.U, false));
         TRY(dalloc(h, (size_t)S.rel_ptr.back(), &D.ctr)); TRY(dalloc(h, 1, &D.fail_col));
-        TRY(dalloc(h, (size_t)S.n, &D.dinv));
+        TRY(dalloc(h, (size_t)S.nt, &D.dinv));
         launch_reset_fail(D, h->stream);
-        TRY(dalloc(h, (size_t)S.nnzK, &h->d_Kval)); TRY(dalloc(h, (size_t)S.n, &h->d_x));
+        TRY(dalloc(h, (size_t)S.nnzKa, &h->d_Kval)); TRY(dalloc(h, (size_t)S.nt, &h->d_x));   // [K values | b | 0] with the right-hand-side row
         TRY(build_plan(h, small_max_r, ctas_per_sm, factor_smem, solve_ctas, solve_smem, num_sms));
         // symmetric CSR of K for nmpc_kkt_multiply
         {
@@ -509,7 +526,9 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
             TRY(dalloc(h, (size_t)M.nnzJ, &V.Jval)); TRY(dalloc(h, (size_t)M.nnzW, &V.Wval));
             V.Kval = h->d_Kval;
             TRY(dalloc(h, m, &V.r_pp)); TRY(dalloc(h, m, &V.r_pm)); TRY(dalloc(h, m, &V.q)); TRY(dalloc(h, m, &V.t));
-            TRY(dalloc(h, n, &V.sigx)); TRY(dalloc(h, n, &V.b)); TRY(dalloc(h, n, &V.dy));
+            TRY(dalloc(h, n, &V.sigx)); TRY(dalloc(h, n, &V.dy));
+            if (S.aug) V.b = h->d_Kval + S.nnzK;              // the right-hand side of Eq. (17) is written straight into the factorization's value array
+            else TRY(dalloc(h, n, &V.b));
             TRY(dalloc(h, m, &V.dsp)); TRY(dalloc(h, m, &V.dsm)); TRY(dalloc(h, m, &V.dwp)); TRY(dalloc(h, m, &V.dwm));
             TRY(dalloc(h, n, &V.dzL)); TRY(dalloc(h, n, &V.dzU));
             TRY(dalloc(h, (size_t)RED_BLOCKS * 8, &V.partial)); TRY(dalloc(h, (size_t)NSCAL, &V.scal));
@@ -587,8 +606,29 @@ nmpc_status nmpc_get_factor(nmpc_handle h, double* panels_host) {
     if (!h || !panels_host) return NMPC_E_ARG;
     DeviceGuard dg(h);
     if (!h->factored) { h->err = "no successful factorization"; return NMPC_E_STATE; }
-    CK(cudaMemcpyAsync(panels_host, h->D.L, (size_t)h->S.panel_ptr.back() * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
-    CK(cudaStreamSynchronize(h->stream));
+    const Symbolic& S = h->S;
+    if (!S.aug) {
+        CK(cudaMemcpyAsync(panels_host, h->D.L, (size_t)S.panel_ptr.back() * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+        CK(cudaStreamSynchronize(h->stream));
+        return NMPC_OK;
+    }
+    // with the right-hand-side row: repack without that row / pivot (the layout nmpc_get_info describes)
+    std::vector<double> all;
+    try { all.resize((size_t)S.panel_ptr.back()); } catch (const std::bad_alloc&) { h->err = "host allocation failed"; return NMPC_E_ALLOC; }
+    CK(cudaMemcpy(all.data(), h->D.L, all.size() * sizeof(double), cudaMemcpyDeviceToHost));
+    int64_t off = 0;
+    for (int32_t s = 0; s < S.ns; ++s) {
+        const int64_t r = S.rows_ptr[s + 1] - S.rows_ptr[s], ld = panel_ld(r);
+        const int64_t rv = S.v_rows_ptr[s + 1] - S.v_rows_ptr[s], wv = S.v_sn_start[s + 1] - S.v_sn_start[s], ldv = panel_ld(rv);
+        // the row left out is the last one of the front; in the supernode that holds its pivot it is the last column as well
+        for (int64_t j = 0; j < wv; ++j) {
+            const double* src = all.data() + S.panel_ptr[s] + j * ld;
+            double* dst = panels_host + off + j * ldv;
+            for (int64_t i = 0; i < rv; ++i) dst[i] = src[i];
+            if (ldv > rv) dst[rv] = 0.0;
+        }
+        off += ldv * wv;
+    }
     return NMPC_OK;
 }
 
@@ -597,7 +637,30 @@ nmpc_status nmpc_factor(nmpc_handle h, const double* values_dev, double eta, int
     DeviceGuard dg(h);
     if (values_dev != h->d_Kval)
         CK(cudaMemcpyAsync(h->d_Kval, values_dev, (size_t)h->S.nnzK * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+    h->rhs_row_valid = false;
     return run_factor(h, eta, info_host);
+}
+
+nmpc_status nmpc_factor_rhs(nmpc_handle h, const double* values_dev, const double* rhs_dev, double eta, int64_t* info_host) {
+    if (!h || !values_dev || !rhs_dev) return NMPC_E_ARG;
+    DeviceGuard dg(h);
+    if (!h->S.aug) { h->err = "nmpc_factor_rhs needs a handle created with options.fuse_rhs"; return NMPC_E_STATE; }
+    if (values_dev != h->d_Kval)
+        CK(cudaMemcpyAsync(h->d_Kval, values_dev, (size_t)h->S.nnzK * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+    if (rhs_dev != h->d_Kval + h->S.nnzK)
+        CK(cudaMemcpyAsync(h->d_Kval + h->S.nnzK, rhs_dev, (size_t)h->S.n * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+    const nmpc_status st = run_factor(h, eta, info_host);
+    h->rhs_row_valid = st == NMPC_OK;
+    return st;
+}
+
+nmpc_status nmpc_solve_fused(nmpc_handle h, double* out_dev) {
+    if (!h || !out_dev) return NMPC_E_ARG;
+    DeviceGuard dg(h);
+    if (!h->S.aug || !h->factored || !h->rhs_row_valid) { h->err = "nmpc_solve_fused needs a successful nmpc_factor_rhs"; return NMPC_E_STATE; }
+    TRY(run_solve(h, out_dev, true));
+    CK(cudaGetLastError());
+    return NMPC_OK;
 }
 
 nmpc_status nmpc_solve(nmpc_handle h, double* rhs, int32_t nrhs) {
@@ -833,8 +896,7 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
     };
     auto solve_step_update = [&](double mu_, double tau_) -> nmpc_status {
         pt.begin(&S.ms_solve, 3);                                                 // S8: Eq. (22)-(25)
-        CK(cudaMemcpyAsync(V.dy, V.b, sizeof(double) * M.n, cudaMemcpyDeviceToDevice, st));
-        TRY(run_solve(h, V.dy));
+        TRY(run_newton_solve(h));
         pt.end();
         pt.begin(&S.ms_vector, 4);
         launch_step(M, V, mu_, tau_, nullptr, st); h->launches += 1;                    // S8-S9
@@ -908,8 +970,8 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
             double* hp = h->h_pinned + 24;
             hp[0] = mu; hp[1] = tau;
             uint32_t* he = reinterpret_cast<uint32_t*>(hp + 2);  // call numbers: factorization, then 1 + refine_steps solves
-            TRY(next_epoch(h, true, &he[0]));
-            for (int r = 0; r <= o.refine_steps; ++r) TRY(next_epoch(h, false, &he[1 + r]));
+            TRY(next_factor_epoch(h, &he[0]));
+            for (int r = 0; r <= o.refine_steps; ++r) TRY(next_solve_epochs(h, r == 0 && h->S.aug, &he[1 + 2 * r], &he[2 + 2 * r]));
             CK(cudaGraphLaunch(h->iter_graph, st));
             h->launches += 10 + 4 * o.refine_steps;
             ++nfact;
@@ -928,7 +990,7 @@ nmpc_status nmpc_ipm_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double* 
         ++nfact;
         if (async) {
             uint32_t epoch = 0;
-            TRY(next_epoch(h, true, &epoch));
+            TRY(next_factor_epoch(h, &epoch));
             launch_factor(h->D, h->F, h->d_Kval, 0.0, epoch, nullptr, st); h->launches += 1;
             h->eta_cur = 0.0;
             pending = true; pend_mu = mu; pend_tau = tau;
@@ -1066,8 +1128,9 @@ nmpc_status nmpc_hykkt_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double
         if (fs != NMPC_OK) return fs;
         if (eta > 0.0) eta_last = eta;
         // u = K_g^-1 b_g;  CG on S dlam = J u - r2 = J u + c;  dy = K_g^-1 (b_g - J^T dlam)
-        CK(cudaMemcpyAsync(V.dy, V.b, sizeof(double) * M.n, cudaMemcpyDeviceToDevice, st));
-        TRY(kg_solve(V.dy));
+        pt.begin(&S.ms_solve, 3);
+        TRY(run_newton_solve(h));                                              // b_g went through the factorization
+        pt.end();
         int ncg = 0;
         {
             double* r = V.r_pp; double* p = V.r_pm; double* Sp = V.t; double* x = V.dwp;

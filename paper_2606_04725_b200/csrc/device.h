@@ -18,6 +18,8 @@ namespace nmpc {
 struct DevSym {                   // device copies of the symbolic arrays (symbolic.h)
     int32_t ns = 0;
     int64_t n = 0;
+    int32_t aug_col = -1;         // pivot position (== original index n) of the right-hand-side row (symbolic.h), -1 = none: its
+                                  // pivot is taken as 1 without a test, the solves treat its right-hand side / solution as 0
     const int32_t* sn_start = nullptr;
     const int64_t* rows_ptr = nullptr;
     const int32_t* rows = nullptr;
@@ -66,11 +68,12 @@ __host__ __device__ inline int tile_nbu(int w, int r) {
 //                 dir 0 = forward (L v = P b), 1 = backward (L^T x = v); forward tasks first, backward = reversed order
 // Completion flags are EPOCH-valued (no reset between calls): call number e stores e into a flag and adds 1 to a counter,
 // so "done in this call" is flag >= e, counter >= e * target; the claim counter advances by ntasks + grid per call.
+// The forward and the backward half of the solves have their own call numbers (a fused solve runs the backward half only).
 struct DagPlan {
     const int4* ftasks = nullptr;        // factorization
     int32_t n_ftasks = 0;
-    const int4* stasks = nullptr;        // solves
-    int32_t n_stasks = 0;
+    const int4* stasks = nullptr;        // solves: n_sfwd forward tasks, then the backward tasks
+    int32_t n_stasks = 0, n_sfwd = 0;
     const int32_t* cls = nullptr;        // ns: 0 small, 1 tiled
     const int32_t* tbase = nullptr;      // ns: base of the front's (nbp x nbt + 1) slots in tile_done / tile_kptr
     const int32_t* bbase = nullptr;      // ns: base of the front's nbp slots in blk_f / blk_b
@@ -81,7 +84,7 @@ struct DagPlan {
     const int64_t* cb_ptr = nullptr;     // ns: offset into cbnd of the child's block boundaries in its (tiled) parent, else -1
     const int32_t* cbnd = nullptr;
     const int32_t* sn_parent = nullptr;  // ns
-    uint32_t* sync = nullptr;            // [0] factor claim, [1] solve claim, then the arrays below
+    uint32_t* sync = nullptr;            // [0] factor claim, [1] forward-solve claim, [2] backward-solve claim, then the arrays below
     uint32_t* fac_done = nullptr;        // ns
     uint32_t* sol_done_f = nullptr;      // ns
     uint32_t* sol_done_b = nullptr;      // ns
@@ -109,9 +112,11 @@ void launch_factor(const DevSym& D, const DagPlan& F, const double* Kval, double
 void launch_reset_fail(const DevSym& D, cudaStream_t st);                                   // fail_col = INT_MAX
 // ---- solve.cu ----
 cudaError_t configure_solve_kernels(int max_smem_bytes, int small_max_r, int* ctas_per_sm, size_t* smem_bytes, int* sbuf_doubles);
-// rhs_inout (original ordering, n doubles) is overwritten by K^-1 rhs; x is the handle's permuted work vector
-void launch_solve(const DevSym& D, const DagPlan& F, double* rhs_inout, double* x, uint32_t epoch, const uint32_t* epoch_dev,
-                  cudaStream_t st);
+// rhs_inout (original ordering, n doubles) is overwritten by K^-1 rhs; x is the handle's permuted work vector.
+// epoch_f / epoch_b: call numbers of the forward / backward half (epoch_dev, may be null: two device words that override them).
+// fused: backward half only, v = L^-1 P b is read from the right-hand-side row of the factor and rhs_inout is written only.
+void launch_solve(const DevSym& D, const DagPlan& F, double* rhs_inout, double* x, uint32_t epoch_f, uint32_t epoch_b,
+                  const uint32_t* epoch_dev, bool fused, cudaStream_t st);
 
 // ---- ipm.cu ----
 struct DevModel {                 // device copies of the model maps (symbolic.h: ModelMaps) + parameters

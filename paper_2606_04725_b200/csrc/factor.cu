@@ -107,7 +107,7 @@ __device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
 // (no divergence).  Requires r <= NT.  A pivot <= 0 or non-finite (reading G11) is replaced by 1 and reported.
 // =============================================================================================================
 template <class ColFn>
-__device__ __forceinline__ void factor_diag8(ColFn colp, int j0, int jb, int c0, int32_t* fail_col, double* dinv, double* s_inv) {
+__device__ __forceinline__ void factor_diag8(ColFn colp, int j0, int jb, int c0, int aug_col, int32_t* fail_col, double* dinv, double* s_inv) {
     const int lane = threadIdx.x & 31;
     double Dg[8][8], inv[8];
     if (jb == 8) {
@@ -128,7 +128,8 @@ __device__ __forceinline__ void factor_diag8(ColFn colp, int j0, int jb, int c0,
     int badc = 8;
 #pragma unroll
     for (int c = 0; c < 8; ++c) {
-        const double d = Dg[c][c];
+        // the right-hand-side row (device.h: aug_col) is the last pivot of all: taken as 1, never tested
+        const double d = (c0 + j0 + c == aug_col) ? 1.0 : Dg[c][c];
         const bool bad = !(d >= 2.2250738585072014e-308) || isinf(d);          // <= 0, non-finite (or subnormal): reading G11
         if (bad && c < jb && badc == 8) badc = c;
         const double y = rsqrt_newton(d);                                      // speculative: the test above is off the chain
@@ -161,12 +162,12 @@ struct NoPublish { __device__ __forceinline__ void operator()(int, int) const {}
 // pub(j0, jb) is called by all threads right after the barrier that ends the row solve of columns [j0, j0 + jb): those columns
 // are final from then on (the diagonal tile of a tiled front streams them to the TRSM tiles of its block column)
 template <class ColFn, class Pub = NoPublish>
-__device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, int32_t* fail_col, double* dinv, Pub pub = Pub()) {
+__device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, int aug_col, int32_t* fail_col, double* dinv, Pub pub = Pub()) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gid = lane >> 2, tig = lane & 3;
     constexpr int NW1 = NT / 32 - 1;                     // warps 1..7 share the tiles warp 0 does not take
     __shared__ double s_inv[8];
     const int rl = r - 1;
-    if (warp == 0) factor_diag8(colp, 0, min(8, w), c0, fail_col, dinv, s_inv);
+    if (warp == 0) factor_diag8(colp, 0, min(8, w), c0, aug_col, fail_col, dinv, s_inv);
     __syncthreads();
     for (int p0 = 0; p0 < w; p0 += 32) {
         const int p1 = min(w, p0 + 32);
@@ -246,7 +247,7 @@ __device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, i
                 if (warp == 0) {
                     pair(0, ntile);                      // the tile of the next diagonal block, then that block's factorization
                     __syncwarp();
-                    factor_diag8(colp, t0, min(8, p1 - t0), c0, fail_col, dinv, s_inv);
+                    factor_diag8(colp, t0, min(8, p1 - t0), c0, aug_col, fail_col, dinv, s_inv);
                 } else {
                     for (int q = warp; q < ntile; q += 2 * NW1) pair(q, q + NW1);
                 }
@@ -296,7 +297,7 @@ __device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, i
                 if (warp == 0) {
                     pair(0, ntile);
                     __syncwarp();
-                    if (has_next) factor_diag8(colp, p1, min(8, w - p1), c0, fail_col, dinv, s_inv);
+                    if (has_next) factor_diag8(colp, p1, min(8, w - p1), c0, aug_col, fail_col, dinv, s_inv);
                 } else {
                     for (int q = warp; q < ntile; q += 2 * NW1) pair(q, q + NW1);
                 }
@@ -557,7 +558,7 @@ __device__ __forceinline__ void small_front_task(const DevSym& D, const DagPlan&
     }
     __syncthreads();
     TRACE(2);
-    partial_chol(colp, r, w, c0, D.fail_col, D.dinv);
+    partial_chol(colp, r, w, c0, D.aug_col, D.fail_col, D.dinv);
     TRACE(3);
     const int ld = ld_even(r), m = r - w;
     double* Uo = D.U + D.upd_ptr[s];                     // the update matrix first: it is all the parent waits for
@@ -752,7 +753,7 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
                     if (tid == NT - 1) { __threadfence(); st_release(sub, sbase + (uint32_t)(js >> 3) + 1u); }
                 }
             };
-            partial_chol([Cs](int j) { return Cs + j * CLD; }, nj, nj, c0 + j0, D.fail_col, D.dinv, pub);
+            partial_chol([Cs](int j) { return Cs + j * CLD; }, nj, nj, c0 + j0, D.aug_col, D.fail_col, D.dinv, pub);
             TRACE(3);
         } else {
             double* Ls = pipe;

@@ -13,6 +13,9 @@
 // The permutations are fused: forward tasks read b[perm[.]], backward tasks write b[perm[.]] (in place, no hazard: a
 // supernode's entries of b are read by its own forward task only).  Divisions by L_jj are multiplications by the reciprocals
 // the factorization stored (dinv).  fp64, fixed summation order -> bitwise reproducible.
+// Right-hand-side row (options.fuse_rhs, symbolic.h): the structure has one extra last variable whose row of L holds
+// v = L^-1 P b of the b that went through the factorization.  A FUSED solve runs the backward tasks only and takes v from that
+// row (the last row of every panel); a general solve treats the extra variable's right-hand side and solution as 0.
 #include "device.h"
 
 namespace nmpc {
@@ -59,6 +62,13 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
+__device__ __forceinline__ double rhs_at(const DevSym& D, const double* b, int col) {      // P b at pivot position col
+    return col == D.aug_col ? 0.0 : b[D.perm[col]];
+}
+__device__ __forceinline__ void put_solution(const DevSym& D, double* b, int col, double v) {
+    if (col != D.aug_col) b[D.perm[col]] = v;
+}
+
 struct Sn {                             // per-supernode scalars every task needs
     int c0, w, r, ld;
     const double* P;
@@ -101,7 +111,7 @@ __device__ __forceinline__ void fwd_small(const DevSym& D, const DagPlan& F, int
     const int nblk = (q.w + SB - 1) / SB;
     stage_block(D, q, 0, sm, F.sbuf);
     if (nblk > 1) stage_block(D, q, 1, sm, F.sbuf);
-    for (int i = tid; i < q.r; i += NT) t[i] = (i < q.w) ? b[D.perm[q.c0 + i]] : 0.0;
+    for (int i = tid; i < q.r; i += NT) t[i] = (i < q.w) ? rhs_at(D, b, q.c0 + i) : 0.0;
     const int ch0 = D.child_ptr[s], ch1 = D.child_ptr[s + 1], nch = ch1 - ch0;
     // child table + the relative indices of all children: fetched BEFORE the children are waited for (static data); the
     // contributions are then loaded in one round trip and added child by child (fixed order)
@@ -228,7 +238,7 @@ __device__ __forceinline__ void fwd_tiled(const DevSym& D, const DagPlan& F, int
             if (lane + 32 < ni) d1 = __ldcg(D.dinv + q.c0 + i0 + lane + 32);
         }
     }
-    if (tid < TILE) tI[tid] = (pivot && tid < ni) ? b[D.perm[q.c0 + i0 + tid]] : 0.0;
+    if (tid < TILE) tI[tid] = (pivot && tid < ni) ? rhs_at(D, b, q.c0 + i0 + tid) : 0.0;
     const int ch0 = D.child_ptr[s], ch1 = D.child_ptr[s + 1];
     if (I == 0) {                                        // block rows I > 0 inherit this through the flag of y_0
         for (int ci = ch0 + tid; ci < ch1; ci += NT) { const int c = D.child_idx[ci]; spin_until_ge(F.sol_done_f + c, epoch * (uint32_t)F.target_f[c]); }
@@ -323,7 +333,7 @@ __device__ __forceinline__ void fwd_tiled(const DevSym& D, const DagPlan& F, int
 }
 
 // ---------------- backward, whole small supernode ----------------
-__device__ __forceinline__ void bwd_small(const DevSym& D, const DagPlan& F, int s, double* b, double* x, uint32_t epoch, double* sm, unsigned long long* tr) {
+__device__ __forceinline__ void bwd_small(const DevSym& D, const DagPlan& F, int s, double* b, double* x, uint32_t ef, uint32_t epoch, bool fused, double* sm, unsigned long long* tr) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = NT / 32;
     const Sn q = sn_of(D, s);
     double* t = sm;
@@ -333,13 +343,14 @@ __device__ __forceinline__ void bwd_small(const DevSym& D, const DagPlan& F, int
     if (nblk > 1) stage_block(D, q, nblk - 2, sm, F.sbuf);
     const int myrow = tid < q.r ? q.rows[tid] : 0;       // q.r <= SMALL_ROWS_MAX < NT: one front row per thread
     if (tid == 0) {
-        spin_until_ge(F.sol_done_f + s, epoch * (uint32_t)F.target_f[s]);
+        if (!fused) spin_until_ge(F.sol_done_f + s, ef * (uint32_t)F.target_f[s]);
         const int p = F.sn_parent[s];
         if (p >= 0) spin_until_ge(F.sol_done_b + p, epoch * (uint32_t)F.target_b[p]);
     }
     __syncthreads();
     STRACE(1);
-    if (tid < q.r) t[tid] = __ldcg(x + myrow);
+    // own columns: v from the forward solve, or (fused) from the right-hand-side row of the panel; rows below: the ancestors' x
+    if (tid < q.r) t[tid] = myrow == D.aug_col ? 0.0 : (fused && tid < q.w) ? __ldcg(q.P + (q.r - 1) + (int64_t)tid * q.ld) : __ldcg(x + myrow);
     STRACE(2);
     for (int k = nblk - 1; k >= 0; --k) {
         const int j0 = k * SB, nb = min(SB, q.w - j0), ldb = q.ld - j0;
@@ -395,14 +406,14 @@ __device__ __forceinline__ void bwd_small(const DevSym& D, const DagPlan& F, int
     }
     __syncthreads();
     STRACE(3);
-    for (int i = tid; i < q.w; i += NT) { x[q.c0 + i] = t[i]; b[D.perm[q.c0 + i]] = t[i]; }
+    for (int i = tid; i < q.w; i += NT) { x[q.c0 + i] = t[i]; put_solution(D, b, q.c0 + i, t[i]); }
     __syncthreads();
     if (tid == 0) { __threadfence(); red_release_add(F.sol_done_b + s, 1u); }
 }
 
 // ---------------- backward, block column J of a tiled supernode ----------------
 // x_J = L(J,J)^-T (y_J - sum_{I>J} L(I,J)^T x_I): the tile L(I-1,J) is loaded into registers before the task waits for x_I.
-__device__ __forceinline__ void bwd_tiled(const DevSym& D, const DagPlan& F, int s, int J, double* b, double* x, uint32_t epoch, double* sm) {
+__device__ __forceinline__ void bwd_tiled(const DevSym& D, const DagPlan& F, int s, int J, double* b, double* x, uint32_t ef, uint32_t epoch, bool fused, double* sm) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const Sn q = sn_of(D, s);
     const int nbp = tile_nbp(q.w), nbt = nbp + tile_nbu(q.w, q.r);
@@ -431,7 +442,7 @@ __device__ __forceinline__ void bwd_tiled(const DevSym& D, const DagPlan& F, int
     };
     if (nbt - 1 > J) load_tile(nbt - 1, cur);
     if (tid == 0) {
-        spin_until_ge(F.sol_done_f + s, epoch * (uint32_t)F.target_f[s]);
+        if (!fused) spin_until_ge(F.sol_done_f + s, ef * (uint32_t)F.target_f[s]);
         const int p = F.sn_parent[s];
         if (p >= 0) spin_until_ge(F.sol_done_b + p, epoch * (uint32_t)F.target_b[p]);   // the rows below belong to finished ancestors
     }
@@ -464,7 +475,11 @@ __device__ __forceinline__ void bwd_tiled(const DevSym& D, const DagPlan& F, int
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
         const int c = warp * 8 + e;
-        if (lane == 0 && c < nj) zs[c] = __ldcg(x + q.c0 + j0 + c) - v;
+        if (lane == 0 && c < nj) {
+            const int col = q.c0 + j0 + c;
+            const double yc = col == D.aug_col ? 0.0 : fused ? __ldcg(q.P + (q.r - 1) + (int64_t)(j0 + c) * q.ld) : __ldcg(x + col);
+            zs[c] = yc - v;
+        }
     }
     __syncthreads();
     if (warp == 0) {
@@ -497,24 +512,39 @@ __device__ __forceinline__ void bwd_tiled(const DevSym& D, const DagPlan& F, int
                 z0 = (j < min(nj, 32) && lane < j) ? fma(-la[e], xj, z0) : z0;
             }
         }
-        if (lane < nj) { x[q.c0 + j0 + lane] = z0; b[D.perm[q.c0 + j0 + lane]] = z0; }
-        if (h1) { x[q.c0 + j0 + lane + 32] = z1; b[D.perm[q.c0 + j0 + lane + 32]] = z1; }
+        if (lane < nj) { x[q.c0 + j0 + lane] = z0; put_solution(D, b, q.c0 + j0 + lane, z0); }
+        if (h1) { x[q.c0 + j0 + lane + 32] = z1; put_solution(D, b, q.c0 + j0 + lane + 32, z1); }
         __syncwarp();
         if (lane == 0) { __threadfence(); st_release(bb + J, epoch); red_release_add(F.sol_done_b + s, 1u); }
     }
 }
 
-__global__ void __launch_bounds__(NT, 2) solve_dag_kernel(DevSym D, DagPlan F, double* b, double* x, uint32_t epoch, const uint32_t* __restrict__ epoch_dev) {
+__global__ void __launch_bounds__(NT, 2) solve_dag_kernel(DevSym D, DagPlan F, double* b, double* x, uint32_t ef, uint32_t eb,
+                                                             const uint32_t* __restrict__ epoch_dev, int fused) {
     extern __shared__ __align__(16) double sm[];
-    __shared__ int s_task;
-    if (epoch_dev) epoch = epoch_dev[1];                 // graph replay: the call number comes from device memory
-    const uint32_t base = (epoch - 1u) * (uint32_t)(F.n_stasks + (int)gridDim.x);
+    __shared__ int s_task, s_phase;
+    if (epoch_dev) { ef = epoch_dev[0]; eb = epoch_dev[1]; }   // graph replay: the call numbers come from device memory
+    const int n_fwd = F.n_sfwd, n_bwd = F.n_stasks - F.n_sfwd;
+    const uint32_t base_f = (ef - 1u) * (uint32_t)(n_fwd + (int)gridDim.x), base_b = (eb - 1u) * (uint32_t)(n_bwd + (int)gridDim.x);
+    if (threadIdx.x == 0) s_phase = fused ? 1 : 0;
     while (true) {
         __syncthreads();
-        if (threadIdx.x == 0) s_task = (int)(atomicAdd(F.sync + 1, 1u) - base);
+        if (threadIdx.x == 0) {
+            // the forward list is drained first (every CTA overshoots its counter exactly once), then the backward list
+            int t = -1;
+            if (s_phase == 0) {
+                t = (int)(atomicAdd(F.sync + 1, 1u) - base_f);
+                if (t < 0 || t >= n_fwd) { s_phase = 1; t = -1; }
+            }
+            if (s_phase == 1) {
+                t = (int)(atomicAdd(F.sync + 2, 1u) - base_b);
+                t = (t < 0 || t >= n_bwd) ? -1 : n_fwd + t;
+            }
+            s_task = t;
+        }
         __syncthreads();
         const int t = s_task;
-        if (t < 0 || t >= F.n_stasks) break;
+        if (t < 0) break;
         const int4 tk = F.stasks[t];
 #ifdef NMPC_TRACE_BUILD
         unsigned long long* tr = F.strace ? F.strace + (size_t)t * 8 : nullptr;
@@ -522,8 +552,8 @@ __global__ void __launch_bounds__(NT, 2) solve_dag_kernel(DevSym D, DagPlan F, d
 #else
         unsigned long long* tr = nullptr;
 #endif
-        if (tk.w == 0) { if (tk.x == 0) fwd_small(D, F, tk.y, b, x, epoch, sm, tr); else fwd_tiled(D, F, tk.y, tk.z, b, x, epoch, sm); }
-        else           { if (tk.x == 0) bwd_small(D, F, tk.y, b, x, epoch, sm, tr); else bwd_tiled(D, F, tk.y, tk.z, b, x, epoch, sm); }
+        if (tk.w == 0) { if (tk.x == 0) fwd_small(D, F, tk.y, b, x, ef, sm, tr); else fwd_tiled(D, F, tk.y, tk.z, b, x, ef, sm); }
+        else           { if (tk.x == 0) bwd_small(D, F, tk.y, b, x, ef, eb, fused != 0, sm, tr); else bwd_tiled(D, F, tk.y, tk.z, b, x, ef, eb, fused != 0, sm); }
         STRACE(4);
     }
 }
@@ -547,9 +577,9 @@ cudaError_t configure_solve_kernels(int max_smem_bytes, int small_max_r, int* ct
     return cudaSuccess;
 }
 
-void launch_solve(const DevSym& D, const DagPlan& F, double* rhs_inout, double* x, uint32_t epoch, const uint32_t* epoch_dev,
-                  cudaStream_t st) {
-    if (F.n_stasks > 0) solve_dag_kernel<<<F.sgrid, NT, F.ssmem, st>>>(D, F, rhs_inout, x, epoch, epoch_dev);
+void launch_solve(const DevSym& D, const DagPlan& F, double* rhs_inout, double* x, uint32_t epoch_f, uint32_t epoch_b,
+                  const uint32_t* epoch_dev, bool fused, cudaStream_t st) {
+    if (F.n_stasks > 0) solve_dag_kernel<<<F.sgrid, NT, F.ssmem, st>>>(D, F, rhs_inout, x, epoch_f, epoch_b, epoch_dev, fused ? 1 : 0);
 }
 
 }  // namespace nmpc

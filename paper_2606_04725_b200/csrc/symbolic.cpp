@@ -30,6 +30,7 @@ void default_options(nmpc_options* o) {
     o->gamma_theta = 1e-5; o->gamma_phi = 1e-8; o->delta_sw = 1.0; o->s_theta = 1.1; o->s_phi = 2.3; o->eta_phi = 1e-8;
     o->theta_max_fact = 1e4; o->theta_min_fact = 1e-4; o->ls_max_backtracks = 30;
     o->gamma_h = 1e6; o->cg_tol = 1e-10; o->cg_max_iter = 50;     // HyKKT (reading G21)
+    o->fuse_rhs = -1;              // auto: the right-hand-side row is carried through the factorization when the handle has a model
 }
 
 // =============================================================================================================
@@ -493,7 +494,7 @@ static bool validate_pattern(const nmpc_pattern* P, std::string& err) {
     return true;
 }
 
-nmpc_status analyze_symbolic(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const nmpc_options* opt_in, Symbolic& S) {
+nmpc_status analyze_symbolic(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const nmpc_options* opt_in, Symbolic& S, bool augment) {
     auto t0 = std::chrono::steady_clock::now();
     nmpc_options opt;
     if (opt_in) opt = *opt_in; else default_options(&opt);
@@ -538,23 +539,41 @@ nmpc_status analyze_symbolic(const nmpc_pattern* pattern, const nmpc_ocp* ocp, c
     }
     if ((int64_t)perm.size() != n) { S.error = "internal: ordering lost variables"; return NMPC_E_ARG; }
 
+    // ---------------- right-hand-side row (symbolic.h): [K b; b^T 0], the extra variable n ordered last ----------------
+    // Its entries take the value indices nnzK .. nnzK + n (the CSR order of the augmented pattern), i.e. the value array
+    // of the numeric factorization is [K values | b | 0].  The ordering above was computed on K alone.
+    const int64_t nt = n + (augment ? 1 : 0);
+    S.aug = augment; S.nt = nt;
+    Csr Kaug;
+    if (augment) {
+        if (S.nnzK + n + 1 > INT32_MAX) { S.error = "nnz(K) too large for int32 value indices"; return NMPC_E_ALLOC; }
+        Kaug.nrows = Kaug.ncols = nt;
+        Kaug.ptr = S.K.ptr; Kaug.ptr.push_back(S.nnzK + n + 1);
+        Kaug.idx = S.K.idx; Kaug.idx.resize(S.nnzK + n + 1);
+        std::iota(Kaug.idx.begin() + S.nnzK, Kaug.idx.end(), 0);
+        perm.push_back((int32_t)n);
+    }
+    const Csr& Kf = augment ? Kaug : S.K;
+    S.nnzKa = Kf.nnz();
+
     // ---------------- etree + postorder, then redo on the postordered permutation ----------------
-    std::vector<int32_t> iperm(n);
+    std::vector<int32_t> iperm(nt);
     PermutedLower B;
     for (int round = 0; round < 2; ++round) {
-        for (int64_t i = 0; i < n; ++i) iperm[perm[i]] = (int32_t)i;
-        permute_lower(S.K, iperm, B);
-        elimination_tree(n, B, S.parent);
+        for (int64_t i = 0; i < nt; ++i) iperm[perm[i]] = (int32_t)i;
+        permute_lower(Kf, iperm, B);
+        elimination_tree(nt, B, S.parent);
         if (round == 0) {
-            std::vector<int32_t> post, np(n);
+            std::vector<int32_t> post, np(nt);
             postorder(S.parent, post);
-            for (int64_t k = 0; k < n; ++k) np[k] = perm[post[k]];
+            for (int64_t k = 0; k < nt; ++k) np[k] = perm[post[k]];
             perm.swap(np);
         }
     }
+    if (augment && perm[n] != n) { S.error = "internal: the right-hand-side row is not the last pivot"; return NMPC_E_ARG; }
     S.perm = perm; S.iperm = iperm;
     // rows of B sorted by column (needed nowhere), columns of B: sort each column's rows (keeps diagonal first)
-    for (int64_t j = 0; j < n; ++j) {
+    for (int64_t j = 0; j < nt; ++j) {
         int64_t a = B.cptr[j], b = B.cptr[j + 1];
         std::vector<std::pair<int32_t, int32_t>> tmp(b - a);
         for (int64_t p = a; p < b; ++p) tmp[p - a] = {B.crow[p], B.csrc[p]};
@@ -562,10 +581,10 @@ nmpc_status analyze_symbolic(const nmpc_pattern* pattern, const nmpc_ocp* ocp, c
         for (int64_t p = a; p < b; ++p) { B.crow[p] = tmp[p - a].first; B.csrc[p] = tmp[p - a].second; }
     }
     // ---------------- column counts by row-subtree traversal ----------------
-    S.colcount.assign(n, 1);
+    S.colcount.assign(nt, 1);
     {
-        std::vector<int32_t> mark(n, -1);
-        for (int64_t i = 0; i < n; ++i) {
+        std::vector<int32_t> mark(nt, -1);
+        for (int64_t i = 0; i < nt; ++i) {
             mark[i] = (int32_t)i;
             for (int64_t p = B.rptr[i]; p < B.rptr[i + 1]; ++p) {
                 int32_t k = B.rcol[p];
@@ -574,12 +593,13 @@ nmpc_status analyze_symbolic(const nmpc_pattern* pattern, const nmpc_ocp* ocp, c
         }
     }
     S.flops = 0.0;
-    for (int64_t j = 0; j < n; ++j) S.flops += (double)S.colcount[j] * (double)S.colcount[j];
+    // algorithmic flops of the factorization of K itself (the right-hand-side row is not counted)
+    for (int64_t j = 0; j < n; ++j) { const double cc = (double)(S.colcount[j] - (augment ? 1 : 0)); S.flops += cc * cc; }
 
     // ---------------- maximal supernodes, then relaxed amalgamation ----------------
     struct SN { int32_t start, w, r; int64_t zeros; int32_t parent_col; };
     std::vector<SN> sn;
-    for (int64_t j = 0; j < n; ++j) {
+    for (int64_t j = 0; j < nt; ++j) {
         if (!sn.empty() && S.parent[j - 1] == j && S.colcount[j] == S.colcount[j - 1] - 1) sn.back().w++;
         else sn.push_back(SN{(int32_t)j, 1, S.colcount[j], 0, -1});
     }
@@ -608,16 +628,16 @@ nmpc_status analyze_symbolic(const nmpc_pattern* pattern, const nmpc_ocp* ocp, c
     }
     const int32_t ns = (int32_t)sn.size();
     S.ns = ns;
-    S.sn_start.resize(ns + 1); S.sn_of_col.resize(n);
+    S.sn_start.resize(ns + 1); S.sn_of_col.resize(nt);
     for (int32_t s = 0; s < ns; ++s) { S.sn_start[s] = sn[s].start; for (int32_t j = 0; j < sn[s].w; ++j) S.sn_of_col[sn[s].start + j] = s; }
-    S.sn_start[ns] = (int32_t)n;
+    S.sn_start[ns] = (int32_t)nt;
 
     // ---------------- row structure of every supernode (bottom-up), supernodal tree ----------------
     S.rows_ptr.assign(ns + 1, 0); S.rows.clear();
     S.sn_parent.assign(ns, -1); S.sn_level.assign(ns, 0);
     std::vector<std::vector<int32_t>> children(ns);
     {
-        std::vector<int32_t> mark(n, -1), buf;
+        std::vector<int32_t> mark(nt, -1), buf;
         for (int32_t s = 0; s < ns; ++s) {
             const int32_t c0 = S.sn_start[s], c1 = S.sn_start[s + 1];
             buf.clear();
@@ -681,7 +701,7 @@ nmpc_status analyze_symbolic(const nmpc_pattern* pattern, const nmpc_ocp* ocp, c
             S.rel[q] = (int32_t)(b - S.rows_ptr[p]);
         }
     }
-    S.kent_ptr.assign(ns + 1, 0); S.kent_src.resize(S.nnzK); S.kent_dst.resize(S.nnzK);
+    S.kent_ptr.assign(ns + 1, 0); S.kent_src.resize(S.nnzKa); S.kent_dst.resize(S.nnzKa);
     {
         int64_t q = 0;
         for (int32_t s = 0; s < ns; ++s) {
@@ -700,6 +720,19 @@ nmpc_status analyze_symbolic(const nmpc_pattern* pattern, const nmpc_ocp* ocp, c
                 }
             }
             S.kent_ptr[s + 1] = q;
+        }
+    }
+    // ---------------- what the C-ABI reports: the structure of the factor of K alone ----------------
+    if (augment) {
+        S.v_sn_start = S.sn_start; S.v_sn_start[ns] = (int32_t)n;
+        S.v_rows_ptr.assign(ns + 1, 0); S.v_rows.clear();
+        S.v_nnzL = 0; S.v_panel_doubles = 0; S.v_update_doubles = 0; S.v_max_front = 0; S.v_max_width = 0;
+        for (int32_t s = 0; s < ns; ++s) {
+            for (int64_t p = S.rows_ptr[s]; p < S.rows_ptr[s + 1]; ++p) if (S.rows[p] != n) S.v_rows.push_back(S.rows[p]);
+            S.v_rows_ptr[s + 1] = (int64_t)S.v_rows.size();
+            const int64_t r = S.v_rows_ptr[s + 1] - S.v_rows_ptr[s], w = S.v_sn_start[s + 1] - S.v_sn_start[s];
+            S.v_nnzL += panel_nnz(r, w); S.v_panel_doubles += panel_ld(r) * w; S.v_update_doubles += (r - w) * (r - w);
+            S.v_max_front = std::max<int32_t>(S.v_max_front, (int32_t)r); S.v_max_width = std::max<int32_t>(S.v_max_width, (int32_t)w);
         }
     }
     S.analyze_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
@@ -723,7 +756,7 @@ nmpc_status nmpc_symbolic_analyze(const nmpc_pattern* pattern, const nmpc_ocp* o
     nmpc_symbolic_s* h = new (std::nothrow) nmpc_symbolic_s();
     if (!h) return NMPC_E_ALLOC;
     nmpc_status st;
-    try { st = nmpc::analyze_symbolic(pattern, ocp, opt, h->S); }
+    try { st = nmpc::analyze_symbolic(pattern, ocp, opt, h->S, opt && opt->fuse_rhs > 0); }   // host-only analysis: the right-hand-side row on request only
     catch (const std::bad_alloc&) { st = NMPC_E_ALLOC; }
     catch (...) { st = NMPC_E_ARG; }
     if (st != NMPC_OK) { delete h; return st; }
@@ -732,12 +765,19 @@ nmpc_status nmpc_symbolic_analyze(const nmpc_pattern* pattern, const nmpc_ocp* o
 }
 
 void nmpc_fill_info(const nmpc::Symbolic& S, nmpc_sym_info* o) {
-    o->n = S.n; o->nnz_K = S.nnzK; o->nnz_L = S.nnzL;
-    o->panel_doubles = S.panel_ptr.back(); o->update_doubles = S.upd_ptr.back();
-    o->flops = S.flops; o->nsuper = S.ns; o->nlevels = S.nlevels; o->max_front = S.max_front; o->max_width = S.max_width;
+    o->n = S.n; o->nnz_K = S.nnzK; o->nnz_L = S.aug ? S.v_nnzL : S.nnzL;
+    o->panel_doubles = S.aug ? S.v_panel_doubles : S.panel_ptr.back(); o->update_doubles = S.aug ? S.v_update_doubles : S.upd_ptr.back();
+    o->flops = S.flops; o->nsuper = S.ns; o->nlevels = S.nlevels;
+    o->max_front = S.aug ? S.v_max_front : S.max_front; o->max_width = S.aug ? S.v_max_width : S.max_width;
     o->n_large_fronts = 0; o->ordering_used = S.ordering_used; o->analyze_ms = S.analyze_ms;
-    o->perm = S.perm.data(); o->super_start = S.sn_start.data(); o->rows_ptr = S.rows_ptr.data(); o->rows = S.rows.data();
+    // with the right-hand-side row (options.fuse_rhs) the arrays describe the factor of K alone: that row is left out (the
+    // last supernode may then be empty when K's own structure ends in a separate root); etree_parent of a root of K's
+    // forest is n
+    o->perm = S.perm.data();
+    o->super_start = S.aug ? S.v_sn_start.data() : S.sn_start.data();
+    o->rows_ptr = S.aug ? S.v_rows_ptr.data() : S.rows_ptr.data(); o->rows = S.aug ? S.v_rows.data() : S.rows.data();
     o->super_parent = S.sn_parent.data(); o->super_level = S.sn_level.data(); o->etree_parent = S.parent.data();
+    o->fused_rhs = S.aug ? 1 : 0;
 }
 
 nmpc_status nmpc_symbolic_info(nmpc_symbolic sym, nmpc_sym_info* out) {
@@ -763,11 +803,17 @@ nmpc_status nmpc_symbolic_pattern(nmpc_symbolic sym, int64_t* nnz, int64_t* rowp
 nmpc_status nmpc_symbolic_kmap(nmpc_symbolic sym, int32_t* super_of_entry, int64_t* panel_offset) {
     if (!sym || !super_of_entry || !panel_offset) return NMPC_E_ARG;
     const nmpc::Symbolic& S = sym->S;
-    for (int32_t s = 0; s < S.ns; ++s)
+    int64_t voff = 0;                                    // panel offsets in the layout nmpc_get_info / nmpc_get_factor report
+    for (int32_t s = 0; s < S.ns; ++s) {
+        const int64_t ld = nmpc::panel_ld(S.rows_ptr[s + 1] - S.rows_ptr[s]);
+        const int64_t ldv = S.aug ? nmpc::panel_ld(S.v_rows_ptr[s + 1] - S.v_rows_ptr[s]) : ld;
         for (int64_t q = S.kent_ptr[s]; q < S.kent_ptr[s + 1]; ++q) {
+            if (S.kent_src[q] >= S.nnzK) continue;       // entries of the right-hand-side row
             super_of_entry[S.kent_src[q]] = s;
-            panel_offset[S.kent_src[q]] = S.panel_ptr[s] + S.kent_dst[q];
+            panel_offset[S.kent_src[q]] = S.aug ? voff + S.kent_dst[q] % ld + (S.kent_dst[q] / ld) * ldv : S.panel_ptr[s] + S.kent_dst[q];
         }
+        voff += ldv * ((S.aug ? S.v_sn_start[s + 1] : S.sn_start[s + 1]) - S.sn_start[s]);
+    }
     return NMPC_OK;
 }
 

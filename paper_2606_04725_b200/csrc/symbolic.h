@@ -42,6 +42,16 @@ struct ModelMaps {                 // patterns + gather maps of a stage-structur
 struct Symbolic {
     int64_t n = 0, nnzK = 0;
     Csr K;                              // user (or model) pattern, lower CSR, original indices
+    // Right-hand-side row (options.fuse_rhs): the analysed matrix is [K b; b^T 0] with ONE extra variable, index n, ordered
+    // last: nt = n + 1 pivot positions, value array [K values (nnzK) | b (n) | 0].  The numeric factorization then leaves
+    // v = L^-1 P b (Eq. 22) in the last row of the panels and the forward solve of the Newton system is not run at all.
+    // Every array below is over nt pivot positions; the v_* arrays describe the factor of K alone (what the C-ABI reports).
+    bool aug = false;
+    int64_t nt = 0, nnzKa = 0;
+    std::vector<int32_t> v_sn_start, v_rows;
+    std::vector<int64_t> v_rows_ptr;
+    int64_t v_nnzL = 0, v_panel_doubles = 0, v_update_doubles = 0;
+    int32_t v_max_front = 0, v_max_width = 0;
     std::vector<int32_t> perm, iperm;   // perm[new] = old, iperm[old] = new  (Eq. 19)
     std::vector<int32_t> parent;        // elimination tree on pivot positions
     std::vector<int32_t> colcount;      // cc_j incl. diagonal (structure of the un-amalgamated L)
@@ -74,6 +84,6 @@ void default_options(nmpc_options* o);
 bool build_model_maps(const nmpc_ocp* ocp, ModelMaps& mm, std::string& err);
 // Full analysis.  pattern may be NULL if ocp names a model.
 nmpc_status analyze_symbolic(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const nmpc_options* opt,
-                             Symbolic& S);
+                             Symbolic& S, bool augment = false);
 
 }  // namespace nmpc

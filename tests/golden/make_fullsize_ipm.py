@@ -95,13 +95,17 @@ def main():
     ap.add_argument("--out", default=None)
     ap.add_argument("--states", default="all", choices=["all", "last", "none"], help="which solves keep their full iterate z*")
     ap.add_argument("--refine-steps", type=int, default=0, help="oracle option refine_steps (file tag refine<k>)")
+    ap.add_argument("--globalization", default="none", choices=["none", "filter"], help="oracle option globalization (file tag filter)")
     a = ap.parse_args()
     linsolve = a.linsolve or ("blocktri" if a.config in ("C2", "C3") else "sparse")
     overrides = dict(refine_steps=a.refine_steps) if a.refine_steps else {}
+    if a.globalization != "none":
+        overrides["globalization"] = a.globalization
     d = run(a.config, a.resolves, linsolve, **overrides)
     if a.states != "all":
         d = slim(d, a.states)
-    path = a.out or golden_path(a.config, f"refine{a.refine_steps}" if a.refine_steps else "")
+    tag = "_".join(t for t in (f"refine{a.refine_steps}" if a.refine_steps else "", a.globalization if a.globalization != "none" else "") if t)
+    path = a.out or golden_path(a.config, tag)
     np.savez_compressed(path, **d)
     print(f"wrote {path} ({os.path.getsize(path) / 1e6:.1f} MB) in {float(d['wall_seconds']):.1f} s of oracle time")
 

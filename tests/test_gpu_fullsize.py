@@ -151,12 +151,14 @@ def test_ipm_fullsize_closed_loop_vs_oracle(name):
     h.close()
 
 
-@pytest.mark.parametrize("name", ["C2", "C4", "C3"])
+@pytest.mark.parametrize("name", ["C2", "C4"])
 def test_ipm_fullsize_with_refinement_vs_oracle(name):
     """options.refine_steps = 1 at BASELINE size: one step of iterative refinement on the un-condensed
-    Newton system makes the IPM path insensitive to the elimination order, so the closed loop (cold solve + 2 warm re-solves,
-    each warm start the GPU's OWN previous z*, replayed x0) matches the oracle STRICTLY on every configuration including the
-    cold solve of C3: counts, mu / eta traces, step lengths to 5e-3 (ten times tighter than without), y* to 1e-6 (C3's oracle run: ipm_full_C3_refine1.npz)."""
+    Newton system removes most of the elimination-order dependence of the step, so the closed loop (cold solve + 2 warm
+    re-solves, each warm start the GPU's OWN previous z*, replayed x0) matches the oracle STRICTLY: counts, mu / eta traces,
+    step lengths to 5e-3 (ten times tighter than without), y* to 1e-6.  C3 is not in this list: its cold solve stays
+    path-sensitive with refinement too (the oracle itself needs 63 iterations with refine_steps = 1 and wanders at
+    E_0 ~ 1e-2) -- C3 is compared in test_ipm_fullsize_closed_loop_vs_oracle."""
     cfg = make_config(name)
     d = oracle_run(name, refine_steps=1)
     h = nb.Handle(None, nb.make_ocp(cfg), nb.default_options(refine_steps=1))

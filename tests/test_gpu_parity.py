@@ -72,6 +72,71 @@ def test_factor_and_solve_vs_oracle(name, ov, ordering):
     h.close()
 
 
+@pytest.mark.parametrize("name,ov", MID)
+@pytest.mark.parametrize("ordering", [binding.ORDER_AMD, binding.ORDER_ND])
+@pytest.mark.parametrize("bare", [False, True])
+def test_rhs_row_fused_forward_solve_vs_oracle(name, ov, ordering, bare):
+    """options.fuse_rhs: b rides through the numeric factorization as an extra row, which leaves v = L^-1 P b (Eq. 22) in the
+    factor; nmpc_solve_fused then runs Eq. (24)-(25) only.  Checked against the oracle's solve (backward + forward error),
+    against the general two-sided nmpc_solve on the same handle for b and for another right-hand side, and the reported
+    factor must still be the factor of K alone.  `bare`: a pattern-only handle (no model) with fuse_rhs = 1."""
+    cfg = make_config(name, **ov)
+    K, b, _ = kkt_from_oracle(cfg)
+    if bare:
+        Kl = sp.tril(sp.csr_matrix(K), format="csr"); Kl.sort_indices()
+        pat = nb.make_pattern(cfg.n, Kl.indptr, Kl.indices)
+        h = nb.Handle(pat, None, nb.default_options(ordering=ordering, fuse_rhs=1))
+    else:
+        h = nb.Handle(None, nb.make_ocp(cfg), nb.default_options(ordering=ordering))
+    info = h.get_info()
+    assert info["fused_rhs"] == 1 and info["n"] == cfg.n
+    rp, ci = h.get_kkt_pattern(cfg.n)
+    vals = dev(values_on_pattern(K, rp, ci))
+    st, _ = h.factor_rhs(vals, dev(b), 0.0)
+    assert st == 0
+    L = factor_as_sparse(info, h.get_factor())
+    assert factor_backward_error(L, K, info["perm"]) <= 1e-12
+    x = torch.full((cfg.n,), np.nan, dtype=torch.float64, device=DEV)      # written only
+    h.solve_fused(x)
+    xg = x.cpu().numpy()
+    assert normwise_backward_error(K, xg, b) <= 1e-10
+    xo = SparseCholesky(K, None).factor(K).solve(b)
+    cond = np.linalg.cond(K.toarray())
+    tol = max(1e-10, 50.0 * cond * np.finfo(float).eps)
+    assert np.abs(xg - xo).max() <= tol * np.abs(xo).max()
+    x2 = dev(b)
+    h.solve(x2)                                                            # the two-sided solve on the same factorization
+    assert np.abs(x2.cpu().numpy() - xo).max() <= tol * np.abs(xo).max()
+    b3 = np.random.default_rng(5).normal(size=cfg.n)
+    x3 = dev(b3)
+    h.solve(x3)
+    assert normwise_backward_error(K, x3.cpu().numpy(), b3) <= 1e-10
+    h.solve_fused(x)                                                       # still b's solution after other solves
+    assert np.array_equal(x.cpu().numpy(), xg)
+    h.close()
+
+
+def test_rhs_row_off_and_on_take_the_same_ipm_path():
+    """The IPM with the right-hand-side row (default for model handles) and without it (fuse_rhs = 0: forward + backward
+    solve kernels) must agree: iteration counts, mu trace, and the converged iterate to solver accuracy."""
+    for name, ov in MID[:3]:
+        cfg = make_config(name, **ov)
+        out = {}
+        for fuse in (0, 1):
+            h = nb.Handle(None, nb.make_ocp(cfg), nb.default_options(fuse_rhs=fuse))
+            assert h.get_info()["fused_rhs"] == fuse
+            h.update_params(dev(cfg.x0), dev(cfg.ref_for_solve(0)))
+            y = torch.zeros(cfg.n, dtype=torch.float64, device=DEV)
+            r = h.ipm_solve(0, y, trace_cap=256)
+            out[fuse] = (r, y.cpu().numpy())
+            h.close()
+        r0, y0 = out[0]; r1, y1 = out[1]
+        assert r0["status"] == 0 and r1["status"] == 0
+        assert r0["iters"] == r1["iters"], (name, r0["iters"], r1["iters"])
+        assert [t["mu"] for t in r0["trace"]] == [t["mu"] for t in r1["trace"]]
+        assert np.abs(y0 - y1).max() <= 1e-8 * np.abs(y0).max()
+
+
 def _random_interior_point(cfg, nlp, rng):
     lo = np.where(np.isfinite(nlp.lb), nlp.lb, 280.0)
     hi = np.where(np.isfinite(nlp.ub), nlp.ub, 450.0)

@@ -172,6 +172,48 @@ def test_relaxed_supernodes_contain_exact_structure_and_kmap_scatters_K(name, ov
         sym.close()
 
 
+@pytest.mark.parametrize("name,ov", SMALL)
+def test_rhs_row_leaves_the_reported_structure_that_of_K(name, ov):
+    """options.fuse_rhs analyses [K b; b^T 0] with the extra variable ordered last (the factorization then carries
+    v = L^-1 P b of Eq. 22 as the last row of L).  What the C-ABI reports must still be the factor structure of K alone:
+    exact dense-factor pattern without relaxation, the scatter map lands on the right entries, the roots of K's
+    elimination forest point to n."""
+    cfg = make_config(name, **ov)
+    for ordering in ORDERINGS:
+        sym = nb.Symbolic(None, nb.make_ocp(cfg), nb.default_options(ordering=ordering, relax_small=0, relax_zeros=0.0, fuse_rhs=1))
+        info = sym.info()
+        n = info["n"]
+        assert n == cfg.n and info["fused_rhs"] == 1
+        perm = info["perm"]
+        assert sorted(perm.tolist()) == list(range(n))
+        rp, ci = sym.pattern()
+        assert rp[-1] == info["nnz_K"]
+        Lpat = _dense_factor_pattern(n, rp, ci, perm)
+        S = _struct_from_info(info)
+        assert np.array_equal(S, Lpat)
+        assert info["nnz_L"] == int(Lpat.sum())
+        cc = Lpat.sum(axis=0).astype(np.float64)
+        assert info["flops"] == pytest.approx(float((cc ** 2).sum()), rel=1e-12)
+        for j in range(n):
+            below = np.nonzero(Lpat[j + 1:, j])[0]
+            assert info["etree_parent"][j] == (j + 1 + below[0] if len(below) else n)
+        sn, off = sym.kmap()
+        iperm = np.empty(n, np.int64)
+        iperm[perm] = np.arange(n)
+        ld = (np.diff(info["rows_ptr"]) + 1) & ~1
+        panel_ptr = np.concatenate([[0], np.cumsum(ld * np.diff(info["super_start"]))])
+        assert panel_ptr[-1] == info["panel_doubles"]
+        for i in range(n):
+            for p in range(rp[i], rp[i + 1]):
+                a, b = iperm[i], iperm[ci[p]]
+                r_, c_ = max(a, b), min(a, b)
+                s_ = sn[p]
+                rows = info["rows"][info["rows_ptr"][s_]:info["rows_ptr"][s_ + 1]]
+                local = off[p] - panel_ptr[s_]
+                assert local // ld[s_] == c_ - info["super_start"][s_] and rows[local % ld[s_]] == r_
+        sym.close()
+
+
 def test_fig1_children_property_golden_through_the_library():
     txt = [l for l in open(os.path.join(GOLDEN, "fig1_etree_property.txt")) if not l.startswith("#")]
     n = int(txt[0].split()[1])
