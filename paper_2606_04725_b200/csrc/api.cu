@@ -125,7 +125,7 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
         slots += (int64_t)nbp[s] * nbt[s] + 1;
         target[s] = nbt[s] * (nbt[s] + 1) / 2;
         bbase[s] = (int32_t)bslots; bslots += nbp[s];
-        target_f[s] = nbt[s]; target_b[s] = nbp[s];
+        target_f[s] = nbt[s]; target_b[s] = 1;             // backward: the chain task finishes the supernode
         if (slots > INT32_MAX / 2) { h->err = "too many tiles"; return NMPC_E_ALLOC; }
     }
     // K scatter map per front class: small = packed lower offset; tiled = tile-local offset, entries sorted by tile slot
@@ -212,7 +212,8 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
     std::vector<int4> tasks(tk.size());
     for (size_t t = 0; t < tk.size(); ++t) tasks[t] = make_int4(tk[t].type, tk[t].s, tk[t].I, tk[t].J);
 
-    // solve tasks: forward in descending rank (children before parents, block rows in order), backward = reversed order
+    // solve tasks: forward in descending rank (children before parents, block rows in order); backward top-down in the order
+    // of an estimated start time (see below)
     struct SK { double rank; int32_t lvl, type, s, I; };
     std::vector<SK> sk;
     {
@@ -235,8 +236,39 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
     stasks.reserve(2 * sk.size());
     for (const SK& t : sk) stasks.push_back(make_int4(t.type, t.s, t.I, 0));
     const int32_t n_sfwd = (int32_t)stasks.size();
-    for (size_t t = sk.size(); t-- > 0;)
-        if (sk[t].type == 0 || sk[t].I < nbp[sk[t].s]) stasks.push_back(make_int4(sk[t].type, sk[t].s, sk[t].I, 1));
+    // Backward: a supernode can start when its parent is done.  CTAs claim tasks in order and WAIT for the dependencies of
+    // what they claimed, so the order must follow the time at which tasks become runnable, or the CTAs fill up with waiting
+    // tasks while runnable ones queue behind them: supernodes in the order of an estimated start time (parent's end; ~3 us
+    // per block column of a chain, ~15 us for the chunk tasks of a supernode, ~4 us per small supernode: task timelines under
+    // profiles/).  The tasks of a tiled supernode are contiguous: chunk tasks (they depend on the parent only), the chain, then
+    // the helper sums in the order the chain needs them.  The chain waits for helpers that come AFTER it in the list, which is
+    // safe for any grid >= 2: the helpers between the chain and the one it waits for depend only on blocks the chain has
+    // already published, so the other CTAs always get to it.
+    std::vector<int64_t> pbase(ns, 0);
+    int64_t part_doubles = 0;
+    {
+        const double HOP_US = 3.0, UPD_US = 15.0, SMALL_US = 4.0;
+        std::vector<double> ready(ns, 0.0), fin(ns, 0.0);
+        std::vector<int32_t> order(ns);
+        for (int s = ns - 1; s >= 0; --s) {              // parents have larger indices (postorder)
+            const int p = S.sn_parent[s];
+            ready[s] = p < 0 ? 0.0 : fin[p];
+            order[s] = s;
+            if (!cls[s]) { fin[s] = ready[s] + SMALL_US + 0.05 * W(s); continue; }
+            const int nchunk = (nbt[s] - nbp[s] + BWD_CH - 1) / BWD_CH;
+            fin[s] = ready[s] + (nchunk > 0 ? UPD_US : 0.0) + HOP_US * nbp[s] + 5.0;
+        }
+        std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return ready[a] != ready[b] ? ready[a] < ready[b] : a > b; });
+        for (int s : order) {
+            if (!cls[s]) { stasks.push_back(make_int4(0, s, 0, 1)); continue; }
+            const int nchunk = (nbt[s] - nbp[s] + BWD_CH - 1) / BWD_CH;
+            pbase[s] = part_doubles; part_doubles += (int64_t)nchunk * W(s);
+            for (int J = nbp[s] - 1; J >= 0; --J)
+                for (int c = 0; c < nchunk; ++c) stasks.push_back(make_int4(2, s, J | (c << 16), 1));
+            stasks.push_back(make_int4(3, s, 0, 1));
+            for (int J = nbp[s] - 4; J >= 0; --J) stasks.push_back(make_int4(1, s, J, 1));
+        }
+    }
 
     DagPlan& F = h->F;
     const int64_t* tl = nullptr; const int4* t4 = nullptr;
@@ -248,11 +280,13 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
     TRY(upload(h, cb_ptr, &tl)); F.cb_ptr = tl;
     TRY(upload(h, cbnd, &F.cbnd));
     TRY(upload(h, S.sn_parent, &F.sn_parent));
+    TRY(upload(h, pbase, &tl)); F.pbase = tl;
+    TRY(dalloc(h, (size_t)part_doubles, &F.bpart, false)); TRY(dalloc(h, (size_t)S.nt, &F.bsum, false)); TRY(dalloc(h, (size_t)S.nt, &F.bva, false));
     TRY(upload(h, ksrc, &h->D.kent_src)); TRY(upload(h, kdst, &h->D.kent_dst));
-    F.sync_words = 3 + 3 * (int64_t)ns + slots + 3 * bslots;
+    F.sync_words = 3 + 3 * (int64_t)ns + slots + 5 * bslots;
     TRY(dalloc(h, (size_t)F.sync_words, &F.sync));
     F.fac_done = F.sync + 3; F.sol_done_f = F.fac_done + ns; F.sol_done_b = F.sol_done_f + ns;
-    F.tile_done = F.sol_done_b + ns; F.blk_f = F.tile_done + slots; F.blk_b = F.blk_f + bslots; F.sub_done = F.blk_b + bslots;
+    F.tile_done = F.sol_done_b + ns; F.blk_f = F.tile_done + slots; F.blk_b = F.blk_f + bslots; F.blk_u = F.blk_b + bslots; F.blk_s = F.blk_u + bslots; F.sub_done = F.blk_s + bslots;
 
 #ifdef NMPC_TRACE_BUILD                                      // measurement build: per-task timestamps (nmpc_get_task_trace, include/nmpc_aids.h)
     TRY(dalloc(h, (size_t)F.n_ftasks * 8, &F.ftrace)); TRY(dalloc(h, (size_t)F.n_stasks * 8, &F.strace));
@@ -261,7 +295,8 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
     F.fsmem = smem_bytes; F.ssmem = solve_smem;
     F.fgrid = (int32_t)std::max<int64_t>(1, std::min<int64_t>((int64_t)tasks.size(), (int64_t)num_sms * ctas_per_sm));
     F.sgrid = (int32_t)std::max<int64_t>(1, std::min<int64_t>((int64_t)stasks.size(), (int64_t)num_sms * solve_ctas_per_sm));
-    if (h->opt.grid_limit > 0) { F.fgrid = std::min(F.fgrid, h->opt.grid_limit); F.sgrid = std::min(F.sgrid, h->opt.grid_limit); }
+    if (h->opt.grid_limit > 0) { F.fgrid = std::min(F.fgrid, h->opt.grid_limit); F.sgrid = std::min(F.sgrid, std::max(2, h->opt.grid_limit)); }
+    if (h->n_big_fronts > 0) F.sgrid = std::max(F.sgrid, 2);          // a chain task and its helpers need two CTAs (see above)
     // epoch-valued flags: counters reach epoch * target and the claim counters epoch * (ntasks + grid); reset before 2^31
     int64_t per_epoch = std::max<int64_t>((int64_t)tasks.size() + F.fgrid, (int64_t)stasks.size() + F.sgrid);
     for (int s = 0; s < ns; ++s) per_epoch = std::max<int64_t>(per_epoch, target[s]);

@@ -42,6 +42,7 @@ struct DevSym {                   // device copies of the symbolic arrays (symbo
 
 constexpr int BIG_NB = 64;        // block size used by the triangular-solve kernels for the diagonal blocks
 constexpr int TILE = 64;          // tile size of the tiled (HBM-resident) fronts
+constexpr int BWD_CH = 8;         // tiles of the ancestors' rows one chunk task of the backward solve takes (solve.cu)
 constexpr int SMALL_ROWS_MAX = 240;  // upper bound on the rows (leading dimension) of a front handled by one CTA in shared memory
 
 __host__ __device__ inline int ld_even(int r) { return (r + 1) & ~1; }   // = symbolic.h: panel_ld
@@ -64,8 +65,10 @@ __host__ __device__ inline int tile_nbu(int w, int r) {
 
 // Task lists of the persistent task-DAG kernels, built once by nmpc_analyze.
 //   factor task   (type, sn, I, J): type 0 = whole small front in shared memory, 1 = tile (I,J) of a tiled front (left-looking)
-//   solve task    (type, sn, I, dir): type 0 = whole supernode, 1 = block row / block column I of a tiled supernode;
-//                 dir 0 = forward (L v = P b), 1 = backward (L^T x = v); forward tasks first, backward = reversed order
+//   solve task    (type, sn, I, dir): type 0 = whole supernode, 1 = block row I (forward) / helper sums of block column I
+//                 (backward) of a tiled supernode, 2 (backward) = chunk c of the ancestors' rows for block column J, I = J | c << 16,
+//                 3 (backward) = the chain of the diagonal blocks of a tiled supernode;
+//                 dir 0 = forward (L v = P b), 1 = backward (L^T x = v); forward tasks first, then the backward tasks top-down
 // Completion flags are EPOCH-valued (no reset between calls): call number e stores e into a flag and adds 1 to a counter,
 // so "done in this call" is flag >= e, counter >= e * target; the claim counter advances by ntasks + grid per call.
 // The forward and the backward half of the solves have their own call numbers (a fused solve runs the backward half only).
@@ -91,6 +94,12 @@ struct DagPlan {
     uint32_t* tile_done = nullptr;       // tile slots
     uint32_t* blk_f = nullptr;           // block slots
     uint32_t* blk_b = nullptr;
+    uint32_t* blk_u = nullptr;           // block slots: finished chunk tasks of the backward solve per block column
+    uint32_t* blk_s = nullptr;           // block slots: helper sum S_J of the backward solve written
+    double* bsum = nullptr;              // nt: the helper sums (pivot positions)
+    double* bva = nullptr;               // nt: v - anc per column of the tiled supernodes (backward chain prologue)
+    const int64_t* pbase = nullptr;      // ns: offset into bpart of a tiled supernode's partial sums [chunk][w]
+    double* bpart = nullptr;
     uint32_t* sub_done = nullptr;        // block slots: published 8-column blocks of the diagonal tile L_JJ, (epoch-1)*16 + count
 #ifdef NMPC_TRACE_BUILD                     // measurement build only (libnmpc_b200_aids.so, include/nmpc_aids.h)
     unsigned long long* ftrace = nullptr;   // 8 timestamps per factor task / per solve task

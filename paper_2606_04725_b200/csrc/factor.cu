@@ -747,7 +747,13 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
                     const int nr = nj - js;
                     for (int idx = tid - NT / 2; idx < jbs * nr; idx += NT / 2) {
                         const int cc = idx / nr, ii = idx - cc * nr;
-                        if (ii >= cc) P[(j0 + js + ii) + (int64_t)(j0 + js + cc) * ld] = Cs[(js + cc) * CLD + js + ii];
+                        if (ii >= cc) {
+                            const double v = Cs[(js + cc) * CLD + js + ii];
+                            P[(j0 + js + ii) + (int64_t)(j0 + js + cc) * ld] = v;
+                            // the unused upper triangle of the diagonal tile receives L_JJ^T: row j of L_JJ becomes a contiguous
+                            // column, which is what the backward substitution of solve.cu (bwd_chain) streams
+                            if (ii > cc) P[(j0 + js + cc) + (int64_t)(j0 + js + ii) * ld] = v;
+                        }
                     }
                     asm volatile("bar.sync 1, %0;" ::"n"(NT / 2) : "memory");
                     if (tid == NT - 1) { __threadfence(); st_release(sub, sbase + (uint32_t)(js >> 3) + 1u); }

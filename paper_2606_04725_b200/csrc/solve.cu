@@ -8,14 +8,22 @@
 //             substitution (only shuffle + fma on the chain), one thread per row for the block below; contribution = t2 - L21 y.
 //   forward,  block row I of a tiled supernode (left-looking): t_I = init_I - sum_{k<I} L(I,k) y_k; the 64x64 tile L(I,k+1)
 //             is in registers before the task waits for y_k; then L(I,I) y_I = t_I by one warp on the staged diagonal tile.
-//   backward, small supernode / block column J of a tiled supernode: x_J = L(J,J)^-T (y_J - sum_{I>J} L(I,J)^T x_I), rows
-//             taken from the ancestors' finished x first, then from this supernode's later blocks as their flags arrive.
+//   backward, small supernode / block column J of a tiled supernode: x_J = L(J,J)^-T (y_J - sum_{I>J} L(I,J)^T x_I).  For a
+//             tiled supernode the rows of the ANCESTORS (block rows I >= nbp, known as soon as the parent is done) are taken by
+//             separate chunk tasks (BWD_CH tiles each, all block columns and chunks in parallel) that leave partial sums.  The
+//             chain of the nbp diagonal blocks runs in ONE CTA (bwd_chain): per block column J it applies L(J+1,J)^T x_{J+1} from
+//             registers and substitutes with L(J,J) in shared memory, while its other warps prepare block J-1 (the product
+//             L(J+1,J-1)^T x_{J+1} from a tile staged with cp.async, the next diagonal tile, v, the partial sums) -- no flag
+//             round trip between consecutive blocks.  The blocks further away, S_J = sum_{I >= J+3} L(I,J)^T x_I, come from one
+//             helper task per block column (bwd_sum) that follows the chain two blocks behind.
 // The permutations are fused: forward tasks read b[perm[.]], backward tasks write b[perm[.]] (in place, no hazard: a
 // supernode's entries of b are read by its own forward task only).  Divisions by L_jj are multiplications by the reciprocals
 // the factorization stored (dinv).  fp64, fixed summation order -> bitwise reproducible.
 // Right-hand-side row (options.fuse_rhs, symbolic.h): the structure has one extra last variable whose row of L holds
 // v = L^-1 P b of the b that went through the factorization.  A FUSED solve runs the backward tasks only and takes v from that
 // row (the last row of every panel); a general solve treats the extra variable's right-hand side and solution as 0.
+#include <algorithm>
+
 #include "device.h"
 
 namespace nmpc {
@@ -103,6 +111,13 @@ __device__ __forceinline__ void stage_block(const DevSym& D, const Sn& q, int k,
 #define STRACE(slot) do { if (tr && threadIdx.x == 0) { unsigned long long g_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g_)); tr[slot] = g_; } } while (0)
 #else
 #define STRACE(slot) do { (void)tr; } while (0)
+#endif
+#ifdef NMPC_TRACE_BUILD                     // measurement build: time accumulated per phase of the chain task
+#define CHT0() unsigned long long cht_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(cht_))
+#define CHT1(slot) do { if (tr) { unsigned long long g_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g_)); tr[slot] += g_ - cht_; } } while (0)
+#else
+#define CHT0() do {} while (0)
+#define CHT1(slot) do { (void)tr; } while (0)
 #endif
 __device__ __forceinline__ void fwd_small(const DevSym& D, const DagPlan& F, int s, const double* b, double* x, uint32_t epoch, double* sm, unsigned long long* tr) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -411,26 +426,12 @@ __device__ __forceinline__ void bwd_small(const DevSym& D, const DagPlan& F, int
     if (tid == 0) { __threadfence(); red_release_add(F.sol_done_b + s, 1u); }
 }
 
-// ---------------- backward, block column J of a tiled supernode ----------------
-// x_J = L(J,J)^-T (y_J - sum_{I>J} L(I,J)^T x_I): the tile L(I-1,J) is loaded into registers before the task waits for x_I.
-__device__ __forceinline__ void bwd_tiled(const DevSym& D, const DagPlan& F, int s, int J, double* b, double* x, uint32_t ef, uint32_t epoch, bool fused, double* sm) {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const Sn q = sn_of(D, s);
-    const int nbp = tile_nbp(q.w), nbt = nbp + tile_nbu(q.w, q.r);
-    const int j0 = J * TILE, nj = min(TILE, q.w - j0);
-    double* xs = sm + OFF_YS; double* zs = sm; double* Ld = sm + OFF_LD;
-    uint32_t* bb = F.blk_b + F.bbase[s];
-    for (int idx = tid; idx < TILE * TILE; idx += NT) {
-        const int i = idx & (TILE - 1), c = idx >> 6;
-        if (i >= c && i < nj) Ld[c * DLD + i] = __ldg(q.P + (j0 + i) + (int64_t)(j0 + c) * q.ld);
-    }
-    double d0 = 1.0, d1 = 1.0;
-    if (warp == 0) {
-        if (lane < nj) d0 = __ldcg(D.dinv + q.c0 + j0 + lane);
-        if (lane + 32 < nj) d1 = __ldcg(D.dinv + q.c0 + j0 + lane + 32);
-    }
-    double cur[16], nxt[16];
-    auto load_tile = [&](int I, double (&v)[16]) {
+// ---------------- backward, tiled supernode ----------------
+// load_tile: the 64x64 tile L(I,J) into registers, warp w holds columns 8w..8w+7, lanes over the rows (two per lane)
+struct BwdTile {
+    const Sn& q; int nbp, j0, nj;
+    __device__ __forceinline__ void load(int I, double (&v)[16]) const {
+        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
         const int i0 = tile_bound(I, q.w, q.r, nbp), ni = tile_bound(I + 1, q.w, q.r, nbp) - i0;
 #pragma unroll
         for (int e = 0; e < 8; ++e) {
@@ -439,28 +440,71 @@ __device__ __forceinline__ void bwd_tiled(const DevSym& D, const DagPlan& F, int
             v[2 * e] = (c < nj && lane < ni) ? __ldg(Pc + lane) : 0.0;
             v[2 * e + 1] = (c < nj && lane + 32 < ni) ? __ldg(Pc + lane + 32) : 0.0;
         }
-    };
-    if (nbt - 1 > J) load_tile(nbt - 1, cur);
-    if (tid == 0) {
-        if (!fused) spin_until_ge(F.sol_done_f + s, ef * (uint32_t)F.target_f[s]);
-        const int p = F.sn_parent[s];
-        if (p >= 0) spin_until_ge(F.sol_done_b + p, epoch * (uint32_t)F.target_b[p]);   // the rows below belong to finished ancestors
     }
+};
+
+// chunk task (s, J, c): partial[c][J] = sum over the ancestors' block rows I in chunk c of L(I,J)^T x_I
+__device__ __forceinline__ void bwd_upd(const DevSym& D, const DagPlan& F, int s, int J, int c, const double* x, uint32_t epoch, double* sm) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const Sn q = sn_of(D, s);
+    const int nbp = tile_nbp(q.w), nbt = nbp + tile_nbu(q.w, q.r);
+    const int j0 = J * TILE, nj = min(TILE, q.w - j0);
+    const int Ia = nbp + c * BWD_CH, Ib = min(nbt, Ia + BWD_CH);
+    double* xs = sm + OFF_YS;
+    const BwdTile T{q, nbp, j0, nj};
+    double cur[16], nxt[16];
+    T.load(Ia, cur);
+    if (tid == 0) { const int p = F.sn_parent[s]; if (p >= 0) spin_until_ge(F.sol_done_b + p, epoch * (uint32_t)F.target_b[p]); }
     __syncthreads();
     double acc[8];
 #pragma unroll
     for (int e = 0; e < 8; ++e) acc[e] = 0.0;
-    for (int I = nbt - 1; I > J; --I) {
-        if (I - 1 > J) load_tile(I - 1, nxt);
+    for (int I = Ia; I < Ib; ++I) {
+        if (I + 1 < Ib) T.load(I + 1, nxt);
         const int i0 = tile_bound(I, q.w, q.r, nbp), ni = tile_bound(I + 1, q.w, q.r, nbp) - i0;
+        if (tid < TILE) xs[tid] = tid < ni ? __ldcg(x + q.rows[i0 + tid]) : 0.0;
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < 8; ++e) acc[e] = fma(cur[2 * e + 1], xs[lane + 32], fma(cur[2 * e], xs[lane], acc[e]));
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < 16; ++e) cur[e] = nxt[e];
+    }
+    double* out = F.bpart + F.pbase[s] + (int64_t)c * q.w + j0;
+#pragma unroll
+    for (int e = 0; e < 8; ++e) {
+        double v = acc[e];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
+        const int cc = warp * 8 + e;
+        if (lane == 0 && cc < nj) out[cc] = v;
+    }
+    __syncthreads();
+    if (tid == 0) { __threadfence(); red_release_add(F.blk_u + F.bbase[s] + J, 1u); }
+}
+
+// helper (s, J), J <= nbp - 4: S_J = sum_{I = nbp-1 .. J+3} L(I,J)^T x_I, each x_I taken as the chain publishes it (the tile
+// L(I-1,J) is in registers before the task waits for x_I); two blocks of slack before the chain needs S_J
+__device__ __forceinline__ void bwd_sum(const DevSym& D, const DagPlan& F, int s, int J, const double* x, uint32_t epoch, double* sm) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const Sn q = sn_of(D, s);
+    const int nbp = tile_nbp(q.w);
+    const int j0 = J * TILE, nj = min(TILE, q.w - j0);
+    double* xs = sm + OFF_YS;
+    uint32_t* bb = F.blk_b + F.bbase[s];
+    const BwdTile T{q, nbp, j0, nj};
+    double cur[16], nxt[16];
+    T.load(nbp - 1, cur);
+    double acc[8];
+#pragma unroll
+    for (int e = 0; e < 8; ++e) acc[e] = 0.0;
+    for (int I = nbp - 1; I >= J + 3; --I) {
+        if (I - 1 >= J + 3) T.load(I - 1, nxt);
+        const int i0 = I * TILE, ni = min(TILE, q.w - i0);
         if (tid < TILE) {
-            if (I < nbp) {
-                if (lane == 0) spin_until_ge(bb + I, epoch);
-                __syncwarp();
-                xs[tid] = tid < ni ? __ldcg(x + q.c0 + i0 + tid) : 0.0;
-            } else {
-                xs[tid] = tid < ni ? __ldcg(x + q.rows[i0 + tid]) : 0.0;
-            }
+            if (lane == 0) spin_until_ge(bb + I, epoch);
+            __syncwarp();
+            xs[tid] = tid < ni ? __ldcg(x + q.c0 + i0 + tid) : 0.0;
         }
         __syncthreads();
 #pragma unroll
@@ -469,54 +513,234 @@ __device__ __forceinline__ void bwd_tiled(const DevSym& D, const DagPlan& F, int
 #pragma unroll
         for (int e = 0; e < 16; ++e) cur[e] = nxt[e];
     }
+    double* out = F.bsum + q.c0 + j0;
 #pragma unroll
     for (int e = 0; e < 8; ++e) {
         double v = acc[e];
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
-        const int c = warp * 8 + e;
-        if (lane == 0 && c < nj) {
-            const int col = q.c0 + j0 + c;
-            const double yc = col == D.aug_col ? 0.0 : fused ? __ldcg(q.P + (q.r - 1) + (int64_t)(j0 + c) * q.ld) : __ldcg(x + col);
-            zs[c] = yc - v;
-        }
+        const int cc = warp * 8 + e;
+        if (lane == 0 && cc < nj) out[cc] = v;
     }
     __syncthreads();
-    if (warp == 0) {
-        const bool h1 = lane + 32 < nj;
-        double z0 = lane < nj ? zs[lane] : 0.0, z1 = h1 ? zs[lane + 32] : 0.0;
-        // pre-scaled substitution (s_i = d_i z_i): only (shuffle, fma) on the chain, scaled entries loaded 8 rows ahead
-        z0 *= d0; z1 *= d1;
-        const int c0l = min(lane, nj - 1), c1l = min(lane + 32, nj - 1);
-        for (int jb = ((nj - 1) >> 3) << 3; jb >= 32; jb -= 8) {
-            double la[8], lb[8];
-#pragma unroll
-            for (int e = 0; e < 8; ++e) { const int jr = min(jb + e, nj - 1); la[e] = Ld[c0l * DLD + jr] * d0; lb[e] = Ld[c1l * DLD + jr] * d1; }
-#pragma unroll
-            for (int e = 7; e >= 0; --e) {
-                const int j = jb + e;
-                const double xj = __shfl_sync(FULL, z1, (j - 32) & 31);
-                const bool on = j < nj;
-                z1 = (on && lane + 32 < j) ? fma(-lb[e], xj, z1) : z1;
-                z0 = (on && lane < nj) ? fma(-la[e], xj, z0) : z0;
-            }
+    if (tid == 0) { __threadfence(); st_release(F.blk_s + F.bbase[s] + J, epoch); }
+}
+
+// the chain of a tiled supernode: x_J = L(J,J)^-T (v_J - anc_J - S_J - L(J+2,J)^T x_{J+2} - L(J+1,J)^T x_{J+1}), J = nbp-1 .. 0, in one CTA.
+// Per block ("hop"): all warps apply L(J+1,J)^T x_{J+1} from the staged tile T1; then
+//   warp 0      substitutes with the staged L(J,J)^T (the factorization leaves it in the upper triangle of the diagonal tile:
+//               row j of L(J,J) is a contiguous column there; staged packed, lanes read consecutive words);
+//   warps 1, 2  write x_{J+1} to global memory and announce it, fetch S_{J-1} from the helper and v - anc of block J-2;
+//   warps 3..7  compute L(J+1,J-1)^T x_{J+1} from the staged tile T2 and request the three tiles of the next hop (cp.async).
+// Shared memory (doubles): zs[64] | pre[2][64] | xs[2][64] | dv[2][64] | Ld[2][2048] | T1[64*64] | T2[64*64]
+constexpr int LDP = TILE * TILE / 2;                                // packed L(J,J)^T: column j (rows 0 .. j-1, rounded up to even) at j*j/2
+constexpr int CH_PRE = 64, CH_XS = CH_PRE + 2 * TILE, CH_DV = CH_XS + 2 * TILE, CH_LD = CH_DV + 2 * TILE, CH_T1 = CH_LD + 2 * LDP,
+              CH_T2 = CH_T1 + TILE * TILE, CH_END = CH_T2 + TILE * TILE;
+__device__ __forceinline__ void bar_named(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
+__device__ __forceinline__ void bwd_chain(const DevSym& D, const DagPlan& F, int s, double* b, double* x, uint32_t ef, uint32_t epoch, bool fused, double* sm, unsigned long long* tr) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const Sn q = sn_of(D, s);
+    const int nbp = tile_nbp(q.w), nbt = nbp + tile_nbu(q.w, q.r);
+    const int nchunk = (nbt - nbp + BWD_CH - 1) / BWD_CH;
+    double* zs = sm;
+    uint32_t* bb = F.blk_b + F.bbase[s];
+    const uint32_t* bu = F.blk_u + F.bbase[s];
+    const uint32_t* bs = F.blk_s + F.bbase[s];
+    double* bva = F.bva + q.c0;                                     // v - anc of this supernode's columns (written by the prologue)
+    auto stage_diag = [&](int J, int buf, int t0, int nthr) {       // L(J,J)^T packed + pivot reciprocals, cp.async
+        const int j0 = J * TILE, nj = min(TILE, q.w - j0);
+        double* Ld = sm + CH_LD + buf * LDP;
+        for (int idx = t0; idx < TILE * TILE / 2; idx += nthr) {
+            const int j = idx >> 5, h = idx & 31;
+            if (j < nj && 2 * h < j) cp_async16(Ld + ((j * j) >> 1) + 2 * h, q.P + j0 + 2 * h + (int64_t)(j0 + j) * q.ld);
         }
-        for (int jb = ((min(nj, 32) - 1) >> 3) << 3; jb >= 0; jb -= 8) {
-            double la[8];
-#pragma unroll
-            for (int e = 0; e < 8; ++e) la[e] = Ld[c0l * DLD + min(jb + e, nj - 1)] * d0;
-#pragma unroll
-            for (int e = 7; e >= 0; --e) {
-                const int j = jb + e;
-                const double xj = __shfl_sync(FULL, z0, j & 31);
-                z0 = (j < min(nj, 32) && lane < j) ? fma(-la[e], xj, z0) : z0;
-            }
+        if (t0 < nj) cp_async8(sm + CH_DV + buf * TILE + t0, D.dinv + q.c0 + j0 + t0);
+    };
+    auto stage_tile = [&](int off, int I, int Jc, int t0, int nthr) {   // L(I,Jc): 64 columns x the 64 rows from the start of block
+        const double* src = q.P + I * TILE + (int64_t)(Jc * TILE) * q.ld;   // I (rows past a ragged block meet zeros of xs), 16 B
+        for (int idx = t0; idx < TILE * TILE / 2; idx += nthr) {
+            const int c = idx >> 5, h = idx & 31;
+            cp_async16(sm + off + c * TILE + 2 * h, src + (int64_t)c * q.ld + 2 * h);
         }
-        if (lane < nj) { x[q.c0 + j0 + lane] = z0; put_solution(D, b, q.c0 + j0 + lane, z0); }
-        if (h1) { x[q.c0 + j0 + lane + 32] = z1; put_solution(D, b, q.c0 + j0 + lane + 32, z1); }
-        __syncwarp();
-        if (lane == 0) { __threadfence(); st_release(bb + J, epoch); red_release_add(F.sol_done_b + s, 1u); }
+    };
+    int J = nbp - 1;
+    stage_diag(J, J & 1, tid, NT);
+    cp_async_commit();
+    if (tid < 2 * TILE) sm[CH_XS + tid] = 0.0;
+    // dependencies: the forward half (two-sided solve), the parent, ALL chunk tasks of this supernode
+    if (tid == 0) {
+        if (!fused) spin_until_ge(F.sol_done_f + s, ef * (uint32_t)F.target_f[s]);
+        const int p = F.sn_parent[s];
+        if (p >= 0) spin_until_ge(F.sol_done_b + p, epoch * (uint32_t)F.target_b[p]);
     }
+    if (nchunk > 0) for (int k = tid; k < nbp; k += NT) spin_until_ge(bu + k, epoch * (uint32_t)nchunk);
+    __syncthreads();
+    // v - anc for every column: v from the right-hand-side row of the panel (fused) or from the forward solve; anc = the chunk
+    // tasks' partial sums in chunk order.  Written to global memory; the hops fetch 64 of them two blocks ahead.
+    for (int c = tid; c < q.w; c += NT) {
+        const int col = q.c0 + c;
+        double a = col == D.aug_col ? 0.0 : fused ? __ldcg(q.P + (q.r - 1) + (int64_t)c * q.ld) : __ldcg(x + col);
+        const double* pp = F.bpart + F.pbase[s] + c;
+        for (int k = 0; k < nchunk; ++k) a -= __ldcg(pp + (int64_t)k * q.w);
+        bva[c] = a;
+        if (c >= J * TILE) sm[CH_PRE + (J & 1) * TILE + c - J * TILE] = a;
+    }
+    {
+        const int nj = min(TILE, q.w - J * TILE);
+        if (tid >= nj && tid < TILE) sm[CH_PRE + (J & 1) * TILE + tid] = 0.0;
+    }
+    cp_async_wait<0>();                                             // the first diagonal tile has landed
+    __syncthreads();                                                // (also orders the bva writes before the loads below)
+    double va_next = 0.0;                                           // threads 32..95: v - anc of the block the NEXT hop prepares
+    if (J >= 1 && tid >= 32 && tid < 32 + TILE) va_next = bva[(J - 1) * TILE + tid - 32];
+#ifdef NMPC_TRACE_BUILD
+    if (tr && tid == 0) { tr[2] = 0; tr[3] = 0; tr[5] = 0; tr[6] = 0; tr[7] = 0; }
+#endif
+    STRACE(1);
+    for (; J >= 0; --J) {
+        const int j0 = J * TILE, nj = min(TILE, q.w - j0);
+        const double* pre = sm + CH_PRE + (J & 1) * TILE;
+        const double* xprev = sm + CH_XS + ((J + 1) & 1) * TILE;    // x_{J+1} (zero padded)
+        double* xcur = sm + CH_XS + (J & 1) * TILE;
+        // A: z_J = pre_J - L(J+1,J)^T x_{J+1}  (block J is a full block when J + 1 < nbp)
+        if (J + 1 < nbp) {
+            const double* T1 = sm + CH_T1;
+            const double xa = xprev[lane], xb = xprev[lane + 32];
+            double v[8];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) { const double* tc = T1 + (warp * 8 + e) * TILE; v[e] = fma(tc[lane + 32], xb, tc[lane] * xa); }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+                for (int e = 0; e < 8; ++e) v[e] += __shfl_xor_sync(FULL, v[e], o);
+            double mine = v[0];
+#pragma unroll
+            for (int e = 1; e < 8; ++e) mine = lane == e ? v[e] : mine;
+            if (lane < 8) zs[warp * 8 + lane] = pre[warp * 8 + lane] - mine;
+        } else if (tid < TILE) {
+            zs[tid] = pre[tid];
+        }
+        __syncthreads();
+        const int Jn = J - 1;
+        double* pren = sm + CH_PRE + (Jn & 1) * TILE;
+        if (warp == 0) {
+            // chain: L(J,J)^T x_J = z_J, pre-scaled substitution (s_i = d_i z_i): only (shuffle, fma) on the chain
+            CHT0();
+            const double* Ld = sm + CH_LD + (J & 1) * LDP;
+            const double* dv = sm + CH_DV + (J & 1) * TILE;
+            const bool h1 = lane + 32 < nj;
+            const double d0 = lane < nj ? dv[lane] : 1.0, d1 = h1 ? dv[lane + 32] : 1.0;
+            double z0 = lane < nj ? zs[lane] : 0.0, z1 = h1 ? zs[lane + 32] : 0.0;
+            z0 *= d0; z1 *= d1;
+            // packed column jr of L(J,J)^T = row jr of L(J,J): entries (jr, lane) and (jr, lane + 32) where they lie below the diagonal
+            for (int jb = ((nj - 1) >> 3) << 3; jb >= 32; jb -= 8) {
+                double la[8], lb[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int jr = min(jb + e, nj - 1);
+                    const double* row = Ld + ((jr * jr) >> 1);
+                    la[e] = row[lane] * d0; lb[e] = row[min(lane + 32, jr - 1)] * d1;
+                }
+#pragma unroll
+                for (int e = 7; e >= 0; --e) {
+                    const int j = jb + e;
+                    const double xj = __shfl_sync(FULL, z1, (j - 32) & 31);
+                    const bool on = j < nj;
+                    z1 = (on && lane + 32 < j) ? fma(-lb[e], xj, z1) : z1;
+                    z0 = (on && lane < nj) ? fma(-la[e], xj, z0) : z0;
+                }
+            }
+            for (int jb = ((min(nj, 32) - 1) >> 3) << 3; jb >= 0; jb -= 8) {
+                double la[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int jr = min(jb + e, nj - 1);
+                    la[e] = Ld[((jr * jr) >> 1) + min(lane, max(jr - 1, 0))] * d0;
+                }
+#pragma unroll
+                for (int e = 7; e >= 0; --e) {
+                    const int j = jb + e;
+                    const double xj = __shfl_sync(FULL, z0, j & 31);
+                    z0 = (j < min(nj, 32) && lane < j) ? fma(-la[e], xj, z0) : z0;
+                }
+            }
+            xcur[lane] = lane < nj ? z0 : 0.0;
+            xcur[lane + 32] = h1 ? z1 : 0.0;
+            if (lane == 0) CHT1(2);                                 // substitution
+        } else if (warp <= 2) {
+            // warps 1, 2 (thread t = column): publication of x_{J+1}, then S_{J-1} and v - anc of block J-2
+            const int t = tid - 32;
+            CHT0();
+            double va2 = 0.0;
+            if (J >= 2) va2 = __ldcg(bva + (J - 2) * TILE + t);     // no dependency on the chain: used in the next hop
+            if (J + 1 < nbp) {
+                const int jp = (J + 1) * TILE, njp = min(TILE, q.w - jp);
+                if (t < njp) { x[q.c0 + jp + t] = xprev[t]; put_solution(D, b, q.c0 + jp + t, xprev[t]); }
+                bar_named(2, 2 * 32);
+                if (t == 0) { __threadfence(); st_release(bb + J + 1, epoch); }   // for the helpers (nobody on the chain reads it)
+            }
+            if (J >= 1) {
+                if (Jn + 3 <= nbp - 1) {                            // block J-1 is a full block
+                    CHT0();
+                    spin_until_ge(bs + Jn, epoch);
+                    if (t == 0) CHT1(5);                            // waiting for the helper sum
+                    va_next -= __ldcg(F.bsum + q.c0 + Jn * TILE + t);
+                }
+                bar_named(1, NT - 32);                              // warps 3..7 have written pren = - L(J+1,J-1)^T x_{J+1}
+                pren[t] += va_next;
+                va_next = va2;
+            }
+            if (t == 1) CHT1(6);
+        } else {
+            // warps 3..7: the product with T2 for block J-1, then the requests for the tiles of the next hop
+            if (J >= 1) {
+                const int ht = tid - 96, hn = NT - 96;
+                CHT0();
+                stage_tile(CH_T1, J, Jn, ht, hn);                   // next hop: L(J,J-1)^T x_J (T1 is free since the barrier after A)
+                stage_diag(Jn, Jn & 1, ht, hn);
+                cp_async_commit();
+                if (J + 1 < nbp) {                                  // thirteen columns per warp, butterflies interleaved
+                    const double* T2 = sm + CH_T2;
+                    const double xa = xprev[lane], xb = xprev[lane + 32];
+#pragma unroll
+                    for (int kb = 0; kb < 13; kb += 5) {
+                        double v[5];
+#pragma unroll
+                        for (int e = 0; e < 5; ++e) {
+                            const int c = min(warp - 3 + 5 * (kb + e), TILE - 1);
+                            v[e] = fma(T2[c * TILE + lane + 32], xb, T2[c * TILE + lane] * xa);
+                        }
+#pragma unroll
+                        for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+                            for (int e = 0; e < 5; ++e) v[e] += __shfl_xor_sync(FULL, v[e], o);
+#pragma unroll
+                        for (int e = 0; e < 5; ++e) {
+                            const int c = warp - 3 + 5 * (kb + e);
+                            if (lane == 0 && kb + e < 13 && c < TILE) pren[c] = -v[e];
+                        }
+                    }
+                } else if (ht < TILE) {
+                    pren[ht] = 0.0;
+                }
+                bar_named(3, NT - 96);                              // the T2 buffer is free
+                if (J >= 2) stage_tile(CH_T2, J, J - 2, ht, hn);    // next hop: L(J,J-2)^T x_J
+                cp_async_commit();
+                if (ht == 0) CHT1(3);
+                bar_named(1, NT - 32);                              // pren is complete for warps 1, 2
+                cp_async_wait<0>();                                 // the tiles of the next hop have landed
+                if (ht == 0) CHT1(7);
+            }
+        }
+        __syncthreads();
+    }
+    {
+        const double* x0s = sm + CH_XS;                             // x_0
+        const int nj0 = min(TILE, q.w);
+        if (tid < nj0) { x[q.c0 + tid] = x0s[tid]; put_solution(D, b, q.c0 + tid, x0s[tid]); }
+    }
+    __syncthreads();
+    if (tid == 0) { __threadfence(); st_release(bb, epoch); red_release_add(F.sol_done_b + s, 1u); }
 }
 
 __global__ void __launch_bounds__(NT, 2) solve_dag_kernel(DevSym D, DagPlan F, double* b, double* x, uint32_t ef, uint32_t eb,
@@ -553,7 +777,10 @@ __global__ void __launch_bounds__(NT, 2) solve_dag_kernel(DevSym D, DagPlan F, d
         unsigned long long* tr = nullptr;
 #endif
         if (tk.w == 0) { if (tk.x == 0) fwd_small(D, F, tk.y, b, x, ef, sm, tr); else fwd_tiled(D, F, tk.y, tk.z, b, x, ef, sm); }
-        else           { if (tk.x == 0) bwd_small(D, F, tk.y, b, x, ef, eb, fused != 0, sm, tr); else bwd_tiled(D, F, tk.y, tk.z, b, x, ef, eb, fused != 0, sm); }
+        else if (tk.x == 0) bwd_small(D, F, tk.y, b, x, ef, eb, fused != 0, sm, tr);
+        else if (tk.x == 1) bwd_sum(D, F, tk.y, tk.z, x, eb, sm);
+        else if (tk.x == 3) bwd_chain(D, F, tk.y, b, x, ef, eb, fused != 0, sm, tr);
+        else                bwd_upd(D, F, tk.y, tk.z & 0xffff, tk.z >> 16, x, eb, sm);
         STRACE(4);
     }
 }
@@ -564,7 +791,8 @@ cudaError_t configure_solve_kernels(int max_smem_bytes, int small_max_r, int* ct
     int sbuf = ld_even(small_max_r) * SB;
     if (2 * sbuf < TILE * DLD) sbuf = (TILE * DLD + 1) / 2 + 1;      // the staged diagonal tile of the tiled tasks aliases the buffers
     sbuf = (sbuf + 1) & ~1;
-    const size_t bytes = (size_t)(OFF_BUF + 2 * sbuf + FWD_WORK_DOUBLES) * sizeof(double);
+    size_t bytes = (size_t)(OFF_BUF + 2 * sbuf + FWD_WORK_DOUBLES) * sizeof(double);
+    bytes = std::max(bytes, (size_t)CH_END * sizeof(double));        // the chain task of the backward solve
     if (bytes > (size_t)max_smem_bytes) return cudaErrorInvalidValue;
     cudaError_t e = cudaFuncSetAttribute(solve_dag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes - 256);
     if (e != cudaSuccess) return e;

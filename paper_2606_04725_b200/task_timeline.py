@@ -185,17 +185,19 @@ def main():
     # ------------------------------------------------------------------ solves
     tasks, st = h.get_task_trace(1)
     st = st.astype(np.int64)
-    if len(tasks):
-        t0 = st[:, 0].min()
-        fwd = tasks[:, 3] == 0
-        P("## Solves (`solve_dag_kernel`)")
+    ran = st[:, 0] > 0                                    # a fused solve (options.fuse_rhs) runs the backward tasks only
+    if ran.any():
+        t0 = st[ran, 0].min()
+        fwd = (tasks[:, 3] == 0) & ran
+        bwd = (tasks[:, 3] == 1) & ran
+        P("## Solves (`solve_dag_kernel`)" + ("" if fwd.any() else " -- fused: v = L^-1 P b came out of the factorization, backward tasks only"))
         P("")
-        for nm, m in (("forward (L v = P b)", fwd), ("backward (L^T x = v)", ~fwd)):
+        for nm, m in (("forward (L v = P b)", fwd), ("backward (L^T x = v)", bwd)):
             if m.any():
                 P(f"* {nm}: {int(m.sum())} tasks, first claim {(st[m, 0].min() - t0) / 1e3:.0f} us, last done {(st[m, 4].max() - t0) / 1e3:.0f} us, "
-                  f"median task {np.median(st[m, 4] - st[m, 0]) / 1e3:.1f} us")
+                  f"median task {np.median(st[m, 4] - st[m, 0]) / 1e3:.1f} us, CTA-time {((st[m, 4] - st[m, 0]).sum()) / 1e6:.1f} CTA-ms")
         tl = tasks[:, 0] == 1
-        for nm, m in (("forward block rows of tiled supernodes", fwd & tl), ("backward block columns of tiled supernodes", ~fwd & tl)):
+        for nm, m in (("forward block rows of tiled supernodes", fwd & tl), ("backward block columns of tiled supernodes", bwd & tl)):
             if m.any():
                 # hop time along the pivot blocks of the largest tiled supernode
                 s = int(np.bincount(tasks[m, 1]).argmax())
@@ -206,6 +208,29 @@ def main():
                 hops = np.diff(np.sort(ends)) / 1e3
                 P(f"* {nm}: supernode {s} (w = {W(s)}, r = {R(s)}): median hop between consecutive pivot blocks {np.median(hops):.2f} us "
                   f"over {len(hops)} hops = {hops.sum():.0f} us")
+        if bwd.any():
+            # chain of the backward solve: from the supernode that finished last up to the root
+            ns = info["nsuper"]
+            done_b = np.zeros(ns); first_b = np.full(ns, 1e30); cnt_b = np.zeros(ns, dtype=np.int64)
+            for k in np.nonzero(bwd)[0]:
+                q = int(tasks[k, 1])
+                done_b[q] = max(done_b[q], (st[k, 4] - t0) / 1e3); first_b[q] = min(first_b[q], (st[k, 0] - t0) / 1e3); cnt_b[q] += 1
+            P("")
+            P("### Backward chain: from the supernode that finished last up to the root (each starts when its parent is done)")
+            P("")
+            P("| supernode | type | w | r | block cols | parent done us | done us | span us | span / block col us |")
+            P("|---|---|---|---|---|---|---|---|---|")
+            q = int(np.argmax(done_b))
+            rows_out = []
+            while q >= 0:
+                pd = done_b[par[q]] if par[q] >= 0 else 0.0
+                nbp = (W(q) + TILE - 1) // TILE
+                tiled = cnt_b[q] > 1 or R(q) > 240
+                rows_out.append(f"| {q} | {'tiled' if tiled else 'smem'} | {W(q)} | {R(q)} | {nbp if tiled else '-'} | {pd:.0f} | {done_b[q]:.0f} | {done_b[q] - pd:.0f} | "
+                                f"{(done_b[q] - pd) / nbp if tiled else float('nan'):.1f} |")
+                q = int(par[q])
+            for ln in rows_out[::-1]:
+                P(ln)
     h.close()
     print("\n".join(out))
 
