@@ -246,6 +246,9 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
     // already published, so the other CTAs always get to it.
     std::vector<int64_t> pbase(ns, 0);
     int64_t part_doubles = 0;
+    std::vector<int32_t> cbase(ns, 0);
+    std::vector<int64_t> cdep_ptr(1, 0);
+    std::vector<uint32_t> cdep;
     {
         const double HOP_US = 3.0, UPD_US = 15.0, SMALL_US = 4.0;
         std::vector<double> ready(ns, 0.0), fin(ns, 0.0);
@@ -258,7 +261,36 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
             const int nchunk = (nbt[s] - nbp[s] + BWD_CH - 1) / BWD_CH;
             fin[s] = ready[s] + (nchunk > 0 ? UPD_US : 0.0) + HOP_US * nbp[s] + 5.0;
         }
-        std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return ready[a] != ready[b] ? ready[a] < ready[b] : a > b; });
+        // equal start estimates (siblings): the one with the longest chain of work below it first
+        std::vector<double> below(ns, 0.0);
+        for (int s = 0; s < ns; ++s) {
+            below[s] += fin[s] - ready[s];
+            const int p = S.sn_parent[s];
+            if (p >= 0) below[p] = std::max(below[p], below[s]);
+        }
+        std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
+            if (ready[a] != ready[b]) return ready[a] < ready[b];
+            return below[a] != below[b] ? below[a] > below[b] : a > b;
+        });
+        for (int s = 0; s < ns; ++s) {                   // what every chunk of ancestors' rows has to wait for
+            cbase[s] = (int32_t)(cdep_ptr.size() - 1);
+            if (!cls[s]) continue;
+            const int nchunk = (nbt[s] - nbp[s] + BWD_CH - 1) / BWD_CH;
+            const int32_t* rw = &S.rows[S.rows_ptr[s]];
+            for (int c = 0; c < nchunk; ++c) {
+                const int i0 = tile_bound(nbp[s] + c * BWD_CH, W(s), R(s), nbp[s]);
+                const int i1 = tile_bound(std::min(nbt[s], nbp[s] + (c + 1) * BWD_CH), W(s), R(s), nbp[s]);
+                const size_t first = cdep.size();
+                for (int i = i0; i < i1; ++i) {
+                    const int a = S.sn_of_col[rw[i]];
+                    // word offsets relative to F.sync (layout below): sol_done_b at 3 + 2 ns, blk_b at 3 + 3 ns + slots + bslots
+                    const uint32_t word = cls[a] ? (uint32_t)(3 + 3 * (int64_t)ns + slots + bslots + bbase[a] + (rw[i] - S.sn_start[a]) / TILE)
+                                                 : (uint32_t)(3 + 2 * (int64_t)ns + a);
+                    if (cdep.size() == first || cdep.back() != word) cdep.push_back(word);   // rows increase: equal words are adjacent
+                }
+                cdep_ptr.push_back((int64_t)cdep.size());
+            }
+        }
         for (int s : order) {
             if (!cls[s]) { stasks.push_back(make_int4(0, s, 0, 1)); continue; }
             const int nchunk = (nbt[s] - nbp[s] + BWD_CH - 1) / BWD_CH;
@@ -281,7 +313,9 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
     TRY(upload(h, cbnd, &F.cbnd));
     TRY(upload(h, S.sn_parent, &F.sn_parent));
     TRY(upload(h, pbase, &tl)); F.pbase = tl;
-    TRY(dalloc(h, (size_t)part_doubles, &F.bpart, false)); TRY(dalloc(h, (size_t)S.nt, &F.bsum, false)); TRY(dalloc(h, (size_t)S.nt, &F.bva, false));
+    TRY(upload(h, cbase, &F.cbase)); TRY(upload(h, cdep_ptr, &tl)); F.cdep_ptr = tl;
+    { const uint32_t* tu = nullptr; TRY(upload(h, cdep, &tu)); F.cdep = tu; }
+    TRY(dalloc(h, (size_t)part_doubles, &F.bpart, false)); TRY(dalloc(h, (size_t)S.nt, &F.bsum, false));
     TRY(upload(h, ksrc, &h->D.kent_src)); TRY(upload(h, kdst, &h->D.kent_dst));
     F.sync_words = 3 + 3 * (int64_t)ns + slots + 5 * bslots;
     TRY(dalloc(h, (size_t)F.sync_words, &F.sync));

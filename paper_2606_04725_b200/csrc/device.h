@@ -97,7 +97,9 @@ struct DagPlan {
     uint32_t* blk_u = nullptr;           // block slots: finished chunk tasks of the backward solve per block column
     uint32_t* blk_s = nullptr;           // block slots: helper sum S_J of the backward solve written
     double* bsum = nullptr;              // nt: the helper sums (pivot positions)
-    double* bva = nullptr;               // nt: v - anc per column of the tiled supernodes (backward chain prologue)
+    const int32_t* cbase = nullptr;      // ns: first chunk of a tiled supernode in cdep_ptr
+    const int64_t* cdep_ptr = nullptr;   // per chunk (supernode, c): the flags (word offsets into sync, all "done when >= call
+    const uint32_t* cdep = nullptr;      // number") of the pieces of x its rows belong to
     const int64_t* pbase = nullptr;      // ns: offset into bpart of a tiled supernode's partial sums [chunk][w]
     double* bpart = nullptr;
     uint32_t* sub_done = nullptr;        // block slots: published 8-column blocks of the diagonal tile L_JJ, (epoch-1)*16 + count

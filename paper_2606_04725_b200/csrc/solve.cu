@@ -443,7 +443,9 @@ struct BwdTile {
     }
 };
 
-// chunk task (s, J, c): partial[c][J] = sum over the ancestors' block rows I in chunk c of L(I,J)^T x_I
+// chunk task (s, J, c): partial[c][J] = sum over the ancestors' block rows I in chunk c of L(I,J)^T x_I.  It waits for exactly the
+// pieces of x its rows touch (the analysis lists their flags: blocks of the ancestors' chains, small ancestors), so the chunk
+// tasks of a supernode run WHILE the chain of its parent is still going down its blocks
 __device__ __forceinline__ void bwd_upd(const DevSym& D, const DagPlan& F, int s, int J, int c, const double* x, uint32_t epoch, double* sm) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const Sn q = sn_of(D, s);
@@ -454,7 +456,10 @@ __device__ __forceinline__ void bwd_upd(const DevSym& D, const DagPlan& F, int s
     const BwdTile T{q, nbp, j0, nj};
     double cur[16], nxt[16];
     T.load(Ia, cur);
-    if (tid == 0) { const int p = F.sn_parent[s]; if (p >= 0) spin_until_ge(F.sol_done_b + p, epoch * (uint32_t)F.target_b[p]); }
+    {
+        const int64_t d0 = F.cdep_ptr[F.cbase[s] + c], d1 = F.cdep_ptr[F.cbase[s] + c + 1];
+        for (int64_t k = d0 + tid; k < d1; k += NT) spin_until_ge(F.sync + F.cdep[k], epoch);
+    }
     __syncthreads();
     double acc[8];
 #pragma unroll
@@ -546,7 +551,16 @@ __device__ __forceinline__ void bwd_chain(const DevSym& D, const DagPlan& F, int
     uint32_t* bb = F.blk_b + F.bbase[s];
     const uint32_t* bu = F.blk_u + F.bbase[s];
     const uint32_t* bs = F.blk_s + F.bbase[s];
-    double* bva = F.bva + q.c0;                                     // v - anc of this supernode's columns (written by the prologue)
+    // v - anc for column t of block Jb: v from the right-hand-side row of the panel (fused) or from the forward solve; anc = the
+    // chunk tasks' partial sums in chunk order (the caller has seen their flag)
+    auto va_of = [&](int Jb, int t) {
+        const int c = Jb * TILE + t, col = q.c0 + c;
+        double a = col == D.aug_col ? 0.0 : fused ? __ldcg(q.P + (q.r - 1) + (int64_t)c * q.ld) : __ldcg(x + col);
+        const double* pp = F.bpart + F.pbase[s] + c;
+#pragma unroll 4
+        for (int k = 0; k < nchunk; ++k) a -= __ldcg(pp + (int64_t)k * q.w);
+        return a;
+    };
     auto stage_diag = [&](int J, int buf, int t0, int nthr) {       // L(J,J)^T packed + pivot reciprocals, cp.async
         const int j0 = J * TILE, nj = min(TILE, q.w - j0);
         double* Ld = sm + CH_LD + buf * LDP;
@@ -567,32 +581,25 @@ __device__ __forceinline__ void bwd_chain(const DevSym& D, const DagPlan& F, int
     stage_diag(J, J & 1, tid, NT);
     cp_async_commit();
     if (tid < 2 * TILE) sm[CH_XS + tid] = 0.0;
-    // dependencies: the forward half (two-sided solve), the parent, ALL chunk tasks of this supernode
+    // dependencies: the forward half (two-sided solve) and the chunk tasks of the first block (the later blocks' chunk tasks are
+    // checked two hops ahead of their use).  The chain itself reads nothing of the ancestors: the chunk tasks carry that
+    // dependency (a supernode without rows below its pivots has no ancestors).
     if (tid == 0) {
         if (!fused) spin_until_ge(F.sol_done_f + s, ef * (uint32_t)F.target_f[s]);
-        const int p = F.sn_parent[s];
-        if (p >= 0) spin_until_ge(F.sol_done_b + p, epoch * (uint32_t)F.target_b[p]);
+        if (nchunk > 0) spin_until_ge(bu + J, epoch * (uint32_t)nchunk);
     }
-    if (nchunk > 0) for (int k = tid; k < nbp; k += NT) spin_until_ge(bu + k, epoch * (uint32_t)nchunk);
     __syncthreads();
-    // v - anc for every column: v from the right-hand-side row of the panel (fused) or from the forward solve; anc = the chunk
-    // tasks' partial sums in chunk order.  Written to global memory; the hops fetch 64 of them two blocks ahead.
-    for (int c = tid; c < q.w; c += NT) {
-        const int col = q.c0 + c;
-        double a = col == D.aug_col ? 0.0 : fused ? __ldcg(q.P + (q.r - 1) + (int64_t)c * q.ld) : __ldcg(x + col);
-        const double* pp = F.bpart + F.pbase[s] + c;
-        for (int k = 0; k < nchunk; ++k) a -= __ldcg(pp + (int64_t)k * q.w);
-        bva[c] = a;
-        if (c >= J * TILE) sm[CH_PRE + (J & 1) * TILE + c - J * TILE] = a;
-    }
+    double va_next = 0.0;                                           // threads 32..95: v - anc of the block the NEXT hop prepares
     {
         const int nj = min(TILE, q.w - J * TILE);
-        if (tid >= nj && tid < TILE) sm[CH_PRE + (J & 1) * TILE + tid] = 0.0;
+        if (tid < TILE) sm[CH_PRE + (J & 1) * TILE + tid] = tid < nj ? va_of(J, tid) : 0.0;
+        if (J >= 1 && tid >= 32 && tid < 32 + TILE) {
+            if (nchunk > 0) spin_until_ge(bu + J - 1, epoch * (uint32_t)nchunk);
+            va_next = va_of(J - 1, tid - 32);
+        }
     }
     cp_async_wait<0>();                                             // the first diagonal tile has landed
-    __syncthreads();                                                // (also orders the bva writes before the loads below)
-    double va_next = 0.0;                                           // threads 32..95: v - anc of the block the NEXT hop prepares
-    if (J >= 1 && tid >= 32 && tid < 32 + TILE) va_next = bva[(J - 1) * TILE + tid - 32];
+    __syncthreads();
 #ifdef NMPC_TRACE_BUILD
     if (tr && tid == 0) { tr[2] = 0; tr[3] = 0; tr[5] = 0; tr[6] = 0; tr[7] = 0; }
 #endif
@@ -672,7 +679,10 @@ __device__ __forceinline__ void bwd_chain(const DevSym& D, const DagPlan& F, int
             const int t = tid - 32;
             CHT0();
             double va2 = 0.0;
-            if (J >= 2) va2 = __ldcg(bva + (J - 2) * TILE + t);     // no dependency on the chain: used in the next hop
+            if (J >= 2) {                                           // no dependency on the chain: used in the next hop
+                if (nchunk > 0) spin_until_ge(bu + J - 2, epoch * (uint32_t)nchunk);
+                va2 = va_of(J - 2, t);
+            }
             if (J + 1 < nbp) {
                 const int jp = (J + 1) * TILE, njp = min(TILE, q.w - jp);
                 if (t < njp) { x[q.c0 + jp + t] = xprev[t]; put_solution(D, b, q.c0 + jp + t, xprev[t]); }
