@@ -66,7 +66,12 @@ typedef struct {
  *   DISTILL [alpha, D, F_feed, x_feed, A_c, A_t, A_r, feed_index, u_bar, w_u]   (Problem 29)
  *   PLATE   [g, a, kappa_r, T_amb, b, nseg, w_T, w_u]    5-point heat equation + radiative loss, edge heaters
  * lb/ub: HOST, length nx+nu (one stage, repeated over stages); +-INFINITY = no bound.
- * u_init: HOST, length nu, cold-start input guess.                                                        */
+ * u_init: HOST, length nu, cold-start input guess.
+ * General linear rows (Problem 5/6: inequality constraints g and the control-horizon constraints
+ * y_c,u = y_c,u_c; reading G22 of DESIGN.md): n_g rows  g_lo <= G y <= g_hi  over the whole y, stacked below the N*nx dynamics
+ * rows; G as HOST CSR (g_rowptr[n_g+1], g_colind strictly increasing per row, g_val), all copied.  g_lo == g_hi: an equality
+ * row, lifted like every equality (Eq. 16: g_lo - gamma <= . <= g_hi + gamma); else an inequality row, either side may be
+ * -+INFINITY (one-sided).  n_g = 0: none (the pointers are ignored).  m = N*nx + n_g rows in all (slacks, multipliers, J). */
 typedef struct {
     int32_t model;
     int32_t N, nx, nu, nr;       /* nr = reference entries per stage                                        */
@@ -76,6 +81,12 @@ typedef struct {
     const double* lb;
     const double* ub;
     const double* u_init;
+    int64_t n_g;
+    const int64_t* g_rowptr;
+    const int32_t* g_colind;
+    const double* g_val;
+    const double* g_lo;
+    const double* g_hi;
 } nmpc_ocp;
 
 /* Options; pass NULL for the defaults (nmpc_default_options).  IPM constants are the readings S0 of

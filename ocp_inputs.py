@@ -14,6 +14,12 @@ Variable layout (both sides):  y = [x_1,u_1, x_2,u_2, ..., x_N,u_N]  (stage-majo
 x_0 is a parameter.  Equality rows: stage k holds rows k*nx .. (k+1)*nx-1 of
 h_k = x_k - x_{k-1} - dt*F(x_k,u_k).
 
+General linear path rows (optional, `make_config(..., Nc=, move_limit=,
+power_limit=)`): rows  lo <= G y <= hi  appended AFTER the N*nx dynamics rows, stated here as plain CSR data:
+  * control-horizon hold:  u_k - u_{k-1} = 0 for the stages k >= Nc (lo = hi = 0),
+  * input move limits:  -move_limit <= u_k - u_{k-1} <= move_limit for 1 <= k < Nc (two-sided inequality rows g),
+  * total input limit:  sum_a u_{k,a} <= power_limit for every stage (one-sided inequality row g, lo = -inf).
+
 Model parameter vectors (`model_params`, float64), by model id:
   MODEL_VDP     : [w_x, w_u]
   MODEL_DISTILL : [alpha, D, F_feed, x_feed, A_c, A_t, A_r, feed_index, u_bar, w_u]
@@ -39,7 +45,9 @@ class OCPConfig:
         self.__dict__.update(kw)
         self.nv = self.nx + self.nu
         self.n = self.N * self.nv
-        self.m = self.N * self.nx
+        self.m_dyn = self.N * self.nx          # dynamics rows h_k
+        self.m = self.m_dyn                    # all constraint rows (dynamics + general linear rows, see add_path_rows)
+        self.g_rows = None
 
     def __repr__(self):
         return (f"OCPConfig({self.name}: model={self.model} N={self.N} nx={self.nx} nu={self.nu} "
@@ -125,11 +133,43 @@ def _plate(rng, name, g, nseg, N, R, noise_sd) -> OCPConfig:
                      ref_seq=[ref], noise_seq=noise, R=R, x0_clip=(-np.inf, 599.0))
 
 
+def add_path_rows(cfg: OCPConfig, Nc=None, move_limit=None, power_limit=None) -> OCPConfig:
+    """Append general linear rows lo <= G y <= hi (module docstring) to `cfg` as CSR data: cfg.g_rows = dict(rowptr, colind,
+    val, lo, hi); cfg.m grows by their number.  Pure index bookkeeping: no arithmetic of the method."""
+    N, nx, nu, nv = cfg.N, cfg.nx, cfg.nu, cfg.nv
+    Nc = N if Nc is None else int(Nc)
+    rowptr, colind, val, lo, hi = [0], [], [], [], []
+
+    def row(cols, vals, l, h):
+        order = np.argsort(cols)
+        colind.extend(int(cols[i]) for i in order); val.extend(float(vals[i]) for i in order)
+        rowptr.append(len(colind)); lo.append(l); hi.append(h)
+
+    for k in range(1, N):
+        for a in range(nu):
+            cols, vals = [(k - 1) * nv + nx + a, k * nv + nx + a], [-1.0, 1.0]
+            if k >= Nc:
+                row(cols, vals, 0.0, 0.0)
+            elif move_limit is not None:
+                row(cols, vals, -float(move_limit), float(move_limit))
+    if power_limit is not None:
+        for k in range(N):
+            row([k * nv + nx + a for a in range(nu)], [1.0] * nu, -np.inf, float(power_limit))
+    if len(lo) == 0:
+        return cfg
+    cfg.g_rows = dict(rowptr=np.array(rowptr, dtype=np.int64), colind=np.array(colind, dtype=np.int32),
+                      val=np.array(val, dtype=np.float64), lo=np.array(lo, dtype=np.float64), hi=np.array(hi, dtype=np.float64))
+    cfg.m = cfg.m_dyn + len(lo)
+    cfg.path_rows = dict(Nc=Nc, move_limit=move_limit, power_limit=power_limit)
+    return cfg
+
+
 def make_config(name: str, **override) -> OCPConfig:
     """Return config `name` in {C0..C4}.  `override` may shrink N / g / trays for small test cases
     (the seeded stream is the same; only the sizes change)."""
     idx = CONFIG_NAMES.index(name)
     rng = np.random.default_rng(MASTER_SEED + idx)
+    path = {k: override.pop(k) for k in ("Nc", "move_limit", "power_limit") if k in override}
     if name == "C0":
         cfg = _vdp(rng)
     elif name == "C1":
@@ -144,6 +184,8 @@ def make_config(name: str, **override) -> OCPConfig:
         cfg = _distill(rng, "C4", override.pop("trays", 128), override.pop("N", 400), override.pop("R", 50))
     if override:
         raise TypeError(f"unknown overrides {sorted(override)}")
+    if path:
+        add_path_rows(cfg, **path)
     return cfg
 
 

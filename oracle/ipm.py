@@ -67,6 +67,12 @@ class LiftedIPM:
         self.hasL, self.hasU = np.isfinite(self.nlp.lb), np.isfinite(self.nlp.ub)
         self.lb = np.where(self.hasL, self.nlp.lb, 0.0)
         self.ub = np.where(self.hasU, self.nlp.ub, 0.0)
+        # Row intervals cl <= c(y) <= cu (oracle/nlp.py: row_bounds): the gamma tube of Eq. (16) for every equality row, the
+        # stated bounds for the inequality rows g of Problem (6).  Slack form: c - cu + s+ = 0, -c + cl + s- = 0; a side that
+        # is infinite has no slack and no multiplier (kept as s = 1, w = 0 and left out of every formula).  Reading G22.
+        cl, cu = self.nlp.row_bounds(self.opt["gamma"])
+        self.rL, self.rU = np.isfinite(cl), np.isfinite(cu)
+        self.cl, self.cu = np.where(self.rL, cl, 0.0), np.where(self.rU, cu, 0.0)
 
     # ---------------------------------------------------------------------------------------------
     def _make_cholesky(self, K):
@@ -85,11 +91,11 @@ class LiftedIPM:
         hasL, hasU = self.hasL, self.hasU
         dL, dU = st.y - self.lb, self.ub - st.y
         r_d = gradf + J.T @ (st.wp - st.wm) - np.where(hasL, st.zL, 0.0) + np.where(hasU, st.zU, 0.0)
-        r_pp = c - o["gamma"] + st.sp
-        r_pm = -c - o["gamma"] + st.sm
-        comp = np.concatenate([st.sp * st.wp - mu, st.sm * st.wm - mu,
+        r_pp = np.where(self.rU, c - self.cu + st.sp, 0.0)
+        r_pm = np.where(self.rL, -c + self.cl + st.sm, 0.0)
+        comp = np.concatenate([(st.sp * st.wp - mu)[self.rU], (st.sm * st.wm - mu)[self.rL],
                                (dL * st.zL - mu)[hasL], (dU * st.zU - mu)[hasU]])
-        nmult = 2 * self.nlp.m + int(hasL.sum()) + int(hasU.sum())
+        nmult = int(self.rU.sum()) + int(self.rL.sum()) + int(hasL.sum()) + int(hasU.sum())
         l1 = st.wp.sum() + st.wm.sum() + st.zL[hasL].sum() + st.zU[hasU].sum()
         s_d = max(o["s_max"], l1 / nmult) / o["s_max"]
         E = max(np.max(np.abs(r_d)) / s_d, np.max(np.abs(r_pp)), np.max(np.abs(r_pm)),
@@ -100,15 +106,14 @@ class LiftedIPM:
     def _theta(self, y, s_p, s_m):
         """Constraint violation of the lifted equalities (the r_p rows of Eq. 9), 1-norm as in [17] Eq. (19)."""
         c = self.nlp.constraints(y)
-        g = self.opt["gamma"]
-        return float(np.sum(np.abs(c - g + s_p)) + np.sum(np.abs(-c - g + s_m)))
+        return float(np.sum(np.abs(c - self.cu + s_p)[self.rU]) + np.sum(np.abs(-c + self.cl + s_m)[self.rL]))
 
     def _phi(self, y, s_p, s_m, mu):
         """Barrier objective of the lifted problem with native bounds: f - mu sum ln(slacks, bound distances)  ([17] Eq. 3a)."""
         hasL, hasU = self.hasL, self.hasU
-        if np.any(s_p <= 0.0) or np.any(s_m <= 0.0) or np.any((y - self.lb)[hasL] <= 0.0) or np.any((self.ub - y)[hasU] <= 0.0):
+        if np.any(s_p[self.rU] <= 0.0) or np.any(s_m[self.rL] <= 0.0) or np.any((y - self.lb)[hasL] <= 0.0) or np.any((self.ub - y)[hasU] <= 0.0):
             return np.inf                                   # outside the domain of the barrier (never the case from alpha_max down)
-        return float(self.nlp.objective(y) - mu * (np.sum(np.log(s_p)) + np.sum(np.log(s_m))
+        return float(self.nlp.objective(y) - mu * (np.sum(np.log(s_p[self.rU])) + np.sum(np.log(s_m[self.rL]))
                                                    + np.sum(np.log((y - self.lb)[hasL])) + np.sum(np.log((self.ub - y)[hasU]))))
 
     def _filter_line_search(self, st, mu, dy, ds_p, ds_m, a_max, gradf, flt, th_min):
@@ -153,11 +158,11 @@ class LiftedIPM:
         y = np.where(self.hasU, np.minimum(y, self.ub - pU), y)
         c = nlp.constraints(y)
         mu0 = o["mu0"]
-        s_p = np.maximum(o["gamma"] - c, o["s_floor"])
-        s_m = np.maximum(o["gamma"] + c, o["s_floor"])
+        s_p = np.where(self.rU, np.maximum(self.cu - c, o["s_floor"]), 1.0)
+        s_m = np.where(self.rL, np.maximum(c - self.cl, o["s_floor"]), 1.0)
         zL = np.where(self.hasL, mu0 / np.where(self.hasL, y - self.lb, 1.0), 0.0)
         zU = np.where(self.hasU, mu0 / np.where(self.hasU, self.ub - y, 1.0), 0.0)
-        return IPMState(y, s_p, s_m, mu0 / s_p, mu0 / s_m, zL, zU), mu0
+        return IPMState(y, s_p, s_m, np.where(self.rU, mu0 / s_p, 0.0), np.where(self.rL, mu0 / s_m, 0.0), zL, zU), mu0
 
     def warm_start(self, prev):
         """S1 warm init: z_{k+1} <- z*_k verbatim (Alg. 1 line 10), smaller mu."""
@@ -212,7 +217,7 @@ class LiftedIPM:
             q_p, q_m = st.wp / st.sp, st.wm / st.sm
             W = nlp.hessian(st.y, st.wp - st.wm)
             K0 = (W + sp.diags(Sigma_x) + J.T @ sp.diags(q_p + q_m) @ J).tocsc()
-            t = q_p * r_pp + mu / st.sp - q_m * r_pm - mu / st.sm
+            t = q_p * r_pp + np.where(self.rU, mu / st.sp, 0.0) - q_m * r_pm - np.where(self.rL, mu / st.sm, 0.0)
             b = -(gradf - np.where(hasL, mu / dL, 0.0) + np.where(hasU, mu / dU, 0.0) + J.T @ t)
             # S7: inertia correction (Eq. 13/15) + NumCholesky      Alg. 2 lines 7-13
             if self.chol is None:
@@ -238,9 +243,10 @@ class LiftedIPM:
 
             def eliminated(dy_):
                 Jdy = J @ dy_
-                ds_p_ = -r_pp - Jdy
-                ds_m_ = -r_pm + Jdy
-                return (ds_p_, ds_m_, -(st.wp - mu / st.sp) - q_p * ds_p_, -(st.wm - mu / st.sm) - q_m * ds_m_,
+                ds_p_ = np.where(self.rU, -r_pp - Jdy, 0.0)
+                ds_m_ = np.where(self.rL, -r_pm + Jdy, 0.0)
+                return (ds_p_, ds_m_, np.where(self.rU, -(st.wp - mu / st.sp) - q_p * ds_p_, 0.0),
+                        np.where(self.rL, -(st.wm - mu / st.sm) - q_m * ds_m_, 0.0),
                         np.where(hasL, -(st.zL - mu / dL) - st.zL / dL * dy_, 0.0),
                         np.where(hasU, -(st.zU - mu / dU) + st.zU / dU * dy_, 0.0))
 

@@ -29,7 +29,8 @@ class nmpc_pattern(C.Structure):
 
 class nmpc_ocp(C.Structure):
     _fields_ = [("model", c_i32), ("N", c_i32), ("nx", c_i32), ("nu", c_i32), ("nr", c_i32), ("dt", c_dbl),
-                ("model_params", c_vp), ("n_model_params", c_i32), ("lb", c_vp), ("ub", c_vp), ("u_init", c_vp)]
+                ("model_params", c_vp), ("n_model_params", c_i32), ("lb", c_vp), ("ub", c_vp), ("u_init", c_vp),
+                ("n_g", c_i64), ("g_rowptr", c_vp), ("g_colind", c_vp), ("g_val", c_vp), ("g_lo", c_vp), ("g_hi", c_vp)]
 
 
 class nmpc_options(C.Structure):
@@ -188,8 +189,15 @@ def make_ocp(cfg):
     keep = dict(mp=np.ascontiguousarray(cfg.model_params, dtype=np.float64),
                 lb=np.ascontiguousarray(cfg.lb, dtype=np.float64), ub=np.ascontiguousarray(cfg.ub, dtype=np.float64),
                 ui=np.ascontiguousarray(cfg.u_init, dtype=np.float64))
+    g = getattr(cfg, "g_rows", None)
+    if g is not None:                                       # general linear rows lo <= G y <= hi (include/nmpc.h)
+        keep.update(grp=np.ascontiguousarray(g["rowptr"], dtype=np.int64), gci=np.ascontiguousarray(g["colind"], dtype=np.int32),
+                    gv=np.ascontiguousarray(g["val"], dtype=np.float64), glo=np.ascontiguousarray(g["lo"], dtype=np.float64),
+                    ghi=np.ascontiguousarray(g["hi"], dtype=np.float64))
+    gargs = ((len(keep["glo"]), keep["grp"].ctypes.data, keep["gci"].ctypes.data, keep["gv"].ctypes.data, keep["glo"].ctypes.data,
+              keep["ghi"].ctypes.data) if g is not None else (0, None, None, None, None, None))
     o = nmpc_ocp(cfg.model, cfg.N, cfg.nx, cfg.nu, cfg.nr, cfg.dt, keep["mp"].ctypes.data, len(keep["mp"]),
-                 keep["lb"].ctypes.data, keep["ub"].ctypes.data, keep["ui"].ctypes.data)
+                 keep["lb"].ctypes.data, keep["ub"].ctypes.data, keep["ui"].ctypes.data, *gargs)
     o._keep = keep
     return o
 

@@ -577,7 +577,18 @@ nmpc_status nmpc_analyze(const nmpc_pattern* pattern, const nmpc_ocp* ocp, const
             TRY(upload(h, mm.k_w, &M.k_w)); TRY(upload(h, mm.k_diag, &M.k_diag));
             const int nv = mm.desc.nv;
             std::vector<double> lb(mm.n), ub(mm.n), ui(std::max(1, mm.desc.nu), 0.0);
-            h->nmult = 2 * (int)mm.m;
+            // row intervals: the gamma tube of Eq. (16) around every equality row (dynamics, general rows with lo == hi), the
+            // stated interval for the inequality rows; an infinite side has no slack and no multiplier
+            std::vector<double> cl(mm.m), cu(mm.m);
+            h->nmult = 0;
+            for (int64_t r = 0; r < mm.m; ++r) {
+                const bool eq = mm.cl[r] == mm.cu[r];
+                cl[r] = eq ? mm.cl[r] - h->opt.gamma : mm.cl[r]; cu[r] = eq ? mm.cu[r] + h->opt.gamma : mm.cu[r];
+                h->nmult += (int)std::isfinite(cl[r]) + (int)std::isfinite(cu[r]);
+                if (!std::isfinite(cl[r]) && !std::isfinite(cu[r])) { h->err = "general row without a finite bound"; return NMPC_E_ARG; }
+            }
+            M.m_dyn = mm.m_dyn;
+            TRY(upload(h, cl, &M.cl)); TRY(upload(h, cu, &M.cu)); TRY(upload(h, mm.g_val, &M.g_val));
             for (int64_t i = 0; i < mm.n; ++i) {
                 lb[i] = ocp->lb ? ocp->lb[i % nv] : -INFINITY; ub[i] = ocp->ub ? ocp->ub[i % nv] : INFINITY;
                 if (std::isfinite(lb[i])) h->nmult++;
@@ -1106,6 +1117,7 @@ nmpc_status nmpc_hykkt_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double
     if (!h) return NMPC_E_ARG;
     DeviceGuard dg(h);
     if (!h->has_model) { h->err = "nmpc_hykkt_solve needs a model (nmpc_ocp)"; return NMPC_E_STATE; }
+    if (h->M.m != h->M.m_dyn) { h->err = "nmpc_hykkt_solve: general rows (nmpc_ocp.n_g) are handled by nmpc_ipm_solve only"; return NMPC_E_STATE; }
     if (use_y0 && !y_inout) return NMPC_E_ARG;
     const nmpc_options& o = h->opt;
     const DevModel& M = h->M;
@@ -1128,7 +1140,7 @@ nmpc_status nmpc_hykkt_solve(nmpc_handle h, int32_t warm, int32_t use_y0, double
     launch_fill(M.m, 0.0, V.wm, st);                                           // the model evaluation's lam = w+ - w-
     launch_fill(M.m, o.gamma_h, V.q, st);                                      // J^T diag(q) J = gamma_h J^T J in the assembly
     h->launches += 2;
-    const int nmult = h->nmult - (int)M.m;                                     // m equality multipliers + the bound multipliers
+    const int nmult = h->nmult - (int)M.m;                                     // m equality multipliers + the bound multipliers (no general rows here)
     double eta_last = 0.0, E0 = 0.0;
     int it = 0, nfact = 0, retries = 0;
     int64_t ncg_total = 0;

@@ -133,6 +133,9 @@ void launch_solve(const DevSym& D, const DagPlan& F, double* rhs_inout, double* 
 struct DevModel {                 // device copies of the model maps (symbolic.h: ModelMaps) + parameters
     ModelDesc desc;
     int64_t n = 0, m = 0, nnzJ = 0, nnzW = 0, nnzK = 0;
+    int64_t m_dyn = 0;                                                  // rows [0, m_dyn): dynamics h_k; [m_dyn, m): general linear rows
+    const double* g_val = nullptr;                                      // their values, in J order from J_ptr[m_dyn] on
+    const double* cl = nullptr; const double* cu = nullptr;             // m: row intervals cl <= c(y) <= cu (gamma tube included), +-inf = no such side
     const int64_t* J_ptr = nullptr; const int32_t* J_idx = nullptr;
     const int64_t* jt_ptr = nullptr; const int32_t* jt_idx = nullptr; const int32_t* jt_row = nullptr;
     const int64_t* trip_ptr = nullptr; const int32_t* trip_a = nullptr; const int32_t* trip_b = nullptr; const int32_t* trip_r = nullptr;

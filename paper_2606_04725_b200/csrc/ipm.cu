@@ -35,7 +35,13 @@ __global__ void __launch_bounds__(NT) model_eval_kernel(DevModel M, const double
     const int hc = hess_count(D);
     const int64_t nW = (int64_t)D.N * hc;
     const int64_t idx = blockIdx.x * (int64_t)NT + threadIdx.x;
-    if (idx < M.m) {                                             // constraint row (k, c): h and its Jacobian row
+    if (idx >= M.m_dyn && idx < M.m) {                           // general linear row: c = G_r y, constant Jacobian row
+        if (!c_out && !Jval) return;
+        const double* gv = M.g_val - M.J_ptr[M.m_dyn];
+        double acc = 0.0;
+        for (int64_t p = M.J_ptr[idx]; p < M.J_ptr[idx + 1]; ++p) { const double v = gv[p]; acc += v * y[M.J_idx[p]]; if (Jval) Jval[p] = v; }
+        if (c_out) c_out[idx] = acc;
+    } else if (idx < M.m) {                                      // constraint row (k, c): h and its Jacobian row
         if (!c_out && !Jval) return;
         const int k = (int)(idx / nx), c = (int)(idx - (int64_t)k * nx);
         const double* x = y + (int64_t)k * nv;
@@ -172,9 +178,11 @@ __global__ void __launch_bounds__(NT) cold_y_kernel(DevModel M, IpmVectors V, co
 __global__ void __launch_bounds__(NT) cold_s_kernel(DevModel M, IpmVectors V, double gamma, double s_floor, double mu0) {
     const int64_t r = blockIdx.x * (int64_t)NT + threadIdx.x;
     if (r >= M.m) return;
-    const double c = V.c[r];
-    const double sp = fmax(gamma - c, s_floor), sm = fmax(gamma + c, s_floor);
-    V.sp[r] = sp; V.sm[r] = sm; V.wp[r] = mu0 / sp; V.wm[r] = mu0 / sm;
+    (void)gamma;                                         // the tube is part of the row interval [cl, cu] (api.cu)
+    const double c = V.c[r], cl = M.cl[r], cu = M.cu[r];
+    const bool hasU = cu < INF, hasL = cl > -INF;
+    const double sp = hasU ? fmax(cu - c, s_floor) : 1.0, sm = hasL ? fmax(c - cl, s_floor) : 1.0;
+    V.sp[r] = sp; V.sm[r] = sm; V.wp[r] = hasU ? mu0 / sp : 0.0; V.wm[r] = hasL ? mu0 / sm : 0.0;
 }
 
 __global__ void __launch_bounds__(NT) warm_push_kernel(DevModel M, IpmVectors V, double wpush) {
@@ -192,6 +200,7 @@ __global__ void __launch_bounds__(NT) warm_push_kernel(DevModel M, IpmVectors V,
 //   partial[b][0..6] = max|r_d|, max|r_p+|, max|r_p-|, max comp product, min comp product, sum multipliers, #non-finite
 // ------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(NT) residual_kernel(DevModel M, IpmVectors V, double gamma) {
+    (void)gamma;                                         // part of the row intervals [cl, cu]
     Red<7> a;
     a.v[0] = a.v[1] = a.v[2] = 0.0; a.v[3] = -INF; a.v[4] = INF; a.v[5] = 0.0; a.v[6] = 0.0;
     // variables: GV lanes share one column of J (the input columns hold 2 nx entries), fixed butterfly order
@@ -220,13 +229,14 @@ __global__ void __launch_bounds__(NT) residual_kernel(DevModel M, IpmVectors V, 
     }
     for (int64_t r = gtid; r < M.m; r += gthreads) {
         const double c = V.c[r], sp = V.sp[r], sm = V.sm[r], wp = V.wp[r], wm = V.wm[r];
-        const double rpp = c - gamma + sp, rpm = -c - gamma + sm;
+        const double cl = M.cl[r], cu = M.cu[r];
+        const bool hasU = cu < INF, hasL = cl > -INF;     // a row side without a bound: s = 1, w = 0, out of every formula
+        const double rpp = hasU ? c - cu + sp : 0.0, rpm = hasL ? -c + cl + sm : 0.0;
         V.r_pp[r] = rpp; V.r_pm[r] = rpm;
         a.v[1] = fmax(a.v[1], fabs(rpp)); a.v[2] = fmax(a.v[2], fabs(rpm));
         if (!isfinite(rpp) || !isfinite(rpm)) a.v[6] += 1.0;
-        const double c1 = sp * wp, c2 = sm * wm;
-        a.v[3] = fmax(a.v[3], fmax(c1, c2)); a.v[4] = fmin(a.v[4], fmin(c1, c2));
-        a.v[5] += wp + wm;
+        if (hasU) { const double c1 = sp * wp; a.v[3] = fmax(a.v[3], c1); a.v[4] = fmin(a.v[4], c1); a.v[5] += wp; }
+        if (hasL) { const double c2 = sm * wm; a.v[3] = fmax(a.v[3], c2); a.v[4] = fmin(a.v[4], c2); a.v[5] += wm; }
     }
     const int ops[7] = {0, 0, 0, 0, 1, 2, 2};
     block_reduce<7>(a, ops, V.partial + (int64_t)blockIdx.x * 8);
@@ -248,9 +258,10 @@ __global__ void __launch_bounds__(NT) sigma_rows_kernel(DevModel M, IpmVectors V
     const int64_t r = blockIdx.x * (int64_t)NT + threadIdx.x;
     if (r >= M.m) return;
     const double sp = V.sp[r], sm = V.sm[r];
-    const double qp = V.wp[r] / sp, qm = V.wm[r] / sm;
+    const bool hasU = M.cu[r] < INF, hasL = M.cl[r] > -INF;
+    const double qp = V.wp[r] / sp, qm = V.wm[r] / sm;   // 0 for a side without a bound (w = 0, s = 1)
     V.q[r] = qp + qm;
-    V.t[r] = qp * V.r_pp[r] + mu / sp - qm * V.r_pm[r] - mu / sm;
+    V.t[r] = qp * V.r_pp[r] + (hasU ? mu / sp : 0.0) - qm * V.r_pm[r] - (hasL ? mu / sm : 0.0);
 }
 
 __global__ void __launch_bounds__(NT) sigma_vars_kernel(DevModel M, IpmVectors V, double mu, const double* __restrict__ par) {
@@ -306,8 +317,9 @@ __global__ void __launch_bounds__(NT) step_kernel(DevModel M, IpmVectors V, doub
             double jdy = 0.0;
             for (int64_t p = M.J_ptr[r]; p < M.J_ptr[r + 1]; ++p) jdy += V.Jval[p] * V.dy[M.J_idx[p]];
             const double sp = V.sp[r], sm = V.sm[r], wp = V.wp[r], wm = V.wm[r];
-            const double dsp = -V.r_pp[r] - jdy, dsm = -V.r_pm[r] + jdy;
-            const double dwp = -(wp - mu / sp) - wp / sp * dsp, dwm = -(wm - mu / sm) - wm / sm * dsm;
+            const bool hasU = M.cu[r] < INF, hasL = M.cl[r] > -INF;
+            const double dsp = hasU ? -V.r_pp[r] - jdy : 0.0, dsm = hasL ? -V.r_pm[r] + jdy : 0.0;
+            const double dwp = hasU ? -(wp - mu / sp) - wp / sp * dsp : 0.0, dwm = hasL ? -(wm - mu / sm) - wm / sm * dsm : 0.0;
             V.dsp[r] = dsp; V.dsm[r] = dsm; V.dwp[r] = dwp; V.dwm[r] = dwm;
             a.v[0] = fmin(a.v[0], fmin(max_step(sp, dsp, tau), max_step(sm, dsm, tau)));
             a.v[1] = fmin(a.v[1], fmin(max_step(wp, dwp, tau), max_step(wm, dwm, tau)));
@@ -386,7 +398,7 @@ __global__ void __launch_bounds__(NT) add_correction_kernel(DevModel M, IpmVecto
 
 // ------------------------------------------------------------------------------------------------------------
 // Filter line search of ref. [17] (options.globalization): the two measures of a trial point (y + alpha dy, s + alpha ds)
-//   theta = |c - gamma + s+|_1 + |-c - gamma + s-|_1,   phi_mu = f - mu (sum ln s+ + sum ln s- + sum ln(y - lb) + sum ln(ub - y))
+//   theta = |c - cu + s+|_1 + |-c + cl + s-|_1 (row sides with a bound),   phi_mu = f - mu (sum ln s+ + sum ln s- + sum ln(y - lb) + sum ln(ub - y))
 // reduced with the fixed tree; scal[0..4] = theta, sum of logs, f, #arguments <= 0, grad phi_mu^T d (alpha = 0 call only)
 // ------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(NT) trial_point_kernel(DevModel M, IpmVectors V, double alpha) {
@@ -395,6 +407,7 @@ __global__ void __launch_bounds__(NT) trial_point_kernel(DevModel M, IpmVectors 
 }
 
 __global__ void __launch_bounds__(NT) merit_kernel(DevModel M, IpmVectors V, double alpha, double mu, double gamma, int with_grad) {
+    (void)gamma;                                         // part of the row intervals [cl, cu]
     Red<5> a;
 #pragma unroll
     for (int k = 0; k < 5; ++k) a.v[k] = 0.0;
@@ -421,10 +434,12 @@ __global__ void __launch_bounds__(NT) merit_kernel(DevModel M, IpmVectors V, dou
             const int64_t r = idx - M.n;
             const double c = V.ct[r];
             const double sp = step ? V.sp[r] + alpha * V.dsp[r] : V.sp[r], sm = step ? V.sm[r] + alpha * V.dsm[r] : V.sm[r];
-            a.v[0] += fabs(c - gamma + sp) + fabs(-c - gamma + sm);
-            if (sp > 0.0) a.v[1] += log(sp); else a.v[3] += 1.0;
-            if (sm > 0.0) a.v[1] += log(sm); else a.v[3] += 1.0;
-            if (with_grad) a.v[4] -= mu * (V.dsp[r] / V.sp[r] + V.dsm[r] / V.sm[r]);
+            const double cl = M.cl[r], cu = M.cu[r];
+            const bool hasU = cu < INF, hasL = cl > -INF;
+            a.v[0] += (hasU ? fabs(c - cu + sp) : 0.0) + (hasL ? fabs(-c + cl + sm) : 0.0);
+            if (hasU) { if (sp > 0.0) a.v[1] += log(sp); else a.v[3] += 1.0; }
+            if (hasL) { if (sm > 0.0) a.v[1] += log(sm); else a.v[3] += 1.0; }
+            if (with_grad) a.v[4] -= mu * (V.dsp[r] / V.sp[r] + V.dsm[r] / V.sm[r]);   // 0 / 1 for a side without a bound
         }
     }
     const int ops[5] = {2, 2, 2, 2, 2};

@@ -63,10 +63,14 @@ bool build_model_maps(const nmpc_ocp* ocp, ModelMaps& mm, std::string& err) {
         default: err = "unknown model"; return false;
     }
     const int N = D.N, nx = D.nx, nv = D.nv;
-    mm.n = (int64_t)N * nv; mm.m = (int64_t)N * nx;
-    if (mm.n > INT32_MAX / 2) { err = "OCP too large for int32 indices"; return false; }
+    mm.n = (int64_t)N * nv; mm.m_dyn = (int64_t)N * nx;
+    const int64_t n_g = ocp->n_g;
+    if (n_g < 0 || (n_g > 0 && (!ocp->g_rowptr || !ocp->g_colind || !ocp->g_val || !ocp->g_lo || !ocp->g_hi))) { err = "bad general rows"; return false; }
+    mm.m = mm.m_dyn + n_g;
+    if (mm.n > INT32_MAX / 2 || mm.m > INT32_MAX / 2) { err = "OCP too large for int32 indices"; return false; }
     mm.present = true;
-    const int64_t n = mm.n, m = mm.m;
+    const int64_t n = mm.n, m = mm.m, m_dyn = mm.m_dyn;
+    mm.cl.assign(m, 0.0); mm.cu.assign(m, 0.0); mm.g_val.clear();
 
     // ---- J pattern: run the row enumerators on a dummy interior point ----
     std::vector<double> xd(nx, 0.5), ud(std::max(1, D.nu), 0.5);
@@ -79,9 +83,23 @@ bool build_model_maps(const nmpc_ocp* ocp, ModelMaps& mm, std::string& err) {
             model_row(D, c, xd.data(), ud.data(), emit);
             mm.J.ptr[(int64_t)k * nx + c + 1] = (int64_t)mm.J.idx.size();
         }
+    // ---- the general linear rows lo <= G y <= hi below the dynamics rows (include/nmpc.h: nmpc_ocp) ----
+    for (int64_t g = 0; g < n_g; ++g) {
+        const int64_t a = ocp->g_rowptr[g], b = ocp->g_rowptr[g + 1];
+        if (g == 0 && a != 0) { err = "g_rowptr[0] != 0"; return false; }
+        if (b <= a) { err = "empty general row"; return false; }
+        for (int64_t p = a; p < b; ++p) {
+            const int32_t col = ocp->g_colind[p];
+            if (col < 0 || col >= n || (p > a && col <= ocp->g_colind[p - 1])) { err = "general row: column out of range or not increasing"; return false; }
+            mm.J.idx.push_back(col); mm.g_val.push_back(ocp->g_val[p]);
+        }
+        mm.J.ptr[m_dyn + g + 1] = (int64_t)mm.J.idx.size();
+        if (!(ocp->g_lo[g] <= ocp->g_hi[g])) { err = "general row: lo > hi"; return false; }
+        mm.cl[m_dyn + g] = ocp->g_lo[g]; mm.cu[m_dyn + g] = ocp->g_hi[g];
+    }
     const int64_t nnzJ = mm.J.nnz();
     for (int64_t r = 0; r < m; ++r) {
-        if (mm.J.ptr[r + 1] - mm.J.ptr[r] > MAX_JROW + 1) { err = "J row too long"; return false; }
+        if (r < m_dyn && mm.J.ptr[r + 1] - mm.J.ptr[r] > MAX_JROW + 1) { err = "J row too long"; return false; }
         for (int64_t p = mm.J.ptr[r] + 1; p < mm.J.ptr[r + 1]; ++p)
             if (mm.J.idx[p] <= mm.J.idx[p - 1]) { err = "J row not sorted"; return false; }
     }

@@ -25,7 +25,9 @@ struct Csr {                       // generic int pattern, row-major
 struct ModelMaps {                 // patterns + gather maps of a stage-structured model (empty if no model)
     bool present = false;
     ModelDesc desc{};
-    int64_t n = 0, m = 0;
+    int64_t n = 0, m = 0, m_dyn = 0;   // m = m_dyn dynamics rows (N nx) + the general linear rows
+    std::vector<double> g_val;     // values of the general linear rows in J order (J entries from J.ptr[m_dyn] on)
+    std::vector<double> cl, cu;    // m: row intervals without the gamma tube: 0 / 0 for the dynamics rows, g_lo / g_hi
     Csr J;                         // m x n, CSR in emission order (sorted columns)
     Csr W;                         // n x n lower CSR
     Csr K;                         // n x n lower CSR: pattern(J^T J) u pattern(W) u diag

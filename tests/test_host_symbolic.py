@@ -229,7 +229,12 @@ def test_fig1_children_property_golden_through_the_library():
     assert [p + 1 for p in info["etree_parent"]] == parent
 
 
-@pytest.mark.parametrize("name,ov", SMALL)
+# general linear rows below the dynamics rows (include/nmpc.h: nmpc_ocp.n_g; reading G22): hold, move limits, input-sum limit
+WITH_ROWS = [("C0", dict(Nc=25, move_limit=0.3)), ("C1", dict(trays=6, N=8, Nc=5, move_limit=0.2)), ("C2", dict(g=5, N=4, power_limit=1.2, Nc=3)),
+             ("C3", dict(g=6, nseg=2, N=3, power_limit=2.0))]
+
+
+@pytest.mark.parametrize("name,ov", SMALL + WITH_ROWS)
 def test_model_K_pattern_matches_oracle(name, ov):
     cfg = make_config(name, **ov)
     sym = nb.Symbolic(None, nb.make_ocp(cfg), None)
