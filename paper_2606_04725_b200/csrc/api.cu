@@ -122,7 +122,7 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
         h->n_big_fronts++;
         nbp[s] = tile_nbp(W(s)); nbt[s] = nbp[s] + tile_nbu(W(s), R(s));
         tbase[s] = (int32_t)slots;
-        slots += (int64_t)nbp[s] * nbt[s] + 1;
+        slots += (int64_t)nbp[s] * nbt[s] + 1 + nbt[s];          // tile flags, one spare, row-progress words (factor.cu)
         target[s] = nbt[s] * (nbt[s] + 1) / 2;
         bbase[s] = (int32_t)bslots; bslots += nbp[s];
         target_f[s] = nbt[s]; target_b[s] = 1;             // backward: the chain task finishes the supernode
@@ -336,6 +336,7 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
     for (int s = 0; s < ns; ++s) per_epoch = std::max<int64_t>(per_epoch, target[s]);
     const int64_t min_limit = 3 + std::max(0, h->opt.refine_steps);
     h->epoch_limit = (uint32_t)std::max<int64_t>(min_limit, ((int64_t)1 << 31) / per_epoch - 2);
+    h->epoch_limit = std::min<uint32_t>(h->epoch_limit, 1u << 19);   // the row-progress words of the factorization hold (call number << 12) | tiles
     if (h->opt.epoch_limit > 0) h->epoch_limit = std::min<uint32_t>(h->epoch_limit, (uint32_t)std::max<int64_t>(min_limit, h->opt.epoch_limit));   // test hook
     return NMPC_OK;
 }

@@ -55,6 +55,9 @@ __device__ __forceinline__ void st_release(uint32_t* p, uint32_t v) {
 __device__ __forceinline__ void red_release_add(uint32_t* p, uint32_t v) {
     asm volatile("red.relaxed.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
+__device__ __forceinline__ void red_release_max(uint32_t* p, uint32_t v) {
+    asm volatile("red.relaxed.gpu.global.max.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
 #ifdef NMPC_TRACE_BUILD                     // measurement build: timestamps per task + the time thread 0 spends waiting on flags
 __device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
 __shared__ unsigned long long s_wait_ns;
@@ -592,6 +595,9 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
     double* P = D.L + D.panel_ptr[s];
     uint32_t* front_done = F.fac_done;
     uint32_t* tdone = F.tile_done + F.tbase[s];
+    // row progress: the panel tiles of a block row finish in the order of their block columns (each waits for the ones to its
+    // left), so ONE word per block row, (call number << 12) | finished tiles, tells a left-looking product how far it can run
+    uint32_t* rowp = tdone + nbp * nbt + 1;
     const int Kend = (J < nbp) ? j0 : w;
     double* pipe = sm;
     double* Cs = sm + PIPE_DOUBLES;
@@ -672,14 +678,22 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
 #pragma unroll
         for (int b = 0; b < 4; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
     const int nch = (Kend + KC - 1) / KC;
+    int safe = 0;                                        // per warp: block columns [0, safe) of rows I and J are known to be finished
     auto wait_flags = [&](int c) {                       // every warp: the 64-column block that chunk c starts must be finished
         if (c < nch && ((c * KC) & (TILE - 1)) == 0) {
-            if (lane == 0) {
-                const int kb = (c * KC) / TILE;
-                spin_until_ge(tdone + kb * nbt + I, epoch);
-                if (J != I) spin_until_ge(tdone + kb * nbt + J, epoch);
+            const int kb = (c * KC) / TILE;
+            if (kb >= safe) {                            // at the frontier only: one acquire per row says how far both rows are
+                int got = 0;
+                if (lane == 0) {
+                    const uint32_t need = (epoch << 12) | (uint32_t)(kb + 1);
+                    uint32_t vi, vj;
+                    while ((vi = ld_acquire(rowp + I)) < need) __nanosleep(40);
+                    vj = vi;
+                    if (J != I) while ((vj = ld_acquire(rowp + J)) < need) __nanosleep(40);
+                    got = (int)(min(vi, vj) & 4095u);
+                }
+                safe = __shfl_sync(0xffffffffu, got, 0);
             }
-            __syncwarp();
         }
     };
     auto issue = [&](int c) {
@@ -768,7 +782,7 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
             TRACE(3);                                    // every row-solving thread has already stored its finished entries
         }
         __syncthreads();
-        if (tid == 0) { __threadfence(); st_release(tdone + J * nbt + I, epoch); red_release_add(front_done + s, 1u); }
+        if (tid == 0) { __threadfence(); red_release_max(rowp + I, (epoch << 12) | (uint32_t)(J + 1)); st_release(tdone + J * nbt + I, epoch); red_release_add(front_done + s, 1u); }
     } else {
         double* Uo = D.U + D.upd_ptr[s];
         TRACE(3);
