@@ -659,8 +659,13 @@ void nmpc_destroy(nmpc_handle h) {
 
 #ifdef NMPC_TRACE_BUILD
 int64_t nmpc_get_task_trace(nmpc_handle h, int32_t kind, int32_t* tasks_host, uint64_t* stamps_host, int64_t cap) {
-    if (!h || kind < 0 || kind > 1) return -1;
+    if (!h || kind < 0 || kind > 2) return -1;
     DeviceGuard dg(h);
+    if (kind == 2) {                                     // phase cycles of the diagonal-tile POTRFs since the last read (8 words)
+        if (!stamps_host || cap < 8) return 8;
+        if (cudaStreamSynchronize(h->stream) != cudaSuccess || read_potrf_cycles(reinterpret_cast<unsigned long long*>(stamps_host), true) != cudaSuccess) return -1;
+        return 8;
+    }
     const int64_t nt = kind == 0 ? h->F.n_ftasks : h->F.n_stasks;
     const unsigned long long* tr = kind == 0 ? h->F.ftrace : h->F.strace;
     if (!tr) return 0;

@@ -121,6 +121,9 @@ cudaError_t configure_factor_kernels(int max_smem_bytes, bool one_cta_per_sm, in
 void launch_factor(const DevSym& D, const DagPlan& F, const double* Kval, double eta, uint32_t epoch, const uint32_t* epoch_dev,
                    cudaStream_t st);
 void launch_reset_fail(const DevSym& D, cudaStream_t st);                                   // fail_col = INT_MAX
+#ifdef NMPC_TRACE_BUILD
+cudaError_t read_potrf_cycles(unsigned long long* out8, bool reset);   // measurement build: phase cycles of the diagonal-tile POTRFs
+#endif
 // ---- solve.cu ----
 cudaError_t configure_solve_kernels(int max_smem_bytes, int small_max_r, int* ctas_per_sm, size_t* smem_bytes, int* sbuf_doubles);
 // rhs_inout (original ordering, n doubles) is overwritten by K^-1 rhs; x is the handle's permuted work vector.

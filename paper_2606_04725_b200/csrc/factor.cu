@@ -111,65 +111,80 @@ __device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
 // =============================================================================================================
 template <class ColFn>
 __device__ __forceinline__ void factor_diag8(ColFn colp, int j0, int jb, int c0, int aug_col, int32_t* fail_col, double* dinv, double* s_inv) {
-    const int lane = threadIdx.x & 31;
-    double Dg[8][8], inv[8];
-    if (jb == 8) {
-#pragma unroll
-        for (int c = 0; c < 8; ++c) {
-            const double* cp = colp(j0 + c) + j0;
-#pragma unroll
-            for (int i = c; i < 8; ++i) Dg[i][c] = cp[i];
-        }
-    } else {
-#pragma unroll
-        for (int c = 0; c < 8; ++c) {
-            const double* cp = colp(j0 + min(c, jb - 1)) + j0;
-#pragma unroll
-            for (int i = c; i < 8; ++i) { const double v = cp[min(i, jb - 1)]; Dg[i][c] = (i < jb) ? v : (i == c ? 1.0 : 0.0); }   // i < jb implies c < jb
-        }
+    // The 8x8 block is spread over the warp: lane (i << 2) | q holds the entries (i, q) and (i, q + 4).  Under the load of the
+    // neighbouring CTA's DMMA stream every fp64 warp instruction of this serial chain waits ~13 cycles for the pipe (measured:
+    // profiles/r02b_potrf_phases.md), so what counts is their NUMBER: per column the reciprocal square root (all lanes, the same
+    // value), one scaling and two fma, the operands broadcast with shuffles (another pipe) -- 80 instead of the ~170 of a
+    // per-lane copy of the whole block.
+    const int lane = threadIdx.x & 31, i = lane >> 2, q = lane & 3;
+    const unsigned FULLM = 0xffffffffu;
+    double a0, a1;                                       // entries (i, q), (i, q + 4); outside the block / above the diagonal: 0 (diagonal 1)
+    {
+        const int il = min(i, jb - 1);
+        const double v0 = colp(j0 + min(q, jb - 1))[j0 + il], v1 = colp(j0 + min(q + 4, jb - 1))[j0 + il];
+        a0 = (i < jb && q < jb && i >= q) ? v0 : ((i == q && i >= jb) ? 1.0 : 0.0);
+        a1 = (i < jb && q + 4 < jb && i >= q + 4) ? v1 : ((i == q + 4 && i >= jb) ? 1.0 : 0.0);
     }
     int badc = 8;
+    double myinv = 1.0;                                  // lane c keeps 1 / L_cc
 #pragma unroll
     for (int c = 0; c < 8; ++c) {
+        const double src = (c < 4) ? a0 : a1;            // the half that holds column c
+        double d = __shfl_sync(FULLM, src, (c << 2) | (c & 3));
         // the right-hand-side row (device.h: aug_col) is the last pivot of all: taken as 1, never tested
-        const double d = (c0 + j0 + c == aug_col) ? 1.0 : Dg[c][c];
+        if (c0 + j0 + c == aug_col) d = 1.0;
         const bool bad = !(d >= 2.2250738585072014e-308) || isinf(d);          // <= 0, non-finite (or subnormal): reading G11
         if (bad && c < jb && badc == 8) badc = c;
-        const double y = rsqrt_newton(d);                                      // speculative: the test above is off the chain
-        inv[c] = bad ? 1.0 : y;
-        Dg[c][c] = bad ? 1.0 : d * y;
-#pragma unroll
-        for (int i = c + 1; i < 8; ++i) Dg[i][c] *= inv[c];
-#pragma unroll
-        for (int k = c + 1; k < 8; ++k)
-#pragma unroll
-            for (int i = k; i < 8; ++i) Dg[i][k] = fma(-Dg[i][c], Dg[k][c], Dg[i][k]);
+        const double y = bad ? 1.0 : rsqrt_newton(d);
+        myinv = (lane == c) ? y : myinv;
+        // column c: L_cc = d y (1 for a bad pivot), L_ic = a_ic y
+        double col = (c < 4) ? a0 : a1;
+        if (q == (c & 3)) { col = (i == c) ? (bad ? 1.0 : d * y) : col * y; if (c < 4) a0 = col; else a1 = col; }
+        // trailing entries (i, k), k > c:  a_ik -= L_ic L_kc
+        const double src2 = (c < 4) ? a0 : a1;
+        const double lic = __shfl_sync(FULLM, src2, (lane & ~3) | (c & 3));
+        const double lk0 = __shfl_sync(FULLM, src2, (q << 2) | (c & 3));
+        const double lk1 = __shfl_sync(FULLM, src2, ((q + 4) << 2) | (c & 3));
+        if (q > c && i >= q) a0 = fma(-lic, lk0, a0);
+        if (q + 4 > c && i >= q + 4) a1 = fma(-lic, lk1, a1);
     }
     if (badc < 8 && lane == 0) atomicMin(fail_col, c0 + j0 + badc);
-    double mine = inv[0];
-#pragma unroll
-    for (int c = 1; c < 8; ++c) mine = (lane == c) ? inv[c] : mine;
-    if (lane < jb) { dinv[c0 + j0 + lane] = mine; s_inv[lane] = mine; }
-    if (lane == 0) {                                     // one lane stores the factored block (immediate offsets, no branches)
-#pragma unroll
-        for (int c = 0; c < 8; ++c) {
-            double* cp = colp(j0 + min(c, jb - 1)) + j0;
-#pragma unroll
-            for (int i = c; i < 8; ++i)
-                if (i < jb) cp[i] = Dg[i][c];
-        }
+    if (lane < jb) { dinv[c0 + j0 + lane] = myinv; s_inv[lane] = myinv; }
+    if (i < jb) {                                        // every lane stores its own entries of the factored block
+        if (q < jb && i >= q) colp(j0 + q)[j0 + i] = a0;
+        if (q + 4 < jb && i >= q + 4) colp(j0 + q + 4)[j0 + i] = a1;
     }
 }
 
+#ifdef NMPC_TRACE_BUILD
+// measurement build: clock cycles thread 0 spends per phase of the POTRF of diagonal tiles (partial_chol with CW = 4), summed
+// over all such tasks: [0] waiting for the row solve, [1] its tile update, [2] factor_diag8, [3] waiting at the end of the update,
+// [4] sub-steps, [5] whole partial_chol
+__device__ unsigned long long g_potrf_cycles[8];
+#define PCLK(v) const long long v = clock64()
+#define PACC(slot, a, b) do { if (r == w && r <= TILE && tid == 0) atomicAdd(&g_potrf_cycles[slot], (unsigned long long)((b) - (a))); } while (0)
+#else
+#define PCLK(v) do {} while (0)
+#define PACC(slot, a, b) do {} while (0)
+#endif
 struct NoPublish { __device__ __forceinline__ void operator()(int, int) const {} };
 // pub(j0, jb) is called by all threads right after the barrier that ends the row solve of columns [j0, j0 + jb): those columns
 // are final from then on (the diagonal tile of a tiled front streams them to the TRSM tiles of its block column)
-template <class ColFn, class Pub = NoPublish>
+// CW = number of warps that COMPUTE (warp 0 .. CW-1; requires r <= 32 CW: one row-solving thread per row).  The diagonal tile of
+// a tiled front runs with CW = 4: warps 4..7 only publish (store the finished columns, fence, flag); they meet the computing warps
+// at the barrier after each row solve and stay out of the update and of the barrier that ends it, so the ~1 us of the
+// publishing thread's fence overlaps the next update / row solve instead of sitting on the chain of every sub-step.
+template <class ColFn, class Pub = NoPublish, int CW = NT / 32>
 __device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, int aug_col, int32_t* fail_col, double* dinv, Pub pub = Pub()) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gid = lane >> 2, tig = lane & 3;
-    constexpr int NW1 = NT / 32 - 1;                     // warps 1..7 share the tiles warp 0 does not take
+    constexpr int NW1 = CW - 1;                          // warps 1..CW-1 share the tiles warp 0 does not take
+    auto end_of_update = [&]() {
+        if (CW == NT / 32) __syncthreads();
+        else if (warp < CW) asm volatile("bar.sync 2, %0;" ::"n"(CW * 32) : "memory");
+    };
     __shared__ double s_inv[8];
     const int rl = r - 1;
+    PCLK(pc_begin);
     if (warp == 0) factor_diag8(colp, 0, min(8, w), c0, aug_col, fail_col, dinv, s_inv);
     __syncthreads();
     for (int p0 = 0; p0 < w; p0 += 32) {
@@ -177,6 +192,7 @@ __device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, i
         for (int j0 = p0; j0 < p1; j0 += 8) {
             const int jb = min(8, p1 - j0);
             const int t0 = j0 + jb;
+            PCLK(pc0);
             if (tid >= jb && j0 + tid < r) {             // a row below the diagonal block: x = f L_D^-T (right-looking over the 8 columns)
                 const int i = j0 + tid;
                 double x[8], Lk[8][8], inv[8];
@@ -211,6 +227,8 @@ __device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, i
                     if (c < jb) colp(j0 + c)[i] = x[c];
             }
             __syncthreads();
+            PCLK(pc1);
+            PACC(0, pc0, pc1); PACC(4, 0, 1);
             pub(j0, jb);
             const bool has_next = t0 < w;
             if (t0 < p1) {                               // rank-8 update of the panel's remaining columns [t0, p1)
@@ -250,8 +268,11 @@ __device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, i
                 if (warp == 0) {
                     pair(0, ntile);                      // the tile of the next diagonal block, then that block's factorization
                     __syncwarp();
+                    PCLK(pc2);
                     factor_diag8(colp, t0, min(8, p1 - t0), c0, aug_col, fail_col, dinv, s_inv);
-                } else {
+                    PCLK(pc3);
+                    PACC(1, pc1, pc2); PACC(2, pc2, pc3);
+                } else if (warp < CW) {
                     for (int q = warp; q < ntile; q += 2 * NW1) pair(q, q + NW1);
                 }
             } else if (p1 < r) {                         // panel end: rank-(p1-p0) update of the trailing columns [p1, r)
@@ -300,14 +321,22 @@ __device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, i
                 if (warp == 0) {
                     pair(0, ntile);
                     __syncwarp();
+                    PCLK(pc2);
                     if (has_next) factor_diag8(colp, p1, min(8, w - p1), c0, aug_col, fail_col, dinv, s_inv);
-                } else {
+                    PCLK(pc3);
+                    PACC(1, pc1, pc2); PACC(2, pc2, pc3);
+                } else if (warp < CW) {
                     for (int q = warp; q < ntile; q += 2 * NW1) pair(q, q + NW1);
                 }
             }
-            __syncthreads();
+            PCLK(pc4);
+            end_of_update();
+            PCLK(pc5);
+            PACC(3, pc4, pc5);
         }
     }
+    PCLK(pc_end);
+    PACC(5, pc_begin, pc_end);
 }
 
 // X = C L^-T for an ni x nj tile C (column-major, CLD) against the nj x nj lower-triangular Ls (column-major, CLD), in
@@ -606,6 +635,19 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
     //         matrices in fixed child order ----
     for (int idx = tid; idx < CT_DOUBLES; idx += NT) Cs[idx] = 0.0;
     const int ch0 = D.child_ptr[s], ch1 = D.child_ptr[s + 1];
+    // the child tables of the first batch are static data: fetched BEFORE the task waits (three dependent index loads per child)
+    int* ctab = reinterpret_cast<int*>(pipe);                            // [TCH][4]: a0, a1, b0, b1
+    long long* cptr = reinterpret_cast<long long*>(pipe + TCH * 2);      // [TCH][3]: update offset, rel offset, rows of the update matrix
+    auto fetch_tables = [&](int base, int nbat) {
+        if (tid < nbat) {
+            const int c = D.child_idx[base + tid];
+            const int32_t* cb = F.cbnd + F.cb_ptr[c];
+            ctab[4 * tid] = cb[I]; ctab[4 * tid + 1] = cb[I + 1]; ctab[4 * tid + 2] = cb[J]; ctab[4 * tid + 3] = cb[J + 1];
+            const long long rp0 = D.rel_ptr[c];
+            cptr[3 * tid] = D.upd_ptr[c]; cptr[3 * tid + 1] = rp0; cptr[3 * tid + 2] = D.rel_ptr[c + 1] - rp0;
+        }
+    };
+    fetch_tables(ch0, min(TCH, ch1 - ch0));
     if (J == 0) {                                        // tiles with J > 0 inherit this through the flag of tile (I,0)
         for (int ci = ch0 + tid; ci < ch1; ci += NT) { const int c = D.child_idx[ci]; spin_until_ge(front_done + c, epoch * (uint32_t)F.target[c]); }
     } else if (tid == 0) {
@@ -623,20 +665,11 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
     // dependent index loads cost one round trip per batch instead of one per child; a child that meets the tile stages its
     // <= 64 + 64 relative indices in shared memory and its <= 64 x 64 values are then loaded eight per thread in flight.
     {
-        int* ctab = reinterpret_cast<int*>(pipe);                            // [TCH][4]: a0, a1, b0, b1
-        long long* cptr = reinterpret_cast<long long*>(pipe + TCH * 2);      // [TCH][3]: update offset, rel offset, rows of the update matrix
         int* relA = reinterpret_cast<int*>(pipe + TCH * 5);                  // [64] row of the tile, [64] column offset in the tile
         int* relB = relA + TILE;
         for (int base = ch0; base < ch1; base += TCH) {
             const int nbat = min(TCH, ch1 - base);
-            __syncthreads();
-            if (tid < nbat) {
-                const int c = D.child_idx[base + tid];
-                const int32_t* cb = F.cbnd + F.cb_ptr[c];
-                ctab[4 * tid] = cb[I]; ctab[4 * tid + 1] = cb[I + 1]; ctab[4 * tid + 2] = cb[J]; ctab[4 * tid + 3] = cb[J + 1];
-                const long long rp0 = D.rel_ptr[c];
-                cptr[3 * tid] = D.upd_ptr[c]; cptr[3 * tid + 1] = rp0; cptr[3 * tid + 2] = D.rel_ptr[c + 1] - rp0;
-            }
+            if (base > ch0) { __syncthreads(); fetch_tables(base, nbat); }
             __syncthreads();
             for (int k = 0; k < nbat; ++k) {
                 const int a0 = ctab[4 * k], a1 = ctab[4 * k + 1], b0 = ctab[4 * k + 2], b1 = ctab[4 * k + 3];
@@ -756,6 +789,7 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
         if (I == J) {
             // every finished 8-column block of L_JJ is stored and announced at once: the TRSM tiles of this block column
             // run one sub-step behind this POTRF instead of after it (the chain POTRF -> TRSM -> POTRF of the front)
+            auto colf = [Cs](int j) { return Cs + j * CLD; };
             auto pub = [&](int js, int jbs) {
                 if (tid >= NT / 2) {                     // warps 4..7 store, warp 0 goes on with the next diagonal block
                     const int nr = nj - js;
@@ -773,7 +807,7 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
                     if (tid == NT - 1) { __threadfence(); st_release(sub, sbase + (uint32_t)(js >> 3) + 1u); }
                 }
             };
-            partial_chol([Cs](int j) { return Cs + j * CLD; }, nj, nj, c0 + j0, D.aug_col, D.fail_col, D.dinv, pub);
+            partial_chol(colf, nj, nj, c0 + j0, D.aug_col, D.fail_col, D.dinv, pub);
             TRACE(3);
         } else {
             double* Ls = pipe;
@@ -823,6 +857,7 @@ __global__ void __launch_bounds__(NT, 2) factor_dag_kernel(DevSym D, DagPlan F, 
 
 __global__ void reset_fail_kernel(int32_t* fail_col) { *fail_col = INT_MAX; }
 
+
 }  // namespace
 
 cudaError_t configure_factor_kernels(int max_smem_bytes, bool one_cta_per_sm, int* ctas_per_sm, size_t* smem_bytes, int* small_max_r) {
@@ -851,5 +886,12 @@ void launch_factor(const DevSym& D, const DagPlan& F, const double* Kval, double
     if (F.n_ftasks > 0) factor_dag_kernel<<<F.fgrid, NT, F.fsmem, st>>>(D, F, Kval, eta, epoch, epoch_dev);
 }
 void launch_reset_fail(const DevSym& D, cudaStream_t st) { reset_fail_kernel<<<1, 1, 0, st>>>(D.fail_col); }
+#ifdef NMPC_TRACE_BUILD
+cudaError_t read_potrf_cycles(unsigned long long* out8, bool reset) {
+    cudaError_t e = cudaMemcpyFromSymbol(out8, g_potrf_cycles, sizeof(unsigned long long) * 8);
+    if (e == cudaSuccess && reset) { unsigned long long z[8] = {0, 0, 0, 0, 0, 0, 0, 0}; e = cudaMemcpyToSymbol(g_potrf_cycles, z, sizeof(z)); }
+    return e;
+}
+#endif
 
 }  // namespace nmpc

@@ -119,7 +119,9 @@ extern "C" nmpc_status nmpc_tile_gemm_peak(int32_t K, int32_t repeats, double* t
     if (!tflops_out || K < 64 || (K % G_KC) || repeats < 1) return NMPC_E_ARG;
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { cudaGetLastError(); return NMPC_E_CUDA; }
-    const int blocks = sms * 2, ld = blocks * G_TILE;
+    // NMPC_GEMM_CTAS_PER_SM=1: one CTA per SM (how fast a LONE tile product runs while its SM neighbour is in a non-GEMM phase)
+    const char* env = getenv("NMPC_GEMM_CTAS_PER_SM");
+    const int blocks = sms * ((env && env[0] == '1') ? 1 : 2), ld = blocks * G_TILE;
     const size_t smem = (size_t)G_NSTAGE * G_STAGE * sizeof(double) + 34 * 1024;   // + the C tile the factorization keeps beside the ring
     double *P = nullptr, *out = nullptr;
     if (cudaMalloc((void**)&P, sizeof(double) * (size_t)ld * K) != cudaSuccess || cudaMalloc((void**)&out, sizeof(double) * (size_t)blocks * PEAK_NT) != cudaSuccess) {
