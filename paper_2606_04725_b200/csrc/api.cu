@@ -236,46 +236,28 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
     stasks.reserve(2 * sk.size());
     for (const SK& t : sk) stasks.push_back(make_int4(t.type, t.s, t.I, 0));
     const int32_t n_sfwd = (int32_t)stasks.size();
-    // Backward: a supernode can start when its parent is done.  CTAs claim tasks in order and WAIT for the dependencies of
-    // what they claimed, so the order must follow the time at which tasks become runnable, or the CTAs fill up with waiting
-    // tasks while runnable ones queue behind them: supernodes in the order of an estimated start time (parent's end; ~3 us
-    // per block column of a chain, ~15 us for the chunk tasks of a supernode, ~4 us per small supernode: task timelines under
-    // profiles/).  The tasks of a tiled supernode are contiguous: chunk tasks (they depend on the parent only), the chain, then
-    // the helper sums in the order the chain needs them.  The chain waits for helpers that come AFTER it in the list, which is
-    // safe for any grid >= 2: the helpers between the chain and the one it waits for depend only on blocks the chain has
-    // already published, so the other CTAs always get to it.
+    // Backward.  CTAs claim tasks in list order and WAIT for the dependencies of what they claimed, so the list must follow the
+    // time at which tasks become runnable, or the CTAs fill up with waiting tasks while runnable ones queue behind them.  Every
+    // item gets an estimated start time from the dependencies it really has (calibrated on the task timelines under profiles/:
+    // ~6 us per block column of a chain, ~8 us chain prologue, ~12 us for a chunk task, ~4 us per small supernode):
+    //   chunk task (s, J, c): when the latest piece of x its rows touch is published (block k of a tiled ancestor's chain, or
+    //                         a small ancestor as a whole);
+    //   chain of s (+ its helper sums, contiguous, in the order the chain needs them): when its last chunk task is done;
+    //   small supernode: when its parent is done.
+    // Estimates increase strictly along every dependency except chain -> helper, so the sorted list is topological up to that
+    // one: the chain waits for helpers that come AFTER it, which is safe for any grid >= 2 -- the helpers between the chain and the
+    // one it waits for depend only on blocks the chain has already published, so the other CTAs always get to it.
     std::vector<int64_t> pbase(ns, 0);
     int64_t part_doubles = 0;
     std::vector<int32_t> cbase(ns, 0);
     std::vector<int64_t> cdep_ptr(1, 0);
     std::vector<uint32_t> cdep;
     {
-        const double HOP_US = 3.0, UPD_US = 15.0, SMALL_US = 4.0;
-        std::vector<double> ready(ns, 0.0), fin(ns, 0.0);
-        std::vector<int32_t> order(ns);
-        for (int s = ns - 1; s >= 0; --s) {              // parents have larger indices (postorder)
-            const int p = S.sn_parent[s];
-            ready[s] = p < 0 ? 0.0 : fin[p];
-            order[s] = s;
-            if (!cls[s]) { fin[s] = ready[s] + SMALL_US + 0.05 * W(s); continue; }
-            const int nchunk = (nbt[s] - nbp[s] + BWD_CH - 1) / BWD_CH;
-            fin[s] = ready[s] + (nchunk > 0 ? UPD_US : 0.0) + HOP_US * nbp[s] + 5.0;
-        }
-        // equal start estimates (siblings): the one with the longest chain of work below it first
-        std::vector<double> below(ns, 0.0);
-        for (int s = 0; s < ns; ++s) {
-            below[s] += fin[s] - ready[s];
-            const int p = S.sn_parent[s];
-            if (p >= 0) below[p] = std::max(below[p], below[s]);
-        }
-        std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
-            if (ready[a] != ready[b]) return ready[a] < ready[b];
-            return below[a] != below[b] ? below[a] > below[b] : a > b;
-        });
         for (int s = 0; s < ns; ++s) {                   // what every chunk of ancestors' rows has to wait for
             cbase[s] = (int32_t)(cdep_ptr.size() - 1);
             if (!cls[s]) continue;
             const int nchunk = (nbt[s] - nbp[s] + BWD_CH - 1) / BWD_CH;
+            pbase[s] = part_doubles; part_doubles += (int64_t)nchunk * W(s);
             const int32_t* rw = &S.rows[S.rows_ptr[s]];
             for (int c = 0; c < nchunk; ++c) {
                 const int i0 = tile_bound(nbp[s] + c * BWD_CH, W(s), R(s), nbp[s]);
@@ -291,14 +273,45 @@ nmpc_status build_plan(nmpc_handle_s* h, int small_max_r, int ctas_per_sm, size_
                 cdep_ptr.push_back((int64_t)cdep.size());
             }
         }
-        for (int s : order) {
-            if (!cls[s]) { stasks.push_back(make_int4(0, s, 0, 1)); continue; }
+        const double HOP_US = 6.0, PRO_US = 8.0, UPD_US = 12.0, SMALL_US = 4.0;
+        std::vector<double> start(ns, 0.0), fin(ns, 0.0);
+        auto published = [&](int g) {                    // when x at pivot position g is available to other CTAs
+            const int a = S.sn_of_col[g];
+            return cls[a] ? start[a] + PRO_US + HOP_US * (nbp[a] - (g - S.sn_start[a]) / TILE) : fin[a];
+        };
+        struct Item { double key; int32_t kind, s, I; };  // kind 0 small supernode, 1 chain + helpers of s, 2 chunk task
+        std::vector<Item> items;
+        for (int s = ns - 1; s >= 0; --s) {              // parents have larger indices (postorder)
+            const int p = S.sn_parent[s];
+            if (!cls[s]) {
+                start[s] = p < 0 ? 0.0 : fin[p];
+                fin[s] = start[s] + SMALL_US + 0.05 * W(s);
+                items.push_back(Item{start[s], 0, s, 0});
+                continue;
+            }
             const int nchunk = (nbt[s] - nbp[s] + BWD_CH - 1) / BWD_CH;
-            pbase[s] = part_doubles; part_doubles += (int64_t)nchunk * W(s);
-            for (int J = nbp[s] - 1; J >= 0; --J)
-                for (int c = 0; c < nchunk; ++c) stasks.push_back(make_int4(2, s, J | (c << 16), 1));
-            stasks.push_back(make_int4(3, s, 0, 1));
-            for (int J = nbp[s] - 4; J >= 0; --J) stasks.push_back(make_int4(1, s, J, 1));
+            const int32_t* rw = &S.rows[S.rows_ptr[s]];
+            double last = 0.0;
+            for (int c = 0; c < nchunk; ++c) {
+                const int i0 = tile_bound(nbp[s] + c * BWD_CH, W(s), R(s), nbp[s]);
+                const int i1 = tile_bound(std::min(nbt[s], nbp[s] + (c + 1) * BWD_CH), W(s), R(s), nbp[s]);
+                double key = 0.0;
+                for (int i = i0; i < i1; ++i) key = std::max(key, published(rw[i]));
+                last = std::max(last, key);
+                for (int J = nbp[s] - 1; J >= 0; --J) items.push_back(Item{key + 1e-4 * (nbp[s] - 1 - J), 2, s, J | (c << 16)});
+            }
+            start[s] = nchunk > 0 ? last + UPD_US : 0.0;
+            fin[s] = start[s] + PRO_US + HOP_US * nbp[s];
+            items.push_back(Item{start[s], 1, s, 0});
+        }
+        std::stable_sort(items.begin(), items.end(), [](const Item& a, const Item& b) { return a.key < b.key; });
+        for (const Item& it : items) {
+            if (it.kind == 0) stasks.push_back(make_int4(0, it.s, 0, 1));
+            else if (it.kind == 2) stasks.push_back(make_int4(2, it.s, it.I, 1));
+            else {
+                stasks.push_back(make_int4(3, it.s, 0, 1));
+                for (int J = nbp[it.s] - 4; J >= 0; --J) stasks.push_back(make_int4(1, it.s, J, 1));
+            }
         }
     }
 

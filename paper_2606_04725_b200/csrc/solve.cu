@@ -446,34 +446,63 @@ struct BwdTile {
 // chunk task (s, J, c): partial[c][J] = sum over the ancestors' block rows I in chunk c of L(I,J)^T x_I.  It waits for exactly the
 // pieces of x its rows touch (the analysis lists their flags: blocks of the ancestors' chains, small ancestors), so the chunk
 // tasks of a supernode run WHILE the chain of its parent is still going down its blocks
+// Everything that does not depend on x is in flight before the task waits: the row indices of the chunk and the first three
+// tiles (cp.async into a three-slot ring in shared memory).  After the wait the <= 512 values of x are gathered in ONE round trip;
+// the tiles are then consumed from the ring, each freed slot refilled three tiles ahead.
+constexpr int UPD_RING = BWD_CH * TILE, UPD_END = UPD_RING + 3 * TILE * TILE;
 __device__ __forceinline__ void bwd_upd(const DevSym& D, const DagPlan& F, int s, int J, int c, const double* x, uint32_t epoch, double* sm) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const Sn q = sn_of(D, s);
     const int nbp = tile_nbp(q.w), nbt = nbp + tile_nbu(q.w, q.r);
     const int j0 = J * TILE, nj = min(TILE, q.w - j0);
-    const int Ia = nbp + c * BWD_CH, Ib = min(nbt, Ia + BWD_CH);
-    double* xs = sm + OFF_YS;
-    const BwdTile T{q, nbp, j0, nj};
-    double cur[16], nxt[16];
-    T.load(Ia, cur);
+    const int Ia = nbp + c * BWD_CH, nt = min(nbt, Ia + BWD_CH) - Ia;
+    double* xs = sm;                                     // [BWD_CH][64]: x of the chunk's rows, zero padded per tile
+    double* ring = sm + UPD_RING;
+    auto stage = [&](int k) {                            // tile Ia + k: 64 columns x 64 rows from the even row at or before its start
+        if (k < nt) {
+            const int ia = tile_bound(Ia + k, q.w, q.r, nbp) & ~1;
+            double* dst = ring + (k % 3) * TILE * TILE;
+            for (int idx = tid; idx < TILE * TILE / 2; idx += NT) {
+                const int cc = idx >> 5, h = idx & 31;
+                cp_async16(dst + cc * TILE + 2 * h, q.P + ia + 2 * h + (int64_t)(j0 + min(cc, nj - 1)) * q.ld);
+            }
+        }
+        cp_async_commit();                               // one group per call, empty past the chunk: wait_group<2> below counts them
+    };
+    stage(0); stage(1); stage(2);
+    int g[2];
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {                        // slot tid + 256 e = (tile, row)
+        const int slot = tid + NT * e, k = slot >> 6, r = slot & (TILE - 1);
+        g[e] = -1;
+        if (k < nt) {
+            const int i0 = tile_bound(Ia + k, q.w, q.r, nbp), ni = tile_bound(Ia + k + 1, q.w, q.r, nbp) - i0;
+            if (r < ni) g[e] = q.rows[i0 + r];
+        }
+    }
     {
         const int64_t d0 = F.cdep_ptr[F.cbase[s] + c], d1 = F.cdep_ptr[F.cbase[s] + c + 1];
         for (int64_t k = d0 + tid; k < d1; k += NT) spin_until_ge(F.sync + F.cdep[k], epoch);
     }
     __syncthreads();
+#pragma unroll
+    for (int e = 0; e < 2; ++e) xs[tid + NT * e] = g[e] >= 0 ? __ldcg(x + g[e]) : 0.0;
     double acc[8];
 #pragma unroll
     for (int e = 0; e < 8; ++e) acc[e] = 0.0;
-    for (int I = Ia; I < Ib; ++I) {
-        if (I + 1 < Ib) T.load(I + 1, nxt);
-        const int i0 = tile_bound(I, q.w, q.r, nbp), ni = tile_bound(I + 1, q.w, q.r, nbp) - i0;
-        if (tid < TILE) xs[tid] = tid < ni ? __ldcg(x + q.rows[i0 + tid]) : 0.0;
-        __syncthreads();
+    for (int k = 0; k < nt; ++k) {
+        cp_async_wait<2>();                              // tile k has landed (two younger groups may still fly)
+        __syncthreads();                                 // ... for everybody; k = 0: xs is complete
+        const int di = tile_bound(Ia + k, q.w, q.r, nbp) & 1;   // the tile starts one row into its staged copy when its first row is odd
+        const double* tk = ring + (k % 3) * TILE * TILE;
+        const double xa = xs[k * TILE + lane], xb = xs[k * TILE + lane + 32];
 #pragma unroll
-        for (int e = 0; e < 8; ++e) acc[e] = fma(cur[2 * e + 1], xs[lane + 32], fma(cur[2 * e], xs[lane], acc[e]));
-        __syncthreads();
-#pragma unroll
-        for (int e = 0; e < 16; ++e) cur[e] = nxt[e];
+        for (int e = 0; e < 8; ++e) {
+            const double* tc = tk + (warp * 8 + e) * TILE;
+            acc[e] = fma(tc[min(lane + 32 + di, TILE - 1)], xb, fma(tc[lane + di], xa, acc[e]));   // row 63 + di = 64 only meets xb = 0
+        }
+        __syncthreads();                                 // the slot is free
+        stage(k + 3);
     }
     double* out = F.bpart + F.pbase[s] + (int64_t)c * q.w + j0;
 #pragma unroll
@@ -484,6 +513,7 @@ __device__ __forceinline__ void bwd_upd(const DevSym& D, const DagPlan& F, int s
         const int cc = warp * 8 + e;
         if (lane == 0 && cc < nj) out[cc] = v;
     }
+    cp_async_wait<0>();
     __syncthreads();
     if (tid == 0) { __threadfence(); red_release_add(F.blk_u + F.bbase[s] + J, 1u); }
 }
@@ -802,7 +832,7 @@ cudaError_t configure_solve_kernels(int max_smem_bytes, int small_max_r, int* ct
     if (2 * sbuf < TILE * DLD) sbuf = (TILE * DLD + 1) / 2 + 1;      // the staged diagonal tile of the tiled tasks aliases the buffers
     sbuf = (sbuf + 1) & ~1;
     size_t bytes = (size_t)(OFF_BUF + 2 * sbuf + FWD_WORK_DOUBLES) * sizeof(double);
-    bytes = std::max(bytes, (size_t)CH_END * sizeof(double));        // the chain task of the backward solve
+    bytes = std::max(bytes, (size_t)std::max(CH_END, UPD_END) * sizeof(double));   // the chain / chunk tasks of the backward solve
     if (bytes > (size_t)max_smem_bytes) return cudaErrorInvalidValue;
     cudaError_t e = cudaFuncSetAttribute(solve_dag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes - 256);
     if (e != cudaSuccess) return e;
