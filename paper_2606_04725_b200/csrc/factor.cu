@@ -111,11 +111,8 @@ __device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
 // =============================================================================================================
 template <class ColFn>
 __device__ __forceinline__ void factor_diag8(ColFn colp, int j0, int jb, int c0, int aug_col, int32_t* fail_col, double* dinv, double* s_inv) {
-    // The 8x8 block is spread over the warp: lane (i << 2) | q holds the entries (i, q) and (i, q + 4).  Under the load of the
-    // neighbouring CTA's DMMA stream every fp64 warp instruction of this serial chain waits ~13 cycles for the pipe (measured:
-    // profiles/r02b_potrf_phases.md), so what counts is their NUMBER: per column the reciprocal square root (all lanes, the same
-    // value), one scaling and two fma, the operands broadcast with shuffles (another pipe) -- 80 instead of the ~170 of a
-    // per-lane copy of the whole block.
+    // The 8x8 block is spread over the warp: lane (i << 2) | q holds the entries (i, q) and (i, q + 4); operands are broadcast with
+    // shuffles (measurements behind this form: profiles/r02b_potrf_phases.md).
     const int lane = threadIdx.x & 31, i = lane >> 2, q = lane & 3;
     const unsigned FULLM = 0xffffffffu;
     double a0, a1;                                       // entries (i, q), (i, q + 4); outside the block / above the diagonal: 0 (diagonal 1)
@@ -125,8 +122,12 @@ __device__ __forceinline__ void factor_diag8(ColFn colp, int j0, int jb, int c0,
         a0 = (i < jb && q < jb && i >= q) ? v0 : ((i == q && i >= jb) ? 1.0 : 0.0);
         a1 = (i < jb && q + 4 < jb && i >= q + 4) ? v1 : ((i == q + 4 && i >= jb) ? 1.0 : 0.0);
     }
+    // The pivots are a serial chain, and every dependent fp64 operation on it costs ~30 cycles behind the neighbour CTA's DMMA stream.
+    // The elimination is therefore square-root free with the columns left UNSCALED: a_ik -= (a_ic a_kc) (1 / d_c), the products formed
+    // while 1 / d_c (approximation + one cubic step) is on its way, so a pivot costs a shuffle, the reciprocal and one fma on the
+    // chain.  The scaling L_ic = a_ic / sqrt(d_c) happens once at the end, the eight reciprocal square roots side by side in lanes 0..7.
     int badc = 8;
-    double myinv = 1.0;                                  // lane c keeps 1 / L_cc
+    double myd = 1.0;                                    // lane c keeps the pivot d_c (1 for a bad one)
 #pragma unroll
     for (int c = 0; c < 8; ++c) {
         const double src = (c < 4) ? a0 : a1;            // the half that holds column c
@@ -135,19 +136,25 @@ __device__ __forceinline__ void factor_diag8(ColFn colp, int j0, int jb, int c0,
         if (c0 + j0 + c == aug_col) d = 1.0;
         const bool bad = !(d >= 2.2250738585072014e-308) || isinf(d);          // <= 0, non-finite (or subnormal): reading G11
         if (bad && c < jb && badc == 8) badc = c;
-        const double y = bad ? 1.0 : rsqrt_newton(d);
-        myinv = (lane == c) ? y : myinv;
-        // column c: L_cc = d y (1 for a bad pivot), L_ic = a_ic y
-        double col = (c < 4) ? a0 : a1;
-        if (q == (c & 3)) { col = (i == c) ? (bad ? 1.0 : d * y) : col * y; if (c < 4) a0 = col; else a1 = col; }
-        // trailing entries (i, k), k > c:  a_ik -= L_ic L_kc
-        const double src2 = (c < 4) ? a0 : a1;
-        const double lic = __shfl_sync(FULLM, src2, (lane & ~3) | (c & 3));
-        const double lk0 = __shfl_sync(FULLM, src2, (q << 2) | (c & 3));
-        const double lk1 = __shfl_sync(FULLM, src2, ((q + 4) << 2) | (c & 3));
-        if (q > c && i >= q) a0 = fma(-lic, lk0, a0);
-        if (q + 4 > c && i >= q + 4) a1 = fma(-lic, lk1, a1);
+        if (bad || c0 + j0 + c == aug_col) {             // the pivot becomes 1: the column below it stays as it is
+            d = 1.0;
+            if (lane == ((c << 2) | (c & 3))) { if (c < 4) a0 = 1.0; else a1 = 1.0; }
+        }
+        myd = (lane == c) ? d : myd;
+        const double lic = __shfl_sync(FULLM, src, (lane & ~3) | (c & 3));
+        const double lk0 = __shfl_sync(FULLM, src, (q << 2) | (c & 3));
+        const double lk1 = __shfl_sync(FULLM, src, ((q + 4) << 2) | (c & 3));
+        const double p0 = lic * lk0, p1 = lic * lk1;     // before 1 / d is known
+        double rc;
+        asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rc) : "d"(d));
+        const double e = fma(-d, rc, 1.0);
+        rc = fma(rc, fma(e, e, e), rc);                  // one cubic step: rc (1 + e + e^2), error e^3 ~ 2^-66 before rounding
+        if (q > c && i >= q) a0 = fma(-p0, rc, a0);
+        if (q + 4 > c && i >= q + 4) a1 = fma(-p1, rc, a1);
     }
+    const double myinv = rsqrt_newton(myd);              // lanes 0..7: 1 / sqrt(d_lane)
+    a0 *= __shfl_sync(FULLM, myinv, q);                  // L_iq = a_iq / sqrt(d_q); the diagonal: d / sqrt(d)
+    a1 *= __shfl_sync(FULLM, myinv, q + 4);
     if (badc < 8 && lane == 0) atomicMin(fail_col, c0 + j0 + badc);
     if (lane < jb) { dinv[c0 + j0 + lane] = myinv; s_inv[lane] = myinv; }
     if (i < jb) {                                        // every lane stores its own entries of the factored block
