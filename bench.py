@@ -441,26 +441,37 @@ def sigma_sweep(nb, torch, cfg, stream, count=200):
         with torch.cuda.stream(stream):
             x = b.clone()
         h.assemble(Jv, Wv, sx, ss, 0.0, Kv); h.factor(Kv, 0.0, check=False); h.solve(x)
-    times = []
-    for sx, ss, b in draws:
-        with torch.cuda.stream(stream):
-            x = b.clone()
+    times, times2 = [], []
+    with torch.cuda.stream(stream):
+        x = torch.empty(cfg.n, dtype=torch.float64, device=dev)
+    for sx, ss, b in draws:                               # b known before the factorization: Eq. (22) inside it, Eq. (24) after it
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
         h.assemble(Jv, Wv, sx, ss, 0.0, Kv)
-        st, _ = h.factor(Kv, 0.0, check=False)
-        h.solve(x)
+        st, _ = h.factor_rhs(Kv, b, 0.0, check=False)
+        h.solve_fused(x)
         e1.record(stream)
         e1.synchronize()
         fails += int(st != 0)
         times.append(e0.elapsed_time(e1) * 1e3)
+    for sx, ss, b in draws[:40]:                          # the same with nmpc_factor + the two-sided nmpc_solve
+        with torch.cuda.stream(stream):
+            x2 = b.clone()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        h.assemble(Jv, Wv, sx, ss, 0.0, Kv)
+        h.factor(Kv, 0.0, check=False)
+        h.solve(x2)
+        e1.record(stream)
+        e1.synchronize()
+        times2.append(e0.elapsed_time(e1) * 1e3)
     worst = 0.0
     with torch.cuda.stream(stream):                       # backward errors, untimed (measurement arithmetic, not the method's)
         for sx, ss, b in draws:
             h.assemble(Jv, Wv, sx, ss, 0.0, Kv)
-            h.factor(Kv, 0.0, check=False)
-            x = b.clone()
-            h.solve(x)
+            h.factor_rhs(Kv, b, 0.0, check=False)
+            x = torch.empty_like(b)
+            h.solve_fused(x)
             kx = torch.empty_like(x)
             h.kkt_multiply(x, kx)
             absrow = torch.zeros(cfg.n, dtype=torch.float64, device=dev)
@@ -471,9 +482,11 @@ def sigma_sweep(nb, torch, cfg, stream, count=200):
             worst = max(worst, float(err))
     h.close()
     return {"calls": count, "pivot_failures": fails, "us_per_refactor_plus_solve": dist_stats(times),
+            "us_per_refactor_plus_two_sided_solve": dist_stats(times2),
             "worst_solve_backward_error": worst, "bar": 1e-10,
-            "note": "assemble + numeric Cholesky + both solves per call (CUDA events per call), host synchronisation on the pivot "
-                    "flag included; backward error of every draw evaluated after the timed loop"}
+            "note": "assemble + numeric Cholesky with the right-hand-side row (nmpc_factor_rhs) + backward solve (nmpc_solve_fused) per call, "
+                    "CUDA events per call, host synchronisation on the pivot flag included; us_per_refactor_plus_two_sided_solve: the first 40 "
+                    "draws through nmpc_factor + nmpc_solve; backward error of every draw (fused path) evaluated after the timed loop"}
 
 
 def batched_throughput(nb, torch, cfg, B, grid_limit, R):
@@ -695,6 +708,16 @@ def run_own(args):
                             extra[name]["sigma_sweep"]["cpu_baseline"] = oracle_sigma_sweep_sample(c2)
                 except Exception as e:  # noqa: BLE001  (a summary must not take the bench line down)
                     extra[name] = {"error": repr(e)}
+            # the same closed loop with general linear rows below the dynamics rows (control-horizon hold + input
+            # move limits on the distillation column, hold + a one-sided total-input limit on the plate)
+            for name, ov in (("C1", dict(Nc=60, move_limit=0.1)), ("C2", dict(Nc=30, power_limit=1.5))):
+                try:
+                    c2 = make_config(name, **ov)
+                    m2 = measure_workload(nb, torch, c2, stream, min(c2.R, 10), 3, flush_buf, c2.x0, local, sample_clocks=False)
+                    extra[name + "+rows"] = workload_report(m2, hbm_peak)
+                    extra[name + "+rows"]["general_rows"] = dict(count=int(c2.m - c2.m_dyn), **{k: v for k, v in c2.path_rows.items() if v is not None})
+                except Exception as e:  # noqa: BLE001
+                    extra[name + "+rows"] = {"error": repr(e)}
             line["other_workloads"] = extra
     print(json.dumps(line), flush=True)
     if world > 1:

@@ -26,7 +26,8 @@ CASES = [("C0", dict(Nc=25, move_limit=0.3)),
          ("C1", dict(trays=18, N=30, Nc=20, move_limit=0.15)),
          ("C2", dict(g=9, N=7, power_limit=1.0, Nc=5)),
          ("C3", dict(g=8, nseg=2, N=5, power_limit=2.5)),
-         ("C4", dict(trays=40, N=25, Nc=15, move_limit=0.2))]
+         ("C4", dict(trays=40, N=25, Nc=15, move_limit=0.2)),
+         ("C1", dict(Nc=60, move_limit=0.1))]                # BASELINE size (n = 3500), the rows bench.py times as "C1+rows"
 STATE = ("y", "sp", "sm", "wp", "wm", "zL", "zU")
 
 
