@@ -655,6 +655,19 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
         }
     };
     fetch_tables(ch0, min(TCH, ch1 - ch0));
+    // the K entries of the tile depend on nothing the task waits for: their (index, index, value) chain of loads runs before /
+    // during the wait, two entries per thread in registers; they are stored after the barrier that ends the zero fill
+    int64_t kq0 = 0, kq1 = 0;
+    int kdst[2] = {-1, -1};
+    double kval[2] = {0.0, 0.0};
+    if (J < nbp) {
+        kq0 = F.tile_kptr[F.tbase[s] + J * nbt + I]; kq1 = F.tile_kptr[F.tbase[s] + J * nbt + I + 1];
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const int64_t qq = kq0 + tid + NT * e;
+            if (qq < kq1) { kdst[e] = D.kent_dst[qq]; kval[e] = Kval[D.kent_src[qq]]; }
+        }
+    }
     if (J == 0) {                                        // tiles with J > 0 inherit this through the flag of tile (I,0)
         for (int ci = ch0 + tid; ci < ch1; ci += NT) { const int c = D.child_idx[ci]; spin_until_ge(front_done + c, epoch * (uint32_t)F.target[c]); }
     } else if (tid == 0) {
@@ -662,8 +675,10 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
     }
     __syncthreads();
     if (J < nbp) {
-        const int64_t q0 = F.tile_kptr[F.tbase[s] + J * nbt + I], q1 = F.tile_kptr[F.tbase[s] + J * nbt + I + 1];
-        for (int64_t q = q0 + tid; q < q1; q += NT) Cs[D.kent_dst[q]] = Kval[D.kent_src[q]];
+#pragma unroll
+        for (int e = 0; e < 2; ++e)
+            if (kdst[e] >= 0) Cs[kdst[e]] = kval[e];
+        for (int64_t qq = kq0 + 2 * NT + tid; qq < kq1; qq += NT) Cs[D.kent_dst[qq]] = Kval[D.kent_src[qq]];
         __syncthreads();
         if (I == J && eta != 0.0) for (int nn = tid; nn < nj; nn += NT) Cs[nn * CLD + nn] += eta;
     }
