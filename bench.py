@@ -522,6 +522,36 @@ def batched_throughput(nb, torch, cfg, B, grid_limit, R):
             "timing": "host wall clock around nmpc_ipm_solve_batch with the device idle on both sides; one host thread per instance"}
 
 
+def hykkt_leg(nb, torch, cfg, stream, R):
+    """the HyKKT variant (nmpc_hykkt_solve) on the same closed loop: cold solve + R warm re-solves, CUDA
+    events around each call; per IPM iteration one factorization of K_g and 2 + #CG two-sided triangular solves."""
+    dev = torch.device("cuda", torch.cuda.current_device())
+    td = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64).to(dev)   # noqa: E731
+    h = nb.Handle(None, nb.make_ocp(cfg), nb.default_options(), stream=stream.cuda_stream)
+    y = torch.zeros(cfg.n, dtype=torch.float64, device=dev)
+    x0 = np.array(cfg.x0, dtype=np.float64)
+    lo, hi = float(cfg.x0_clip[0]), float(cfg.x0_clip[1])
+    ms, iters, cg, bad = 0.0, 0, 0, 0
+    for j in range(R + 1):
+        with torch.cuda.stream(stream):
+            h.update_params(td(x0), td(cfg.ref_for_solve(j)))
+        stream.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        r = h.hykkt_solve(int(j > 0), y, trace_cap=256, check=False)
+        e1.record(stream)
+        e1.synchronize()
+        bad += int(r["status"] != 0)
+        if j > 0:
+            ms += e0.elapsed_time(e1); iters += r["iters"]; cg += int(sum(t["backtracks"] for t in r["trace"]))
+        x0 = np.clip(y[: cfg.nx].cpu().numpy() + cfg.noise_for_solve(j), lo, hi)
+    h.close()
+    return {"warm_resolves": R, "ipm_iters": iters, "cg_iterations": cg, "not_converged": bad,
+            "us_per_ipm_iter": ms * 1e3 / max(1, iters), "ms_per_resolve": ms / max(1, R),
+            "note": "nmpc_hykkt_solve: K_g = W + Sigma_x + gamma_h J^T J factored once per IPM iteration, CG on the Schur complement "
+                    "with one two-sided triangular solve per CG iteration; host-synchronous CG scalars"}
+
+
 def measure_workload(nb, torch, cfg, stream, K, W, flush_buf, x0_first, gpu_index, sample_clocks=True):
     """Everything bench.py reports about one configuration: analysis (a0), the device-resident closed loop with L2 flush
     and clock record, the HOST-buffer (e2e) loop on the recorded x0 sequence, and the phase split."""
@@ -702,6 +732,8 @@ def run_own(args):
                         extra[name]["cpu_baseline"] = oracle_sample(name)
                     if name in ("C0", "C1"):            # latency-bound single instances: what concurrent instances make of the GPU
                         extra[name]["batched"] = batched_throughput(nb, torch, c2, 16, 18 if name == "C1" else 9, 10)
+                    if name in ("C1", "C2"):            # the HyKKT variant on the same closed loop
+                        extra[name]["hykkt"] = hykkt_leg(nb, torch, c2, stream, 5)
                     if name == "C4":
                         extra[name]["sigma_sweep"] = sigma_sweep(nb, torch, c2, stream)
                         if not args.no_cpu:
