@@ -616,16 +616,20 @@ __device__ __forceinline__ void small_front_task(const DevSym& D, const DagPlan&
 }
 
 // =============================================================================================================
-// task type 1: tile (I,J) of a tiled front, left-looking
+// tiles of a tiled front (left-looking): tile_build (assembly + product), then tile_task / pair_task
 // =============================================================================================================
-__device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int s, int I, int J, const double* __restrict__ Kval,
-                                          double eta, uint32_t epoch, double* sm, unsigned long long* tr) {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = NT / 32;
+// Tile (I,J) of a tiled front up to the point where only its own column block is missing: Cs <- assembled tile (K entries, eta,
+// children's update matrices) - sum_{k < Kend} X(I,k) X(J,k)^T.  NST = stages of the operand ring in `pipe` (4 for a tile task,
+// 2 for the pair task that keeps two C tiles in shared memory).
+template <int NST>
+__device__ __forceinline__ void tile_build(const DevSym& D, const DagPlan& F, int s, int I, int J, int Kend, const double* __restrict__ Kval,
+                                           double eta, uint32_t epoch, double* pipe, double* Cs, unsigned long long* tr) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int gid = lane >> 2, tig = lane & 3, wm = warp >> 1, wn = warp & 1;
     const int c0 = D.sn_start[s], w = D.sn_start[s + 1] - c0;
-    const int r = (int)(D.rows_ptr[s + 1] - D.rows_ptr[s]), ld = ld_even(r), m = r - w;
+    const int r = (int)(D.rows_ptr[s + 1] - D.rows_ptr[s]), ld = ld_even(r);
     const int nbp = tile_nbp(w), nbt = nbp + tile_nbu(w, r);
-    const int i0 = tile_bound(I, w, r, nbp), i1 = tile_bound(I + 1, w, r, nbp), ni = i1 - i0;
+    const int i0 = tile_bound(I, w, r, nbp);
     const int j0 = tile_bound(J, w, r, nbp), j1 = tile_bound(J + 1, w, r, nbp), nj = j1 - j0;
     const int ia = i0 & ~1, ja = j0 & ~1, di = i0 - ia, dj = j0 - ja;
     double* P = D.L + D.panel_ptr[s];
@@ -634,9 +638,7 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
     // row progress: the panel tiles of a block row finish in the order of their block columns (each waits for the ones to its
     // left), so ONE word per block row, (call number << 12) | finished tiles, tells a left-looking product how far it can run
     uint32_t* rowp = tdone + nbp * nbt + 1;
-    const int Kend = (J < nbp) ? j0 : w;
-    double* pipe = sm;
-    double* Cs = sm + PIPE_DOUBLES;
+    (void)c0;
 
     // ---- 1. assemble the tile first (independent of the tiles to the left): zero, K entries, eta, children's update
     //         matrices in fixed child order ----
@@ -754,7 +756,7 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
     auto issue = [&](int c) {
         if (c < nch) {
             const int kc = c * KC;
-            double* st = pipe + (c % NSTAGE) * STAGE_DOUBLES;
+            double* st = pipe + (c % NST) * STAGE_DOUBLES;
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 const int p = tid + NT * q;
@@ -769,14 +771,14 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
     };
     // chunk c is multiplied BEFORE the warps wait for the flags of chunk c+3 (and request it): when a flag is late, the chunks
     // already in shared memory are finished first and the newly released columns only add their own latency
-    wait_flags(0); issue(0);
-    wait_flags(1); issue(1);
-    wait_flags(2); issue(2);
+#pragma unroll
+    for (int c = 0; c < NST - 1; ++c) { wait_flags(c); issue(c); }
     for (int c = 0; c < nch; ++c) {
-        cp_async_wait<2>();
+        cp_async_wait<NST - 2>();
         __syncthreads();
-        const double* As = pipe + (c % NSTAGE) * STAGE_DOUBLES + wm * 16 + gid + di;
-        const double* Bs = pipe + (c % NSTAGE) * STAGE_DOUBLES + KC * ALD + wn * 32 + gid + dj;
+        if (NST == 2) { wait_flags(c + 1); issue(c + 1); }   // two stages: the other one is free since this barrier
+        const double* As = pipe + (c % NST) * STAGE_DOUBLES + wm * 16 + gid + di;
+        const double* Bs = pipe + (c % NST) * STAGE_DOUBLES + KC * ALD + wn * 32 + gid + dj;
 #pragma unroll
         for (int ks = 0; ks < KC; ks += 4) {
             double a[2], b[4];
@@ -789,8 +791,7 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
 #pragma unroll
                 for (int nt = 0; nt < 4; ++nt) dmma(acc[mt][nt], a[mt], b[nt]);
         }
-        wait_flags(c + 3);                               // stage (c+3) % 4 held chunk c-1: free since this iteration's barrier
-        issue(c + 3);
+        if (NST > 2) { wait_flags(c + NST - 1); issue(c + NST - 1); }   // that stage held chunk c-1: free since this iteration's barrier
     }
     cp_async_wait<0>();
     TRACE(2);
@@ -803,6 +804,27 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
 #pragma unroll
             for (int e = 0; e < 2; ++e) Cs[(wn * 32 + nt * 8 + 2 * tig + e) * CLD + wm * 16 + mt * 8 + gid] -= acc[mt][nt][e];
     __syncthreads();
+
+}
+
+// =============================================================================================================
+// task type 1: tile (I,J) of a tiled front, left-looking
+// =============================================================================================================
+__device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int s, int I, int J, const double* __restrict__ Kval,
+                                          double eta, uint32_t epoch, double* sm, unsigned long long* tr) {
+    const int tid = threadIdx.x;
+    const int c0 = D.sn_start[s], w = D.sn_start[s + 1] - c0;
+    const int r = (int)(D.rows_ptr[s + 1] - D.rows_ptr[s]), ld = ld_even(r), m = r - w;
+    const int nbp = tile_nbp(w), nbt = nbp + tile_nbu(w, r);
+    const int i0 = tile_bound(I, w, r, nbp), i1 = tile_bound(I + 1, w, r, nbp), ni = i1 - i0;
+    const int j0 = tile_bound(J, w, r, nbp), j1 = tile_bound(J + 1, w, r, nbp), nj = j1 - j0;
+    double* P = D.L + D.panel_ptr[s];
+    uint32_t* front_done = F.fac_done;
+    uint32_t* tdone = F.tile_done + F.tbase[s];
+    uint32_t* rowp = tdone + nbp * nbt + 1;
+    double* pipe = sm;
+    double* Cs = sm + PIPE_DOUBLES;
+    tile_build<NSTAGE>(D, F, s, I, J, (J < nbp) ? j0 : w, Kval, eta, epoch, pipe, Cs, tr);
 
     // ---- 3. finish: POTRF / TRSM for panel tiles, then store (each tile is written once) ----
     if (J < nbp) {
