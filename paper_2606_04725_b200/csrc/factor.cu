@@ -365,9 +365,16 @@ __device__ __forceinline__ void trsm_tile(double* Cs, double* Ls, double* rinv, 
     __syncthreads();
     const bool all = s_all != 0;
     if (all) {
-        for (int idx = tid; idx < nj * nj; idx += NT) {
-            const int cc = idx / nj, ii = idx - cc * nj;
-            if (ii >= cc) Ls[cc * CLD + ii] = __ldcg(Lg + ii + (int64_t)cc * ldg);
+        {
+            const int ii = tid & (TILE - 1);
+            if (ii < nj)
+                for (int cc0 = tid >> 6; cc0 <= ii; cc0 += 8 * (NT / TILE)) {   // eight loads in flight
+                    double v[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) { const int cc = cc0 + e * (NT / TILE); v[e] = cc <= ii ? __ldcg(Lg + ii + (int64_t)cc * ldg) : 0.0; }
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) { const int cc = cc0 + e * (NT / TILE); if (cc <= ii) Ls[cc * CLD + ii] = v[e]; }
+                }
         }
         if (tid < nj) rinv[tid] = __ldcg(dinv_g + tid);
         __syncthreads();
@@ -380,10 +387,8 @@ __device__ __forceinline__ void trsm_tile(double* Cs, double* Ls, double* rinv, 
                 if (lane == 0) spin_until_ge(sub, sbase + (uint32_t)(j0 >> 3) + 1u);
                 __syncwarp();
                 const int nr = nj - j0;
-                for (int idx = tid; idx < jb * nr; idx += NT) {
-                    const int cc = idx / nr, ii = idx - cc * nr;
-                    Ls[(j0 + cc) * CLD + j0 + ii] = __ldcg(Lg + (j0 + ii) + (int64_t)(j0 + cc) * ldg);
-                }
+                if (warp < jb)                           // one warp per column of the block
+                    for (int ii = lane; ii < nr; ii += 32) Ls[(j0 + warp) * CLD + j0 + ii] = __ldcg(Lg + (j0 + ii) + (int64_t)(j0 + warp) * ldg);
                 if (tid < jb) rinv[j0 + tid] = __ldcg(dinv_g + j0 + tid);
                 __syncthreads();
             }
@@ -706,17 +711,20 @@ __device__ __forceinline__ void tile_build(const DevSym& D, const DagPlan& F, in
                 if (tid < na) relA[tid] = rel[a0 + tid] - i0;
                 else if (tid >= NT / 2 && tid - NT / 2 < nb) relB[tid - NT / 2] = (rel[b0 + tid - NT / 2] - j0) * CLD;
                 __syncthreads();
-                const int tot = na * nb;
+                // flat index f = bb * na + aa over the na x nb block, NT apart per step: (aa, bb) advance by the CTA-uniform
+                // (NT % na, NT / na) with one carry -- one division per thread and child instead of one per entry
+                const int tot = na * nb, qa = NT / na, ra = NT - qa * na;
+                int bb = tid / na, aa = tid - bb * na;
                 for (int f0 = tid; f0 < tot; f0 += 8 * NT) {
                     double v[8];
                     int dst[8];
 #pragma unroll
                     for (int e = 0; e < 8; ++e) {
-                        const int f = f0 + e * NT;
-                        const int bb = f / na, aa = f - bb * na;
-                        const bool on = f < tot && a0 + aa >= b0 + bb;       // the child's update matrix is stored as a lower triangle
+                        const bool on = bb < nb && a0 + aa >= b0 + bb;       // the child's update matrix is stored as a lower triangle
                         v[e] = on ? __ldcg(Uc + (a0 + aa) + (long long)(b0 + bb) * mc) : 0.0;
-                        dst[e] = on ? relB[bb] + relA[aa] : -1;
+                        dst[e] = on ? relB[on ? bb : 0] + relA[aa] : -1;
+                        aa += ra; bb += qa;
+                        if (aa >= na) { aa -= na; ++bb; }
                     }
 #pragma unroll
                     for (int e = 0; e < 8; ++e)
@@ -837,8 +845,8 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
             auto pub = [&](int js, int jbs) {
                 if (tid >= NT / 2) {                     // warps 4..7 store, warp 0 goes on with the next diagonal block
                     const int nr = nj - js;
-                    for (int idx = tid - NT / 2; idx < jbs * nr; idx += NT / 2) {
-                        const int cc = idx / nr, ii = idx - cc * nr;
+                    const int cc = (tid - NT / 2) >> 4;  // 16 threads per column of the block
+                    for (int ii = (tid & 15); ii < nr && cc < jbs; ii += 16) {
                         if (ii >= cc) {
                             const double v = Cs[(js + cc) * CLD + js + ii];
                             P[(j0 + js + ii) + (int64_t)(j0 + js + cc) * ld] = v;
@@ -864,9 +872,11 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
     } else {
         double* Uo = D.U + D.upd_ptr[s];
         TRACE(3);
-        for (int idx = tid; idx < ni * nj; idx += NT) {
-            const int mm = idx % ni, nn = idx / ni;
-            if (I != J || mm >= nn) Uo[(i0 + mm - w) + (int64_t)(j0 + nn - w) * m] = Cs[nn * CLD + mm];
+        {
+            const int mm = tid & (TILE - 1);
+            if (mm < ni)
+                for (int nn = tid >> 6; nn < nj; nn += NT / TILE)
+                    if (I != J || mm >= nn) Uo[(i0 + mm - w) + (int64_t)(j0 + nn - w) * m] = Cs[nn * CLD + mm];
         }
         __syncthreads();
         if (tid == 0) { __threadfence(); red_release_add(front_done + s, 1u); }
