@@ -17,6 +17,7 @@
 // In-order claiming of a topological order cannot deadlock: the lowest-numbered unfinished task depends only on finished ones.
 // fp64 throughout, no floating-point atomics, fixed summation order -> bitwise reproducible.
 #include <climits>
+#include <type_traits>
 
 #include "device.h"
 
@@ -243,15 +244,17 @@ __device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, i
                 const double* ck0 = colp(j0 + (k0 ? tig : 0));
                 const double* ck1 = colp(j0 + (k1 ? tig + 4 : 0));
                 const int TU = (r - t0 + 7) >> 3, TV = (p1 - t0 + 7) >> 3, ntile = TU * TV;
-                auto pair = [&](int qa, int qb) {
+                const float rTU = 1.0f / (float)TU;       // V = q / TU as (q + 0.5) * (1 / TU): exact for q < 2^12, three instructions
+                auto pair = [&](int qa, int qb, auto cnt) {
+                    constexpr int NE = decltype(cnt)::value;      // 2: two tiles in flight; 1: warp 0, whose one tile is on the chain
                     double acc[2][2], cold[2][2];
                     double* pc[2][2];
                     bool ok[2][2];
 #pragma unroll
-                    for (int e = 0; e < 2; ++e) {
+                    for (int e = 0; e < NE; ++e) {
                         const int qq = e ? qb : qa;
                         const int q = min(qq, ntile - 1);
-                        const int V = q / TU, U = q - V * TU;
+                        const int V = (int)(((float)q + 0.5f) * rTU), U = q - V * TU;
                         const int u = t0 + 8 * U + gid, vb = t0 + 8 * V + gid, vc = t0 + 8 * V + 2 * tig;
                         const bool live = qq < ntile && U >= V;
                         const int ucl = min(u, rl), vbl = min(vb, rl);
@@ -267,20 +270,20 @@ __device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, i
                         dmma(acc[e], (live && k1) ? a1 : 0.0, k1 ? b1 : 0.0);
                     }
 #pragma unroll
-                    for (int e = 0; e < 2; ++e) {
+                    for (int e = 0; e < NE; ++e) {
                         if (ok[e][0]) *pc[e][0] = cold[e][0] - acc[e][0];
                         if (ok[e][1]) *pc[e][1] = cold[e][1] - acc[e][1];
                     }
                 };
                 if (warp == 0) {
-                    pair(0, ntile);                      // the tile of the next diagonal block, then that block's factorization
+                    pair(0, ntile, std::integral_constant<int, 1>());   // the tile of the next diagonal block, then that block's factorization
                     __syncwarp();
                     PCLK(pc2);
                     factor_diag8(colp, t0, min(8, p1 - t0), c0, aug_col, fail_col, dinv, s_inv);
                     PCLK(pc3);
                     PACC(1, pc1, pc2); PACC(2, pc2, pc3);
                 } else if (warp < CW) {
-                    for (int q = warp; q < ntile; q += 2 * NW1) pair(q, q + NW1);
+                    for (int q = warp; q < ntile; q += 2 * NW1) pair(q, q + NW1, std::integral_constant<int, 2>());
                 }
             } else if (p1 < r) {                         // panel end: rank-(p1-p0) update of the trailing columns [p1, r)
                 const double* ck[8];
@@ -288,13 +291,14 @@ __device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, i
 #pragma unroll
                 for (int s8 = 0; s8 < 8; ++s8) { const int kc = p0 + 4 * s8 + tig; kv[s8] = kc < p1; ck[s8] = colp(kv[s8] ? kc : p0); }
                 const int T = (r - p1 + 7) >> 3, ntile = (T * (T + 1)) >> 1;
-                auto pair = [&](int qa, int qb) {
+                auto pair = [&](int qa, int qb, auto cnt) {
+                    constexpr int NE = decltype(cnt)::value;
                     double acc[2][2], cold[2][2];
                     double* pc[2][2];
                     bool ok[2][2];
                     int ucl[2], vbl[2];
 #pragma unroll
-                    for (int e = 0; e < 2; ++e) {
+                    for (int e = 0; e < NE; ++e) {
                         const int qq = e ? qb : qa;
                         const int q = min(qq, ntile - 1);
                         int U = (int)((sqrtf(8.0f * (float)q + 1.0f) - 1.0f) * 0.5f);
@@ -315,25 +319,25 @@ __device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, i
                     for (int s8 = 0; s8 < 8; ++s8) {
                         double a[2], b[2];
 #pragma unroll
-                        for (int e = 0; e < 2; ++e) { a[e] = ck[s8][ucl[e]]; b[e] = ck[s8][vbl[e]]; }
+                        for (int e = 0; e < NE; ++e) { a[e] = ck[s8][ucl[e]]; b[e] = ck[s8][vbl[e]]; }
 #pragma unroll
-                        for (int e = 0; e < 2; ++e) dmma(acc[e], kv[s8] ? a[e] : 0.0, kv[s8] ? b[e] : 0.0);
+                        for (int e = 0; e < NE; ++e) dmma(acc[e], kv[s8] ? a[e] : 0.0, kv[s8] ? b[e] : 0.0);
                     }
 #pragma unroll
-                    for (int e = 0; e < 2; ++e) {
+                    for (int e = 0; e < NE; ++e) {
                         if (ok[e][0]) *pc[e][0] = cold[e][0] - acc[e][0];
                         if (ok[e][1]) *pc[e][1] = cold[e][1] - acc[e][1];
                     }
                 };
                 if (warp == 0) {
-                    pair(0, ntile);
+                    pair(0, ntile, std::integral_constant<int, 1>());
                     __syncwarp();
                     PCLK(pc2);
                     if (has_next) factor_diag8(colp, p1, min(8, w - p1), c0, aug_col, fail_col, dinv, s_inv);
                     PCLK(pc3);
                     PACC(1, pc1, pc2); PACC(2, pc2, pc3);
                 } else if (warp < CW) {
-                    for (int q = warp; q < ntile; q += 2 * NW1) pair(q, q + NW1);
+                    for (int q = warp; q < ntile; q += 2 * NW1) pair(q, q + NW1, std::integral_constant<int, 2>());
                 }
             }
             PCLK(pc4);
@@ -358,6 +362,7 @@ __device__ __forceinline__ void trsm_tile(double* Cs, double* Ls, double* rinv, 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gid = lane >> 2, tig = lane & 3;
     constexpr int NW = NT / 32;
     const int TU = (ni + 7) >> 3;
+    const float rTU = 1.0f / (float)TU;                  // q / TU as (q + 0.5) * (1 / TU): exact for q < 2^12
     // a tile that is not right behind its POTRF finds L_JJ complete: one fetch of the whole triangle instead of one round trip
     // to L2 per sub-step
     __shared__ int s_all;
@@ -419,7 +424,7 @@ __device__ __forceinline__ void trsm_tile(double* Cs, double* Ls, double* rinv, 
                 const int kc0 = j0 + (k0 ? tig : 0), kc1 = j0 + (k1 ? tig + 4 : 0);
                 const int TV = (p1 - t0 + 7) >> 3;
                 for (int q = warp; q < TU * TV; q += NW) {
-                    const int U = q % TU, V = q / TU;
+                    const int V = (int)(((float)q + 0.5f) * rTU), U = q - V * TU;
                     const int u = 8 * U + gid, v0 = t0 + 8 * V + 2 * tig, vb = min(t0 + 8 * V + gid, TILE - 1);
                     const double a0 = Cs[kc0 * CLD + u], a1 = Cs[kc1 * CLD + u];
                     const double b0 = Ls[kc0 * CLD + vb], b1 = Ls[kc1 * CLD + vb];
@@ -438,7 +443,7 @@ __device__ __forceinline__ void trsm_tile(double* Cs, double* Ls, double* rinv, 
         if (p1 < nj) {
             const int TV = (nj - p1 + 7) >> 3;
             for (int q = warp; q < TU * TV; q += NW) {
-                const int U = q % TU, V = q / TU;
+                const int V = (int)(((float)q + 0.5f) * rTU), U = q - V * TU;
                 const int u = 8 * U + gid, v0 = p1 + 8 * V + 2 * tig, vb = min(p1 + 8 * V + gid, TILE - 1);
                 const bool ok0 = v0 < nj, ok1 = v0 + 1 < nj;
                 double* pc = Cs + min(v0, TILE - 2) * CLD + u;
