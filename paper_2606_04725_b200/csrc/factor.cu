@@ -175,6 +175,8 @@ __device__ unsigned long long g_potrf_cycles[8];
 #define PCLK(v) do {} while (0)
 #define PACC(slot, a, b) do {} while (0)
 #endif
+__shared__ double s_inv8[8];                            // reciprocal pivots of the current 8 x 8 diagonal block (partial_chol)
+__shared__ int s_all;                                   // trsm_tile: L_JJ was complete when the task looked
 struct NoPublish { __device__ __forceinline__ void operator()(int, int) const {} };
 // pub(j0, jb) is called by all threads right after the barrier that ends the row solve of columns [j0, j0 + jb): those columns
 // are final from then on (the diagonal tile of a tiled front streams them to the TRSM tiles of its block column)
@@ -182,15 +184,18 @@ struct NoPublish { __device__ __forceinline__ void operator()(int, int) const {}
 // a tiled front runs with CW = 4: warps 4..7 only publish (store the finished columns, fence, flag); they meet the computing warps
 // at the barrier after each row solve and stay out of the update and of the barrier that ends it, so the ~1 us of the
 // publishing thread's fence overlaps the next update / row solve instead of sitting on the chain of every sub-step.
-template <class ColFn, class Pub = NoPublish, int CW = NT / 32>
-__device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, int aug_col, int32_t* fail_col, double* dinv, Pub pub = Pub()) {
+// RW > 0: r = w = RW at compile time (the full 64 x 64 diagonal tile of a tiled front: every clamp, mask and ragged-edge test of
+// the general code folds away on the chain of the front).
+template <class ColFn, class Pub = NoPublish, int CW = NT / 32, int RW = 0>
+__device__ __forceinline__ void partial_chol(ColFn colp, int r_in, int w_in, int c0, int aug_col, int32_t* fail_col, double* dinv, Pub pub = Pub()) {
+    const int r = RW ? RW : r_in, w = RW ? RW : w_in;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gid = lane >> 2, tig = lane & 3;
     constexpr int NW1 = CW - 1;                          // warps 1..CW-1 share the tiles warp 0 does not take
     auto end_of_update = [&]() {
         if (CW == NT / 32) __syncthreads();
         else if (warp < CW) asm volatile("bar.sync 2, %0;" ::"n"(CW * 32) : "memory");
     };
-    __shared__ double s_inv[8];
+    double* const s_inv = s_inv8;
     const int rl = r - 1;
     PCLK(pc_begin);
     if (warp == 0) factor_diag8(colp, 0, min(8, w), c0, aug_col, fail_col, dinv, s_inv);
@@ -357,15 +362,16 @@ __device__ __forceinline__ void partial_chol(ColFn colp, int r, int w, int c0, i
 // this call's first block): block k is fetched from the panel in global memory (Lg, leading dimension ldg) right before
 // sub-step k needs it, so the TRSM runs one sub-step behind the POTRF instead of after it.  Xg: the tile of the panel that
 // receives X (same leading dimension ldg); finished entries are stored by the thread that solved them.
-__device__ __forceinline__ void trsm_tile(double* Cs, double* Ls, double* rinv, int ni, int nj, const uint32_t* sub, uint32_t sbase,
+template <bool FULL>                                    // FULL: ni = nj = TILE at compile time (no ragged-edge masks)
+__device__ __forceinline__ void trsm_tile(double* Cs, double* Ls, double* rinv, int ni_in, int nj_in, const uint32_t* sub, uint32_t sbase,
                                           const double* __restrict__ Lg, int ldg, const double* __restrict__ dinv_g, double* __restrict__ Xg) {
+    const int ni = FULL ? TILE : ni_in, nj = FULL ? TILE : nj_in;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gid = lane >> 2, tig = lane & 3;
     constexpr int NW = NT / 32;
     const int TU = (ni + 7) >> 3;
     const float rTU = 1.0f / (float)TU;                  // q / TU as (q + 0.5) * (1 / TU): exact for q < 2^12
     // a tile that is not right behind its POTRF finds L_JJ complete: one fetch of the whole triangle instead of one round trip
     // to L2 per sub-step
-    __shared__ int s_all;
     if (tid == 0) s_all = ld_acquire(sub) >= sbase + (uint32_t)((nj + 7) >> 3);
     __syncthreads();
     const bool all = s_all != 0;
@@ -864,12 +870,14 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
                     if (tid == NT - 1) { __threadfence(); st_release(sub, sbase + (uint32_t)(js >> 3) + 1u); }
                 }
             };
-            partial_chol(colf, nj, nj, c0 + j0, D.aug_col, D.fail_col, D.dinv, pub);
+            if (nj == TILE) partial_chol<decltype(colf), decltype(pub), NT / 32, TILE>(colf, nj, nj, c0 + j0, D.aug_col, D.fail_col, D.dinv, pub);
+            else partial_chol(colf, nj, nj, c0 + j0, D.aug_col, D.fail_col, D.dinv, pub);
             TRACE(3);
         } else {
             double* Ls = pipe;
             double* rinv = pipe + CT_DOUBLES;
-            trsm_tile(Cs, Ls, rinv, ni, nj, sub, sbase, P + j0 + (int64_t)j0 * ld, ld, D.dinv + c0 + j0, P + i0 + (int64_t)j0 * ld);
+            if (ni == TILE && nj == TILE) trsm_tile<true>(Cs, Ls, rinv, ni, nj, sub, sbase, P + j0 + (int64_t)j0 * ld, ld, D.dinv + c0 + j0, P + i0 + (int64_t)j0 * ld);
+            else trsm_tile<false>(Cs, Ls, rinv, ni, nj, sub, sbase, P + j0 + (int64_t)j0 * ld, ld, D.dinv + c0 + j0, P + i0 + (int64_t)j0 * ld);
             TRACE(3);                                    // every row-solving thread has already stored its finished entries
         }
         __syncthreads();
