@@ -82,6 +82,16 @@ __device__ __forceinline__ void cp_async16(double* dst_smem, const double* src, 
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+// mbarrier helpers (shared-memory arrive / wait objects): the operand ring of the tile product hands its stages over with a
+// "full" word per stage (every thread's cp.async group arrives on it when it has landed) and an "empty" word (one arrival per
+// warp that has finished multiplying the stage), so no CTA-wide barrier sits in the product loop and the warps may drift by a chunk.
+__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* b, int n) { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(b)), "r"(n) : "memory"); }
+__device__ __forceinline__ void mbar_arrive(uint64_t* b) { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_addr(b)) : "memory"); }
+__device__ __forceinline__ void mbar_cp_async_arrive(uint64_t* b) { asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_addr(b)) : "memory"); }
+__device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity) {
+    asm volatile("{\n.reg .pred p;\nMBW: mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra MBD;\nbra MBW;\nMBD:\n}" ::"r"(smem_addr(b)), "r"(parity) : "memory");
+}
 // 1/sqrt(d) for a normal d > 0: hardware approximation (rsqrt.approx.f64, ~2^-22) + two Newton steps -> rounding level
 __device__ __forceinline__ double rsqrt_newton(double d) {
     double y;
@@ -175,6 +185,7 @@ __device__ unsigned long long g_potrf_cycles[8];
 #define PCLK(v) do {} while (0)
 #define PACC(slot, a, b) do {} while (0)
 #endif
+__shared__ uint64_t s_full[NSTAGE], s_empty[NSTAGE];    // operand ring of the tile product (initialised once per kernel)
 __shared__ double s_inv8[8];                            // reciprocal pivots of the current 8 x 8 diagonal block (partial_chol)
 __shared__ int s_all;                                   // trsm_tile: L_JJ was complete when the task looked
 struct NoPublish { __device__ __forceinline__ void operator()(int, int) const {} };
@@ -639,9 +650,11 @@ __device__ __forceinline__ void small_front_task(const DevSym& D, const DagPlan&
 // 2 for the pair task that keeps two C tiles in shared memory).
 template <int NST>
 __device__ __forceinline__ void tile_build(const DevSym& D, const DagPlan& F, int s, int I, int J, int Kend, const double* __restrict__ Kval,
-                                           double eta, uint32_t epoch, double* pipe, double* Cs, unsigned long long* tr) {
+                                           double eta, uint32_t epoch, double* pipe, double* Cs, unsigned long long* tr, uint32_t& gchunk) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int gid = lane >> 2, tig = lane & 3, wm = warp >> 1, wn = warp & 1;
+    static_assert(NST == NSTAGE && (NST & (NST - 1)) == 0, "ring stages: the mbarrier words are sized for NSTAGE, a power of two");
+    const uint32_t gbase = gchunk;                       // chunks this CTA has multiplied so far (same in every thread): stage and phase of chunk c follow from gbase + c
     const int c0 = D.sn_start[s], w = D.sn_start[s + 1] - c0;
     const int r = (int)(D.rows_ptr[s + 1] - D.rows_ptr[s]), ld = ld_even(r);
     const int nbp = tile_nbp(w), nbt = nbp + tile_nbu(w, r);
@@ -775,7 +788,9 @@ __device__ __forceinline__ void tile_build(const DevSym& D, const DagPlan& F, in
     auto issue = [&](int c) {
         if (c < nch) {
             const int kc = c * KC;
-            double* st = pipe + (c % NST) * STAGE_DOUBLES;
+            const uint32_t g = gbase + (uint32_t)c, sg = g & (NST - 1);
+            if (g >= (uint32_t)NST) mbar_wait(&s_empty[sg], ((g / NST) - 1u) & 1u);   // every warp is done with the chunk that was here
+            double* st = pipe + sg * STAGE_DOUBLES;
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 const int p = tid + NT * q;
@@ -785,19 +800,18 @@ __device__ __forceinline__ void tile_build(const DevSym& D, const DagPlan& F, in
                 const double* src = P + (op ? ja : ia) + 2 * seg + (int64_t)kcl * ld;
                 cp_async16(st + op * (KC * ALD) + kk * ALD + 2 * seg, src, k < Kend ? 16 : 0);
             }
+            mbar_cp_async_arrive(&s_full[sg]);
         }
-        cp_async_commit();
     };
     // chunk c is multiplied BEFORE the warps wait for the flags of chunk c+3 (and request it): when a flag is late, the chunks
     // already in shared memory are finished first and the newly released columns only add their own latency
 #pragma unroll
     for (int c = 0; c < NST - 1; ++c) { wait_flags(c); issue(c); }
     for (int c = 0; c < nch; ++c) {
-        cp_async_wait<NST - 2>();
-        __syncthreads();
-        if (NST == 2) { wait_flags(c + 1); issue(c + 1); }   // two stages: the other one is free since this barrier
-        const double* As = pipe + (c % NST) * STAGE_DOUBLES + wm * 16 + gid + di;
-        const double* Bs = pipe + (c % NST) * STAGE_DOUBLES + KC * ALD + wn * 32 + gid + dj;
+        const uint32_t g = gbase + (uint32_t)c, sg = g & (NST - 1);
+        mbar_wait(&s_full[sg], (g / NST) & 1u);          // all 256 threads' copies of this chunk have landed
+        const double* As = pipe + sg * STAGE_DOUBLES + wm * 16 + gid + di;
+        const double* Bs = pipe + sg * STAGE_DOUBLES + KC * ALD + wn * 32 + gid + dj;
 #pragma unroll
         for (int ks = 0; ks < KC; ks += 4) {
             double a[2], b[4];
@@ -810,9 +824,11 @@ __device__ __forceinline__ void tile_build(const DevSym& D, const DagPlan& F, in
 #pragma unroll
                 for (int nt = 0; nt < 4; ++nt) dmma(acc[mt][nt], a[mt], b[nt]);
         }
-        if (NST > 2) { wait_flags(c + NST - 1); issue(c + NST - 1); }   // that stage held chunk c-1: free since this iteration's barrier
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&s_empty[sg]);
+        wait_flags(c + NST - 1); issue(c + NST - 1);     // that stage held chunk c-1: refilled once every warp has left it
     }
-    cp_async_wait<0>();
+    gchunk = gbase + (uint32_t)nch;
     TRACE(2);
 
     __syncthreads();
@@ -830,7 +846,7 @@ __device__ __forceinline__ void tile_build(const DevSym& D, const DagPlan& F, in
 // task type 1: tile (I,J) of a tiled front, left-looking
 // =============================================================================================================
 __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int s, int I, int J, const double* __restrict__ Kval,
-                                          double eta, uint32_t epoch, double* sm, unsigned long long* tr) {
+                                          double eta, uint32_t epoch, double* sm, unsigned long long* tr, uint32_t& gchunk) {
     const int tid = threadIdx.x;
     const int c0 = D.sn_start[s], w = D.sn_start[s + 1] - c0;
     const int r = (int)(D.rows_ptr[s + 1] - D.rows_ptr[s]), ld = ld_even(r), m = r - w;
@@ -843,7 +859,7 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
     uint32_t* rowp = tdone + nbp * nbt + 1;
     double* pipe = sm;
     double* Cs = sm + PIPE_DOUBLES;
-    tile_build<NSTAGE>(D, F, s, I, J, (J < nbp) ? j0 : w, Kval, eta, epoch, pipe, Cs, tr);
+    tile_build<NSTAGE>(D, F, s, I, J, (J < nbp) ? j0 : w, Kval, eta, epoch, pipe, Cs, tr, gchunk);
 
     // ---- 3. finish: POTRF / TRSM for panel tiles, then store (each tile is written once) ----
     if (J < nbp) {
@@ -903,6 +919,11 @@ __global__ void __launch_bounds__(NT, 2) factor_dag_kernel(DevSym D, DagPlan F, 
     __shared__ int s_task;
     if (epoch_dev) epoch = epoch_dev[0];                 // graph replay: the call number comes from device memory
     const uint32_t base = (epoch - 1u) * (uint32_t)(F.n_ftasks + (int)gridDim.x);
+    if (threadIdx.x == 0) {
+        for (int q = 0; q < NSTAGE; ++q) { mbar_init(&s_full[q], NT); mbar_init(&s_empty[q], NT / 32); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    uint32_t gchunk = 0;                                 // chunks of tile products this CTA has run (stage / phase bookkeeping of the ring)
     while (true) {
         __syncthreads();
         if (threadIdx.x == 0) s_task = (int)(atomicAdd(F.sync, 1u) - base);
@@ -918,7 +939,7 @@ __global__ void __launch_bounds__(NT, 2) factor_dag_kernel(DevSym D, DagPlan F, 
         unsigned long long* tr = nullptr;
 #endif
         if (tk.x == 0) small_front_task(D, F, tk.y, Kval, eta, epoch, sm, tr);
-        else tile_task(D, F, tk.y, tk.z, tk.w, Kval, eta, epoch, sm, tr);
+        else tile_task(D, F, tk.y, tk.z, tk.w, Kval, eta, epoch, sm, tr, gchunk);
     }
 }
 
