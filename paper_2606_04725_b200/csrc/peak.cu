@@ -54,12 +54,18 @@ __global__ void __launch_bounds__(PEAK_NT) dmma_peak_kernel(double* out, int ite
 
 // ---- the left-looking tile GEMM of factor.cu (tile_task, step 2) in isolation: one 64 x 64 tile per CTA, 256 threads, fp64
 //      DMMA m8n8k4 (2 x 4 accumulator tiles per thread), operands streamed from a column-major panel with cp.async.cg through
-//      a 4-stage ring of 16 columns -- same tile shape, ring and fragment mapping as the factorization, no flags, no assembly,
+//      a 4-stage ring of 16 columns handed over with mbarrier words -- same tile shape, ring and fragment mapping as the factorization, no flags, no assembly,
 //      no POTRF / TRSM.  CTA b multiplies the rows of block b with the rows of block b + 1 of one tall panel. ----
 constexpr int G_TILE = 64, G_KC = 16, G_ALD = 68, G_NSTAGE = 4, G_STAGE = 2 * G_KC * G_ALD;
 
+__device__ __forceinline__ unsigned g_saddr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void g_mbar_wait(uint64_t* b, uint32_t parity) {
+    asm volatile("{\n.reg .pred p;\nGW: mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra GD;\nbra GW;\nGD:\n}" ::"r"(g_saddr(b)), "r"(parity) : "memory");
+}
+
 __global__ void __launch_bounds__(PEAK_NT, 2) tile_gemm_kernel(const double* __restrict__ P, int ld, int K, int nblocks, double* __restrict__ out) {
     extern __shared__ __align__(16) double pipe[];
+    __shared__ uint64_t full[G_NSTAGE], empty[G_NSTAGE];  // the ring is handed over as in factor.cu: cp.async arrivals / one arrival per warp
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gid = lane >> 2, tig = lane & 3, wm = warp >> 1, wn = warp & 1;
     const int ia = (int)(blockIdx.x % nblocks) * G_TILE, ja = (int)((blockIdx.x + 1) % nblocks) * G_TILE;
     double acc[2][4][2];
@@ -67,27 +73,36 @@ __global__ void __launch_bounds__(PEAK_NT, 2) tile_gemm_kernel(const double* __r
     for (int a = 0; a < 2; ++a)
 #pragma unroll
         for (int b = 0; b < 4; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
+    if (tid == 0) {
+        for (int q = 0; q < G_NSTAGE; ++q) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(g_saddr(&full[q])), "r"(PEAK_NT) : "memory");
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(g_saddr(&empty[q])), "r"(PEAK_NT / 32) : "memory");
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
     const int nch = K / G_KC;
     auto issue = [&](int c) {
         if (c < nch) {
-            double* st = pipe + (c % G_NSTAGE) * G_STAGE;
+            const int sg = c % G_NSTAGE;
+            if (c >= G_NSTAGE) g_mbar_wait(&empty[sg], (uint32_t)((c / G_NSTAGE) - 1) & 1u);
+            double* st = pipe + sg * G_STAGE;
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 const int p = tid + PEAK_NT * q;
                 const int op = p >> 9, rem = p & 511, kk = rem >> 5, seg = rem & 31;
                 const double* src = P + (op ? ja : ia) + 2 * seg + (int64_t)(c * G_KC + kk) * ld;
-                const unsigned d = (unsigned)__cvta_generic_to_shared(st + op * (G_KC * G_ALD) + kk * G_ALD + 2 * seg);
-                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(src) : "memory");
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(g_saddr(st + op * (G_KC * G_ALD) + kk * G_ALD + 2 * seg)), "l"(src) : "memory");
             }
+            asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(g_saddr(&full[sg])) : "memory");
         }
-        asm volatile("cp.async.commit_group;" ::: "memory");
     };
     issue(0); issue(1); issue(2);
     for (int c = 0; c < nch; ++c) {
-        asm volatile("cp.async.wait_group 2;" ::: "memory");
-        __syncthreads();
-        const double* As = pipe + (c % G_NSTAGE) * G_STAGE + wm * 16 + gid;
-        const double* Bs = pipe + (c % G_NSTAGE) * G_STAGE + G_KC * G_ALD + wn * 32 + gid;
+        const int sg = c % G_NSTAGE;
+        g_mbar_wait(&full[sg], (uint32_t)(c / G_NSTAGE) & 1u);
+        const double* As = pipe + sg * G_STAGE + wm * 16 + gid;
+        const double* Bs = pipe + sg * G_STAGE + G_KC * G_ALD + wn * 32 + gid;
 #pragma unroll
         for (int ks = 0; ks < G_KC; ks += 4) {
             double a[2], b[4];
@@ -102,9 +117,10 @@ __global__ void __launch_bounds__(PEAK_NT, 2) tile_gemm_kernel(const double* __r
                     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                                  : "+d"(acc[mt][nt][0]), "+d"(acc[mt][nt][1]) : "d"(a[mt]), "d"(b[nt]));
         }
+        __syncwarp();
+        if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(g_saddr(&empty[sg])) : "memory");
         issue(c + 3);
     }
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
     double s = 0.0;
 #pragma unroll
     for (int a = 0; a < 2; ++a)
