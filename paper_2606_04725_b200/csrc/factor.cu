@@ -92,6 +92,13 @@ __device__ __forceinline__ void mbar_cp_async_arrive(uint64_t* b) { asm volatile
 __device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity) {
     asm volatile("{\n.reg .pred p;\nMBW: mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra MBD;\nbra MBW;\nMBD:\n}" ::"r"(smem_addr(b)), "r"(parity) : "memory");
 }
+// the same on shared-window addresses (the product loop converts its pointers once per tile, not once per instruction)
+__device__ __forceinline__ void mbar_arrive_s(unsigned a) { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(a) : "memory"); }
+__device__ __forceinline__ void mbar_cp_async_arrive_s(unsigned a) { asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(a) : "memory"); }
+__device__ __forceinline__ void mbar_wait_s(unsigned a, uint32_t parity) {
+    asm volatile("{\n.reg .pred p;\nMBWS: mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra MBDS;\nbra MBWS;\nMBDS:\n}" ::"r"(a), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void cp_async16_s(unsigned d, const double* src) { asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(src) : "memory"); }
 // 1/sqrt(d) for a normal d > 0: hardware approximation (rsqrt.approx.f64, ~2^-22) + two Newton steps -> rounding level
 __device__ __forceinline__ double rsqrt_newton(double d) {
     double y;
@@ -785,22 +792,38 @@ __device__ __forceinline__ void tile_build(const DevSym& D, const DagPlan& F, in
             }
         }
     };
+    // operand copies of a chunk: thread = (k-column tid >> 5 and that + 8, 16-byte segment tid & 31) of operand A and of operand B.
+    // Everything that does not change from chunk to chunk is formed once per tile (shared-window addresses, the thread's source
+    // pointer in chunk 0); a full chunk is then four copies at fixed offsets, and only a ragged last chunk takes the clamped form.
+    const unsigned pipe_s = smem_addr(pipe), full_s = smem_addr(s_full), empty_s = smem_addr(s_empty);
+    const unsigned dst0 = pipe_s + (unsigned)(((tid >> 5) * ALD + 2 * (tid & 31)) * 8);
+    const double* const src0 = P + ia + 2 * (tid & 31) + (int64_t)(tid >> 5) * ld;
+    const int64_t dAB = (int64_t)ja - ia, d8 = 8 * (int64_t)ld;
     auto issue = [&](int c) {
         if (c < nch) {
             const int kc = c * KC;
             const uint32_t g = gbase + (uint32_t)c, sg = g & (NST - 1);
-            if (g >= (uint32_t)NST) mbar_wait(&s_empty[sg], ((g / NST) - 1u) & 1u);   // every warp is done with the chunk that was here
-            double* st = pipe + sg * STAGE_DOUBLES;
+            if (g >= (uint32_t)NST) mbar_wait_s(empty_s + 8 * sg, ((g / NST) - 1u) & 1u);   // every warp is done with the chunk that was here
+            if (kc + KC <= Kend) {
+                const unsigned d = dst0 + sg * (unsigned)(STAGE_DOUBLES * 8);
+                const double* sa = src0 + (int64_t)kc * ld;
+                cp_async16_s(d, sa);
+                cp_async16_s(d + 8 * ALD * 8, sa + d8);
+                cp_async16_s(d + KC * ALD * 8, sa + dAB);
+                cp_async16_s(d + (KC + 8) * ALD * 8, sa + dAB + d8);
+            } else {
+                double* st = pipe + sg * STAGE_DOUBLES;
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const int p = tid + NT * q;
-                const int op = p >> 9, rem = p & 511, kk = rem >> 5, seg = rem & 31;
-                const int k = kc + kk;
-                const int kcl = k < Kend ? k : Kend - 1;
-                const double* src = P + (op ? ja : ia) + 2 * seg + (int64_t)kcl * ld;
-                cp_async16(st + op * (KC * ALD) + kk * ALD + 2 * seg, src, k < Kend ? 16 : 0);
+                for (int q = 0; q < 4; ++q) {
+                    const int p = tid + NT * q;
+                    const int op = p >> 9, rem = p & 511, kk = rem >> 5, seg = rem & 31;
+                    const int k = kc + kk;
+                    const int kcl = k < Kend ? k : Kend - 1;
+                    const double* src = P + (op ? ja : ia) + 2 * seg + (int64_t)kcl * ld;
+                    cp_async16(st + op * (KC * ALD) + kk * ALD + 2 * seg, src, k < Kend ? 16 : 0);
+                }
             }
-            mbar_cp_async_arrive(&s_full[sg]);
+            mbar_cp_async_arrive_s(full_s + 8 * sg);
         }
     };
     // chunk c is multiplied BEFORE the warps wait for the flags of chunk c+3 (and request it): when a flag is late, the chunks
@@ -809,7 +832,7 @@ __device__ __forceinline__ void tile_build(const DevSym& D, const DagPlan& F, in
     for (int c = 0; c < NST - 1; ++c) { wait_flags(c); issue(c); }
     for (int c = 0; c < nch; ++c) {
         const uint32_t g = gbase + (uint32_t)c, sg = g & (NST - 1);
-        mbar_wait(&s_full[sg], (g / NST) & 1u);          // all 256 threads' copies of this chunk have landed
+        mbar_wait_s(full_s + 8 * sg, (g / NST) & 1u);     // all 256 threads' copies of this chunk have landed
         const double* As = pipe + sg * STAGE_DOUBLES + wm * 16 + gid + di;
         const double* Bs = pipe + sg * STAGE_DOUBLES + KC * ALD + wn * 32 + gid + dj;
 #pragma unroll
@@ -825,7 +848,7 @@ __device__ __forceinline__ void tile_build(const DevSym& D, const DagPlan& F, in
                 for (int nt = 0; nt < 4; ++nt) dmma(acc[mt][nt], a[mt], b[nt]);
         }
         __syncwarp();
-        if (lane == 0) mbar_arrive(&s_empty[sg]);
+        if (lane == 0) mbar_arrive_s(empty_s + 8 * sg);
         wait_flags(c + NST - 1); issue(c + NST - 1);     // that stage held chunk c-1: refilled once every warp has left it
     }
     gchunk = gbase + (uint32_t)nch;
