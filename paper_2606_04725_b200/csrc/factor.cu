@@ -98,7 +98,11 @@ __device__ __forceinline__ void mbar_cp_async_arrive_s(unsigned a) { asm volatil
 __device__ __forceinline__ void mbar_wait_s(unsigned a, uint32_t parity) {
     asm volatile("{\n.reg .pred p;\nMBWS: mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra MBDS;\nbra MBWS;\nMBDS:\n}" ::"r"(a), "r"(parity) : "memory");
 }
-__device__ __forceinline__ void cp_async16_s(unsigned d, const double* src) { asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(src) : "memory"); }
+// two 16-byte copies 256 bytes apart on both sides (one k-column of an operand is 512 contiguous bytes): immediate offsets, one address each
+template <int DOFF>
+__device__ __forceinline__ void cp_async16x2_s(unsigned d, const double* src) {
+    asm volatile("cp.async.cg.shared.global [%0+%2], [%1], 16;\n\tcp.async.cg.shared.global [%0+%3], [%1+256], 16;" ::"r"(d), "l"(src), "n"(DOFF), "n"(DOFF + 256) : "memory");
+}
 // 1/sqrt(d) for a normal d > 0: hardware approximation (rsqrt.approx.f64, ~2^-22) + two Newton steps -> rounding level
 __device__ __forceinline__ double rsqrt_newton(double d) {
     double y;
@@ -744,6 +748,27 @@ __device__ __forceinline__ void tile_build(const DevSym& D, const DagPlan& F, in
                 __syncthreads();
                 // flat index f = bb * na + aa over the na x nb block, NT apart per step: (aa, bb) advance by the CTA-uniform
                 // (NT % na, NT / na) with one carry -- one division per thread and child instead of one per entry
+                if (na == TILE) {
+                    // the child covers all 64 rows of the tile (the usual case inside a large front): thread = (row, column mod 4),
+                    // no index carry, the row's offset read once
+                    const int aa = tid & (TILE - 1), da = relA[aa], adl = a0 + aa - b0;
+                    const double* Ua = Uc + (a0 + aa) + (long long)b0 * mc;
+                    for (int bb0 = tid >> 6; bb0 < nb; bb0 += 8 * (NT / TILE)) {
+                        double v[8];
+                        int dst[8];
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) {
+                            const int bb = bb0 + e * (NT / TILE);
+                            const bool on = bb < nb && adl >= bb;
+                            v[e] = on ? __ldcg(Ua + (long long)bb * mc) : 0.0;
+                            dst[e] = on ? relB[on ? bb : 0] + da : -1;
+                        }
+#pragma unroll
+                        for (int e = 0; e < 8; ++e)
+                            if (dst[e] >= 0) Cs[dst[e]] += v[e];
+                    }
+                    continue;
+                }
                 const int tot = na * nb, qa = NT / na, ra = NT - qa * na;
                 int bb = tid / na, aa = tid - bb * na;
                 for (int f0 = tid; f0 < tot; f0 += 8 * NT) {
@@ -792,13 +817,13 @@ __device__ __forceinline__ void tile_build(const DevSym& D, const DagPlan& F, in
             }
         }
     };
-    // operand copies of a chunk: thread = (k-column tid >> 5 and that + 8, 16-byte segment tid & 31) of operand A and of operand B.
+    // operand copies of a chunk: thread = (k-column tid >> 4, 16-byte segments tid & 15 and that + 16) of operand A and of operand B.
     // Everything that does not change from chunk to chunk is formed once per tile (shared-window addresses, the thread's source
     // pointer in chunk 0); a full chunk is then four copies at fixed offsets, and only a ragged last chunk takes the clamped form.
     const unsigned pipe_s = smem_addr(pipe), full_s = smem_addr(s_full), empty_s = smem_addr(s_empty);
-    const unsigned dst0 = pipe_s + (unsigned)(((tid >> 5) * ALD + 2 * (tid & 31)) * 8);
-    const double* const src0 = P + ia + 2 * (tid & 31) + (int64_t)(tid >> 5) * ld;
-    const int64_t dAB = (int64_t)ja - ia, d8 = 8 * (int64_t)ld;
+    const unsigned dst0 = pipe_s + (unsigned)(((tid >> 4) * ALD + 2 * (tid & 15)) * 8);
+    const double* const src0 = P + ia + 2 * (tid & 15) + (int64_t)(tid >> 4) * ld;
+    const int64_t dAB = (int64_t)ja - ia;
     auto issue = [&](int c) {
         if (c < nch) {
             const int kc = c * KC;
@@ -807,10 +832,8 @@ __device__ __forceinline__ void tile_build(const DevSym& D, const DagPlan& F, in
             if (kc + KC <= Kend) {
                 const unsigned d = dst0 + sg * (unsigned)(STAGE_DOUBLES * 8);
                 const double* sa = src0 + (int64_t)kc * ld;
-                cp_async16_s(d, sa);
-                cp_async16_s(d + 8 * ALD * 8, sa + d8);
-                cp_async16_s(d + KC * ALD * 8, sa + dAB);
-                cp_async16_s(d + (KC + 8) * ALD * 8, sa + dAB + d8);
+                cp_async16x2_s<0>(d, sa);
+                cp_async16x2_s<KC * ALD * 8>(d, sa + dAB);
             } else {
                 double* st = pipe + sg * STAGE_DOUBLES;
 #pragma unroll
@@ -925,10 +948,14 @@ __device__ __forceinline__ void tile_task(const DevSym& D, const DagPlan& F, int
         double* Uo = D.U + D.upd_ptr[s];
         TRACE(3);
         {
-            const int mm = tid & (TILE - 1);
-            if (mm < ni)
-                for (int nn = tid >> 6; nn < nj; nn += NT / TILE)
-                    if (I != J || mm >= nn) Uo[(i0 + mm - w) + (int64_t)(j0 + nn - w) * m] = Cs[nn * CLD + mm];
+            const int mm = tid & (TILE - 1), n0 = tid >> 6;
+            if (mm < ni) {
+                double* po = Uo + (i0 + mm - w) + (int64_t)(j0 + n0 - w) * m;
+                const double* pc = Cs + n0 * CLD + mm;
+                const int64_t so = (int64_t)(NT / TILE) * m;
+                for (int nn = n0; nn < nj; nn += NT / TILE, po += so, pc += (NT / TILE) * CLD)
+                    if (I != J || mm >= nn) *po = *pc;
+            }
         }
         __syncthreads();
         if (tid == 0) { __threadfence(); red_release_add(front_done + s, 1u); }
