@@ -96,7 +96,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity) {
 __device__ __forceinline__ void mbar_arrive_s(unsigned a) { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(a) : "memory"); }
 __device__ __forceinline__ void mbar_cp_async_arrive_s(unsigned a) { asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(a) : "memory"); }
 __device__ __forceinline__ void mbar_wait_s(unsigned a, uint32_t parity) {
-    asm volatile("{\n.reg .pred p;\nMBWS: mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra MBDS;\nbra MBWS;\nMBDS:\n}" ::"r"(a), "r"(parity) : "memory");
+    asm volatile("{\n.reg .pred p;\nMBWS: mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@!p bra MBWS;\n}" ::"r"(a), "r"(parity) : "memory");
 }
 // two 16-byte copies 256 bytes apart on both sides (one k-column of an operand is 512 contiguous bytes): immediate offsets, one address each
 template <int DOFF>
