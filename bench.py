@@ -50,7 +50,7 @@ from ocp_inputs import make_config  # noqa: E402
 METRIC = "kkt_refactor_solve_us_per_ipm_iteration"
 UNIT = "us/IPM-iteration"
 FP64_DERIVED_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # 64 DFMA lanes/SM at clocks.max.sm
-NCU_RAW = os.path.join("profiles", "r02c_c3_ncu_raw.csv")  # `ncu --page raw --csv` export of the --set full capture (C3)
+NCU_RAW = os.path.join("profiles", "r02d_c3_ncu_raw.csv")  # `ncu --page raw --csv` export of the --set full capture (C3)
 C3_SAMPLE_N = 4                                           # stages of the sub-horizon instance the oracle is timed on for C3
 
 
