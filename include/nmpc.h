@@ -200,6 +200,20 @@ nmpc_status nmpc_factor(nmpc_handle h, const double* values_dev, double eta, int
 /* ---- Eq. (22)-(25): rhs_inout_dev DEVICE n*nrhs doubles (column-major), overwritten by K^-1 rhs.  Async.   */
 nmpc_status nmpc_solve(nmpc_handle h, double* rhs_inout_dev, int32_t nrhs);
 
+/* ---- Eq. (22)-(25) with NO allocation behind it: the same two-sided solve as nmpc_solve, for callers that cannot have
+ *      cudaMalloc on their path (CUDA-graph capture, tight serving loops).  The permuted work vector of the solve kernel is a
+ *      file-scope device array of the library, NMPC_STATIC_SOLVE_DOUBLES doubles = 2 MiB, which every GPU that loads the
+ *      library holds until the process exits; the call makes no cudaMalloc / cudaFree and calls no allocating routine (the
+ *      first call on a device looks the array's device address up once, cudaGetSymbolAddress).
+ *      rhs_dev: DEVICE, n doubles, read only.  out_dev: DEVICE, n doubles, receives K^-1 rhs (may equal rhs_dev: in place).
+ *      Asynchronous on the handle's stream.  Errors: NMPC_E_STATE before a successful nmpc_factor / nmpc_factor_rhs;
+ *      NMPC_E_ARG when the structure needs more than NMPC_STATIC_SOLVE_DOUBLES work doubles (n + 1 with the right-hand-side
+ *      row, else n) -- nmpc_last_error says so; use nmpc_solve then.
+ *      ALL calls on one device share the array (any handle, any stream); it keeps the last call's contents and the part a
+ *      call uses is cleared first.  Calls that OVERLAP on the GPU (different streams or handles) race on it: serialise them. */
+#define NMPC_STATIC_SOLVE_DOUBLES 262144
+nmpc_status nmpc_solve_static(nmpc_handle h, const double* rhs_dev, double* out_dev);
+
 /* ---- Eq. (20)-(22) in one pass (handles with the right-hand-side row, options.fuse_rhs; else NMPC_E_STATE): numeric
  *      Cholesky of K + eta I with b = rhs_dev (DEVICE, n doubles, copied) carried as an extra row, which leaves v = L^-1 P b
  *      in the factor.  nmpc_solve_fused then runs the backward solve only: out_dev (DEVICE, n) <- P^T L^-T v = K^-1 b

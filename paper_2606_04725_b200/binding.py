@@ -84,6 +84,7 @@ SIGNATURES = {
     "nmpc_solve": (c_i32, [c_vp, c_vp, c_i32]),
     "nmpc_factor_rhs": (c_i32, [c_vp, c_vp, c_vp, c_dbl, P(c_i64)]),
     "nmpc_solve_fused": (c_i32, [c_vp, c_vp]),
+    "nmpc_solve_static": (c_i32, [c_vp, c_vp, c_vp]),
     "nmpc_kkt_multiply": (c_i32, [c_vp, c_vp, c_vp]),
     "nmpc_ipm_solve": (c_i32, [c_vp, c_i32, c_i32, c_vp, P(nmpc_stats), c_vp, c_i32]),
     "nmpc_hykkt_solve": (c_i32, [c_vp, c_i32, c_i32, c_vp, P(nmpc_stats), c_vp, c_i32]),
@@ -342,6 +343,13 @@ class Handle:
 
     def solve_fused(self, out_dev):
         self._ck(self.lib.nmpc_solve_fused(self._h, _ptr(out_dev)), "nmpc_solve_fused")
+
+    def solve_static(self, rhs_dev, out_dev, check=True):
+        """nmpc_solve_static: the two-sided solve with its work vector in the library's static device array (no allocation)."""
+        st = self.lib.nmpc_solve_static(self._h, _ptr(rhs_dev), _ptr(out_dev))
+        if check:
+            self._ck(st, "nmpc_solve_static")
+        return st
 
     def kkt_multiply(self, x_dev, y_dev):
         self._ck(self.lib.nmpc_kkt_multiply(self._h, _ptr(x_dev), _ptr(y_dev)), "nmpc_kkt_multiply")

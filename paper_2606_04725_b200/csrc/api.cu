@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <thread>
@@ -767,6 +768,63 @@ nmpc_status nmpc_solve(nmpc_handle h, double* rhs, int32_t nrhs) {
     DeviceGuard dg(h);
     if (!h->factored) { h->err = "nmpc_solve before a successful nmpc_factor"; return NMPC_E_STATE; }
     for (int k = 0; k < nrhs; ++k) TRY(run_solve(h, rhs + (int64_t)k * h->S.n));
+    CK(cudaGetLastError());
+    return NMPC_OK;
+}
+
+// ---- nmpc_solve_static: the two-sided solve with its work vector in a file-scope device array (no allocation anywhere on the
+//      path, not even at analysis time, for this vector).  The array is part of the library image: every GPU that loads the
+//      library holds NMPC_STATIC_SOLVE_DOUBLES * 8 bytes = 2 MiB of it until the process exits.  In host code the NAME of the
+//      array is a host-side stand-in, not a device address; the device address comes from cudaGetSymbolAddress, once per
+//      device with that device current (static_solve_scratch), and THAT pointer goes to the kernel.  Every call on a device
+//      shares the array, which keeps the last call's contents: the part a call uses is cleared first, and calls that overlap
+//      on the GPU (two streams, two handles) race. ----
+#define NMPC_STATIC_SOLVE_DOUBLES_IMPL 262144
+static_assert(NMPC_STATIC_SOLVE_DOUBLES_IMPL == NMPC_STATIC_SOLVE_DOUBLES, "include/nmpc.h states the size of the static work vector");
+static __device__ __align__(256) double g_static_solve_x[NMPC_STATIC_SOLVE_DOUBLES_IMPL];
+
+namespace {
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mu;
+double* g_static_ptr[STATIC_MAX_DEVICES] = {};            // device address of g_static_solve_x per device ordinal (0: not looked up yet)
+
+// the handle's device is current (DeviceGuard of the caller)
+nmpc_status static_solve_scratch(nmpc_handle_s* h, double** out) {
+    if (h->dev < 0 || h->dev >= STATIC_MAX_DEVICES) { h->err = "nmpc_solve_static: device ordinal beyond " + std::to_string(STATIC_MAX_DEVICES - 1); return NMPC_E_ARG; }
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    if (!g_static_ptr[h->dev]) {
+        double* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress((void**)&p, g_static_solve_x);
+        if (e != cudaSuccess || !p) {
+            cudaGetLastError();
+            h->err = std::string("nmpc_solve_static: cudaGetSymbolAddress failed (") + cudaGetErrorString(e) + ")";
+            return NMPC_E_CUDA;
+        }
+        g_static_ptr[h->dev] = p;
+    }
+    *out = g_static_ptr[h->dev];
+    return NMPC_OK;
+}
+}  // namespace
+
+nmpc_status nmpc_solve_static(nmpc_handle h, const double* rhs_dev, double* out_dev) {
+    if (!h || !rhs_dev || !out_dev) return NMPC_E_ARG;
+    DeviceGuard dg(h);
+    if ((int64_t)h->S.nt > (int64_t)NMPC_STATIC_SOLVE_DOUBLES) {
+        h->err = "nmpc_solve_static: the structure needs a work vector of " + std::to_string((long long)h->S.nt) + " doubles, the static one holds " +
+                 std::to_string((long long)NMPC_STATIC_SOLVE_DOUBLES) + " (NMPC_STATIC_SOLVE_DOUBLES); use nmpc_solve";
+        return NMPC_E_ARG;
+    }
+    if (!h->factored) { h->err = "nmpc_solve_static before a successful nmpc_factor"; return NMPC_E_STATE; }
+    double* xs = nullptr;
+    TRY(static_solve_scratch(h, &xs));
+    // the array keeps what the last call left (possibly of another handle): the part this call uses starts at zero, like the
+    // handle's own work vector did after nmpc_analyze
+    CK(cudaMemsetAsync(xs, 0, sizeof(double) * (size_t)h->S.nt, h->stream));
+    if (out_dev != rhs_dev) CK(cudaMemcpyAsync(out_dev, rhs_dev, sizeof(double) * (size_t)h->S.n, cudaMemcpyDeviceToDevice, h->stream));
+    uint32_t ef = 0, eb = 0;
+    TRY(next_solve_epochs(h, false, &ef, &eb));
+    launch_solve(h->D, h->F, out_dev, xs, ef, eb, nullptr, false, h->stream); h->launches += 1;
     CK(cudaGetLastError());
     return NMPC_OK;
 }
