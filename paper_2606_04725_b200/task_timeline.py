@@ -152,6 +152,39 @@ def main():
             P(f"| {s} | {info['super_level'][s]} | {w} | {r} | {nbp} | {(st[m, 0].min() - t0) / 1e3:.0f} | {(st[m, 4].max() - t0) / 1e3:.0f} | "
               f"{med(steps):.1f} | {med(a1):.1f} | {med(a2):.1f} | {med(a3):.1f} | {fl[s] / 296 / 100e3:.0f} |")
         P("")
+        # tile tasks by kind: where the CTA time of the panel tiles goes (the wait for the diagonal tile's POTRF)
+        P("### Tile tasks by kind (CTA-ms; mean us per task in brackets)")
+        P("")
+        T, Ss = tasks[tile], st[tile]
+        nbp_t = np.zeros(len(T), dtype=np.int64); w_t = np.zeros(len(T), dtype=np.int64)
+        for s in big:
+            ms = T[:, 1] == s
+            nbp_t[ms] = tile_bounds(W(s), R(s))[0]; w_t[ms] = W(s)
+        Ti, Tj = T[:, 2], T[:, 3]
+        kind = np.where(Tj >= nbp_t, 2, np.where(Ti == Tj, 0, 1))
+        Kt = np.where(Tj < nbp_t, Tj * TILE, w_t)
+        pht = [(Ss[:, k + 1] - Ss[:, k]) / 1e3 for k in range(4)]
+        ideal = 2.0 * TILE * TILE * Kt / 100e9 * 1e6
+        P("| kind | tasks | assemble | product (its flops at 100 GFLOP/s per CTA) | POTRF / TRSM | store + publish |")
+        P("|---|---|---|---|---|---|")
+        for k, nm in enumerate(("diagonal panel tile (POTRF)", "panel tile below the diagonal (TRSM)", "update tile")):
+            mk = kind == k
+            if mk.any():
+                P(f"| {nm} | {int(mk.sum())} | {pht[0][mk].sum() / 1e3:.1f} ({pht[0][mk].mean():.1f}) | {pht[1][mk].sum() / 1e3:.1f} ({pht[1][mk].mean():.1f}; "
+                  f"{ideal[mk].sum() / 1e3:.1f}) | {pht[2][mk].sum() / 1e3:.1f} ({pht[2][mk].mean():.1f}) | {pht[3][mk].sum() / 1e3:.1f} ({pht[3][mk].mean():.1f}) |")
+        mk = kind == 1
+        if mk.any():
+            pdone = {(int(a), int(c)): t for a, b, c, t in zip(T[:, 1], Ti, Tj, Ss[:, 3]) if b == c}
+            pd_ = np.array([pdone[(int(a), int(c))] for a, c in zip(T[mk, 1], Tj[mk])])
+            g_, e_ = Ss[mk, 2], Ss[mk, 3]
+            waitp = np.maximum(0, pd_ - g_) / 1e3
+            after = (e_ - np.maximum(pd_, g_)) / 1e3
+            P("")
+            P(f"Panel tiles below the diagonal: {100 * (g_ < pd_).mean():.1f} % finish their product BEFORE the POTRF of their block column's diagonal "
+              f"tile has ended; they wait {waitp.sum() / 1e3:.1f} CTA-ms for it (mean {waitp.mean():.1f} us per tile, "
+              f"{100 * waitp.sum() / (dur.sum()):.1f} % of all CTA time) and need {after.mean():.1f} us after it "
+              f"(tiles that arrive later: {after[g_ >= pd_].mean() if (g_ >= pd_).any() else float('nan'):.1f} us).")
+        P("")
         # chain of fronts from the last finished root
         P("### Chain of fronts from the last-finished root down the tree (each: the child that finished last)")
         P("")
